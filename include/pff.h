@@ -1,0 +1,194 @@
+/*
+ * pff.h -- C ABI of the B200-native explicit phase-field fracture hot path.
+ *
+ * Implements the staggered explicit-dynamics step on linear (P1) triangles of
+ * arxiv/paper_2606_23458 (section 2): fused element force + history, scatter to
+ * nodes, lumped-mass velocity-Verlet update, and the matrix-free (projected) Jacobi-PCG
+ * damage solve.  Every entry point cites the passage that defines the operation.
+ *
+ * General rules
+ *  - Every function returns a pff_status code (0 = PFF_OK) except pff_mesh_destroy / pff_last_error.
+ *    No exceptions, no abort.  pff_last_error() returns a thread-local, NUL-terminated
+ *    description of the last failure.
+ *  - "host" pointers are ordinary CPU memory, read (or written) before the call returns.
+ *    "device" pointers are CUDA device memory of the GPU that was current at pff_mesh_create.
+ *  - The library owns the pff_mesh object and all of its workspaces.  The caller owns every
+ *    state buffer (pff_state) and keeps it alive; the library never frees or reallocates it.
+ *  - All device work is enqueued on the CUDA stream passed to pff_mesh_create (NULL = default
+ *    stream).  pff_explicit_step and pff_init_accel never synchronise; pff_damage_solve and
+ *    pff_energies synchronise that stream before returning (they return host scalars).
+ *  - INTERNAL ORDER.  pff_mesh_create renumbers nodes and elements (domain-decomposition /
+ *    Morton order).  All device arrays in pff_state and all device
+ *    vectors passed to test hooks are in internal order and in the precision of the mesh
+ *    (double for PFF_F64, float for PFF_F32), SoA.  pff_mesh_permutations returns the maps;
+ *    host-side index sets (Dirichlet dofs, traction edges) are given in USER numbering.
+ *  - One mesh = one homogeneous material, unit thickness (energies per unit thickness,
+ *    PAPER.md L225).
+ */
+#ifndef PFF_H
+#define PFF_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    PFF_OK = 0,
+    PFF_EINVAL = 1,       /* null pointer, bad enum, nu outside (-1, 0.5), E/rho/Gc/l0 <= 0, dt <= 0 ... */
+    PFF_EMESH = 2,        /* node index out of range, (near-)zero-area element, orphan node           */
+    PFF_ENOMEM = 3,
+    PFF_ECUDA = 4,        /* CUDA runtime error; text in pff_last_error()                             */
+    PFF_ENOCONV = 5,      /* damage CG used max_iter mat-vecs: the result IS written                  */
+    PFF_EUNSUPPORTED = 6
+} pff_status;
+
+typedef enum { PFF_AT1 = 1, PFF_AT2 = 2 } pff_model;                      /* PAPER.md L69, Eq. 6 / Eq. 8 */
+typedef enum {
+    PFF_SPLIT_ISOTROPIC = 0,   /* psi+ = psi (L79)                                        */
+    PFF_SPLIT_SPECTRAL = 1,    /* Miehe, Eq. 2 (L71-75), closed-form 2x2 principal strains  */
+    PFF_SPLIT_VOLDEV = 2,      /* Amor, Eq. 3 (L75-79), 3-D bulk modulus (L85)              */
+    PFF_SPLIT_STARCONVEX = 3   /* vol-dev with gamma_star (L51, L85; reading R5)  */
+} pff_split;
+typedef enum { PFF_PLANE_STRAIN = 0, PFF_PLANE_STRESS = 1 } pff_plane;  /* L85 */
+typedef enum { PFF_F64 = 0, PFF_F32 = 1 } pff_precision;                /* L189: fp64 is the reference */
+typedef enum {
+    PFF_SCATTER_GATHER = 0,    /* deterministic: chunk-local CSR gather in shared memory + ordered
+                                  interface sums; bit-reproducible run to run (default)            */
+    PFF_SCATTER_ATOMIC = 1     /* element kernel with global floating-point atomics (L43, L124)    */
+} pff_scatter;
+typedef enum { PFF_ORDER_NONE = 0, PFF_ORDER_MORTON = 1 } pff_order;
+
+/* Material and model.  g(d) = (1-d)^2 + eta. */
+typedef struct {
+    double E, nu, rho, Gc, l0;
+    double eta;          /* residual stiffness, paper value 1e-7 (L79); 0 allowed            */
+    double gamma_star;   /* star-convex parameter (>= -1); ignored by the other splits        */
+    int32_t model;       /* pff_model  */
+    int32_t split;       /* pff_split  */
+    int32_t plane;       /* pff_plane  */
+} pff_material;
+
+typedef struct {
+    int32_t precision;    /* pff_precision */
+    int32_t order;        /* pff_order     */
+    int32_t scatter;      /* pff_scatter   */
+    int32_t chunk_elems;  /* elements per CTA chunk, 0 = library default; multiple of 32, <= 8192 */
+} pff_options;
+
+typedef struct pff_mesh pff_mesh;
+
+/* Caller-owned device arrays, internal order, precision of the mesh.  Nodal arrays have n_nodes
+ * entries, H has n_elems entries (one history value per element, R2). */
+typedef struct {
+    void *ux, *uy;       /* displacement u          (Eq. 16) */
+    void *vx, *vy;       /* velocity v              (Eq. 18) */
+    void *ax, *ay;       /* acceleration a          (Eq. 17) */
+    void *d;             /* damage, in [0, 1]                 */
+    void *H;             /* history max psi+  [n_elems] (L98) */
+    void *fext_x, *fext_y; /* nodal external force (Eq. 17)   */
+} pff_state;
+
+/* Per-step boundary data.  dir_u / dir_v: device arrays of n_dir values (precision of the mesh),
+ * ordered like the dof list given to pff_set_dirichlet; may be NULL when n_dir == 0.
+ * load_scale multiplies fext in Eq. 17: S(t_{n+1}) of Eq. 19. */
+typedef struct {
+    const void *dir_u;   /* u_bar(t_{n+1}) */
+    const void *dir_v;   /* v_bar(t_{n+1}) */
+    double load_scale;
+} pff_bc;
+
+/* ---- mesh setup (Eq. 9) ------------------------------------------
+ * xy[n_nodes][2] (host, fp64), tri[n_elems][3] (host, int32, either orientation: clockwise
+ * elements are re-oriented, R1).  Computes areas, shape gradients (Eq. 9), inverse
+ * lumped mass (L169), h_min, the renumbering, the CTA chunks and their shared-memory gather
+ * tables, and uploads everything.  Input arrays are copied; *out is owned by the library.
+ * Errors: PFF_EINVAL (arguments/material), PFF_EMESH (bad index, degenerate element, orphan
+ * node, n_nodes >= 2^30), PFF_ENOMEM, PFF_ECUDA. */
+pff_status pff_mesh_create(int64_t n_nodes, const double *xy, int64_t n_elems, const int32_t *tri,
+                           const pff_material *material, const pff_options *options,
+                           void *cuda_stream, pff_mesh **out);
+void pff_mesh_destroy(pff_mesh *mesh);
+
+/* h_min = minimum element incircle diameter; dt_crit = h_min / c_p with
+ * c_p = sqrt((lambda + 2 mu) / rho) (L169; the caller applies the safety factor alpha).
+ * n_chunks / n_shared_nodes describe the decomposition (may be NULL). */
+pff_status pff_mesh_info(const pff_mesh *mesh, int64_t *n_nodes, int64_t *n_elems, double *h_min,
+                         double *dt_crit, int64_t *n_chunks, int64_t *n_shared_nodes);
+
+/* node_new_of_old[n_nodes], elem_new_of_old[n_elems] (host, may be NULL): internal index of
+ * each user node / element. */
+pff_status pff_mesh_permutations(const pff_mesh *mesh, int32_t *node_new_of_old, int32_t *elem_new_of_old);
+
+/* Host-only dry run of the mesh setup (no CUDA call): validates the mesh exactly like pff_mesh_create
+ * and returns the renumbering and the decomposition statistics.  Any output pointer may be NULL. */
+pff_status pff_mesh_plan(int64_t n_nodes, const double *xy, int64_t n_elems, const int32_t *tri,
+                         const pff_options *options, int32_t *node_new_of_old, int32_t *elem_new_of_old,
+                         int64_t *n_chunks, int64_t *n_shared_nodes, int32_t *chunk_elems, int32_t *max_local_nodes,
+                         double *h_min);
+
+/* Displacement Dirichlet set (Eq. 5): dir_dof[n_dir] (host, USER numbering, 2*node + comp).
+ * Replaces any previous set.  Values come per step through pff_bc. */
+pff_status pff_set_dirichlet(pff_mesh *mesh, int64_t n_dir, const int32_t *dir_dof);
+
+/* Damage Dirichlet set: nodes[n] (host, USER numbering) keep the value found in state->d during
+ * pff_damage_solve (notches / seeds, R14).  Replaces any previous set. */
+pff_status pff_set_damage_dirichlet(pff_mesh *mesh, int64_t n, const int32_t *nodes);
+
+/* Traction boundary (Eq. 5): edge_nodes[n_edges][2] (host, USER ids), t[n_edges][2] (host, force per
+ * unit length ... per unit thickness, i.e. Pa).  OVERWRITES state->fext_x/y with the consistent
+ * nodal load sum t L / 2 per end node (R8). */
+pff_status pff_set_traction(pff_mesh *mesh, pff_state *state, int64_t n_edges, const int32_t *edge_nodes,
+                            const double *t);
+
+/* a_0 = m^-1 (S f_ext - f_int(u_0, d_0)), zero on Dirichlet dofs (Eq. 17 at t = 0); u, v, H untouched. */
+pff_status pff_init_accel(pff_mesh *mesh, pff_state *state, const pff_bc *bc);
+
+/* One explicit step n -> n+1 with d fixed:
+ *   Eq. 16 predictor, Dirichlet overwrite; element strain -> split -> degraded stress -> internal
+ *   force (L42, L71-93, L124); scatter to nodes; Eq. 17; Eq. 18; H <- max(H, psi+) (L98, L114).
+ * On return (stream order) state holds (u, v, a, H)_{n+1}.  Asynchronous.  dt > 0. */
+pff_status pff_explicit_step(pff_mesh *mesh, pff_state *state, const pff_bc *bc, double dt);
+
+/* Damage solve for d_{n+1} from H_{n+1}, warm-started at d_n = state->d:
+ * matrix-free operator with consistent mass (L173, L185), Jacobi preconditioner (L177),
+ * AT2: PCG then d <- min(1, max(d_n, d)) (L179); AT1: projected PCG with lower bound d_n (L181).
+ * Stops when ||r_free||_2 <= rel_tol * max(||b||_2, ||b - A d_n||_2) (R10) or after max_iter
+ * operator applications (then returns PFF_ENOCONV with the result written).
+ * iters_out / relres_out (host, may be NULL) receive the mat-vec count and final relative residual.
+ * Synchronises the stream. */
+pff_status pff_damage_solve(pff_mesh *mesh, pff_state *state, double rel_tol, int32_t max_iter,
+                            int32_t *iters_out, double *relres_out);
+
+/* out = { E_el, E_kin, E_frac, E_tot } per unit thickness (Eq. 1), accumulated in fp64
+ * with a fixed reduction order.  Synchronises the stream. */
+pff_status pff_energies(pff_mesh *mesh, const pff_state *state, double out[4]);
+
+/* ---- test hooks (device vectors, internal order, precision of the mesh) ---------------------- */
+/* f_int(u, d) of the current state (no predictor), and psi+ per element (psi_plus may be NULL). */
+pff_status pff_internal_force(pff_mesh *mesh, const pff_state *state, void *fx, void *fy, void *psi_plus);
+/* q = A p with the damage operator built from state->H (L173). */
+pff_status pff_damage_matvec(pff_mesh *mesh, const pff_state *state, const void *p, void *q);
+/* Right-hand side b and Jacobi diagonal D of the damage system (either may be NULL). */
+pff_status pff_damage_rhs_diag(pff_mesh *mesh, const pff_state *state, void *b, void *D);
+
+/* ---- host-buffer convenience path (end-to-end timing, small problems) ------------------------
+ * State in USER numbering, fp64, AoS on the HOST: u, v, a, fext [n_nodes][2]; d [n_nodes];
+ * H [n_elems].  Uploads, converts to internal order / mesh precision on the device, runs n_steps of
+ * { pff_explicit_step ; pff_damage_solve every damage_every-th step (0 = never) } with constant
+ * Dirichlet values (dir_u, dir_v: host, n_dir entries, may be NULL) and load_scale, then downloads
+ * u, v, a, d, H back into the same host arrays.  Synchronous. */
+typedef struct {
+    double *u, *v, *a, *d, *H, *fext;
+} pff_host_state;
+pff_status pff_run_host(pff_mesh *mesh, pff_host_state *hs, const double *dir_u, const double *dir_v,
+                        double load_scale, double dt, int64_t n_steps, int32_t damage_every,
+                        double rel_tol, int32_t max_iter);
+
+const char *pff_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PFF_H */

@@ -1,0 +1,218 @@
+// Host-side mesh setup (Eq. 9): orientation, P1 geometry, lumped mass,
+// h_min, element ordering along a Morton curve, CTA chunks with interior-first / interface-last node
+// numbering, chunk-local connectivity and the shared-memory gather tables.
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <limits>
+#include <numeric>
+
+#include "pff_internal.h"
+
+namespace pff {
+
+static inline uint32_t spread16(uint32_t v)
+{
+    v &= 0xFFFFu;
+    v = (v | (v << 8)) & 0x00FF00FFu;
+    v = (v | (v << 4)) & 0x0F0F0F0Fu;
+    v = (v | (v << 2)) & 0x33333333u;
+    v = (v | (v << 1)) & 0x55555555u;
+    return v;
+}
+
+pff_status build_host_mesh(int64_t N, const double* xy, int64_t Ne, const int32_t* tri_in, double rho,
+                           int order, int chunk_elems, size_t real_bytes, size_t smem_limit, HostMesh& hm,
+                           std::string& err)
+{
+    if (N < 3 || Ne < 1) { err = "mesh needs at least 3 nodes and 1 element"; return PFF_EINVAL; }
+    if (N >= (int64_t(1) << 30) || Ne >= (int64_t(1) << 30)) { err = "mesh too large (>= 2^30)"; return PFF_EMESH; }
+    hm.N = N; hm.Ne = Ne;
+    hm.xy_user.assign(xy, xy + 2 * N);
+
+    // ---- orientation, areas, Eq. 9 gradients (fp64), h_min, in user order
+    std::vector<int32_t> tri(3 * Ne);
+    std::vector<double> g12u(4 * Ne), areau(Ne);
+    double xmin = std::numeric_limits<double>::infinity(), xmax = -xmin, ymin = xmin, ymax = -xmin;
+    for (int64_t i = 0; i < N; ++i) {
+        double x = xy[2 * i], y = xy[2 * i + 1];
+        if (!std::isfinite(x) || !std::isfinite(y)) { err = "non-finite node coordinate"; return PFF_EMESH; }
+        xmin = std::min(xmin, x); xmax = std::max(xmax, x);
+        ymin = std::min(ymin, y); ymax = std::max(ymax, y);
+    }
+    double hmin = std::numeric_limits<double>::infinity();
+    for (int64_t e = 0; e < Ne; ++e) {
+        int32_t n1 = tri_in[3 * e], n2 = tri_in[3 * e + 1], n3 = tri_in[3 * e + 2];
+        if (n1 < 0 || n2 < 0 || n3 < 0 || n1 >= N || n2 >= N || n3 >= N) {
+            err = "element " + std::to_string(e) + ": node index out of range"; return PFF_EMESH;
+        }
+        double x1 = xy[2 * n1], y1 = xy[2 * n1 + 1], x2 = xy[2 * n2], y2 = xy[2 * n2 + 1];
+        double x3 = xy[2 * n3], y3 = xy[2 * n3 + 1];
+        double twoA = (x2 - x1) * (y3 - y1) - (x3 - x1) * (y2 - y1);
+        if (twoA < 0.0) { std::swap(n2, n3); std::swap(x2, x3); std::swap(y2, y3); twoA = -twoA; }
+        double l12 = std::hypot(x2 - x1, y2 - y1), l23 = std::hypot(x3 - x2, y3 - y2), l31 = std::hypot(x1 - x3, y1 - y3);
+        double lmax = std::max(l12, std::max(l23, l31));
+        if (!(0.5 * twoA > 1e-14 * lmax * lmax)) {
+            err = "element " + std::to_string(e) + ": zero or near-zero area"; return PFF_EMESH;
+        }
+        tri[3 * e] = n1; tri[3 * e + 1] = n2; tri[3 * e + 2] = n3;
+        areau[e] = 0.5 * twoA;
+        g12u[4 * e + 0] = (y2 - y3) / twoA; g12u[4 * e + 1] = (x3 - x2) / twoA;
+        g12u[4 * e + 2] = (y3 - y1) / twoA; g12u[4 * e + 3] = (x1 - x3) / twoA;
+        hmin = std::min(hmin, 4.0 * areau[e] / (l12 + l23 + l31));
+    }
+    hm.hmin = hmin;
+
+    // ---- element order: Morton key of the centroid (or user order)
+    std::vector<int32_t> elem_old_of_new(Ne);
+    if (order == PFF_ORDER_MORTON) {
+        std::vector<uint64_t> keyed(Ne);
+        double sx = (xmax > xmin) ? 65535.0 / (xmax - xmin) : 0.0, sy = (ymax > ymin) ? 65535.0 / (ymax - ymin) : 0.0;
+        for (int64_t e = 0; e < Ne; ++e) {
+            const int32_t* t = &tri[3 * e];
+            double cx = (xy[2 * t[0]] + xy[2 * t[1]] + xy[2 * t[2]]) / 3.0;
+            double cy = (xy[2 * t[0] + 1] + xy[2 * t[1] + 1] + xy[2 * t[2] + 1]) / 3.0;
+            uint32_t qx = (uint32_t)std::min(65535.0, std::max(0.0, (cx - xmin) * sx));
+            uint32_t qy = (uint32_t)std::min(65535.0, std::max(0.0, (cy - ymin) * sy));
+            uint32_t key = spread16(qx) | (spread16(qy) << 1);
+            keyed[e] = (uint64_t(key) << 32) | uint64_t(uint32_t(e));
+        }
+        std::sort(keyed.begin(), keyed.end());
+        for (int64_t e = 0; e < Ne; ++e) elem_old_of_new[e] = int32_t(keyed[e] & 0xFFFFFFFFu);
+    } else {
+        std::iota(elem_old_of_new.begin(), elem_old_of_new.end(), 0);
+    }
+    hm.elem_new_of_old.resize(Ne);
+    for (int64_t e = 0; e < Ne; ++e) hm.elem_new_of_old[elem_old_of_new[e]] = int32_t(e);
+
+    // ---- chunks; shrink the chunk until the worst-case shared-memory footprint fits
+    int EC = chunk_elems > 0 ? chunk_elems : 1024;
+    EC = std::max(32, std::min(8192, (EC / 32) * 32));
+    std::vector<int32_t> cmin(N), cmax(N);
+    for (;;) {
+        std::fill(cmin.begin(), cmin.end(), std::numeric_limits<int32_t>::max());
+        std::fill(cmax.begin(), cmax.end(), -1);
+        for (int64_t en = 0; en < Ne; ++en) {
+            int32_t c = int32_t(en / EC);
+            const int32_t* t = &tri[3 * elem_old_of_new[en]];
+            for (int k = 0; k < 3; ++k) { cmin[t[k]] = std::min(cmin[t[k]], c); cmax[t[k]] = std::max(cmax[t[k]], c); }
+        }
+        // per-chunk local node count (interior + interface) via first-touch stamps
+        int64_t C = (Ne + EC - 1) / EC;
+        std::vector<int32_t> stamp(N, -1);
+        int32_t max_nloc = 0;
+        for (int64_t c = 0; c < C; ++c) {
+            int32_t nloc = 0;
+            for (int64_t en = c * EC; en < std::min<int64_t>(Ne, (c + 1) * EC); ++en) {
+                const int32_t* t = &tri[3 * elem_old_of_new[en]];
+                for (int k = 0; k < 3; ++k) if (stamp[t[k]] != c) { stamp[t[k]] = int32_t(c); ++nloc; }
+            }
+            max_nloc = std::max(max_nloc, nloc);
+        }
+        size_t smem = (size_t(3) * max_nloc + size_t(7) * EC) * real_bytes + 64;
+        if (smem <= smem_limit || EC <= 32) {
+            if (smem > smem_limit) { err = "chunk does not fit shared memory"; return PFF_EMESH; }
+            hm.max_nloc = max_nloc; hm.C = C;
+            break;
+        }
+        EC = std::max(32, (EC / 2 / 32) * 32);
+    }
+    hm.chunk_elems = EC;
+    const int64_t C = hm.C;
+    for (int64_t i = 0; i < N; ++i)
+        if (cmax[i] < 0) { err = "node " + std::to_string(i) + " belongs to no element (orphan)"; return PFF_EMESH; }
+
+    // ---- node numbering: chunk by chunk the interior nodes in first-touch order, then interface nodes
+    hm.node_new_of_old.assign(N, -1);
+    hm.meta.resize(C);
+    int32_t next = 0;
+    for (int64_t c = 0; c < C; ++c) {
+        ChunkMeta& m = hm.meta[c];
+        m.elem_start = int32_t(c * EC);
+        m.n_elem = int32_t(std::min<int64_t>(Ne, (c + 1) * EC) - c * EC);
+        m.node_start = next;
+        for (int64_t en = m.elem_start; en < m.elem_start + m.n_elem; ++en) {
+            const int32_t* t = &tri[3 * elem_old_of_new[en]];
+            for (int k = 0; k < 3; ++k)
+                if (cmin[t[k]] == cmax[t[k]] && hm.node_new_of_old[t[k]] < 0) hm.node_new_of_old[t[k]] = next++;
+        }
+        m.n_int = next - m.node_start;
+    }
+    hm.N_int = next;
+    for (int64_t en = 0; en < Ne; ++en) {
+        const int32_t* t = &tri[3 * elem_old_of_new[en]];
+        for (int k = 0; k < 3; ++k)
+            if (hm.node_new_of_old[t[k]] < 0) hm.node_new_of_old[t[k]] = next++;
+    }
+    hm.N_sh = N - hm.N_int;
+    hm.node_old_of_new.resize(N);
+    for (int64_t i = 0; i < N; ++i) hm.node_old_of_new[hm.node_new_of_old[i]] = int32_t(i);
+
+    // ---- per-chunk tables
+    hm.conn4.assign(4 * Ne, 0);
+    hm.lconn4.assign(4 * Ne, 0);
+    hm.g12.resize(4 * Ne);
+    hm.area.resize(Ne);
+    hm.mass.assign(N, 0.0);
+    std::vector<int32_t> sh_stamp(hm.N_sh, -1), sh_local(hm.N_sh, 0), sh_count(hm.N_sh + 1, 0);
+    std::vector<int32_t> val;  // valence per local node
+    hm.halo_ids.clear();
+    hm.ell.clear();
+    for (int64_t c = 0; c < C; ++c) {
+        ChunkMeta& m = hm.meta[c];
+        m.halo_off = int32_t(hm.halo_ids.size());
+        int32_t nh = 0;
+        for (int64_t en = m.elem_start; en < m.elem_start + m.n_elem; ++en) {
+            int64_t eo = elem_old_of_new[en];
+            for (int k = 0; k < 3; ++k) {
+                int32_t g = hm.node_new_of_old[tri[3 * eo + k]];
+                int32_t l;
+                if (g < hm.N_int) l = g - m.node_start;
+                else {
+                    int32_t s = g - int32_t(hm.N_int);
+                    if (sh_stamp[s] != c) { sh_stamp[s] = int32_t(c); sh_local[s] = nh++; hm.halo_ids.push_back(g); ++sh_count[s + 1]; }
+                    l = m.n_int + sh_local[s];
+                }
+                hm.conn4[4 * en + k] = g;
+                hm.lconn4[4 * en + k] = uint16_t(l);
+            }
+            for (int k = 0; k < 4; ++k) hm.g12[4 * en + k] = g12u[4 * eo + k];
+            hm.area[en] = areau[eo];
+        }
+        m.n_halo = nh;
+        const int32_t nloc = m.n_int + nh;
+        val.assign(nloc, 0);
+        for (int64_t en = m.elem_start; en < m.elem_start + m.n_elem; ++en)
+            for (int k = 0; k < 3; ++k) ++val[hm.lconn4[4 * en + k]];
+        int32_t w = 0;
+        for (int32_t i = 0; i < nloc; ++i) w = std::max(w, val[i]);
+        m.ell_w = w;
+        m.ell_off = int32_t(hm.ell.size());
+        if (hm.ell.size() + size_t(w) * nloc > size_t(std::numeric_limits<int32_t>::max())) {
+            err = "gather table too large"; return PFF_EMESH;
+        }
+        hm.ell.resize(hm.ell.size() + size_t(w) * nloc, uint16_t(0xFFFF));
+        std::fill(val.begin(), val.end(), 0);
+        for (int64_t en = m.elem_start; en < m.elem_start + m.n_elem; ++en)
+            for (int k = 0; k < 3; ++k) {
+                int32_t l = hm.lconn4[4 * en + k];
+                hm.ell[size_t(m.ell_off) + size_t(val[l]++) * nloc + l] = uint16_t(((en - m.elem_start) << 2) | k);
+            }
+        hm.max_ell_w = std::max(hm.max_ell_w, w);
+    }
+    // interface-node CSR over halo slots, ascending chunk (chunks were visited in order)
+    hm.sh_rowptr.assign(hm.N_sh + 1, 0);
+    for (int64_t s = 0; s < hm.N_sh; ++s) hm.sh_rowptr[s + 1] = hm.sh_rowptr[s] + sh_count[s + 1];
+    hm.sh_slots.resize(hm.halo_ids.size());
+    std::vector<int32_t> fill(hm.sh_rowptr.begin(), hm.sh_rowptr.end() - 1);
+    for (size_t slot = 0; slot < hm.halo_ids.size(); ++slot) {
+        int32_t s = hm.halo_ids[slot] - int32_t(hm.N_int);
+        hm.sh_slots[fill[s]++] = int32_t(slot);
+    }
+    // lumped mass m_i = rho sum A_e / 3 (L169), summed in internal element order
+    for (int64_t en = 0; en < Ne; ++en)
+        for (int k = 0; k < 3; ++k) hm.mass[hm.conn4[4 * en + k]] += rho * hm.area[en] / 3.0;
+    return PFF_OK;
+}
+
+}  // namespace pff

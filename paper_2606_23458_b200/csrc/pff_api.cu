@@ -1,0 +1,338 @@
+// C-ABI entry points of libpff (include/pff.h): argument checking, uploads, dispatch.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "pff_device.cuh"
+#include "pff_mesh.h"
+
+namespace pff {
+
+static thread_local std::string g_err;
+void set_error(const std::string& s) { g_err = s; }
+
+pff_status cuda_check(cudaError_t e, const char* what)
+{
+    if (e == cudaSuccess) return PFF_OK;
+    set_error(std::string(what) + ": " + cudaGetErrorString(e));
+    return PFF_ECUDA;
+}
+
+#define PFF_CUDA(call)                                                   \
+    do {                                                                 \
+        pff_status st__ = pff::cuda_check((call), #call);                \
+        if (st__ != PFF_OK) return st__;                                 \
+    } while (0)
+
+template <typename T>
+static pff_status upload(T** dst, const void* src, size_t count, cudaStream_t st)
+{
+    *dst = nullptr;
+    if (count == 0) count = 1;  // keep pointers valid
+    PFF_CUDA(cudaMalloc((void**)dst, count * sizeof(T)));
+    if (src) PFF_CUDA(cudaMemcpyAsync(*dst, src, count * sizeof(T), cudaMemcpyHostToDevice, st));
+    else PFF_CUDA(cudaMemsetAsync(*dst, 0, count * sizeof(T), st));
+    return PFF_OK;
+}
+
+// upload a fp64 host array narrowed to the mesh precision
+static pff_status upload_real(void** dst, const double* src, size_t count, size_t rb, cudaStream_t st)
+{
+    if (rb == 8) return upload((double**)dst, src, count, st);
+    std::vector<float> tmp(count);
+    for (size_t i = 0; i < count; ++i) tmp[i] = (float)src[i];
+    pff_status s = upload((float**)dst, tmp.data(), count, st);
+    if (s == PFF_OK) s = cuda_check(cudaStreamSynchronize(st), "upload sync");  // tmp dies at return
+    return s;
+}
+
+static bool valid_state(const pff_state* s)
+{
+    return s && s->ux && s->uy && s->vx && s->vy && s->ax && s->ay && s->d && s->H && s->fext_x && s->fext_y;
+}
+
+}  // namespace pff
+
+using namespace pff;
+
+extern "C" {
+
+const char* pff_last_error(void) { return g_err.c_str(); }
+
+void pff_mesh_destroy(pff_mesh* m)
+{
+    if (!m) return;
+    cudaStreamSynchronize(m->stream);
+    void* ptrs[] = {m->d_meta, m->d_lconn, m->d_conn, m->d_ga, m->d_gb, m->d_area, m->d_minv, m->d_mass,
+                    m->d_halo_ids, m->d_sh_rowptr, m->d_sh_slots, m->d_ell, m->d_flags, m->d_halo_part,
+                    m->d_fwx, m->d_fwy, m->d_dir_dof, m->d_lb, m->d_r, m->d_p, m->d_q, m->d_dinv, m->d_mask,
+                    m->d_part, m->d_ctrl, m->d_ticket, m->d_stage, m->d_hstate, m->d_node_old_of_new,
+                    m->d_elem_old_of_new};
+    for (void* p : ptrs) if (p) cudaFree(p);
+    if (m->h_ctrl) cudaFreeHost(m->h_ctrl);
+    delete m;
+}
+
+pff_status pff_mesh_create(int64_t n_nodes, const double* xy, int64_t n_elems, const int32_t* tri,
+                           const pff_material* mat, const pff_options* opt_in, void* cuda_stream, pff_mesh** out)
+{
+    if (out) *out = nullptr;
+    if (!xy || !tri || !mat || !out) { set_error("pff_mesh_create: null argument"); return PFF_EINVAL; }
+    pff_options opt{PFF_F64, PFF_ORDER_MORTON, PFF_SCATTER_GATHER, 0};
+    if (opt_in) opt = *opt_in;
+    if (!(mat->E > 0) || !(mat->rho > 0) || !(mat->Gc > 0) || !(mat->l0 > 0) || !(mat->nu > -1.0) || !(mat->nu < 0.5) ||
+        !(mat->eta >= 0) || !std::isfinite(mat->E + mat->rho + mat->Gc + mat->l0 + mat->eta)) {
+        set_error("pff_mesh_create: material out of range (need E, rho, Gc, l0 > 0, -1 < nu < 0.5, eta >= 0)");
+        return PFF_EINVAL;
+    }
+    if ((mat->model != PFF_AT1 && mat->model != PFF_AT2) || mat->split < 0 || mat->split > 3 ||
+        (mat->plane != PFF_PLANE_STRAIN && mat->plane != PFF_PLANE_STRESS) ||
+        (opt.precision != PFF_F64 && opt.precision != PFF_F32) ||
+        (opt.order != PFF_ORDER_NONE && opt.order != PFF_ORDER_MORTON) ||
+        (opt.scatter != PFF_SCATTER_GATHER && opt.scatter != PFF_SCATTER_ATOMIC) || opt.chunk_elems < 0) {
+        set_error("pff_mesh_create: bad enum value"); return PFF_EINVAL;
+    }
+    if (mat->split == PFF_SPLIT_STARCONVEX && !(mat->gamma_star >= -1.0)) {
+        set_error("pff_mesh_create: gamma_star must be >= -1"); return PFF_EINVAL;
+    }
+    pff_mesh* m = new (std::nothrow) pff_mesh;
+    if (!m) { set_error("out of host memory"); return PFF_ENOMEM; }
+    m->mat = *mat; m->opt = opt; m->stream = (cudaStream_t)cuda_stream;
+    m->rb = opt.precision == PFF_F32 ? 4 : 8;
+    std::string err;
+    pff_status st;
+    try {
+        st = build_host_mesh(n_nodes, xy, n_elems, tri, mat->rho, opt.order, opt.chunk_elems, m->rb, 200 * 1024, m->hm, err);
+    } catch (const std::bad_alloc&) { st = PFF_ENOMEM; err = "out of host memory in mesh setup"; }
+    if (st != PFF_OK) { set_error("pff_mesh_create: " + err); delete m; return st; }
+    HostMesh& hm = m->hm;
+    opt.chunk_elems = m->opt.chunk_elems = hm.chunk_elems;
+    {
+        const double mu = mat->E / (2 * (1 + mat->nu));
+        const double lam = mat->plane == PFF_PLANE_STRESS ? mat->E * mat->nu / (1 - mat->nu * mat->nu)
+                                                           : mat->E * mat->nu / ((1 + mat->nu) * (1 - 2 * mat->nu));
+        m->dt_crit = hm.hmin / std::sqrt((lam + 2 * mu) / mat->rho);
+    }
+    m->smem_step = int((size_t(3) * hm.max_nloc + size_t(6) * hm.chunk_elems) * m->rb);
+    m->smem_dmg = int((size_t(3) * hm.max_nloc + size_t(7) * hm.chunk_elems) * m->rb);
+
+    auto fail = [&](pff_status s) { pff_mesh_destroy(m); return s; };
+    cudaStream_t cs = m->stream;
+    if ((st = cuda_check(cudaGetDevice(&m->device), "cudaGetDevice")) != PFF_OK) return fail(st);
+    const size_t N = hm.N, Ne = hm.Ne;
+#define UP(call) if ((st = (call)) != PFF_OK) return fail(st)
+    UP(upload(&m->d_meta, hm.meta.data(), hm.meta.size(), cs));
+    UP(upload((uint16_t**)&m->d_lconn, hm.lconn4.data(), 4 * Ne, cs));
+    UP(upload((int32_t**)&m->d_conn, hm.conn4.data(), 4 * Ne, cs));
+    if (m->rb == 8) {
+        std::vector<double> ga(2 * Ne), gb(2 * Ne);
+        for (size_t e = 0; e < Ne; ++e) {
+            ga[2 * e] = hm.g12[4 * e]; ga[2 * e + 1] = hm.g12[4 * e + 1];
+            gb[2 * e] = hm.g12[4 * e + 2]; gb[2 * e + 1] = hm.g12[4 * e + 3];
+        }
+        UP(upload((double**)&m->d_ga, ga.data(), 2 * Ne, cs));
+        UP(upload((double**)&m->d_gb, gb.data(), 2 * Ne, cs));
+        UP(cuda_check(cudaStreamSynchronize(cs), "sync"));
+    } else {
+        UP(upload_real(&m->d_ga, hm.g12.data(), 4 * Ne, 4, cs));
+    }
+    UP(upload_real(&m->d_area, hm.area.data(), Ne, m->rb, cs));
+    {
+        std::vector<double> minv(N);
+        for (size_t i = 0; i < N; ++i) minv[i] = 1.0 / hm.mass[i];
+        UP(upload_real(&m->d_minv, minv.data(), N, m->rb, cs));
+        UP(upload_real(&m->d_mass, hm.mass.data(), N, m->rb, cs));
+        UP(cuda_check(cudaStreamSynchronize(cs), "sync"));
+    }
+    m->n_slots = (int64_t)hm.halo_ids.size();
+    UP(upload(&m->d_halo_ids, hm.halo_ids.data(), hm.halo_ids.size(), cs));
+    UP(upload(&m->d_sh_rowptr, hm.sh_rowptr.data(), hm.sh_rowptr.size(), cs));
+    UP(upload(&m->d_sh_slots, hm.sh_slots.data(), hm.sh_slots.size(), cs));
+    UP(upload(&m->d_ell, hm.ell.data(), hm.ell.size(), cs));
+    m->h_flags.assign(N, 0);
+    UP(upload(&m->d_flags, m->h_flags.data(), N, cs));
+    UP(upload((uint8_t**)&m->d_halo_part, nullptr, size_t(3) * std::max<int64_t>(m->n_slots, 1) * m->rb, cs));
+    UP(upload((uint8_t**)&m->d_fwx, nullptr, N * m->rb, cs));
+    UP(upload((uint8_t**)&m->d_fwy, nullptr, N * m->rb, cs));
+    UP(upload((uint8_t**)&m->d_lb, nullptr, N * m->rb, cs));
+    UP(upload((uint8_t**)&m->d_r, nullptr, N * m->rb, cs));
+    UP(upload((uint8_t**)&m->d_p, nullptr, N * m->rb, cs));
+    UP(upload((uint8_t**)&m->d_q, nullptr, N * m->rb, cs));
+    UP(upload((uint8_t**)&m->d_dinv, nullptr, N * m->rb, cs));
+    UP(upload(&m->d_mask, nullptr, 2 * N, cs));
+    UP(upload(&m->d_node_old_of_new, hm.node_old_of_new.data(), N, cs));
+    {
+        std::vector<int32_t> eon(Ne);
+        for (size_t e = 0; e < Ne; ++e) eon[hm.elem_new_of_old[e]] = (int32_t)e;
+        UP(upload(&m->d_elem_old_of_new, eon.data(), Ne, cs));
+        UP(cuda_check(cudaStreamSynchronize(cs), "sync"));
+    }
+#undef UP
+    if ((st = cuda_check(cudaStreamSynchronize(cs), "mesh upload")) != PFF_OK) return fail(st);
+    // the big host tables are no longer needed
+    std::vector<uint16_t>().swap(hm.lconn4); std::vector<uint16_t>().swap(hm.ell);
+    std::vector<double>().swap(hm.g12);
+    *out = m;
+    return PFF_OK;
+}
+
+pff_status pff_mesh_plan(int64_t n_nodes, const double* xy, int64_t n_elems, const int32_t* tri, const pff_options* opt_in,
+                         int32_t* node_new_of_old, int32_t* elem_new_of_old, int64_t* n_chunks, int64_t* n_shared,
+                         int32_t* chunk_elems, int32_t* max_local_nodes, double* h_min)
+{
+    if (!xy || !tri) { set_error("pff_mesh_plan: null argument"); return PFF_EINVAL; }
+    pff_options opt{PFF_F64, PFF_ORDER_MORTON, PFF_SCATTER_GATHER, 0};
+    if (opt_in) opt = *opt_in;
+    HostMesh hm;
+    std::string err;
+    pff_status st;
+    try {
+        st = build_host_mesh(n_nodes, xy, n_elems, tri, 1.0, opt.order, opt.chunk_elems, opt.precision == PFF_F32 ? 4 : 8,
+                             200 * 1024, hm, err);
+    } catch (const std::bad_alloc&) { st = PFF_ENOMEM; err = "out of host memory in mesh setup"; }
+    if (st != PFF_OK) { set_error("pff_mesh_plan: " + err); return st; }
+    if (node_new_of_old) std::memcpy(node_new_of_old, hm.node_new_of_old.data(), sizeof(int32_t) * hm.N);
+    if (elem_new_of_old) std::memcpy(elem_new_of_old, hm.elem_new_of_old.data(), sizeof(int32_t) * hm.Ne);
+    if (n_chunks) *n_chunks = hm.C;
+    if (n_shared) *n_shared = hm.N_sh;
+    if (chunk_elems) *chunk_elems = hm.chunk_elems;
+    if (max_local_nodes) *max_local_nodes = hm.max_nloc;
+    if (h_min) *h_min = hm.hmin;
+    return PFF_OK;
+}
+
+pff_status pff_mesh_info(const pff_mesh* m, int64_t* n_nodes, int64_t* n_elems, double* h_min, double* dt_crit,
+                         int64_t* n_chunks, int64_t* n_shared)
+{
+    if (!m) { set_error("pff_mesh_info: null mesh"); return PFF_EINVAL; }
+    if (n_nodes) *n_nodes = m->hm.N;
+    if (n_elems) *n_elems = m->hm.Ne;
+    if (h_min) *h_min = m->hm.hmin;
+    if (dt_crit) *dt_crit = m->dt_crit;
+    if (n_chunks) *n_chunks = m->hm.C;
+    if (n_shared) *n_shared = m->hm.N_sh;
+    return PFF_OK;
+}
+
+pff_status pff_mesh_permutations(const pff_mesh* m, int32_t* node_new_of_old, int32_t* elem_new_of_old)
+{
+    if (!m) { set_error("pff_mesh_permutations: null mesh"); return PFF_EINVAL; }
+    if (node_new_of_old) std::memcpy(node_new_of_old, m->hm.node_new_of_old.data(), sizeof(int32_t) * m->hm.N);
+    if (elem_new_of_old) std::memcpy(elem_new_of_old, m->hm.elem_new_of_old.data(), sizeof(int32_t) * m->hm.Ne);
+    return PFF_OK;
+}
+
+static pff_status push_flags(pff_mesh* m)
+{
+    PFF_CUDA(cudaMemcpyAsync(m->d_flags, m->h_flags.data(), m->h_flags.size(), cudaMemcpyHostToDevice, m->stream));
+    PFF_CUDA(cudaStreamSynchronize(m->stream));
+    return PFF_OK;
+}
+
+pff_status pff_set_dirichlet(pff_mesh* m, int64_t n_dir, const int32_t* dir_dof)
+{
+    if (!m || n_dir < 0 || (n_dir > 0 && !dir_dof)) { set_error("pff_set_dirichlet: bad argument"); return PFF_EINVAL; }
+    std::vector<int32_t> idof(n_dir);
+    for (int64_t k = 0; k < n_dir; ++k) {
+        if (dir_dof[k] < 0 || dir_dof[k] >= 2 * m->hm.N) { set_error("pff_set_dirichlet: dof out of range"); return PFF_EINVAL; }
+    }
+    for (auto& f : m->h_flags) f &= uint8_t(~3);
+    for (int64_t k = 0; k < n_dir; ++k) {
+        const int32_t node = m->hm.node_new_of_old[dir_dof[k] >> 1], comp = dir_dof[k] & 1;
+        idof[k] = 2 * node + comp;
+        m->h_flags[node] |= uint8_t(1 << comp);
+    }
+    PFF_CUDA(cudaStreamSynchronize(m->stream));
+    if (m->d_dir_dof) { cudaFree(m->d_dir_dof); m->d_dir_dof = nullptr; }
+    m->n_dir = n_dir;
+    pff_status st = upload(&m->d_dir_dof, idof.data(), (size_t)n_dir, m->stream);
+    if (st != PFF_OK) return st;
+    return push_flags(m);
+}
+
+pff_status pff_set_damage_dirichlet(pff_mesh* m, int64_t n, const int32_t* nodes)
+{
+    if (!m || n < 0 || (n > 0 && !nodes)) { set_error("pff_set_damage_dirichlet: bad argument"); return PFF_EINVAL; }
+    for (int64_t k = 0; k < n; ++k)
+        if (nodes[k] < 0 || nodes[k] >= m->hm.N) { set_error("pff_set_damage_dirichlet: node out of range"); return PFF_EINVAL; }
+    for (auto& f : m->h_flags) f &= uint8_t(~4);
+    for (int64_t k = 0; k < n; ++k) m->h_flags[m->hm.node_new_of_old[nodes[k]]] |= 4;
+    return push_flags(m);
+}
+
+pff_status pff_set_traction(pff_mesh* m, pff_state* s, int64_t n_edges, const int32_t* edge_nodes, const double* t)
+{
+    if (!m || !s || !s->fext_x || !s->fext_y || n_edges < 0 || (n_edges > 0 && (!edge_nodes || !t))) {
+        set_error("pff_set_traction: bad argument"); return PFF_EINVAL;
+    }
+    const int64_t N = m->hm.N;
+    std::vector<double> fx(N, 0.0), fy(N, 0.0);
+    const double* xy = m->hm.xy_user.data();
+    for (int64_t k = 0; k < n_edges; ++k) {
+        const int32_t a = edge_nodes[2 * k], b = edge_nodes[2 * k + 1];
+        if (a < 0 || b < 0 || a >= N || b >= N) { set_error("pff_set_traction: node out of range"); return PFF_EINVAL; }
+        const double L = std::hypot(xy[2 * a] - xy[2 * b], xy[2 * a + 1] - xy[2 * b + 1]);
+        const int32_t ia = m->hm.node_new_of_old[a], ib = m->hm.node_new_of_old[b];
+        fx[ia] += 0.5 * L * t[2 * k]; fx[ib] += 0.5 * L * t[2 * k];
+        fy[ia] += 0.5 * L * t[2 * k + 1]; fy[ib] += 0.5 * L * t[2 * k + 1];
+    }
+    if (m->rb == 8) {
+        PFF_CUDA(cudaMemcpyAsync(s->fext_x, fx.data(), N * 8, cudaMemcpyHostToDevice, m->stream));
+        PFF_CUDA(cudaMemcpyAsync(s->fext_y, fy.data(), N * 8, cudaMemcpyHostToDevice, m->stream));
+    } else {
+        std::vector<float> gx(fx.begin(), fx.end()), gy(fy.begin(), fy.end());
+        PFF_CUDA(cudaMemcpyAsync(s->fext_x, gx.data(), N * 4, cudaMemcpyHostToDevice, m->stream));
+        PFF_CUDA(cudaMemcpyAsync(s->fext_y, gy.data(), N * 4, cudaMemcpyHostToDevice, m->stream));
+        PFF_CUDA(cudaStreamSynchronize(m->stream));
+    }
+    PFF_CUDA(cudaStreamSynchronize(m->stream));
+    return PFF_OK;
+}
+
+pff_status pff_init_accel(pff_mesh* m, pff_state* s, const pff_bc* bc)
+{
+    if (!m || !valid_state(s)) { set_error("pff_init_accel: null mesh or state pointer"); return PFF_EINVAL; }
+    return launch_step(m, s, bc, 0.0, /*MODE_INIT*/ 1, nullptr, nullptr, nullptr);
+}
+
+pff_status pff_explicit_step(pff_mesh* m, pff_state* s, const pff_bc* bc, double dt)
+{
+    if (!m || !valid_state(s)) { set_error("pff_explicit_step: null mesh or state pointer"); return PFF_EINVAL; }
+    if (!(dt > 0) || !std::isfinite(dt)) { set_error("pff_explicit_step: dt must be > 0"); return PFF_EINVAL; }
+    return launch_step(m, s, bc, dt, /*MODE_STEP*/ 0, nullptr, nullptr, nullptr);
+}
+
+pff_status pff_internal_force(pff_mesh* m, const pff_state* s, void* fx, void* fy, void* psi_plus)
+{
+    if (!m || !valid_state(s) || !fx || !fy) { set_error("pff_internal_force: null argument"); return PFF_EINVAL; }
+    if (m->opt.scatter == PFF_SCATTER_ATOMIC) { set_error("pff_internal_force: gather meshes only"); return PFF_EUNSUPPORTED; }
+    return launch_step(m, const_cast<pff_state*>(s), nullptr, 0.0, /*MODE_FORCE*/ 2, fx, fy, psi_plus);
+}
+
+pff_status pff_damage_solve(pff_mesh* m, pff_state* s, double rel_tol, int32_t max_iter, int32_t* iters, double* relres)
+{
+    if (!m || !valid_state(s)) { set_error("pff_damage_solve: null mesh or state pointer"); return PFF_EINVAL; }
+    if (!(rel_tol > 0) || max_iter < 1) { set_error("pff_damage_solve: need rel_tol > 0, max_iter >= 1"); return PFF_EINVAL; }
+    return damage_solve(m, s, rel_tol, max_iter, iters, relres);
+}
+
+pff_status pff_damage_matvec(pff_mesh* m, const pff_state* s, const void* p, void* q)
+{
+    if (!m || !valid_state(s) || !p || !q) { set_error("pff_damage_matvec: null argument"); return PFF_EINVAL; }
+    return damage_matvec(m, s, p, q);
+}
+
+pff_status pff_damage_rhs_diag(pff_mesh* m, const pff_state* s, void* b, void* D)
+{
+    if (!m || !valid_state(s)) { set_error("pff_damage_rhs_diag: null argument"); return PFF_EINVAL; }
+    return damage_rhs_diag(m, s, b, D);
+}
+
+pff_status pff_energies(pff_mesh* m, const pff_state* s, double out[4])
+{
+    if (!m || !valid_state(s) || !out) { set_error("pff_energies: null argument"); return PFF_EINVAL; }
+    return energies(m, s, out);
+}
+
+}  // extern "C"

@@ -1,0 +1,154 @@
+// Device-side building blocks of libpff (sm_100a): element constitutive response, geometry loads,
+// block reductions.  Formulas cite PAPER.md; they are written independently of oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdint>
+
+#include "pff_internal.h"
+
+namespace pff {
+
+constexpr int kTPB = 256;  // threads per CTA of the chunk kernels
+
+template <typename R>
+struct MatC {  // material constants folded on the host
+    R lam;     // lambda_PE or lambda_PS
+    R mu;
+    R K;       // 3-D bulk modulus
+    R cz;      // eps_zz = cz * tr_2D (0 in plane strain, -nu/(1-nu) in plane stress)
+    R gs;      // gamma_star (0 for vol-dev)
+    R eta;
+    // damage equation (Eq. 6 / Eq. 8): c_e = c0 + 2 H_e, kappa, s_e = 2 H_e - s0
+    R c0, kappa, s0;
+    // fracture energy (L69)
+    R Gc, l0;
+    int model;
+};
+
+// Host: fold the material into kernel constants (Eq. 6, Eq. 8).
+template <typename R>
+inline MatC<R> make_matc(const pff_material& m)
+{
+    MatC<R> c;
+    const double mu = m.E / (2.0 * (1.0 + m.nu));
+    const double lam = (m.plane == PFF_PLANE_STRESS) ? m.E * m.nu / (1.0 - m.nu * m.nu)
+                                                      : m.E * m.nu / ((1.0 + m.nu) * (1.0 - 2.0 * m.nu));
+    c.lam = R(lam); c.mu = R(mu); c.K = R(m.E / (3.0 * (1.0 - 2.0 * m.nu)));
+    c.cz = R((m.plane == PFF_PLANE_STRESS) ? -m.nu / (1.0 - m.nu) : 0.0);
+    c.gs = R(m.split == PFF_SPLIT_STARCONVEX ? m.gamma_star : 0.0);
+    c.eta = R(m.eta);
+    if (m.model == PFF_AT2) { c.c0 = R(m.Gc / m.l0); c.kappa = R(m.Gc * m.l0); c.s0 = R(0); }
+    else { c.c0 = R(0); c.kappa = R(0.75 * m.Gc * m.l0); c.s0 = R(3.0 * m.Gc / (8.0 * m.l0)); }
+    c.Gc = R(m.Gc); c.l0 = R(m.l0); c.model = m.model;
+    return c;
+}
+
+template <typename R> __device__ __forceinline__ R rmax(R a, R b) { return a > b ? a : b; }
+template <typename R> __device__ __forceinline__ R rmin(R a, R b) { return a < b ? a : b; }
+__device__ __forceinline__ double rsqrt_(double x) { return sqrt(x); }
+__device__ __forceinline__ float rsqrt_(float x) { return sqrtf(x); }
+__device__ __forceinline__ double rfma(double a, double b, double c) { return fma(a, b, c); }
+__device__ __forceinline__ float rfma(float a, float b, float c) { return fmaf(a, b, c); }
+
+// Element response: undegraded psi+ / psi- and degraded in-plane stress
+//   sigma = g dpsi+/deps + dpsi-/deps,  g = (1 - d_e)^2 + eta (L79).
+// SPLIT 1: spectral (Eq. 2) with closed-form principal strains of the 2x2 strain, eigenvector-free
+//          stress  sigma+- = lam <tr>+- I + mu (s+-) I + mu (q+-) (eps - m I)/R.
+// SPLIT 2/3: vol-dev (Eq. 3) / star-convex on the 3-D strain with eps_zz slaved (L85).
+// SPLIT 0: isotropic (L79).
+template <typename R, int SPLIT>
+__device__ __forceinline__ void elem_response(const MatC<R>& m, R exx, R eyy, R exy, R g, R& psi_p, R& psi_m,
+                                              R& sxx, R& syy, R& sxy)
+{
+    const R zero = R(0), half = R(0.5), two = R(2);
+    if (SPLIT == PFF_SPLIT_SPECTRAL) {
+        const R tr = exx + eyy, mean = half * tr, dd = half * (exx - eyy);
+        const R rad = rsqrt_(dd * dd + exy * exy);
+        const R e1 = mean + rad, e2 = mean - rad;
+        const R e1p = rmax(e1, zero), e2p = rmax(e2, zero), e1m = rmin(e1, zero), e2m = rmin(e2, zero);
+        const R trp = rmax(tr, zero), trm = rmin(tr, zero);
+        psi_p = half * m.lam * trp * trp + m.mu * (e1p * e1p + e2p * e2p);
+        psi_m = half * m.lam * trm * trm + m.mu * (e1m * e1m + e2m * e2m);
+        const R inv = rad > zero ? R(1) / rad : zero;
+        const R qp = (e1p - e2p) * inv, qm = (e1m - e2m) * inv;
+        const R hp = m.lam * trp + m.mu * (e1p + e2p), hm = m.lam * trm + m.mu * (e1m + e2m);
+        const R dev = m.mu * (g * qp + qm);  // multiplies (eps - mean I)
+        const R hyd = g * hp + hm;
+        sxx = hyd + dev * dd;
+        syy = hyd - dev * dd;
+        sxy = dev * exy;
+    } else if (SPLIT == PFF_SPLIT_ISOTROPIC) {
+        const R tr = exx + eyy;
+        psi_p = half * m.lam * tr * tr + m.mu * (exx * exx + eyy * eyy + two * exy * exy);
+        psi_m = zero;
+        sxx = g * (m.lam * tr + two * m.mu * exx);
+        syy = g * (m.lam * tr + two * m.mu * eyy);
+        sxy = g * (two * m.mu * exy);
+    } else {
+        const R gs = (SPLIT == PFF_SPLIT_STARCONVEX) ? m.gs : zero;
+        const R tr2 = exx + eyy, ezz = m.cz * tr2, tr3 = tr2 + ezz, third = tr3 * R(1.0 / 3.0);
+        const R dxx = exx - third, dyy = eyy - third, dzz = ezz - third;
+        const R e2 = dxx * dxx + dyy * dyy + dzz * dzz + two * exy * exy;
+        const R trp = rmax(tr3, zero), trm = rmin(tr3, zero);
+        psi_p = half * m.K * (trp * trp - gs * trm * trm) + m.mu * e2;
+        psi_m = (R(1) + gs) * half * m.K * trm * trm;
+        const R p = m.K * (R(1) + m.cz) * (g * (trp - gs * trm) + (R(1) + gs) * trm);
+        const R tmg = two * m.mu * g;
+        sxx = p + tmg * (dxx + m.cz * dzz);
+        syy = p + tmg * (dyy + m.cz * dzz);
+        sxy = tmg * exy;
+    }
+}
+
+// Compact P1 geometry: grad phi1 = (b1, c1), grad phi2 = (b2, c2), grad phi3 = -(grad phi1 + grad phi2)
+// (rows of Eq. 9 sum to zero), read as 128-bit loads.
+template <typename R> struct Geo;
+template <> struct Geo<double> {
+    static __device__ __forceinline__ void load(const void* ga, const void* gb, int e, double& b1, double& c1,
+                                                double& b2, double& c2)
+    {
+        const double2 p = __ldg(reinterpret_cast<const double2*>(ga) + e);
+        const double2 q = __ldg(reinterpret_cast<const double2*>(gb) + e);
+        b1 = p.x; c1 = p.y; b2 = q.x; c2 = q.y;
+    }
+};
+template <> struct Geo<float> {
+    static __device__ __forceinline__ void load(const void* ga, const void*, int e, float& b1, float& c1,
+                                                float& b2, float& c2)
+    {
+        const float4 p = __ldg(reinterpret_cast<const float4*>(ga) + e);
+        b1 = p.x; c1 = p.y; b2 = p.z; c2 = p.w;
+    }
+};
+
+// Deterministic block sum in fp64 (fixed shuffle tree, fixed warp order); result valid in thread 0.
+__device__ __forceinline__ double block_sum(double v, double* s_red /* >= 32 doubles */)
+{
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31, nw = (blockDim.x + 31) >> 5;
+    __syncthreads();
+    if (l == 0) s_red[w] = v;
+    __syncthreads();
+    double t = 0.0;
+    if (w == 0) {
+        t = l < nw ? s_red[l] : 0.0;
+        for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+    }
+    return t;
+}
+__device__ __forceinline__ double block_min(double v, double* s_red)
+{
+    for (int o = 16; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o));
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31, nw = (blockDim.x + 31) >> 5;
+    __syncthreads();
+    if (l == 0) s_red[w] = v;
+    __syncthreads();
+    double t = INFINITY;
+    if (w == 0) {
+        t = l < nw ? s_red[l] : INFINITY;
+        for (int o = 16; o > 0; o >>= 1) t = fmin(t, __shfl_xor_sync(0xffffffffu, t, o));
+    }
+    return t;
+}
+
+}  // namespace pff

@@ -1,0 +1,62 @@
+// The opaque pff_mesh object: host tables + device copies + workspaces.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <string>
+#include <vector>
+
+#include "pff_internal.h"
+
+struct DamageCtrl;  // device-resident CG control block (pff_damage.cu)
+
+struct pff_mesh {
+    pff::HostMesh hm;
+    pff_material mat{};
+    pff_options opt{};
+    cudaStream_t stream = nullptr;
+    int device = 0;
+    size_t rb = 8;  // bytes per real
+    double dt_crit = 0.0;
+    int smem_step = 0, smem_dmg = 0;
+
+    // device mesh tables
+    pff::ChunkMeta* d_meta = nullptr;
+    void* d_lconn = nullptr;  // ushort4[Ne]
+    void* d_conn = nullptr;   // int4[Ne]
+    void *d_ga = nullptr, *d_gb = nullptr, *d_area = nullptr, *d_minv = nullptr, *d_mass = nullptr;
+    int32_t *d_halo_ids = nullptr, *d_sh_rowptr = nullptr, *d_sh_slots = nullptr;
+    uint16_t* d_ell = nullptr;
+    uint8_t* d_flags = nullptr;  // bit0: u_x Dirichlet, bit1: u_y Dirichlet, bit2: damage Dirichlet
+    void* d_halo_part = nullptr;  // [3][n_slots] reals: per (chunk, interface node) partial sums
+    int64_t n_slots = 0;
+    void *d_fwx = nullptr, *d_fwy = nullptr;  // atomic-scatter force accumulators (kept zero between steps)
+
+    // Dirichlet set
+    int64_t n_dir = 0;
+    int32_t* d_dir_dof = nullptr;  // internal node * 2 + comp
+    std::vector<uint8_t> h_flags;
+
+    // damage solve workspaces (reals [N] unless noted)
+    void *d_lb = nullptr, *d_r = nullptr, *d_p = nullptr, *d_q = nullptr, *d_dinv = nullptr;
+    uint8_t* d_mask = nullptr;   // [2][N] free-set masks (ping-pong)
+    double* d_part = nullptr;    // block partials [kPartStride * n_part_blocks]
+    int64_t n_part_blocks = 0;
+    DamageCtrl* d_ctrl = nullptr;
+    DamageCtrl* h_ctrl = nullptr;  // pinned
+    unsigned int* d_ticket = nullptr;
+
+    // host-path staging (pff_run_host)
+    void* d_stage = nullptr; size_t stage_bytes = 0;
+    void* d_hstate = nullptr;  // device state arrays owned by the library for pff_run_host
+    int32_t *d_node_old_of_new = nullptr, *d_elem_old_of_new = nullptr;
+};
+
+namespace pff {
+// implemented in pff_step.cu / pff_damage.cu / pff_energy.cu
+pff_status launch_step(pff_mesh* m, pff_state* s, const pff_bc* bc, double dt, int mode, void* fx, void* fy, void* psi);
+pff_status damage_solve(pff_mesh* m, pff_state* s, double rel_tol, int max_iter, int* iters, double* relres);
+pff_status damage_matvec(pff_mesh* m, const pff_state* s, const void* p, void* q);
+pff_status damage_rhs_diag(pff_mesh* m, const pff_state* s, void* b, void* D);
+pff_status energies(pff_mesh* m, const pff_state* s, double out[4]);
+pff_status cuda_check(cudaError_t e, const char* what);
+}  // namespace pff

@@ -1,0 +1,232 @@
+"""GPU-vs-oracle parity through the C ABI (run with -m gpu on a B200).
+
+Tolerances (north_star): max-norm relative error <= 1e-11 in fp64 (gather path bit-identical run to run),
+<= 2e-5 in fp32; 1e-6 relative on trajectory energies.  Both sides get the same seeded inputs.
+"""
+import itertools
+
+import numpy as np
+import pytest
+
+from pff_inputs import GLASS, config, random_mesh, grid_mesh, shear_bc
+from _harness import gpu_fields, gpu_from, oracle_from, relmax
+
+pytestmark = pytest.mark.gpu
+
+TOL64, TOL32 = 1e-11, 2e-5
+
+
+def _random_cfg(n_side, seed, **mat):
+    xy, tri = random_mesh(n_side, seed=seed)
+    rng = np.random.default_rng(seed + 1000)
+    N = len(xy)
+    material = dict(GLASS, model=2, split=1, plane=0)
+    material.update(mat)
+    return dict(name="random", xy=xy, tri=tri, material=material, notch=np.zeros(0, np.int32),
+                edges=np.zeros((0, 2), np.int32), traction=np.zeros((0, 2)), dir_dof=np.zeros(0, np.int32),
+                d0=rng.uniform(0, 0.9, N), u0=rng.normal(0, 2e-5, (N, 2)), dt_factor=0.5, steps=10)
+
+
+@pytest.mark.parametrize("split,plane", list(itertools.product([0, 1, 2, 3], [0, 1])))
+def test_internal_force_and_history_parity(split, plane):
+    cfg = _random_cfg(40, seed=split * 2 + plane, split=split, plane=plane, gamma_star=0.8)
+    orc = oracle_from(cfg)
+    f_ref, pp_ref = orc.internal_force()
+    for chunk in (0, 64):
+        mesh, st = gpu_from(cfg, chunk_elems=chunk)
+        fx, fy, pp = mesh.pff_internal_force(st)
+        f = np.stack([mesh.nodes_to_user(fx), mesh.nodes_to_user(fy)], 1)
+        assert relmax(f, f_ref) <= TOL64
+        assert relmax(mesh.elems_to_user(pp), pp_ref) <= TOL64
+
+
+@pytest.mark.parametrize("scatter", [0, 1])
+@pytest.mark.parametrize("precision", [0, 1])
+def test_single_step_parity_config1(scatter, precision):
+    cfg = config(1)
+    tol = TOL64 if precision == 0 else TOL32
+    orc = oracle_from(cfg)
+    mesh, st = gpu_from(cfg, precision=precision, scatter=scatter)
+    dt = cfg["dt_factor"] * orc.dt_crit()
+    assert abs(mesh.dt_crit - orc.dt_crit()) <= 1e-14 * orc.dt_crit()
+    orc.init_accel()
+    mesh.pff_init_accel(st, mesh.bc())
+    _, _, a, _, _ = gpu_fields(mesh, st)
+    assert relmax(a, orc.a) <= tol
+    for _ in range(3):
+        orc.explicit_step(dt)
+        mesh.pff_explicit_step(st, mesh.bc(), dt)
+    u, v, a, d, H = gpu_fields(mesh, st)
+    assert relmax(u, orc.u) <= tol and relmax(v, orc.v) <= tol and relmax(a, orc.a) <= tol
+    assert relmax(H, orc.H) <= tol
+
+
+def test_gather_path_bit_identical_across_runs():
+    cfg = config(2, scale=0.25)
+    outs = []
+    for rep in range(2):
+        mesh, st = gpu_from(cfg)
+        dt = 0.5 * mesh.dt_crit
+        mesh.pff_init_accel(st, mesh.bc())
+        for _ in range(20):
+            mesh.pff_explicit_step(st, mesh.bc(), dt)
+            mesh.pff_damage_solve(st, rel_tol=1e-8)
+        outs.append([x.copy() for x in gpu_fields(mesh, st)] + [mesh.pff_energies(st)])
+    for a, b in zip(*outs):
+        assert np.array_equal(a, b)
+
+
+@pytest.mark.parametrize("precision", [0, 1])
+def test_step_parity_config2_jittered_permuted(precision):
+    cfg = config(2, scale=0.5)
+    tol = TOL64 if precision == 0 else TOL32
+    orc = oracle_from(cfg)
+    mesh, st = gpu_from(cfg, precision=precision)
+    assert mesh.n_chunks > 4 and mesh.n_shared > 0
+    dt = 0.5 * orc.dt_crit()
+    orc.init_accel()
+    mesh.pff_init_accel(st, mesh.bc())
+    for _ in range(5):
+        orc.explicit_step(dt)
+        mesh.pff_explicit_step(st, mesh.bc(), dt)
+    u, v, a, d, H = gpu_fields(mesh, st)
+    assert relmax(u, orc.u) <= tol and relmax(v, orc.v) <= tol and relmax(a, orc.a) <= tol and relmax(H, orc.H) <= tol
+
+
+@pytest.mark.parametrize("model", [1, 2])
+@pytest.mark.parametrize("precision", [0, 1])
+def test_damage_operator_rhs_diag_parity(model, precision):
+    cfg = _random_cfg(40, seed=77, model=model, Gc=2.0, l0=0.05)
+    orc = oracle_from(cfg)
+    rng = np.random.default_rng(5)
+    orc.H = rng.uniform(0, 40, orc.Ne)
+    mesh, st = gpu_from(cfg, precision=precision, chunk_elems=128)
+    st.H.copy_(mesh.elems_to_internal(orc.H))
+    p = rng.normal(0, 1, orc.N)
+    q = mesh.pff_damage_matvec(st, mesh.nodes_to_internal(p))
+    tol = 1e-13 if precision == 0 else TOL32
+    assert relmax(mesh.nodes_to_user(q), orc.damage_matvec(p)) <= tol
+    b, D = mesh.pff_damage_rhs_diag(st)
+    b_ref, D_ref = orc.damage_rhs_diag()
+    assert relmax(mesh.nodes_to_user(b), b_ref) <= tol and relmax(mesh.nodes_to_user(D), D_ref) <= tol
+
+
+@pytest.mark.parametrize("model", [1, 2])
+def test_damage_solve_parity(model):
+    """Both sides converge to rel_tol = 1e-13, i.e. to the unique solution (R13)."""
+    cfg = config(1)
+    cfg["material"] = dict(cfg["material"], model=model)
+    orc = oracle_from(cfg)
+    mesh, st = gpu_from(cfg)
+    dt = 0.5 * orc.dt_crit()
+    orc.init_accel()
+    mesh.pff_init_accel(st, mesh.bc())
+    # load hard enough that H exceeds the AT1 threshold near the notch tip
+    for k in range(30):
+        orc.explicit_step(dt, S=40.0)
+        mesh.pff_explicit_step(st, mesh.bc(load_scale=40.0), dt)
+    rc, it, rr = orc.damage_solve(rel_tol=1e-13, max_iter=4000)
+    stt, it_g, rr_g = mesh.pff_damage_solve(st, rel_tol=1e-13, max_iter=4000)
+    assert rc == 0 and stt == 0
+    d = mesh.nodes_to_user(st.d)
+    assert orc.d.max() == 1.0 and np.any((orc.d > 1e-3) & (orc.d < 1.0))
+    assert relmax(d, orc.d) <= TOL64
+    assert np.all(d >= cfg["d0"]) and d.max() <= 1.0 and d.min() >= 0.0
+
+
+@pytest.mark.parametrize("model,split,plane", [(2, 2, 0), (1, 3, 1), (2, 1, 0)])
+def test_trajectory_energies_config1(model, split, plane):
+    """200 staggered steps of config 1 (and AT1 / star-convex / plane-stress variants): energies to 1e-6."""
+    cfg = config(1)
+    cfg["material"] = dict(cfg["material"], model=model, split=split, plane=plane, gamma_star=1.0)
+    orc = oracle_from(cfg)
+    mesh, st = gpu_from(cfg)
+    dt = 0.5 * orc.dt_crit()
+    S = 8.0
+    orc.init_accel(S)
+    mesh.pff_init_accel(st, mesh.bc(load_scale=S))
+    for k in range(200):
+        orc.explicit_step(dt, S=S)
+        rc, _, _ = orc.damage_solve(rel_tol=1e-10)
+        mesh.pff_explicit_step(st, mesh.bc(load_scale=S), dt)
+        stt, _, _ = mesh.pff_damage_solve(st, rel_tol=1e-10)
+        assert rc == 0 and stt == 0
+    e_ref, e = orc.energies(), mesh.pff_energies(st)
+    assert np.all(np.abs(e - e_ref) <= 1e-6 * np.abs(e_ref).max())
+    u, v, a, d, H = gpu_fields(mesh, st)
+    assert relmax(d, orc.d) <= 1e-7 and relmax(u, orc.u) <= 1e-7
+    # crack tip (furthest x with d >= 0.5) within one element width
+    tip = lambda dd: cfg["xy"][dd >= 0.5, 0].max()
+    assert abs(tip(d) - tip(orc.d)) <= 1e-3 + 1e-12
+
+
+def test_config3_dirichlet_shear_at1_starconvex():
+    cfg = config(3, scale=0.06)
+    orc = oracle_from(cfg)
+    mesh, st = gpu_from(cfg, chunk_elems=256)
+    dt = 0.5 * orc.dt_crit()
+    orc.init_accel()
+    mesh.pff_init_accel(st, mesh.bc())
+    for k in range(1, 61):
+        du, dv = shear_bc(cfg, k, dt)
+        orc.explicit_step(dt, dir_u=du, dir_v=dv)
+        rc, _, _ = orc.damage_solve(rel_tol=1e-12, max_iter=4000)
+        mesh.pff_explicit_step(st, mesh.bc(du, dv), dt)
+        stt, _, _ = mesh.pff_damage_solve(st, rel_tol=1e-12, max_iter=4000)
+        assert rc == 0 and stt == 0
+    u, v, a, d, H = gpu_fields(mesh, st)
+    assert relmax(u, orc.u) <= 1e-9 and relmax(v, orc.v) <= 1e-9 and relmax(H, orc.H) <= 1e-9
+    assert relmax(d, orc.d) <= 1e-8
+    e_ref, e = orc.energies(), mesh.pff_energies(st)
+    assert np.all(np.abs(e - e_ref) <= 1e-6 * np.abs(e_ref).max())
+
+
+def test_edge_cases_tiny_and_ragged():
+    # single element; two elements; chunk tail of 1 element; user order without renumbering
+    xy = np.array([[0.0, 0.0], [1e-3, 0.0], [0.0, 1e-3], [1e-3, 1e-3]])
+    for tri in (np.array([[0, 1, 2]], np.int32), np.array([[0, 1, 2], [1, 3, 2]], np.int32)):
+        n = tri.max() + 1
+        cfg = dict(xy=xy[:n], tri=tri, material=dict(GLASS, model=2, split=1, plane=0), notch=np.zeros(0, np.int32),
+                   edges=np.zeros((0, 2), np.int32), traction=np.zeros((0, 2)), dir_dof=np.zeros(0, np.int32),
+                   d0=np.linspace(0, 0.5, n), u0=1e-6 * np.arange(2 * n).reshape(n, 2) ** 1.5)
+        orc = oracle_from(cfg)
+        mesh, st = gpu_from(cfg)
+        fx, fy, pp = mesh.pff_internal_force(st)
+        f_ref, pp_ref = orc.internal_force()
+        assert relmax(np.stack([mesh.nodes_to_user(fx), mesh.nodes_to_user(fy)], 1), f_ref) <= TOL64
+    cfg = _random_cfg(9, seed=3)  # 128 elements
+    cfg["tri"] = cfg["tri"][:97]  # ragged: 3 chunks of 32 + tail of 1; drop orphan nodes
+    used = np.unique(cfg["tri"])
+    remap = -np.ones(len(cfg["xy"]), dtype=np.int64)
+    remap[used] = np.arange(len(used))
+    cfg["tri"] = remap[cfg["tri"]].astype(np.int32)
+    for k in ("xy", "d0", "u0"):
+        cfg[k] = cfg[k][used]
+    orc = oracle_from(cfg)
+    for order in (0, 1):
+        mesh, st = gpu_from(cfg, chunk_elems=32, order=order)
+        assert mesh.n_chunks == 4
+        dt = 0.5 * orc.dt_crit()
+        o2 = oracle_from(cfg)
+        o2.init_accel()
+        mesh.pff_init_accel(st, mesh.bc())
+        o2.explicit_step(dt)
+        mesh.pff_explicit_step(st, mesh.bc(), dt)
+        u, v, a, d, H = gpu_fields(mesh, st)
+        assert relmax(u, o2.u) <= TOL64 and relmax(a, o2.a) <= TOL64 and relmax(H, o2.H) <= TOL64
+
+
+def test_run_host_matches_device_path():
+    cfg = config(1, scale=0.5)
+    orc = oracle_from(cfg)
+    mesh, st = gpu_from(cfg)
+    dt = 0.5 * orc.dt_crit()
+    orc.init_accel(5.0)
+    u, v, a = orc.u.copy(), orc.v.copy(), orc.a.copy()
+    d, H, fext = orc.d.copy(), orc.H.copy(), orc.fext.copy()
+    mesh.pff_run_host(u, v, a, d, H, fext, dt, 25, damage_every=1, rel_tol=1e-12, load_scale=5.0)
+    for _ in range(25):
+        orc.explicit_step(dt, S=5.0)
+        assert orc.damage_solve(rel_tol=1e-12)[0] == 0
+    assert relmax(u, orc.u) <= 1e-10 and relmax(v, orc.v) <= 1e-10 and relmax(d, orc.d) <= 1e-10
+    assert relmax(H, orc.H) <= 1e-10

@@ -1,0 +1,120 @@
+"""CPU-only checks of the C-ABI library: it loads, exports every symbol include/pff.h declares, rejects
+bad input before touching CUDA, and its host-side mesh planning (renumbering / chunk decomposition) is
+consistent.  No kernel is launched here."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+from pff_inputs import GLASS, config, grid_mesh, random_mesh
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2606_23458_b200 import build, _lib
+    build.build()
+    return _lib.load()
+
+
+def test_library_exports_every_declared_symbol(lib):
+    from paper_2606_23458_b200 import _lib
+    header = open(os.path.join(ROOT, "include", "pff.h")).read()
+    declared = set(re.findall(r"\b(pff_[a-z_]+)\s*\(", header))
+    assert declared == set(_lib.SYMBOLS), declared ^ set(_lib.SYMBOLS)
+    for name in declared:
+        assert hasattr(lib, name), name
+
+
+def _plan(lib, xy, tri, chunk=0, order=1, precision=0):
+    from paper_2606_23458_b200 import _lib
+    xy = np.ascontiguousarray(xy, dtype=np.float64)
+    tri = np.ascontiguousarray(tri, dtype=np.int32)
+    opt = _lib.pff_options(precision, order, 0, chunk)
+    nn = np.empty(len(xy), np.int32)
+    en = np.empty(len(tri), np.int32)
+    nc, ns = C.c_int64(), C.c_int64()
+    ec, ml = C.c_int32(), C.c_int32()
+    hm = C.c_double()
+    st = lib.pff_mesh_plan(len(xy), xy.ctypes.data, len(tri), tri.ctypes.data, C.byref(opt), nn.ctypes.data,
+                           en.ctypes.data, C.byref(nc), C.byref(ns), C.byref(ec), C.byref(ml), C.byref(hm))
+    return st, nn, en, nc.value, ns.value, ec.value, ml.value, hm.value
+
+
+@pytest.mark.parametrize("order", [0, 1])
+def test_plan_is_a_valid_decomposition(lib, order):
+    cfg = config(2, scale=0.2)
+    xy, tri = cfg["xy"], cfg["tri"]
+    st, nn, en, nc, ns, ec, ml, hmin = _plan(lib, xy, tri, chunk=256, order=order)
+    assert st == 0
+    N, Ne = len(xy), len(tri)
+    assert sorted(nn) == list(range(N)) and sorted(en) == list(range(Ne))  # bijections
+    assert ec == 256 and nc == -(-Ne // 256)
+    # recompute interior / interface classification from the permutations alone
+    chunk_of_elem = en // ec
+    cmin = np.full(N, 1 << 30)
+    cmax = np.full(N, -1)
+    for k in range(3):
+        np.minimum.at(cmin, tri[:, k], chunk_of_elem)
+        np.maximum.at(cmax, tri[:, k], chunk_of_elem)
+    shared = cmin != cmax
+    assert ns == shared.sum()
+    assert np.all(nn[shared] >= N - ns) and np.all(nn[~shared] < N - ns)  # interface nodes numbered last
+    # interior nodes of a chunk are contiguous and ordered by chunk
+    order_int = np.argsort(nn[~shared])
+    assert np.all(np.diff(cmin[~shared][order_int]) >= 0)
+    if order == 1:
+        assert ns < 0.5 * N  # Morton order undoes the random element permutation of config 2
+    # h_min against the closed form of the unjittered grid
+    xy0, tri0 = grid_mesh(21, 9, 0.02, 0.008)
+    assert abs(_plan(lib, xy0, tri0)[7] - (2 - np.sqrt(2)) * 1e-3) < 1e-15
+
+
+def test_chunk_shrinks_to_fit_shared_memory(lib):
+    # user order + random element permutation => every node is an interface node, 3 local nodes per element
+    xy, tri = random_mesh(40, seed=1)
+    st, nn, en, nc, ns, ec, ml, _ = _plan(lib, xy, tri, chunk=8192, order=0)
+    assert st == 0 and (3 * ml + 7 * ec) * 8 + 64 <= 200 * 1024
+
+
+def test_bad_input_is_rejected_without_cuda(lib):
+    from paper_2606_23458_b200 import _lib
+    xy, tri = grid_mesh(4, 4, 1.0, 1.0)
+    mat = _lib.pff_material(**dict(GLASS, model=2, split=1, plane=0))
+    h = C.c_void_p()
+
+    def create(xy_, tri_, mat_, opt_=None):
+        xy_ = np.ascontiguousarray(xy_, dtype=np.float64)
+        tri_ = np.ascontiguousarray(tri_, dtype=np.int32)
+        return lib.pff_mesh_create(len(xy_), xy_.ctypes.data, len(tri_), tri_.ctypes.data, C.byref(mat_),
+                                   C.byref(opt_) if opt_ else None, None, C.byref(h))
+
+    bad = tri.copy(); bad[3, 1] = 99
+    assert create(xy, bad, mat) == _lib.PFF_EMESH and b"out of range" in lib.pff_last_error()
+    deg = tri.copy(); deg[0] = [0, 1, 1]
+    assert create(xy, deg, mat) == _lib.PFF_EMESH and b"area" in lib.pff_last_error()
+    assert create(np.vstack([xy, [[5.0, 5.0]]]), tri, mat) == _lib.PFF_EMESH and b"orphan" in lib.pff_last_error()
+    for field, val in (("nu", 0.5), ("E", -1.0), ("rho", 0.0), ("l0", 0.0), ("Gc", float("nan")), ("model", 3),
+                       ("split", 7), ("plane", 2)):
+        m2 = _lib.pff_material(**dict(GLASS, model=2, split=1, plane=0))
+        setattr(m2, field, val)
+        assert create(xy, tri, m2) == _lib.PFF_EINVAL, field
+    assert create(xy, tri, mat, _lib.pff_options(5, 1, 0, 0)) == _lib.PFF_EINVAL
+    assert lib.pff_mesh_create(16, None, 18, None, C.byref(mat), None, None, C.byref(h)) == _lib.PFF_EINVAL
+    assert lib.pff_explicit_step(None, None, None, 1.0) == _lib.PFF_EINVAL
+    assert lib.pff_damage_solve(None, None, 1e-8, 10, None, None) == _lib.PFF_EINVAL
+    assert lib.pff_energies(None, None, None) == _lib.PFF_EINVAL
+
+
+def test_no_cpu_fallback():
+    """Without a CUDA device the product path must fail loudly, never compute on the CPU."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    import paper_2606_23458_b200 as pff
+    xy, tri = grid_mesh(4, 4, 1.0, 1.0)
+    with pytest.raises(RuntimeError):
+        pff.Mesh(xy, tri, dict(GLASS, model=2, split=1, plane=0))
