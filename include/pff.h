@@ -173,6 +173,16 @@ pff_status pff_damage_matvec(pff_mesh *mesh, const pff_state *state, const void 
 /* Right-hand side b and Jacobi diagonal D of the damage system (either may be NULL). */
 pff_status pff_damage_rhs_diag(pff_mesh *mesh, const pff_state *state, void *b, void *D);
 
+/* ---- instrumentation --------------------------------------------------------------------- */
+/* Number of CUDA kernels this mesh has launched since creation (host counter). */
+pff_status pff_mesh_counters(const pff_mesh *mesh, int64_t *kernel_launches);
+/* Launches ONE kernel of the hot path `reps` times back to back on the mesh stream between two CUDA
+ * events (after one untimed launch) and returns the mean milliseconds per launch.  which: 0 = fused
+ * chunk step kernel (PFF_SCATTER_ATOMIC: element kernel), 1 = interface-node step kernel (ATOMIC: node
+ * kernel), 2 = damage mat-vec chunk kernel, 3 = damage mat-vec interface kernel.  The step kernels
+ * advance the state with a negligible dt; the mat-vec reads state->d as the trial vector.  Synchronises. */
+pff_status pff_time_kernel(pff_mesh *mesh, pff_state *state, int32_t which, int32_t reps, float *ms_per_launch);
+
 /* ---- host-buffer convenience path (end-to-end timing, small problems) ------------------------
  * State in USER numbering, fp64, AoS on the HOST: u, v, a, fext [n_nodes][2]; d [n_nodes];
  * H [n_elems].  Uploads, converts to internal order / mesh precision on the device, runs n_steps of

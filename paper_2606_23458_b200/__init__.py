@@ -178,6 +178,16 @@ class Mesh:
         _check(self.L.pff_damage_rhs_diag(self.h, C.byref(state.c), b.data_ptr(), D.data_ptr()))
         return b, D
 
+    def pff_mesh_counters(self) -> int:
+        n = C.c_int64()
+        _check(self.L.pff_mesh_counters(self.h, C.byref(n)))
+        return n.value
+
+    def pff_time_kernel(self, state: State, which: int, reps: int) -> float:
+        ms = C.c_float()
+        _check(self.L.pff_time_kernel(self.h, C.byref(state.c), which, reps, C.byref(ms)))
+        return ms.value
+
     def pff_run_host(self, u, v, a, d, H, fext, dt, n_steps, damage_every=1, rel_tol=1e-8, max_iter=1000,
                      dir_u=None, dir_v=None, load_scale=1.0, allow_noconv=False):
         """Host-buffer path: numpy fp64 arrays in USER numbering, updated in place."""
@@ -186,7 +196,9 @@ class Mesh:
             assert x.dtype == np.float64 and x.flags.c_contiguous
         dp = C.POINTER(C.c_double)
         hs = _lib.pff_host_state(*[x.ctypes.data_as(dp) for x in arrs])
-        du = np.ascontiguousarray(dir_u, dtype=np.float64).ctypes.data if dir_u is not None else None
-        dv = np.ascontiguousarray(dir_v, dtype=np.float64).ctypes.data if dir_v is not None else None
+        ku = np.ascontiguousarray(dir_u, dtype=np.float64) if dir_u is not None else None
+        kv = np.ascontiguousarray(dir_v, dtype=np.float64) if dir_v is not None else None
+        du = ku.ctypes.data if ku is not None else None
+        dv = kv.ctypes.data if kv is not None else None
         return _check(self.L.pff_run_host(self.h, C.byref(hs), du, dv, load_scale, dt, n_steps, damage_every,
                                           rel_tol, max_iter), allow=(PFF_ENOCONV,) if allow_noconv else ())

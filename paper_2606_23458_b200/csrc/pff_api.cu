@@ -329,6 +329,46 @@ pff_status pff_damage_rhs_diag(pff_mesh* m, const pff_state* s, void* b, void* D
     return damage_rhs_diag(m, s, b, D);
 }
 
+pff_status pff_mesh_counters(const pff_mesh* m, int64_t* kernel_launches)
+{
+    if (!m || !kernel_launches) { set_error("pff_mesh_counters: null argument"); return PFF_EINVAL; }
+    *kernel_launches = m->n_launches;
+    return PFF_OK;
+}
+
+pff_status pff_time_kernel(pff_mesh* m, pff_state* s, int32_t which, int32_t reps, float* ms_per_launch)
+{
+    if (!m || !valid_state(s) || !ms_per_launch || reps < 1 || which < 0 || which > 3) {
+        set_error("pff_time_kernel: bad argument"); return PFF_EINVAL;
+    }
+    if (m->opt.scatter != PFF_SCATTER_GATHER && which >= 2) { set_error("pff_time_kernel: gather meshes only"); return PFF_EUNSUPPORTED; }
+    cudaEvent_t e0, e1;
+    PFF_CUDA(cudaEventCreate(&e0));
+    PFF_CUDA(cudaEventCreate(&e1));
+    pff_bc bc{nullptr, nullptr, 1.0};
+    pff_status st = PFF_OK;
+    m->only_kernel = which;
+    // one untimed launch (attribute setup, instruction cache), then the timed train
+    for (int pass = 0; pass < 2 && st == PFF_OK; ++pass) {
+        const int n = pass == 0 ? 1 : reps;
+        if (pass == 1) cudaEventRecord(e0, m->stream);
+        for (int k = 0; k < n && st == PFF_OK; ++k) {
+            if (which < 2) st = launch_step(m, s, &bc, 1e-12 * m->dt_crit, 0, nullptr, nullptr, nullptr);
+            else st = damage_matvec(m, s, s->d, m->d_q);
+        }
+    }
+    cudaEventRecord(e1, m->stream);
+    m->only_kernel = -1;
+    cudaError_t e = cudaEventSynchronize(e1);
+    float ms = 0.f;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    if (st != PFF_OK) return st;
+    PFF_CUDA(e);
+    *ms_per_launch = ms / float(reps);
+    return PFF_OK;
+}
+
 pff_status pff_energies(pff_mesh* m, const pff_state* s, double out[4])
 {
     if (!m || !valid_state(s) || !out) { set_error("pff_energies: null argument"); return PFF_EINVAL; }

@@ -428,10 +428,15 @@ static pff_status ensure_workspace(pff_mesh* m)
     return PFF_OK;
 }
 
+// Opt a kernel instantiation in to `bytes` of dynamic shared memory (kept as a per-instantiation high-water
+// mark: the limit is 227 KB minus the kernel's static shared memory, so only what is needed is requested).
 template <typename K>
-static pff_status set_smem(K kern)
+static pff_status set_smem(K kern, int bytes, int& granted)
 {
-    return cuda_check(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024), "cudaFuncSetAttribute");
+    if (bytes <= granted) return PFF_OK;
+    pff_status st = cuda_check(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes), "cudaFuncSetAttribute(damage kernel)");
+    if (st == PFF_OK) granted = bytes;
+    return st;
 }
 
 template <typename R, bool PROJ>
@@ -442,22 +447,20 @@ static pff_status damage_solve_t(pff_mesh* m, pff_state* s, double rel_tol, int 
     const HostMesh& hm = m->hm;
     DmgArgs<R> a = make_args<R>(m, s);
     cudaStream_t cs = m->stream;
-    static bool attr = false;
-    if (!attr) {
-        if ((st = set_smem(dmg_matvec_chunk<R, DM_CG, PROJ>)) != PFF_OK) return st;
-        if ((st = set_smem(dmg_setup_chunk<R, false>)) != PFF_OK) return st;
-        attr = true;
-    }
+    const int smem_mv = int((size_t(hm.max_nloc) + size_t(3) * hm.chunk_elems) * sizeof(R));
+    const int smem_su = int((size_t(hm.max_nloc) + size_t(7) * hm.chunk_elems) * sizeof(R));
+    static int g_mv = 48 * 1024, g_su = 48 * 1024;
+    if ((st = set_smem(dmg_matvec_chunk<R, DM_CG, PROJ>, smem_mv, g_mv)) != PFF_OK) return st;
+    if ((st = set_smem(dmg_setup_chunk<R, false>, smem_su, g_su)) != PFF_OK) return st;
     DamageCtrl* h = m->h_ctrl;  // [0]: upload image, [1]: download image
     std::memset(&h[0], 0, sizeof(DamageCtrl));
     h[0].tol = rel_tol; h[0].max_iter = max_iter; h[0].first = 1; h[0].status = PFF_ENOCONV;
     if ((st = cuda_check(cudaMemcpyAsync(m->d_ctrl, &h[0], sizeof(DamageCtrl), cudaMemcpyHostToDevice, cs), "damage: ctrl upload")) != PFF_OK) return st;
     const unsigned nbv = (unsigned)((hm.N + kTPB - 1) / kTPB);
-    const int smem_mv = int((size_t(hm.max_nloc) + size_t(3) * hm.chunk_elems) * sizeof(R));
-    const int smem_su = int((size_t(hm.max_nloc) + size_t(7) * hm.chunk_elems) * sizeof(R));
     dmg_setup_chunk<R, false><<<(unsigned)hm.C, kTPB, smem_su, cs>>>(a);
     dmg_setup_shared<R, false><<<(unsigned)a.nbs, kTPB, 0, cs>>>(a);
     dmg_vector<R, PROJ><<<nbv, kTPB, 0, cs>>>(a);
+    m->n_launches += 3;
     int launched = 0, batch = 2;
     for (;;) {
         for (int k = 0; k < batch; ++k) {
@@ -466,12 +469,14 @@ static pff_status damage_solve_t(pff_mesh* m, pff_state* s, double rel_tol, int 
             dmg_vector<R, PROJ><<<nbv, kTPB, 0, cs>>>(a);
         }
         launched += batch;
+        m->n_launches += 3 * batch;
         if ((st = cuda_check(cudaMemcpyAsync(&h[1], m->d_ctrl, sizeof(DamageCtrl), cudaMemcpyDeviceToHost, cs), "damage: ctrl download")) != PFF_OK) return st;
         if ((st = cuda_check(cudaStreamSynchronize(cs), "damage: sync")) != PFF_OK) return st;
         if (h[1].done || launched >= max_iter + 1) break;
         batch = std::min(8, batch * 2);
     }
     dmg_finalize<R><<<nbv, kTPB, 0, cs>>>((int)hm.N, a.x, a.lb, a.flags);
+    ++m->n_launches;
     if ((st = cuda_check(cudaGetLastError(), "damage solve launch")) != PFF_OK) return st;
     if ((st = cuda_check(cudaStreamSynchronize(cs), "damage: final sync")) != PFF_OK) return st;
     if (iters) *iters = h[1].iters;
@@ -500,11 +505,17 @@ static pff_status damage_matvec_t(pff_mesh* m, const pff_state* s, const void* p
     if (st != PFF_OK) return st;
     DmgArgs<R> a = make_args<R>(m, s);
     a.p_in = (const R*)p; a.q_out = (R*)q;
-    static bool attr = false;
-    if (!attr) { if ((st = set_smem(dmg_matvec_chunk<R, DM_PLAIN, false>)) != PFF_OK) return st; attr = true; }
     const int smem_mv = int((size_t(m->hm.max_nloc) + size_t(3) * m->hm.chunk_elems) * sizeof(R));
-    dmg_matvec_chunk<R, DM_PLAIN, false><<<(unsigned)m->hm.C, kTPB, smem_mv, m->stream>>>(a);
-    dmg_matvec_shared<R, DM_PLAIN, false><<<(unsigned)a.nbs, kTPB, 0, m->stream>>>(a);
+    static int g_mv = 48 * 1024;
+    if ((st = set_smem(dmg_matvec_chunk<R, DM_PLAIN, false>, smem_mv, g_mv)) != PFF_OK) return st;
+    if (m->only_kernel != 3) {
+        dmg_matvec_chunk<R, DM_PLAIN, false><<<(unsigned)m->hm.C, kTPB, smem_mv, m->stream>>>(a);
+        ++m->n_launches;
+    }
+    if (m->only_kernel != 2) {
+        dmg_matvec_shared<R, DM_PLAIN, false><<<(unsigned)a.nbs, kTPB, 0, m->stream>>>(a);
+        ++m->n_launches;
+    }
     return cuda_check(cudaGetLastError(), "damage matvec launch");
 }
 
@@ -520,11 +531,12 @@ static pff_status damage_rhs_diag_t(pff_mesh* m, const pff_state* s, void* b, vo
     if (st != PFF_OK) return st;
     DmgArgs<R> a = make_args<R>(m, s);
     a.b_out = (R*)b; a.D_out = (R*)D;
-    static bool attr = false;
-    if (!attr) { if ((st = set_smem(dmg_setup_chunk<R, true>)) != PFF_OK) return st; attr = true; }
     const int smem_su = int((size_t(m->hm.max_nloc) + size_t(7) * m->hm.chunk_elems) * sizeof(R));
+    static int g_su = 48 * 1024;
+    if ((st = set_smem(dmg_setup_chunk<R, true>, smem_su, g_su)) != PFF_OK) return st;
     dmg_setup_chunk<R, true><<<(unsigned)m->hm.C, kTPB, smem_su, m->stream>>>(a);
     dmg_setup_shared<R, true><<<(unsigned)a.nbs, kTPB, 0, m->stream>>>(a);
+    m->n_launches += 2;
     return cuda_check(cudaGetLastError(), "damage rhs/diag launch");
 }
 

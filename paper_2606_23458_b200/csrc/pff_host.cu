@@ -73,6 +73,7 @@ static pff_status run_host_t(pff_mesh* m, pff_host_state* hs, const double* dir_
     CP(io.d, hs->d, N, cudaMemcpyHostToDevice); CP(io.H, hs->H, Ne, cudaMemcpyHostToDevice);
     const unsigned nb = (unsigned)((std::max(N, Ne) + 255) / 256);
     host_in_kernel<R><<<nb, 256, 0, cs>>>(io);
+    m->n_launches += 2;  // host_in + host_out
     pff_bc bc{nullptr, nullptr, S};
     std::vector<R> hu, hv;
     if (m->n_dir > 0 && dir_u && dir_v) {

@@ -18,6 +18,8 @@ struct pff_mesh {
     size_t rb = 8;  // bytes per real
     double dt_crit = 0.0;
     int smem_step = 0, smem_dmg = 0;
+    int64_t n_launches = 0;  // kernels launched so far (pff_mesh_counters)
+    int only_kernel = -1;    // profiling hook: restrict multi-kernel entry points to one kernel (pff_time_kernel)
 
     // device mesh tables
     pff::ChunkMeta* d_meta = nullptr;

@@ -231,19 +231,30 @@ static pff_status launch_step_t(pff_mesh* m, const StepArgs<R>& a)
 {
     const HostMesh& hm = m->hm;
     if (m->opt.scatter == PFF_SCATTER_ATOMIC) {
-        elem_atomic_kernel<R, SPLIT, MODE><<<(unsigned)((hm.Ne + kTPB - 1) / kTPB), kTPB, 0, m->stream>>>(a);
-        node_atomic_kernel<R, MODE><<<(unsigned)((hm.N + kTPB - 1) / kTPB), kTPB, 0, m->stream>>>(a);
+        if (m->only_kernel != 1) {
+            elem_atomic_kernel<R, SPLIT, MODE><<<(unsigned)((hm.Ne + kTPB - 1) / kTPB), kTPB, 0, m->stream>>>(a);
+            ++m->n_launches;
+        }
+        if (m->only_kernel != 0) {
+            node_atomic_kernel<R, MODE><<<(unsigned)((hm.N + kTPB - 1) / kTPB), kTPB, 0, m->stream>>>(a);
+            ++m->n_launches;
+        }
     } else {
         auto kern = step_chunk_kernel<R, SPLIT, MODE>;
-        static bool attr_set = false;  // per instantiation
-        if (!attr_set) {
-            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        static int granted = 48 * 1024;  // per instantiation high-water mark of the dynamic smem opt-in
+        if (m->smem_step > granted) {
+            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, m->smem_step);
             if (e != cudaSuccess) return cuda_check(e, "cudaFuncSetAttribute(step_chunk_kernel)");
-            attr_set = true;
+            granted = m->smem_step;
         }
-        kern<<<(unsigned)hm.C, kTPB, m->smem_step, m->stream>>>(a);
-        if (hm.N_sh > 0)
+        if (m->only_kernel != 1) {
+            kern<<<(unsigned)hm.C, kTPB, m->smem_step, m->stream>>>(a);
+            ++m->n_launches;
+        }
+        if (hm.N_sh > 0 && m->only_kernel != 0) {
             step_shared_kernel<R, MODE><<<(unsigned)((hm.N_sh + kTPB - 1) / kTPB), kTPB, 0, m->stream>>>(a);
+            ++m->n_launches;
+        }
     }
     return cuda_check(cudaGetLastError(), "explicit step launch");
 }
@@ -283,6 +294,7 @@ static pff_status launch_step_r(pff_mesh* m, pff_state* s, const pff_bc* bc, dou
     if (mode == MODE_STEP && m->n_dir > 0 && bc && bc->dir_u && bc->dir_v) {
         dirichlet_kernel<R><<<(unsigned)((m->n_dir + 127) / 128), 128, 0, m->stream>>>(
             (int)m->n_dir, m->d_dir_dof, (const R*)bc->dir_u, (const R*)bc->dir_v, a.ux, a.uy, a.vx, a.vy);
+        ++m->n_launches;
     }
     switch (mode) {
         case MODE_STEP: return launch_step_s<R, MODE_STEP>(m, a);
