@@ -147,9 +147,9 @@ def test_trajectory_energies_config1(model, split, plane):
     mesh.pff_init_accel(st, mesh.bc(load_scale=S))
     for k in range(200):
         orc.explicit_step(dt, S=S)
-        rc, _, _ = orc.damage_solve(rel_tol=1e-10)
+        rc, _, _ = orc.damage_solve(rel_tol=1e-12, max_iter=4000)
         mesh.pff_explicit_step(st, mesh.bc(load_scale=S), dt)
-        stt, _, _ = mesh.pff_damage_solve(st, rel_tol=1e-10)
+        stt, _, _ = mesh.pff_damage_solve(st, rel_tol=1e-12, max_iter=4000)
         assert rc == 0 and stt == 0
     e_ref, e = orc.energies(), mesh.pff_energies(st)
     assert np.all(np.abs(e - e_ref) <= 1e-6 * np.abs(e_ref).max())
