@@ -183,6 +183,24 @@ pff_status pff_mesh_counters(const pff_mesh *mesh, int64_t *kernel_launches);
  * advance the state with a negligible dt; the mat-vec reads state->d as the trial vector.  Synchronises. */
 pff_status pff_time_kernel(pff_mesh *mesh, pff_state *state, int32_t which, int32_t reps, float *ms_per_launch);
 
+/* Kernel classes of the hot path, for per-kernel timing inside a real run (bench.py's roofline block). */
+typedef enum {
+    PFF_K_STEP_CHUNK = 0,      /* fused element force + history + node update, one CTA per chunk (ATOMIC: element kernel) */
+    PFF_K_STEP_SHARED = 1,     /* interface-node update (ATOMIC: node kernel)                                            */
+    PFF_K_MATVEC_CHUNK = 2,    /* damage operator apply + direction update + p.q partials                                */
+    PFF_K_MATVEC_SHARED = 3,   /* interface nodes of the operator apply + alpha                                          */
+    PFF_K_CG_VECTOR = 4,       /* x, r update, free set, r.z / ||r|| partials, beta                                      */
+    PFF_K_DAMAGE_SETUP = 5,    /* rhs, Jacobi diagonal, r0 (chunk + interface kernels), finalize clamp                    */
+    PFF_K_OTHER = 6,           /* Dirichlet overwrite, energies, host-path permutation kernels                            */
+    PFF_NUM_KERNEL_CLASSES = 7
+} pff_kernel_class;
+/* enable != 0: every following kernel launch of this mesh is bracketed by two CUDA events on the mesh
+ * stream (adds ~2 event records per launch; use for attribution, not for headline throughput).
+ * pff_profile_read synchronises the stream, returns per class the summed device milliseconds and the number
+ * of launches since the last read (host arrays of PFF_NUM_KERNEL_CLASSES entries) and resets the tallies. */
+pff_status pff_profile_enable(pff_mesh *mesh, int32_t enable);
+pff_status pff_profile_read(pff_mesh *mesh, double *ms_sum, int64_t *launches);
+
 /* ---- host-buffer convenience path (end-to-end timing, small problems) ------------------------
  * State in USER numbering, fp64, AoS on the HOST: u, v, a, fext [n_nodes][2]; d [n_nodes];
  * H [n_elems].  Uploads, converts to internal order / mesh precision on the device, runs n_steps of

@@ -188,6 +188,16 @@ class Mesh:
         _check(self.L.pff_time_kernel(self.h, C.byref(state.c), which, reps, C.byref(ms)))
         return ms.value
 
+    def pff_profile_enable(self, enable: bool):
+        _check(self.L.pff_profile_enable(self.h, int(enable)))
+
+    def pff_profile_read(self):
+        """{kernel class: (summed device ms, launches)} since the last read."""
+        n = len(_lib.KERNEL_CLASSES)
+        ms, cnt = (C.c_double * n)(), (C.c_int64 * n)()
+        _check(self.L.pff_profile_read(self.h, ms, cnt))
+        return {k: (ms[i], cnt[i]) for i, k in enumerate(_lib.KERNEL_CLASSES)}
+
     def pff_run_host(self, u, v, a, d, H, fext, dt, n_steps, damage_every=1, rel_tol=1e-8, max_iter=1000,
                      dir_u=None, dir_v=None, load_scale=1.0, allow_noconv=False):
         """Host-buffer path: numpy fp64 arrays in USER numbering, updated in place."""

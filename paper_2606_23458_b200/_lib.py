@@ -14,12 +14,14 @@ PFF_PLANE_STRAIN, PFF_PLANE_STRESS = 0, 1
 PFF_F64, PFF_F32 = 0, 1
 PFF_SCATTER_GATHER, PFF_SCATTER_ATOMIC = 0, 1
 PFF_ORDER_NONE, PFF_ORDER_MORTON = 0, 1
+KERNEL_CLASSES = ("step_chunk", "step_shared", "matvec_chunk", "matvec_shared", "cg_vector", "damage_setup", "other")
 
 # every symbol include/pff.h declares
 SYMBOLS = [
     "pff_mesh_create", "pff_mesh_plan", "pff_mesh_destroy", "pff_mesh_info", "pff_mesh_permutations", "pff_set_dirichlet",
     "pff_set_damage_dirichlet", "pff_set_traction", "pff_init_accel", "pff_explicit_step", "pff_damage_solve",
     "pff_energies", "pff_internal_force", "pff_damage_matvec", "pff_damage_rhs_diag", "pff_run_host", "pff_mesh_counters", "pff_time_kernel",
+    "pff_profile_enable", "pff_profile_read",
     "pff_last_error",
 ]
 
@@ -79,6 +81,8 @@ def load() -> C.CDLL:
     L.pff_run_host.argtypes = [vp, C.POINTER(pff_host_state), vp, vp, C.c_double, C.c_double, i64, i32, C.c_double, i32]
     L.pff_mesh_counters.argtypes = [vp, C.POINTER(i64)]
     L.pff_time_kernel.argtypes = [vp, C.POINTER(pff_state), i32, i32, C.POINTER(C.c_float)]
+    L.pff_profile_enable.argtypes = [vp, i32]
+    L.pff_profile_read.argtypes = [vp, dp, C.POINTER(i64)]
     L.pff_last_error.restype = C.c_char_p
     for name in SYMBOLS:
         if name not in ("pff_mesh_destroy", "pff_last_error"):

@@ -71,6 +71,7 @@ void pff_mesh_destroy(pff_mesh* m)
                     m->d_elem_old_of_new};
     for (void* p : ptrs) if (p) cudaFree(p);
     if (m->h_ctrl) cudaFreeHost(m->h_ctrl);
+    for (auto& v : m->prof_ev) for (cudaEvent_t e : v) cudaEventDestroy(e);
     delete m;
 }
 
@@ -333,6 +334,33 @@ pff_status pff_mesh_counters(const pff_mesh* m, int64_t* kernel_launches)
 {
     if (!m || !kernel_launches) { set_error("pff_mesh_counters: null argument"); return PFF_EINVAL; }
     *kernel_launches = m->n_launches;
+    return PFF_OK;
+}
+
+pff_status pff_profile_enable(pff_mesh* m, int32_t enable)
+{
+    if (!m) { set_error("pff_profile_enable: null mesh"); return PFF_EINVAL; }
+    PFF_CUDA(cudaStreamSynchronize(m->stream));
+    m->prof_on = enable != 0;
+    for (auto& u : m->prof_used) u = 0;
+    return PFF_OK;
+}
+
+pff_status pff_profile_read(pff_mesh* m, double* ms_sum, int64_t* launches)
+{
+    if (!m || !ms_sum || !launches) { set_error("pff_profile_read: null argument"); return PFF_EINVAL; }
+    PFF_CUDA(cudaStreamSynchronize(m->stream));
+    for (int c = 0; c < PFF_NUM_KERNEL_CLASSES; ++c) {
+        double sum = 0.0;
+        for (size_t k = 0; k + 1 < m->prof_used[c]; k += 2) {
+            float ms = 0.f;
+            PFF_CUDA(cudaEventElapsedTime(&ms, m->prof_ev[c][k], m->prof_ev[c][k + 1]));
+            sum += ms;
+        }
+        ms_sum[c] = sum;
+        launches[c] = (int64_t)(m->prof_used[c] / 2);
+        m->prof_used[c] = 0;
+    }
     return PFF_OK;
 }
 

@@ -457,26 +457,23 @@ static pff_status damage_solve_t(pff_mesh* m, pff_state* s, double rel_tol, int 
     h[0].tol = rel_tol; h[0].max_iter = max_iter; h[0].first = 1; h[0].status = PFF_ENOCONV;
     if ((st = cuda_check(cudaMemcpyAsync(m->d_ctrl, &h[0], sizeof(DamageCtrl), cudaMemcpyHostToDevice, cs), "damage: ctrl upload")) != PFF_OK) return st;
     const unsigned nbv = (unsigned)((hm.N + kTPB - 1) / kTPB);
-    dmg_setup_chunk<R, false><<<(unsigned)hm.C, kTPB, smem_su, cs>>>(a);
-    dmg_setup_shared<R, false><<<(unsigned)a.nbs, kTPB, 0, cs>>>(a);
-    dmg_vector<R, PROJ><<<nbv, kTPB, 0, cs>>>(a);
-    m->n_launches += 3;
+    PFF_LAUNCH(m, PFF_K_DAMAGE_SETUP, (dmg_setup_chunk<R, false><<<(unsigned)hm.C, kTPB, smem_su, cs>>>(a)));
+    PFF_LAUNCH(m, PFF_K_DAMAGE_SETUP, (dmg_setup_shared<R, false><<<(unsigned)a.nbs, kTPB, 0, cs>>>(a)));
+    PFF_LAUNCH(m, PFF_K_CG_VECTOR, (dmg_vector<R, PROJ><<<nbv, kTPB, 0, cs>>>(a)));
     int launched = 0, batch = 2;
     for (;;) {
         for (int k = 0; k < batch; ++k) {
-            dmg_matvec_chunk<R, DM_CG, PROJ><<<(unsigned)hm.C, kTPB, smem_mv, cs>>>(a);
-            dmg_matvec_shared<R, DM_CG, PROJ><<<(unsigned)a.nbs, kTPB, 0, cs>>>(a);
-            dmg_vector<R, PROJ><<<nbv, kTPB, 0, cs>>>(a);
+            PFF_LAUNCH(m, PFF_K_MATVEC_CHUNK, (dmg_matvec_chunk<R, DM_CG, PROJ><<<(unsigned)hm.C, kTPB, smem_mv, cs>>>(a)));
+            PFF_LAUNCH(m, PFF_K_MATVEC_SHARED, (dmg_matvec_shared<R, DM_CG, PROJ><<<(unsigned)a.nbs, kTPB, 0, cs>>>(a)));
+            PFF_LAUNCH(m, PFF_K_CG_VECTOR, (dmg_vector<R, PROJ><<<nbv, kTPB, 0, cs>>>(a)));
         }
         launched += batch;
-        m->n_launches += 3 * batch;
         if ((st = cuda_check(cudaMemcpyAsync(&h[1], m->d_ctrl, sizeof(DamageCtrl), cudaMemcpyDeviceToHost, cs), "damage: ctrl download")) != PFF_OK) return st;
         if ((st = cuda_check(cudaStreamSynchronize(cs), "damage: sync")) != PFF_OK) return st;
         if (h[1].done || launched >= max_iter + 1) break;
         batch = std::min(8, batch * 2);
     }
-    dmg_finalize<R><<<nbv, kTPB, 0, cs>>>((int)hm.N, a.x, a.lb, a.flags);
-    ++m->n_launches;
+    PFF_LAUNCH(m, PFF_K_DAMAGE_SETUP, (dmg_finalize<R><<<nbv, kTPB, 0, cs>>>((int)hm.N, a.x, a.lb, a.flags)));
     if ((st = cuda_check(cudaGetLastError(), "damage solve launch")) != PFF_OK) return st;
     if ((st = cuda_check(cudaStreamSynchronize(cs), "damage: final sync")) != PFF_OK) return st;
     if (iters) *iters = h[1].iters;
@@ -509,12 +506,10 @@ static pff_status damage_matvec_t(pff_mesh* m, const pff_state* s, const void* p
     static int g_mv = 48 * 1024;
     if ((st = set_smem(dmg_matvec_chunk<R, DM_PLAIN, false>, smem_mv, g_mv)) != PFF_OK) return st;
     if (m->only_kernel != 3) {
-        dmg_matvec_chunk<R, DM_PLAIN, false><<<(unsigned)m->hm.C, kTPB, smem_mv, m->stream>>>(a);
-        ++m->n_launches;
+        PFF_LAUNCH(m, PFF_K_MATVEC_CHUNK, (dmg_matvec_chunk<R, DM_PLAIN, false><<<(unsigned)m->hm.C, kTPB, smem_mv, m->stream>>>(a)));
     }
     if (m->only_kernel != 2) {
-        dmg_matvec_shared<R, DM_PLAIN, false><<<(unsigned)a.nbs, kTPB, 0, m->stream>>>(a);
-        ++m->n_launches;
+        PFF_LAUNCH(m, PFF_K_MATVEC_SHARED, (dmg_matvec_shared<R, DM_PLAIN, false><<<(unsigned)a.nbs, kTPB, 0, m->stream>>>(a)));
     }
     return cuda_check(cudaGetLastError(), "damage matvec launch");
 }
@@ -534,9 +529,8 @@ static pff_status damage_rhs_diag_t(pff_mesh* m, const pff_state* s, void* b, vo
     const int smem_su = int((size_t(m->hm.max_nloc) + size_t(7) * m->hm.chunk_elems) * sizeof(R));
     static int g_su = 48 * 1024;
     if ((st = set_smem(dmg_setup_chunk<R, true>, smem_su, g_su)) != PFF_OK) return st;
-    dmg_setup_chunk<R, true><<<(unsigned)m->hm.C, kTPB, smem_su, m->stream>>>(a);
-    dmg_setup_shared<R, true><<<(unsigned)a.nbs, kTPB, 0, m->stream>>>(a);
-    m->n_launches += 2;
+    PFF_LAUNCH(m, PFF_K_DAMAGE_SETUP, (dmg_setup_chunk<R, true><<<(unsigned)m->hm.C, kTPB, smem_su, m->stream>>>(a)));
+    PFF_LAUNCH(m, PFF_K_DAMAGE_SETUP, (dmg_setup_shared<R, true><<<(unsigned)a.nbs, kTPB, 0, m->stream>>>(a)));
     return cuda_check(cudaGetLastError(), "damage rhs/diag launch");
 }
 

@@ -20,6 +20,10 @@ struct pff_mesh {
     int smem_step = 0, smem_dmg = 0;
     int64_t n_launches = 0;  // kernels launched so far (pff_mesh_counters)
     int only_kernel = -1;    // profiling hook: restrict multi-kernel entry points to one kernel (pff_time_kernel)
+    // per-kernel-class CUDA-event timing (pff_profile_enable / pff_profile_read)
+    bool prof_on = false;
+    std::vector<cudaEvent_t> prof_ev[PFF_NUM_KERNEL_CLASSES];  // start/stop pairs
+    size_t prof_used[PFF_NUM_KERNEL_CLASSES] = {};
 
     // device mesh tables
     pff::ChunkMeta* d_meta = nullptr;
@@ -54,6 +58,21 @@ struct pff_mesh {
 };
 
 namespace pff {
+// Event bracket around one launch of kernel class `cls` (no-ops unless profiling is enabled).
+inline void prof_mark(pff_mesh* m, int cls)
+{
+    if (!m->prof_on) return;
+    auto& v = m->prof_ev[cls];
+    if (m->prof_used[cls] == v.size()) { cudaEvent_t e; cudaEventCreate(&e); v.push_back(e); }
+    cudaEventRecord(v[m->prof_used[cls]++], m->stream);
+}
+#define PFF_LAUNCH(m, cls, ...)            \
+    do {                                   \
+        pff::prof_mark((m), (cls));        \
+        __VA_ARGS__;                       \
+        pff::prof_mark((m), (cls));        \
+        ++(m)->n_launches;                 \
+    } while (0)
 // implemented in pff_step.cu / pff_damage.cu / pff_energy.cu
 pff_status launch_step(pff_mesh* m, pff_state* s, const pff_bc* bc, double dt, int mode, void* fx, void* fy, void* psi);
 pff_status damage_solve(pff_mesh* m, pff_state* s, double rel_tol, int max_iter, int* iters, double* relres);

@@ -232,12 +232,10 @@ static pff_status launch_step_t(pff_mesh* m, const StepArgs<R>& a)
     const HostMesh& hm = m->hm;
     if (m->opt.scatter == PFF_SCATTER_ATOMIC) {
         if (m->only_kernel != 1) {
-            elem_atomic_kernel<R, SPLIT, MODE><<<(unsigned)((hm.Ne + kTPB - 1) / kTPB), kTPB, 0, m->stream>>>(a);
-            ++m->n_launches;
+            PFF_LAUNCH(m, PFF_K_STEP_CHUNK, (elem_atomic_kernel<R, SPLIT, MODE><<<(unsigned)((hm.Ne + kTPB - 1) / kTPB), kTPB, 0, m->stream>>>(a)));
         }
         if (m->only_kernel != 0) {
-            node_atomic_kernel<R, MODE><<<(unsigned)((hm.N + kTPB - 1) / kTPB), kTPB, 0, m->stream>>>(a);
-            ++m->n_launches;
+            PFF_LAUNCH(m, PFF_K_STEP_SHARED, (node_atomic_kernel<R, MODE><<<(unsigned)((hm.N + kTPB - 1) / kTPB), kTPB, 0, m->stream>>>(a)));
         }
     } else {
         auto kern = step_chunk_kernel<R, SPLIT, MODE>;
@@ -248,12 +246,10 @@ static pff_status launch_step_t(pff_mesh* m, const StepArgs<R>& a)
             granted = m->smem_step;
         }
         if (m->only_kernel != 1) {
-            kern<<<(unsigned)hm.C, kTPB, m->smem_step, m->stream>>>(a);
-            ++m->n_launches;
+            PFF_LAUNCH(m, PFF_K_STEP_CHUNK, (kern<<<(unsigned)hm.C, kTPB, m->smem_step, m->stream>>>(a)));
         }
         if (hm.N_sh > 0 && m->only_kernel != 0) {
-            step_shared_kernel<R, MODE><<<(unsigned)((hm.N_sh + kTPB - 1) / kTPB), kTPB, 0, m->stream>>>(a);
-            ++m->n_launches;
+            PFF_LAUNCH(m, PFF_K_STEP_SHARED, (step_shared_kernel<R, MODE><<<(unsigned)((hm.N_sh + kTPB - 1) / kTPB), kTPB, 0, m->stream>>>(a)));
         }
     }
     return cuda_check(cudaGetLastError(), "explicit step launch");
@@ -292,9 +288,8 @@ static pff_status launch_step_r(pff_mesh* m, pff_state* s, const pff_bc* bc, dou
     a.S = R(bc ? bc->load_scale : 1.0);
     a.mat = make_matc<R>(m->mat);
     if (mode == MODE_STEP && m->n_dir > 0 && bc && bc->dir_u && bc->dir_v) {
-        dirichlet_kernel<R><<<(unsigned)((m->n_dir + 127) / 128), 128, 0, m->stream>>>(
-            (int)m->n_dir, m->d_dir_dof, (const R*)bc->dir_u, (const R*)bc->dir_v, a.ux, a.uy, a.vx, a.vy);
-        ++m->n_launches;
+        PFF_LAUNCH(m, PFF_K_OTHER, (dirichlet_kernel<R><<<(unsigned)((m->n_dir + 127) / 128), 128, 0, m->stream>>>(
+            (int)m->n_dir, m->d_dir_dof, (const R*)bc->dir_u, (const R*)bc->dir_v, a.ux, a.uy, a.vx, a.vy)));
     }
     switch (mode) {
         case MODE_STEP: return launch_step_s<R, MODE_STEP>(m, a);
