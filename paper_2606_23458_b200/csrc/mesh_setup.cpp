@@ -22,8 +22,7 @@ static inline uint32_t spread16(uint32_t v)
 }
 
 pff_status build_host_mesh(int64_t N, const double* xy, int64_t Ne, const int32_t* tri_in, double rho,
-                           int order, int chunk_elems, size_t real_bytes, size_t smem_limit, HostMesh& hm,
-                           std::string& err)
+                           int order, int chunk_elems, size_t real_bytes, HostMesh& hm, std::string& err)
 {
     if (N < 3 || Ne < 1) { err = "mesh needs at least 3 nodes and 1 element"; return PFF_EINVAL; }
     if (N >= (int64_t(1) << 30) || Ne >= (int64_t(1) << 30)) { err = "mesh too large (>= 2^30)"; return PFF_EMESH; }
@@ -85,9 +84,13 @@ pff_status build_host_mesh(int64_t N, const double* xy, int64_t Ne, const int32_
     hm.elem_new_of_old.resize(Ne);
     for (int64_t e = 0; e < Ne; ++e) hm.elem_new_of_old[elem_old_of_new[e]] = int32_t(e);
 
-    // ---- chunks; shrink the chunk until the worst-case shared-memory footprint fits
-    int EC = chunk_elems > 0 ? chunk_elems : 1024;
+    // ---- chunks; shrink the chunk until the worst-case shared-memory footprint of every chunk kernel fits
+    // (default chunk: three resident CTAs per SM; explicit chunk: one CTA)
+    const int A = int(16 / real_bytes);  // reals per 16-byte TMA granule
+    const bool user_chunk = chunk_elems > 0;
+    int EC = user_chunk ? chunk_elems : (real_bytes == 8 ? 512 : 1024);
     EC = std::max(32, std::min(8192, (EC / 32) * 32));
+    const size_t smem_limit = (user_chunk ? kSmemPerSM : kSmemPerSM / 3) - kSmemCtaReserve - kSmemStatic;
     std::vector<int32_t> cmin(N), cmax(N);
     for (;;) {
         std::fill(cmin.begin(), cmin.end(), std::numeric_limits<int32_t>::max());
@@ -97,21 +100,29 @@ pff_status build_host_mesh(int64_t N, const double* xy, int64_t Ne, const int32_
             const int32_t* t = &tri[3 * elem_old_of_new[en]];
             for (int k = 0; k < 3; ++k) { cmin[t[k]] = std::min(cmin[t[k]], c); cmax[t[k]] = std::max(cmax[t[k]], c); }
         }
-        // per-chunk local node count (interior + interface) via first-touch stamps
+        // per-chunk local node count and valence (bounds for the staged array lengths) via first-touch stamps
         int64_t C = (Ne + EC - 1) / EC;
-        std::vector<int32_t> stamp(N, -1);
-        int32_t max_nloc = 0;
+        std::vector<int32_t> stamp(N, -1), valence(N, 0);
+        int32_t max_nloc = 0, max_ell = 0;
         for (int64_t c = 0; c < C; ++c) {
-            int32_t nloc = 0;
+            int32_t nloc = 0, w = 0;
             for (int64_t en = c * EC; en < std::min<int64_t>(Ne, (c + 1) * EC); ++en) {
                 const int32_t* t = &tri[3 * elem_old_of_new[en]];
-                for (int k = 0; k < 3; ++k) if (stamp[t[k]] != c) { stamp[t[k]] = int32_t(c); ++nloc; }
+                for (int k = 0; k < 3; ++k) {
+                    if (stamp[t[k]] != c) { stamp[t[k]] = int32_t(c); valence[t[k]] = 0; ++nloc; }
+                    w = std::max(w, ++valence[t[k]]);
+                }
             }
             max_nloc = std::max(max_nloc, nloc);
+            max_ell = std::max(max_ell, w * nloc);
         }
-        size_t smem = (size_t(3) * max_nloc + size_t(7) * EC) * real_bytes + 64;
-        if (smem <= smem_limit || EC <= 32) {
-            if (smem > smem_limit) { err = "chunk does not fit shared memory"; return PFF_EMESH; }
+        const int node_len_b = (max_nloc + 2 * A + A - 1) / A * A, flag_len_b = (max_nloc + 32 + 15) / 16 * 16;
+        const int ell_len_b = (max_ell + 7) / 8 * 8;
+        size_t smem = 0;
+        for (int kind = 0; kind < 3; ++kind)
+            smem = std::max(smem, chunk_smem_bytes(kind, EC, node_len_b, flag_len_b, ell_len_b, real_bytes));
+        if ((smem <= smem_limit && max_nloc < 16384) || EC <= 32) {
+            if (smem > kSmemPerSM - kSmemCtaReserve - kSmemStatic) { err = "chunk does not fit shared memory"; return PFF_EMESH; }
             hm.max_nloc = max_nloc; hm.C = C;
             break;
         }
@@ -156,6 +167,7 @@ pff_status build_host_mesh(int64_t N, const double* xy, int64_t Ne, const int32_
     hm.mass.assign(N, 0.0);
     std::vector<int32_t> sh_stamp(hm.N_sh, -1), sh_local(hm.N_sh, 0), sh_count(hm.N_sh + 1, 0);
     std::vector<int32_t> val;  // valence per local node
+    std::vector<int32_t> lloc(size_t(3) * EC);  // chunk-local node index of each element corner
     hm.halo_ids.clear();
     hm.ell.clear();
     for (int64_t c = 0; c < C; ++c) {
@@ -166,7 +178,7 @@ pff_status build_host_mesh(int64_t N, const double* xy, int64_t Ne, const int32_
             int64_t eo = elem_old_of_new[en];
             for (int k = 0; k < 3; ++k) {
                 int32_t g = hm.node_new_of_old[tri[3 * eo + k]];
-                int32_t l;
+                int32_t l;  // chunk-local node index: interior first, then halo in first-touch order
                 if (g < hm.N_int) l = g - m.node_start;
                 else {
                     int32_t s = g - int32_t(hm.N_int);
@@ -174,40 +186,53 @@ pff_status build_host_mesh(int64_t N, const double* xy, int64_t Ne, const int32_
                     l = m.n_int + sh_local[s];
                 }
                 hm.conn4[4 * en + k] = g;
-                hm.lconn4[4 * en + k] = uint16_t(l);
+                lloc[3 * (en - m.elem_start) + k] = l;
             }
             for (int k = 0; k < 4; ++k) hm.g12[4 * en + k] = g12u[4 * eo + k];
             hm.area[en] = areau[eo];
         }
         m.n_halo = nh;
         const int32_t nloc = m.n_int + nh;
+        // shared-memory slot of a local node: staged arrays hold [shift | interior | pad to 16 B | halo]
+        const int32_t shift = m.node_start % A, hb = (shift + m.n_int + A - 1) / A * A;
+        for (int64_t en = m.elem_start; en < m.elem_start + m.n_elem; ++en)
+            for (int k = 0; k < 3; ++k) {
+                const int32_t l = lloc[3 * (en - m.elem_start) + k];
+                hm.lconn4[4 * en + k] = uint16_t(l < m.n_int ? shift + l : hb + (l - m.n_int));
+            }
+        hm.node_len = std::max(hm.node_len, (hb + nh + A - 1) / A * A);
+        hm.flag_len = std::max(hm.flag_len, (m.node_start % 16 + m.n_int + 15) / 16 * 16);
+        hm.max_nhalo = std::max(hm.max_nhalo, nh);
         val.assign(nloc, 0);
         for (int64_t en = m.elem_start; en < m.elem_start + m.n_elem; ++en)
-            for (int k = 0; k < 3; ++k) ++val[hm.lconn4[4 * en + k]];
+            for (int k = 0; k < 3; ++k) ++val[lloc[3 * (en - m.elem_start) + k]];
         int32_t w = 0;
         for (int32_t i = 0; i < nloc; ++i) w = std::max(w, val[i]);
         m.ell_w = w;
+        hm.ell.resize((hm.ell.size() + 7) / 8 * 8, uint16_t(3 * EC));  // 16-byte aligned table start
         m.ell_off = int32_t(hm.ell.size());
+        hm.ell_len = std::max(hm.ell_len, (w * nloc + 7) / 8 * 8);
         if (hm.ell.size() + size_t(w) * nloc > size_t(std::numeric_limits<int32_t>::max())) {
             err = "gather table too large"; return PFF_EMESH;
         }
-        hm.ell.resize(hm.ell.size() + size_t(w) * nloc, uint16_t(0xFFFF));
+        hm.ell.resize(hm.ell.size() + size_t(w) * nloc, uint16_t(3 * EC));  // padding -> zero slot
         std::fill(val.begin(), val.end(), 0);
         for (int64_t en = m.elem_start; en < m.elem_start + m.n_elem; ++en)
             for (int k = 0; k < 3; ++k) {
-                int32_t l = hm.lconn4[4 * en + k];
-                hm.ell[size_t(m.ell_off) + size_t(val[l]++) * nloc + l] = uint16_t(((en - m.elem_start) << 2) | k);
+                int32_t l = lloc[3 * (en - m.elem_start) + k];
+                hm.ell[size_t(m.ell_off) + size_t(val[l]++) * nloc + l] = uint16_t(k * EC + (en - m.elem_start));
             }
         hm.max_ell_w = std::max(hm.max_ell_w, w);
     }
+    hm.ell.resize((hm.ell.size() + 7) / 8 * 8 + 8, uint16_t(3 * EC));  // the widened TMA copy stays in bounds
     // interface-node CSR over halo slots, ascending chunk (chunks were visited in order)
     hm.sh_rowptr.assign(hm.N_sh + 1, 0);
     for (int64_t s = 0; s < hm.N_sh; ++s) hm.sh_rowptr[s + 1] = hm.sh_rowptr[s] + sh_count[s + 1];
-    hm.sh_slots.resize(hm.halo_ids.size());
+    hm.halo_dst.resize(hm.halo_ids.size());
     std::vector<int32_t> fill(hm.sh_rowptr.begin(), hm.sh_rowptr.end() - 1);
     for (size_t slot = 0; slot < hm.halo_ids.size(); ++slot) {
         int32_t s = hm.halo_ids[slot] - int32_t(hm.N_int);
-        hm.sh_slots[fill[s]++] = int32_t(slot);
+        hm.halo_dst[slot] = fill[s]++;
     }
     // lumped mass m_i = rho sum A_e / 3 (L169), summed in internal element order
     for (int64_t en = 0; en < Ne; ++en)

@@ -47,9 +47,13 @@ static pff_status upload_real(void** dst, const double* src, size_t count, size_
     return s;
 }
 
+// all ten arrays present and 16-byte aligned (they are streamed with bulk-asynchronous copies)
 static bool valid_state(const pff_state* s)
 {
-    return s && s->ux && s->uy && s->vx && s->vy && s->ax && s->ay && s->d && s->H && s->fext_x && s->fext_y;
+    if (!(s && s->ux && s->uy && s->vx && s->vy && s->ax && s->ay && s->d && s->H && s->fext_x && s->fext_y)) return false;
+    const void* p[] = {s->ux, s->uy, s->vx, s->vy, s->ax, s->ay, s->d, s->H, s->fext_x, s->fext_y};
+    for (const void* q : p) if (reinterpret_cast<uintptr_t>(q) & 15) return false;
+    return true;
 }
 
 }  // namespace pff
@@ -65,9 +69,9 @@ void pff_mesh_destroy(pff_mesh* m)
     if (!m) return;
     cudaStreamSynchronize(m->stream);
     void* ptrs[] = {m->d_meta, m->d_lconn, m->d_conn, m->d_ga, m->d_gb, m->d_area, m->d_minv, m->d_mass,
-                    m->d_halo_ids, m->d_sh_rowptr, m->d_sh_slots, m->d_ell, m->d_flags, m->d_halo_part,
+                    m->d_halo_ids, m->d_sh_rowptr, m->d_halo_dst, m->d_ell, m->d_flags, m->d_halo_part,
                     m->d_fwx, m->d_fwy, m->d_dir_dof, m->d_lb, m->d_r, m->d_p, m->d_q, m->d_dinv, m->d_mask,
-                    m->d_part, m->d_ctrl, m->d_ticket, m->d_stage, m->d_hstate, m->d_node_old_of_new,
+                    m->d_part, m->d_part2, m->d_ctrl, m->d_ticket, m->d_stage, m->d_hstate, m->d_node_old_of_new,
                     m->d_elem_old_of_new};
     for (void* p : ptrs) if (p) cudaFree(p);
     if (m->h_ctrl) cudaFreeHost(m->h_ctrl);
@@ -104,7 +108,7 @@ pff_status pff_mesh_create(int64_t n_nodes, const double* xy, int64_t n_elems, c
     std::string err;
     pff_status st;
     try {
-        st = build_host_mesh(n_nodes, xy, n_elems, tri, mat->rho, opt.order, opt.chunk_elems, m->rb, 200 * 1024, m->hm, err);
+        st = build_host_mesh(n_nodes, xy, n_elems, tri, mat->rho, opt.order, opt.chunk_elems, m->rb, m->hm, err);
     } catch (const std::bad_alloc&) { st = PFF_ENOMEM; err = "out of host memory in mesh setup"; }
     if (st != PFF_OK) { set_error("pff_mesh_create: " + err); delete m; return st; }
     HostMesh& hm = m->hm;
@@ -115,8 +119,10 @@ pff_status pff_mesh_create(int64_t n_nodes, const double* xy, int64_t n_elems, c
                                                            : mat->E * mat->nu / ((1 + mat->nu) * (1 - 2 * mat->nu));
         m->dt_crit = hm.hmin / std::sqrt((lam + 2 * mu) / mat->rho);
     }
-    m->smem_step = int((size_t(3) * hm.max_nloc + size_t(6) * hm.chunk_elems) * m->rb);
-    m->smem_dmg = int((size_t(3) * hm.max_nloc + size_t(7) * hm.chunk_elems) * m->rb);
+    m->lay_step = make_stage_layout(0, hm.chunk_elems, hm.node_len, hm.flag_len, hm.ell_len, m->rb);
+    m->lay_mv = make_stage_layout(1, hm.chunk_elems, hm.node_len, hm.flag_len, hm.ell_len, m->rb);
+    m->lay_su = make_stage_layout(2, hm.chunk_elems, hm.node_len, hm.flag_len, hm.ell_len, m->rb);
+    m->ell_total = (int64_t)hm.ell.size();
 
     auto fail = [&](pff_status s) { pff_mesh_destroy(m); return s; };
     cudaStream_t cs = m->stream;
@@ -149,7 +155,7 @@ pff_status pff_mesh_create(int64_t n_nodes, const double* xy, int64_t n_elems, c
     m->n_slots = (int64_t)hm.halo_ids.size();
     UP(upload(&m->d_halo_ids, hm.halo_ids.data(), hm.halo_ids.size(), cs));
     UP(upload(&m->d_sh_rowptr, hm.sh_rowptr.data(), hm.sh_rowptr.size(), cs));
-    UP(upload(&m->d_sh_slots, hm.sh_slots.data(), hm.sh_slots.size(), cs));
+    UP(upload(&m->d_halo_dst, hm.halo_dst.data(), hm.halo_dst.size(), cs));
     UP(upload(&m->d_ell, hm.ell.data(), hm.ell.size(), cs));
     m->h_flags.assign(N, 0);
     UP(upload(&m->d_flags, m->h_flags.data(), N, cs));
@@ -190,7 +196,7 @@ pff_status pff_mesh_plan(int64_t n_nodes, const double* xy, int64_t n_elems, con
     pff_status st;
     try {
         st = build_host_mesh(n_nodes, xy, n_elems, tri, 1.0, opt.order, opt.chunk_elems, opt.precision == PFF_F32 ? 4 : 8,
-                             200 * 1024, hm, err);
+                             hm, err);
     } catch (const std::bad_alloc&) { st = PFF_ENOMEM; err = "out of host memory in mesh setup"; }
     if (st != PFF_OK) { set_error("pff_mesh_plan: " + err); return st; }
     if (node_new_of_old) std::memcpy(node_new_of_old, hm.node_new_of_old.data(), sizeof(int32_t) * hm.N);
@@ -293,13 +299,13 @@ pff_status pff_set_traction(pff_mesh* m, pff_state* s, int64_t n_edges, const in
 
 pff_status pff_init_accel(pff_mesh* m, pff_state* s, const pff_bc* bc)
 {
-    if (!m || !valid_state(s)) { set_error("pff_init_accel: null mesh or state pointer"); return PFF_EINVAL; }
+    if (!m || !valid_state(s)) { set_error("pff_init_accel: null mesh, null or misaligned (16 B) state pointer"); return PFF_EINVAL; }
     return launch_step(m, s, bc, 0.0, /*MODE_INIT*/ 1, nullptr, nullptr, nullptr);
 }
 
 pff_status pff_explicit_step(pff_mesh* m, pff_state* s, const pff_bc* bc, double dt)
 {
-    if (!m || !valid_state(s)) { set_error("pff_explicit_step: null mesh or state pointer"); return PFF_EINVAL; }
+    if (!m || !valid_state(s)) { set_error("pff_explicit_step: null mesh, null or misaligned (16 B) state pointer"); return PFF_EINVAL; }
     if (!(dt > 0) || !std::isfinite(dt)) { set_error("pff_explicit_step: dt must be > 0"); return PFF_EINVAL; }
     return launch_step(m, s, bc, dt, /*MODE_STEP*/ 0, nullptr, nullptr, nullptr);
 }
@@ -313,7 +319,7 @@ pff_status pff_internal_force(pff_mesh* m, const pff_state* s, void* fx, void* f
 
 pff_status pff_damage_solve(pff_mesh* m, pff_state* s, double rel_tol, int32_t max_iter, int32_t* iters, double* relres)
 {
-    if (!m || !valid_state(s)) { set_error("pff_damage_solve: null mesh or state pointer"); return PFF_EINVAL; }
+    if (!m || !valid_state(s)) { set_error("pff_damage_solve: null mesh, null or misaligned (16 B) state pointer"); return PFF_EINVAL; }
     if (!(rel_tol > 0) || max_iter < 1) { set_error("pff_damage_solve: need rel_tol > 0, max_iter >= 1"); return PFF_EINVAL; }
     return damage_solve(m, s, rel_tol, max_iter, iters, relres);
 }

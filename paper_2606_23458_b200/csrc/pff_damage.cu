@@ -1,29 +1,36 @@
 // Damage sub-problem (Eq. 6-8): matrix-free operator with consistent mass,
 // Jacobi-preconditioned CG (AT2, then clamp, L179) and projected CG with an active set (AT1, L181).
 //
-// Kernels per CG iteration (all early-exit when the device-resident control block says done):
-//   dmg_matvec_chunk   one CTA per chunk: forms the new search direction p = z + beta p for the nodes it
-//                      touches (z = D^-1 r on the free set), stages it in shared memory, element pass
-//                      q^e = (c_e M^e + kappa K^e) p^e into slots, ordered node gather, q and the p.q partial.
-//   dmg_matvec_shared  interface nodes; the last CTA reduces the partials in a fixed order and sets
-//                      alpha = rho / p.q (and the AT1 step bound) in the control block.
-//   dmg_vector         x += alpha p, r -= alpha q, next free set, r.z and ||r|| partials; the last CTA
-//                      decides continue / restart / converged and sets beta, rho.
-// alpha, beta, rho, norms never leave the device; the host polls the control block every few iterations.
+// ONE chunk kernel + one small interface kernel per CG iteration:
+//   dmg_iter_chunk   one CTA per chunk.  Every contiguous array of the chunk is streamed into shared memory
+//                    by TMA.  Prologue per node: apply the PREVIOUS iteration's step (x += alpha p,
+//                    r -= alpha q), re-derive the free set on a restart, form the new direction
+//                    p = z + beta p (z = D^-1 r on the free set).  Then the element pass
+//                    q^e = (c_e M^e + kappa K^e) p^e, the ordered node gather, and the block partials of
+//                    p.q, r.z, r.r and of the four sums that PREDICT r.z and r.r after the coming step
+//                    (z.q, q.D^-1 q, r.q, q.q), so that beta is known without another pass over the vectors.
+//   dmg_iter_shared  interface nodes (same prologue, ordered sum of the chunk partials); its blocks fold the
+//                    chunk partials in a fixed order and the last block sets alpha, beta, the restart /
+//                    truncation / convergence flags in the device-resident control block.
+// alpha, beta, norms never leave the device; the host polls the control block every few iterations.
+// Convergence is declared on the TRUE residual norm, or on the predicted one when its rounding error bound
+// is far below the tolerance (AT2); the pending last step is then applied by dmg_finalize.
 #include <algorithm>
 #include <cstring>
 
 #include "pff_device.cuh"
 #include "pff_mesh.h"
+#include "pff_tma.cuh"
 
 struct DamageCtrl {
-    double rho, pq, alpha, beta, amax, nb, tol, relres;
-    int iters, max_iter, done, status, sel, first, truncated, restarts;
+    double rz, alpha, beta, amax, nb, tol, relres;
+    int iters, max_iter, done, status, first, restart, trunc, pending, restarts;
 };
 
 namespace pff {
 
-constexpr int kPartStride = 4;  // partial-sum channels per block
+constexpr int kCh = 8;          // partial-sum channels: p.q, r.z, r.r, z.q, q.Dinv.q, r.q, q.q, min step bound
+constexpr int kMaxSharedBlocks = 1184;  // interface kernel grid cap (8 CTAs per SM, grid-stride)
 
 template <typename R>
 struct DmgArgs {
@@ -35,17 +42,20 @@ struct DmgArgs {
     const uint16_t* ell;
     const uint8_t* flags;
     R* halo_part;  // [3][n_slots]
-    int64_t n_slots;
-    int EC, max_nloc, N, N_int, N_sh, C, nbs;
-    const int32_t *sh_rowptr, *sh_slots;
+    int64_t n_slots, ell_total;
+    int EC, N, Ne, N_int, N_sh, C;
+    const int32_t *sh_rowptr, *halo_dst;
+    StageLayout lay;
+    StagePlan plan;
     const R* H;
     R* x;  // = state.d
     R *lb, *r, *p, *q, *dinv;
-    uint8_t* mask;  // [2][N]
+    uint8_t* mask;  // [N]: bit0 = in the free set, bit1 = damage-Dirichlet
     const R* p_in;  // plain mat-vec / hooks
     R *q_out, *b_out, *D_out;
-    double* part;
-    int64_t part_n;  // blocks per channel
+    double* part;    // [kCh][part_n] chunk-kernel block partials
+    double* part2;   // [kCh][kMaxSharedBlocks] interface-kernel block partials (chunk partials folded in)
+    int64_t part_n;
     DamageCtrl* ctrl;
     unsigned int* ticket;
     MatC<R> mat;
@@ -66,264 +76,391 @@ __device__ __forceinline__ bool last_block(unsigned int* ticket)
     return s_last;
 }
 
-// fixed-order sum / min of n block partials by one CTA
-__device__ __forceinline__ double reduce_partials_sum(const double* part, int64_t n, double* s_red)
+// Deterministic block reduction of kCh values at once (channels 0..6 summed, channel 7 minimised): fixed
+// shuffle tree, fixed warp order, two barriers.  Results land in s_out[0..kCh) (visible after the call).
+__device__ __forceinline__ void block_reduce_ch(double v[kCh], double* s_w /* [kCh][32] */, double* s_out /* [kCh] */)
 {
-    double v = 0.0;
-    for (int64_t i = threadIdx.x; i < n; i += blockDim.x) v += __ldcg(part + i);
-    return block_sum(v, s_red);
-}
-__device__ __forceinline__ double reduce_partials_min(const double* part, int64_t n, double* s_red)
-{
-    double v = INFINITY;
-    for (int64_t i = threadIdx.x; i < n; i += blockDim.x) v = fmin(v, __ldcg(part + i));
-    return block_min(v, s_red);
+#pragma unroll
+    for (int c = 0; c < kCh; ++c)
+        for (int o = 16; o > 0; o >>= 1) {
+            const double t = __shfl_xor_sync(0xffffffffu, v[c], o);
+            v[c] = (c == kCh - 1) ? fmin(v[c], t) : v[c] + t;
+        }
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31, nw = (blockDim.x + 31) >> 5;
+    __syncthreads();
+    if (l == 0) {
+#pragma unroll
+        for (int c = 0; c < kCh; ++c) s_w[c * 32 + w] = v[c];
+    }
+    __syncthreads();
+    if (w < kCh) {  // warp c reduces channel c
+        double t = l < nw ? s_w[w * 32 + l] : (w == kCh - 1 ? INFINITY : 0.0);
+        for (int o = 16; o > 0; o >>= 1) {
+            const double u = __shfl_xor_sync(0xffffffffu, t, o);
+            t = (w == kCh - 1) ? fmin(t, u) : t + u;
+        }
+        if (l == 0) s_out[w] = t;
+    }
+    __syncthreads();
 }
 
 enum { DM_CG = 0, DM_PLAIN = 1 };
 
-// new search direction of node gid (identical expression in the chunk and the interface kernel)
-template <typename R>
-__device__ __forceinline__ R new_direction(const DmgArgs<R>& a, int gid, int sel, double beta)
+struct IterScalars {
+    double alpha, beta;
+    int first, restart, trunc;
+};
+
+// The per-node prologue of one CG iteration, identical for interior, halo and interface nodes:
+// applies the previous step, re-derives the free set on a restart and returns the new direction.
+// x, r, mk are updated in place (mk: bit0 free, bit1 fixed).
+template <typename R, bool PROJ>
+__device__ __forceinline__ R cg_node_prologue(const IterScalars& sc, R& x, R& r, R p, R q, R dinv, R lb, uint8_t& mk)
 {
-    if (!a.mask[(int64_t)sel * a.N + gid]) return R(0);
-    const R z = a.r[gid] * a.dinv[gid];
-    return beta == 0.0 ? z : rfma(R(beta), a.p[gid], z);
+    bool free = (mk & 1) != 0;
+    const bool fixed = (mk & 2) != 0;
+    if (!sc.first) {
+        if (free) {
+            R xn = rfma(R(sc.alpha), p, x);
+            if (PROJ) {
+                // snap the node(s) that define a truncated step, and never leave the feasible set
+                if (sc.trunc && p < R(0) && (double(lb) - double(x)) / double(p) <= sc.alpha * (1.0 + 1e-12)) xn = lb;
+                if (xn < lb) xn = lb;
+            }
+            x = xn;
+        }
+        r = rfma(R(-sc.alpha), q, r);  // residual kept current on ALL nodes
+    }
+    if (sc.restart) {
+        free = !fixed && (!PROJ || x > lb || r > R(0));
+        mk = uint8_t((free ? 1 : 0) | (fixed ? 2 : 0));
+    }
+    if (!free) return R(0);
+    const R z = r * dinv;
+    return sc.restart ? z : rfma(R(sc.beta), p, z);
 }
 
-template <typename R, int MODE, bool PROJ>
-__global__ void __launch_bounds__(kTPB) dmg_matvec_chunk(const DmgArgs<R> a)
+// element operator: q^e = (c_e M^e + kappa K^e) p^e with M^e = A (1 + delta_ij) / 12 (L185)
+template <typename R>
+__device__ __forceinline__ void elem_damage_apply(const MatC<R>& mat, R b1, R c1, R b2, R c2, R A, R He, R p1, R p2, R p3,
+                                                  R& q1, R& q2, R& q3)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    __shared__ double s_red[32];
-    R* s_p = reinterpret_cast<R*>(smem_raw);
-    R* s_q = s_p + a.max_nloc;  // [3][EC]
-    int sel = 0;
-    double beta = 0.0;
-    if (MODE == DM_CG) {
-        if (a.ctrl->done) return;
-        sel = a.ctrl->sel; beta = a.ctrl->beta;
-    }
-    const ChunkMeta cm = a.meta[blockIdx.x];
-    const int nloc = cm.n_int + cm.n_halo, tid = threadIdx.x;
-    double amax = INFINITY;
+    const R ce = mat.c0 + R(2) * He;  // reaction coefficient (Eq. 6 / Eq. 8)
+    const R m12 = ce * A * R(1.0 / 12.0), sum = p1 + p2 + p3;
+    const R gx = b1 * (p1 - p3) + b2 * (p2 - p3), gy = c1 * (p1 - p3) + c2 * (p2 - p3);
+    const R kA = mat.kappa * A;
+    const R k1 = kA * (b1 * gx + c1 * gy), k2 = kA * (b2 * gx + c2 * gy);
+    q1 = m12 * (p1 + sum) + k1;
+    q2 = m12 * (p2 + sum) + k2;
+    q3 = m12 * (p3 + sum) - (k1 + k2);
+}
 
-    for (int i = tid; i < nloc; i += kTPB) {
-        const int gid = i < cm.n_int ? cm.node_start + i : a.halo_ids[cm.halo_off + i - cm.n_int];
+// One CTA per chunk; stage = StageLayout kind 1 (pff_internal.h): lconn | geometry | scalar slots [3 EC + 1] |
+// area | H | x r p q 1/D lb [node_len] | mask | gather table | mbarrier.
+template <typename R, int MODE, bool PROJ>
+__global__ void __launch_bounds__(kTPB) dmg_iter_chunk(const DmgArgs<R> a)
+{
+    extern __shared__ __align__(128) unsigned char smem[];
+    __shared__ double s_w[kCh * 32], s_out[kCh];
+    constexpr int A = 16 / sizeof(R);
+    IterScalars sc{0.0, 0.0, 1, 1, 0};
+    if (MODE == DM_CG) {
+        const DamageCtrl* c = a.ctrl;
+        if (c->done) return;
+        sc.alpha = c->alpha; sc.beta = c->beta; sc.first = c->first; sc.restart = c->restart; sc.trunc = c->trunc;
+    }
+    const StageLayout& L = a.lay;
+    const ushort4* s_lconn = reinterpret_cast<const ushort4*>(smem + L.lconn);
+    const unsigned char* s_geo = smem + L.geo;
+    R* s_slot = reinterpret_cast<R*>(smem + L.slots);
+    const R* s_area = reinterpret_cast<const R*>(smem + L.area);
+    const R* s_H = reinterpret_cast<const R*>(smem + L.H);
+    R* s_x = reinterpret_cast<R*>(smem + L.node[0]);
+    R* s_r = reinterpret_cast<R*>(smem + L.node[1]);
+    R* s_p = reinterpret_cast<R*>(smem + L.node[2]);
+    const R* s_q = reinterpret_cast<const R*>(smem + L.node[3]);
+    const R* s_dinv = reinterpret_cast<const R*>(smem + L.node[4]);
+    const R* s_lb = reinterpret_cast<const R*>(smem + L.node[5]);
+    uint8_t* s_mask = smem + L.flags;
+    const uint16_t* s_ell = reinterpret_cast<const uint16_t*>(smem + L.ell);
+    uint64_t* bar = reinterpret_cast<uint64_t*>(smem + L.bar);
+
+    const int tid = threadIdx.x;
+    const ChunkMeta cm = a.meta[blockIdx.x];
+    if (tid == 0) { mbar_init(bar, 2); s_slot[3 * a.EC] = R(0); }
+    __syncthreads();
+    if (tid < 32)  // element arrays first: their range follows from blockIdx (in flight while the meta is fetched)
+        stage_issue_plan(a.plan, smem, bar, tid, true, blockIdx.x * a.EC, min(a.EC, a.Ne - blockIdx.x * a.EC), a.Ne, 0, 0, a.N,
+                         0, 0, 0);
+    const int nloc = cm.n_int + cm.n_halo;
+    const int shift = cm.node_start & (A - 1), hb = (shift + cm.n_int + A - 1) & ~(A - 1), fshift = cm.node_start & 15;
+    int* s_fwd = reinterpret_cast<int*>(smem + L.node[3]);  // halo part of the q array: forwards the partial slots
+    if (tid < 32)
+        stage_issue_plan(a.plan, smem, bar, tid, false, 0, 0, a.Ne, cm.node_start, cm.n_int, a.N, cm.ell_off, cm.ell_w * nloc,
+                         (int)a.ell_total);
+    // halo nodes: indexed gathers + the same prologue (no global writes: the interface kernel owns them)
+    for (int j = tid; j < cm.n_halo; j += kTPB) {
+        const int gid = __ldg(a.halo_ids + cm.halo_off + j);
         R pn;
         if (MODE == DM_CG) {
-            pn = new_direction<R>(a, gid, sel, beta);
-            if (i < cm.n_int) {
-                a.p[gid] = pn;
-                if (PROJ && pn < R(0)) amax = fmin(amax, (double(a.lb[gid]) - double(a.x[gid])) / double(pn));
-            }
+            R x = R(0), r = a.r[gid], p = R(0), q = R(0), lb = R(0);
+            const R dinv = a.dinv[gid];
+            uint8_t mk = a.mask[gid];
+            if (!sc.first) { x = a.x[gid]; p = a.p[gid]; q = a.q[gid]; }
+            if (PROJ) { if (sc.first) x = a.x[gid]; lb = a.lb[gid]; }
+            pn = cg_node_prologue<R, PROJ>(sc, x, r, p, q, dinv, lb, mk);
         } else {
             pn = a.p_in[gid];
         }
-        s_p[i] = pn;
+        s_p[hb + j] = pn;
+        s_fwd[(hb + j) * (int)(sizeof(R) / 4)] = __ldg(a.halo_dst + cm.halo_off + j);
+    }
+    mbar_wait(bar, 0);
+
+    double acc[kCh];
+#pragma unroll
+    for (int c = 0; c < kCh; ++c) acc[c] = 0.0;
+    acc[kCh - 1] = INFINITY;
+    if (MODE == DM_CG) {
+        for (int i = tid; i < cm.n_int; i += kTPB) {
+            const int s = shift + i, gid = cm.node_start + i;
+            R x = R(0), r = s_r[s], p = R(0), q = R(0), lb = R(0);
+            const R dinv = s_dinv[s];
+            uint8_t mk = s_mask[fshift + i];
+            const uint8_t mk0 = mk;
+            if (!sc.first) { x = s_x[s]; p = s_p[s]; q = s_q[s]; }
+            if (PROJ) { if (sc.first) x = s_x[s]; lb = s_lb[s]; }
+            const R pn = cg_node_prologue<R, PROJ>(sc, x, r, p, q, dinv, lb, mk);
+            if (!sc.first) { if (mk0 & 1) a.x[gid] = x; a.r[gid] = r; }
+            if (mk != mk0) a.mask[gid] = mk;
+            a.p[gid] = pn;
+            s_p[s] = pn; s_r[s] = r; s_mask[fshift + i] = mk;
+            if (mk & 1) {
+                const double rd = double(r), zd = rd * double(dinv);
+                acc[1] += rd * zd; acc[2] += rd * rd;
+                if (PROJ && pn < R(0)) acc[kCh - 1] = fmin(acc[kCh - 1], (double(lb) - double(x)) / double(pn));
+            }
+        }
     }
     __syncthreads();
 
     for (int e = tid; e < cm.n_elem; e += kTPB) {
-        const int ge = cm.elem_start + e;
-        const ushort4 c = __ldg(a.lconn + ge);
-        R b1, c1, b2, c2;
-        Geo<R>::load(a.ga, a.gb, ge, b1, c1, b2, c2);
-        const R A = __ldg(a.area + ge);
-        const R ce = a.mat.c0 + R(2) * a.H[ge];  // reaction coefficient (Eq. 6 / Eq. 8)
-        const R p1 = s_p[c.x], p2 = s_p[c.y], p3 = s_p[c.z];
-        const R m12 = ce * A * R(1.0 / 12.0), sum = p1 + p2 + p3;  // consistent mass A(1+delta_ij)/12 (L185)
-        const R gx = b1 * (p1 - p3) + b2 * (p2 - p3), gy = c1 * (p1 - p3) + c2 * (p2 - p3);
-        const R kA = a.mat.kappa * A;
-        const R k1 = kA * (b1 * gx + c1 * gy), k2 = kA * (b2 * gx + c2 * gy);
-        s_q[e] = m12 * (p1 + sum) + k1;
-        s_q[a.EC + e] = m12 * (p2 + sum) + k2;
-        s_q[2 * a.EC + e] = m12 * (p3 + sum) - (k1 + k2);
+        const ushort4 c = s_lconn[e];
+        R b1, c1, b2, c2, q1, q2, q3;
+        Geo<R>::load_smem(s_geo, e, a.EC, b1, c1, b2, c2);
+        elem_damage_apply<R>(a.mat, b1, c1, b2, c2, s_area[e], s_H[e], s_p[c.x], s_p[c.y], s_p[c.z], q1, q2, q3);
+        s_slot[e] = q1; s_slot[a.EC + e] = q2; s_slot[2 * a.EC + e] = q3;
     }
     __syncthreads();
 
-    const uint16_t* ell = a.ell + cm.ell_off;
-    double pq = 0.0;
     for (int i = tid; i < nloc; i += kTPB) {
         R qs = R(0);
-        for (int k = 0; k < cm.ell_w; ++k) {
-            const unsigned ent = ell[k * nloc + i];
-            if (ent != 0xFFFFu) qs += s_q[(ent & 3) * a.EC + (ent >> 2)];
-        }
+        const uint16_t* row = s_ell + i;
+#pragma unroll 4
+        for (int k = 0; k < cm.ell_w; ++k) qs += s_slot[row[k * nloc]];
         if (i < cm.n_int) {
-            const int gid = cm.node_start + i;
-            if (MODE == DM_CG) { a.q[gid] = qs; pq += double(s_p[i]) * double(qs); }
-            else a.q_out[gid] = qs;
+            const int gid = cm.node_start + i, s = shift + i;
+            if (MODE == DM_CG) {
+                a.q[gid] = qs;
+                const double qd = double(qs);
+                acc[0] += double(s_p[s]) * qd;
+                if (s_mask[fshift + i] & 1) {
+                    const double rd = double(s_r[s]), dv = double(s_dinv[s]);
+                    acc[3] += rd * dv * qd; acc[4] += dv * qd * qd; acc[5] += rd * qd; acc[6] += qd * qd;
+                }
+            } else {
+                a.q_out[gid] = qs;
+            }
         } else {
-            a.halo_part[cm.halo_off + i - cm.n_int] = qs;
+            a.halo_part[s_fwd[(hb + i - cm.n_int) * (int)(sizeof(R) / 4)]] = qs;
         }
     }
     if (MODE == DM_CG) {
-        const double t = block_sum(pq, s_red);
-        const double tm = PROJ ? block_min(amax, s_red) : INFINITY;
-        if (tid == 0) { a.part[blockIdx.x] = t; a.part[a.part_n + blockIdx.x] = tm; }
+        block_reduce_ch(acc, s_w, s_out);
+        if (tid < kCh) a.part[(int64_t)tid * a.part_n + blockIdx.x] = s_out[tid];
     }
 }
 
-template <typename R, int MODE, bool PROJ>
-__global__ void __launch_bounds__(kTPB) dmg_matvec_shared(const DmgArgs<R> a)
+// Scalar step of the recurrence, run by one thread after the fixed-order reduction of all partials.
+// t[]: p.q, r.z, r.r (free set, residual BEFORE the coming step), z.q, q.Dinv.q, r.q, q.q, step bound.
+template <bool PROJ>
+__device__ __forceinline__ void cg_scalar_step(DamageCtrl* c, const double t[kCh])
 {
-    __shared__ double s_red[32];
-    int sel = 0;
-    double beta = 0.0;
-    if (MODE == DM_CG) {
-        if (a.ctrl->done) return;
-        sel = a.ctrl->sel; beta = a.ctrl->beta;
+    const double pq = t[0], rz = t[1], rr = t[2], lim = c->tol * c->nb;
+    const int was_restart = c->restart;
+    c->iters += 1;
+    c->first = 0;
+    c->relres = sqrt(rr) / c->nb;
+    // true residual norm: AT2 every iteration; AT1 on the freshly derived free set (then KKT holds)
+    if ((was_restart || !PROJ) && sqrt(rr) <= lim) { c->done = 1; c->status = PFF_OK; c->pending = 0; return; }
+    if (was_restart) c->restarts += 1;
+    double alpha = pq > 0.0 ? rz / pq : 0.0;
+    const int trunc = (PROJ && alpha >= t[kCh - 1]) ? 1 : 0;
+    if (trunc) alpha = t[kCh - 1];
+    // r.z and r.r after the step, from the sums gathered in this pass (no extra pass over the vectors)
+    const double rz_pred = fmax(rz - 2.0 * alpha * t[3] + alpha * alpha * t[4], 0.0);
+    const double rr_pred = rr - 2.0 * alpha * t[5] + alpha * alpha * t[6];
+    c->alpha = alpha; c->trunc = trunc; c->amax = t[kCh - 1]; c->rz = rz;
+    c->beta = rz > 0.0 ? rz_pred / rz : 0.0;
+    c->pending = 1;
+    if (PROJ) {
+        c->restart = (trunc || sqrt(fmax(rr_pred, 0.0)) <= lim) ? 1 : 0;
+    } else {
+        c->restart = 0;
+        // predicted norm trusted only when its rounding-error bound is itself far below the tolerance
+        const double err = 64.0 * 2.220446049250313e-16 * (rr + 2.0 * alpha * fabs(t[5]) + alpha * alpha * t[6]);
+        if (rr_pred + err <= lim * lim) {
+            c->done = 1; c->status = PFF_OK; c->relres = sqrt(fmax(rr_pred, 0.0)) / c->nb;
+            return;
+        }
     }
-    const int s = blockIdx.x * kTPB + threadIdx.x;
-    double pq = 0.0, amax = INFINITY;
-    if (s < a.N_sh) {
+    if (c->iters >= c->max_iter) { c->done = 1; c->status = PFF_ENOCONV; }
+}
+
+// Folds this block's own values (s_out) with its slice of the chunk-kernel partials, publishes them, and in
+// the last block reduces everything in a fixed order.  Returns true in the last block with t[] valid in thread 0.
+__device__ __forceinline__ bool fold_and_finish(const double* part, int64_t part_n, int n_chunk_blocks, double* part2,
+                                                unsigned int* ticket, double* s_w, double* s_out, double t[kCh])
+{
+    const int tid = threadIdx.x, G = gridDim.x, b = blockIdx.x;
+    if (tid < kCh) {
+        const int per = (n_chunk_blocks + G - 1) / G;
+        const int c0 = b * per, c1 = min(n_chunk_blocks, c0 + per);
+        double v = s_out[tid];
+        for (int c = c0; c < c1; ++c) {
+            const double u = __ldcg(part + (int64_t)tid * part_n + c);
+            v = (tid == kCh - 1) ? fmin(v, u) : v + u;
+        }
+        part2[tid * kMaxSharedBlocks + b] = v;
+    }
+    if (!last_block(ticket)) return false;
+    const int w = tid >> 5, l = tid & 31;
+    if (w < kCh) {  // warp c: fixed-order strided sum of channel c, then the fixed shuffle tree
+        double v = (w == kCh - 1) ? INFINITY : 0.0;
+        for (int i = l; i < G; i += 32) {
+            const double u = __ldcg(part2 + w * kMaxSharedBlocks + i);
+            v = (w == kCh - 1) ? fmin(v, u) : v + u;
+        }
+        for (int o = 16; o > 0; o >>= 1) {
+            const double u = __shfl_xor_sync(0xffffffffu, v, o);
+            v = (w == kCh - 1) ? fmin(v, u) : v + u;
+        }
+        if (l == 0) s_w[w] = v;
+    }
+    __syncthreads();
+    if (tid == 0)
+        for (int c = 0; c < kCh; ++c) t[c] = s_w[c];
+    return true;
+}
+
+template <typename R, int MODE, bool PROJ>
+__global__ void __launch_bounds__(kTPB) dmg_iter_shared(const DmgArgs<R> a)
+{
+    __shared__ double s_w[kCh * 32], s_out[kCh];
+    IterScalars sc{0.0, 0.0, 1, 1, 0};
+    if (MODE == DM_CG) {
+        const DamageCtrl* c = a.ctrl;
+        if (c->done) return;
+        sc.alpha = c->alpha; sc.beta = c->beta; sc.first = c->first; sc.restart = c->restart; sc.trunc = c->trunc;
+    }
+    double acc[kCh];
+#pragma unroll
+    for (int c = 0; c < kCh; ++c) acc[c] = 0.0;
+    acc[kCh - 1] = INFINITY;
+    for (int s = blockIdx.x * kTPB + threadIdx.x; s < a.N_sh; s += gridDim.x * kTPB) {
         const int gid = a.N_int + s;
         R qs = R(0);
-        for (int k = a.sh_rowptr[s]; k < a.sh_rowptr[s + 1]; ++k) qs += a.halo_part[a.sh_slots[k]];
+        for (int k = a.sh_rowptr[s]; k < a.sh_rowptr[s + 1]; ++k) qs += a.halo_part[k];  // contiguous, ascending chunk
         if (MODE == DM_CG) {
-            const R pn = new_direction<R>(a, gid, sel, beta);
+            R x = R(0), r = a.r[gid], p = R(0), q = R(0), lb = R(0);
+            const R dinv = a.dinv[gid];
+            uint8_t mk = a.mask[gid];
+            const uint8_t mk0 = mk;
+            if (!sc.first) { x = a.x[gid]; p = a.p[gid]; q = a.q[gid]; }
+            if (PROJ) { if (sc.first) x = a.x[gid]; lb = a.lb[gid]; }
+            const R pn = cg_node_prologue<R, PROJ>(sc, x, r, p, q, dinv, lb, mk);
+            if (!sc.first) { if (mk0 & 1) a.x[gid] = x; a.r[gid] = r; }
+            if (mk != mk0) a.mask[gid] = mk;
             a.p[gid] = pn; a.q[gid] = qs;
-            pq = double(pn) * double(qs);
-            if (PROJ && pn < R(0)) amax = (double(a.lb[gid]) - double(a.x[gid])) / double(pn);
+            const double qd = double(qs);
+            acc[0] += double(pn) * qd;
+            if (mk & 1) {
+                const double rd = double(r), dv = double(dinv);
+                acc[1] += rd * rd * dv; acc[2] += rd * rd;
+                acc[3] += rd * dv * qd; acc[4] += dv * qd * qd; acc[5] += rd * qd; acc[6] += qd * qd;
+                if (PROJ && pn < R(0)) acc[kCh - 1] = fmin(acc[kCh - 1], (double(lb) - double(x)) / double(pn));
+            }
         } else {
             a.q_out[gid] = qs;
         }
     }
     if (MODE != DM_CG) return;
-    const double t = block_sum(pq, s_red);
-    const double tm = PROJ ? block_min(amax, s_red) : INFINITY;
-    if (threadIdx.x == 0) { a.part[a.C + blockIdx.x] = t; a.part[a.part_n + a.C + blockIdx.x] = tm; }
-    if (last_block(a.ticket)) {
-        const int64_t nb = a.C + gridDim.x;
-        const double pqs = reduce_partials_sum(a.part, nb, s_red);
-        const double am = PROJ ? reduce_partials_min(a.part + a.part_n, nb, s_red) : INFINITY;
-        if (threadIdx.x == 0) {
-            DamageCtrl* c = a.ctrl;
-            double alpha = c->rho / pqs;
-            c->pq = pqs; c->amax = am;
-            c->truncated = (PROJ && alpha >= am) ? 1 : 0;
-            if (c->truncated) alpha = am;
-            c->alpha = alpha;
-            c->iters += 1;
-        }
-    }
+    block_reduce_ch(acc, s_w, s_out);
+    double t[kCh];
+    if (fold_and_finish(a.part, a.part_n, a.C, a.part2, a.ticket, s_w, s_out, t) && threadIdx.x == 0)
+        cg_scalar_step<PROJ>(a.ctrl, t);
 }
 
-// x += alpha p, r -= alpha q; candidate free set; partial sums.  One thread per node.
-template <typename R, bool PROJ>
-__global__ void __launch_bounds__(kTPB) dmg_vector(const DmgArgs<R> a)
-{
-    __shared__ double s_red[32];
-    DamageCtrl* c = a.ctrl;
-    if (c->done) return;
-    const int first = c->first, sel = c->sel, trunc = c->truncated;
-    const double alpha = first ? 0.0 : c->alpha;
-    const int i = blockIdx.x * kTPB + threadIdx.x;
-    double rn_old = 0.0, rz_old = 0.0, rn_new = 0.0, rz_new = 0.0;
-    if (i < a.N) {
-        const bool fixed = (a.flags[i] & 4) != 0;
-        const bool m_old = !first && a.mask[(int64_t)sel * a.N + i];
-        R x = a.x[i], r = a.r[i];
-        const R lb = a.lb[i];
-        if (!first) {
-            const R p = a.p[i], q = a.q[i];
-            if (m_old) {
-                R xn = rfma(R(alpha), p, x);
-                if (PROJ) {
-                    // snap the node(s) that define the truncated step, and never leave the feasible set
-                    if (trunc && p < R(0) && (double(lb) - double(x)) / double(p) <= alpha * (1.0 + 1e-12)) xn = lb;
-                    if (xn < lb) xn = lb;
-                }
-                x = xn;
-                a.x[i] = x;
-            }
-            r = rfma(R(-alpha), q, r);  // residual kept current on ALL nodes
-            a.r[i] = r;
-        }
-        const bool m_new = !fixed && (!PROJ || x > lb || r > R(0));
-        a.mask[(int64_t)(1 - sel) * a.N + i] = m_new ? 1 : 0;
-        const double rr = double(r) * double(r), rz = rr * double(a.dinv[i]);
-        if (m_old) { rn_old = rr; rz_old = rz; }
-        if (m_new) { rn_new = rr; rz_new = rz; }
-    }
-    const double t0 = block_sum(rn_old, s_red), t1 = block_sum(rz_old, s_red);
-    const double t2 = block_sum(rn_new, s_red), t3 = block_sum(rz_new, s_red);
-    if (threadIdx.x == 0) {
-        a.part[blockIdx.x] = t0; a.part[a.part_n + blockIdx.x] = t1;
-        a.part[2 * a.part_n + blockIdx.x] = t2; a.part[3 * a.part_n + blockIdx.x] = t3;
-    }
-    if (last_block(a.ticket)) {
-        const double rno = reduce_partials_sum(a.part, gridDim.x, s_red);
-        const double rzo = reduce_partials_sum(a.part + a.part_n, gridDim.x, s_red);
-        const double rnn = reduce_partials_sum(a.part + 2 * a.part_n, gridDim.x, s_red);
-        const double rzn = reduce_partials_sum(a.part + 3 * a.part_n, gridDim.x, s_red);
-        if (threadIdx.x == 0) {
-            const double lim = c->tol * c->nb;
-            bool restart = first || trunc || sqrt(rno) <= lim;
-            if (restart) {
-                c->relres = sqrt(rnn) / c->nb;
-                if (sqrt(rnn) <= lim) { c->done = 1; c->status = PFF_OK; }
-                else { c->sel = 1 - sel; c->rho = rzn; c->beta = 0.0; c->restarts += 1; }
-            } else {
-                c->relres = sqrt(rno) / c->nb;
-                c->beta = rzo / c->rho;
-                c->rho = rzo;
-            }
-            if (!c->done && c->iters >= c->max_iter) { c->done = 1; c->status = PFF_ENOCONV; }
-            c->first = 0; c->truncated = 0;
-        }
-    }
-}
-
-// setup: r0 = b - A x0, D^-1, lb = d_n, norms (one chunk pass + interface pass).  HOOK: only b / D out.
+// setup: r0 = b - A x0, D^-1, lb = d_n, mask, norms (one chunk pass + interface pass).  HOOK: only b / D out.
+// Stage = StageLayout kind 2: lconn | geometry | slots q, D, b (each [3 EC + 1]) | area | H | x [node_len] | gather table
 template <typename R, bool HOOK>
 __global__ void __launch_bounds__(kTPB) dmg_setup_chunk(const DmgArgs<R> a)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    __shared__ double s_red[32];
-    R* s_p = reinterpret_cast<R*>(smem_raw);
-    R* s_q = s_p + a.max_nloc;  // [7][EC]: q1 q2 q3 D1 D2 D3 b
+    extern __shared__ __align__(128) unsigned char smem[];
+    __shared__ double s_w[kCh * 32], s_out[kCh];
+    constexpr int A = 16 / sizeof(R);
+    const StageLayout& L = a.lay;
+    const ushort4* s_lconn = reinterpret_cast<const ushort4*>(smem + L.lconn);
+    const unsigned char* s_geo = smem + L.geo;
+    R* s_sq = reinterpret_cast<R*>(smem + L.slots);
+    R* s_sD = reinterpret_cast<R*>(smem + L.slots + L.slot_stride);
+    R* s_sb = reinterpret_cast<R*>(smem + L.slots + 2 * L.slot_stride);
+    const R* s_area = reinterpret_cast<const R*>(smem + L.area);
+    const R* s_H = reinterpret_cast<const R*>(smem + L.H);
+    R* s_x = reinterpret_cast<R*>(smem + L.node[0]);
+    const uint16_t* s_ell = reinterpret_cast<const uint16_t*>(smem + L.ell);
+    uint64_t* bar = reinterpret_cast<uint64_t*>(smem + L.bar);
+    const int tid = threadIdx.x, EC = a.EC;
     const ChunkMeta cm = a.meta[blockIdx.x];
-    const int nloc = cm.n_int + cm.n_halo, tid = threadIdx.x;
-    for (int i = tid; i < nloc; i += kTPB) {
-        const int gid = i < cm.n_int ? cm.node_start + i : a.halo_ids[cm.halo_off + i - cm.n_int];
-        s_p[i] = a.x[gid];
-    }
+    if (tid == 0) { mbar_init(bar, 2); s_sq[3 * EC] = R(0); s_sD[3 * EC] = R(0); s_sb[3 * EC] = R(0); }
     __syncthreads();
+    if (tid < 32)
+        stage_issue_plan(a.plan, smem, bar, tid, true, blockIdx.x * EC, min(EC, a.Ne - blockIdx.x * EC), a.Ne, 0, 0, a.N, 0, 0, 0);
+    const int nloc = cm.n_int + cm.n_halo;
+    const int shift = cm.node_start & (A - 1), hb = (shift + cm.n_int + A - 1) & ~(A - 1);
+    if (tid < 32)
+        stage_issue_plan(a.plan, smem, bar, tid, false, 0, 0, a.Ne, cm.node_start, cm.n_int, a.N, cm.ell_off, cm.ell_w * nloc,
+                         (int)a.ell_total);
+    for (int j = tid; j < cm.n_halo; j += kTPB) s_x[hb + j] = a.x[__ldg(a.halo_ids + cm.halo_off + j)];
+    mbar_wait(bar, 0);
+    __syncthreads();
+
     for (int e = tid; e < cm.n_elem; e += kTPB) {
-        const int ge = cm.elem_start + e;
-        const ushort4 c = __ldg(a.lconn + ge);
-        R b1, c1, b2, c2;
-        Geo<R>::load(a.ga, a.gb, ge, b1, c1, b2, c2);
-        const R A = __ldg(a.area + ge);
-        const R He = a.H[ge];
+        const ushort4 c = s_lconn[e];
+        R b1, c1, b2, c2, q1, q2, q3;
+        Geo<R>::load_smem(s_geo, e, EC, b1, c1, b2, c2);
+        const R Ar = s_area[e], He = s_H[e];
+        elem_damage_apply<R>(a.mat, b1, c1, b2, c2, Ar, He, s_x[c.x], s_x[c.y], s_x[c.z], q1, q2, q3);
+        s_sq[e] = q1; s_sq[EC + e] = q2; s_sq[2 * EC + e] = q3;
         const R ce = a.mat.c0 + R(2) * He, se = R(2) * He - a.mat.s0;
-        const R p1 = s_p[c.x], p2 = s_p[c.y], p3 = s_p[c.z];
-        const R m12 = ce * A * R(1.0 / 12.0), sum = p1 + p2 + p3;
-        const R gx = b1 * (p1 - p3) + b2 * (p2 - p3), gy = c1 * (p1 - p3) + c2 * (p2 - p3);
-        const R kA = a.mat.kappa * A;
-        const R k1 = kA * (b1 * gx + c1 * gy), k2 = kA * (b2 * gx + c2 * gy);
-        s_q[e] = m12 * (p1 + sum) + k1;
-        s_q[a.EC + e] = m12 * (p2 + sum) + k2;
-        s_q[2 * a.EC + e] = m12 * (p3 + sum) - (k1 + k2);
+        const R m12 = ce * Ar * R(1.0 / 12.0), kA = a.mat.kappa * Ar;
         const R b3 = -(b1 + b2), c3 = -(c1 + c2);
-        s_q[3 * a.EC + e] = R(2) * m12 + kA * (b1 * b1 + c1 * c1);  // A_ii = c A/6 + kappa A |grad phi_i|^2
-        s_q[4 * a.EC + e] = R(2) * m12 + kA * (b2 * b2 + c2 * c2);
-        s_q[5 * a.EC + e] = R(2) * m12 + kA * (b3 * b3 + c3 * c3);
-        s_q[6 * a.EC + e] = se * A * R(1.0 / 3.0);  // int s phi_i
+        s_sD[e] = R(2) * m12 + kA * (b1 * b1 + c1 * c1);  // A_ii = c A/6 + kappa A |grad phi_i|^2
+        s_sD[EC + e] = R(2) * m12 + kA * (b2 * b2 + c2 * c2);
+        s_sD[2 * EC + e] = R(2) * m12 + kA * (b3 * b3 + c3 * c3);
+        const R be = se * Ar * R(1.0 / 3.0);  // int s phi_i
+        s_sb[e] = be; s_sb[EC + e] = be; s_sb[2 * EC + e] = be;
     }
     __syncthreads();
-    const uint16_t* ell = a.ell + cm.ell_off;
-    double nb2 = 0.0, nr2 = 0.0;
+    double acc[kCh];
+#pragma unroll
+    for (int c = 0; c < kCh; ++c) acc[c] = 0.0;
     for (int i = tid; i < nloc; i += kTPB) {
         R qs = R(0), Ds = R(0), bs = R(0);
+        const uint16_t* row = s_ell + i;
         for (int k = 0; k < cm.ell_w; ++k) {
-            const unsigned ent = ell[k * nloc + i];
-            if (ent != 0xFFFFu) {
-                const int e = ent >> 2, cn = ent & 3;
-                qs += s_q[cn * a.EC + e]; Ds += s_q[(3 + cn) * a.EC + e]; bs += s_q[6 * a.EC + e];
-            }
+            const int idx = row[k * nloc];
+            qs += s_sq[idx]; Ds += s_sD[idx]; bs += s_sb[idx];
         }
         if (i < cm.n_int) {
             const int gid = cm.node_start + i;
@@ -332,66 +469,78 @@ __global__ void __launch_bounds__(kTPB) dmg_setup_chunk(const DmgArgs<R> a)
                 if (a.D_out) a.D_out[gid] = Ds;
             } else {
                 const R r = bs - qs;
-                a.r[gid] = r; a.dinv[gid] = R(1) / Ds; a.lb[gid] = s_p[i];
-                nb2 += double(bs) * double(bs);
-                if (!(a.flags[gid] & 4)) nr2 += double(r) * double(r);
+                const bool fixed = (a.flags[gid] & 4) != 0;
+                a.r[gid] = r; a.dinv[gid] = R(1) / Ds; a.lb[gid] = s_x[shift + i];
+                a.mask[gid] = fixed ? 2 : 1;
+                acc[0] += double(bs) * double(bs);
+                if (!fixed) acc[1] += double(r) * double(r);
             }
         } else {
-            const int64_t slot = cm.halo_off + i - cm.n_int;
+            const int slot = __ldg(a.halo_dst + cm.halo_off + i - cm.n_int);
             a.halo_part[slot] = qs; a.halo_part[a.n_slots + slot] = Ds; a.halo_part[2 * a.n_slots + slot] = bs;
         }
     }
     if (!HOOK) {
-        const double t0 = block_sum(nb2, s_red), t1 = block_sum(nr2, s_red);
-        if (tid == 0) { a.part[blockIdx.x] = t0; a.part[a.part_n + blockIdx.x] = t1; }
+        block_reduce_ch(acc, s_w, s_out);
+        if (tid < kCh) a.part[(int64_t)tid * a.part_n + blockIdx.x] = s_out[tid];
     }
 }
 
 template <typename R, bool HOOK>
 __global__ void __launch_bounds__(kTPB) dmg_setup_shared(const DmgArgs<R> a)
 {
-    __shared__ double s_red[32];
-    const int s = blockIdx.x * kTPB + threadIdx.x;
-    double nb2 = 0.0, nr2 = 0.0;
-    if (s < a.N_sh) {
+    __shared__ double s_w[kCh * 32], s_out[kCh];
+    double acc[kCh];
+#pragma unroll
+    for (int c = 0; c < kCh; ++c) acc[c] = 0.0;
+    for (int s = blockIdx.x * kTPB + threadIdx.x; s < a.N_sh; s += gridDim.x * kTPB) {
         const int gid = a.N_int + s;
         R qs = R(0), Ds = R(0), bs = R(0);
         for (int k = a.sh_rowptr[s]; k < a.sh_rowptr[s + 1]; ++k) {
-            const int slot = a.sh_slots[k];
-            qs += a.halo_part[slot]; Ds += a.halo_part[a.n_slots + slot]; bs += a.halo_part[2 * a.n_slots + slot];
+            qs += a.halo_part[k]; Ds += a.halo_part[a.n_slots + k]; bs += a.halo_part[2 * a.n_slots + k];
         }
         if (HOOK) {
             if (a.b_out) a.b_out[gid] = bs;
             if (a.D_out) a.D_out[gid] = Ds;
         } else {
             const R r = bs - qs;
+            const bool fixed = (a.flags[gid] & 4) != 0;
             a.r[gid] = r; a.dinv[gid] = R(1) / Ds; a.lb[gid] = a.x[gid];
-            nb2 = double(bs) * double(bs);
-            if (!(a.flags[gid] & 4)) nr2 = double(r) * double(r);
+            a.mask[gid] = fixed ? 2 : 1;
+            acc[0] += double(bs) * double(bs);
+            if (!fixed) acc[1] += double(r) * double(r);
         }
     }
     if (HOOK) return;
-    const double t0 = block_sum(nb2, s_red), t1 = block_sum(nr2, s_red);
-    if (threadIdx.x == 0) { a.part[a.C + blockIdx.x] = t0; a.part[a.part_n + a.C + blockIdx.x] = t1; }
-    if (last_block(a.ticket)) {
-        const int64_t nb = a.C + gridDim.x;
-        const double sb = reduce_partials_sum(a.part, nb, s_red);
-        const double sr = reduce_partials_sum(a.part + a.part_n, nb, s_red);
-        if (threadIdx.x == 0) a.ctrl->nb = fmax(fmax(sqrt(sb), sqrt(sr)), 1e-300);
-    }
+    acc[kCh - 1] = INFINITY;
+    block_reduce_ch(acc, s_w, s_out);
+    double t[kCh];
+    if (fold_and_finish(a.part, a.part_n, a.C, a.part2, a.ticket, s_w, s_out, t) && threadIdx.x == 0)
+        a.ctrl->nb = fmax(fmax(sqrt(t[0]), sqrt(t[1])), 1e-300);
 }
 
-// d <- min(1, max(d_n, x)) on the non-Dirichlet nodes (L179)
-template <typename R>
-__global__ void __launch_bounds__(kTPB) dmg_finalize(int N, R* x, const R* lb, const uint8_t* flags)
+// applies the pending last step (if any), then d <- min(1, max(d_n, x)) on the non-Dirichlet nodes (L179)
+template <typename R, bool PROJ>
+__global__ void __launch_bounds__(kTPB) dmg_finalize(const DmgArgs<R> a)
 {
-    const int i = blockIdx.x * kTPB + threadIdx.x;
-    if (i >= N || (flags[i] & 4)) return;
-    R v = x[i];
-    const R l = lb[i];
-    if (v < l) v = l;
-    if (v > R(1)) v = R(1);
-    x[i] = v;
+    const DamageCtrl* c = a.ctrl;
+    const bool pending = c->pending != 0;
+    IterScalars sc{c->alpha, 0.0, 0, 0, c->trunc};
+    for (int i = blockIdx.x * kTPB + threadIdx.x; i < a.N; i += gridDim.x * kTPB) {
+        const uint8_t mk = a.mask[i];
+        if (mk & 2) continue;
+        R v = a.x[i];
+        const R l = a.lb[i];
+        if (pending && (mk & 1)) {
+            const R p = a.p[i];
+            R xn = rfma(R(sc.alpha), p, v);
+            if (PROJ && sc.trunc && p < R(0) && (double(l) - double(v)) / double(p) <= sc.alpha * (1.0 + 1e-12)) xn = l;
+            v = xn;
+        }
+        if (v < l) v = l;
+        if (v > R(1)) v = R(1);
+        a.x[i] = v;
+    }
 }
 
 template <typename R>
@@ -401,26 +550,60 @@ static DmgArgs<R> make_args(pff_mesh* m, const pff_state* s)
     DmgArgs<R> a{};
     a.meta = m->d_meta; a.lconn = (const ushort4*)m->d_lconn; a.ga = m->d_ga; a.gb = m->d_gb;
     a.area = (const R*)m->d_area; a.halo_ids = m->d_halo_ids; a.ell = m->d_ell; a.flags = m->d_flags;
-    a.halo_part = (R*)m->d_halo_part; a.n_slots = m->n_slots;
-    a.EC = hm.chunk_elems; a.max_nloc = hm.max_nloc; a.N = (int)hm.N; a.N_int = (int)hm.N_int; a.N_sh = (int)hm.N_sh;
-    a.C = (int)hm.C; a.nbs = (int)std::max<int64_t>(1, (hm.N_sh + kTPB - 1) / kTPB);
-    a.sh_rowptr = m->d_sh_rowptr; a.sh_slots = m->d_sh_slots;
+    a.halo_part = (R*)m->d_halo_part; a.n_slots = m->n_slots; a.ell_total = m->ell_total;
+    a.EC = hm.chunk_elems;
+    a.N = (int)hm.N; a.Ne = (int)hm.Ne; a.N_int = (int)hm.N_int; a.N_sh = (int)hm.N_sh; a.C = (int)hm.C;
+    a.sh_rowptr = m->d_sh_rowptr; a.halo_dst = m->d_halo_dst;
     a.H = (const R*)s->H; a.x = (R*)s->d;
     a.lb = (R*)m->d_lb; a.r = (R*)m->d_r; a.p = (R*)m->d_p; a.q = (R*)m->d_q; a.dinv = (R*)m->d_dinv;
-    a.mask = m->d_mask; a.part = m->d_part; a.part_n = m->n_part_blocks;
+    a.mask = m->d_mask; a.part = m->d_part; a.part2 = m->d_part2; a.part_n = m->n_part_blocks;
     a.ctrl = m->d_ctrl; a.ticket = m->d_ticket;
     a.mat = make_matc<R>(m->mat);
     return a;
+}
+
+// TMA plan of a damage chunk kernel: which = 0 CG iteration (lb only for the projected variant), 1 plain
+// mat-vec (trial vector only), 2 setup (x only).  Kinds: 0 elements, 1 interior nodes, 2 gather table.
+template <typename R>
+static void set_plan(pff_mesh* m, DmgArgs<R>& a, int which, bool proj)
+{
+    const StageLayout& L = which == 2 ? m->lay_su : m->lay_mv;
+    a.lay = L;
+    StagePlan& P = a.plan;
+    P.n = 0;
+    const uint16_t lr = sizeof(R) == 8 ? 3 : 2;
+    auto add = [&](const void* src, uint32_t off, uint16_t l, uint16_t kind) { P.d[P.n++] = StageDesc{src, off, l, kind}; };
+    add(m->d_lconn, L.lconn, 3, 0);
+    if (sizeof(R) == 8) { add(m->d_ga, L.geo, 4, 0); add(m->d_gb, L.geo + 16u * (uint32_t)m->hm.chunk_elems, 4, 0); }
+    else add(m->d_ga, L.geo, 4, 0);
+    add(m->d_area, L.area, lr, 0);
+    add(a.H, L.H, lr, 0);
+    add(m->d_ell, L.ell, 1, 2);
+    if (which == 0) {
+        add(a.x, L.node[0], lr, 1); add(a.r, L.node[1], lr, 1); add(a.p, L.node[2], lr, 1); add(a.q, L.node[3], lr, 1);
+        add(a.dinv, L.node[4], lr, 1);
+        if (proj) add(a.lb, L.node[5], lr, 1);
+        add(a.mask, L.flags, 0, 1);
+    } else if (which == 1) {
+        add(a.p_in, L.node[2], lr, 1);
+    } else {
+        add(a.x, L.node[0], lr, 1);
+    }
+}
+
+static unsigned shared_grid(const HostMesh& hm)
+{
+    return (unsigned)std::min<int64_t>(kMaxSharedBlocks, std::max<int64_t>(1, (hm.N_sh + kTPB - 1) / kTPB));
 }
 
 static pff_status ensure_workspace(pff_mesh* m)
 {
     if (m->d_ctrl) return PFF_OK;
     const HostMesh& hm = m->hm;
-    const int64_t nbs = std::max<int64_t>(1, (hm.N_sh + kTPB - 1) / kTPB), nbv = (hm.N + kTPB - 1) / kTPB;
-    m->n_part_blocks = std::max<int64_t>(hm.C + nbs, nbv);
+    m->n_part_blocks = hm.C;
     pff_status st;
-    if ((st = cuda_check(cudaMalloc((void**)&m->d_part, sizeof(double) * kPartStride * m->n_part_blocks), "damage: partials")) != PFF_OK) return st;
+    if ((st = cuda_check(cudaMalloc((void**)&m->d_part, sizeof(double) * kCh * m->n_part_blocks), "damage: partials")) != PFF_OK) return st;
+    if ((st = cuda_check(cudaMalloc((void**)&m->d_part2, sizeof(double) * kCh * kMaxSharedBlocks), "damage: partials 2")) != PFF_OK) return st;
     if ((st = cuda_check(cudaMalloc((void**)&m->d_ctrl, sizeof(DamageCtrl)), "damage: ctrl")) != PFF_OK) return st;
     if ((st = cuda_check(cudaMalloc((void**)&m->d_ticket, sizeof(unsigned int)), "damage: ticket")) != PFF_OK) return st;
     if ((st = cuda_check(cudaMemset(m->d_ticket, 0, sizeof(unsigned int)), "damage: ticket")) != PFF_OK) return st;
@@ -445,37 +628,39 @@ static pff_status damage_solve_t(pff_mesh* m, pff_state* s, double rel_tol, int 
     pff_status st = ensure_workspace(m);
     if (st != PFF_OK) return st;
     const HostMesh& hm = m->hm;
-    DmgArgs<R> a = make_args<R>(m, s);
+    DmgArgs<R> a = make_args<R>(m, s), asu = a;
+    set_plan<R>(m, a, 0, PROJ);
+    set_plan<R>(m, asu, 2, PROJ);
+    const int smem_mv = (int)m->lay_mv.total, smem_su = (int)m->lay_su.total;
     cudaStream_t cs = m->stream;
-    const int smem_mv = int((size_t(hm.max_nloc) + size_t(3) * hm.chunk_elems) * sizeof(R));
-    const int smem_su = int((size_t(hm.max_nloc) + size_t(7) * hm.chunk_elems) * sizeof(R));
-    static int g_mv = 48 * 1024, g_su = 48 * 1024;
-    if ((st = set_smem(dmg_matvec_chunk<R, DM_CG, PROJ>, smem_mv, g_mv)) != PFF_OK) return st;
+    static int g_mv = 0, g_su = 0;  // static + dynamic shared memory may exceed 48 KB: always opt in
+    if ((st = set_smem(dmg_iter_chunk<R, DM_CG, PROJ>, smem_mv, g_mv)) != PFF_OK) return st;
     if ((st = set_smem(dmg_setup_chunk<R, false>, smem_su, g_su)) != PFF_OK) return st;
     DamageCtrl* h = m->h_ctrl;  // [0]: upload image, [1]: download image
     std::memset(&h[0], 0, sizeof(DamageCtrl));
-    h[0].tol = rel_tol; h[0].max_iter = max_iter; h[0].first = 1; h[0].status = PFF_ENOCONV;
+    h[0].tol = rel_tol; h[0].max_iter = max_iter; h[0].first = 1; h[0].restart = 1; h[0].status = PFF_ENOCONV;
     if ((st = cuda_check(cudaMemcpyAsync(m->d_ctrl, &h[0], sizeof(DamageCtrl), cudaMemcpyHostToDevice, cs), "damage: ctrl upload")) != PFF_OK) return st;
-    const unsigned nbv = (unsigned)((hm.N + kTPB - 1) / kTPB);
-    PFF_LAUNCH(m, PFF_K_DAMAGE_SETUP, (dmg_setup_chunk<R, false><<<(unsigned)hm.C, kTPB, smem_su, cs>>>(a)));
-    PFF_LAUNCH(m, PFF_K_DAMAGE_SETUP, (dmg_setup_shared<R, false><<<(unsigned)a.nbs, kTPB, 0, cs>>>(a)));
-    PFF_LAUNCH(m, PFF_K_CG_VECTOR, (dmg_vector<R, PROJ><<<nbv, kTPB, 0, cs>>>(a)));
-    int launched = 0, batch = 2;
+    const unsigned gs = shared_grid(hm), gn = (unsigned)std::min<int64_t>(4 * 148, (hm.N + kTPB - 1) / kTPB);
+    PFF_LAUNCH(m, PFF_K_DAMAGE_SETUP, (dmg_setup_chunk<R, false><<<(unsigned)hm.C, kTPB, smem_su, cs>>>(asu)));
+    PFF_LAUNCH(m, PFF_K_DAMAGE_SETUP, (dmg_setup_shared<R, false><<<gs, kTPB, 0, cs>>>(asu)));
+    // the host polls the control block; the first batch is sized from the previous solve (warm start, L468)
+    int launched = 0, batch = std::max(2, std::min(m->last_cg_iters > 0 ? m->last_cg_iters : 4, 64));
     for (;;) {
+        batch = std::min(batch, max_iter + 1 - launched);
         for (int k = 0; k < batch; ++k) {
-            PFF_LAUNCH(m, PFF_K_MATVEC_CHUNK, (dmg_matvec_chunk<R, DM_CG, PROJ><<<(unsigned)hm.C, kTPB, smem_mv, cs>>>(a)));
-            PFF_LAUNCH(m, PFF_K_MATVEC_SHARED, (dmg_matvec_shared<R, DM_CG, PROJ><<<(unsigned)a.nbs, kTPB, 0, cs>>>(a)));
-            PFF_LAUNCH(m, PFF_K_CG_VECTOR, (dmg_vector<R, PROJ><<<nbv, kTPB, 0, cs>>>(a)));
+            PFF_LAUNCH(m, PFF_K_MATVEC_CHUNK, (dmg_iter_chunk<R, DM_CG, PROJ><<<(unsigned)hm.C, kTPB, smem_mv, cs>>>(a)));
+            PFF_LAUNCH(m, PFF_K_MATVEC_SHARED, (dmg_iter_shared<R, DM_CG, PROJ><<<gs, kTPB, 0, cs>>>(a)));
         }
         launched += batch;
         if ((st = cuda_check(cudaMemcpyAsync(&h[1], m->d_ctrl, sizeof(DamageCtrl), cudaMemcpyDeviceToHost, cs), "damage: ctrl download")) != PFF_OK) return st;
         if ((st = cuda_check(cudaStreamSynchronize(cs), "damage: sync")) != PFF_OK) return st;
         if (h[1].done || launched >= max_iter + 1) break;
-        batch = std::min(8, batch * 2);
+        batch = 4;
     }
-    PFF_LAUNCH(m, PFF_K_DAMAGE_SETUP, (dmg_finalize<R><<<nbv, kTPB, 0, cs>>>((int)hm.N, a.x, a.lb, a.flags)));
+    PFF_LAUNCH(m, PFF_K_DAMAGE_SETUP, (dmg_finalize<R, PROJ><<<gn, kTPB, 0, cs>>>(a)));
     if ((st = cuda_check(cudaGetLastError(), "damage solve launch")) != PFF_OK) return st;
     if ((st = cuda_check(cudaStreamSynchronize(cs), "damage: final sync")) != PFF_OK) return st;
+    m->last_cg_iters = h[1].iters;
     if (iters) *iters = h[1].iters;
     if (relres) *relres = h[1].relres;
     if (!h[1].done || h[1].status == PFF_ENOCONV) {
@@ -502,14 +687,15 @@ static pff_status damage_matvec_t(pff_mesh* m, const pff_state* s, const void* p
     if (st != PFF_OK) return st;
     DmgArgs<R> a = make_args<R>(m, s);
     a.p_in = (const R*)p; a.q_out = (R*)q;
-    const int smem_mv = int((size_t(m->hm.max_nloc) + size_t(3) * m->hm.chunk_elems) * sizeof(R));
-    static int g_mv = 48 * 1024;
-    if ((st = set_smem(dmg_matvec_chunk<R, DM_PLAIN, false>, smem_mv, g_mv)) != PFF_OK) return st;
+    set_plan<R>(m, a, 1, false);
+    const int smem_mv = (int)m->lay_mv.total;
+    static int g_mv = 0;
+    if ((st = set_smem(dmg_iter_chunk<R, DM_PLAIN, false>, smem_mv, g_mv)) != PFF_OK) return st;
     if (m->only_kernel != 3) {
-        PFF_LAUNCH(m, PFF_K_MATVEC_CHUNK, (dmg_matvec_chunk<R, DM_PLAIN, false><<<(unsigned)m->hm.C, kTPB, smem_mv, m->stream>>>(a)));
+        PFF_LAUNCH(m, PFF_K_MATVEC_CHUNK, (dmg_iter_chunk<R, DM_PLAIN, false><<<(unsigned)m->hm.C, kTPB, smem_mv, m->stream>>>(a)));
     }
     if (m->only_kernel != 2) {
-        PFF_LAUNCH(m, PFF_K_MATVEC_SHARED, (dmg_matvec_shared<R, DM_PLAIN, false><<<(unsigned)a.nbs, kTPB, 0, m->stream>>>(a)));
+        PFF_LAUNCH(m, PFF_K_MATVEC_SHARED, (dmg_iter_shared<R, DM_PLAIN, false><<<shared_grid(m->hm), kTPB, 0, m->stream>>>(a)));
     }
     return cuda_check(cudaGetLastError(), "damage matvec launch");
 }
@@ -526,11 +712,12 @@ static pff_status damage_rhs_diag_t(pff_mesh* m, const pff_state* s, void* b, vo
     if (st != PFF_OK) return st;
     DmgArgs<R> a = make_args<R>(m, s);
     a.b_out = (R*)b; a.D_out = (R*)D;
-    const int smem_su = int((size_t(m->hm.max_nloc) + size_t(7) * m->hm.chunk_elems) * sizeof(R));
-    static int g_su = 48 * 1024;
+    set_plan<R>(m, a, 2, false);
+    const int smem_su = (int)m->lay_su.total;
+    static int g_su = 0;
     if ((st = set_smem(dmg_setup_chunk<R, true>, smem_su, g_su)) != PFF_OK) return st;
     PFF_LAUNCH(m, PFF_K_DAMAGE_SETUP, (dmg_setup_chunk<R, true><<<(unsigned)m->hm.C, kTPB, smem_su, m->stream>>>(a)));
-    PFF_LAUNCH(m, PFF_K_DAMAGE_SETUP, (dmg_setup_shared<R, true><<<(unsigned)a.nbs, kTPB, 0, m->stream>>>(a)));
+    PFF_LAUNCH(m, PFF_K_DAMAGE_SETUP, (dmg_setup_shared<R, true><<<shared_grid(m->hm), kTPB, 0, m->stream>>>(a)));
     return cuda_check(cudaGetLastError(), "damage rhs/diag launch");
 }
 

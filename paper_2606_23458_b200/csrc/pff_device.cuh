@@ -5,6 +5,7 @@
 #include <cstdint>
 
 #include "pff_internal.h"
+#include "pff_tma.cuh"
 
 namespace pff {
 
@@ -47,6 +48,8 @@ template <typename R> __device__ __forceinline__ R rmax(R a, R b) { return a > b
 template <typename R> __device__ __forceinline__ R rmin(R a, R b) { return a < b ? a : b; }
 __device__ __forceinline__ double rsqrt_(double x) { return sqrt(x); }
 __device__ __forceinline__ float rsqrt_(float x) { return sqrtf(x); }
+__device__ __forceinline__ double rrsqrt_(double x) { return rsqrt(x); }
+__device__ __forceinline__ float rrsqrt_(float x) { return rsqrtf(x); }
 __device__ __forceinline__ double rfma(double a, double b, double c) { return fma(a, b, c); }
 __device__ __forceinline__ float rfma(float a, float b, float c) { return fmaf(a, b, c); }
 
@@ -63,13 +66,15 @@ __device__ __forceinline__ void elem_response(const MatC<R>& m, R exx, R eyy, R 
     const R zero = R(0), half = R(0.5), two = R(2);
     if (SPLIT == PFF_SPLIT_SPECTRAL) {
         const R tr = exx + eyy, mean = half * tr, dd = half * (exx - eyy);
-        const R rad = rsqrt_(dd * dd + exy * exy);
+        // one reciprocal square root gives both the radius of Mohr's circle and its inverse (0 when eps = m I, R7)
+        const R rad2 = dd * dd + exy * exy;
+        const R inv = rad2 > zero ? rrsqrt_(rad2) : zero;
+        const R rad = rad2 * inv;
         const R e1 = mean + rad, e2 = mean - rad;
         const R e1p = rmax(e1, zero), e2p = rmax(e2, zero), e1m = rmin(e1, zero), e2m = rmin(e2, zero);
         const R trp = rmax(tr, zero), trm = rmin(tr, zero);
         psi_p = half * m.lam * trp * trp + m.mu * (e1p * e1p + e2p * e2p);
         psi_m = half * m.lam * trm * trm + m.mu * (e1m * e1m + e2m * e2m);
-        const R inv = rad > zero ? R(1) / rad : zero;
         const R qp = (e1p - e2p) * inv, qm = (e1m - e2m) * inv;
         const R hp = m.lam * trp + m.mu * (e1p + e2p), hm = m.lam * trm + m.mu * (e1m + e2m);
         const R dev = m.mu * (g * qp + qm);  // multiplies (eps - mean I)
@@ -101,9 +106,12 @@ __device__ __forceinline__ void elem_response(const MatC<R>& m, R exx, R eyy, R 
 }
 
 // Compact P1 geometry: grad phi1 = (b1, c1), grad phi2 = (b2, c2), grad phi3 = -(grad phi1 + grad phi2)
-// (rows of Eq. 9 sum to zero), read as 128-bit loads.
+// (rows of Eq. 9 sum to zero), read as 128-bit loads.  In the chunk kernels the geometry is staged in shared
+// memory by TMA: fp64 as double2 ga[EC] followed by double2 gb[EC], fp32 as float4[EC].
 template <typename R> struct Geo;
 template <> struct Geo<double> {
+    typedef double2 Pair;  // (x, y) force pair of one element corner
+    static constexpr int kArrays = 2;  // global streams: ga, gb (16 B per element each)
     static __device__ __forceinline__ void load(const void* ga, const void* gb, int e, double& b1, double& c1,
                                                 double& b2, double& c2)
     {
@@ -111,14 +119,31 @@ template <> struct Geo<double> {
         const double2 q = __ldg(reinterpret_cast<const double2*>(gb) + e);
         b1 = p.x; c1 = p.y; b2 = q.x; c2 = q.y;
     }
+    static __device__ __forceinline__ void load_smem(const unsigned char* geo, int e, int EC, double& b1, double& c1,
+                                                     double& b2, double& c2)
+    {
+        const double2* g = reinterpret_cast<const double2*>(geo);
+        const double2 p = g[e], q = g[EC + e];
+        b1 = p.x; c1 = p.y; b2 = q.x; c2 = q.y;
+    }
+    static __device__ __forceinline__ double2 pair(double x, double y) { return make_double2(x, y); }
 };
 template <> struct Geo<float> {
+    typedef float2 Pair;
+    static constexpr int kArrays = 1;  // one float4 stream
     static __device__ __forceinline__ void load(const void* ga, const void*, int e, float& b1, float& c1,
                                                 float& b2, float& c2)
     {
         const float4 p = __ldg(reinterpret_cast<const float4*>(ga) + e);
         b1 = p.x; c1 = p.y; b2 = p.z; c2 = p.w;
     }
+    static __device__ __forceinline__ void load_smem(const unsigned char* geo, int e, int, float& b1, float& c1, float& b2,
+                                                     float& c2)
+    {
+        const float4 p = reinterpret_cast<const float4*>(geo)[e];
+        b1 = p.x; c1 = p.y; b2 = p.z; c2 = p.w;
+    }
+    static __device__ __forceinline__ float2 pair(float x, float y) { return make_float2(x, y); }
 };
 
 // Deterministic block sum in fp64 (fixed shuffle tree, fixed warp order); result valid in thread 0.

@@ -53,17 +53,18 @@ static pff_status run_host_t(pff_mesh* m, pff_host_state* hs, const double* dir_
     cudaStream_t cs = m->stream;
     pff_status st;
     const size_t stage_doubles = size_t(9) * N + Ne;
+    const int64_t Np = (N + 3) / 4 * 4, Nep = (Ne + 3) / 4 * 4;  // every device state array starts 16-byte aligned
     if (!m->d_stage) {
         if ((st = cuda_check(cudaMalloc(&m->d_stage, stage_doubles * sizeof(double)), "run_host: staging")) != PFF_OK) return st;
-        if ((st = cuda_check(cudaMalloc(&m->d_hstate, (size_t(9) * N + Ne) * sizeof(R) + 2 * size_t(std::max<int64_t>(m->n_dir, 1)) * sizeof(R)), "run_host: state")) != PFF_OK) return st;
+        if ((st = cuda_check(cudaMalloc(&m->d_hstate, (size_t(9) * Np + Nep) * sizeof(R) + 2 * size_t(std::max<int64_t>(m->n_dir, 1)) * sizeof(R)), "run_host: state")) != PFF_OK) return st;
     }
     double* sg = (double*)m->d_stage;
     HostIO<R> io{};
     io.u = sg; io.v = sg + 2 * N; io.a = sg + 4 * N; io.fext = sg + 6 * N; io.d = sg + 8 * N; io.H = sg + 9 * N;
     R* ds = (R*)m->d_hstate;
-    io.ux = ds; io.uy = ds + N; io.vx = ds + 2 * N; io.vy = ds + 3 * N; io.ax = ds + 4 * N; io.ay = ds + 5 * N;
-    io.dd = ds + 6 * N; io.fex = ds + 7 * N; io.fey = ds + 8 * N; io.HH = ds + 9 * N;
-    R* d_du = ds + 9 * N + Ne;
+    io.ux = ds; io.uy = ds + Np; io.vx = ds + 2 * Np; io.vy = ds + 3 * Np; io.ax = ds + 4 * Np; io.ay = ds + 5 * Np;
+    io.dd = ds + 6 * Np; io.fex = ds + 7 * Np; io.fey = ds + 8 * Np; io.HH = ds + 9 * Np;
+    R* d_du = ds + 9 * Np + Nep;
     R* d_dv = d_du + std::max<int64_t>(m->n_dir, 1);
     io.node_old_of_new = m->d_node_old_of_new; io.elem_old_of_new = m->d_elem_old_of_new;
     io.N = (int)N; io.Ne = (int)Ne;

@@ -17,7 +17,8 @@ struct pff_mesh {
     int device = 0;
     size_t rb = 8;  // bytes per real
     double dt_crit = 0.0;
-    int smem_step = 0, smem_dmg = 0;
+    pff::StageLayout lay_step{}, lay_mv{}, lay_su{};  // shared-memory stages of the step / CG iteration / setup chunk kernels
+    int64_t ell_total = 0;                       // entries of d_ell (padded)
     int64_t n_launches = 0;  // kernels launched so far (pff_mesh_counters)
     int only_kernel = -1;    // profiling hook: restrict multi-kernel entry points to one kernel (pff_time_kernel)
     // per-kernel-class CUDA-event timing (pff_profile_enable / pff_profile_read)
@@ -30,7 +31,7 @@ struct pff_mesh {
     void* d_lconn = nullptr;  // ushort4[Ne]
     void* d_conn = nullptr;   // int4[Ne]
     void *d_ga = nullptr, *d_gb = nullptr, *d_area = nullptr, *d_minv = nullptr, *d_mass = nullptr;
-    int32_t *d_halo_ids = nullptr, *d_sh_rowptr = nullptr, *d_sh_slots = nullptr;
+    int32_t *d_halo_ids = nullptr, *d_sh_rowptr = nullptr, *d_halo_dst = nullptr;
     uint16_t* d_ell = nullptr;
     uint8_t* d_flags = nullptr;  // bit0: u_x Dirichlet, bit1: u_y Dirichlet, bit2: damage Dirichlet
     void* d_halo_part = nullptr;  // [3][n_slots] reals: per (chunk, interface node) partial sums
@@ -44,8 +45,10 @@ struct pff_mesh {
 
     // damage solve workspaces (reals [N] unless noted)
     void *d_lb = nullptr, *d_r = nullptr, *d_p = nullptr, *d_q = nullptr, *d_dinv = nullptr;
-    uint8_t* d_mask = nullptr;   // [2][N] free-set masks (ping-pong)
-    double* d_part = nullptr;    // block partials [kPartStride * n_part_blocks]
+    uint8_t* d_mask = nullptr;   // [N] bit0: in the free set, bit1: damage-Dirichlet
+    double* d_part = nullptr;    // chunk-kernel block partials [channels][n_part_blocks]
+    double* d_part2 = nullptr;   // interface-kernel block partials
+    int last_cg_iters = 0;       // iterations of the previous solve (sizes the first launch batch)
     int64_t n_part_blocks = 0;
     DamageCtrl* d_ctrl = nullptr;
     DamageCtrl* h_ctrl = nullptr;  // pinned

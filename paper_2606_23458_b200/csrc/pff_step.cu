@@ -12,6 +12,7 @@
 //   dirichlet_kernel    writes u_bar, v_bar into the Dirichlet dofs before the step (Eq. 5, R8).
 #include "pff_device.cuh"
 #include "pff_mesh.h"
+#include "pff_tma.cuh"
 
 namespace pff {
 
@@ -30,8 +31,11 @@ struct StepArgs {
     const R* minv;
     R* halo_part;  // [2][n_slots]
     int64_t n_slots;
-    int EC, max_nloc, N, Ne, N_int, N_sh;
-    const int32_t *sh_rowptr, *sh_slots;
+    int EC, N, Ne, N_int, N_sh;
+    int64_t ell_total;
+    const int32_t *sh_rowptr, *halo_dst;
+    StageLayout lay;
+    StagePlan plan;
     R *ux, *uy, *vx, *vy, *ax, *ay;
     const R* d;
     R* H;
@@ -95,61 +99,119 @@ __device__ __forceinline__ void element_forces(const MatC<R>& mat, R b1, R c1, R
     f[4] = -(f[0] + f[2]); f[5] = -(f[1] + f[3]);
 }
 
+// One CTA per chunk.  The stage (StageLayout kind 0, pff_internal.h) is filled by ONE burst of bulk-asynchronous
+// copies issued by the first warp (one lane per array); the halo gathers overlap with it.
 template <typename R, int SPLIT, int MODE>
 __global__ void __launch_bounds__(kTPB) step_chunk_kernel(const StepArgs<R> a)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    R* s_ux = reinterpret_cast<R*>(smem_raw);
-    R* s_uy = s_ux + a.max_nloc;
-    R* s_d = s_uy + a.max_nloc;
-    R* s_f = s_d + a.max_nloc;  // [6][EC]
-    const ChunkMeta cm = a.meta[blockIdx.x];
-    const int nloc = cm.n_int + cm.n_halo;
-    const int tid = threadIdx.x;
+    extern __shared__ __align__(128) unsigned char smem[];
+    typedef typename Geo<R>::Pair Pair;
+    constexpr int A = 16 / sizeof(R);
+    const StageLayout& L = a.lay;
+    const ushort4* s_lconn = reinterpret_cast<const ushort4*>(smem + L.lconn);
+    const unsigned char* s_geo = smem + L.geo;
+    Pair* s_slot = reinterpret_cast<Pair*>(smem + L.slots);
+    const R* s_area = reinterpret_cast<const R*>(smem + L.area);
+    const R* s_H = reinterpret_cast<const R*>(smem + L.H);
+    R* s_ux = reinterpret_cast<R*>(smem + L.node[0]);
+    R* s_uy = reinterpret_cast<R*>(smem + L.node[1]);
+    R* s_d = reinterpret_cast<R*>(smem + L.node[2]);
+    const R* s_vx = reinterpret_cast<const R*>(smem + L.node[3]);
+    R* s_fwd = reinterpret_cast<R*>(smem + L.node[3]);  // halo part of the v_x array: forwards each halo node's partial slot
+    const R* s_vy = reinterpret_cast<const R*>(smem + L.node[4]);
+    const R* s_ax = reinterpret_cast<const R*>(smem + L.node[5]);
+    const R* s_ay = reinterpret_cast<const R*>(smem + L.node[6]);
+    const R* s_fex = reinterpret_cast<const R*>(smem + L.node[7]);
+    const R* s_fey = reinterpret_cast<const R*>(smem + L.node[8]);
+    const R* s_minv = reinterpret_cast<const R*>(smem + L.node[9]);
+    const uint8_t* s_flags = smem + L.flags;
+    const uint16_t* s_ell = reinterpret_cast<const uint16_t*>(smem + L.ell);
+    uint64_t* bar = reinterpret_cast<uint64_t*>(smem + L.bar);
 
-    for (int i = tid; i < nloc; i += kTPB) {
-        const int gid = i < cm.n_int ? cm.node_start + i : a.halo_ids[cm.halo_off + i - cm.n_int];
+    // ---- phase 0: stream every contiguous array of the chunk into the stage (TMA).  The element arrays go first:
+    // their range follows from blockIdx, so they are in flight while the chunk meta is still being fetched.
+    const int tid = threadIdx.x;
+    const ChunkMeta cm = a.meta[blockIdx.x];
+    if (tid == 0) { mbar_init(bar, 2); s_slot[3 * a.EC] = Geo<R>::pair(R(0), R(0)); }
+    __syncthreads();
+    if (tid < 32)
+        stage_issue_plan(a.plan, smem, bar, tid, true, blockIdx.x * a.EC, min(a.EC, a.Ne - blockIdx.x * a.EC), a.Ne, 0, 0, a.N,
+                         0, 0, 0);
+    const int nloc = cm.n_int + cm.n_halo;
+    const int shift = cm.node_start & (A - 1), hb = (shift + cm.n_int + A - 1) & ~(A - 1), fshift = cm.node_start & 15;
+    if (tid < 32)
+        stage_issue_plan(a.plan, smem, bar, tid, false, 0, 0, a.Ne, cm.node_start, cm.n_int, a.N, cm.ell_off, cm.ell_w * nloc,
+                         (int)a.ell_total);
+    // halo (interface) nodes: indexed gathers, predictor (Eq. 16), straight into their stage slots
+    for (int j = tid; j < cm.n_halo; j += kTPB) {
+        const int gid = __ldg(a.halo_ids + cm.halo_off + j);
         R px, py;
         predict<R, MODE>(a, gid, px, py);
-        s_ux[i] = px; s_uy[i] = py; s_d[i] = a.d[gid];
+        s_ux[hb + j] = px; s_uy[hb + j] = py; s_d[hb + j] = a.d[gid];
+        reinterpret_cast<int*>(s_fwd + hb + j)[0] = __ldg(a.halo_dst + cm.halo_off + j);  // partial slot, used in phase 3
     }
-    __syncthreads();
+    mbar_wait(bar, 0);
 
-    for (int e = tid; e < cm.n_elem; e += kTPB) {
-        const int ge = cm.elem_start + e;
-        const ushort4 c = __ldg(a.lconn + ge);
-        R b1, c1, b2, c2;
-        Geo<R>::load(a.ga, a.gb, ge, b1, c1, b2, c2);
-        const R A = __ldg(a.area + ge);
-        R psi_p, f[6];
-        element_forces<R, SPLIT>(a.mat, b1, c1, b2, c2, A, s_ux[c.x], s_uy[c.x], s_ux[c.y], s_uy[c.y], s_ux[c.z],
-                                 s_uy[c.z], s_d[c.x] + s_d[c.y] + s_d[c.z], psi_p, f);
-#pragma unroll
-        for (int k = 0; k < 6; ++k) s_f[k * a.EC + e] = f[k];
-        if (MODE == MODE_STEP) {
-            const R h = a.H[ge];
-            if (psi_p > h) a.H[ge] = psi_p;  // H <- max(H, psi+)  (L98, L114)
-        } else if (MODE == MODE_FORCE) {
-            if (a.psi_out) a.psi_out[ge] = psi_p;
+    // ---- phase 1: predictor of the interior nodes, in place (Eq. 16; Dirichlet dofs hold u_bar already)
+    if (MODE == MODE_STEP) {
+        for (int i = tid; i < cm.n_int; i += kTPB) {
+            const int s = shift + i;
+            const uint8_t fl = s_flags[fshift + i];
+            const R ux = s_ux[s], uy = s_uy[s];
+            const R px = rfma(a.hdt2, s_ax[s], rfma(a.dt, s_vx[s], ux));
+            const R py = rfma(a.hdt2, s_ay[s], rfma(a.dt, s_vy[s], uy));
+            s_ux[s] = (fl & 1) ? ux : px;
+            s_uy[s] = (fl & 2) ? uy : py;
         }
     }
     __syncthreads();
 
-    const uint16_t* ell = a.ell + cm.ell_off;
+    // ---- phase 2: fused element pass; nodal force pairs go to the slots corner * EC + e
+    for (int e = tid; e < cm.n_elem; e += kTPB) {
+        const ushort4 c = s_lconn[e];
+        R b1, c1, b2, c2;
+        Geo<R>::load_smem(s_geo, e, a.EC, b1, c1, b2, c2);
+        R psi_p, f[6];
+        element_forces<R, SPLIT>(a.mat, b1, c1, b2, c2, s_area[e], s_ux[c.x], s_uy[c.x], s_ux[c.y], s_uy[c.y], s_ux[c.z],
+                                 s_uy[c.z], s_d[c.x] + s_d[c.y] + s_d[c.z], psi_p, f);
+        s_slot[e] = Geo<R>::pair(f[0], f[1]);
+        s_slot[a.EC + e] = Geo<R>::pair(f[2], f[3]);
+        s_slot[2 * a.EC + e] = Geo<R>::pair(f[4], f[5]);
+        if (MODE == MODE_STEP) {
+            if (psi_p > s_H[e]) a.H[cm.elem_start + e] = psi_p;  // H <- max(H, psi+)  (L98, L114)
+        } else if (MODE == MODE_FORCE) {
+            if (a.psi_out) a.psi_out[cm.elem_start + e] = psi_p;
+        }
+    }
+    __syncthreads();
+
+    // ---- phase 3: ordered gather of each node's incident force pairs, then Eq. 17-18 for interior nodes
     for (int i = tid; i < nloc; i += kTPB) {
         R fx = R(0), fy = R(0);
+        const uint16_t* row = s_ell + i;
+#pragma unroll 4
         for (int k = 0; k < cm.ell_w; ++k) {
-            const unsigned ent = ell[k * nloc + i];
-            if (ent != 0xFFFFu) {
-                const int e = ent >> 2, cnr = ent & 3;
-                fx += s_f[(2 * cnr) * a.EC + e];
-                fy += s_f[(2 * cnr + 1) * a.EC + e];
-            }
+            const Pair v = s_slot[row[k * nloc]];
+            fx += v.x; fy += v.y;
         }
         if (i < cm.n_int) {
-            finish_node<R, MODE>(a, cm.node_start + i, s_ux[i], s_uy[i], fx, fy);
+            const int gid = cm.node_start + i, s = shift + i;
+            if (MODE == MODE_FORCE) { a.fx_out[gid] = fx; a.fy_out[gid] = fy; continue; }
+            const uint8_t fl = s_flags[fshift + i];
+            const R minv = s_minv[s];
+            R axn = (a.S * s_fex[s] - fx) * minv;
+            R ayn = (a.S * s_fey[s] - fy) * minv;
+            if (fl & 1) axn = R(0);
+            if (fl & 2) ayn = R(0);
+            if (MODE == MODE_STEP) {
+                const R vxo = s_vx[s], vyo = s_vy[s];
+                a.ux[gid] = s_ux[s]; a.uy[gid] = s_uy[s];
+                a.vx[gid] = (fl & 1) ? vxo : rfma(a.hdt, s_ax[s] + axn, vxo);
+                a.vy[gid] = (fl & 2) ? vyo : rfma(a.hdt, s_ay[s] + ayn, vyo);
+            }
+            a.ax[gid] = axn; a.ay[gid] = ayn;
         } else {
-            const int64_t slot = cm.halo_off + i - cm.n_int;
+            const int slot = reinterpret_cast<const int*>(s_fwd + hb + i - cm.n_int)[0];
             a.halo_part[slot] = fx;
             a.halo_part[a.n_slots + slot] = fy;
         }
@@ -163,10 +225,9 @@ __global__ void __launch_bounds__(kTPB) step_shared_kernel(const StepArgs<R> a)
     if (s >= a.N_sh) return;
     const int gid = a.N_int + s;
     R fx = R(0), fy = R(0);
-    for (int k = a.sh_rowptr[s]; k < a.sh_rowptr[s + 1]; ++k) {
-        const int slot = a.sh_slots[k];
-        fx += a.halo_part[slot];
-        fy += a.halo_part[a.n_slots + slot];
+    for (int k = a.sh_rowptr[s]; k < a.sh_rowptr[s + 1]; ++k) {  // partials of one node are contiguous, ascending chunk
+        fx += a.halo_part[k];
+        fy += a.halo_part[a.n_slots + k];
     }
     R px, py;
     predict<R, MODE>(a, gid, px, py);
@@ -239,14 +300,14 @@ static pff_status launch_step_t(pff_mesh* m, const StepArgs<R>& a)
         }
     } else {
         auto kern = step_chunk_kernel<R, SPLIT, MODE>;
-        static int granted = 48 * 1024;  // per instantiation high-water mark of the dynamic smem opt-in
-        if (m->smem_step > granted) {
-            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, m->smem_step);
+        static int granted = 0;  // per instantiation high-water mark of the dynamic smem opt-in
+        if ((int)m->lay_step.total > granted) {
+            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)m->lay_step.total);
             if (e != cudaSuccess) return cuda_check(e, "cudaFuncSetAttribute(step_chunk_kernel)");
-            granted = m->smem_step;
+            granted = (int)m->lay_step.total;
         }
         if (m->only_kernel != 1) {
-            PFF_LAUNCH(m, PFF_K_STEP_CHUNK, (kern<<<(unsigned)hm.C, kTPB, m->smem_step, m->stream>>>(a)));
+            PFF_LAUNCH(m, PFF_K_STEP_CHUNK, (kern<<<(unsigned)hm.C, kTPB, (int)m->lay_step.total, m->stream>>>(a)));
         }
         if (hm.N_sh > 0 && m->only_kernel != 0) {
             PFF_LAUNCH(m, PFF_K_STEP_SHARED, (step_shared_kernel<R, MODE><<<(unsigned)((hm.N_sh + kTPB - 1) / kTPB), kTPB, 0, m->stream>>>(a)));
@@ -277,9 +338,9 @@ static pff_status launch_step_r(pff_mesh* m, pff_state* s, const pff_bc* bc, dou
     a.ga = m->d_ga; a.gb = m->d_gb; a.area = (const R*)m->d_area;
     a.halo_ids = m->d_halo_ids; a.ell = m->d_ell; a.flags = m->d_flags; a.minv = (const R*)m->d_minv;
     a.halo_part = (R*)m->d_halo_part; a.n_slots = m->n_slots;
-    a.EC = hm.chunk_elems; a.max_nloc = hm.max_nloc; a.N = (int)hm.N; a.Ne = (int)hm.Ne;
+    a.EC = hm.chunk_elems; a.ell_total = m->ell_total; a.N = (int)hm.N; a.Ne = (int)hm.Ne;
     a.N_int = (int)hm.N_int; a.N_sh = (int)hm.N_sh;
-    a.sh_rowptr = m->d_sh_rowptr; a.sh_slots = m->d_sh_slots;
+    a.sh_rowptr = m->d_sh_rowptr; a.halo_dst = m->d_halo_dst;
     a.ux = (R*)s->ux; a.uy = (R*)s->uy; a.vx = (R*)s->vx; a.vy = (R*)s->vy; a.ax = (R*)s->ax; a.ay = (R*)s->ay;
     a.d = (const R*)s->d; a.H = (R*)s->H; a.fex = (const R*)s->fext_x; a.fey = (const R*)s->fext_y;
     a.fx_out = (R*)fx; a.fy_out = (R*)fy; a.psi_out = (R*)psi;
@@ -287,6 +348,29 @@ static pff_status launch_step_r(pff_mesh* m, pff_state* s, const pff_bc* bc, dou
     a.dt = R(dt); a.hdt = R(0.5 * dt); a.hdt2 = R(0.5 * dt * dt);
     a.S = R(bc ? bc->load_scale : 1.0);
     a.mat = make_matc<R>(m->mat);
+    {   // TMA plan: one descriptor per contiguous array the chosen mode reads (kind 0 elements, 1 nodes, 2 gather table)
+        const StageLayout& L = m->lay_step;
+        a.lay = L;
+        StagePlan& P = a.plan;
+        P.n = 0;
+        const uint16_t lr = sizeof(R) == 8 ? 3 : 2;
+        auto add = [&](const void* src, uint32_t off, uint16_t l, uint16_t kind) { P.d[P.n++] = StageDesc{src, off, l, kind}; };
+        add(m->d_lconn, L.lconn, 3, 0);
+        if (sizeof(R) == 8) { add(m->d_ga, L.geo, 4, 0); add(m->d_gb, L.geo + 16u * (uint32_t)hm.chunk_elems, 4, 0); }
+        else add(m->d_ga, L.geo, 4, 0);
+        add(m->d_area, L.area, lr, 0);
+        if (mode == MODE_STEP) add(s->H, L.H, lr, 0);
+        add(m->d_ell, L.ell, 1, 2);
+        add(s->ux, L.node[0], lr, 1); add(s->uy, L.node[1], lr, 1); add(s->d, L.node[2], lr, 1);
+        if (mode == MODE_STEP) {
+            add(s->vx, L.node[3], lr, 1); add(s->vy, L.node[4], lr, 1);
+            add(s->ax, L.node[5], lr, 1); add(s->ay, L.node[6], lr, 1);
+        }
+        if (mode != MODE_FORCE) {
+            add(s->fext_x, L.node[7], lr, 1); add(s->fext_y, L.node[8], lr, 1); add(m->d_minv, L.node[9], lr, 1);
+            add(m->d_flags, L.flags, 0, 1);
+        }
+    }
     if (mode == MODE_STEP && m->n_dir > 0 && bc && bc->dir_u && bc->dir_v) {
         PFF_LAUNCH(m, PFF_K_OTHER, (dirichlet_kernel<R><<<(unsigned)((m->n_dir + 127) / 128), 128, 0, m->stream>>>(
             (int)m->n_dir, m->d_dir_dof, (const R*)bc->dir_u, (const R*)bc->dir_v, a.ux, a.uy, a.vx, a.vy)));

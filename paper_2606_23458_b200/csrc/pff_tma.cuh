@@ -1,0 +1,99 @@
+// sm_100a bulk-asynchronous copy (TMA, 1-D `cp.async.bulk`, SASS UBLKCP) + mbarrier wrappers, and the
+// chunk-stage helper used by the step and damage kernels: one thread streams every contiguous array of a
+// chunk into shared memory in a single burst, all threads wait on one mbarrier.
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdint>
+
+namespace pff {
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+
+// one arrival + the number of bytes the bulk copies will signal
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
+{
+    const uint32_t addr = smem_u32(bar);
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n"
+            "}\n" : "=r"(done) : "r"(addr), "r"(parity) : "memory");
+    } while (!done);
+}
+
+// global -> shared bulk copy; dst, src 16-byte aligned, bytes a multiple of 16; completion on `bar`
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+// One contiguous array of a chunk stage.  kind selects the index range of the chunk that is copied:
+// 0 = elements [elem_start, +n_elem) of Ne, 1 = interior nodes [node_start, +n_int) of N,
+// 2 = gather-table entries [ell_off, +ell_w * nloc) of ell_total.
+struct StageDesc {
+    const void* src;
+    uint32_t dst_off;      // byte offset inside the stage (16-byte aligned)
+    uint16_t esize_log2;   // log2 of the element size in bytes (0..4)
+    uint16_t kind;
+};
+constexpr int kMaxStageArrays = 20;
+struct StagePlan {
+    StageDesc d[kMaxStageArrays];
+    int n;
+};
+
+// Issued by the first warp of the CTA, one lane per array (uniform code, no divergence): element
+// start + i of the global array lands at byte offset dst_off + ((start % A) + i) * esize, A = 16 / esize.
+// The copy is widened to 16-byte boundaries (the few neighbours fetched with it are never read); whatever
+// would reach past the last full 16-byte group of the array is fetched with plain loads.  Lane 0 then
+// arrives on the mbarrier with the total byte count.
+// elems_pass: true = only the element arrays (kind 0; their range follows from blockIdx alone, so they are issued
+// before the chunk meta has arrived), false = everything else; each pass makes one arrival (mbarrier count 2).
+__device__ __forceinline__ void stage_issue_plan(const StagePlan& plan, unsigned char* stage, uint64_t* bar, int lane,
+                                                 bool elems_pass, int elem_start, int n_elem, int Ne, int node_start,
+                                                 int n_int, int N, int ell_off, int ell_cnt, int ell_total)
+{
+    uint32_t bytes = 0;
+    if (lane < plan.n && (plan.d[lane].kind == 0) == elems_pass) {
+        const StageDesc d = plan.d[lane];
+        const int start = d.kind == 0 ? elem_start : (d.kind == 1 ? node_start : ell_off);
+        const int count = d.kind == 0 ? n_elem : (d.kind == 1 ? n_int : ell_cnt);
+        const int total = d.kind == 0 ? Ne : (d.kind == 1 ? N : ell_total);
+        if (count > 0) {
+            const int l = d.esize_log2, A1 = (16 >> l) - 1;
+            const int a0 = start & ~A1, end = start + count;
+            int a1 = min((end + A1) & ~A1, total & ~A1);
+            const unsigned char* src = reinterpret_cast<const unsigned char*>(d.src);
+            unsigned char* dst = stage + d.dst_off;
+            if (a1 > a0) {
+                bytes = uint32_t(a1 - a0) << l;
+                bulk_g2s(dst, src + (size_t(a0) << l), bytes, bar);
+            } else {
+                a1 = a0;
+            }
+            for (size_t b = size_t(a1) << l; b < (size_t(end) << l); ++b) dst[b - (size_t(a0) << l)] = src[b];
+        }
+    }
+    for (int o = 16; o > 0; o >>= 1) bytes += __shfl_xor_sync(0xffffffffu, bytes, o);
+    if (lane == 0) mbar_arrive_expect_tx(bar, bytes);
+}
+
+__host__ __device__ __forceinline__ int round_up(int v, int a) { return (v + a - 1) / a * a; }
+
+}  // namespace pff
