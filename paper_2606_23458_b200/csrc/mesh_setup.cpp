@@ -120,7 +120,7 @@ pff_status build_host_mesh(int64_t N, const double* xy, int64_t Ne, const int32_
         const int ell_len_b = (max_ell + 7) / 8 * 8;
         size_t smem = 0;
         for (int kind = 0; kind < 3; ++kind)
-            smem = std::max(smem, chunk_smem_bytes(kind, EC, node_len_b, flag_len_b, ell_len_b, real_bytes));
+            smem = std::max(smem, chunk_smem_bytes(kind, EC, node_len_b, flag_len_b, ell_len_b, max_nloc, real_bytes));
         if ((smem <= smem_limit && max_nloc < 16384) || EC <= 32) {
             if (smem > kSmemPerSM - kSmemCtaReserve - kSmemStatic) { err = "chunk does not fit shared memory"; return PFF_EMESH; }
             hm.max_nloc = max_nloc; hm.C = C;

@@ -44,6 +44,7 @@ struct DmgArgs {
     R* halo_part;  // [3][n_slots]
     int64_t n_slots, ell_total;
     int EC, N, Ne, N_int, N_sh, C;
+    int n_chunk_blocks;  // CTAs of the chunk kernel that wrote block partials (persistent iteration kernel: its grid)
     const int32_t *sh_rowptr, *halo_dst;
     StageLayout lay;
     StagePlan plan;
@@ -155,10 +156,49 @@ __device__ __forceinline__ void elem_damage_apply(const MatC<R>& mat, R b1, R c1
     q3 = m12 * (p3 + sum) - (k1 + k2);
 }
 
-// One CTA per chunk; stage = StageLayout kind 1 (pff_internal.h): lconn | geometry | scalar slots [3 EC + 1] |
-// area | H | x r p q 1/D lb [node_len] | mask | gather table | mbarrier.
+// Indexed gather of one halo node's CG vectors into the halo slots of a stage, as asynchronous copies (LDGSTS):
+// no register or scoreboard is held while the data is in flight.  The flag byte travels inside its 32-bit word.
 template <typename R, int MODE, bool PROJ>
-__global__ void __launch_bounds__(kTPB) dmg_iter_chunk(const DmgArgs<R> a)
+__device__ __forceinline__ void halo_gather_async(const DmgArgs<R>& a, const StageLayout& L, unsigned char* stg, int slot,
+                                                  int j, int gid)
+{
+    constexpr int B = sizeof(R);
+    reinterpret_cast<int*>(stg + L.hids)[j] = gid;
+    if (MODE == DM_CG) {
+        cp_async<B>(reinterpret_cast<R*>(stg + L.node[0]) + slot, a.x + gid);
+        cp_async<B>(reinterpret_cast<R*>(stg + L.node[1]) + slot, a.r + gid);
+        cp_async<B>(reinterpret_cast<R*>(stg + L.node[2]) + slot, a.p + gid);
+        cp_async<B>(reinterpret_cast<R*>(stg + L.node[3]) + slot, a.q + gid);
+        cp_async<B>(reinterpret_cast<R*>(stg + L.node[4]) + slot, a.dinv + gid);
+        if (PROJ) cp_async<B>(reinterpret_cast<R*>(stg + L.node[5]) + slot, a.lb + gid);
+        cp_async<4>(reinterpret_cast<int*>(stg + L.hflag) + j, a.mask + (gid & ~3));
+    } else {
+        cp_async<B>(reinterpret_cast<R*>(stg + L.node[2]) + slot, a.p_in + gid);
+    }
+}
+
+// prologue of one halo node from the gathered values in its stage slot; leaves the new direction in s_p[slot]
+template <typename R, int MODE, bool PROJ>
+__device__ __forceinline__ void halo_prologue(const IterScalars& sc, const StageLayout& L, unsigned char* stg, int slot, int j)
+{
+    if (MODE != DM_CG) return;
+    R* s_p = reinterpret_cast<R*>(stg + L.node[2]);
+    R x = reinterpret_cast<const R*>(stg + L.node[0])[slot], r = reinterpret_cast<const R*>(stg + L.node[1])[slot];
+    const R p = s_p[slot], q = reinterpret_cast<const R*>(stg + L.node[3])[slot];
+    const R dinv = reinterpret_cast<const R*>(stg + L.node[4])[slot];
+    const R lb = PROJ ? reinterpret_cast<const R*>(stg + L.node[5])[slot] : R(0);
+    const int gid = reinterpret_cast<const int*>(stg + L.hids)[j];
+    uint8_t mk = uint8_t(reinterpret_cast<const unsigned*>(stg + L.hflag)[j] >> (8 * (gid & 3)));
+    s_p[slot] = cg_node_prologue<R, PROJ>(sc, x, r, p, q, dinv, lb, mk);
+}
+
+// PERSISTENT, double-buffered CG iteration kernel: gridDim.x CTAs, CTA b owns chunks b, b + G, b + 2G, ...
+// While chunk k is computed, the bulk copies of chunk k + 1 are in flight into the other stage and its halo
+// gathers sit in registers, so no load latency is exposed between chunks.  Shared memory (StageLayout kind 1,
+// two stages): per stage lconn | geometry | area | H | x r p q 1/D lb [node_len] | mask | gather table;
+// shared by both stages: scalar slots [3 EC + 1], the chunk-meta ring, two mbarriers.
+template <typename R, int MODE, bool PROJ>
+__global__ void __launch_bounds__(kTPB, 3) dmg_iter_chunk(const DmgArgs<R> a)
 {
     extern __shared__ __align__(128) unsigned char smem[];
     __shared__ double s_w[kCh * 32], s_out[kCh];
@@ -170,109 +210,156 @@ __global__ void __launch_bounds__(kTPB) dmg_iter_chunk(const DmgArgs<R> a)
         sc.alpha = c->alpha; sc.beta = c->beta; sc.first = c->first; sc.restart = c->restart; sc.trunc = c->trunc;
     }
     const StageLayout& L = a.lay;
-    const ushort4* s_lconn = reinterpret_cast<const ushort4*>(smem + L.lconn);
-    const unsigned char* s_geo = smem + L.geo;
-    R* s_slot = reinterpret_cast<R*>(smem + L.slots);
-    const R* s_area = reinterpret_cast<const R*>(smem + L.area);
-    const R* s_H = reinterpret_cast<const R*>(smem + L.H);
-    R* s_x = reinterpret_cast<R*>(smem + L.node[0]);
-    R* s_r = reinterpret_cast<R*>(smem + L.node[1]);
-    R* s_p = reinterpret_cast<R*>(smem + L.node[2]);
-    const R* s_q = reinterpret_cast<const R*>(smem + L.node[3]);
-    const R* s_dinv = reinterpret_cast<const R*>(smem + L.node[4]);
-    const R* s_lb = reinterpret_cast<const R*>(smem + L.node[5]);
-    uint8_t* s_mask = smem + L.flags;
-    const uint16_t* s_ell = reinterpret_cast<const uint16_t*>(smem + L.ell);
+    R* s_slot = reinterpret_cast<R*>(smem + L.slot_base);
+    ChunkMeta* s_meta = reinterpret_cast<ChunkMeta*>(smem + L.meta);
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem + L.bar);
+    const int tid = threadIdx.x, G = gridDim.x, EC = a.EC;
+    const int n_my = (a.C - (int)blockIdx.x + G - 1) / G;  // chunks this CTA owns
+    // the LAST warp issues the bulk copies (one lane per array); the halo gathers are issued from the top thread
+    // downwards: both are idle while the low warps run the node prologue
+    const int lane = tid & 31;
+    const bool issuer = tid >= kTPB - 32;
+    const bool have_desc = issuer && lane < a.plan.n;
+    StageDesc my_desc{};
+    if (have_desc) my_desc = a.plan.d[lane];
+    const int gj = kTPB - 1 - tid;  // halo node whose gather this thread issues
 
-    const int tid = threadIdx.x;
-    const ChunkMeta cm = a.meta[blockIdx.x];
-    if (tid == 0) { mbar_init(bar, 2); s_slot[3 * a.EC] = R(0); }
-    __syncthreads();
-    if (tid < 32)  // element arrays first: their range follows from blockIdx (in flight while the meta is fetched)
-        stage_issue_plan(a.plan, smem, bar, tid, true, blockIdx.x * a.EC, min(a.EC, a.Ne - blockIdx.x * a.EC), a.Ne, 0, 0, a.N,
-                         0, 0, 0);
-    const int nloc = cm.n_int + cm.n_halo;
-    const int shift = cm.node_start & (A - 1), hb = (shift + cm.n_int + A - 1) & ~(A - 1), fshift = cm.node_start & 15;
-    int* s_fwd = reinterpret_cast<int*>(smem + L.node[3]);  // halo part of the q array: forwards the partial slots
-    if (tid < 32)
-        stage_issue_plan(a.plan, smem, bar, tid, false, 0, 0, a.Ne, cm.node_start, cm.n_int, a.N, cm.ell_off, cm.ell_w * nloc,
-                         (int)a.ell_total);
-    // halo nodes: indexed gathers + the same prologue (no global writes: the interface kernel owns them)
-    for (int j = tid; j < cm.n_halo; j += kTPB) {
-        const int gid = __ldg(a.halo_ids + cm.halo_off + j);
-        R pn;
-        if (MODE == DM_CG) {
-            R x = R(0), r = a.r[gid], p = R(0), q = R(0), lb = R(0);
-            const R dinv = a.dinv[gid];
-            uint8_t mk = a.mask[gid];
-            if (!sc.first) { x = a.x[gid]; p = a.p[gid]; q = a.q[gid]; }
-            if (PROJ) { if (sc.first) x = a.x[gid]; lb = a.lb[gid]; }
-            pn = cg_node_prologue<R, PROJ>(sc, x, r, p, q, dinv, lb, mk);
-        } else {
-            pn = a.p_in[gid];
-        }
-        s_p[hb + j] = pn;
-        s_fwd[(hb + j) * (int)(sizeof(R) / 4)] = __ldg(a.halo_dst + cm.halo_off + j);
-    }
-    mbar_wait(bar, 0);
-
+    if (tid == 0) { mbar_init(bar, 1 + kTPB); mbar_init(bar + 2, 1 + kTPB); s_slot[3 * EC] = R(0); }
     double acc[kCh];
 #pragma unroll
     for (int c = 0; c < kCh; ++c) acc[c] = 0.0;
     acc[kCh - 1] = INFINITY;
-    if (MODE == DM_CG) {
-        for (int i = tid; i < cm.n_int; i += kTPB) {
-            const int s = shift + i, gid = cm.node_start + i;
-            R x = R(0), r = s_r[s], p = R(0), q = R(0), lb = R(0);
-            const R dinv = s_dinv[s];
-            uint8_t mk = s_mask[fshift + i];
-            const uint8_t mk0 = mk;
-            if (!sc.first) { x = s_x[s]; p = s_p[s]; q = s_q[s]; }
-            if (PROJ) { if (sc.first) x = s_x[s]; lb = s_lb[s]; }
-            const R pn = cg_node_prologue<R, PROJ>(sc, x, r, p, q, dinv, lb, mk);
-            if (!sc.first) { if (mk0 & 1) a.x[gid] = x; a.r[gid] = r; }
-            if (mk != mk0) a.mask[gid] = mk;
-            a.p[gid] = pn;
-            s_p[s] = pn; s_r[s] = r; s_mask[fshift + i] = mk;
-            if (mk & 1) {
-                const double rd = double(r), zd = rd * double(dinv);
-                acc[1] += rd * zd; acc[2] += rd * rd;
-                if (PROJ && pn < R(0)) acc[kCh - 1] = fmin(acc[kCh - 1], (double(lb) - double(x)) / double(pn));
+
+    int it = 0;  // stage uses so far (global over epochs): stage = it & 1, mbarrier parity = (it >> 1) & 1
+    for (int e0 = 0; e0 < n_my; e0 += kMetaCap) {
+        const int n_ep = min(kMetaCap, n_my - e0);
+        __syncthreads();  // previous epoch fully consumed (also publishes the mbarrier init)
+        if (tid < n_ep) s_meta[tid] = a.meta[blockIdx.x + (e0 + tid) * G];
+        __syncthreads();
+        // epoch prologue: chunk 0 of the epoch is loaded with exposed latency (once per kMetaCap chunks)
+        {
+            const ChunkMeta cm = s_meta[0];
+            unsigned char* stg = smem + (it & 1) * L.stage_bytes;
+            if (issuer) {
+                const ChunkRange cr{cm.elem_start, cm.n_elem, a.Ne, cm.node_start, cm.n_int, a.N, cm.ell_off,
+                                    cm.ell_w * (cm.n_int + cm.n_halo), (int)a.ell_total, cm.halo_off, cm.n_halo, (int)a.n_slots,
+                                    n_ep > 1 ? s_meta[1].halo_off : 0, n_ep > 1 ? s_meta[1].n_halo : 0};
+                fence_proxy_async();
+                stage_issue_desc(my_desc, have_desc, stg, bar + 2 * (it & 1), lane, cr);
             }
+            if (gj < cm.n_halo) {
+                const int hb0 = ((cm.node_start & (A - 1)) + cm.n_int + A - 1) & ~(A - 1);
+                halo_gather_async<R, MODE, PROJ>(a, L, stg, hb0 + gj, gj, __ldg(a.halo_ids + cm.halo_off + gj));
+            }
+            cp_async_mbar_arrive(bar + 2 * (it & 1));
         }
-    }
-    __syncthreads();
+        for (int k = 0; k < n_ep; ++k, ++it) {
+            const int st = it & 1;
+            unsigned char* stg = smem + st * L.stage_bytes;
+            const ushort4* s_lconn = reinterpret_cast<const ushort4*>(stg + L.lconn);
+            const unsigned char* s_geo = stg + L.geo;
+            const R* s_area = reinterpret_cast<const R*>(stg + L.area);
+            const R* s_H = reinterpret_cast<const R*>(stg + L.H);
+            R* s_x = reinterpret_cast<R*>(stg + L.node[0]);
+            R* s_r = reinterpret_cast<R*>(stg + L.node[1]);
+            R* s_p = reinterpret_cast<R*>(stg + L.node[2]);
+            R* s_q = reinterpret_cast<R*>(stg + L.node[3]);
+            const R* s_dinv = reinterpret_cast<const R*>(stg + L.node[4]);
+            const R* s_lb = reinterpret_cast<const R*>(stg + L.node[5]);
+            uint8_t* s_mask = stg + L.flags;
+            const uint16_t* s_ell = reinterpret_cast<const uint16_t*>(stg + L.ell);
+            const ChunkMeta cm = s_meta[k];
+            const int nloc = cm.n_int + cm.n_halo;
+            const int shift = cm.node_start & (A - 1), hb = (shift + cm.n_int + A - 1) & ~(A - 1), fshift = cm.node_start & 15;
+            const int* s_hdst = reinterpret_cast<const int*>(stg + L.hdst) + (cm.halo_off & 3);
 
-    for (int e = tid; e < cm.n_elem; e += kTPB) {
-        const ushort4 c = s_lconn[e];
-        R b1, c1, b2, c2, q1, q2, q3;
-        Geo<R>::load_smem(s_geo, e, a.EC, b1, c1, b2, c2);
-        elem_damage_apply<R>(a.mat, b1, c1, b2, c2, s_area[e], s_H[e], s_p[c.x], s_p[c.y], s_p[c.z], q1, q2, q3);
-        s_slot[e] = q1; s_slot[a.EC + e] = q2; s_slot[2 * a.EC + e] = q3;
-    }
-    __syncthreads();
-
-    for (int i = tid; i < nloc; i += kTPB) {
-        R qs = R(0);
-        const uint16_t* row = s_ell + i;
-#pragma unroll 4
-        for (int k = 0; k < cm.ell_w; ++k) qs += s_slot[row[k * nloc]];
-        if (i < cm.n_int) {
-            const int gid = cm.node_start + i, s = shift + i;
-            if (MODE == DM_CG) {
-                a.q[gid] = qs;
-                const double qd = double(qs);
-                acc[0] += double(s_p[s]) * qd;
-                if (s_mask[fshift + i] & 1) {
-                    const double rd = double(s_r[s]), dv = double(s_dinv[s]);
-                    acc[3] += rd * dv * qd; acc[4] += dv * qd * qd; acc[5] += rd * qd; acc[6] += qd * qd;
+            // bulk copies AND every thread's halo gathers of this chunk (all issued one iteration ago)
+            mbar_wait(bar + 2 * st, (it >> 1) & 1);
+            // ---- prefetch chunk k + 1 into the other stage: bulk copies (with the halo ids of chunk k + 2) and
+            // asynchronous halo gathers; the ids it needs arrived with THIS stage.  No register is held in flight.
+            if (k + 1 < n_ep) {
+                const ChunkMeta cn = s_meta[k + 1];
+                unsigned char* stn = smem + (st ^ 1) * L.stage_bytes;
+                if (issuer) {
+                    const ChunkRange cr{cn.elem_start, cn.n_elem, a.Ne, cn.node_start, cn.n_int, a.N, cn.ell_off,
+                                        cn.ell_w * (cn.n_int + cn.n_halo), (int)a.ell_total, cn.halo_off, cn.n_halo, (int)a.n_slots,
+                                        k + 2 < n_ep ? s_meta[k + 2].halo_off : 0, k + 2 < n_ep ? s_meta[k + 2].n_halo : 0};
+                    fence_proxy_async();
+                    stage_issue_desc(my_desc, have_desc, stn, bar + 2 * (st ^ 1), lane, cr);
                 }
-            } else {
-                a.q_out[gid] = qs;
+                if (gj < cn.n_halo) {
+                    const int hbn = ((cn.node_start & (A - 1)) + cn.n_int + A - 1) & ~(A - 1);
+                    const int gid = reinterpret_cast<const int*>(stg + L.hnext)[(cn.halo_off & 3) + gj];
+                    halo_gather_async<R, MODE, PROJ>(a, L, stn, hbn + gj, gj, gid);
+                }
+                cp_async_mbar_arrive(bar + 2 * (st ^ 1));
             }
-        } else {
-            a.halo_part[s_fwd[(hb + i - cm.n_int) * (int)(sizeof(R) / 4)]] = qs;
+            // ---- halo nodes of this chunk: gathered values -> prologue -> new direction in their stage slots
+            for (int j = tid; j < min(cm.n_halo, kTPB); j += kTPB) halo_prologue<R, MODE, PROJ>(sc, L, stg, hb + j, j);
+            for (int j = tid + kTPB; j < cm.n_halo; j += kTPB) {  // more halo nodes than threads: not prefetched
+                halo_gather_async<R, MODE, PROJ>(a, L, stg, hb + j, j, __ldg(a.halo_ids + cm.halo_off + j));
+                cp_async_wait_all();
+                halo_prologue<R, MODE, PROJ>(sc, L, stg, hb + j, j);
+            }
+
+            // ---- interior nodes: apply the previous step, form the new direction (owner writes)
+            if (MODE == DM_CG) {
+                for (int i = tid; i < cm.n_int; i += kTPB) {
+                    const int s = shift + i, gid = cm.node_start + i;
+                    R x = R(0), r = s_r[s], p = R(0), q = R(0), lb = R(0);
+                    const R dinv = s_dinv[s];
+                    uint8_t mk = s_mask[fshift + i];
+                    const uint8_t mk0 = mk;
+                    if (!sc.first) { x = s_x[s]; p = s_p[s]; q = s_q[s]; }
+                    if (PROJ) { if (sc.first) x = s_x[s]; lb = s_lb[s]; }
+                    const R pn = cg_node_prologue<R, PROJ>(sc, x, r, p, q, dinv, lb, mk);
+                    if (!sc.first) { if (mk0 & 1) a.x[gid] = x; a.r[gid] = r; }
+                    if (mk != mk0) a.mask[gid] = mk;
+                    a.p[gid] = pn;
+                    s_p[s] = pn; s_r[s] = r; s_mask[fshift + i] = mk;
+                    if (mk & 1) {
+                        const double rd = double(r), zd = rd * double(dinv);
+                        acc[1] += rd * zd; acc[2] += rd * rd;
+                        if (PROJ && pn < R(0)) acc[kCh - 1] = fmin(acc[kCh - 1], (double(lb) - double(x)) / double(pn));
+                    }
+                }
+            }
+            __syncthreads();
+
+            // ---- element pass
+            for (int e = tid; e < cm.n_elem; e += kTPB) {
+                const ushort4 c = s_lconn[e];
+                R b1, c1, b2, c2, q1, q2, q3;
+                Geo<R>::load_smem(s_geo, e, EC, b1, c1, b2, c2);
+                elem_damage_apply<R>(a.mat, b1, c1, b2, c2, s_area[e], s_H[e], s_p[c.x], s_p[c.y], s_p[c.z], q1, q2, q3);
+                s_slot[e] = q1; s_slot[EC + e] = q2; s_slot[2 * EC + e] = q3;
+            }
+            __syncthreads();
+
+            // ---- ordered node gather, q, partial sums
+            for (int i = tid; i < nloc; i += kTPB) {
+                R qs = R(0);
+                const uint16_t* row = s_ell + i;
+#pragma unroll 4
+                for (int w = 0; w < cm.ell_w; ++w) qs += s_slot[row[w * nloc]];
+                if (i < cm.n_int) {
+                    const int gid = cm.node_start + i, s = shift + i;
+                    if (MODE == DM_CG) {
+                        a.q[gid] = qs;
+                        const double qd = double(qs);
+                        acc[0] += double(s_p[s]) * qd;
+                        if (s_mask[fshift + i] & 1) {
+                            const double rd = double(s_r[s]), dv = double(s_dinv[s]);
+                            acc[3] += rd * dv * qd; acc[4] += dv * qd * qd; acc[5] += rd * qd; acc[6] += qd * qd;
+                        }
+                    } else {
+                        a.q_out[gid] = qs;
+                    }
+                } else {
+                    a.halo_part[s_hdst[i - cm.n_int]] = qs;
+                }
+            }
+            __syncthreads();  // stage st and the slots are free again
         }
     }
     if (MODE == DM_CG) {
@@ -397,7 +484,7 @@ __global__ void __launch_bounds__(kTPB) dmg_iter_shared(const DmgArgs<R> a)
     if (MODE != DM_CG) return;
     block_reduce_ch(acc, s_w, s_out);
     double t[kCh];
-    if (fold_and_finish(a.part, a.part_n, a.C, a.part2, a.ticket, s_w, s_out, t) && threadIdx.x == 0)
+    if (fold_and_finish(a.part, a.part_n, a.n_chunk_blocks, a.part2, a.ticket, s_w, s_out, t) && threadIdx.x == 0)
         cg_scalar_step<PROJ>(a.ctrl, t);
 }
 
@@ -412,9 +499,9 @@ __global__ void __launch_bounds__(kTPB) dmg_setup_chunk(const DmgArgs<R> a)
     const StageLayout& L = a.lay;
     const ushort4* s_lconn = reinterpret_cast<const ushort4*>(smem + L.lconn);
     const unsigned char* s_geo = smem + L.geo;
-    R* s_sq = reinterpret_cast<R*>(smem + L.slots);
-    R* s_sD = reinterpret_cast<R*>(smem + L.slots + L.slot_stride);
-    R* s_sb = reinterpret_cast<R*>(smem + L.slots + 2 * L.slot_stride);
+    R* s_sq = reinterpret_cast<R*>(smem + L.slot_base);
+    R* s_sD = reinterpret_cast<R*>(smem + L.slot_base + L.slot_stride);
+    R* s_sb = reinterpret_cast<R*>(smem + L.slot_base + 2 * L.slot_stride);
     const R* s_area = reinterpret_cast<const R*>(smem + L.area);
     const R* s_H = reinterpret_cast<const R*>(smem + L.H);
     R* s_x = reinterpret_cast<R*>(smem + L.node[0]);
@@ -425,11 +512,11 @@ __global__ void __launch_bounds__(kTPB) dmg_setup_chunk(const DmgArgs<R> a)
     if (tid == 0) { mbar_init(bar, 2); s_sq[3 * EC] = R(0); s_sD[3 * EC] = R(0); s_sb[3 * EC] = R(0); }
     __syncthreads();
     if (tid < 32)
-        stage_issue_plan(a.plan, smem, bar, tid, true, blockIdx.x * EC, min(EC, a.Ne - blockIdx.x * EC), a.Ne, 0, 0, a.N, 0, 0, 0);
+        stage_issue_plan(a.plan, smem, bar, tid, 1, blockIdx.x * EC, min(EC, a.Ne - blockIdx.x * EC), a.Ne, 0, 0, a.N, 0, 0, 0);
     const int nloc = cm.n_int + cm.n_halo;
     const int shift = cm.node_start & (A - 1), hb = (shift + cm.n_int + A - 1) & ~(A - 1);
     if (tid < 32)
-        stage_issue_plan(a.plan, smem, bar, tid, false, 0, 0, a.Ne, cm.node_start, cm.n_int, a.N, cm.ell_off, cm.ell_w * nloc,
+        stage_issue_plan(a.plan, smem, bar, tid, 2, 0, 0, a.Ne, cm.node_start, cm.n_int, a.N, cm.ell_off, cm.ell_w * nloc,
                          (int)a.ell_total);
     for (int j = tid; j < cm.n_halo; j += kTPB) s_x[hb + j] = a.x[__ldg(a.halo_ids + cm.halo_off + j)];
     mbar_wait(bar, 0);
@@ -515,7 +602,7 @@ __global__ void __launch_bounds__(kTPB) dmg_setup_shared(const DmgArgs<R> a)
     acc[kCh - 1] = INFINITY;
     block_reduce_ch(acc, s_w, s_out);
     double t[kCh];
-    if (fold_and_finish(a.part, a.part_n, a.C, a.part2, a.ticket, s_w, s_out, t) && threadIdx.x == 0)
+    if (fold_and_finish(a.part, a.part_n, a.n_chunk_blocks, a.part2, a.ticket, s_w, s_out, t) && threadIdx.x == 0)
         a.ctrl->nb = fmax(fmax(sqrt(t[0]), sqrt(t[1])), 1e-300);
 }
 
@@ -553,6 +640,7 @@ static DmgArgs<R> make_args(pff_mesh* m, const pff_state* s)
     a.halo_part = (R*)m->d_halo_part; a.n_slots = m->n_slots; a.ell_total = m->ell_total;
     a.EC = hm.chunk_elems;
     a.N = (int)hm.N; a.Ne = (int)hm.Ne; a.N_int = (int)hm.N_int; a.N_sh = (int)hm.N_sh; a.C = (int)hm.C;
+    a.n_chunk_blocks = (int)hm.C;
     a.sh_rowptr = m->d_sh_rowptr; a.halo_dst = m->d_halo_dst;
     a.H = (const R*)s->H; a.x = (R*)s->d;
     a.lb = (R*)m->d_lb; a.r = (R*)m->d_r; a.p = (R*)m->d_p; a.q = (R*)m->d_q; a.dinv = (R*)m->d_dinv;
@@ -579,6 +667,10 @@ static void set_plan(pff_mesh* m, DmgArgs<R>& a, int which, bool proj)
     add(m->d_area, L.area, lr, 0);
     add(a.H, L.H, lr, 0);
     add(m->d_ell, L.ell, 1, 2);
+    if (which != 2) {
+        add(m->d_halo_dst, L.hdst, 2, 3);   // partial slots of the chunk's halo nodes
+        add(m->d_halo_ids, L.hnext, 2, 4);  // ids of the next chunk's halo nodes
+    }
     if (which == 0) {
         add(a.x, L.node[0], lr, 1); add(a.r, L.node[1], lr, 1); add(a.p, L.node[2], lr, 1); add(a.q, L.node[3], lr, 1);
         add(a.dinv, L.node[4], lr, 1);
@@ -589,6 +681,18 @@ static void set_plan(pff_mesh* m, DmgArgs<R>& a, int which, bool proj)
     } else {
         add(a.x, L.node[0], lr, 1);
     }
+}
+
+// grid of a persistent chunk kernel: every SM filled with as many CTAs as its shared memory / registers allow
+template <typename K>
+static pff_status persistent_grid(pff_mesh* m, K kern, int smem, int* grid)
+{
+    int per_sm = 0, sms = 0;
+    pff_status st = cuda_check(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kTPB, (size_t)smem), "occupancy query");
+    if (st != PFF_OK) return st;
+    if ((st = cuda_check(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, m->device), "SM count")) != PFF_OK) return st;
+    *grid = (int)std::min<int64_t>(m->hm.C, (int64_t)std::max(1, per_sm) * sms);
+    return PFF_OK;
 }
 
 static unsigned shared_grid(const HostMesh& hm)
@@ -636,6 +740,13 @@ static pff_status damage_solve_t(pff_mesh* m, pff_state* s, double rel_tol, int 
     static int g_mv = 0, g_su = 0;  // static + dynamic shared memory may exceed 48 KB: always opt in
     if ((st = set_smem(dmg_iter_chunk<R, DM_CG, PROJ>, smem_mv, g_mv)) != PFF_OK) return st;
     if ((st = set_smem(dmg_setup_chunk<R, false>, smem_su, g_su)) != PFF_OK) return st;
+    static int grid_mv = 0, grid_mv_smem = -1;
+    if (grid_mv_smem != smem_mv) {
+        if ((st = persistent_grid(m, dmg_iter_chunk<R, DM_CG, PROJ>, smem_mv, &grid_mv)) != PFF_OK) return st;
+        grid_mv_smem = smem_mv;
+    }
+    const unsigned gmv = (unsigned)std::min<int64_t>(grid_mv, hm.C);
+    a.n_chunk_blocks = (int)gmv;
     DamageCtrl* h = m->h_ctrl;  // [0]: upload image, [1]: download image
     std::memset(&h[0], 0, sizeof(DamageCtrl));
     h[0].tol = rel_tol; h[0].max_iter = max_iter; h[0].first = 1; h[0].restart = 1; h[0].status = PFF_ENOCONV;
@@ -648,7 +759,7 @@ static pff_status damage_solve_t(pff_mesh* m, pff_state* s, double rel_tol, int 
     for (;;) {
         batch = std::min(batch, max_iter + 1 - launched);
         for (int k = 0; k < batch; ++k) {
-            PFF_LAUNCH(m, PFF_K_MATVEC_CHUNK, (dmg_iter_chunk<R, DM_CG, PROJ><<<(unsigned)hm.C, kTPB, smem_mv, cs>>>(a)));
+            PFF_LAUNCH(m, PFF_K_MATVEC_CHUNK, (dmg_iter_chunk<R, DM_CG, PROJ><<<gmv, kTPB, smem_mv, cs>>>(a)));
             PFF_LAUNCH(m, PFF_K_MATVEC_SHARED, (dmg_iter_shared<R, DM_CG, PROJ><<<gs, kTPB, 0, cs>>>(a)));
         }
         launched += batch;
@@ -691,8 +802,10 @@ static pff_status damage_matvec_t(pff_mesh* m, const pff_state* s, const void* p
     const int smem_mv = (int)m->lay_mv.total;
     static int g_mv = 0;
     if ((st = set_smem(dmg_iter_chunk<R, DM_PLAIN, false>, smem_mv, g_mv)) != PFF_OK) return st;
+    int grid_mv = 0;
+    if ((st = persistent_grid(m, dmg_iter_chunk<R, DM_PLAIN, false>, smem_mv, &grid_mv)) != PFF_OK) return st;
     if (m->only_kernel != 3) {
-        PFF_LAUNCH(m, PFF_K_MATVEC_CHUNK, (dmg_iter_chunk<R, DM_PLAIN, false><<<(unsigned)m->hm.C, kTPB, smem_mv, m->stream>>>(a)));
+        PFF_LAUNCH(m, PFF_K_MATVEC_CHUNK, (dmg_iter_chunk<R, DM_PLAIN, false><<<(unsigned)grid_mv, kTPB, smem_mv, m->stream>>>(a)));
     }
     if (m->only_kernel != 2) {
         PFF_LAUNCH(m, PFF_K_MATVEC_SHARED, (dmg_iter_shared<R, DM_PLAIN, false><<<shared_grid(m->hm), kTPB, 0, m->stream>>>(a)));

@@ -28,23 +28,30 @@ struct ChunkMeta {
 //   kind 1: damage iteration  x r p q 1/D lb + mask; scalar slots [3 EC + 1]
 //   kind 2: damage setup      x; scalar slots q, D, b each [3 EC + 1]
 struct StageLayout {
-    uint32_t lconn, geo, slots, area, H, node[10], flags, ell, bar, total;
+    // offsets relative to the base of a stage (stage s starts at s * stage_bytes)
+    uint32_t lconn, geo, slots, area, H, node[10], flags, ell;
+    uint32_t hids, hflag, hdst;  // per halo node: global id, the 32-bit word holding its flag byte, its partial slot
+    uint32_t hnext;              // global ids of the NEXT chunk's halo nodes (arrive with this stage, feed its gathers)
+    uint32_t stage_bytes, n_stages;
+    // absolute offsets of what the stages share
+    uint32_t slot_base;    // kind 1, 2: the per-element result slots (one copy; only one stage computes at a time)
     uint32_t slot_stride;  // kind 2: bytes between the q, D, b slot arrays
+    uint32_t meta;         // persistent kernels: ring of ChunkMeta of the chunks this CTA owns
+    uint32_t bar;          // one mbarrier per stage
+    uint32_t total;
 };
-inline StageLayout make_stage_layout(int kind, int EC, int node_len, int flag_len, int ell_len, size_t rb)
+constexpr int kMetaCap = 64;  // chunk metas a persistent CTA keeps in shared memory per epoch
+inline StageLayout make_stage_layout(int kind, int EC, int node_len, int flag_len, int ell_len, int max_nhalo, size_t rb,
+                                     int n_stages = 1)
 {
     StageLayout L{};
     auto up16 = [](size_t v) { return uint32_t((v + 15) / 16 * 16); };
     uint32_t o = 0;
     L.lconn = o; o += up16(size_t(8) * EC);
     L.geo = o; o += up16(size_t(4) * rb * EC);
-    if (kind == 0) {
+    if (kind == 0) {  // force-pair slots live inside the stage (fp64: corners 1, 2 overwrite the element's own geometry)
         if (rb == 8) { L.slots = L.geo; o += up16(size_t(16) * (EC + 1)); }      // [ga | gb | third | zero] as double2
         else { L.slots = o; o += up16(size_t(8) * (3 * EC + 1)); }                // float2 [3 EC + 1]
-    } else if (kind == 1) {
-        L.slots = o; o += up16(rb * (size_t(3) * EC + 1));
-    } else {
-        L.slots = o; L.slot_stride = up16(rb * (size_t(3) * EC + 1)); o += 3 * L.slot_stride;
     }
     L.area = o; o += up16(rb * EC);
     L.H = o; o += up16(rb * EC);
@@ -52,13 +59,25 @@ inline StageLayout make_stage_layout(int kind, int EC, int node_len, int flag_le
     for (int k = 0; k < nn; ++k) { L.node[k] = o; o += up16(rb * node_len); }
     L.flags = o; o += up16(kind == 2 ? 0 : flag_len);
     L.ell = o; o += up16(size_t(2) * ell_len);
-    L.bar = o; o += 16;
+    L.hids = o; o += up16(size_t(4) * max_nhalo);
+    L.hflag = o; o += up16(size_t(4) * max_nhalo);
+    L.hdst = o; o += up16(size_t(4) * (max_nhalo + 4));
+    L.hnext = o; o += up16(n_stages > 1 ? size_t(4) * (max_nhalo + 4) : 0);
+    L.stage_bytes = (o + 127) / 128 * 128;
+    L.n_stages = uint32_t(n_stages);
+    o = L.stage_bytes * uint32_t(n_stages);
+    if (kind == 1) { L.slot_base = o; o += up16(rb * (size_t(3) * EC + 1)); }
+    if (kind == 2) { L.slot_base = o; L.slot_stride = up16(rb * (size_t(3) * EC + 1)); o += 3 * L.slot_stride; }
+    L.meta = o; o += n_stages > 1 ? uint32_t(32 * kMetaCap) : 0;
+    L.bar = o; o += 16 * uint32_t(n_stages);
     L.total = o;
     return L;
 }
-inline size_t chunk_smem_bytes(int kind, int EC, int node_len, int flag_len, int ell_len, size_t rb)
+// stages of each chunk kernel: the CG iteration kernel is persistent and double-buffered
+inline int chunk_kernel_stages(int kind) { return kind == 1 ? 2 : 1; }
+inline size_t chunk_smem_bytes(int kind, int EC, int node_len, int flag_len, int ell_len, int max_nhalo, size_t rb)
 {
-    return make_stage_layout(kind, EC, node_len, flag_len, ell_len, rb).total;
+    return make_stage_layout(kind, EC, node_len, flag_len, ell_len, max_nhalo, rb, chunk_kernel_stages(kind)).total;
 }
 
 struct HostMesh {

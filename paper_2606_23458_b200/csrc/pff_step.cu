@@ -135,12 +135,12 @@ __global__ void __launch_bounds__(kTPB) step_chunk_kernel(const StepArgs<R> a)
     if (tid == 0) { mbar_init(bar, 2); s_slot[3 * a.EC] = Geo<R>::pair(R(0), R(0)); }
     __syncthreads();
     if (tid < 32)
-        stage_issue_plan(a.plan, smem, bar, tid, true, blockIdx.x * a.EC, min(a.EC, a.Ne - blockIdx.x * a.EC), a.Ne, 0, 0, a.N,
+        stage_issue_plan(a.plan, smem, bar, tid, 1, blockIdx.x * a.EC, min(a.EC, a.Ne - blockIdx.x * a.EC), a.Ne, 0, 0, a.N,
                          0, 0, 0);
     const int nloc = cm.n_int + cm.n_halo;
     const int shift = cm.node_start & (A - 1), hb = (shift + cm.n_int + A - 1) & ~(A - 1), fshift = cm.node_start & 15;
     if (tid < 32)
-        stage_issue_plan(a.plan, smem, bar, tid, false, 0, 0, a.Ne, cm.node_start, cm.n_int, a.N, cm.ell_off, cm.ell_w * nloc,
+        stage_issue_plan(a.plan, smem, bar, tid, 2, 0, 0, a.Ne, cm.node_start, cm.n_int, a.N, cm.ell_off, cm.ell_w * nloc,
                          (int)a.ell_total);
     // halo (interface) nodes: indexed gathers, predictor (Eq. 16), straight into their stage slots
     for (int j = tid; j < cm.n_halo; j += kTPB) {

@@ -36,6 +36,25 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
     } while (!done);
 }
 
+// orders earlier generic-proxy accesses of shared memory before later asynchronous-proxy (TMA) writes to it
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+// Ampere-style asynchronous copy of ONE small element global -> shared (SASS LDGSTS): used for the indexed
+// halo gathers, which must not hold register scoreboards across a whole chunk iteration.
+template <int BYTES>
+__device__ __forceinline__ void cp_async(void* dst, const void* src)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" ::"r"(smem_u32(dst)), "l"(src), "n"(BYTES) : "memory");
+}
+// every cp.async this thread has issued so far arrives on `bar` when it completes (counts against the mbarrier's
+// expected arrivals: .noinc), so ONE mbarrier wait covers the bulk copies and all threads' gathers of a stage
+__device__ __forceinline__ void cp_async_mbar_arrive(uint64_t* bar)
+{
+    asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
 // global -> shared bulk copy; dst, src 16-byte aligned, bytes a multiple of 16; completion on `bar`
 __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar)
 {
@@ -45,7 +64,8 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
 
 // One contiguous array of a chunk stage.  kind selects the index range of the chunk that is copied:
 // 0 = elements [elem_start, +n_elem) of Ne, 1 = interior nodes [node_start, +n_int) of N,
-// 2 = gather-table entries [ell_off, +ell_w * nloc) of ell_total.
+// 2 = gather-table entries [ell_off, +ell_w * nloc) of ell_total, 3 = halo entries [halo_off, +n_halo) of n_slots,
+// 4 = halo entries of the NEXT chunk of a persistent CTA [next_halo_off, +next_n_halo) of n_slots.
 struct StageDesc {
     const void* src;
     uint32_t dst_off;      // byte offset inside the stage (16-byte aligned)
@@ -58,23 +78,25 @@ struct StagePlan {
     int n;
 };
 
-// Issued by the first warp of the CTA, one lane per array (uniform code, no divergence): element
-// start + i of the global array lands at byte offset dst_off + ((start % A) + i) * esize, A = 16 / esize.
+// One lane's share of a stage burst: lane `lane` of the issuing warp copies the array described by d (if have):
+// element start + i of the global array lands at byte offset dst_off + ((start % A) + i) * esize, A = 16 / esize.
 // The copy is widened to 16-byte boundaries (the few neighbours fetched with it are never read); whatever
 // would reach past the last full 16-byte group of the array is fetched with plain loads.  Lane 0 then
-// arrives on the mbarrier with the total byte count.
-// elems_pass: true = only the element arrays (kind 0; their range follows from blockIdx alone, so they are issued
-// before the chunk meta has arrived), false = everything else; each pass makes one arrival (mbarrier count 2).
-__device__ __forceinline__ void stage_issue_plan(const StagePlan& plan, unsigned char* stage, uint64_t* bar, int lane,
-                                                 bool elems_pass, int elem_start, int n_elem, int Ne, int node_start,
-                                                 int n_int, int N, int ell_off, int ell_cnt, int ell_total)
+// arrives on the mbarrier with the total byte count of the warp.
+struct ChunkRange {  // index ranges of one chunk, per descriptor kind
+    int elem_start, n_elem, Ne, node_start, n_int, N, ell_off, ell_cnt, ell_total, halo_off, n_halo, n_slots, next_halo_off,
+        next_n_halo;
+};
+__device__ __forceinline__ void stage_issue_desc(const StageDesc& d, bool have, unsigned char* stage, uint64_t* bar, int lane,
+                                                 const ChunkRange& c)
 {
     uint32_t bytes = 0;
-    if (lane < plan.n && (plan.d[lane].kind == 0) == elems_pass) {
-        const StageDesc d = plan.d[lane];
-        const int start = d.kind == 0 ? elem_start : (d.kind == 1 ? node_start : ell_off);
-        const int count = d.kind == 0 ? n_elem : (d.kind == 1 ? n_int : ell_cnt);
-        const int total = d.kind == 0 ? Ne : (d.kind == 1 ? N : ell_total);
+    if (have) {
+        int start = c.elem_start, count = c.n_elem, total = c.Ne;
+        if (d.kind == 1) { start = c.node_start; count = c.n_int; total = c.N; }
+        else if (d.kind == 2) { start = c.ell_off; count = c.ell_cnt; total = c.ell_total; }
+        else if (d.kind == 3) { start = c.halo_off; count = c.n_halo; total = c.n_slots; }
+        else if (d.kind == 4) { start = c.next_halo_off; count = c.next_n_halo; total = c.n_slots; }
         if (count > 0) {
             const int l = d.esize_log2, A1 = (16 >> l) - 1;
             const int a0 = start & ~A1, end = start + count;
@@ -92,6 +114,23 @@ __device__ __forceinline__ void stage_issue_plan(const StagePlan& plan, unsigned
     }
     for (int o = 16; o > 0; o >>= 1) bytes += __shfl_xor_sync(0xffffffffu, bytes, o);
     if (lane == 0) mbar_arrive_expect_tx(bar, bytes);
+}
+
+// Issued by one warp of the CTA, one lane per array (uniform code, no divergence).
+// pass: 0 = every array (one arrival); 1 = only the element arrays (kind 0; their range follows from blockIdx alone,
+// so they can be issued before the chunk meta has arrived), 2 = everything else (passes 1 + 2: mbarrier count 2).
+__device__ __forceinline__ void stage_issue_plan(const StagePlan& plan, unsigned char* stage, uint64_t* bar, int lane,
+                                                 int pass, int elem_start, int n_elem, int Ne, int node_start,
+                                                 int n_int, int N, int ell_off, int ell_cnt, int ell_total,
+                                                 int halo_off = 0, int n_halo = 0, int n_slots = 0, int next_halo_off = 0,
+                                                 int next_n_halo = 0)
+{
+    const bool have = lane < plan.n && (pass == 0 || (plan.d[lane].kind == 0) == (pass == 1));
+    StageDesc d{};
+    if (have) d = plan.d[lane];
+    const ChunkRange c{elem_start, n_elem, Ne, node_start, n_int, N, ell_off, ell_cnt, ell_total, halo_off, n_halo, n_slots,
+                       next_halo_off, next_n_halo};
+    stage_issue_desc(d, have, stage, bar, lane, c);
 }
 
 __host__ __device__ __forceinline__ int round_up(int v, int a) { return (v + a - 1) / a * a; }
