@@ -226,13 +226,18 @@ pff_status build_host_mesh(int64_t N, const double* xy, int64_t Ne, const int32_
     }
     hm.ell.resize((hm.ell.size() + 7) / 8 * 8 + 8, uint16_t(3 * EC));  // the widened TMA copy stays in bounds
     // interface-node CSR over halo slots, ascending chunk (chunks were visited in order)
+    // Partial slots: kIfaceWidth fixed slots per interface node (slot kIfaceWidth * s + k for the k-th touching chunk,
+    // ascending chunk order; never-written slots stay zero), the rare further ones in an overflow CSR behind them.
     hm.sh_rowptr.assign(hm.N_sh + 1, 0);
-    for (int64_t s = 0; s < hm.N_sh; ++s) hm.sh_rowptr[s + 1] = hm.sh_rowptr[s] + sh_count[s + 1];
+    for (int64_t s = 0; s < hm.N_sh; ++s)
+        hm.sh_rowptr[s + 1] = hm.sh_rowptr[s] + std::max(0, sh_count[s + 1] - kIfaceWidth);
+    hm.n_ovf = hm.sh_rowptr[hm.N_sh];
     hm.halo_dst.resize(hm.halo_ids.size());
-    std::vector<int32_t> fill(hm.sh_rowptr.begin(), hm.sh_rowptr.end() - 1);
+    std::vector<int32_t> fill(hm.N_sh, 0);
     for (size_t slot = 0; slot < hm.halo_ids.size(); ++slot) {
         int32_t s = hm.halo_ids[slot] - int32_t(hm.N_int);
-        hm.halo_dst[slot] = fill[s]++;
+        const int32_t k = fill[s]++;
+        hm.halo_dst[slot] = k < kIfaceWidth ? kIfaceWidth * s + k : int32_t(kIfaceWidth * hm.N_sh) + hm.sh_rowptr[s] + (k - kIfaceWidth);
     }
     // lumped mass m_i = rho sum A_e / 3 (L169), summed in internal element order
     for (int64_t en = 0; en < Ne; ++en)

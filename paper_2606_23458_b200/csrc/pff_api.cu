@@ -152,7 +152,8 @@ pff_status pff_mesh_create(int64_t n_nodes, const double* xy, int64_t n_elems, c
         UP(upload_real(&m->d_mass, hm.mass.data(), N, m->rb, cs));
         UP(cuda_check(cudaStreamSynchronize(cs), "sync"));
     }
-    m->n_slots = (int64_t)hm.halo_ids.size();
+    m->n_entries = (int64_t)hm.halo_ids.size();
+    m->n_slots = (int64_t)kIfaceWidth * hm.N_sh + hm.n_ovf;
     UP(upload(&m->d_halo_ids, hm.halo_ids.data(), hm.halo_ids.size(), cs));
     UP(upload(&m->d_sh_rowptr, hm.sh_rowptr.data(), hm.sh_rowptr.size(), cs));
     UP(upload(&m->d_halo_dst, hm.halo_dst.data(), hm.halo_dst.size(), cs));

@@ -146,6 +146,18 @@ template <> struct Geo<float> {
     static __device__ __forceinline__ float2 pair(float x, float y) { return make_float2(x, y); }
 };
 
+// Ordered sum of one interface node's per-chunk partials: kIfaceWidth fixed slots (unused ones hold zero) and,
+// on irregular meshes only, its overflow slots.  No index has to be loaded first on regular meshes.
+template <typename R>
+__device__ __forceinline__ R iface_sum(const R* plane, int s, int N_sh, int n_ovf, const int32_t* ovf_rowptr)
+{
+    const R* hp = plane + (size_t)kIfaceWidth * s;
+    R v = ((hp[0] + hp[1]) + hp[2]) + hp[3];
+    if (n_ovf > 0)
+        for (int k = ovf_rowptr[s]; k < ovf_rowptr[s + 1]; ++k) v += plane[(size_t)kIfaceWidth * N_sh + k];
+    return v;
+}
+
 // Deterministic block sum in fp64 (fixed shuffle tree, fixed warp order); result valid in thread 0.
 __device__ __forceinline__ double block_sum(double v, double* s_red /* >= 32 doubles */)
 {

@@ -40,6 +40,7 @@ struct StageLayout {
     uint32_t bar;          // one mbarrier per stage
     uint32_t total;
 };
+constexpr int kIfaceWidth = 4;  // fixed partial slots per interface node (one per touching chunk)
 constexpr int kMetaCap = 64;  // chunk metas a persistent CTA keeps in shared memory per epoch
 inline StageLayout make_stage_layout(int kind, int EC, int node_len, int flag_len, int ell_len, int max_nhalo, size_t rb,
                                      int n_stages = 1)
@@ -97,7 +98,8 @@ struct HostMesh {
     std::vector<ChunkMeta> meta;
     std::vector<int32_t> halo_ids;  // global internal ids (all >= N_int)
     std::vector<uint16_t> ell;      // slot index corner * EC + local element; padding entries = 3 * EC (zero slot)
-    std::vector<int32_t> sh_rowptr;  // per interface node: its range of partial slots (ascending chunk order)
+    std::vector<int32_t> sh_rowptr;  // per interface node: its range in the OVERFLOW partial slots (all zero on regular meshes)
+    int32_t n_ovf = 0;               // overflow partial slots
     std::vector<int32_t> halo_dst;   // per (chunk, halo node) entry: the partial slot it writes
     std::vector<double> xy_user;    // copy of the input coordinates (traction lengths)
 };

@@ -35,7 +35,8 @@ struct pff_mesh {
     uint16_t* d_ell = nullptr;
     uint8_t* d_flags = nullptr;  // bit0: u_x Dirichlet, bit1: u_y Dirichlet, bit2: damage Dirichlet
     void* d_halo_part = nullptr;  // [3][n_slots] reals: per (chunk, interface node) partial sums
-    int64_t n_slots = 0;
+    int64_t n_slots = 0;    // partial slots per plane: kIfaceWidth per interface node + overflow
+    int64_t n_entries = 0;  // (chunk, halo node) entries = length of d_halo_ids / d_halo_dst
     void *d_fwx = nullptr, *d_fwy = nullptr;  // atomic-scatter force accumulators (kept zero between steps)
 
     // Dirichlet set

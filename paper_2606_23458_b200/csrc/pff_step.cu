@@ -31,7 +31,7 @@ struct StepArgs {
     const R* minv;
     R* halo_part;  // [2][n_slots]
     int64_t n_slots;
-    int EC, N, Ne, N_int, N_sh;
+    int EC, N, Ne, N_int, N_sh, n_ovf;
     int64_t ell_total;
     const int32_t *sh_rowptr, *halo_dst;
     StageLayout lay;
@@ -224,11 +224,8 @@ __global__ void __launch_bounds__(kTPB) step_shared_kernel(const StepArgs<R> a)
     const int s = blockIdx.x * kTPB + threadIdx.x;
     if (s >= a.N_sh) return;
     const int gid = a.N_int + s;
-    R fx = R(0), fy = R(0);
-    for (int k = a.sh_rowptr[s]; k < a.sh_rowptr[s + 1]; ++k) {  // partials of one node are contiguous, ascending chunk
-        fx += a.halo_part[k];
-        fy += a.halo_part[a.n_slots + k];
-    }
+    const R fx = iface_sum<R>(a.halo_part, s, a.N_sh, a.n_ovf, a.sh_rowptr);
+    const R fy = iface_sum<R>(a.halo_part + a.n_slots, s, a.N_sh, a.n_ovf, a.sh_rowptr);
     R px, py;
     predict<R, MODE>(a, gid, px, py);
     finish_node<R, MODE>(a, gid, px, py, fx, fy);
@@ -340,7 +337,7 @@ static pff_status launch_step_r(pff_mesh* m, pff_state* s, const pff_bc* bc, dou
     a.halo_part = (R*)m->d_halo_part; a.n_slots = m->n_slots;
     a.EC = hm.chunk_elems; a.ell_total = m->ell_total; a.N = (int)hm.N; a.Ne = (int)hm.Ne;
     a.N_int = (int)hm.N_int; a.N_sh = (int)hm.N_sh;
-    a.sh_rowptr = m->d_sh_rowptr; a.halo_dst = m->d_halo_dst;
+    a.sh_rowptr = m->d_sh_rowptr; a.halo_dst = m->d_halo_dst; a.n_ovf = hm.n_ovf;
     a.ux = (R*)s->ux; a.uy = (R*)s->uy; a.vx = (R*)s->vx; a.vy = (R*)s->vy; a.ax = (R*)s->ax; a.ay = (R*)s->ay;
     a.d = (const R*)s->d; a.H = (R*)s->H; a.fex = (const R*)s->fext_x; a.fey = (const R*)s->fext_y;
     a.fx_out = (R*)fx; a.fy_out = (R*)fy; a.psi_out = (R*)psi;

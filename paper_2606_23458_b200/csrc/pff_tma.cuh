@@ -39,6 +39,9 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
 // orders earlier generic-proxy accesses of shared memory before later asynchronous-proxy (TMA) writes to it
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
+// generic-proxy writes to global memory before a grid-wide barrier / asynchronous-proxy reads of them after it
+__device__ __forceinline__ void fence_proxy_async_global() { asm volatile("fence.proxy.async.global;" ::: "memory"); }
+
 // Ampere-style asynchronous copy of ONE small element global -> shared (SASS LDGSTS): used for the indexed
 // halo gathers, which must not hold register scoreboards across a whole chunk iteration.
 template <int BYTES>
