@@ -90,7 +90,7 @@ pff_status build_host_mesh(int64_t N, const double* xy, int64_t Ne, const int32_
     const bool user_chunk = chunk_elems > 0;
     int EC = user_chunk ? chunk_elems : (real_bytes == 8 ? 512 : 1024);
     EC = std::max(32, std::min(8192, (EC / 32) * 32));
-    const size_t smem_limit = (user_chunk ? kSmemPerSM : kSmemPerSM / 3) - kSmemCtaReserve - kSmemStatic;
+    const size_t smem_limit = (user_chunk ? kSmemPerSM : kSmemPerSM / 3) - kSmemCtaReserve;
     std::vector<int32_t> cmin(N), cmax(N);
     for (;;) {
         std::fill(cmin.begin(), cmin.end(), std::numeric_limits<int32_t>::max());
@@ -103,30 +103,32 @@ pff_status build_host_mesh(int64_t N, const double* xy, int64_t Ne, const int32_
         // per-chunk local node count and valence (bounds for the staged array lengths) via first-touch stamps
         int64_t C = (Ne + EC - 1) / EC;
         std::vector<int32_t> stamp(N, -1), valence(N, 0);
-        int32_t max_nloc = 0, max_ell = 0;
+        int32_t max_nloc = 0, max_ell = 0, max_nh = 0;
         for (int64_t c = 0; c < C; ++c) {
-            int32_t nloc = 0, w = 0;
+            int32_t nloc = 0, w = 0, nh = 0;
             for (int64_t en = c * EC; en < std::min<int64_t>(Ne, (c + 1) * EC); ++en) {
                 const int32_t* t = &tri[3 * elem_old_of_new[en]];
                 for (int k = 0; k < 3; ++k) {
-                    if (stamp[t[k]] != c) { stamp[t[k]] = int32_t(c); valence[t[k]] = 0; ++nloc; }
+                    if (stamp[t[k]] != c) { stamp[t[k]] = int32_t(c); valence[t[k]] = 0; ++nloc; nh += cmin[t[k]] != cmax[t[k]]; }
                     w = std::max(w, ++valence[t[k]]);
                 }
             }
             max_nloc = std::max(max_nloc, nloc);
+            max_nh = std::max(max_nh, nh);
             max_ell = std::max(max_ell, w * nloc);
         }
         const int node_len_b = (max_nloc + 2 * A + A - 1) / A * A, flag_len_b = (max_nloc + 32 + 15) / 16 * 16;
         const int ell_len_b = (max_ell + 7) / 8 * 8;
-        size_t smem = 0;
+        size_t smem = 0;  // dynamic + static shared memory of the most demanding chunk kernel (the step kernel has no static part)
         for (int kind = 0; kind < 3; ++kind)
-            smem = std::max(smem, chunk_smem_bytes(kind, EC, node_len_b, flag_len_b, ell_len_b, max_nloc, real_bytes));
+            smem = std::max(smem, chunk_smem_bytes(kind, EC, node_len_b, flag_len_b, ell_len_b, max_nh, real_bytes) +
+                                      (kind == 0 ? 0 : kSmemStatic));
         if ((smem <= smem_limit && max_nloc < 16384) || EC <= 32) {
-            if (smem > kSmemPerSM - kSmemCtaReserve - kSmemStatic) { err = "chunk does not fit shared memory"; return PFF_EMESH; }
+            if (smem > kSmemPerSM - kSmemCtaReserve) { err = "chunk does not fit shared memory"; return PFF_EMESH; }
             hm.max_nloc = max_nloc; hm.C = C;
             break;
         }
-        EC = std::max(32, (EC / 2 / 32) * 32);
+        EC = std::max(32, (EC * 7 / 8 / 32) * 32);  // 512, 448, 384, 320, 256, 224, 192, 160, 128, 96, 64, 32
     }
     hm.chunk_elems = EC;
     const int64_t C = hm.C;

@@ -119,7 +119,7 @@ pff_status pff_mesh_create(int64_t n_nodes, const double* xy, int64_t n_elems, c
                                                            : mat->E * mat->nu / ((1 + mat->nu) * (1 - 2 * mat->nu));
         m->dt_crit = hm.hmin / std::sqrt((lam + 2 * mu) / mat->rho);
     }
-    m->lay_step = make_stage_layout(0, hm.chunk_elems, hm.node_len, hm.flag_len, hm.ell_len, hm.max_nhalo, m->rb);
+    m->lay_step = make_stage_layout(0, hm.chunk_elems, hm.node_len, hm.flag_len, hm.ell_len, hm.max_nhalo, m->rb, chunk_kernel_stages(0));
     m->lay_mv = make_stage_layout(1, hm.chunk_elems, hm.node_len, hm.flag_len, hm.ell_len, hm.max_nhalo, m->rb, chunk_kernel_stages(1));
     m->lay_su = make_stage_layout(2, hm.chunk_elems, hm.node_len, hm.flag_len, hm.ell_len, hm.max_nhalo, m->rb);
     m->ell_total = (int64_t)hm.ell.size();

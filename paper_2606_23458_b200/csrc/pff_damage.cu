@@ -340,7 +340,10 @@ __global__ void __launch_bounds__(kTPB, 3) dmg_iter_chunk(const DmgArgs<R> a)
                 cp_async_mbar_arrive(bar + 2 * (st ^ 1));
             }
             // ---- halo nodes of this chunk: gathered values -> prologue -> new direction in their stage slots
-            for (int j = tid; j < min(cm.n_halo, kTPB); j += kTPB) halo_prologue<R, MODE, PROJ>(sc, L, stg, hb + j, j);
+            {   // by the middle warps (the low warps run the interior prologue, the top ones issue the prefetch)
+                const int j = (tid + kTPB / 2) & (kTPB - 1);  // thread kTPB/2 takes halo node 0
+                if (j < cm.n_halo) halo_prologue<R, MODE, PROJ>(sc, L, stg, hb + j, j);
+            }
             for (int j = tid + kTPB; j < cm.n_halo; j += kTPB) {  // more halo nodes than threads: not prefetched
                 halo_gather_async<R, MODE, PROJ>(a, L, stg, hb + j, j, __ldg(a.halo_ids + cm.halo_off + j));
                 cp_async_wait_all();

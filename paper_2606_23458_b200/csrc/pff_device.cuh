@@ -127,6 +127,12 @@ template <> struct Geo<double> {
         b1 = p.x; c1 = p.y; b2 = q.x; c2 = q.y;
     }
     static __device__ __forceinline__ double2 pair(double x, double y) { return make_double2(x, y); }
+    // force-pair slot idx = corner * EC + e: corners 1, 2 overwrite the element's own staged geometry, corner 3 and
+    // the zero pair (idx 3 EC) live in the shared slot region
+    static __device__ __forceinline__ double2* slot(unsigned char* geo, unsigned char* shared_slots, int idx, int EC)
+    {
+        return idx < 2 * EC ? reinterpret_cast<double2*>(geo) + idx : reinterpret_cast<double2*>(shared_slots) + (idx - 2 * EC);
+    }
 };
 template <> struct Geo<float> {
     typedef float2 Pair;
@@ -144,6 +150,10 @@ template <> struct Geo<float> {
         b1 = p.x; c1 = p.y; b2 = p.z; c2 = p.w;
     }
     static __device__ __forceinline__ float2 pair(float x, float y) { return make_float2(x, y); }
+    static __device__ __forceinline__ float2* slot(unsigned char*, unsigned char* shared_slots, int idx, int)
+    {
+        return reinterpret_cast<float2*>(shared_slots) + idx;
+    }
 };
 
 // Ordered sum of one interface node's per-chunk partials: kIfaceWidth fixed slots (unused ones hold zero) and,

@@ -29,19 +29,19 @@ struct ChunkMeta {
 //   kind 2: damage setup      x; scalar slots q, D, b each [3 EC + 1]
 struct StageLayout {
     // offsets relative to the base of a stage (stage s starts at s * stage_bytes)
-    uint32_t lconn, geo, slots, area, H, node[10], flags, ell;
+    uint32_t lconn, geo, area, H, node[10], flags, ell;
     uint32_t hids, hflag, hdst;  // per halo node: global id, the 32-bit word holding its flag byte, its partial slot
     uint32_t hnext;              // global ids of the NEXT chunk's halo nodes (arrive with this stage, feed its gathers)
     uint32_t stage_bytes, n_stages;
     // absolute offsets of what the stages share
-    uint32_t slot_base;    // kind 1, 2: the per-element result slots (one copy; only one stage computes at a time)
+    uint32_t slot_base;    // the per-element result slots (one copy; only one stage computes at a time)
     uint32_t slot_stride;  // kind 2: bytes between the q, D, b slot arrays
     uint32_t meta;         // persistent kernels: ring of ChunkMeta of the chunks this CTA owns
     uint32_t bar;          // one mbarrier per stage
     uint32_t total;
 };
 constexpr int kIfaceWidth = 4;  // fixed partial slots per interface node (one per touching chunk)
-constexpr int kMetaCap = 64;  // chunk metas a persistent CTA keeps in shared memory per epoch
+constexpr int kMetaCap = 32;  // chunk metas a persistent CTA keeps in shared memory per epoch
 inline StageLayout make_stage_layout(int kind, int EC, int node_len, int flag_len, int ell_len, int max_nhalo, size_t rb,
                                      int n_stages = 1)
 {
@@ -50,10 +50,6 @@ inline StageLayout make_stage_layout(int kind, int EC, int node_len, int flag_le
     uint32_t o = 0;
     L.lconn = o; o += up16(size_t(8) * EC);
     L.geo = o; o += up16(size_t(4) * rb * EC);
-    if (kind == 0) {  // force-pair slots live inside the stage (fp64: corners 1, 2 overwrite the element's own geometry)
-        if (rb == 8) { L.slots = L.geo; o += up16(size_t(16) * (EC + 1)); }      // [ga | gb | third | zero] as double2
-        else { L.slots = o; o += up16(size_t(8) * (3 * EC + 1)); }                // float2 [3 EC + 1]
-    }
     L.area = o; o += up16(rb * EC);
     L.H = o; o += up16(rb * EC);
     const int nn = kind == 0 ? 10 : (kind == 1 ? 6 : 1);
@@ -67,6 +63,10 @@ inline StageLayout make_stage_layout(int kind, int EC, int node_len, int flag_le
     L.stage_bytes = (o + 127) / 128 * 128;
     L.n_stages = uint32_t(n_stages);
     o = L.stage_bytes * uint32_t(n_stages);
+    if (kind == 0) {  // force-pair slots corner * EC + e (+ one zero pair).  fp64: corners 1, 2 overwrite the element's
+        // own staged geometry (pair index into the stage's geometry) and only corner 3 + the zero pair live here
+        L.slot_base = o; o += up16(rb == 8 ? size_t(16) * (EC + 1) : size_t(8) * (3 * EC + 1));
+    }
     if (kind == 1) { L.slot_base = o; o += up16(rb * (size_t(3) * EC + 1)); }
     if (kind == 2) { L.slot_base = o; L.slot_stride = up16(rb * (size_t(3) * EC + 1)); o += 3 * L.slot_stride; }
     L.meta = o; o += n_stages > 1 ? uint32_t(32 * kMetaCap) : 0;
@@ -74,8 +74,8 @@ inline StageLayout make_stage_layout(int kind, int EC, int node_len, int flag_le
     L.total = o;
     return L;
 }
-// stages of each chunk kernel: the CG iteration kernel is persistent and double-buffered
-inline int chunk_kernel_stages(int kind) { return kind == 1 ? 2 : 1; }
+// stages of each chunk kernel: the step and CG kernels are persistent and double-buffered
+inline int chunk_kernel_stages(int kind) { return kind == 2 ? 1 : 2; }
 inline size_t chunk_smem_bytes(int kind, int EC, int node_len, int flag_len, int ell_len, int max_nhalo, size_t rb)
 {
     return make_stage_layout(kind, EC, node_len, flag_len, ell_len, max_nhalo, rb, chunk_kernel_stages(kind)).total;

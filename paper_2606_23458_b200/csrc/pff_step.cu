@@ -10,6 +10,8 @@
 //   elem_atomic_kernel / node_atomic_kernel   PFF_SCATTER_ATOMIC variant: thread per element, global
 //                       floating-point atomics (the paper's "atomic indexed accumulation", L43, L124).
 //   dirichlet_kernel    writes u_bar, v_bar into the Dirichlet dofs before the step (Eq. 5, R8).
+#include <algorithm>
+
 #include "pff_device.cuh"
 #include "pff_mesh.h"
 #include "pff_tma.cuh"
@@ -31,8 +33,8 @@ struct StepArgs {
     const R* minv;
     R* halo_part;  // [2][n_slots]
     int64_t n_slots;
-    int EC, N, Ne, N_int, N_sh, n_ovf;
-    int64_t ell_total;
+    int EC, N, Ne, N_int, N_sh, n_ovf, C;
+    int64_t ell_total, n_entries;
     const int32_t *sh_rowptr, *halo_dst;
     StageLayout lay;
     StagePlan plan;
@@ -99,121 +101,201 @@ __device__ __forceinline__ void element_forces(const MatC<R>& mat, R b1, R c1, R
     f[4] = -(f[0] + f[2]); f[5] = -(f[1] + f[3]);
 }
 
-// One CTA per chunk.  The stage (StageLayout kind 0, pff_internal.h) is filled by ONE burst of bulk-asynchronous
-// copies issued by the first warp (one lane per array); the halo gathers overlap with it.
+// Indexed gather of one halo node's kinematic state into the halo slots of a stage, as asynchronous copies
+// (LDGSTS): nothing is held in registers while the data is in flight.  The flag byte travels in its 32-bit word.
+template <typename R, int MODE>
+__device__ __forceinline__ void step_halo_gather(const StepArgs<R>& a, const StageLayout& L, unsigned char* stg, int slot, int j,
+                                                 int gid)
+{
+    constexpr int B = sizeof(R);
+    reinterpret_cast<int*>(stg + L.hids)[j] = gid;
+    cp_async<B>(reinterpret_cast<R*>(stg + L.node[0]) + slot, a.ux + gid);
+    cp_async<B>(reinterpret_cast<R*>(stg + L.node[1]) + slot, a.uy + gid);
+    cp_async<B>(reinterpret_cast<R*>(stg + L.node[2]) + slot, a.d + gid);
+    if (MODE == MODE_STEP) {
+        cp_async<B>(reinterpret_cast<R*>(stg + L.node[3]) + slot, a.vx + gid);
+        cp_async<B>(reinterpret_cast<R*>(stg + L.node[4]) + slot, a.vy + gid);
+        cp_async<B>(reinterpret_cast<R*>(stg + L.node[5]) + slot, a.ax + gid);
+        cp_async<B>(reinterpret_cast<R*>(stg + L.node[6]) + slot, a.ay + gid);
+        cp_async<4>(reinterpret_cast<int*>(stg + L.hflag) + j, a.flags + (gid & ~3));
+    }
+}
+
+// PERSISTENT, double-buffered explicit-step kernel: gridDim.x CTAs, CTA b owns chunks b, b + G, b + 2G, ...
+// While chunk k is computed, the bulk copies (TMA) of chunk k + 1 stream into the other stage and its halo
+// gathers (cp.async) land in that stage's halo slots; one mbarrier per stage counts the TMA arrival and every
+// thread's cp.async arrival.  Per chunk: predictor (Eq. 16) -> fused element pass (strain, split, degradation,
+// stress, force, history) -> ordered gather + Eq. 17-18.  Stage = StageLayout kind 0 (pff_internal.h).
 template <typename R, int SPLIT, int MODE>
-__global__ void __launch_bounds__(kTPB) step_chunk_kernel(const StepArgs<R> a)
+__global__ void __launch_bounds__(kTPB, 3) step_chunk_kernel(const StepArgs<R> a)
 {
     extern __shared__ __align__(128) unsigned char smem[];
     typedef typename Geo<R>::Pair Pair;
     constexpr int A = 16 / sizeof(R);
     const StageLayout& L = a.lay;
-    const ushort4* s_lconn = reinterpret_cast<const ushort4*>(smem + L.lconn);
-    const unsigned char* s_geo = smem + L.geo;
-    Pair* s_slot = reinterpret_cast<Pair*>(smem + L.slots);
-    const R* s_area = reinterpret_cast<const R*>(smem + L.area);
-    const R* s_H = reinterpret_cast<const R*>(smem + L.H);
-    R* s_ux = reinterpret_cast<R*>(smem + L.node[0]);
-    R* s_uy = reinterpret_cast<R*>(smem + L.node[1]);
-    R* s_d = reinterpret_cast<R*>(smem + L.node[2]);
-    const R* s_vx = reinterpret_cast<const R*>(smem + L.node[3]);
-    R* s_fwd = reinterpret_cast<R*>(smem + L.node[3]);  // halo part of the v_x array: forwards each halo node's partial slot
-    const R* s_vy = reinterpret_cast<const R*>(smem + L.node[4]);
-    const R* s_ax = reinterpret_cast<const R*>(smem + L.node[5]);
-    const R* s_ay = reinterpret_cast<const R*>(smem + L.node[6]);
-    const R* s_fex = reinterpret_cast<const R*>(smem + L.node[7]);
-    const R* s_fey = reinterpret_cast<const R*>(smem + L.node[8]);
-    const R* s_minv = reinterpret_cast<const R*>(smem + L.node[9]);
-    const uint8_t* s_flags = smem + L.flags;
-    const uint16_t* s_ell = reinterpret_cast<const uint16_t*>(smem + L.ell);
+    unsigned char* s_shared_slots = smem + L.slot_base;
+    ChunkMeta* s_meta = reinterpret_cast<ChunkMeta*>(smem + L.meta);
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem + L.bar);
+    const int tid = threadIdx.x, lane = tid & 31, G = gridDim.x, EC = a.EC;
+    const int n_my = (a.C - (int)blockIdx.x + G - 1) / G;  // chunks this CTA owns
+    // the LAST warp issues the bulk copies (one lane per array); the halo gathers are issued from the top thread down
+    const bool issuer = tid >= kTPB - 32;
+    const bool have_desc = issuer && lane < a.plan.n;
+    StageDesc my_desc{};
+    if (have_desc) my_desc = a.plan.d[lane];
+    const int gj = kTPB - 1 - tid;
 
-    // ---- phase 0: stream every contiguous array of the chunk into the stage (TMA).  The element arrays go first:
-    // their range follows from blockIdx, so they are in flight while the chunk meta is still being fetched.
-    const int tid = threadIdx.x;
-    const ChunkMeta cm = a.meta[blockIdx.x];
-    if (tid == 0) { mbar_init(bar, 2); s_slot[3 * a.EC] = Geo<R>::pair(R(0), R(0)); }
-    __syncthreads();
-    if (tid < 32)
-        stage_issue_plan(a.plan, smem, bar, tid, 1, blockIdx.x * a.EC, min(a.EC, a.Ne - blockIdx.x * a.EC), a.Ne, 0, 0, a.N,
-                         0, 0, 0);
-    const int nloc = cm.n_int + cm.n_halo;
-    const int shift = cm.node_start & (A - 1), hb = (shift + cm.n_int + A - 1) & ~(A - 1), fshift = cm.node_start & 15;
-    if (tid < 32)
-        stage_issue_plan(a.plan, smem, bar, tid, 2, 0, 0, a.Ne, cm.node_start, cm.n_int, a.N, cm.ell_off, cm.ell_w * nloc,
-                         (int)a.ell_total);
-    // halo (interface) nodes: indexed gathers, predictor (Eq. 16), straight into their stage slots
-    for (int j = tid; j < cm.n_halo; j += kTPB) {
-        const int gid = __ldg(a.halo_ids + cm.halo_off + j);
-        R px, py;
-        predict<R, MODE>(a, gid, px, py);
-        s_ux[hb + j] = px; s_uy[hb + j] = py; s_d[hb + j] = a.d[gid];
-        reinterpret_cast<int*>(s_fwd + hb + j)[0] = __ldg(a.halo_dst + cm.halo_off + j);  // partial slot, used in phase 3
+    if (tid == 0) {
+        mbar_init(bar, 1 + kTPB); mbar_init(bar + 2, 1 + kTPB);
+        *Geo<R>::slot(smem, s_shared_slots, 3 * EC, EC) = Geo<R>::pair(R(0), R(0));  // the zero pair (lives in the shared region)
     }
-    mbar_wait(bar, 0);
-
-    // ---- phase 1: predictor of the interior nodes, in place (Eq. 16; Dirichlet dofs hold u_bar already)
-    if (MODE == MODE_STEP) {
-        for (int i = tid; i < cm.n_int; i += kTPB) {
-            const int s = shift + i;
-            const uint8_t fl = s_flags[fshift + i];
-            const R ux = s_ux[s], uy = s_uy[s];
-            const R px = rfma(a.hdt2, s_ax[s], rfma(a.dt, s_vx[s], ux));
-            const R py = rfma(a.hdt2, s_ay[s], rfma(a.dt, s_vy[s], uy));
-            s_ux[s] = (fl & 1) ? ux : px;
-            s_uy[s] = (fl & 2) ? uy : py;
-        }
-    }
-    __syncthreads();
-
-    // ---- phase 2: fused element pass; nodal force pairs go to the slots corner * EC + e
-    for (int e = tid; e < cm.n_elem; e += kTPB) {
-        const ushort4 c = s_lconn[e];
-        R b1, c1, b2, c2;
-        Geo<R>::load_smem(s_geo, e, a.EC, b1, c1, b2, c2);
-        R psi_p, f[6];
-        element_forces<R, SPLIT>(a.mat, b1, c1, b2, c2, s_area[e], s_ux[c.x], s_uy[c.x], s_ux[c.y], s_uy[c.y], s_ux[c.z],
-                                 s_uy[c.z], s_d[c.x] + s_d[c.y] + s_d[c.z], psi_p, f);
-        s_slot[e] = Geo<R>::pair(f[0], f[1]);
-        s_slot[a.EC + e] = Geo<R>::pair(f[2], f[3]);
-        s_slot[2 * a.EC + e] = Geo<R>::pair(f[4], f[5]);
-        if (MODE == MODE_STEP) {
-            if (psi_p > s_H[e]) a.H[cm.elem_start + e] = psi_p;  // H <- max(H, psi+)  (L98, L114)
-        } else if (MODE == MODE_FORCE) {
-            if (a.psi_out) a.psi_out[cm.elem_start + e] = psi_p;
-        }
-    }
-    __syncthreads();
-
-    // ---- phase 3: ordered gather of each node's incident force pairs, then Eq. 17-18 for interior nodes
-    for (int i = tid; i < nloc; i += kTPB) {
-        R fx = R(0), fy = R(0);
-        const uint16_t* row = s_ell + i;
-#pragma unroll 4
-        for (int k = 0; k < cm.ell_w; ++k) {
-            const Pair v = s_slot[row[k * nloc]];
-            fx += v.x; fy += v.y;
-        }
-        if (i < cm.n_int) {
-            const int gid = cm.node_start + i, s = shift + i;
-            if (MODE == MODE_FORCE) { a.fx_out[gid] = fx; a.fy_out[gid] = fy; continue; }
-            const uint8_t fl = s_flags[fshift + i];
-            const R minv = s_minv[s];
-            R axn = (a.S * s_fex[s] - fx) * minv;
-            R ayn = (a.S * s_fey[s] - fy) * minv;
-            if (fl & 1) axn = R(0);
-            if (fl & 2) ayn = R(0);
-            if (MODE == MODE_STEP) {
-                const R vxo = s_vx[s], vyo = s_vy[s];
-                a.ux[gid] = s_ux[s]; a.uy[gid] = s_uy[s];
-                a.vx[gid] = (fl & 1) ? vxo : rfma(a.hdt, s_ax[s] + axn, vxo);
-                a.vy[gid] = (fl & 2) ? vyo : rfma(a.hdt, s_ay[s] + ayn, vyo);
+    int it = 0;  // stage uses so far: stage = it & 1, mbarrier parity = (it >> 1) & 1
+    for (int e0 = 0; e0 < n_my; e0 += kMetaCap) {
+        const int n_ep = min(kMetaCap, n_my - e0);
+        __syncthreads();  // previous epoch fully consumed (also publishes the mbarrier init)
+        if (tid < n_ep) s_meta[tid] = a.meta[blockIdx.x + (e0 + tid) * G];
+        __syncthreads();
+        {   // epoch prologue: chunk 0 of the epoch is loaded with exposed latency (once per kMetaCap chunks)
+            const ChunkMeta cm = s_meta[0];
+            unsigned char* stg = smem + (it & 1) * L.stage_bytes;
+            if (issuer) {
+                const ChunkRange cr{cm.elem_start, cm.n_elem, a.Ne, cm.node_start, cm.n_int, a.N, cm.ell_off,
+                                    cm.ell_w * (cm.n_int + cm.n_halo), (int)a.ell_total, cm.halo_off, cm.n_halo, (int)a.n_entries,
+                                    n_ep > 1 ? s_meta[1].halo_off : 0, n_ep > 1 ? s_meta[1].n_halo : 0};
+                fence_proxy_async();
+                stage_issue_desc(my_desc, have_desc, stg, bar + 2 * (it & 1), lane, cr);
             }
-            a.ax[gid] = axn; a.ay[gid] = ayn;
-        } else {
-            const int slot = reinterpret_cast<const int*>(s_fwd + hb + i - cm.n_int)[0];
-            a.halo_part[slot] = fx;
-            a.halo_part[a.n_slots + slot] = fy;
+            if (gj < cm.n_halo) {
+                const int hb0 = ((cm.node_start & (A - 1)) + cm.n_int + A - 1) & ~(A - 1);
+                step_halo_gather<R, MODE>(a, L, stg, hb0 + gj, gj, __ldg(a.halo_ids + cm.halo_off + gj));
+            }
+            cp_async_mbar_arrive(bar + 2 * (it & 1));
+        }
+        for (int k = 0; k < n_ep; ++k, ++it) {
+            const int st = it & 1;
+            unsigned char* stg = smem + st * L.stage_bytes;
+            const ushort4* s_lconn = reinterpret_cast<const ushort4*>(stg + L.lconn);
+            unsigned char* s_geo = stg + L.geo;
+            const R* s_area = reinterpret_cast<const R*>(stg + L.area);
+            const R* s_H = reinterpret_cast<const R*>(stg + L.H);
+            R* s_ux = reinterpret_cast<R*>(stg + L.node[0]);
+            R* s_uy = reinterpret_cast<R*>(stg + L.node[1]);
+            const R* s_d = reinterpret_cast<const R*>(stg + L.node[2]);
+            const R* s_vx = reinterpret_cast<const R*>(stg + L.node[3]);
+            const R* s_vy = reinterpret_cast<const R*>(stg + L.node[4]);
+            const R* s_ax = reinterpret_cast<const R*>(stg + L.node[5]);
+            const R* s_ay = reinterpret_cast<const R*>(stg + L.node[6]);
+            const R* s_fex = reinterpret_cast<const R*>(stg + L.node[7]);
+            const R* s_fey = reinterpret_cast<const R*>(stg + L.node[8]);
+            const R* s_minv = reinterpret_cast<const R*>(stg + L.node[9]);
+            const uint8_t* s_flags = stg + L.flags;
+            const uint16_t* s_ell = reinterpret_cast<const uint16_t*>(stg + L.ell);
+            const ChunkMeta cm = s_meta[k];
+            const int nloc = cm.n_int + cm.n_halo;
+            const int shift = cm.node_start & (A - 1), hb = (shift + cm.n_int + A - 1) & ~(A - 1), fshift = cm.node_start & 15;
+            const int* s_hdst = reinterpret_cast<const int*>(stg + L.hdst) + (cm.halo_off & 3);
+
+            // bulk copies AND every thread's halo gathers of this chunk (all issued one iteration ago)
+            mbar_wait(bar + 2 * st, (it >> 1) & 1);
+            // ---- prefetch chunk k + 1 into the other stage (its halo ids arrived with THIS stage)
+            if (k + 1 < n_ep) {
+                const ChunkMeta cn = s_meta[k + 1];
+                unsigned char* stn = smem + (st ^ 1) * L.stage_bytes;
+                if (issuer) {
+                    const ChunkRange cr{cn.elem_start, cn.n_elem, a.Ne, cn.node_start, cn.n_int, a.N, cn.ell_off,
+                                        cn.ell_w * (cn.n_int + cn.n_halo), (int)a.ell_total, cn.halo_off, cn.n_halo, (int)a.n_entries,
+                                        k + 2 < n_ep ? s_meta[k + 2].halo_off : 0, k + 2 < n_ep ? s_meta[k + 2].n_halo : 0};
+                    fence_proxy_async();
+                    stage_issue_desc(my_desc, have_desc, stn, bar + 2 * (st ^ 1), lane, cr);
+                }
+                if (gj < cn.n_halo) {
+                    const int hbn = ((cn.node_start & (A - 1)) + cn.n_int + A - 1) & ~(A - 1);
+                    const int gid = reinterpret_cast<const int*>(stg + L.hnext)[(cn.halo_off & 3) + gj];
+                    step_halo_gather<R, MODE>(a, L, stn, hbn + gj, gj, gid);
+                }
+                cp_async_mbar_arrive(bar + 2 * (st ^ 1));
+            }
+            for (int j = tid + kTPB; j < cm.n_halo; j += kTPB) {  // more halo nodes than threads: not prefetched
+                step_halo_gather<R, MODE>(a, L, stg, hb + j, j, __ldg(a.halo_ids + cm.halo_off + j));
+                cp_async_wait_all();
+            }
+            if (cm.n_halo > kTPB) __syncthreads();
+
+            // ---- phase 1: predictor (Eq. 16) in place, halo nodes by the middle warps, interior by the low warps;
+            // Dirichlet dofs hold u_bar already (dirichlet_kernel)
+            if (MODE == MODE_STEP) {
+                for (int j = (tid + kTPB / 2) & (kTPB - 1); j < cm.n_halo; j += kTPB) {
+                    const int s = hb + j, gid = reinterpret_cast<const int*>(stg + L.hids)[j];
+                    const unsigned fl = reinterpret_cast<const unsigned*>(stg + L.hflag)[j] >> (8 * (gid & 3));
+                    const R ux = s_ux[s], uy = s_uy[s];
+                    const R px = rfma(a.hdt2, s_ax[s], rfma(a.dt, s_vx[s], ux));
+                    const R py = rfma(a.hdt2, s_ay[s], rfma(a.dt, s_vy[s], uy));
+                    s_ux[s] = (fl & 1) ? ux : px;
+                    s_uy[s] = (fl & 2) ? uy : py;
+                }
+                for (int i = tid; i < cm.n_int; i += kTPB) {
+                    const int s = shift + i;
+                    const uint8_t fl = s_flags[fshift + i];
+                    const R ux = s_ux[s], uy = s_uy[s];
+                    const R px = rfma(a.hdt2, s_ax[s], rfma(a.dt, s_vx[s], ux));
+                    const R py = rfma(a.hdt2, s_ay[s], rfma(a.dt, s_vy[s], uy));
+                    s_ux[s] = (fl & 1) ? ux : px;
+                    s_uy[s] = (fl & 2) ? uy : py;
+                }
+            }
+            __syncthreads();
+
+            // ---- phase 2: fused element pass; nodal force pairs go to the slots corner * EC + e
+            for (int e = tid; e < cm.n_elem; e += kTPB) {
+                const ushort4 c = s_lconn[e];
+                R b1, c1, b2, c2;
+                Geo<R>::load_smem(s_geo, e, EC, b1, c1, b2, c2);
+                R psi_p, f[6];
+                element_forces<R, SPLIT>(a.mat, b1, c1, b2, c2, s_area[e], s_ux[c.x], s_uy[c.x], s_ux[c.y], s_uy[c.y], s_ux[c.z],
+                                         s_uy[c.z], s_d[c.x] + s_d[c.y] + s_d[c.z], psi_p, f);
+                *Geo<R>::slot(s_geo, s_shared_slots, e, EC) = Geo<R>::pair(f[0], f[1]);
+                *Geo<R>::slot(s_geo, s_shared_slots, EC + e, EC) = Geo<R>::pair(f[2], f[3]);
+                *Geo<R>::slot(s_geo, s_shared_slots, 2 * EC + e, EC) = Geo<R>::pair(f[4], f[5]);
+                if (MODE == MODE_STEP) {
+                    if (psi_p > s_H[e]) a.H[cm.elem_start + e] = psi_p;  // H <- max(H, psi+)  (L98, L114)
+                } else if (MODE == MODE_FORCE) {
+                    if (a.psi_out) a.psi_out[cm.elem_start + e] = psi_p;
+                }
+            }
+            __syncthreads();
+
+            // ---- phase 3: ordered gather of each node's incident force pairs, then Eq. 17-18 for interior nodes
+            for (int i = tid; i < nloc; i += kTPB) {
+                R fx = R(0), fy = R(0);
+                const uint16_t* row = s_ell + i;
+#pragma unroll 4
+                for (int w = 0; w < cm.ell_w; ++w) {
+                    const Pair v = *Geo<R>::slot(s_geo, s_shared_slots, row[w * nloc], EC);
+                    fx += v.x; fy += v.y;
+                }
+                if (i < cm.n_int) {
+                    const int gid = cm.node_start + i, s = shift + i;
+                    if (MODE == MODE_FORCE) { a.fx_out[gid] = fx; a.fy_out[gid] = fy; continue; }
+                    const uint8_t fl = s_flags[fshift + i];
+                    const R minv = s_minv[s];
+                    R axn = (a.S * s_fex[s] - fx) * minv;
+                    R ayn = (a.S * s_fey[s] - fy) * minv;
+                    if (fl & 1) axn = R(0);
+                    if (fl & 2) ayn = R(0);
+                    if (MODE == MODE_STEP) {
+                        const R vxo = s_vx[s], vyo = s_vy[s];
+                        a.ux[gid] = s_ux[s]; a.uy[gid] = s_uy[s];
+                        a.vx[gid] = (fl & 1) ? vxo : rfma(a.hdt, s_ax[s] + axn, vxo);
+                        a.vy[gid] = (fl & 2) ? vyo : rfma(a.hdt, s_ay[s] + ayn, vyo);
+                    }
+                    a.ax[gid] = axn; a.ay[gid] = ayn;
+                } else {
+                    const int slot = s_hdst[i - cm.n_int];
+                    a.halo_part[slot] = fx;
+                    a.halo_part[a.n_slots + slot] = fy;
+                }
+            }
+            __syncthreads();  // stage st and the slots are free again
         }
     }
 }
@@ -303,8 +385,17 @@ static pff_status launch_step_t(pff_mesh* m, const StepArgs<R>& a)
             if (e != cudaSuccess) return cuda_check(e, "cudaFuncSetAttribute(step_chunk_kernel)");
             granted = (int)m->lay_step.total;
         }
+        static int grid = 0, grid_smem = -1;  // persistent grid: every SM filled with as many CTAs as fit
+        if (grid_smem != (int)m->lay_step.total) {
+            int per_sm = 0, sms = 0;
+            cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kTPB, (size_t)m->lay_step.total);
+            if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, m->device);
+            if (e != cudaSuccess) return cuda_check(e, "step_chunk_kernel occupancy");
+            grid = std::max(1, per_sm) * sms;
+            grid_smem = (int)m->lay_step.total;
+        }
         if (m->only_kernel != 1) {
-            PFF_LAUNCH(m, PFF_K_STEP_CHUNK, (kern<<<(unsigned)hm.C, kTPB, (int)m->lay_step.total, m->stream>>>(a)));
+            PFF_LAUNCH(m, PFF_K_STEP_CHUNK, (kern<<<(unsigned)std::min<int64_t>(grid, hm.C), kTPB, (int)m->lay_step.total, m->stream>>>(a)));
         }
         if (hm.N_sh > 0 && m->only_kernel != 0) {
             PFF_LAUNCH(m, PFF_K_STEP_SHARED, (step_shared_kernel<R, MODE><<<(unsigned)((hm.N_sh + kTPB - 1) / kTPB), kTPB, 0, m->stream>>>(a)));
@@ -335,7 +426,7 @@ static pff_status launch_step_r(pff_mesh* m, pff_state* s, const pff_bc* bc, dou
     a.ga = m->d_ga; a.gb = m->d_gb; a.area = (const R*)m->d_area;
     a.halo_ids = m->d_halo_ids; a.ell = m->d_ell; a.flags = m->d_flags; a.minv = (const R*)m->d_minv;
     a.halo_part = (R*)m->d_halo_part; a.n_slots = m->n_slots;
-    a.EC = hm.chunk_elems; a.ell_total = m->ell_total; a.N = (int)hm.N; a.Ne = (int)hm.Ne;
+    a.EC = hm.chunk_elems; a.ell_total = m->ell_total; a.n_entries = m->n_entries; a.C = (int)hm.C; a.N = (int)hm.N; a.Ne = (int)hm.Ne;
     a.N_int = (int)hm.N_int; a.N_sh = (int)hm.N_sh;
     a.sh_rowptr = m->d_sh_rowptr; a.halo_dst = m->d_halo_dst; a.n_ovf = hm.n_ovf;
     a.ux = (R*)s->ux; a.uy = (R*)s->uy; a.vx = (R*)s->vx; a.vy = (R*)s->vy; a.ax = (R*)s->ax; a.ay = (R*)s->ay;
@@ -358,6 +449,8 @@ static pff_status launch_step_r(pff_mesh* m, pff_state* s, const pff_bc* bc, dou
         add(m->d_area, L.area, lr, 0);
         if (mode == MODE_STEP) add(s->H, L.H, lr, 0);
         add(m->d_ell, L.ell, 1, 2);
+        add(m->d_halo_dst, L.hdst, 2, 3);   // partial slots of the chunk's halo nodes
+        add(m->d_halo_ids, L.hnext, 2, 4);  // ids of the next chunk's halo nodes
         add(s->ux, L.node[0], lr, 1); add(s->uy, L.node[1], lr, 1); add(s->d, L.node[2], lr, 1);
         if (mode == MODE_STEP) {
             add(s->vx, L.node[3], lr, 1); add(s->vy, L.node[4], lr, 1);
