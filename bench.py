@@ -4,7 +4,8 @@
     python bench.py --impl reference ...      # the CPU oracle on the host cores (slow by design)
 
 One "step" = one staggered pass of the whole hot path: pff_explicit_step (Eq. 16-18 with
-the fused element force + history) followed by pff_damage_solve (Jacobi-PCG, rel_tol 1e-8) on one mesh.
+the fused element force + history) followed by pff_damage_solve (Jacobi-PCG, rel_tol 1e-8: two setup kernels and
+ONE cooperative kernel that runs every CG iteration) on one mesh.
 metric = element-updates/s = n_elems * steps / time (PAPER.md L456 reports the same quantity).  Inputs are
 seeded synthetic meshes/fields (pff_inputs.config), resident in HBM for `value`, host buffers for `e2e`.
 Rank 0 prints ONE JSON line.  N > 1: one independent mesh per GPU (weak scaling, no data-path collective).
@@ -40,6 +41,22 @@ def algorithmic_bytes(N: int, Ne: int, w: int) -> dict:
     step = Ne * (12 + 5 * w + 2 * w) + N * 16 * w          # conn + geometry + H r/w ; u,v,a r/w, d, f_ext, m^-1
     matvec = Ne * (12 + 5 * w + w) + N * 2 * w             # conn + geometry + H ; p read, q write
     return dict(step=step, matvec=matvec, cg_iter=matvec + N * 8 * w)
+
+
+def reduce_max(value: float, world: int, device) -> float:
+    """Max over ranks of a per-rank scalar (device time in ms / wall seconds): the N > 1 reporting rule.
+    `device` is the rank's CUDA device under NCCL, "cpu" under gloo (tests/test_multirank_cpu.py)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(n_elems_per_rank: int, steps: int, world: int, seconds_max: float) -> float:
+    """Weak scaling over independent replicas: every rank advances its own mesh, no data-path collective."""
+    return world * n_elems_per_rank * steps / seconds_max
 
 
 class ClockSampler:
@@ -126,10 +143,7 @@ def run_ours(args, rank: int, world: int):
         out = [fn() for _ in range(k)]
         e1.record()
         barrier()
-        ms = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=f"cuda:{dev}")
-        if world > 1:
-            dist.all_reduce(ms, op=dist.ReduceOp.MAX)
-        return float(ms.item()), out
+        return reduce_max(e0.elapsed_time(e1), world, f"cuda:{dev}"), out
 
     for _ in range(args.warmup):
         step()
@@ -166,12 +180,24 @@ def run_ours(args, rank: int, world: int):
     for _ in range(ke):
         e2e_step()
     barrier()
-    sec = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=f"cuda:{dev}")
-    if world > 1:
-        dist.all_reduce(sec, op=dist.ReduceOp.MAX)
-    e2e_val = world * Ne * ke / float(sec.item())
+    e2e_val = whole_job_value(Ne, ke, world, reduce_max(time.perf_counter() - t0, world, f"cuda:{dev}"))
     return dict(mesh=mesh, cfg=cfg, N=N, Ne=Ne, w=w, ms_total=ms_total, iters=iters, launches=launches, clk=clk, prof=prof,
                 iters_p=iters_p, ms_exp=ms_exp, e2e_val=e2e_val, h2d=(9 * N + Ne) * 8, d2h=(7 * N + Ne) * 8, snapshot=snapshot)
+
+
+def ncu_traffic(workload: str, dtype: str, kernel: str, k: dict):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
+    `ncu --set full` capture of this workload (profiles/traffic.csv: a table of numbers, nothing that runs);
+    scaled to this run's iterations per launch for the CG kernel.  None when no capture matches."""
+    path = os.path.join(ROOT, "profiles", "traffic.csv")
+    if not os.path.exists(path):
+        return None
+    for line in open(path).read().splitlines()[1:]:
+        f = line.split(",")
+        if len(f) >= 5 and f[0] == workload and f[1] == dtype and f[2] == kernel:
+            per_unit = float(f[3]) / float(f[4])  # bytes per iteration (CG) / per launch (step)
+            return per_unit * (k.get("iterations_per_launch", 1.0) if kernel == "cg_solve" else 1.0)
+    return None
 
 
 def peaks():
@@ -234,15 +260,23 @@ def main():
     prof = r["prof"]
     total_prof_ms = sum(v[0] for v in prof.values())
     kern = {}
-    for name, key in (("step_chunk", "step"), ("matvec_chunk", "matvec")):
-        ms, cnt = prof[name]
+    iters_prof = int(sum(r["iters_p"]))  # CG iterations of the event-bracketed pass
+    # step_chunk: one launch = one explicit step of the whole mesh; cg_solve: one cooperative launch = ALL CG iterations
+    # of one damage solve, credited with the per-iteration algorithmic bytes x the iterations it ran
+    for name, cls, nbytes in (("step_chunk", "step_chunk", ab["step"]),
+                              ("cg_solve", "matvec_chunk", ab["cg_iter"] * iters_prof / max(prof["matvec_chunk"][1], 1))):
+        ms, cnt = prof[cls]
         if cnt:
             per = ms / cnt
             kern[name] = dict(us_per_launch=1e3 * per, launches=cnt, share_of_kernel_time=ms / total_prof_ms,
-                              algorithmic_bytes=ab[key], achieved_gbs=ab[key] / per / 1e6, frac=ab[key] / per / 1e6 / peak)
-    dom = max(kern, key=lambda k: prof[k][0])
+                              algorithmic_bytes=int(nbytes), achieved_gbs=nbytes / per / 1e6, frac=nbytes / per / 1e6 / peak)
+    if "cg_solve" in kern:
+        kern["cg_solve"]["iterations_per_launch"] = iters_prof / prof["matvec_chunk"][1]
+        kern["cg_solve"]["us_per_iteration"] = 1e3 * prof["matvec_chunk"][0] / max(iters_prof, 1)
+    dom = max(kern, key=lambda k: kern[k]["share_of_kernel_time"])
+    traffic = ncu_traffic(args.workload, "f64" if w == 8 else "f32", dom, kern[dom])
     iters_total = int(sum(r["iters"]))
-    line = dict(metric=METRIC, value=world * Ne * K / sec, unit=UNIT, n_gpus=world, steps=K, warmup=args.warmup,
+    line = dict(metric=METRIC, value=whole_job_value(Ne, K, world, sec), unit=UNIT, n_gpus=world, steps=K, warmup=args.warmup,
                 ms_per_step=r["ms_total"] / K, higher_is_better=True, scaling="weak", vs_baseline=None,
                 dtype="f64" if w == 8 else "f32", data="synthetic",
                 config=dict(workload=args.workload, name=r["cfg"]["name"], n_nodes=N, n_elems=Ne, rel_tol=REL_TOL,
@@ -251,10 +285,12 @@ def main():
                             parallelism=f"replicas x{world}"),
                 explicit_steps_per_s=world * K / (r["ms_exp"] / 1e3),
                 explicit_step_hbm_frac=ab["step"] / (r["ms_exp"] / K / 1e3) / 1e9 / peak,
+                cg_iterations_per_s=world * iters_prof / (prof["matvec_chunk"][0] / 1e3) if prof["matvec_chunk"][0] else None,
+                cg_iteration_hbm_frac=kern["cg_solve"]["frac"] if "cg_solve" in kern else None,
                 clocks=r["clk"], gpu_launches=int(r["launches"]),
                 e2e=dict(value=r["e2e_val"], unit=UNIT, h2d_bytes_per_step=r["h2d"], d2h_bytes_per_step=r["d2h"]),
                 roofline=dict(bound="hbm", kernel=dom, achieved=kern[dom]["achieved_gbs"], peak=peak, unit="GB/s",
-                              frac=kern[dom]["frac"], traffic=None, peak_source=peak_src, kernels=kern,
+                              frac=kern[dom]["frac"], traffic=traffic, peak_source=peak_src, kernels=kern,
                               kernel_time_ms_by_class={k: v[0] for k, v in prof.items()}))
     if not args.no_cpu_baseline:
         import oracle

@@ -230,3 +230,59 @@ def test_run_host_matches_device_path():
         assert orc.damage_solve(rel_tol=1e-12)[0] == 0
     assert relmax(u, orc.u) <= 1e-10 and relmax(v, orc.v) <= 1e-10 and relmax(d, orc.d) <= 1e-10
     assert relmax(H, orc.H) <= 1e-10
+
+
+def test_full_size_bench_configuration_cfg5_1001():
+    """BASELINE's metric size (1e6 nodes, 2e6 elements) in the launch configuration bench.py times (default
+    options: Morton order, default chunk, gather scatter, fp64): two staggered steps, every node and element
+    compared with the oracle (it finishes this size in seconds)."""
+    cfg = config(5, n=1001)
+    orc = oracle_from(cfg)
+    mesh, st = gpu_from(cfg)
+    assert mesh.n_nodes == 1002001 and mesh.n_elems == 2000000
+    dt = cfg["dt_factor"] * orc.dt_crit()
+    orc.init_accel()
+    mesh.pff_init_accel(st, mesh.bc())
+    for _ in range(2):
+        orc.explicit_step(dt)
+        rc, _, _ = orc.damage_solve(rel_tol=1e-12, max_iter=4000)
+        mesh.pff_explicit_step(st, mesh.bc(), dt)
+        stt, _, _ = mesh.pff_damage_solve(st, rel_tol=1e-12, max_iter=4000)
+        assert rc == 0 and stt == 0
+    u, v, a, d, H = gpu_fields(mesh, st)
+    assert relmax(u, orc.u) <= TOL64 and relmax(v, orc.v) <= TOL64 and relmax(a, orc.a) <= TOL64
+    assert relmax(H, orc.H) <= TOL64
+    assert relmax(d, orc.d) <= 1e-10  # two converged solves (1e-12 relative residual, condition number of the operator)
+    e_ref, e = orc.energies(), mesh.pff_energies(st)
+    assert np.all(np.abs(e - e_ref) <= 1e-11 * np.abs(e_ref).max())
+
+
+@pytest.mark.parametrize("model", [1, 2])
+def test_many_chunks_per_cta_big_halos_and_overflow_slots(model):
+    """Corners of the persistent kernels: more chunks per CTA than the shared-memory meta ring holds (several
+    epochs), more halo nodes in a chunk than threads (un-prefetched gathers), interface nodes touched by more
+    chunks than the fixed partial slots (overflow slots): random element order, no renumbering."""
+    cfg = config(5, n=501)  # 500,000 elements: 15,625 chunks of 32 = 35 per CTA on 444 CTAs (ring holds 32)
+    rng = np.random.default_rng(11)
+    cfg["tri"] = cfg["tri"][rng.permutation(len(cfg["tri"]))]
+    cfg["material"] = dict(cfg["material"], model=model)
+    orc = oracle_from(cfg)
+    orc.H = rng.uniform(0, 3e4, orc.Ne)
+    p = rng.normal(0, 1, orc.N)
+    q_ref = orc.damage_matvec(p)
+    f_ref, _ = orc.internal_force()
+    for order, chunk in ((0, 128), (1, 32)):  # (random order: every node is an interface node), (tiny chunks)
+        mesh, st = gpu_from(cfg, order=order, chunk_elems=chunk)
+        st.H.copy_(mesh.elems_to_internal(orc.H))
+        q = mesh.pff_damage_matvec(st, mesh.nodes_to_internal(p))
+        assert relmax(mesh.nodes_to_user(q), q_ref) <= 1e-13
+        fx, fy, _ = mesh.pff_internal_force(st)
+        assert relmax(np.stack([mesh.nodes_to_user(fx), mesh.nodes_to_user(fy)], 1), f_ref) <= TOL64
+    o2 = oracle_from(cfg)
+    o2.H = orc.H.copy()
+    rc, _, _ = o2.damage_solve(rel_tol=1e-12, max_iter=4000)
+    mesh, st = gpu_from(cfg, order=0, chunk_elems=128)
+    st.H.copy_(mesh.elems_to_internal(orc.H))
+    stt, _, _ = mesh.pff_damage_solve(st, rel_tol=1e-12, max_iter=4000)
+    assert rc == 0 and stt == 0
+    assert relmax(mesh.nodes_to_user(st.d), o2.d) <= 1e-10
