@@ -13,7 +13,8 @@
  *  - "host" pointers are ordinary CPU memory, read (or written) before the call returns.
  *    "device" pointers are CUDA device memory of the GPU that was current at pff_mesh_create.
  *  - The library owns the pff_mesh object and all of its workspaces.  The caller owns every
- *    state buffer (pff_state) and keeps it alive; the library never frees or reallocates it.
+ *    state buffer (pff_state) and keeps it alive; the library never frees or reallocates it.  Every state
+ *    array must be 16-byte aligned (they are sources of bulk-asynchronous copies); PFF_EINVAL otherwise.
  *  - All device work is enqueued on the CUDA stream passed to pff_mesh_create (NULL = default
  *    stream).  pff_explicit_step and pff_init_accel never synchronise; pff_damage_solve and
  *    pff_energies synchronise that stream before returning (they return host scalars).
@@ -74,7 +75,8 @@ typedef struct {
     int32_t precision;    /* pff_precision */
     int32_t order;        /* pff_order     */
     int32_t scatter;      /* pff_scatter   */
-    int32_t chunk_elems;  /* elements per CTA chunk, 0 = library default; multiple of 32, <= 8192 */
+    int32_t chunk_elems;  /* elements per chunk, 0 = library default (largest size with 3 double-buffered CTAs per SM);
+                             rounded down to a multiple of 32, shrunk if one CTA would not fit shared memory */
 } pff_options;
 
 typedef struct pff_mesh pff_mesh;
@@ -157,6 +159,8 @@ pff_status pff_explicit_step(pff_mesh *mesh, pff_state *state, const pff_bc *bc,
  * Stops when ||r_free||_2 <= rel_tol * max(||b||_2, ||b - A d_n||_2) (R10) or after max_iter
  * operator applications (then returns PFF_ENOCONV with the result written).
  * iters_out / relres_out (host, may be NULL) receive the mat-vec count and final relative residual.
+ * Device work: two setup kernels and ONE cooperative kernel that runs every CG iteration (the GPU must support
+ * cooperative launches and must not be shared with other kernels of the same stream priority during the call).
  * Synchronises the stream. */
 pff_status pff_damage_solve(pff_mesh *mesh, pff_state *state, double rel_tol, int32_t max_iter,
                             int32_t *iters_out, double *relres_out);
