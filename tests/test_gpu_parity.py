@@ -286,3 +286,46 @@ def test_many_chunks_per_cta_big_halos_and_overflow_slots(model):
     stt, _, _ = mesh.pff_damage_solve(st, rel_tol=1e-12, max_iter=4000)
     assert rc == 0 and stt == 0
     assert relmax(mesh.nodes_to_user(st.d), o2.d) <= 1e-10
+
+
+def test_full_size_config3_at1_starconvex_plane_stress():
+    """Config 3 at BASELINE's full size (1001^2 nodes, 2.0M elements): AT1 projected CG, star-convex split, plane stress,
+    seeded damage disks (damage-Dirichlet), sheared top edge (displacement-Dirichlet ramp): two staggered steps."""
+    cfg = config(3)
+    orc = oracle_from(cfg)
+    mesh, st = gpu_from(cfg)
+    assert mesh.n_elems == 2000000
+    dt = cfg["dt_factor"] * orc.dt_crit()
+    orc.init_accel()
+    mesh.pff_init_accel(st, mesh.bc())
+    for k in range(1, 3):
+        du, dv = shear_bc(cfg, k, dt)
+        orc.explicit_step(dt, dir_u=du, dir_v=dv)
+        rc, _, _ = orc.damage_solve(rel_tol=1e-12, max_iter=4000)
+        mesh.pff_explicit_step(st, mesh.bc(du, dv), dt)
+        stt, _, _ = mesh.pff_damage_solve(st, rel_tol=1e-12, max_iter=4000)
+        assert rc == 0 and stt == 0
+    u, v, a, d, H = gpu_fields(mesh, st)
+    assert relmax(u, orc.u) <= TOL64 and relmax(v, orc.v) <= TOL64 and relmax(a, orc.a) <= TOL64
+    assert relmax(H, orc.H) <= TOL64
+    assert relmax(d, orc.d) <= 1e-9 and d.min() >= 0.0 and d.max() <= 1.0 and np.all(d >= cfg["d0"])
+
+
+def test_full_size_config4_perforated_plate():
+    """Config 4 at full size (2001 x 1001 grid minus 40 holes: ~3.6M elements): one staggered step."""
+    cfg = config(4)
+    orc = oracle_from(cfg)
+    mesh, st = gpu_from(cfg)
+    assert mesh.n_elems > 3_000_000
+    dt = cfg["dt_factor"] * orc.dt_crit()
+    orc.init_accel()
+    mesh.pff_init_accel(st, mesh.bc())
+    orc.explicit_step(dt)
+    rc, _, _ = orc.damage_solve(rel_tol=1e-11, max_iter=4000)
+    mesh.pff_explicit_step(st, mesh.bc(), dt)
+    stt, _, _ = mesh.pff_damage_solve(st, rel_tol=1e-11, max_iter=4000)
+    assert rc == 0 and stt == 0
+    u, v, a, d, H = gpu_fields(mesh, st)
+    assert relmax(u, orc.u) <= TOL64 and relmax(v, orc.v) <= TOL64 and relmax(a, orc.a) <= TOL64
+    assert relmax(H, orc.H) <= TOL64
+    assert relmax(d, orc.d) <= 1e-9
