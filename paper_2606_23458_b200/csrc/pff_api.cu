@@ -70,7 +70,7 @@ void pff_mesh_destroy(pff_mesh* m)
     cudaStreamSynchronize(m->stream);
     void* ptrs[] = {m->d_meta, m->d_lconn, m->d_conn, m->d_ga, m->d_gb, m->d_area, m->d_minv, m->d_mass,
                     m->d_halo_ids, m->d_sh_rowptr, m->d_halo_dst, m->d_ell, m->d_flags, m->d_halo_part,
-                    m->d_fwx, m->d_fwy, m->d_dir_dof, m->d_lb, m->d_r, m->d_p, m->d_q, m->d_dinv, m->d_mask,
+                    m->d_fwx, m->d_fwy, m->d_dir_dof, m->d_ca, m->d_cb, m->d_lb, m->d_r, m->d_p, m->d_q, m->d_dinv, m->d_mask,
                     m->d_part, m->d_part2, m->d_ctrl, m->d_ticket, m->d_stage, m->d_hstate, m->d_node_old_of_new,
                     m->d_elem_old_of_new};
     for (void* p : ptrs) if (p) cudaFree(p);
@@ -163,6 +163,8 @@ pff_status pff_mesh_create(int64_t n_nodes, const double* xy, int64_t n_elems, c
     UP(upload((uint8_t**)&m->d_halo_part, nullptr, size_t(3) * std::max<int64_t>(m->n_slots, 1) * m->rb, cs));
     UP(upload((uint8_t**)&m->d_fwx, nullptr, N * m->rb, cs));
     UP(upload((uint8_t**)&m->d_fwy, nullptr, N * m->rb, cs));
+    UP(upload((uint8_t**)&m->d_ca, nullptr, (m->rb == 8 ? 2 : 4) * Ne * m->rb, cs));
+    if (m->rb == 8) UP(upload((uint8_t**)&m->d_cb, nullptr, 2 * Ne * m->rb, cs));
     UP(upload((uint8_t**)&m->d_lb, nullptr, N * m->rb, cs));
     UP(upload((uint8_t**)&m->d_r, nullptr, N * m->rb, cs));
     UP(upload((uint8_t**)&m->d_p, nullptr, N * m->rb, cs));

@@ -39,6 +39,7 @@ struct DmgArgs {
     const ChunkMeta* meta;
     const ushort4* lconn;
     const void *ga, *gb;
+    void *ca, *cb;  // element-operator coefficients of the current solve (written by the setup pass)
     const R* area;
     const int32_t* halo_ids;
     const uint16_t* ell;
@@ -144,7 +145,7 @@ __device__ __forceinline__ R cg_node_prologue(const IterScalars& sc, R& x, R& r,
     return sc.restart ? z : rfma(R(sc.beta), p, z);
 }
 
-// element operator: q^e = (c_e M^e + kappa K^e) p^e with M^e = A (1 + delta_ij) / 12 (L185)
+// element operator q^e = (c_e M^e + kappa K^e) p^e with M^e = A (1 + delta_ij) / 12 (L185), from the geometry
 template <typename R>
 __device__ __forceinline__ void elem_damage_apply(const MatC<R>& mat, R b1, R c1, R b2, R c2, R A, R He, R p1, R p2, R p3,
                                                   R& q1, R& q2, R& q3)
@@ -157,6 +158,28 @@ __device__ __forceinline__ void elem_damage_apply(const MatC<R>& mat, R b1, R c1
     q1 = m12 * (p1 + sum) + k1;
     q2 = m12 * (p2 + sum) + k2;
     q3 = m12 * (p3 + sum) - (k1 + k2);
+}
+
+// The same operator from its 4 coefficients (what the CG iterations stream instead of geometry + area + H):
+// m = c_e A / 12 and the edge weights w_ij = -kappa A grad phi_i . grad phi_j of the P1 stiffness (rows sum to zero,
+// so K^e p = sum_j w_ij (p_i - p_j)).
+template <typename R>
+__device__ __forceinline__ void elem_coefficients(const MatC<R>& mat, R b1, R c1, R b2, R c2, R A, R He, R& m, R& w12, R& w13,
+                                                  R& w23)
+{
+    const R kA = mat.kappa * A;
+    m = (mat.c0 + R(2) * He) * A * R(1.0 / 12.0);
+    w12 = -kA * (b1 * b2 + c1 * c2);
+    w13 = kA * (b1 * (b1 + b2) + c1 * (c1 + c2));
+    w23 = kA * (b2 * (b1 + b2) + c2 * (c1 + c2));
+}
+template <typename R>
+__device__ __forceinline__ void elem_damage_apply_coef(R m, R w12, R w13, R w23, R p1, R p2, R p3, R& q1, R& q2, R& q3)
+{
+    const R sum = p1 + p2 + p3, d12 = p1 - p2, d13 = p1 - p3, d23 = p2 - p3;
+    q1 = m * (p1 + sum) + (w12 * d12 + w13 * d13);
+    q2 = m * (p2 + sum) + (w23 * d23 - w12 * d12);
+    q3 = m * (p3 + sum) - (w13 * d13 + w23 * d23);
 }
 
 // Scalar step of the recurrence, run by one thread after the fixed-order reduction of all partials.
@@ -303,8 +326,6 @@ __global__ void __launch_bounds__(kTPB, 3) dmg_iter_chunk(const DmgArgs<R> a)
             unsigned char* stg = smem + st * L.stage_bytes;
             const ushort4* s_lconn = reinterpret_cast<const ushort4*>(stg + L.lconn);
             const unsigned char* s_geo = stg + L.geo;
-            const R* s_area = reinterpret_cast<const R*>(stg + L.area);
-            const R* s_H = reinterpret_cast<const R*>(stg + L.H);
             R* s_x = reinterpret_cast<R*>(stg + L.node[0]);
             R* s_r = reinterpret_cast<R*>(stg + L.node[1]);
             R* s_p = reinterpret_cast<R*>(stg + L.node[2]);
@@ -377,9 +398,9 @@ __global__ void __launch_bounds__(kTPB, 3) dmg_iter_chunk(const DmgArgs<R> a)
             // ---- element pass
             for (int e = tid; e < cm.n_elem; e += kTPB) {
                 const ushort4 c = s_lconn[e];
-                R b1, c1, b2, c2, q1, q2, q3;
-                Geo<R>::load_smem(s_geo, e, EC, b1, c1, b2, c2);
-                elem_damage_apply<R>(a.mat, b1, c1, b2, c2, s_area[e], s_H[e], s_p[c.x], s_p[c.y], s_p[c.z], q1, q2, q3);
+                R cm_, w12, w13, w23, q1, q2, q3;
+                Geo<R>::load_smem(s_geo, e, EC, cm_, w12, w13, w23);  // the staged "geometry" is the coefficient stream
+                elem_damage_apply_coef<R>(cm_, w12, w13, w23, s_p[c.x], s_p[c.y], s_p[c.z], q1, q2, q3);
                 s_slot[e] = q1; s_slot[EC + e] = q2; s_slot[2 * EC + e] = q3;
             }
             __syncthreads();
@@ -599,6 +620,18 @@ __global__ void __launch_bounds__(kTPB) dmg_iter_shared(const DmgArgs<R> a)
         cg_scalar_step<PROJ>(a.ctrl, t);
 }
 
+// operator coefficients from the geometry and the current history field (hook path: the solve gets them from the setup pass)
+template <typename R>
+__global__ void __launch_bounds__(kTPB) dmg_coef_kernel(const DmgArgs<R> a)
+{
+    const int e = blockIdx.x * kTPB + threadIdx.x;
+    if (e >= a.Ne) return;
+    R b1, c1, b2, c2, m, w12, w13, w23;
+    Geo<R>::load(a.ga, a.gb, e, b1, c1, b2, c2);
+    elem_coefficients<R>(a.mat, b1, c1, b2, c2, a.area[e], a.H[e], m, w12, w13, w23);
+    Geo<R>::store_global(a.ca, a.cb, e, m, w12, w13, w23);
+}
+
 // setup: r0 = b - A x0, D^-1, lb = d_n, mask, norms (one chunk pass + interface pass).  HOOK: only b / D out.
 // Stage = StageLayout kind 2: lconn | geometry | slots q, D, b (each [3 EC + 1]) | area | H | x [node_len] | gather table
 template <typename R, bool HOOK>
@@ -639,6 +672,11 @@ __global__ void __launch_bounds__(kTPB) dmg_setup_chunk(const DmgArgs<R> a)
         Geo<R>::load_smem(s_geo, e, EC, b1, c1, b2, c2);
         const R Ar = s_area[e], He = s_H[e];
         elem_damage_apply<R>(a.mat, b1, c1, b2, c2, Ar, He, s_x[c.x], s_x[c.y], s_x[c.z], q1, q2, q3);
+        {   // the operator of this solve in coefficient form, streamed by every CG iteration
+            R m, w12, w13, w23;
+            elem_coefficients<R>(a.mat, b1, c1, b2, c2, Ar, He, m, w12, w13, w23);
+            Geo<R>::store_global(a.ca, a.cb, cm.elem_start + e, m, w12, w13, w23);
+        }
         s_sq[e] = q1; s_sq[EC + e] = q2; s_sq[2 * EC + e] = q3;
         const R ce = a.mat.c0 + R(2) * He, se = R(2) * He - a.mat.s0;
         const R m12 = ce * Ar * R(1.0 / 12.0), kA = a.mat.kappa * Ar;
@@ -745,7 +783,7 @@ static DmgArgs<R> make_args(pff_mesh* m, const pff_state* s)
 {
     const HostMesh& hm = m->hm;
     DmgArgs<R> a{};
-    a.meta = m->d_meta; a.lconn = (const ushort4*)m->d_lconn; a.ga = m->d_ga; a.gb = m->d_gb;
+    a.meta = m->d_meta; a.lconn = (const ushort4*)m->d_lconn; a.ga = m->d_ga; a.gb = m->d_gb; a.ca = m->d_ca; a.cb = m->d_cb;
     a.area = (const R*)m->d_area; a.halo_ids = m->d_halo_ids; a.ell = m->d_ell; a.flags = m->d_flags;
     a.halo_part = (R*)m->d_halo_part; a.n_slots = m->n_slots; a.n_entries = m->n_entries; a.ell_total = m->ell_total; a.n_ovf = hm.n_ovf;
     a.EC = hm.chunk_elems;
@@ -772,10 +810,10 @@ static void set_plan(pff_mesh* m, DmgArgs<R>& a, int which, bool proj)
     const uint16_t lr = sizeof(R) == 8 ? 3 : 2;
     auto add = [&](const void* src, uint32_t off, uint16_t l, uint16_t kind) { P.d[P.n++] = StageDesc{src, off, l, kind}; };
     add(m->d_lconn, L.lconn, 3, 0);
-    if (sizeof(R) == 8) { add(m->d_ga, L.geo, 4, 0); add(m->d_gb, L.geo + 16u * (uint32_t)m->hm.chunk_elems, 4, 0); }
-    else add(m->d_ga, L.geo, 4, 0);
-    add(m->d_area, L.area, lr, 0);
-    add(a.H, L.H, lr, 0);
+    const void *g0 = which == 2 ? m->d_ga : m->d_ca, *g1 = which == 2 ? m->d_gb : m->d_cb;  // geometry / coefficients
+    if (sizeof(R) == 8) { add(g0, L.geo, 4, 0); add(g1, L.geo + 16u * (uint32_t)m->hm.chunk_elems, 4, 0); }
+    else add(g0, L.geo, 4, 0);
+    if (which == 2) { add(m->d_area, L.area, lr, 0); add(a.H, L.H, lr, 0); }
     add(m->d_ell, L.ell, 1, 2);
     if (which != 2) {
         add(m->d_halo_dst, L.hdst, 2, 3);   // partial slots of the chunk's halo nodes
@@ -910,6 +948,9 @@ static pff_status damage_matvec_t(pff_mesh* m, const pff_state* s, const void* p
     if ((st = set_smem(dmg_iter_chunk<R, DM_PLAIN, false>, smem_mv, g_mv)) != PFF_OK) return st;
     int grid_mv = 0;
     if ((st = persistent_grid(m, dmg_iter_chunk<R, DM_PLAIN, false>, smem_mv, &grid_mv)) != PFF_OK) return st;
+    if (m->only_kernel < 0) {  // the operator of state->H in coefficient form (timing hook: reuse the previous one)
+        PFF_LAUNCH(m, PFF_K_DAMAGE_SETUP, (dmg_coef_kernel<R><<<(unsigned)((m->hm.Ne + kTPB - 1) / kTPB), kTPB, 0, m->stream>>>(a)));
+    }
     if (m->only_kernel != 3) {
         PFF_LAUNCH(m, PFF_K_MATVEC_CHUNK, (dmg_iter_chunk<R, DM_PLAIN, false><<<(unsigned)grid_mv, kTPB, smem_mv, m->stream>>>(a)));
     }

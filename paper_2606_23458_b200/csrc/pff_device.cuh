@@ -126,6 +126,11 @@ template <> struct Geo<double> {
         const double2 p = g[e], q = g[EC + e];
         b1 = p.x; c1 = p.y; b2 = q.x; c2 = q.y;
     }
+    static __device__ __forceinline__ void store_global(void* ga, void* gb, int e, double v0, double v1, double v2, double v3)
+    {
+        reinterpret_cast<double2*>(ga)[e] = make_double2(v0, v1);
+        reinterpret_cast<double2*>(gb)[e] = make_double2(v2, v3);
+    }
     static __device__ __forceinline__ double2 pair(double x, double y) { return make_double2(x, y); }
     // force-pair slot idx = corner * EC + e: corners 1, 2 overwrite the element's own staged geometry, corner 3 and
     // the zero pair (idx 3 EC) live in the shared slot region
@@ -148,6 +153,10 @@ template <> struct Geo<float> {
     {
         const float4 p = reinterpret_cast<const float4*>(geo)[e];
         b1 = p.x; c1 = p.y; b2 = p.z; c2 = p.w;
+    }
+    static __device__ __forceinline__ void store_global(void* ga, void*, int e, float v0, float v1, float v2, float v3)
+    {
+        reinterpret_cast<float4*>(ga)[e] = make_float4(v0, v1, v2, v3);
     }
     static __device__ __forceinline__ float2 pair(float x, float y) { return make_float2(x, y); }
     static __device__ __forceinline__ float2* slot(unsigned char*, unsigned char* shared_slots, int idx, int)

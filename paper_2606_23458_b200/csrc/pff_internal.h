@@ -50,8 +50,8 @@ inline StageLayout make_stage_layout(int kind, int EC, int node_len, int flag_le
     uint32_t o = 0;
     L.lconn = o; o += up16(size_t(8) * EC);
     L.geo = o; o += up16(size_t(4) * rb * EC);
-    L.area = o; o += up16(rb * EC);
-    L.H = o; o += up16(rb * EC);
+    L.area = o; o += up16(kind == 1 ? 0 : rb * EC);  // kind 1 stages the 4 element-operator coefficients as "geometry"
+    L.H = o; o += up16(kind == 1 ? 0 : rb * EC);
     const int nn = kind == 0 ? 10 : (kind == 1 ? 6 : 1);
     for (int k = 0; k < nn; ++k) { L.node[k] = o; o += up16(rb * node_len); }
     L.flags = o; o += up16(kind == 2 ? 0 : flag_len);

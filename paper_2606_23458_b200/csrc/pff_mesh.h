@@ -46,6 +46,9 @@ struct pff_mesh {
 
     // damage solve workspaces (reals [N] unless noted)
     void *d_lb = nullptr, *d_r = nullptr, *d_p = nullptr, *d_q = nullptr, *d_dinv = nullptr;
+    // element operator of the current solve, 4 reals per element (mass coefficient m_e and the three edge weights w_12,
+    // w_13, w_23 of the P1 stiffness): fp64 two double2 streams, fp32 one float4 stream (written by the setup pass)
+    void *d_ca = nullptr, *d_cb = nullptr;
     uint8_t* d_mask = nullptr;   // [N] bit0: in the free set, bit1: damage-Dirichlet
     double* d_part = nullptr;    // chunk-kernel block partials [channels][n_part_blocks]
     double* d_part2 = nullptr;   // interface-kernel block partials
