@@ -84,13 +84,15 @@ pff_status build_host_mesh(int64_t N, const double* xy, int64_t Ne, const int32_
     hm.elem_new_of_old.resize(Ne);
     for (int64_t e = 0; e < Ne; ++e) hm.elem_new_of_old[elem_old_of_new[e]] = int32_t(e);
 
-    // ---- chunks; shrink the chunk until the worst-case shared-memory footprint of every chunk kernel fits
-    // (default chunk: three resident CTAs per SM; explicit chunk: one CTA)
+    // ---- chunks; shrink the chunk until the shared-memory footprints of the chunk kernels fit.  Default chunk: the
+    // largest size for which THREE double-buffered CTAs of the CG kernel (12 of 13 launches-worth of work per step)
+    // and TWO of the step / setup kernels fit one SM (measured best, profiles/r1c); explicit chunk: one CTA of each.
     const int A = int(16 / real_bytes);  // reals per 16-byte TMA granule
     const bool user_chunk = chunk_elems > 0;
     int EC = user_chunk ? chunk_elems : (real_bytes == 8 ? 512 : 1024);
     EC = std::max(32, std::min(8192, (EC / 32) * 32));
-    const size_t smem_limit = (user_chunk ? kSmemPerSM : kSmemPerSM / 3) - kSmemCtaReserve;
+    const size_t limit_cg = (user_chunk ? kSmemPerSM : kSmemPerSM / 3) - kSmemCtaReserve;
+    const size_t limit_other = (user_chunk ? kSmemPerSM : kSmemPerSM / 2) - kSmemCtaReserve;
     std::vector<int32_t> cmin(N), cmax(N);
     for (;;) {
         std::fill(cmin.begin(), cmin.end(), std::numeric_limits<int32_t>::max());
@@ -119,16 +121,19 @@ pff_status build_host_mesh(int64_t N, const double* xy, int64_t Ne, const int32_
         }
         const int node_len_b = (max_nloc + 2 * A + A - 1) / A * A, flag_len_b = (max_nloc + 32 + 15) / 16 * 16;
         const int ell_len_b = (max_ell + 7) / 8 * 8;
-        size_t smem = 0;  // dynamic + static shared memory of the most demanding chunk kernel (the step kernel has no static part)
-        for (int kind = 0; kind < 3; ++kind)
-            smem = std::max(smem, chunk_smem_bytes(kind, EC, node_len_b, flag_len_b, ell_len_b, max_nh, real_bytes) +
-                                      (kind == 0 ? 0 : kSmemStatic));
-        if ((smem <= smem_limit && max_nloc < 16384) || EC <= 32) {
-            if (smem > kSmemPerSM - kSmemCtaReserve) { err = "chunk does not fit shared memory"; return PFF_EMESH; }
+        // dynamic + static shared memory per kernel (the step kernel has no static part)
+        const size_t smem_step = chunk_smem_bytes(0, EC, node_len_b, flag_len_b, ell_len_b, max_nh, real_bytes);
+        const size_t smem_cg = chunk_smem_bytes(1, EC, node_len_b, flag_len_b, ell_len_b, max_nh, real_bytes) + kSmemStatic;
+        const size_t smem_su = chunk_smem_bytes(2, EC, node_len_b, flag_len_b, ell_len_b, max_nh, real_bytes) + kSmemStatic;
+        const bool fits = smem_cg <= limit_cg && std::max(smem_step, smem_su) <= limit_other && max_nloc < 16384;
+        if (fits || EC <= 32) {
+            if (std::max(smem_cg, std::max(smem_step, smem_su)) > kSmemPerSM - kSmemCtaReserve) {
+                err = "chunk does not fit shared memory"; return PFF_EMESH;
+            }
             hm.max_nloc = max_nloc; hm.C = C;
             break;
         }
-        EC = std::max(32, (EC * 7 / 8 / 32) * 32);  // 512, 448, 384, 320, 256, 224, 192, 160, 128, 96, 64, 32
+        EC -= EC > 512 ? 64 : 32;  // 1024, 960, ..., 512, 480, 448, ..., 32
     }
     hm.chunk_elems = EC;
     const int64_t C = hm.C;
