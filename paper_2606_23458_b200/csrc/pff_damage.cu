@@ -632,88 +632,143 @@ __global__ void __launch_bounds__(kTPB) dmg_coef_kernel(const DmgArgs<R> a)
     Geo<R>::store_global(a.ca, a.cb, e, m, w12, w13, w23);
 }
 
-// setup: r0 = b - A x0, D^-1, lb = d_n, mask, norms (one chunk pass + interface pass).  HOOK: only b / D out.
-// Stage = StageLayout kind 2: lconn | geometry | slots q, D, b (each [3 EC + 1]) | area | H | x [node_len] | gather table
+// setup: r0 = b - A x0, D^-1, lb = d_n, mask, operator coefficients, norms (chunk pass + interface pass).  HOOK: only
+// b / D out.  PERSISTENT and double-buffered like the step and CG kernels (same pipeline: TMA burst + cp.async halo
+// gathers of chunk k + 1 while chunk k is computed).  Stage = StageLayout kind 2: lconn | geometry | area | H |
+// x [node_len] | gather table | halo ids / partial slots; shared by both stages: slots q, D, b (each [3 EC + 1]).
 template <typename R, bool HOOK>
-__global__ void __launch_bounds__(kTPB) dmg_setup_chunk(const DmgArgs<R> a)
+__global__ void __launch_bounds__(kTPB, 2) dmg_setup_chunk(const DmgArgs<R> a)
 {
     extern __shared__ __align__(128) unsigned char smem[];
     __shared__ double s_w[kCh * 32], s_out[kCh];
-    constexpr int A = 16 / sizeof(R);
+    constexpr int A = 16 / sizeof(R), B = sizeof(R);
     const StageLayout& L = a.lay;
-    const ushort4* s_lconn = reinterpret_cast<const ushort4*>(smem + L.lconn);
-    const unsigned char* s_geo = smem + L.geo;
     R* s_sq = reinterpret_cast<R*>(smem + L.slot_base);
     R* s_sD = reinterpret_cast<R*>(smem + L.slot_base + L.slot_stride);
     R* s_sb = reinterpret_cast<R*>(smem + L.slot_base + 2 * L.slot_stride);
-    const R* s_area = reinterpret_cast<const R*>(smem + L.area);
-    const R* s_H = reinterpret_cast<const R*>(smem + L.H);
-    R* s_x = reinterpret_cast<R*>(smem + L.node[0]);
-    const uint16_t* s_ell = reinterpret_cast<const uint16_t*>(smem + L.ell);
+    ChunkMeta* s_meta = reinterpret_cast<ChunkMeta*>(smem + L.meta);
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem + L.bar);
-    const int tid = threadIdx.x, EC = a.EC;
-    const ChunkMeta cm = a.meta[blockIdx.x];
-    if (tid == 0) { mbar_init(bar, 2); s_sq[3 * EC] = R(0); s_sD[3 * EC] = R(0); s_sb[3 * EC] = R(0); }
-    __syncthreads();
-    if (tid < 32)
-        stage_issue_plan(a.plan, smem, bar, tid, 1, blockIdx.x * EC, min(EC, a.Ne - blockIdx.x * EC), a.Ne, 0, 0, a.N, 0, 0, 0);
-    const int nloc = cm.n_int + cm.n_halo;
-    const int shift = cm.node_start & (A - 1), hb = (shift + cm.n_int + A - 1) & ~(A - 1);
-    if (tid < 32)
-        stage_issue_plan(a.plan, smem, bar, tid, 2, 0, 0, a.Ne, cm.node_start, cm.n_int, a.N, cm.ell_off, cm.ell_w * nloc,
-                         (int)a.ell_total);
-    for (int j = tid; j < cm.n_halo; j += kTPB) s_x[hb + j] = a.x[__ldg(a.halo_ids + cm.halo_off + j)];
-    mbar_wait(bar, 0);
-    __syncthreads();
+    const int tid = threadIdx.x, lane = tid & 31, G = gridDim.x, EC = a.EC;
+    const int n_my = (a.C - (int)blockIdx.x + G - 1) / G;
+    const bool issuer = tid >= kTPB - 32;
+    const bool have_desc = issuer && lane < a.plan.n;
+    StageDesc my_desc{};
+    if (have_desc) my_desc = a.plan.d[lane];
+    const int gj = kTPB - 1 - tid;  // halo node whose gather this thread issues
 
-    for (int e = tid; e < cm.n_elem; e += kTPB) {
-        const ushort4 c = s_lconn[e];
-        R b1, c1, b2, c2, q1, q2, q3;
-        Geo<R>::load_smem(s_geo, e, EC, b1, c1, b2, c2);
-        const R Ar = s_area[e], He = s_H[e];
-        elem_damage_apply<R>(a.mat, b1, c1, b2, c2, Ar, He, s_x[c.x], s_x[c.y], s_x[c.z], q1, q2, q3);
-        {   // the operator of this solve in coefficient form, streamed by every CG iteration
-            R m, w12, w13, w23;
-            elem_coefficients<R>(a.mat, b1, c1, b2, c2, Ar, He, m, w12, w13, w23);
-            Geo<R>::store_global(a.ca, a.cb, cm.elem_start + e, m, w12, w13, w23);
-        }
-        s_sq[e] = q1; s_sq[EC + e] = q2; s_sq[2 * EC + e] = q3;
-        const R ce = a.mat.c0 + R(2) * He, se = R(2) * He - a.mat.s0;
-        const R m12 = ce * Ar * R(1.0 / 12.0), kA = a.mat.kappa * Ar;
-        const R b3 = -(b1 + b2), c3 = -(c1 + c2);
-        s_sD[e] = R(2) * m12 + kA * (b1 * b1 + c1 * c1);  // A_ii = c A/6 + kappa A |grad phi_i|^2
-        s_sD[EC + e] = R(2) * m12 + kA * (b2 * b2 + c2 * c2);
-        s_sD[2 * EC + e] = R(2) * m12 + kA * (b3 * b3 + c3 * c3);
-        const R be = se * Ar * R(1.0 / 3.0);  // int s phi_i
-        s_sb[e] = be; s_sb[EC + e] = be; s_sb[2 * EC + e] = be;
+    if (tid == 0) {
+        mbar_init(bar, 1 + kTPB); mbar_init(bar + 2, 1 + kTPB);
+        s_sq[3 * EC] = R(0); s_sD[3 * EC] = R(0); s_sb[3 * EC] = R(0);
     }
-    __syncthreads();
     double acc[kCh];
 #pragma unroll
     for (int c = 0; c < kCh; ++c) acc[c] = 0.0;
-    for (int i = tid; i < nloc; i += kTPB) {
-        R qs = R(0), Ds = R(0), bs = R(0);
-        const uint16_t* row = s_ell + i;
-        for (int k = 0; k < cm.ell_w; ++k) {
-            const int idx = row[k * nloc];
-            qs += s_sq[idx]; Ds += s_sD[idx]; bs += s_sb[idx];
-        }
-        if (i < cm.n_int) {
-            const int gid = cm.node_start + i;
-            if (HOOK) {
-                if (a.b_out) a.b_out[gid] = bs;
-                if (a.D_out) a.D_out[gid] = Ds;
-            } else {
-                const R r = bs - qs;
-                const bool fixed = (a.flags[gid] & 4) != 0;
-                a.r[gid] = r; a.dinv[gid] = R(1) / Ds; a.lb[gid] = s_x[shift + i];
-                a.mask[gid] = fixed ? 2 : 1;
-                acc[0] += double(bs) * double(bs);
-                if (!fixed) acc[1] += double(r) * double(r);
+    int it = 0;
+    for (int e0 = 0; e0 < n_my; e0 += kMetaCap) {
+        const int n_ep = min(kMetaCap, n_my - e0);
+        __syncthreads();
+        if (tid < n_ep) s_meta[tid] = a.meta[blockIdx.x + (e0 + tid) * G];
+        __syncthreads();
+        {   // epoch prologue: first chunk with exposed latency
+            const ChunkMeta cm = s_meta[0];
+            unsigned char* stg = smem + (it & 1) * L.stage_bytes;
+            if (issuer) {
+                const ChunkRange cr{cm.elem_start, cm.n_elem, a.Ne, cm.node_start, cm.n_int, a.N, cm.ell_off,
+                                    cm.ell_w * (cm.n_int + cm.n_halo), (int)a.ell_total, cm.halo_off, cm.n_halo, (int)a.n_entries,
+                                    n_ep > 1 ? s_meta[1].halo_off : 0, n_ep > 1 ? s_meta[1].n_halo : 0};
+                fence_proxy_async();
+                stage_issue_desc(my_desc, have_desc, stg, bar + 2 * (it & 1), lane, cr);
             }
-        } else {
-            const int slot = __ldg(a.halo_dst + cm.halo_off + i - cm.n_int);
-            a.halo_part[slot] = qs; a.halo_part[a.n_slots + slot] = Ds; a.halo_part[2 * a.n_slots + slot] = bs;
+            if (gj < cm.n_halo) {
+                const int hb0 = ((cm.node_start & (A - 1)) + cm.n_int + A - 1) & ~(A - 1);
+                cp_async<B>(reinterpret_cast<R*>(stg + L.node[0]) + hb0 + gj, a.x + __ldg(a.halo_ids + cm.halo_off + gj));
+            }
+            cp_async_mbar_arrive(bar + 2 * (it & 1));
+        }
+        for (int k = 0; k < n_ep; ++k, ++it) {
+            const int st = it & 1;
+            unsigned char* stg = smem + st * L.stage_bytes;
+            const ushort4* s_lconn = reinterpret_cast<const ushort4*>(stg + L.lconn);
+            const unsigned char* s_geo = stg + L.geo;
+            const R* s_area = reinterpret_cast<const R*>(stg + L.area);
+            const R* s_H = reinterpret_cast<const R*>(stg + L.H);
+            R* s_x = reinterpret_cast<R*>(stg + L.node[0]);
+            const uint16_t* s_ell = reinterpret_cast<const uint16_t*>(stg + L.ell);
+            const ChunkMeta cm = s_meta[k];
+            const int nloc = cm.n_int + cm.n_halo;
+            const int shift = cm.node_start & (A - 1), hb = (shift + cm.n_int + A - 1) & ~(A - 1), fshift = cm.node_start & 15;
+            const int* s_hdst = reinterpret_cast<const int*>(stg + L.hdst) + (cm.halo_off & 3);
+            const uint8_t* s_flags = stg + L.flags;
+
+            mbar_wait(bar + 2 * st, (it >> 1) & 1);
+            if (k + 1 < n_ep) {  // prefetch chunk k + 1 (its halo ids arrived with this stage)
+                const ChunkMeta cn = s_meta[k + 1];
+                unsigned char* stn = smem + (st ^ 1) * L.stage_bytes;
+                if (issuer) {
+                    const ChunkRange cr{cn.elem_start, cn.n_elem, a.Ne, cn.node_start, cn.n_int, a.N, cn.ell_off,
+                                        cn.ell_w * (cn.n_int + cn.n_halo), (int)a.ell_total, cn.halo_off, cn.n_halo, (int)a.n_entries,
+                                        k + 2 < n_ep ? s_meta[k + 2].halo_off : 0, k + 2 < n_ep ? s_meta[k + 2].n_halo : 0};
+                    fence_proxy_async();
+                    stage_issue_desc(my_desc, have_desc, stn, bar + 2 * (st ^ 1), lane, cr);
+                }
+                if (gj < cn.n_halo) {
+                    const int hbn = ((cn.node_start & (A - 1)) + cn.n_int + A - 1) & ~(A - 1);
+                    const int gid = reinterpret_cast<const int*>(stg + L.hnext)[(cn.halo_off & 3) + gj];
+                    cp_async<B>(reinterpret_cast<R*>(stn + L.node[0]) + hbn + gj, a.x + gid);
+                }
+                cp_async_mbar_arrive(bar + 2 * (st ^ 1));
+            }
+            for (int j = tid + kTPB; j < cm.n_halo; j += kTPB) s_x[hb + j] = a.x[__ldg(a.halo_ids + cm.halo_off + j)];
+            if (cm.n_halo > kTPB) __syncthreads();
+
+            for (int e = tid; e < cm.n_elem; e += kTPB) {
+                const ushort4 c = s_lconn[e];
+                R b1, c1, b2, c2, q1, q2, q3;
+                Geo<R>::load_smem(s_geo, e, EC, b1, c1, b2, c2);
+                const R Ar = s_area[e], He = s_H[e];
+                elem_damage_apply<R>(a.mat, b1, c1, b2, c2, Ar, He, s_x[c.x], s_x[c.y], s_x[c.z], q1, q2, q3);
+                {   // the operator of this solve in coefficient form, streamed by every CG iteration
+                    R m, w12, w13, w23;
+                    elem_coefficients<R>(a.mat, b1, c1, b2, c2, Ar, He, m, w12, w13, w23);
+                    Geo<R>::store_global(a.ca, a.cb, cm.elem_start + e, m, w12, w13, w23);
+                }
+                s_sq[e] = q1; s_sq[EC + e] = q2; s_sq[2 * EC + e] = q3;
+                const R ce = a.mat.c0 + R(2) * He, se = R(2) * He - a.mat.s0;
+                const R m12 = ce * Ar * R(1.0 / 12.0), kA = a.mat.kappa * Ar;
+                const R b3 = -(b1 + b2), c3 = -(c1 + c2);
+                s_sD[e] = R(2) * m12 + kA * (b1 * b1 + c1 * c1);  // A_ii = c A/6 + kappa A |grad phi_i|^2
+                s_sD[EC + e] = R(2) * m12 + kA * (b2 * b2 + c2 * c2);
+                s_sD[2 * EC + e] = R(2) * m12 + kA * (b3 * b3 + c3 * c3);
+                const R be = se * Ar * R(1.0 / 3.0);  // int s phi_i
+                s_sb[e] = be; s_sb[EC + e] = be; s_sb[2 * EC + e] = be;
+            }
+            __syncthreads();
+            for (int i = tid; i < nloc; i += kTPB) {
+                R qs = R(0), Ds = R(0), bs = R(0);
+                const uint16_t* row = s_ell + i;
+                for (int w = 0; w < cm.ell_w; ++w) {
+                    const int idx = row[w * nloc];
+                    qs += s_sq[idx]; Ds += s_sD[idx]; bs += s_sb[idx];
+                }
+                if (i < cm.n_int) {
+                    const int gid = cm.node_start + i;
+                    if (HOOK) {
+                        if (a.b_out) a.b_out[gid] = bs;
+                        if (a.D_out) a.D_out[gid] = Ds;
+                    } else {
+                        const R r = bs - qs;
+                        const bool fixed = (s_flags[fshift + i] & 4) != 0;
+                        a.r[gid] = r; a.dinv[gid] = R(1) / Ds; a.lb[gid] = s_x[shift + i];
+                        a.mask[gid] = fixed ? 2 : 1;
+                        acc[0] += double(bs) * double(bs);
+                        if (!fixed) acc[1] += double(r) * double(r);
+                    }
+                } else {
+                    const int slot = s_hdst[i - cm.n_int];
+                    a.halo_part[slot] = qs; a.halo_part[a.n_slots + slot] = Ds; a.halo_part[2 * a.n_slots + slot] = bs;
+                }
+            }
+            __syncthreads();  // stage st and the slots are free again
         }
     }
     if (!HOOK) {
@@ -815,10 +870,8 @@ static void set_plan(pff_mesh* m, DmgArgs<R>& a, int which, bool proj)
     else add(g0, L.geo, 4, 0);
     if (which == 2) { add(m->d_area, L.area, lr, 0); add(a.H, L.H, lr, 0); }
     add(m->d_ell, L.ell, 1, 2);
-    if (which != 2) {
-        add(m->d_halo_dst, L.hdst, 2, 3);   // partial slots of the chunk's halo nodes
-        add(m->d_halo_ids, L.hnext, 2, 4);  // ids of the next chunk's halo nodes
-    }
+    add(m->d_halo_dst, L.hdst, 2, 3);   // partial slots of the chunk's halo nodes
+    add(m->d_halo_ids, L.hnext, 2, 4);  // ids of the next chunk's halo nodes
     if (which == 0) {
         add(a.x, L.node[0], lr, 1); add(a.r, L.node[1], lr, 1); add(a.p, L.node[2], lr, 1); add(a.q, L.node[3], lr, 1);
         add(a.dinv, L.node[4], lr, 1);
@@ -828,6 +881,7 @@ static void set_plan(pff_mesh* m, DmgArgs<R>& a, int which, bool proj)
         add(a.p_in, L.node[2], lr, 1);
     } else {
         add(a.x, L.node[0], lr, 1);
+        add(m->d_flags, L.flags, 0, 1);
     }
 }
 
@@ -900,7 +954,14 @@ static pff_status damage_solve_t(pff_mesh* m, pff_state* s, double rel_tol, int 
     h[0].tol = rel_tol; h[0].max_iter = max_iter; h[0].first = 1; h[0].restart = 1; h[0].status = PFF_ENOCONV;
     if ((st = cuda_check(cudaMemcpyAsync(m->d_ctrl, &h[0], sizeof(DamageCtrl), cudaMemcpyHostToDevice, cs), "damage: ctrl upload")) != PFF_OK) return st;
     const unsigned gs = shared_grid(hm);
-    PFF_LAUNCH(m, PFF_K_DAMAGE_SETUP, (dmg_setup_chunk<R, false><<<(unsigned)hm.C, kTPB, smem_su, cs>>>(asu)));
+    static int grid_su = 0, grid_su_smem = -1;
+    if (grid_su_smem != smem_su) {
+        if ((st = persistent_grid(m, dmg_setup_chunk<R, false>, smem_su, &grid_su)) != PFF_OK) return st;
+        grid_su_smem = smem_su;
+    }
+    const unsigned gsu = (unsigned)std::min<int64_t>(grid_su, hm.C);
+    asu.n_chunk_blocks = (int)gsu;
+    PFF_LAUNCH(m, PFF_K_DAMAGE_SETUP, (dmg_setup_chunk<R, false><<<gsu, kTPB, smem_su, cs>>>(asu)));
     PFF_LAUNCH(m, PFF_K_DAMAGE_SETUP, (dmg_setup_shared<R, false><<<gs, kTPB, 0, cs>>>(asu)));
     // ONE cooperative launch runs every CG iteration (grid-wide barriers between the chunk phase, the interface
     // phase and the scalar recurrence), applies the last step and the clamp, and writes the control block back
@@ -976,7 +1037,9 @@ static pff_status damage_rhs_diag_t(pff_mesh* m, const pff_state* s, void* b, vo
     const int smem_su = (int)m->lay_su.total;
     static int g_su = 0;
     if ((st = set_smem(dmg_setup_chunk<R, true>, smem_su, g_su)) != PFF_OK) return st;
-    PFF_LAUNCH(m, PFF_K_DAMAGE_SETUP, (dmg_setup_chunk<R, true><<<(unsigned)m->hm.C, kTPB, smem_su, m->stream>>>(a)));
+    int grid_su = 0;
+    if ((st = persistent_grid(m, dmg_setup_chunk<R, true>, smem_su, &grid_su)) != PFF_OK) return st;
+    PFF_LAUNCH(m, PFF_K_DAMAGE_SETUP, (dmg_setup_chunk<R, true><<<(unsigned)grid_su, kTPB, smem_su, m->stream>>>(a)));
     PFF_LAUNCH(m, PFF_K_DAMAGE_SETUP, (dmg_setup_shared<R, true><<<shared_grid(m->hm), kTPB, 0, m->stream>>>(a)));
     return cuda_check(cudaGetLastError(), "damage rhs/diag launch");
 }

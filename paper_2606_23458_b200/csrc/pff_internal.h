@@ -54,7 +54,7 @@ inline StageLayout make_stage_layout(int kind, int EC, int node_len, int flag_le
     L.H = o; o += up16(kind == 1 ? 0 : rb * EC);
     const int nn = kind == 0 ? 10 : (kind == 1 ? 6 : 1);
     for (int k = 0; k < nn; ++k) { L.node[k] = o; o += up16(rb * node_len); }
-    L.flags = o; o += up16(kind == 2 ? 0 : flag_len);
+    L.flags = o; o += up16(flag_len);
     L.ell = o; o += up16(size_t(2) * ell_len);
     L.hids = o; o += up16(size_t(4) * max_nhalo);
     L.hflag = o; o += up16(size_t(4) * max_nhalo);
@@ -74,8 +74,8 @@ inline StageLayout make_stage_layout(int kind, int EC, int node_len, int flag_le
     L.total = o;
     return L;
 }
-// stages of each chunk kernel: the step and CG kernels are persistent and double-buffered
-inline int chunk_kernel_stages(int kind) { return kind == 2 ? 1 : 2; }
+// stages of each chunk kernel: all three (step, CG, damage setup) are persistent and double-buffered
+inline int chunk_kernel_stages(int) { return 2; }
 inline size_t chunk_smem_bytes(int kind, int EC, int node_len, int flag_len, int ell_len, int max_nhalo, size_t rb)
 {
     return make_stage_layout(kind, EC, node_len, flag_len, ell_len, max_nhalo, rb, chunk_kernel_stages(kind)).total;
