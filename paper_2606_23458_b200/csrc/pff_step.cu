@@ -127,7 +127,7 @@ __device__ __forceinline__ void step_halo_gather(const StepArgs<R>& a, const Sta
 // thread's cp.async arrival.  Per chunk: predictor (Eq. 16) -> fused element pass (strain, split, degradation,
 // stress, force, history) -> ordered gather + Eq. 17-18.  Stage = StageLayout kind 0 (pff_internal.h).
 template <typename R, int SPLIT, int MODE>
-__global__ void __launch_bounds__(kTPB, 3) step_chunk_kernel(const StepArgs<R> a)
+__global__ void __launch_bounds__(kTPB, 2) step_chunk_kernel(const StepArgs<R> a)
 {
     extern __shared__ __align__(128) unsigned char smem[];
     typedef typename Geo<R>::Pair Pair;
