@@ -1,20 +1,23 @@
 // Damage sub-problem (Eq. 6-8): matrix-free operator with consistent mass,
 // Jacobi-preconditioned CG (AT2, then clamp, L179) and projected CG with an active set (AT1, L181).
 //
-// ONE chunk kernel + one small interface kernel per CG iteration:
-//   dmg_iter_chunk   one CTA per chunk.  Every contiguous array of the chunk is streamed into shared memory
-//                    by TMA.  Prologue per node: apply the PREVIOUS iteration's step (x += alpha p,
-//                    r -= alpha q), re-derive the free set on a restart, form the new direction
-//                    p = z + beta p (z = D^-1 r on the free set).  Then the element pass
-//                    q^e = (c_e M^e + kappa K^e) p^e, the ordered node gather, and the block partials of
-//                    p.q, r.z, r.r and of the four sums that PREDICT r.z and r.r after the coming step
-//                    (z.q, q.D^-1 q, r.q, q.q), so that beta is known without another pass over the vectors.
-//   dmg_iter_shared  interface nodes (same prologue, ordered sum of the chunk partials); its blocks fold the
-//                    chunk partials in a fixed order and the last block sets alpha, beta, the restart /
-//                    truncation / convergence flags in the device-resident control block.
-// alpha, beta, norms never leave the device; the host polls the control block every few iterations.
-// Convergence is declared on the TRUE residual norm, or on the predicted one when its rounding error bound
-// is far below the tolerance (AT2); the pending last step is then applied by dmg_finalize.
+// pff_damage_solve = dmg_setup_chunk + dmg_setup_shared + ONE cooperative launch of dmg_iter_chunk<DM_CG>
+// (DESIGN.md "Damage solve"):
+//   dmg_setup_chunk   persistent, TMA-fed: rhs b, Jacobi diagonal, r0 = b - A d_n, lb = d_n, free-set mask, the
+//                     element operator in coefficient form (4 reals per element) and the block partials of the norms.
+//   dmg_setup_shared  the same for the interface nodes; its last block sets ||b||, ||r0|| in the control block.
+//   dmg_iter_chunk    persistent + cooperative: runs EVERY CG iteration.  Per iteration: chunk phase (double-buffered
+//                     TMA stages, cp.async halo gathers one chunk ahead; node prologue applies the PREVIOUS step
+//                     x += alpha p, r -= alpha q, re-derives the free set on a restart and forms p = z + beta p;
+//                     element pass q^e = (c_e M^e + kappa K^e) p^e; ordered node gather; partial sums of p.q, r.z,
+//                     r.r and of the four sums that PREDICT r.z and r.r after the coming step, so beta is known
+//                     without another pass over the vectors), grid barrier, interface phase, grid barrier, then
+//                     every CTA reduces the block partials in the same fixed order and advances its own copy of
+//                     alpha, beta and the restart / truncation / convergence flags.  After the last iteration the
+//                     same kernel applies the pending step and the clamp d <- min(1, max(d_n, d)) (L179).
+// alpha, beta and the norms never leave the device; the host reads one 128-byte control block per solve.
+// Convergence is declared on the TRUE residual norm, or (AT2) on the predicted one when its rounding error bound
+// is far below the tolerance.
 #include <algorithm>
 #include <cstring>
 
@@ -573,51 +576,12 @@ __device__ __forceinline__ bool fold_and_finish(const double* part, int64_t part
     return true;
 }
 
-template <typename R, int MODE, bool PROJ>
-__global__ void __launch_bounds__(kTPB) dmg_iter_shared(const DmgArgs<R> a)
+// interface nodes of a plain operator apply (test hook pff_damage_matvec): ordered sum of the chunk partials
+template <typename R>
+__global__ void __launch_bounds__(kTPB) dmg_plain_shared(const DmgArgs<R> a)
 {
-    __shared__ double s_w[kCh * 32], s_out[kCh];
-    IterScalars sc{0.0, 0.0, 1, 1, 0};
-    if (MODE == DM_CG) {
-        const DamageCtrl* c = a.ctrl;
-        if (c->done) return;
-        sc.alpha = c->alpha; sc.beta = c->beta; sc.first = c->first; sc.restart = c->restart; sc.trunc = c->trunc;
-    }
-    double acc[kCh];
-#pragma unroll
-    for (int c = 0; c < kCh; ++c) acc[c] = 0.0;
-    acc[kCh - 1] = INFINITY;
-    for (int s = blockIdx.x * kTPB + threadIdx.x; s < a.N_sh; s += gridDim.x * kTPB) {
-        const int gid = a.N_int + s;
-        const R qs = iface_sum<R>(a.halo_part, s, a.N_sh, a.n_ovf, a.sh_rowptr);
-        if (MODE == DM_CG) {
-            R x = R(0), r = a.r[gid], p = R(0), q = R(0), lb = R(0);
-            const R dinv = a.dinv[gid];
-            uint8_t mk = a.mask[gid];
-            const uint8_t mk0 = mk;
-            if (!sc.first) { x = a.x[gid]; p = a.p[gid]; q = a.q[gid]; }
-            if (PROJ) { if (sc.first) x = a.x[gid]; lb = a.lb[gid]; }
-            const R pn = cg_node_prologue<R, PROJ>(sc, x, r, p, q, dinv, lb, mk);
-            if (!sc.first) { if (mk0 & 1) a.x[gid] = x; a.r[gid] = r; }
-            if (mk != mk0) a.mask[gid] = mk;
-            a.p[gid] = pn; a.q[gid] = qs;
-            const double qd = double(qs);
-            acc[0] += double(pn) * qd;
-            if (mk & 1) {
-                const double rd = double(r), dv = double(dinv);
-                acc[1] += rd * rd * dv; acc[2] += rd * rd;
-                acc[3] += rd * dv * qd; acc[4] += dv * qd * qd; acc[5] += rd * qd; acc[6] += qd * qd;
-                if (PROJ && pn < R(0)) acc[kCh - 1] = fmin(acc[kCh - 1], (double(lb) - double(x)) / double(pn));
-            }
-        } else {
-            a.q_out[gid] = qs;
-        }
-    }
-    if (MODE != DM_CG) return;
-    block_reduce_ch(acc, s_w, s_out);
-    double t[kCh];
-    if (fold_and_finish(a.part, a.part_n, a.n_chunk_blocks, a.part2, a.ticket, s_w, s_out, t) && threadIdx.x == 0)
-        cg_scalar_step<PROJ>(a.ctrl, t);
+    for (int s = blockIdx.x * kTPB + threadIdx.x; s < a.N_sh; s += gridDim.x * kTPB)
+        a.q_out[a.N_int + s] = iface_sum<R>(a.halo_part, s, a.N_sh, a.n_ovf, a.sh_rowptr);
 }
 
 // operator coefficients from the geometry and the current history field (hook path: the solve gets them from the setup pass)
@@ -809,30 +773,6 @@ __global__ void __launch_bounds__(kTPB) dmg_setup_shared(const DmgArgs<R> a)
         a.ctrl->nb = fmax(fmax(sqrt(t[0]), sqrt(t[1])), 1e-300);
 }
 
-// applies the pending last step (if any), then d <- min(1, max(d_n, x)) on the non-Dirichlet nodes (L179)
-template <typename R, bool PROJ>
-__global__ void __launch_bounds__(kTPB) dmg_finalize(const DmgArgs<R> a)
-{
-    const DamageCtrl* c = a.ctrl;
-    const bool pending = c->pending != 0;
-    IterScalars sc{c->alpha, 0.0, 0, 0, c->trunc};
-    for (int i = blockIdx.x * kTPB + threadIdx.x; i < a.N; i += gridDim.x * kTPB) {
-        const uint8_t mk = a.mask[i];
-        if (mk & 2) continue;
-        R v = a.x[i];
-        const R l = a.lb[i];
-        if (pending && (mk & 1)) {
-            const R p = a.p[i];
-            R xn = rfma(R(sc.alpha), p, v);
-            if (PROJ && sc.trunc && p < R(0) && (double(l) - double(v)) / double(p) <= sc.alpha * (1.0 + 1e-12)) xn = l;
-            v = xn;
-        }
-        if (v < l) v = l;
-        if (v > R(1)) v = R(1);
-        a.x[i] = v;
-    }
-}
-
 template <typename R>
 static DmgArgs<R> make_args(pff_mesh* m, const pff_state* s)
 {
@@ -1016,7 +956,7 @@ static pff_status damage_matvec_t(pff_mesh* m, const pff_state* s, const void* p
         PFF_LAUNCH(m, PFF_K_MATVEC_CHUNK, (dmg_iter_chunk<R, DM_PLAIN, false><<<(unsigned)grid_mv, kTPB, smem_mv, m->stream>>>(a)));
     }
     if (m->only_kernel != 2) {
-        PFF_LAUNCH(m, PFF_K_MATVEC_SHARED, (dmg_iter_shared<R, DM_PLAIN, false><<<shared_grid(m->hm), kTPB, 0, m->stream>>>(a)));
+        PFF_LAUNCH(m, PFF_K_MATVEC_SHARED, (dmg_plain_shared<R><<<shared_grid(m->hm), kTPB, 0, m->stream>>>(a)));
     }
     return cuda_check(cudaGetLastError(), "damage matvec launch");
 }

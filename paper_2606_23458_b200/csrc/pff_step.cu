@@ -1,11 +1,13 @@
 // Explicit step kernels (Eq. 16-18; element math L42, L71-93, L124):
 //
-//   step_chunk_kernel   one CTA per chunk of elements.  Phase 1 forms the predictor u_{n+1} (Eq. 16) of all
-//                       nodes the chunk touches and stages it with d in shared memory; phase 2 is the fused
-//                       element pass (strain -> split -> degradation -> stress -> force -> history) writing
-//                       element forces to shared-memory slots; phase 3 gathers each node's incident slots
-//                       in a fixed order (chunk-local ELL table) and, for interior nodes, completes Eq. 17-18
-//                       in the same kernel -- f_int never reaches HBM.  Interface nodes get a partial sum.
+//   step_chunk_kernel   PERSISTENT CTAs, each owning every G-th chunk of elements; two shared-memory stages: the
+//                       contiguous arrays of chunk k + 1 stream in by TMA (cp.async.bulk) and its halo nodes by
+//                       cp.async while chunk k is computed.  Phase 1 forms the predictor u_{n+1} (Eq. 16) of all
+//                       nodes the chunk touches in place in the stage; phase 2 is the fused element pass
+//                       (strain -> split -> degradation -> stress -> force -> history) writing element forces
+//                       to shared-memory slots; phase 3 gathers each node's incident slots in a fixed order
+//                       (chunk-local ELL table) and, for interior nodes, completes Eq. 17-18 in the same
+//                       kernel -- f_int never reaches HBM.  Interface nodes get one partial sum per chunk.
 //   step_shared_kernel  interface nodes: ordered sum of the per-chunk partials, then the same Eq. 16-18.
 //   elem_atomic_kernel / node_atomic_kernel   PFF_SCATTER_ATOMIC variant: thread per element, global
 //                       floating-point atomics (the paper's "atomic indexed accumulation", L43, L124).
