@@ -115,7 +115,8 @@ def run_ours(args, rank: int, world: int):
     prec = pff.PFF_F32 if args.precision == "f32" else pff.PFF_F64
     w = 4 if prec == pff.PFF_F32 else 8
     cfg = make_workload(args.workload)
-    mesh = pff.Mesh(cfg["xy"], cfg["tri"], cfg["material"], precision=prec, chunk_elems=args.chunk, device=f"cuda:{dev}")
+    mesh = pff.Mesh(cfg["xy"], cfg["tri"], cfg["material"], precision=prec, chunk_elems=args.chunk, device=f"cuda:{dev}",
+                    scatter=pff.PFF_SCATTER_ATOMIC if args.scatter == "atomic" else pff.PFF_SCATTER_GATHER)
     st = mesh.new_state(u=cfg["u0"], d=cfg["d0"])
     if len(cfg["edges"]):
         mesh.pff_set_traction(st, cfg["edges"], cfg["traction"])
@@ -234,6 +235,8 @@ def main():
     ap.add_argument("--workload", default="cfg5_1001")
     ap.add_argument("--precision", default="f64", choices=["f64", "f32"])
     ap.add_argument("--chunk", type=int, default=0)
+    ap.add_argument("--scatter", default="gather", choices=["gather", "atomic"],
+                    help="explicit-step scatter: deterministic shared-memory gather (default) or warp-aggregated atomics")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
@@ -279,7 +282,7 @@ def main():
     line = dict(metric=METRIC, value=whole_job_value(Ne, K, world, sec), unit=UNIT, n_gpus=world, steps=K, warmup=args.warmup,
                 ms_per_step=r["ms_total"] / K, higher_is_better=True, scaling="weak", vs_baseline=None,
                 dtype="f64" if w == 8 else "f32", data="synthetic",
-                config=dict(workload=args.workload, name=r["cfg"]["name"], n_nodes=N, n_elems=Ne, rel_tol=REL_TOL,
+                config=dict(workload=args.workload, scatter=args.scatter, name=r["cfg"]["name"], n_nodes=N, n_elems=Ne, rel_tol=REL_TOL,
                             cg_iters_per_solve=iters_total / K, chunks=r["mesh"].n_chunks, interface_nodes=r["mesh"].n_shared,
                             l2="working set > L2 (no flush needed)" if ab["step"] > 126e6 else "L2-resident workload",
                             parallelism=f"replicas x{world}"),

@@ -57,7 +57,8 @@ typedef enum { PFF_F64 = 0, PFF_F32 = 1 } pff_precision;                /* L189:
 typedef enum {
     PFF_SCATTER_GATHER = 0,    /* deterministic: chunk-local CSR gather in shared memory + ordered
                                   interface sums; bit-reproducible run to run (default)            */
-    PFF_SCATTER_ATOMIC = 1     /* element kernel with global floating-point atomics (L43, L124)    */
+    PFF_SCATTER_ATOMIC = 1     /* thread-per-element kernel with warp-aggregated floating-point atomics
+                                  (the paper's atomic accumulation, L43, L124); order not reproducible  */
 } pff_scatter;
 typedef enum { PFF_ORDER_NONE = 0, PFF_ORDER_MORTON = 1 } pff_order;
 

@@ -315,15 +315,33 @@ __global__ void __launch_bounds__(kTPB) step_shared_kernel(const StepArgs<R> a)
     finish_node<R, MODE>(a, gid, px, py, fx, fy);
 }
 
-// ---- atomic variant ------------------------------------------------------------------------
+// ---- atomic variant: warp-aggregated floating-point atomics -------------------------------------------
+// Lanes of a warp that target the same node (frequent after the Morton element order) are matched with
+// __match_any_sync, their contributions summed in lane order through shuffles, and ONE atomicAdd per distinct node
+// is issued by the lowest matching lane.  Order across warps is still arbitrary: not bit-reproducible.
 __device__ __forceinline__ void red_add(double* p, double v) { atomicAdd(p, v); }
 __device__ __forceinline__ void red_add(float* p, float v) { atomicAdd(p, v); }
+
+template <typename R>
+__device__ __forceinline__ void warp_aggregated_add(R* fx, R* fy, int node, R vx, R vy, unsigned active)
+{
+    const unsigned peers = __match_any_sync(active, node);
+    R sx = R(0), sy = R(0);
+    for (unsigned m = peers; m; m &= m - 1) {
+        const int l = __ffs(m) - 1;
+        sx += __shfl_sync(peers, vx, l);
+        sy += __shfl_sync(peers, vy, l);
+    }
+    if ((int)(threadIdx.x & 31) == __ffs(peers) - 1) { red_add(fx + node, sx); red_add(fy + node, sy); }
+}
 
 template <typename R, int SPLIT, int MODE>
 __global__ void __launch_bounds__(kTPB) elem_atomic_kernel(const StepArgs<R> a)
 {
     const int e = blockIdx.x * kTPB + threadIdx.x;
-    if (e >= a.Ne) return;
+    const bool live = e < a.Ne;
+    const unsigned active = __ballot_sync(0xffffffffu, live);
+    if (!live) return;
     const int4 c = __ldg(a.conn + e);
     R b1, c1, b2, c2;
     Geo<R>::load(a.ga, a.gb, e, b1, c1, b2, c2);
@@ -335,9 +353,9 @@ __global__ void __launch_bounds__(kTPB) elem_atomic_kernel(const StepArgs<R> a)
     R psi_p, f[6];
     element_forces<R, SPLIT>(a.mat, b1, c1, b2, c2, A, u1x, u1y, u2x, u2y, u3x, u3y, a.d[c.x] + a.d[c.y] + a.d[c.z],
                              psi_p, f);
-    red_add(a.fwx + c.x, f[0]); red_add(a.fwy + c.x, f[1]);
-    red_add(a.fwx + c.y, f[2]); red_add(a.fwy + c.y, f[3]);
-    red_add(a.fwx + c.z, f[4]); red_add(a.fwy + c.z, f[5]);
+    warp_aggregated_add<R>(a.fwx, a.fwy, c.x, f[0], f[1], active);
+    warp_aggregated_add<R>(a.fwx, a.fwy, c.y, f[2], f[3], active);
+    warp_aggregated_add<R>(a.fwx, a.fwy, c.z, f[4], f[5], active);
     if (MODE == MODE_STEP) {
         const R h = a.H[e];
         if (psi_p > h) a.H[e] = psi_p;

@@ -329,3 +329,21 @@ def test_full_size_config4_perforated_plate():
     assert relmax(u, orc.u) <= TOL64 and relmax(v, orc.v) <= TOL64 and relmax(a, orc.a) <= TOL64
     assert relmax(H, orc.H) <= TOL64
     assert relmax(d, orc.d) <= 1e-9
+
+
+@pytest.mark.parametrize("precision", [0, 1])
+def test_atomic_scatter_variant_config2(precision):
+    """PFF_SCATTER_ATOMIC (warp-aggregated atomics): same results as the oracle up to summation order, on the
+    jittered / permuted mesh of config 2 (lanes of a warp share nodes after the Morton order: the aggregation path)."""
+    cfg = config(2, scale=0.5)
+    tol = TOL64 if precision == 0 else TOL32
+    orc = oracle_from(cfg)
+    mesh, st = gpu_from(cfg, precision=precision, scatter=1)
+    dt = 0.5 * orc.dt_crit()
+    orc.init_accel()
+    mesh.pff_init_accel(st, mesh.bc())
+    for _ in range(5):
+        orc.explicit_step(dt)
+        mesh.pff_explicit_step(st, mesh.bc(), dt)
+    u, v, a, d, H = gpu_fields(mesh, st)
+    assert relmax(u, orc.u) <= tol and relmax(v, orc.v) <= tol and relmax(a, orc.a) <= tol and relmax(H, orc.H) <= tol
