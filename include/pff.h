@@ -60,7 +60,12 @@ typedef enum {
     PFF_SCATTER_ATOMIC = 1     /* thread-per-element kernel with warp-aggregated floating-point atomics
                                   (the paper's atomic accumulation, L43, L124); order not reproducible  */
 } pff_scatter;
-typedef enum { PFF_ORDER_NONE = 0, PFF_ORDER_MORTON = 1 } pff_order;
+typedef enum {
+    PFF_ORDER_NONE = 0,       /* keep the user's element order                                             */
+    PFF_ORDER_MORTON = 1,     /* elements along the Morton curve of their centroids, chunks = curve ranges  */
+    PFF_ORDER_BISECTION = 2   /* Morton order, then recursive coordinate bisection into compact chunks of
+                                 exactly chunk_elems elements (fewest interface nodes; default of the binding) */
+} pff_order;
 
 /* Material and model.  g(d) = (1-d)^2 + eta. */
 typedef struct {

@@ -12,7 +12,8 @@ import ctypes as C
 import numpy as np
 
 from . import _lib
-from ._lib import (PFF_AT1, PFF_AT2, PFF_ENOCONV, PFF_F32, PFF_F64, PFF_OK, PFF_ORDER_MORTON, PFF_ORDER_NONE,  # noqa: F401
+from ._lib import (PFF_AT1, PFF_AT2, PFF_ENOCONV, PFF_F32, PFF_F64, PFF_OK, PFF_ORDER_BISECTION, PFF_ORDER_MORTON,  # noqa: F401
+                   PFF_ORDER_NONE,
                    PFF_PLANE_STRAIN, PFF_PLANE_STRESS, PFF_SCATTER_ATOMIC, PFF_SCATTER_GATHER,
                    PFF_SPLIT_ISOTROPIC, PFF_SPLIT_SPECTRAL, PFF_SPLIT_STARCONVEX, PFF_SPLIT_VOLDEV)
 
@@ -46,7 +47,7 @@ class State:
 class Mesh:
     """pff_mesh handle.  Host index sets are in USER numbering; device vectors in internal order."""
 
-    def __init__(self, xy, tri, material: dict, precision=PFF_F64, order=PFF_ORDER_MORTON,
+    def __init__(self, xy, tri, material: dict, precision=PFF_F64, order=PFF_ORDER_BISECTION,
                  scatter=PFF_SCATTER_GATHER, chunk_elems=0, device="cuda:0"):
         import torch
         if not torch.cuda.is_available():

@@ -13,7 +13,7 @@ PFF_SPLIT_ISOTROPIC, PFF_SPLIT_SPECTRAL, PFF_SPLIT_VOLDEV, PFF_SPLIT_STARCONVEX 
 PFF_PLANE_STRAIN, PFF_PLANE_STRESS = 0, 1
 PFF_F64, PFF_F32 = 0, 1
 PFF_SCATTER_GATHER, PFF_SCATTER_ATOMIC = 0, 1
-PFF_ORDER_NONE, PFF_ORDER_MORTON = 0, 1
+PFF_ORDER_NONE, PFF_ORDER_MORTON, PFF_ORDER_BISECTION = 0, 1, 2
 KERNEL_CLASSES = ("step_chunk", "step_shared", "matvec_chunk", "matvec_shared", "cg_vector", "damage_setup", "other")
 
 # every symbol include/pff.h declares

@@ -21,6 +21,38 @@ static inline uint32_t spread16(uint32_t v)
     return v;
 }
 
+// Recursive coordinate bisection of the (Morton-ordered) elements into chunks of exactly EC elements (the last one
+// ragged): every cut is a median cut across the longer side of the bounding box of the centroids, placed at a
+// multiple of EC, so the chunks are compact near-square patches whatever EC is (a Morton range of a length that is
+// not a power of two is ragged and has ~1.7x more interface nodes).  Leaves keep Morton order inside.
+static void bisect_into_chunks(const std::vector<int32_t>& morton_order, const std::vector<float>& cx,
+                               const std::vector<float>& cy, int EC, std::vector<int32_t>& elem_old_of_new)
+{
+    const int64_t Ne = (int64_t)morton_order.size();
+    std::vector<int32_t> pos(Ne);  // positions in Morton order, permuted in place
+    std::iota(pos.begin(), pos.end(), 0);
+    struct Range { int64_t lo, hi; };
+    std::vector<Range> stack{{0, Ne}};
+    while (!stack.empty()) {
+        const Range r = stack.back();
+        stack.pop_back();
+        const int64_t n = r.hi - r.lo, chunks = (n + EC - 1) / EC;
+        if (chunks <= 1) { std::sort(pos.begin() + r.lo, pos.begin() + r.hi); continue; }
+        float x0 = 3.4e38f, x1 = -3.4e38f, y0 = 3.4e38f, y1 = -3.4e38f;
+        for (int64_t i = r.lo; i < r.hi; ++i) {
+            const int32_t e = pos[i];
+            x0 = std::min(x0, cx[e]); x1 = std::max(x1, cx[e]); y0 = std::min(y0, cy[e]); y1 = std::max(y1, cy[e]);
+        }
+        const std::vector<float>& key = (x1 - x0 >= y1 - y0) ? cx : cy;
+        const int64_t mid = r.lo + (chunks / 2) * EC;
+        std::nth_element(pos.begin() + r.lo, pos.begin() + mid, pos.begin() + r.hi,
+                         [&](int32_t a, int32_t b) { return key[a] < key[b] || (key[a] == key[b] && a < b); });
+        stack.push_back({mid, r.hi});
+        stack.push_back({r.lo, mid});
+    }
+    for (int64_t i = 0; i < Ne; ++i) elem_old_of_new[i] = morton_order[pos[i]];
+}
+
 pff_status build_host_mesh(int64_t N, const double* xy, int64_t Ne, const int32_t* tri_in, double rho,
                            int order, int chunk_elems, size_t real_bytes, HostMesh& hm, std::string& err)
 {
@@ -64,7 +96,8 @@ pff_status build_host_mesh(int64_t N, const double* xy, int64_t Ne, const int32_
 
     // ---- element order: Morton key of the centroid (or user order)
     std::vector<int32_t> elem_old_of_new(Ne);
-    if (order == PFF_ORDER_MORTON) {
+    std::vector<float> ccx, ccy;  // centroids in Morton order (bisection only)
+    if (order == PFF_ORDER_MORTON || order == PFF_ORDER_BISECTION) {
         std::vector<uint64_t> keyed(Ne);
         double sx = (xmax > xmin) ? 65535.0 / (xmax - xmin) : 0.0, sy = (ymax > ymin) ? 65535.0 / (ymax - ymin) : 0.0;
         for (int64_t e = 0; e < Ne; ++e) {
@@ -78,11 +111,18 @@ pff_status build_host_mesh(int64_t N, const double* xy, int64_t Ne, const int32_
         }
         std::sort(keyed.begin(), keyed.end());
         for (int64_t e = 0; e < Ne; ++e) elem_old_of_new[e] = int32_t(keyed[e] & 0xFFFFFFFFu);
+        if (order == PFF_ORDER_BISECTION) {
+            ccx.resize(Ne); ccy.resize(Ne);
+            for (int64_t e = 0; e < Ne; ++e) {
+                const int32_t* t = &tri[3 * elem_old_of_new[e]];
+                ccx[e] = float((xy[2 * t[0]] + xy[2 * t[1]] + xy[2 * t[2]]) / 3.0 - xmin);
+                ccy[e] = float((xy[2 * t[0] + 1] + xy[2 * t[1] + 1] + xy[2 * t[2] + 1]) / 3.0 - ymin);
+            }
+        }
     } else {
         std::iota(elem_old_of_new.begin(), elem_old_of_new.end(), 0);
     }
-    hm.elem_new_of_old.resize(Ne);
-    for (int64_t e = 0; e < Ne; ++e) hm.elem_new_of_old[elem_old_of_new[e]] = int32_t(e);
+    const std::vector<int32_t> morton_order = elem_old_of_new;  // bisection re-partitions this order per chunk size
 
     // ---- chunks; shrink the chunk until the shared-memory footprints of the chunk kernels fit.  Default chunk: the
     // largest size for which THREE double-buffered CTAs of the CG kernel (12 of 13 launches-worth of work per step)
@@ -95,6 +135,7 @@ pff_status build_host_mesh(int64_t N, const double* xy, int64_t Ne, const int32_
     const size_t limit_other = (user_chunk ? kSmemPerSM : kSmemPerSM / 2) - kSmemCtaReserve;
     std::vector<int32_t> cmin(N), cmax(N);
     for (;;) {
+        if (order == PFF_ORDER_BISECTION) bisect_into_chunks(morton_order, ccx, ccy, EC, elem_old_of_new);
         std::fill(cmin.begin(), cmin.end(), std::numeric_limits<int32_t>::max());
         std::fill(cmax.begin(), cmax.end(), -1);
         for (int64_t en = 0; en < Ne; ++en) {
@@ -136,6 +177,8 @@ pff_status build_host_mesh(int64_t N, const double* xy, int64_t Ne, const int32_
         EC -= EC > 512 ? 64 : 32;  // 1024, 960, ..., 512, 480, 448, ..., 32
     }
     hm.chunk_elems = EC;
+    hm.elem_new_of_old.resize(Ne);
+    for (int64_t e = 0; e < Ne; ++e) hm.elem_new_of_old[elem_old_of_new[e]] = int32_t(e);
     const int64_t C = hm.C;
     for (int64_t i = 0; i < N; ++i)
         if (cmax[i] < 0) { err = "node " + std::to_string(i) + " belongs to no element (orphan)"; return PFF_EMESH; }

@@ -94,7 +94,7 @@ pff_status pff_mesh_create(int64_t n_nodes, const double* xy, int64_t n_elems, c
     if ((mat->model != PFF_AT1 && mat->model != PFF_AT2) || mat->split < 0 || mat->split > 3 ||
         (mat->plane != PFF_PLANE_STRAIN && mat->plane != PFF_PLANE_STRESS) ||
         (opt.precision != PFF_F64 && opt.precision != PFF_F32) ||
-        (opt.order != PFF_ORDER_NONE && opt.order != PFF_ORDER_MORTON) ||
+        (opt.order != PFF_ORDER_NONE && opt.order != PFF_ORDER_MORTON && opt.order != PFF_ORDER_BISECTION) ||
         (opt.scatter != PFF_SCATTER_GATHER && opt.scatter != PFF_SCATTER_ATOMIC) || opt.chunk_elems < 0) {
         set_error("pff_mesh_create: bad enum value"); return PFF_EINVAL;
     }
