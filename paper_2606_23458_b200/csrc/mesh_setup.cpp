@@ -114,9 +114,17 @@ pff_status build_host_mesh(int64_t N, const double* xy, int64_t Ne, const int32_
         if (order == PFF_ORDER_BISECTION) {
             ccx.resize(Ne); ccy.resize(Ne);
             for (int64_t e = 0; e < Ne; ++e) {
+                // key = midpoint of the LONGEST edge: two triangles that share it (the two halves of a quad) get the
+                // same key and stay on the same side of a cut, which keeps the cut lines straight
                 const int32_t* t = &tri[3 * elem_old_of_new[e]];
-                ccx[e] = float((xy[2 * t[0]] + xy[2 * t[1]] + xy[2 * t[2]]) / 3.0 - xmin);
-                ccy[e] = float((xy[2 * t[0] + 1] + xy[2 * t[1] + 1] + xy[2 * t[2] + 1]) / 3.0 - ymin);
+                double best = -1.0, mx = 0.0, my = 0.0;
+                for (int k = 0; k < 3; ++k) {
+                    const int32_t p = t[k], q = t[(k + 1) % 3];
+                    const double dx = xy[2 * p] - xy[2 * q], dy = xy[2 * p + 1] - xy[2 * q + 1], l2 = dx * dx + dy * dy;
+                    if (l2 > best) { best = l2; mx = 0.5 * (xy[2 * p] + xy[2 * q]); my = 0.5 * (xy[2 * p + 1] + xy[2 * q + 1]); }
+                }
+                ccx[e] = float(mx - xmin);
+                ccy[e] = float(my - ymin);
             }
         }
     } else {
