@@ -182,7 +182,11 @@ pff_status build_host_mesh(int64_t N, const double* xy, int64_t Ne, const int32_
             hm.max_nloc = max_nloc; hm.C = C;
             break;
         }
-        EC -= EC > 512 ? 64 : 32;  // 1024, 960, ..., 512, 480, 448, ..., 32
+        {   // footprints are nearly linear in EC: jump close to the fitting size, then step down by 32
+            const double ratio = std::min(double(limit_cg) / double(smem_cg), double(limit_other) / double(std::max(smem_step, smem_su)));
+            const int jump = int(EC * std::min(ratio, 1.0)) / 32 * 32 + 32;
+            EC = std::max(32, std::min(EC - 32, jump));
+        }
     }
     hm.chunk_elems = EC;
     hm.elem_new_of_old.resize(Ne);
