@@ -44,7 +44,7 @@ def _plan(lib, xy, tri, chunk=0, order=1, precision=0):
     return st, nn, en, nc.value, ns.value, ec.value, ml.value, hm.value
 
 
-@pytest.mark.parametrize("order", [0, 1])
+@pytest.mark.parametrize("order", [0, 1, 2])
 def test_plan_is_a_valid_decomposition(lib, order):
     cfg = config(2, scale=0.2)
     xy, tri = cfg["xy"], cfg["tri"]
@@ -66,11 +66,22 @@ def test_plan_is_a_valid_decomposition(lib, order):
     # interior nodes of a chunk are contiguous and ordered by chunk
     order_int = np.argsort(nn[~shared])
     assert np.all(np.diff(cmin[~shared][order_int]) >= 0)
-    if order == 1:
-        assert ns < 0.5 * N  # Morton order undoes the random element permutation of config 2
+    if order >= 1:
+        assert ns < 0.5 * N  # Morton order / bisection undo the random element permutation of config 2
     # h_min against the closed form of the unjittered grid
     xy0, tri0 = grid_mesh(21, 9, 0.02, 0.008)
     assert abs(_plan(lib, xy0, tri0)[7] - (2 - np.sqrt(2)) * 1e-3) < 1e-15
+
+
+def test_bisection_chunks_are_more_compact_than_morton_ranges(lib):
+    """PFF_ORDER_BISECTION (default of the binding): fewer interface nodes than Morton ranges at a chunk size that is not
+    a power of two, and the default chunk size keeps 3 double-buffered CG CTAs per SM (shared-memory budget)."""
+    cfg = config(5, n=201)
+    ns_m = _plan(lib, cfg["xy"], cfg["tri"], chunk=352, order=1)[4]
+    ns_b = _plan(lib, cfg["xy"], cfg["tri"], chunk=352, order=2)[4]
+    assert ns_b < 0.7 * ns_m
+    st, _, _, nc, _, ec, ml, _ = _plan(lib, cfg["xy"], cfg["tri"], chunk=0, order=2)
+    assert st == 0 and ec % 32 == 0 and 256 <= ec <= 512 and nc == -(-len(cfg["tri"]) // ec)
 
 
 def test_chunk_shrinks_to_fit_shared_memory(lib):
