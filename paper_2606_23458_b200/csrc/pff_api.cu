@@ -84,7 +84,7 @@ pff_status pff_mesh_create(int64_t n_nodes, const double* xy, int64_t n_elems, c
 {
     if (out) *out = nullptr;
     if (!xy || !tri || !mat || !out) { set_error("pff_mesh_create: null argument"); return PFF_EINVAL; }
-    pff_options opt{PFF_F64, PFF_ORDER_MORTON, PFF_SCATTER_GATHER, 0};
+    pff_options opt{PFF_F64, PFF_ORDER_BISECTION, PFF_SCATTER_GATHER, 0};
     if (opt_in) opt = *opt_in;
     if (!(mat->E > 0) || !(mat->rho > 0) || !(mat->Gc > 0) || !(mat->l0 > 0) || !(mat->nu > -1.0) || !(mat->nu < 0.5) ||
         !(mat->eta >= 0) || !std::isfinite(mat->E + mat->rho + mat->Gc + mat->l0 + mat->eta)) {
@@ -192,7 +192,7 @@ pff_status pff_mesh_plan(int64_t n_nodes, const double* xy, int64_t n_elems, con
                          int32_t* chunk_elems, int32_t* max_local_nodes, double* h_min)
 {
     if (!xy || !tri) { set_error("pff_mesh_plan: null argument"); return PFF_EINVAL; }
-    pff_options opt{PFF_F64, PFF_ORDER_MORTON, PFF_SCATTER_GATHER, 0};
+    pff_options opt{PFF_F64, PFF_ORDER_BISECTION, PFF_SCATTER_GATHER, 0};
     if (opt_in) opt = *opt_in;
     HostMesh hm;
     std::string err;
