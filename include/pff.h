@@ -112,6 +112,7 @@ typedef struct {
  * elements are re-oriented, R1).  Computes areas, shape gradients (Eq. 9), inverse
  * lumped mass (L169), h_min, the renumbering, the CTA chunks and their shared-memory gather
  * tables, and uploads everything.  Input arrays are copied; *out is owned by the library.
+ * options may be NULL: { PFF_F64, PFF_ORDER_BISECTION, PFF_SCATTER_GATHER, chunk_elems 0 }.
  * Errors: PFF_EINVAL (arguments/material), PFF_EMESH (bad index, degenerate element, orphan
  * node, n_nodes >= 2^30), PFF_ENOMEM, PFF_ECUDA. */
 pff_status pff_mesh_create(int64_t n_nodes, const double *xy, int64_t n_elems, const int32_t *tri,
