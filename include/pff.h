@@ -176,6 +176,21 @@ pff_status pff_damage_solve(pff_mesh *mesh, pff_state *state, double rel_tol, in
  * with a fixed reduction order.  Synchronises the stream. */
 pff_status pff_energies(pff_mesh *mesh, const pff_state *state, double out[4]);
 
+/* ---- damage subcycling ---------------------------------------
+ * Admissible subcycling factor N_max = floor(c_p / (0.6 c_R)): the damage front moves at <= ~0.6 c_R while the explicit
+ * step is limited by c_p.  c_p = sqrt((lambda + 2 mu) / rho) with the plane-assumption lambda (as in the CFL step,
+ * DESIGN.md R19), c_s = sqrt(mu / rho), c_R = c_s (0.862 + 1.14 nu) / (1 + nu) (Bergmann-Viktorov approximation of the
+ * Rayleigh speed; the paper does not print its formula: DESIGN.md R22).  Host-only, no CUDA call.  ratio (may be NULL)
+ * receives the continuous value c_p / (0.6 c_R).  PMMA-like nu = 0.35 gives N_max = 3 (the paper's printed value). */
+pff_status pff_subcycle_limit(const pff_material *material, int32_t *n_max, double *ratio);
+
+/* n_steps staggered steps on DEVICE-RESIDENT state (no host copies): pff_explicit_step every step (so the history
+ * field and irreversibility follow the mechanical time scale, L187) and pff_damage_solve every damage_every-th step
+ * (0 = never; 1 = the plain staggered scheme of L114).  Constant boundary data bc.  cg_iters_total (host, may be NULL)
+ * receives the summed CG iterations.  Returns PFF_ENOCONV if any solve did (results are written).  Synchronises. */
+pff_status pff_run_steps(pff_mesh *mesh, pff_state *state, const pff_bc *bc, double dt, int64_t n_steps,
+                         int32_t damage_every, double rel_tol, int32_t max_iter, int64_t *cg_iters_total);
+
 /* ---- test hooks (device vectors, internal order, precision of the mesh) ---------------------- */
 /* f_int(u, d) of the current state (no predictor), and psi+ per element (psi_plus may be NULL). */
 pff_status pff_internal_force(pff_mesh *mesh, const pff_state *state, void *fx, void *fy, void *psi_plus);

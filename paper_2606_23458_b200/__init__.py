@@ -153,6 +153,15 @@ class Mesh:
                     allow=(PFF_ENOCONV,) if allow_noconv else ())
         return st, it.value, rr.value
 
+    def pff_run_steps(self, state: State, bc, dt: float, n_steps: int, damage_every=1, rel_tol=1e-8, max_iter=1000,
+                      allow_noconv=False):
+        """n_steps staggered steps on the device-resident state, damage solve every damage_every-th step."""
+        tot = C.c_int64(0)
+        st = _check(self.L.pff_run_steps(self.h, C.byref(state.c), C.byref(bc) if bc is not None else None, dt, n_steps,
+                                         damage_every, rel_tol, max_iter, C.byref(tot)),
+                    allow=(PFF_ENOCONV,) if allow_noconv else ())
+        return st, tot.value
+
     def pff_energies(self, state: State):
         out = (C.c_double * 4)()
         _check(self.L.pff_energies(self.h, C.byref(state.c), out))
@@ -213,3 +222,11 @@ class Mesh:
         dv = kv.ctypes.data if kv is not None else None
         return _check(self.L.pff_run_host(self.h, C.byref(hs), du, dv, load_scale, dt, n_steps, damage_every,
                                           rel_tol, max_iter), allow=(PFF_ENOCONV,) if allow_noconv else ())
+
+
+def pff_subcycle_limit(material: dict):
+    """(N_max, continuous ratio c_p / (0.6 c_R)) of PAPER.md L187; host-only."""
+    m = _lib.pff_material(**material)
+    n, r = C.c_int32(0), C.c_double(0.0)
+    _check(_lib.load().pff_subcycle_limit(C.byref(m), C.byref(n), C.byref(r)))
+    return n.value, r.value

@@ -327,6 +327,48 @@ pff_status pff_damage_solve(pff_mesh* m, pff_state* s, double rel_tol, int32_t m
     return damage_solve(m, s, rel_tol, max_iter, iters, relres);
 }
 
+pff_status pff_subcycle_limit(const pff_material* mat, int32_t* n_max, double* ratio)
+{
+    if (!mat || !n_max) { set_error("pff_subcycle_limit: null argument"); return PFF_EINVAL; }
+    if (!(mat->E > 0) || !(mat->rho > 0) || !(mat->nu > -1.0) || !(mat->nu < 0.5)) {
+        set_error("pff_subcycle_limit: material out of range"); return PFF_EINVAL;
+    }
+    const double mu = mat->E / (2 * (1 + mat->nu));
+    const double lam = mat->plane == PFF_PLANE_STRESS ? mat->E * mat->nu / (1 - mat->nu * mat->nu)
+                                                       : mat->E * mat->nu / ((1 + mat->nu) * (1 - 2 * mat->nu));
+    const double cp = std::sqrt((lam + 2 * mu) / mat->rho), cs = std::sqrt(mu / mat->rho);
+    const double cR = cs * (0.862 + 1.14 * mat->nu) / (1 + mat->nu);
+    const double r = cp / (0.6 * cR);
+    if (ratio) *ratio = r;
+    *n_max = (int32_t)std::floor(r);
+    return PFF_OK;
+}
+
+pff_status pff_run_steps(pff_mesh* m, pff_state* s, const pff_bc* bc, double dt, int64_t n_steps, int32_t damage_every,
+                         double rel_tol, int32_t max_iter, int64_t* cg_iters_total)
+{
+    if (!m || !valid_state(s)) { set_error("pff_run_steps: null mesh, null or misaligned (16 B) state pointer"); return PFF_EINVAL; }
+    if (!(dt > 0) || !std::isfinite(dt) || n_steps < 0 || damage_every < 0 ||
+        (damage_every > 0 && (!(rel_tol > 0) || max_iter < 1))) {
+        set_error("pff_run_steps: need dt > 0, n_steps >= 0, damage_every >= 0, rel_tol > 0, max_iter >= 1"); return PFF_EINVAL;
+    }
+    pff_status worst = PFF_OK, st;
+    int64_t total = 0;
+    for (int64_t k = 1; k <= n_steps; ++k) {
+        if ((st = launch_step(m, s, bc, dt, /*MODE_STEP*/ 0, nullptr, nullptr, nullptr)) != PFF_OK) return st;
+        if (damage_every > 0 && k % damage_every == 0) {
+            int it = 0;
+            st = damage_solve(m, s, rel_tol, max_iter, &it, nullptr);
+            total += it;
+            if (st == PFF_ENOCONV) worst = st;
+            else if (st != PFF_OK) return st;
+        }
+    }
+    if (cg_iters_total) *cg_iters_total = total;
+    PFF_CUDA(cudaStreamSynchronize(m->stream));
+    return worst;
+}
+
 pff_status pff_damage_matvec(pff_mesh* m, const pff_state* s, const void* p, void* q)
 {
     if (!m || !valid_state(s) || !p || !q) { set_error("pff_damage_matvec: null argument"); return PFF_EINVAL; }

@@ -347,3 +347,26 @@ def test_atomic_scatter_variant_config2(precision):
         mesh.pff_explicit_step(st, mesh.bc(), dt)
     u, v, a, d, H = gpu_fields(mesh, st)
     assert relmax(u, orc.u) <= tol and relmax(v, orc.v) <= tol and relmax(a, orc.a) <= tol and relmax(H, orc.H) <= tol
+
+
+def test_damage_subcycling_run_steps():
+    """pff_run_steps with damage_every = 3 (damage solved every N_sub-th step, history every step)
+    against the oracle driven the same way, and damage_every = 1 against the plain staggered loop."""
+    cfg = config(1)
+    for every in (3, 1):
+        orc = oracle_from(cfg)
+        mesh, st = gpu_from(cfg)
+        dt = 0.5 * orc.dt_crit()
+        S = 8.0
+        orc.init_accel(S)
+        bc = mesh.bc(load_scale=S)
+        mesh.pff_init_accel(st, bc)
+        for k in range(1, 31):
+            orc.explicit_step(dt, S=S)
+            if k % every == 0:
+                assert orc.damage_solve(rel_tol=1e-12, max_iter=4000)[0] == 0
+        stt, iters = mesh.pff_run_steps(st, bc, dt, 30, damage_every=every, rel_tol=1e-12, max_iter=4000)
+        assert stt == 0 and iters > 0
+        u, v, a, d, H = gpu_fields(mesh, st)
+        assert relmax(u, orc.u) <= 1e-10 and relmax(v, orc.v) <= 1e-10 and relmax(H, orc.H) <= 1e-10
+        assert relmax(d, orc.d) <= 1e-10
