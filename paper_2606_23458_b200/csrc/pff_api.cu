@@ -75,6 +75,7 @@ void pff_mesh_destroy(pff_mesh* m)
                     m->d_elem_old_of_new};
     for (void* p : ptrs) if (p) cudaFree(p);
     if (m->h_ctrl) cudaFreeHost(m->h_ctrl);
+    if (m->h_ring) cudaFreeHost(m->h_ring);
     for (auto& v : m->prof_ev) for (cudaEvent_t e : v) cudaEventDestroy(e);
     delete m;
 }
@@ -352,20 +353,38 @@ pff_status pff_run_steps(pff_mesh* m, pff_state* s, const pff_bc* bc, double dt,
         (damage_every > 0 && (!(rel_tol > 0) || max_iter < 1))) {
         set_error("pff_run_steps: need dt > 0, n_steps >= 0, damage_every >= 0, rel_tol > 0, max_iter >= 1"); return PFF_EINVAL;
     }
-    pff_status worst = PFF_OK, st;
+    // The whole loop is asynchronous: every solve copies its control block into a pinned ring; the host synchronises and
+    // inspects the ring only every kRing solves and at the end, so the GPU never waits for the host between steps.
+    constexpr int kRing = 64;
+    if (!m->h_ring) PFF_CUDA(cudaMallocHost((void**)&m->h_ring, kRing * sizeof(DamageCtrl)));
+    pff_status worst = PFF_OK, st = PFF_OK;
     int64_t total = 0;
-    for (int64_t k = 1; k <= n_steps; ++k) {
-        if ((st = launch_step(m, s, bc, dt, /*MODE_STEP*/ 0, nullptr, nullptr, nullptr)) != PFF_OK) return st;
+    int pending = 0;
+    auto drain = [&]() -> pff_status {
+        pff_status e = cuda_check(cudaStreamSynchronize(m->stream), "pff_run_steps: sync");
+        if (e != PFF_OK) return e;
+        for (int i = 0; i < pending; ++i) {
+            total += m->h_ring[i].iters;
+            if (!m->h_ring[i].done || m->h_ring[i].status == PFF_ENOCONV) worst = PFF_ENOCONV;
+        }
+        pending = 0;
+        return PFF_OK;
+    };
+    for (int64_t k = 1; k <= n_steps && st == PFF_OK; ++k) {
+        if ((st = launch_step(m, s, bc, dt, /*MODE_STEP*/ 0, nullptr, nullptr, nullptr)) != PFF_OK) break;
         if (damage_every > 0 && k % damage_every == 0) {
-            int it = 0;
-            st = damage_solve(m, s, rel_tol, max_iter, &it, nullptr);
-            total += it;
-            if (st == PFF_ENOCONV) worst = st;
-            else if (st != PFF_OK) return st;
+            m->defer_slot = &m->h_ring[pending];
+            st = damage_solve(m, s, rel_tol, max_iter, nullptr, nullptr);
+            m->defer_slot = nullptr;
+            if (st != PFF_OK) break;
+            if (++pending == kRing) st = drain();
         }
     }
+    const pff_status e = drain();
+    if (st != PFF_OK) return st;
+    if (e != PFF_OK) return e;
     if (cg_iters_total) *cg_iters_total = total;
-    PFF_CUDA(cudaStreamSynchronize(m->stream));
+    if (worst == PFF_ENOCONV) set_error("pff_run_steps: a damage solve reached max_iter");
     return worst;
 }
 

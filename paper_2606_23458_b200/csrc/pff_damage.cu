@@ -27,10 +27,6 @@
 
 #include "pff_tma.cuh"
 
-struct DamageCtrl {
-    double rz, alpha, beta, amax, nb, tol, relres;
-    int iters, max_iter, done, status, first, restart, trunc, pending, restarts;
-};
 
 namespace pff {
 
@@ -913,6 +909,9 @@ static pff_status damage_solve_t(pff_mesh* m, pff_state* s, double rel_tol, int 
         prof_mark(m, PFF_K_MATVEC_CHUNK);
         ++m->n_launches;
         if ((st = cuda_check(e, "damage: cooperative launch")) != PFF_OK) return st;
+    }
+    if (m->defer_slot) {  // pff_run_steps: the control block is read back asynchronously and inspected later, no sync here
+        return cuda_check(cudaMemcpyAsync(m->defer_slot, m->d_ctrl, sizeof(DamageCtrl), cudaMemcpyDeviceToHost, cs), "damage: ctrl download");
     }
     if ((st = cuda_check(cudaMemcpyAsync(&h[1], m->d_ctrl, sizeof(DamageCtrl), cudaMemcpyDeviceToHost, cs), "damage: ctrl download")) != PFF_OK) return st;
     if ((st = cuda_check(cudaStreamSynchronize(cs), "damage: sync")) != PFF_OK) return st;

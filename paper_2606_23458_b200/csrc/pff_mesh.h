@@ -7,7 +7,11 @@
 
 #include "pff_internal.h"
 
-struct DamageCtrl;  // device-resident CG control block (pff_damage.cu)
+// device-resident control block of the CG recurrence (pff_damage.cu); one 128-byte read-back per solve
+struct DamageCtrl {
+    double rz, alpha, beta, amax, nb, tol, relres;
+    int iters, max_iter, done, status, first, restart, trunc, pending, restarts;
+};
 
 struct pff_mesh {
     pff::HostMesh hm;
@@ -56,6 +60,8 @@ struct pff_mesh {
     int64_t n_part_blocks = 0;
     DamageCtrl* d_ctrl = nullptr;
     DamageCtrl* h_ctrl = nullptr;  // pinned
+    DamageCtrl* h_ring = nullptr;      // pinned ring of deferred read-backs (pff_run_steps)
+    DamageCtrl* defer_slot = nullptr;  // non-null: damage_solve copies the control block here and does not synchronise
     unsigned int* d_ticket = nullptr;
 
     // host-path staging (pff_run_host)
