@@ -288,6 +288,10 @@ __global__ void __launch_bounds__(kTPB, 3) dmg_iter_chunk(const DmgArgs<R> a)
     bool pre_issued = false;  // the next CG iteration's first chunk is already streaming in
     int hid0 = -1;            // global id of the halo node of this CTA's first chunk whose gather this thread issues
     int it = 0;  // stage uses so far (global over epochs and CG iterations): stage = it & 1, mbarrier parity = (it >> 1) & 1
+    if (MODE == DM_CG) {
+        __syncthreads();  // s_ctrl loaded
+        if (s_ctrl.done) goto finalize;  // converged before the first iteration (setup pass)
+    }
   for (;;) {  // CG iterations (DM_CG); one pass otherwise
 #pragma unroll
     for (int c = 0; c < kCh; ++c) acc[c] = 0.0;
@@ -514,6 +518,7 @@ __global__ void __launch_bounds__(kTPB, 3) dmg_iter_chunk(const DmgArgs<R> a)
     }
   }
     if (MODE != DM_CG) return;
+finalize:
     // ---- converged (or out of iterations): apply the pending last step, then d <- min(1, max(d_n, x)) (L179)
     {
         const bool pending = s_ctrl.pending != 0;
@@ -722,6 +727,7 @@ __global__ void __launch_bounds__(kTPB, 2) dmg_setup_chunk(const DmgArgs<R> a)
                         a.mask[gid] = fixed ? 2 : 1;
                         acc[0] += double(bs) * double(bs);
                         if (!fixed) acc[1] += double(r) * double(r);
+                        if (!fixed && (a.mat.model != PFF_AT1 || r > R(0))) acc[2] += double(r) * double(r);  // solver's first free set
                     }
                 } else {
                     const int slot = s_hdst[i - cm.n_int];
@@ -759,6 +765,7 @@ __global__ void __launch_bounds__(kTPB) dmg_setup_shared(const DmgArgs<R> a)
             a.mask[gid] = fixed ? 2 : 1;
             acc[0] += double(bs) * double(bs);
             if (!fixed) acc[1] += double(r) * double(r);
+            if (!fixed && (a.mat.model != PFF_AT1 || r > R(0))) acc[2] += double(r) * double(r);
         }
     }
     if (HOOK) return;
@@ -766,7 +773,13 @@ __global__ void __launch_bounds__(kTPB) dmg_setup_shared(const DmgArgs<R> a)
     block_reduce_ch(acc, s_w, s_out);
     double t[kCh];
     if (fold_and_finish(a.part, a.part_n, a.n_chunk_blocks, a.part2, a.ticket, s_w, s_out, t) && threadIdx.x == 0)
-        a.ctrl->nb = fmax(fmax(sqrt(t[0]), sqrt(t[1])), 1e-300);
+    {
+        DamageCtrl* c = a.ctrl;
+        c->nb = fmax(fmax(sqrt(t[0]), sqrt(t[1])), 1e-300);
+        // d_n already solves the system to the tolerance (no history growth since the last solve; AT1: KKT holds with the
+        // free set the solver would start from): no CG iteration is needed, the cooperative kernel only clamps
+        if (sqrt(t[2]) <= c->tol * c->nb) { c->done = 1; c->status = PFF_OK; c->relres = sqrt(t[2]) / c->nb; c->pending = 0; }
+    }
 }
 
 template <typename R>
