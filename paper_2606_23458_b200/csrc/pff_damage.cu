@@ -273,20 +273,21 @@ __global__ void __launch_bounds__(kTPB, 3) dmg_iter_chunk(const DmgArgs<R> a)
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem + L.bar);
     const int tid = threadIdx.x, G = gridDim.x, EC = a.EC;
     const int n_my = (a.C - (int)blockIdx.x + G - 1) / G;  // chunks this CTA owns
-    // the LAST warp issues the bulk copies (one lane per array); the halo gathers are issued from the top thread
-    // downwards: both are idle while the low warps run the node prologue
+    // The LAST warp is the producer: it issues the bulk copies (one lane per array) and ALL halo gathers of the next
+    // chunk and takes no part in the node prologue and the element pass (the other kWorkers threads synchronise on a
+    // named barrier between those two phases); it rejoins for the node gather.
+    constexpr int kWorkers = kTPB - 32;
     const int lane = tid & 31;
-    const bool issuer = tid >= kTPB - 32;
+    const bool issuer = tid >= kWorkers;
     const bool have_desc = issuer && lane < a.plan.n;
     StageDesc my_desc{};
     if (have_desc) my_desc = a.plan.d[lane];
-    const int gj = kTPB - 1 - tid;  // halo node whose gather this thread issues
+    int* s_hid0 = reinterpret_cast<int*>(smem + L.hid0);
 
     if (tid == 0) { mbar_init(bar, 1 + kTPB); mbar_init(bar + 2, 1 + kTPB); s_slot[3 * EC] = R(0); }
     double acc[kCh];
     const bool single_epoch = n_my <= kMetaCap;
     bool pre_issued = false;  // the next CG iteration's first chunk is already streaming in
-    int hid0 = -1;            // global id of the halo node of this CTA's first chunk whose gather this thread issues
     int it = 0;  // stage uses so far (global over epochs and CG iterations): stage = it & 1, mbarrier parity = (it >> 1) & 1
     if (MODE == DM_CG) {
         __syncthreads();  // s_ctrl loaded
@@ -316,10 +317,13 @@ __global__ void __launch_bounds__(kTPB, 3) dmg_iter_chunk(const DmgArgs<R> a)
                 fence_proxy_async();
                 stage_issue_desc(my_desc, have_desc, stg, bar + 2 * (it & 1), lane, cr);
             }
-            if (gj < cm.n_halo) {
+            if (issuer) {
                 const int hb0 = ((cm.node_start & (A - 1)) + cm.n_int + A - 1) & ~(A - 1);
-                if (!pre_issued) hid0 = __ldg(a.halo_ids + cm.halo_off + gj);
-                halo_gather_async<R, MODE, PROJ>(a, L, stg, hb0 + gj, gj, hid0);
+                for (int j = lane; j < cm.n_halo; j += 32) {
+                    if (!pre_issued && e0 == 0) s_hid0[j] = __ldg(a.halo_ids + cm.halo_off + j);
+                    const int gid = e0 == 0 ? s_hid0[j] : __ldg(a.halo_ids + cm.halo_off + j);
+                    halo_gather_async<R, MODE, PROJ>(a, L, stg, hb0 + j, j, gid);
+                }
             }
             cp_async_mbar_arrive(bar + 2 * (it & 1));
             pre_issued = false;
@@ -356,27 +360,19 @@ __global__ void __launch_bounds__(kTPB, 3) dmg_iter_chunk(const DmgArgs<R> a)
                     fence_proxy_async();
                     stage_issue_desc(my_desc, have_desc, stn, bar + 2 * (st ^ 1), lane, cr);
                 }
-                if (gj < cn.n_halo) {
+                if (issuer) {
                     const int hbn = ((cn.node_start & (A - 1)) + cn.n_int + A - 1) & ~(A - 1);
-                    const int gid = reinterpret_cast<const int*>(stg + L.hnext)[(cn.halo_off & 3) + gj];
-                    halo_gather_async<R, MODE, PROJ>(a, L, stn, hbn + gj, gj, gid);
+                    const int* ids = reinterpret_cast<const int*>(stg + L.hnext) + (cn.halo_off & 3);
+                    for (int j = lane; j < cn.n_halo; j += 32) halo_gather_async<R, MODE, PROJ>(a, L, stn, hbn + j, j, ids[j]);
                 }
                 cp_async_mbar_arrive(bar + 2 * (st ^ 1));
             }
-            // ---- halo nodes of this chunk: gathered values -> prologue -> new direction in their stage slots
-            {   // by the middle warps (the low warps run the interior prologue, the top ones issue the prefetch)
-                const int j = (tid + kTPB / 2) & (kTPB - 1);  // thread kTPB/2 takes halo node 0
-                if (j < cm.n_halo) halo_prologue<R, MODE, PROJ>(sc, L, stg, hb + j, j);
-            }
-            for (int j = tid + kTPB; j < cm.n_halo; j += kTPB) {  // more halo nodes than threads: not prefetched
-                halo_gather_async<R, MODE, PROJ>(a, L, stg, hb + j, j, __ldg(a.halo_ids + cm.halo_off + j));
-                cp_async_wait_all();
-                halo_prologue<R, MODE, PROJ>(sc, L, stg, hb + j, j);
-            }
-
             // ---- interior nodes: apply the previous step, form the new direction (owner writes)
-            if (MODE == DM_CG) {
-                for (int i = tid; i < cm.n_int; i += kTPB) {
+            // (workers only, one local node each: interior nodes, then the halo nodes whose gathered values become the
+            // new direction in their stage slots)
+            if (MODE == DM_CG && !issuer) {
+                for (int i = tid; i < nloc; i += kWorkers) {
+                    if (i >= cm.n_int) { halo_prologue<R, MODE, PROJ>(sc, L, stg, hb + i - cm.n_int, i - cm.n_int); continue; }
                     const int s = shift + i, gid = cm.node_start + i;
                     R x = R(0), r = s_r[s], p = R(0), q = R(0), lb = R(0);
                     const R dinv = s_dinv[s];
@@ -396,10 +392,10 @@ __global__ void __launch_bounds__(kTPB, 3) dmg_iter_chunk(const DmgArgs<R> a)
                     }
                 }
             }
-            __syncthreads();
+            if (!issuer) asm volatile("bar.sync 1, %0;" ::"n"(kWorkers) : "memory");  // workers only
 
-            // ---- element pass
-            for (int e = tid; e < cm.n_elem; e += kTPB) {
+            // ---- element pass (workers)
+            for (int e = tid; e < (issuer ? 0 : cm.n_elem); e += kWorkers) {
                 const ushort4 c = s_lconn[e];
                 R cm_, w12, w13, w23, q1, q2, q3;
                 Geo<R>::load_smem(s_geo, e, EC, cm_, w12, w13, w23);  // the staged "geometry" is the coefficient stream

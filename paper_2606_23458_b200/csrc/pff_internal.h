@@ -37,6 +37,7 @@ struct StageLayout {
     uint32_t slot_base;    // the per-element result slots (one copy; only one stage computes at a time)
     uint32_t slot_stride;  // kind 2: bytes between the q, D, b slot arrays
     uint32_t meta;         // persistent kernels: ring of ChunkMeta of the chunks this CTA owns
+    uint32_t hid0;         // persistent kernels: halo ids of the CTA's FIRST chunk (re-gathered every CG iteration)
     uint32_t bar;          // one mbarrier per stage
     uint32_t total;
 };
@@ -70,6 +71,7 @@ inline StageLayout make_stage_layout(int kind, int EC, int node_len, int flag_le
     if (kind == 1) { L.slot_base = o; o += up16(rb * (size_t(3) * EC + 1)); }
     if (kind == 2) { L.slot_base = o; L.slot_stride = up16(rb * (size_t(3) * EC + 1)); o += 3 * L.slot_stride; }
     L.meta = o; o += n_stages > 1 ? uint32_t(32 * kMetaCap) : 0;
+    L.hid0 = o; o += up16(n_stages > 1 ? size_t(4) * max_nhalo : 0);
     L.bar = o; o += 16 * uint32_t(n_stages);
     L.total = o;
     return L;
