@@ -611,11 +611,11 @@ __global__ void __launch_bounds__(kTPB, 2) dmg_setup_chunk(const DmgArgs<R> a)
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem + L.bar);
     const int tid = threadIdx.x, lane = tid & 31, G = gridDim.x, EC = a.EC;
     const int n_my = (a.C - (int)blockIdx.x + G - 1) / G;
-    const bool issuer = tid >= kTPB - 32;
+    constexpr int kWorkers = kTPB - 32;  // the last warp is the producer (bulk copies + halo gathers), as in the CG kernel
+    const bool issuer = tid >= kWorkers;
     const bool have_desc = issuer && lane < a.plan.n;
     StageDesc my_desc{};
     if (have_desc) my_desc = a.plan.d[lane];
-    const int gj = kTPB - 1 - tid;  // halo node whose gather this thread issues
 
     if (tid == 0) {
         mbar_init(bar, 1 + kTPB); mbar_init(bar + 2, 1 + kTPB);
@@ -640,9 +640,10 @@ __global__ void __launch_bounds__(kTPB, 2) dmg_setup_chunk(const DmgArgs<R> a)
                 fence_proxy_async();
                 stage_issue_desc(my_desc, have_desc, stg, bar + 2 * (it & 1), lane, cr);
             }
-            if (gj < cm.n_halo) {
+            if (issuer) {
                 const int hb0 = ((cm.node_start & (A - 1)) + cm.n_int + A - 1) & ~(A - 1);
-                cp_async<B>(reinterpret_cast<R*>(stg + L.node[0]) + hb0 + gj, a.x + __ldg(a.halo_ids + cm.halo_off + gj));
+                for (int j = lane; j < cm.n_halo; j += 32)
+                    cp_async<B>(reinterpret_cast<R*>(stg + L.node[0]) + hb0 + j, a.x + __ldg(a.halo_ids + cm.halo_off + j));
             }
             cp_async_mbar_arrive(bar + 2 * (it & 1));
         }
@@ -672,17 +673,15 @@ __global__ void __launch_bounds__(kTPB, 2) dmg_setup_chunk(const DmgArgs<R> a)
                     fence_proxy_async();
                     stage_issue_desc(my_desc, have_desc, stn, bar + 2 * (st ^ 1), lane, cr);
                 }
-                if (gj < cn.n_halo) {
+                if (issuer) {
                     const int hbn = ((cn.node_start & (A - 1)) + cn.n_int + A - 1) & ~(A - 1);
-                    const int gid = reinterpret_cast<const int*>(stg + L.hnext)[(cn.halo_off & 3) + gj];
-                    cp_async<B>(reinterpret_cast<R*>(stn + L.node[0]) + hbn + gj, a.x + gid);
+                    const int* ids = reinterpret_cast<const int*>(stg + L.hnext) + (cn.halo_off & 3);
+                    for (int j = lane; j < cn.n_halo; j += 32) cp_async<B>(reinterpret_cast<R*>(stn + L.node[0]) + hbn + j, a.x + ids[j]);
                 }
                 cp_async_mbar_arrive(bar + 2 * (st ^ 1));
             }
-            for (int j = tid + kTPB; j < cm.n_halo; j += kTPB) s_x[hb + j] = a.x[__ldg(a.halo_ids + cm.halo_off + j)];
-            if (cm.n_halo > kTPB) __syncthreads();
 
-            for (int e = tid; e < cm.n_elem; e += kTPB) {
+            for (int e = tid; e < (issuer ? 0 : cm.n_elem); e += kWorkers) {  // element pass: workers only
                 const ushort4 c = s_lconn[e];
                 R b1, c1, b2, c2, q1, q2, q3;
                 Geo<R>::load_smem(s_geo, e, EC, b1, c1, b2, c2);

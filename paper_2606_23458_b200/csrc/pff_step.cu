@@ -141,11 +141,13 @@ __global__ void __launch_bounds__(kTPB, 2) step_chunk_kernel(const StepArgs<R> a
     const int tid = threadIdx.x, lane = tid & 31, G = gridDim.x, EC = a.EC;
     const int n_my = (a.C - (int)blockIdx.x + G - 1) / G;  // chunks this CTA owns
     // the LAST warp issues the bulk copies (one lane per array); the halo gathers are issued from the top thread down
-    const bool issuer = tid >= kTPB - 32;
+    // the LAST warp is the producer (bulk copies + all halo gathers of the next chunk); the other kWorkers threads run the
+    // predictor and the element pass and synchronise between them on a named barrier; the producer rejoins for the gather
+    constexpr int kWorkers = kTPB - 32;
+    const bool issuer = tid >= kWorkers;
     const bool have_desc = issuer && lane < a.plan.n;
     StageDesc my_desc{};
     if (have_desc) my_desc = a.plan.d[lane];
-    const int gj = kTPB - 1 - tid;
 
     if (tid == 0) {
         mbar_init(bar, 1 + kTPB); mbar_init(bar + 2, 1 + kTPB);
@@ -167,9 +169,10 @@ __global__ void __launch_bounds__(kTPB, 2) step_chunk_kernel(const StepArgs<R> a
                 fence_proxy_async();
                 stage_issue_desc(my_desc, have_desc, stg, bar + 2 * (it & 1), lane, cr);
             }
-            if (gj < cm.n_halo) {
+            if (issuer) {
                 const int hb0 = ((cm.node_start & (A - 1)) + cm.n_int + A - 1) & ~(A - 1);
-                step_halo_gather<R, MODE>(a, L, stg, hb0 + gj, gj, __ldg(a.halo_ids + cm.halo_off + gj));
+                for (int j = lane; j < cm.n_halo; j += 32)
+                    step_halo_gather<R, MODE>(a, L, stg, hb0 + j, j, __ldg(a.halo_ids + cm.halo_off + j));
             }
             cp_async_mbar_arrive(bar + 2 * (it & 1));
         }
@@ -210,23 +213,17 @@ __global__ void __launch_bounds__(kTPB, 2) step_chunk_kernel(const StepArgs<R> a
                     fence_proxy_async();
                     stage_issue_desc(my_desc, have_desc, stn, bar + 2 * (st ^ 1), lane, cr);
                 }
-                if (gj < cn.n_halo) {
+                if (issuer) {
                     const int hbn = ((cn.node_start & (A - 1)) + cn.n_int + A - 1) & ~(A - 1);
-                    const int gid = reinterpret_cast<const int*>(stg + L.hnext)[(cn.halo_off & 3) + gj];
-                    step_halo_gather<R, MODE>(a, L, stn, hbn + gj, gj, gid);
+                    const int* ids = reinterpret_cast<const int*>(stg + L.hnext) + (cn.halo_off & 3);
+                    for (int j = lane; j < cn.n_halo; j += 32) step_halo_gather<R, MODE>(a, L, stn, hbn + j, j, ids[j]);
                 }
                 cp_async_mbar_arrive(bar + 2 * (st ^ 1));
             }
-            for (int j = tid + kTPB; j < cm.n_halo; j += kTPB) {  // more halo nodes than threads: not prefetched
-                step_halo_gather<R, MODE>(a, L, stg, hb + j, j, __ldg(a.halo_ids + cm.halo_off + j));
-                cp_async_wait_all();
-            }
-            if (cm.n_halo > kTPB) __syncthreads();
-
             // ---- phase 1: predictor (Eq. 16) in place, halo nodes by the middle warps, interior by the low warps;
             // Dirichlet dofs hold u_bar already (dirichlet_kernel)
-            if (MODE == MODE_STEP) {
-                for (int j = (tid + kTPB / 2) & (kTPB - 1); j < cm.n_halo; j += kTPB) {
+            if (MODE == MODE_STEP && !issuer) {
+                for (int j = (tid + kWorkers / 2) % kWorkers; j < cm.n_halo; j += kWorkers) {
                     const int s = hb + j, gid = reinterpret_cast<const int*>(stg + L.hids)[j];
                     const unsigned fl = reinterpret_cast<const unsigned*>(stg + L.hflag)[j] >> (8 * (gid & 3));
                     const R ux = s_ux[s], uy = s_uy[s];
@@ -235,7 +232,7 @@ __global__ void __launch_bounds__(kTPB, 2) step_chunk_kernel(const StepArgs<R> a
                     s_ux[s] = (fl & 1) ? ux : px;
                     s_uy[s] = (fl & 2) ? uy : py;
                 }
-                for (int i = tid; i < cm.n_int; i += kTPB) {
+                for (int i = tid; i < cm.n_int; i += kWorkers) {
                     const int s = shift + i;
                     const uint8_t fl = s_flags[fshift + i];
                     const R ux = s_ux[s], uy = s_uy[s];
@@ -245,10 +242,10 @@ __global__ void __launch_bounds__(kTPB, 2) step_chunk_kernel(const StepArgs<R> a
                     s_uy[s] = (fl & 2) ? uy : py;
                 }
             }
-            __syncthreads();
+            if (!issuer) asm volatile("bar.sync 1, %0;" ::"n"(kWorkers) : "memory");  // workers only
 
-            // ---- phase 2: fused element pass; nodal force pairs go to the slots corner * EC + e
-            for (int e = tid; e < cm.n_elem; e += kTPB) {
+            // ---- phase 2: fused element pass (workers); nodal force pairs go to the slots corner * EC + e
+            for (int e = tid; e < (issuer ? 0 : cm.n_elem); e += kWorkers) {
                 const ushort4 c = s_lconn[e];
                 R b1, c1, b2, c2;
                 Geo<R>::load_smem(s_geo, e, EC, b1, c1, b2, c2);
