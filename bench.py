@@ -68,7 +68,7 @@ class ClockSampler:
         self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                       "-lms", "100"], stdout=self.f, stderr=subprocess.DEVNULL)
+                                       "-lms", "20"], stdout=self.f, stderr=subprocess.DEVNULL)
         except OSError:
             self.p = None
 
@@ -146,9 +146,9 @@ def run_ours(args, rank: int, world: int):
         barrier()
         return reduce_max(e0.elapsed_time(e1), world, f"cuda:{dev}"), out
 
+    clocks = ClockSampler(dev)  # started before the warm-up so that nvidia-smi is sampling when the timed region runs
     for _ in range(args.warmup):
         step()
-    clocks = ClockSampler(dev)
     l0 = mesh.pff_mesh_counters()
     # the timed region: K staggered steps through ONE C-ABI call (pff_run_steps: device-resident state, the time loop
     # runs in the library and never waits for the host between steps; control blocks are read back asynchronously)
