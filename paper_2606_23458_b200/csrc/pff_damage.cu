@@ -23,7 +23,6 @@
 
 #include "pff_device.cuh"
 #include "pff_mesh.h"
-#include <cooperative_groups.h>
 
 #include "pff_tma.cuh"
 
@@ -108,6 +107,25 @@ __device__ __forceinline__ void block_reduce_ch(double v[kCh], double* s_w /* [k
 }
 
 enum { DM_CG = 0, DM_PLAIN = 1 };
+
+// Grid-wide barrier of the cooperative CG kernel (all CTAs are co-resident): one arrival per CTA on a counter that only
+// grows during a launch (zeroed by the host before it), thread 0 spins with acquire loads until the epoch's target.
+// The gpu-scope fences order the CTA's global writes before the arrival and invalidate L1 after the wait.
+__device__ __forceinline__ void grid_barrier(unsigned int* counter, unsigned int& target, unsigned int G)
+{
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        target += G;
+        __threadfence();
+        atomicAdd(counter, 1u);
+        unsigned int seen;
+        do {
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(counter) : "memory");
+        } while (seen < target);
+        __threadfence();
+    }
+    __syncthreads();
+}
 
 
 struct IterScalars {
@@ -288,6 +306,7 @@ __global__ void __launch_bounds__(kTPB, 3) dmg_iter_chunk(const DmgArgs<R> a)
     double acc[kCh];
     const bool single_epoch = n_my <= kMetaCap;
     bool pre_issued = false;  // the next CG iteration's first chunk is already streaming in
+    unsigned int gb_target = 0;  // grid-barrier epoch target (thread 0)
     int it = 0;  // stage uses so far (global over epochs and CG iterations): stage = it & 1, mbarrier parity = (it >> 1) & 1
     if (MODE == DM_CG) {
         __syncthreads();  // s_ctrl loaded
@@ -433,7 +452,7 @@ __global__ void __launch_bounds__(kTPB, 3) dmg_iter_chunk(const DmgArgs<R> a)
     if (MODE != DM_CG) break;
     // ---- interface nodes (owned by no chunk): ordered sum of the chunk partials, same prologue; grid-wide phase
     fence_proxy_async_global();
-    cooperative_groups::this_grid().sync();
+    grid_barrier(a.ticket + 1, gb_target, (unsigned)G);
     if (single_epoch) {  // every interior value is final: start streaming the first chunk of the next CG iteration
         if (issuer) {
             const ChunkMeta cm = s_meta[0];
@@ -472,7 +491,7 @@ __global__ void __launch_bounds__(kTPB, 3) dmg_iter_chunk(const DmgArgs<R> a)
     block_reduce_ch(acc, s_w, s_out);
     if (tid < kCh) a.part[(int64_t)tid * a.part_n + blockIdx.x] = s_out[tid];
     fence_proxy_async_global();
-    cooperative_groups::this_grid().sync();
+    grid_barrier(a.ticket + 1, gb_target, (unsigned)G);
     // ---- every CTA reduces all block partials in the same fixed order and advances its copy of the scalars
     {
         const int w = tid >> 5;
@@ -855,8 +874,8 @@ static pff_status ensure_workspace(pff_mesh* m)
     if ((st = cuda_check(cudaMalloc((void**)&m->d_part, sizeof(double) * kCh * m->n_part_blocks), "damage: partials")) != PFF_OK) return st;
     if ((st = cuda_check(cudaMalloc((void**)&m->d_part2, sizeof(double) * kCh * kMaxSharedBlocks), "damage: partials 2")) != PFF_OK) return st;
     if ((st = cuda_check(cudaMalloc((void**)&m->d_ctrl, sizeof(DamageCtrl)), "damage: ctrl")) != PFF_OK) return st;
-    if ((st = cuda_check(cudaMalloc((void**)&m->d_ticket, sizeof(unsigned int)), "damage: ticket")) != PFF_OK) return st;
-    if ((st = cuda_check(cudaMemset(m->d_ticket, 0, sizeof(unsigned int)), "damage: ticket")) != PFF_OK) return st;
+    if ((st = cuda_check(cudaMalloc((void**)&m->d_ticket, 2 * sizeof(unsigned int)), "damage: ticket")) != PFF_OK) return st;  // [0] last-block ticket, [1] grid barrier
+    if ((st = cuda_check(cudaMemset(m->d_ticket, 0, 2 * sizeof(unsigned int)), "damage: ticket")) != PFF_OK) return st;
     if ((st = cuda_check(cudaMallocHost((void**)&m->h_ctrl, 2 * sizeof(DamageCtrl)), "damage: pinned ctrl")) != PFF_OK) return st;
     return PFF_OK;
 }
@@ -907,6 +926,7 @@ static pff_status damage_solve_t(pff_mesh* m, pff_state* s, double rel_tol, int 
     asu.n_chunk_blocks = (int)gsu;
     PFF_LAUNCH(m, PFF_K_DAMAGE_SETUP, (dmg_setup_chunk<R, false><<<gsu, kTPB, smem_su, cs>>>(asu)));
     PFF_LAUNCH(m, PFF_K_DAMAGE_SETUP, (dmg_setup_shared<R, false><<<gs, kTPB, 0, cs>>>(asu)));
+    if ((st = cuda_check(cudaMemsetAsync(m->d_ticket + 1, 0, sizeof(unsigned int), cs), "damage: barrier reset")) != PFF_OK) return st;
     // ONE cooperative launch runs every CG iteration (grid-wide barriers between the chunk phase, the interface
     // phase and the scalar recurrence), applies the last step and the clamp, and writes the control block back
     {
