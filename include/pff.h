@@ -204,18 +204,18 @@ pff_status pff_damage_rhs_diag(pff_mesh *mesh, const pff_state *state, void *b, 
 pff_status pff_mesh_counters(const pff_mesh *mesh, int64_t *kernel_launches);
 /* Launches ONE kernel of the hot path `reps` times back to back on the mesh stream between two CUDA
  * events (after one untimed launch) and returns the mean milliseconds per launch.  which: 0 = fused
- * chunk step kernel (PFF_SCATTER_ATOMIC: element kernel), 1 = interface-node step kernel (ATOMIC: node
- * kernel), 2 = damage mat-vec chunk kernel, 3 = damage mat-vec interface kernel.  The step kernels
+ * explicit step kernel (PFF_SCATTER_ATOMIC: element kernel), 1 = the same kernel for gather meshes, whose interface-node
+ * pass is fused into it (ATOMIC: node kernel), 2 = damage mat-vec chunk kernel, 3 = damage mat-vec interface kernel.  The step kernels
  * advance the state with a negligible dt; the mat-vec reads state->d as the trial vector.  Synchronises. */
 pff_status pff_time_kernel(pff_mesh *mesh, pff_state *state, int32_t which, int32_t reps, float *ms_per_launch);
 
 /* Kernel classes of the hot path, for per-kernel timing inside a real run (bench.py's roofline block). */
 typedef enum {
-    PFF_K_STEP_CHUNK = 0,      /* fused element force + history + node update, one CTA per chunk (ATOMIC: element kernel) */
-    PFF_K_STEP_SHARED = 1,     /* interface-node update (ATOMIC: node kernel)                                            */
-    PFF_K_MATVEC_CHUNK = 2,    /* damage operator apply + direction update + p.q partials                                */
-    PFF_K_MATVEC_SHARED = 3,   /* interface nodes of the operator apply + alpha                                          */
-    PFF_K_CG_VECTOR = 4,       /* x, r update, free set, r.z / ||r|| partials, beta                                      */
+    PFF_K_STEP_CHUNK = 0,      /* the explicit step kernel: chunk phase + interface phase (ATOMIC: element kernel)       */
+    PFF_K_STEP_SHARED = 1,     /* ATOMIC only: node kernel                                                               */
+    PFF_K_MATVEC_CHUNK = 2,    /* the cooperative CG kernel (all iterations of one solve); plain mat-vec of the hook     */
+    PFF_K_MATVEC_SHARED = 3,   /* interface nodes of the hook's plain mat-vec                                            */
+    PFF_K_CG_VECTOR = 4,       /* unused (the vector updates are fused into the CG kernel)                               */
     PFF_K_DAMAGE_SETUP = 5,    /* rhs, Jacobi diagonal, r0 (chunk + interface kernels), finalize clamp                    */
     PFF_K_OTHER = 6,           /* Dirichlet overwrite, energies, host-path permutation kernels                            */
     PFF_NUM_KERNEL_CLASSES = 7

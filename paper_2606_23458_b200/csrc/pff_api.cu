@@ -71,7 +71,7 @@ void pff_mesh_destroy(pff_mesh* m)
     void* ptrs[] = {m->d_meta, m->d_lconn, m->d_conn, m->d_ga, m->d_gb, m->d_area, m->d_minv, m->d_mass,
                     m->d_halo_ids, m->d_sh_rowptr, m->d_halo_dst, m->d_ell, m->d_flags, m->d_halo_part,
                     m->d_fwx, m->d_fwy, m->d_dir_dof, m->d_ca, m->d_cb, m->d_lb, m->d_r, m->d_p, m->d_q, m->d_dinv, m->d_mask,
-                    m->d_part, m->d_part2, m->d_ctrl, m->d_ticket, m->d_stage, m->d_hstate, m->d_node_old_of_new,
+                    m->d_part, m->d_part2, m->d_ctrl, m->d_ticket, m->d_step_bar, m->d_stage, m->d_hstate, m->d_node_old_of_new,
                     m->d_elem_old_of_new};
     for (void* p : ptrs) if (p) cudaFree(p);
     if (m->h_ctrl) cudaFreeHost(m->h_ctrl);
@@ -172,6 +172,7 @@ pff_status pff_mesh_create(int64_t n_nodes, const double* xy, int64_t n_elems, c
     UP(upload((uint8_t**)&m->d_q, nullptr, N * m->rb, cs));
     UP(upload((uint8_t**)&m->d_dinv, nullptr, N * m->rb, cs));
     UP(upload(&m->d_mask, nullptr, 2 * N, cs));
+    UP(upload(&m->d_step_bar, nullptr, 1, cs));
     UP(upload(&m->d_node_old_of_new, hm.node_old_of_new.data(), N, cs));
     {
         std::vector<int32_t> eon(Ne);

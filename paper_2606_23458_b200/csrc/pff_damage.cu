@@ -108,25 +108,6 @@ __device__ __forceinline__ void block_reduce_ch(double v[kCh], double* s_w /* [k
 
 enum { DM_CG = 0, DM_PLAIN = 1 };
 
-// Grid-wide barrier of the cooperative CG kernel (all CTAs are co-resident): one arrival per CTA on a counter that only
-// grows during a launch (zeroed by the host before it), thread 0 spins with acquire loads until the epoch's target.
-// The gpu-scope fences order the CTA's global writes before the arrival and invalidate L1 after the wait.
-__device__ __forceinline__ void grid_barrier(unsigned int* counter, unsigned int& target, unsigned int G)
-{
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        target += G;
-        __threadfence();
-        atomicAdd(counter, 1u);
-        unsigned int seen;
-        do {
-            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(counter) : "memory");
-        } while (seen < target);
-        __threadfence();
-    }
-    __syncthreads();
-}
-
 
 struct IterScalars {
     double alpha, beta;

@@ -63,6 +63,8 @@ struct pff_mesh {
     DamageCtrl* h_ring = nullptr;      // pinned ring of deferred read-backs (pff_run_steps)
     DamageCtrl* defer_slot = nullptr;  // non-null: damage_solve copies the control block here and does not synchronise
     unsigned int* d_ticket = nullptr;
+    unsigned int* d_step_bar = nullptr;  // grid-barrier counter of the step kernel
+    unsigned int step_bar_count = 0;     // its value after the launches enqueued so far
 
     // host-path staging (pff_run_host)
     void* d_stage = nullptr; size_t stage_bytes = 0;

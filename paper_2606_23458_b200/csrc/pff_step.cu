@@ -8,7 +8,8 @@
 //                       to shared-memory slots; phase 3 gathers each node's incident slots in a fixed order
 //                       (chunk-local ELL table) and, for interior nodes, completes Eq. 17-18 in the same
 //                       kernel -- f_int never reaches HBM.  Interface nodes get one partial sum per chunk.
-//   step_shared_kernel  interface nodes: ordered sum of the per-chunk partials, then the same Eq. 16-18.
+//                       After a grid-wide barrier (cooperative launch) the same kernel finishes the interface
+//                       nodes: ordered sum of the per-chunk partials, then the same Eq. 16-18.
 //   elem_atomic_kernel / node_atomic_kernel   PFF_SCATTER_ATOMIC variant: thread per element, global
 //                       floating-point atomics (the paper's "atomic indexed accumulation", L43, L124).
 //   dirichlet_kernel    writes u_bar, v_bar into the Dirichlet dofs before the step (Eq. 5, R8).
@@ -38,6 +39,8 @@ struct StepArgs {
     int EC, N, Ne, N_int, N_sh, n_ovf, C;
     int64_t ell_total, n_entries;
     const int32_t *sh_rowptr, *halo_dst;
+    unsigned int* gbar;    // grid-barrier arrival counter (grows from launch to launch)
+    unsigned int gb_base;  // its value before this launch
     StageLayout lay;
     StagePlan plan;
     R *ux, *uy, *vx, *vy, *ax, *ay;
@@ -297,19 +300,21 @@ __global__ void __launch_bounds__(kTPB, 2) step_chunk_kernel(const StepArgs<R> a
             __syncthreads();  // stage st and the slots are free again
         }
     }
-}
-
-template <typename R, int MODE>
-__global__ void __launch_bounds__(kTPB) step_shared_kernel(const StepArgs<R> a)
-{
-    const int s = blockIdx.x * kTPB + threadIdx.x;
-    if (s >= a.N_sh) return;
-    const int gid = a.N_int + s;
-    const R fx = iface_sum<R>(a.halo_part, s, a.N_sh, a.n_ovf, a.sh_rowptr);
-    const R fy = iface_sum<R>(a.halo_part + a.n_slots, s, a.N_sh, a.n_ovf, a.sh_rowptr);
-    R px, py;
-    predict<R, MODE>(a, gid, px, py);
-    finish_node<R, MODE>(a, gid, px, py, fx, fy);
+    // ---- interface nodes (owned by no chunk), after a grid-wide barrier: ordered sum of the per-chunk partials, then the
+    // same Eq. 16-18.  Every read of the OLD interface state by the chunk phase (halo gathers) precedes the barrier.
+    if (a.N_sh > 0) {
+        unsigned int target = a.gb_base;
+        grid_barrier(a.gbar, target, (unsigned)G);
+        const int per = (a.N_sh + G - 1) / G, end = min(a.N_sh, ((int)blockIdx.x + 1) * per);  // equal slice per CTA
+        for (int s = blockIdx.x * per + tid; s < end; s += kTPB) {
+            const int gid = a.N_int + s;
+            const R fx = iface_sum<R>(a.halo_part, s, a.N_sh, a.n_ovf, a.sh_rowptr);
+            const R fy = iface_sum<R>(a.halo_part + a.n_slots, s, a.N_sh, a.n_ovf, a.sh_rowptr);
+            R px, py;
+            predict<R, MODE>(a, gid, px, py);
+            finish_node<R, MODE>(a, gid, px, py, fx, fy);
+        }
+    }
 }
 
 // ---- atomic variant: warp-aggregated floating-point atomics -------------------------------------------
@@ -411,11 +416,22 @@ static pff_status launch_step_t(pff_mesh* m, const StepArgs<R>& a)
             grid = std::max(1, per_sm) * sms;
             grid_smem = (int)m->lay_step.total;
         }
-        if (m->only_kernel != 1) {
-            PFF_LAUNCH(m, PFF_K_STEP_CHUNK, (kern<<<(unsigned)std::min<int64_t>(grid, hm.C), kTPB, (int)m->lay_step.total, m->stream>>>(a)));
-        }
-        if (hm.N_sh > 0 && m->only_kernel != 0) {
-            PFF_LAUNCH(m, PFF_K_STEP_SHARED, (step_shared_kernel<R, MODE><<<(unsigned)((hm.N_sh + kTPB - 1) / kTPB), kTPB, 0, m->stream>>>(a)));
+        {   // ONE cooperative launch: chunk phase, grid barrier, interface phase (all CTAs co-resident by construction)
+            const unsigned g = (unsigned)std::min<int64_t>(grid, hm.C);
+            StepArgs<R> b = a;
+            b.gbar = m->d_step_bar;
+            b.gb_base = m->step_bar_count;
+            if (hm.N_sh > 0) m->step_bar_count += g;
+            if (m->step_bar_count > 0xF0000000u) {  // far from wrapping: restart the counter (stream-ordered)
+                cudaMemsetAsync(m->d_step_bar, 0, sizeof(unsigned int), m->stream);
+                b.gb_base = 0; m->step_bar_count = hm.N_sh > 0 ? g : 0;
+            }
+            void* kargs[] = {(void*)&b};
+            prof_mark(m, PFF_K_STEP_CHUNK);
+            cudaError_t e = cudaLaunchCooperativeKernel((const void*)kern, dim3(g), dim3(kTPB), kargs, (size_t)m->lay_step.total, m->stream);
+            prof_mark(m, PFF_K_STEP_CHUNK);
+            ++m->n_launches;
+            if (e != cudaSuccess) return cuda_check(e, "explicit step: cooperative launch");
         }
     }
     return cuda_check(cudaGetLastError(), "explicit step launch");

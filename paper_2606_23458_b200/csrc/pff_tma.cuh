@@ -136,6 +136,25 @@ __device__ __forceinline__ void stage_issue_plan(const StagePlan& plan, unsigned
     stage_issue_desc(d, have, stage, bar, lane, c);
 }
 
+// Grid-wide barrier of the cooperatively launched kernels (all CTAs are co-resident): one arrival per CTA on a counter that only
+// grows (zeroed by the host before the launch, or continued from launch to launch with a host-side epoch base), thread 0 spins with acquire loads until the epoch's target.
+// The gpu-scope fences order the CTA's global writes before the arrival and invalidate L1 after the wait.
+__device__ __forceinline__ void grid_barrier(unsigned int* counter, unsigned int& target, unsigned int G)
+{
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        target += G;
+        __threadfence();
+        atomicAdd(counter, 1u);
+        unsigned int seen;
+        do {
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(counter) : "memory");
+        } while (seen < target);
+        __threadfence();
+    }
+    __syncthreads();
+}
+
 __host__ __device__ __forceinline__ int round_up(int v, int a) { return (v + a - 1) / a * a; }
 
 }  // namespace pff
