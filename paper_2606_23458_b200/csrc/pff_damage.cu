@@ -1,11 +1,12 @@
 // Damage sub-problem (Eq. 6-8): matrix-free operator with consistent mass,
 // Jacobi-preconditioned CG (AT2, then clamp, L179) and projected CG with an active set (AT1, L181).
 //
-// pff_damage_solve = dmg_setup_chunk + dmg_setup_shared + ONE cooperative launch of dmg_iter_chunk<DM_CG>
+// pff_damage_solve = ONE cooperative launch of dmg_setup_chunk + ONE cooperative launch of dmg_iter_chunk<DM_CG>
 // (DESIGN.md "Damage solve"):
 //   dmg_setup_chunk   persistent, TMA-fed: rhs b, Jacobi diagonal, r0 = b - A d_n, lb = d_n, free-set mask, the
 //                     element operator in coefficient form (4 reals per element) and the block partials of the norms.
-//   dmg_setup_shared  the same for the interface nodes; its last block sets ||b||, ||r0|| in the control block.
+//                     After a grid barrier the same kernel handles the interface nodes; the last CTA to finish sets
+//                     ||b||, ||r0|| (and the zero-iteration flag) in the control block.
 //   dmg_iter_chunk    persistent + cooperative: runs EVERY CG iteration.  Per iteration: chunk phase (double-buffered
 //                     TMA stages, cp.async halo gathers one chunk ahead; node prologue applies the PREVIOUS step
 //                     x += alpha p, r -= alpha q, re-derives the free set on a restart and forms p = z + beta p;
@@ -537,42 +538,6 @@ finalize:
     }
 }
 
-// Folds this block's own values (s_out) with its slice of the chunk-kernel partials, publishes them, and in
-// the last block reduces everything in a fixed order.  Returns true in the last block with t[] valid in thread 0.
-__device__ __forceinline__ bool fold_and_finish(const double* part, int64_t part_n, int n_chunk_blocks, double* part2,
-                                                unsigned int* ticket, double* s_w, double* s_out, double t[kCh])
-{
-    const int tid = threadIdx.x, G = gridDim.x, b = blockIdx.x;
-    if (tid < kCh) {
-        const int per = (n_chunk_blocks + G - 1) / G;
-        const int c0 = b * per, c1 = min(n_chunk_blocks, c0 + per);
-        double v = s_out[tid];
-        for (int c = c0; c < c1; ++c) {
-            const double u = __ldcg(part + (int64_t)tid * part_n + c);
-            v = (tid == kCh - 1) ? fmin(v, u) : v + u;
-        }
-        part2[tid * kMaxSharedBlocks + b] = v;
-    }
-    if (!last_block(ticket)) return false;
-    const int w = tid >> 5, l = tid & 31;
-    if (w < kCh) {  // warp c: fixed-order strided sum of channel c, then the fixed shuffle tree
-        double v = (w == kCh - 1) ? INFINITY : 0.0;
-        for (int i = l; i < G; i += 32) {
-            const double u = __ldcg(part2 + w * kMaxSharedBlocks + i);
-            v = (w == kCh - 1) ? fmin(v, u) : v + u;
-        }
-        for (int o = 16; o > 0; o >>= 1) {
-            const double u = __shfl_xor_sync(0xffffffffu, v, o);
-            v = (w == kCh - 1) ? fmin(v, u) : v + u;
-        }
-        if (l == 0) s_w[w] = v;
-    }
-    __syncthreads();
-    if (tid == 0)
-        for (int c = 0; c < kCh; ++c) t[c] = s_w[c];
-    return true;
-}
-
 // interface nodes of a plain operator apply (test hook pff_damage_matvec): ordered sum of the chunk partials
 template <typename R>
 __global__ void __launch_bounds__(kTPB) dmg_plain_shared(const DmgArgs<R> a)
@@ -732,48 +697,51 @@ __global__ void __launch_bounds__(kTPB, 2) dmg_setup_chunk(const DmgArgs<R> a)
             __syncthreads();  // stage st and the slots are free again
         }
     }
-    if (!HOOK) {
-        block_reduce_ch(acc, s_w, s_out);
-        if (tid < kCh) a.part[(int64_t)tid * a.part_n + blockIdx.x] = s_out[tid];
-    }
-}
-
-template <typename R, bool HOOK>
-__global__ void __launch_bounds__(kTPB) dmg_setup_shared(const DmgArgs<R> a)
-{
-    __shared__ double s_w[kCh * 32], s_out[kCh];
-    double acc[kCh];
-#pragma unroll
-    for (int c = 0; c < kCh; ++c) acc[c] = 0.0;
-    for (int s = blockIdx.x * kTPB + threadIdx.x; s < a.N_sh; s += gridDim.x * kTPB) {
-        const int gid = a.N_int + s;
-        const R qs = iface_sum<R>(a.halo_part, s, a.N_sh, a.n_ovf, a.sh_rowptr);
-        const R Ds = iface_sum<R>(a.halo_part + a.n_slots, s, a.N_sh, a.n_ovf, a.sh_rowptr);
-        const R bs = iface_sum<R>(a.halo_part + 2 * a.n_slots, s, a.N_sh, a.n_ovf, a.sh_rowptr);
-        if (HOOK) {
-            if (a.b_out) a.b_out[gid] = bs;
-            if (a.D_out) a.D_out[gid] = Ds;
-        } else {
-            const R r = bs - qs;
-            const bool fixed = (a.flags[gid] & 4) != 0;
-            a.r[gid] = r; a.dinv[gid] = R(1) / Ds; a.lb[gid] = a.x[gid];
-            a.mask[gid] = fixed ? 2 : 1;
-            acc[0] += double(bs) * double(bs);
-            if (!fixed) acc[1] += double(r) * double(r);
-            if (!fixed && (a.mat.model != PFF_AT1 || r > R(0))) acc[2] += double(r) * double(r);
+    // ---- interface nodes after a grid-wide barrier: ordered sums of the three partial planes, same outputs
+    if (a.N_sh > 0) {
+        unsigned int target = 0;
+        grid_barrier(a.ticket + 2, target, (unsigned)G);
+        const int per = (a.N_sh + G - 1) / G, end = min(a.N_sh, ((int)blockIdx.x + 1) * per);  // equal slice per CTA
+        for (int sn = blockIdx.x * per + tid; sn < end; sn += kTPB) {
+            const int gid = a.N_int + sn;
+            const R qs = iface_sum<R>(a.halo_part, sn, a.N_sh, a.n_ovf, a.sh_rowptr);
+            const R Ds = iface_sum<R>(a.halo_part + a.n_slots, sn, a.N_sh, a.n_ovf, a.sh_rowptr);
+            const R bs = iface_sum<R>(a.halo_part + 2 * a.n_slots, sn, a.N_sh, a.n_ovf, a.sh_rowptr);
+            if (HOOK) {
+                if (a.b_out) a.b_out[gid] = bs;
+                if (a.D_out) a.D_out[gid] = Ds;
+            } else {
+                const R r = bs - qs;
+                const bool fixed = (a.flags[gid] & 4) != 0;
+                a.r[gid] = r; a.dinv[gid] = R(1) / Ds; a.lb[gid] = a.x[gid];
+                a.mask[gid] = fixed ? 2 : 1;
+                acc[0] += double(bs) * double(bs);
+                if (!fixed) acc[1] += double(r) * double(r);
+                if (!fixed && (a.mat.model != PFF_AT1 || r > R(0))) acc[2] += double(r) * double(r);
+            }
         }
     }
     if (HOOK) return;
-    acc[kCh - 1] = INFINITY;
+    // ---- norms: one block reduction per CTA; the last CTA to arrive sums the block partials in a fixed order
+    __syncthreads();
     block_reduce_ch(acc, s_w, s_out);
-    double t[kCh];
-    if (fold_and_finish(a.part, a.part_n, a.n_chunk_blocks, a.part2, a.ticket, s_w, s_out, t) && threadIdx.x == 0)
-    {
-        DamageCtrl* c = a.ctrl;
-        c->nb = fmax(fmax(sqrt(t[0]), sqrt(t[1])), 1e-300);
-        // d_n already solves the system to the tolerance (no history growth since the last solve; AT1: KKT holds with the
-        // free set the solver would start from): no CG iteration is needed, the cooperative kernel only clamps
-        if (sqrt(t[2]) <= c->tol * c->nb) { c->done = 1; c->status = PFF_OK; c->relres = sqrt(t[2]) / c->nb; c->pending = 0; }
+    if (tid < kCh) a.part[(int64_t)tid * a.part_n + blockIdx.x] = s_out[tid];
+    if (last_block(a.ticket)) {
+        const int w = tid >> 5;
+        if (w < 3) {
+            double v = 0.0;
+            for (int i = lane; i < G; i += 32) v += __ldcg(a.part + (int64_t)w * a.part_n + i);
+            for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+            if (lane == 0) s_out[w] = v;
+        }
+        __syncthreads();
+        if (tid == 0) {
+            DamageCtrl* c = a.ctrl;
+            c->nb = fmax(fmax(sqrt(s_out[0]), sqrt(s_out[1])), 1e-300);
+            // d_n already solves the system to the tolerance (no history growth since the last solve; AT1: KKT holds with
+            // the free set the solver would start from): no CG iteration is needed, the cooperative kernel only clamps
+            if (sqrt(s_out[2]) <= c->tol * c->nb) { c->done = 1; c->status = PFF_OK; c->relres = sqrt(s_out[2]) / c->nb; c->pending = 0; }
+        }
     }
 }
 
@@ -855,8 +823,8 @@ static pff_status ensure_workspace(pff_mesh* m)
     if ((st = cuda_check(cudaMalloc((void**)&m->d_part, sizeof(double) * kCh * m->n_part_blocks), "damage: partials")) != PFF_OK) return st;
     if ((st = cuda_check(cudaMalloc((void**)&m->d_part2, sizeof(double) * kCh * kMaxSharedBlocks), "damage: partials 2")) != PFF_OK) return st;
     if ((st = cuda_check(cudaMalloc((void**)&m->d_ctrl, sizeof(DamageCtrl)), "damage: ctrl")) != PFF_OK) return st;
-    if ((st = cuda_check(cudaMalloc((void**)&m->d_ticket, 2 * sizeof(unsigned int)), "damage: ticket")) != PFF_OK) return st;  // [0] last-block ticket, [1] grid barrier
-    if ((st = cuda_check(cudaMemset(m->d_ticket, 0, 2 * sizeof(unsigned int)), "damage: ticket")) != PFF_OK) return st;
+    if ((st = cuda_check(cudaMalloc((void**)&m->d_ticket, 3 * sizeof(unsigned int)), "damage: ticket")) != PFF_OK) return st;  // [0] last-block ticket, [1] CG grid barrier, [2] setup grid barrier
+    if ((st = cuda_check(cudaMemset(m->d_ticket, 0, 3 * sizeof(unsigned int)), "damage: ticket")) != PFF_OK) return st;
     if ((st = cuda_check(cudaMallocHost((void**)&m->h_ctrl, 2 * sizeof(DamageCtrl)), "damage: pinned ctrl")) != PFF_OK) return st;
     return PFF_OK;
 }
@@ -897,7 +865,6 @@ static pff_status damage_solve_t(pff_mesh* m, pff_state* s, double rel_tol, int 
     std::memset(&h[0], 0, sizeof(DamageCtrl));
     h[0].tol = rel_tol; h[0].max_iter = max_iter; h[0].first = 1; h[0].restart = 1; h[0].status = PFF_ENOCONV;
     if ((st = cuda_check(cudaMemcpyAsync(m->d_ctrl, &h[0], sizeof(DamageCtrl), cudaMemcpyHostToDevice, cs), "damage: ctrl upload")) != PFF_OK) return st;
-    const unsigned gs = shared_grid(hm);
     static int grid_su = 0, grid_su_smem = -1;
     if (grid_su_smem != smem_su) {
         if ((st = persistent_grid(m, dmg_setup_chunk<R, false>, smem_su, &grid_su)) != PFF_OK) return st;
@@ -905,9 +872,15 @@ static pff_status damage_solve_t(pff_mesh* m, pff_state* s, double rel_tol, int 
     }
     const unsigned gsu = (unsigned)std::min<int64_t>(grid_su, hm.C);
     asu.n_chunk_blocks = (int)gsu;
-    PFF_LAUNCH(m, PFF_K_DAMAGE_SETUP, (dmg_setup_chunk<R, false><<<gsu, kTPB, smem_su, cs>>>(asu)));
-    PFF_LAUNCH(m, PFF_K_DAMAGE_SETUP, (dmg_setup_shared<R, false><<<gs, kTPB, 0, cs>>>(asu)));
-    if ((st = cuda_check(cudaMemsetAsync(m->d_ticket + 1, 0, sizeof(unsigned int), cs), "damage: barrier reset")) != PFF_OK) return st;
+    if ((st = cuda_check(cudaMemsetAsync(m->d_ticket + 1, 0, 2 * sizeof(unsigned int), cs), "damage: barrier reset")) != PFF_OK) return st;
+    {   // setup pass: chunk phase, grid barrier, interface phase, norms (cooperative: all CTAs co-resident)
+        void* kargs[] = {(void*)&asu};
+        prof_mark(m, PFF_K_DAMAGE_SETUP);
+        cudaError_t e = cudaLaunchCooperativeKernel((const void*)dmg_setup_chunk<R, false>, dim3(gsu), dim3(kTPB), kargs, (size_t)smem_su, cs);
+        prof_mark(m, PFF_K_DAMAGE_SETUP);
+        ++m->n_launches;
+        if ((st = cuda_check(e, "damage: setup launch")) != PFF_OK) return st;
+    }
     // ONE cooperative launch runs every CG iteration (grid-wide barriers between the chunk phase, the interface
     // phase and the scalar recurrence), applies the last step and the clamp, and writes the control block back
     {
@@ -987,8 +960,16 @@ static pff_status damage_rhs_diag_t(pff_mesh* m, const pff_state* s, void* b, vo
     if ((st = set_smem(dmg_setup_chunk<R, true>, smem_su, g_su)) != PFF_OK) return st;
     int grid_su = 0;
     if ((st = persistent_grid(m, dmg_setup_chunk<R, true>, smem_su, &grid_su)) != PFF_OK) return st;
-    PFF_LAUNCH(m, PFF_K_DAMAGE_SETUP, (dmg_setup_chunk<R, true><<<(unsigned)grid_su, kTPB, smem_su, m->stream>>>(a)));
-    PFF_LAUNCH(m, PFF_K_DAMAGE_SETUP, (dmg_setup_shared<R, true><<<shared_grid(m->hm), kTPB, 0, m->stream>>>(a)));
+    if ((st = cuda_check(cudaMemsetAsync(m->d_ticket + 1, 0, 2 * sizeof(unsigned int), m->stream), "damage: barrier reset")) != PFF_OK) return st;
+    {
+        void* kargs[] = {(void*)&a};
+        prof_mark(m, PFF_K_DAMAGE_SETUP);
+        cudaError_t e = cudaLaunchCooperativeKernel((const void*)dmg_setup_chunk<R, true>, dim3((unsigned)std::min<int64_t>(grid_su, m->hm.C)), dim3(kTPB), kargs,
+                                                    (size_t)smem_su, m->stream);
+        prof_mark(m, PFF_K_DAMAGE_SETUP);
+        ++m->n_launches;
+        if ((st = cuda_check(e, "damage rhs/diag launch")) != PFF_OK) return st;
+    }
     return cuda_check(cudaGetLastError(), "damage rhs/diag launch");
 }
 
