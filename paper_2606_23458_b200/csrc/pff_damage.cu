@@ -623,7 +623,7 @@ __global__ void __launch_bounds__(kTPB, 2) dmg_setup_chunk(const DmgArgs<R> a)
             const uint16_t* s_ell = reinterpret_cast<const uint16_t*>(stg + L.ell);
             const ChunkMeta cm = s_meta[k];
             const int nloc = cm.n_int + cm.n_halo;
-            const int shift = cm.node_start & (A - 1), hb = (shift + cm.n_int + A - 1) & ~(A - 1), fshift = cm.node_start & 15;
+            const int shift = cm.node_start & (A - 1), fshift = cm.node_start & 15;
             const int* s_hdst = reinterpret_cast<const int*>(stg + L.hdst) + (cm.halo_off & 3);
             const uint8_t* s_flags = stg + L.flags;
 
