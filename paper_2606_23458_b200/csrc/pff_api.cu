@@ -76,6 +76,8 @@ void pff_mesh_destroy(pff_mesh* m)
     for (void* p : ptrs) if (p) cudaFree(p);
     if (m->h_ctrl) cudaFreeHost(m->h_ctrl);
     if (m->h_ring) cudaFreeHost(m->h_ring);
+    if (m->copy_stream) { cudaStreamSynchronize(m->copy_stream); cudaStreamDestroy(m->copy_stream); }
+    if (m->ev_step) cudaEventDestroy(m->ev_step);
     for (auto& v : m->prof_ev) for (cudaEvent_t e : v) cudaEventDestroy(e);
     delete m;
 }

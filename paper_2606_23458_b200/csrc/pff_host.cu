@@ -31,18 +31,21 @@ __global__ void host_in_kernel(const HostIO<R> io)
     if (i < io.Ne) io.HH[i] = R(io.H[io.elem_old_of_new[i]]);
 }
 
+// parts: 1 = what the explicit step produces (u, v, a, H), 2 = what the damage solve produces (d)
 template <typename R>
-__global__ void host_out_kernel(const HostIO<R> io)
+__global__ void host_out_kernel(const HostIO<R> io, int parts)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < io.N) {
         const int o = io.node_old_of_new[i];
-        io.u[2 * o] = double(io.ux[i]); io.u[2 * o + 1] = double(io.uy[i]);
-        io.v[2 * o] = double(io.vx[i]); io.v[2 * o + 1] = double(io.vy[i]);
-        io.a[2 * o] = double(io.ax[i]); io.a[2 * o + 1] = double(io.ay[i]);
-        io.d[o] = double(io.dd[i]);
+        if (parts & 1) {
+            io.u[2 * o] = double(io.ux[i]); io.u[2 * o + 1] = double(io.uy[i]);
+            io.v[2 * o] = double(io.vx[i]); io.v[2 * o + 1] = double(io.vy[i]);
+            io.a[2 * o] = double(io.ax[i]); io.a[2 * o + 1] = double(io.ay[i]);
+        }
+        if (parts & 2) io.d[o] = double(io.dd[i]);
     }
-    if (i < io.Ne) io.H[io.elem_old_of_new[i]] = double(io.HH[i]);
+    if ((parts & 1) && i < io.Ne) io.H[io.elem_old_of_new[i]] = double(io.HH[i]);
 }
 
 template <typename R>
@@ -85,18 +88,38 @@ static pff_status run_host_t(pff_mesh* m, pff_host_state* hs, const double* dir_
     }
     pff_state s{io.ux, io.uy, io.vx, io.vy, io.ax, io.ay, io.dd, io.HH, io.fex, io.fey};
     pff_status worst = PFF_OK;
+    // The results of the LAST explicit step (u, v, a, H) are final before its damage solve: they are permuted and copied
+    // back on a second stream while the solve runs on the mesh stream; d follows when the solve is done.
+    if (!m->copy_stream) {
+        if ((st = cuda_check(cudaStreamCreateWithFlags(&m->copy_stream, cudaStreamNonBlocking), "run_host: stream")) != PFF_OK) return st;
+        if ((st = cuda_check(cudaEventCreateWithFlags(&m->ev_step, cudaEventDisableTiming), "run_host: event")) != PFF_OK) return st;
+    }
+    cudaStream_t cp = m->copy_stream;
+    bool mech_out = false;
+    auto mechanics_out = [&]() -> pff_status {
+        pff_status e;
+        if ((e = cuda_check(cudaEventRecord(m->ev_step, cs), "run_host: record")) != PFF_OK) return e;
+        if ((e = cuda_check(cudaStreamWaitEvent(cp, m->ev_step, 0), "run_host: wait")) != PFF_OK) return e;
+        host_out_kernel<R><<<nb, 256, 0, cp>>>(io, 1);
+#define CPC(dst, src, n) if ((e = cuda_check(cudaMemcpyAsync(dst, src, (n) * sizeof(double), cudaMemcpyDeviceToHost, cp), "run_host: copy")) != PFF_OK) return e
+        CPC(hs->u, io.u, 2 * N); CPC(hs->v, io.v, 2 * N); CPC(hs->a, io.a, 2 * N); CPC(hs->H, io.H, Ne);
+#undef CPC
+        mech_out = true;
+        return PFF_OK;
+    };
     for (int64_t k = 1; k <= n_steps; ++k) {
         if ((st = launch_step(m, &s, &bc, dt, 0, nullptr, nullptr, nullptr)) != PFF_OK) return st;
+        if (k == n_steps && (st = mechanics_out()) != PFF_OK) return st;
         if (damage_every > 0 && k % damage_every == 0) {
             st = damage_solve(m, &s, rel_tol, max_iter, nullptr, nullptr);
             if (st == PFF_ENOCONV) worst = st;
             else if (st != PFF_OK) return st;
         }
     }
-    host_out_kernel<R><<<nb, 256, 0, cs>>>(io);
-    CP(hs->u, io.u, 2 * N, cudaMemcpyDeviceToHost); CP(hs->v, io.v, 2 * N, cudaMemcpyDeviceToHost);
-    CP(hs->a, io.a, 2 * N, cudaMemcpyDeviceToHost); CP(hs->d, io.d, N, cudaMemcpyDeviceToHost);
-    CP(hs->H, io.H, Ne, cudaMemcpyDeviceToHost);
+    if (!mech_out && (st = mechanics_out()) != PFF_OK) return st;  // n_steps == 0
+    host_out_kernel<R><<<nb, 256, 0, cs>>>(io, 2);
+    CP(hs->d, io.d, N, cudaMemcpyDeviceToHost);
+    if ((st = cuda_check(cudaStreamSynchronize(cp), "run_host: copy sync")) != PFF_OK) return st;
 #undef CP
     if ((st = cuda_check(cudaStreamSynchronize(cs), "run_host: sync")) != PFF_OK) return st;
     return worst;

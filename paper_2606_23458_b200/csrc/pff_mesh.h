@@ -67,6 +67,8 @@ struct pff_mesh {
     unsigned int step_bar_count = 0;     // its value after the launches enqueued so far
 
     // host-path staging (pff_run_host)
+    cudaStream_t copy_stream = nullptr;  // second stream: copies the mechanics results back while the damage solve runs
+    cudaEvent_t ev_step = nullptr;
     void* d_stage = nullptr; size_t stage_bytes = 0;
     void* d_hstate = nullptr;  // device state arrays owned by the library for pff_run_host
     int32_t *d_node_old_of_new = nullptr, *d_elem_old_of_new = nullptr;
