@@ -191,6 +191,23 @@ pff_status pff_subcycle_limit(const pff_material *material, int32_t *n_max, doub
 pff_status pff_run_steps(pff_mesh *mesh, pff_state *state, const pff_bc *bc, double dt, int64_t n_steps,
                          int32_t damage_every, double rel_tol, int32_t max_iter, int64_t *cg_iters_total);
 
+/* ---- implicit differentiation of the damage solve (section 4.2) -----------
+ * Backward pass of A(theta) d = b(theta) (Eq. 22): ONE adjoint solve A^T lambda = g with the same matrix-free operator
+ * (Eq. 23; A is symmetric), linearised at the active set realised by the forward solve (L446).
+ * g: upstream gradient dL/dd, device [n_nodes], precision of the mesh, internal order.  free_mask: device uint8
+ * [n_nodes] or NULL; nodes with free_mask == 0 and the damage-Dirichlet nodes are outside the free set F and get
+ * lambda = 0 (NULL: F = every non-Dirichlet node, the AT2 case where the solve is unconstrained and the clamp acts
+ * afterwards; the caller routes g of clamped nodes to d_prev, L446).  lambda: device [n_nodes] out, 16-byte aligned.
+ * Solves A_FF lambda_F = g_F by Jacobi-PCG from lambda = 0 with the operator of state->H (state->d is not read) until
+ * ||g_F - A_FF lambda_F||_2 <= rel_tol ||g_F||_2; same kernels, status codes and synchronisation as pff_damage_solve. */
+pff_status pff_damage_adjoint(pff_mesh *mesh, const pff_state *state, const void *g, const uint8_t *free_mask, void *lambda,
+                              double rel_tol, int32_t max_iter, int32_t *iters_out, double *relres_out);
+/* out = { lambda^T M d, lambda^T K d } with the consistent mass M (L185) and the P1 stiffness K of the mesh (unit
+ * coefficients), accumulated in fp64 in a fixed order: the two scalars from which the (G_c, l0) gradients follow, e.g.
+ * AT2: dL/dG_c = -[(1/l0) out[0] + l0 out[1]] (Eq. 24), dL/dl0 = -[-(G_c/l0^2) out[0] + G_c out[1]].
+ * lambda, d: device [n_nodes], precision of the mesh, internal order.  Synchronises the stream. */
+pff_status pff_damage_param_terms(pff_mesh *mesh, const void *lambda, const void *d, double out[2]);
+
 /* ---- test hooks (device vectors, internal order, precision of the mesh) ---------------------- */
 /* f_int(u, d) of the current state (no predictor), and psi+ per element (psi_plus may be NULL). */
 pff_status pff_internal_force(pff_mesh *mesh, const pff_state *state, void *fx, void *fy, void *psi_plus);

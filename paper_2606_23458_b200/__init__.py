@@ -167,6 +167,22 @@ class Mesh:
         _check(self.L.pff_energies(self.h, C.byref(state.c), out))
         return np.array(list(out))
 
+    def pff_damage_adjoint(self, state: State, g, free_mask=None, rel_tol=1e-8, max_iter=1000, allow_noconv=False):
+        """lambda with A_FF lambda_F = g_F (operator of state.H); g, free_mask (uint8) device tensors in internal order."""
+        import torch
+        lam = torch.empty(self.n_nodes, dtype=self.dtype, device=self.device)
+        it, rr = C.c_int32(0), C.c_double(0.0)
+        st = _check(self.L.pff_damage_adjoint(self.h, C.byref(state.c), g.data_ptr(),
+                                              free_mask.data_ptr() if free_mask is not None else None, lam.data_ptr(),
+                                              rel_tol, max_iter, C.byref(it), C.byref(rr)),
+                    allow=(PFF_ENOCONV,) if allow_noconv else ())
+        return lam, st, it.value, rr.value
+
+    def pff_damage_param_terms(self, lam, d):
+        out = (C.c_double * 2)()
+        _check(self.L.pff_damage_param_terms(self.h, lam.data_ptr(), d.data_ptr(), out))
+        return out[0], out[1]
+
     def pff_internal_force(self, state: State):
         import torch
         fx = torch.empty(self.n_nodes, dtype=self.dtype, device=self.device)

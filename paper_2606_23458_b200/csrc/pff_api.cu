@@ -391,6 +391,23 @@ pff_status pff_run_steps(pff_mesh* m, pff_state* s, const pff_bc* bc, double dt,
     return worst;
 }
 
+pff_status pff_damage_adjoint(pff_mesh* m, const pff_state* s, const void* g, const uint8_t* free_mask, void* lambda, double rel_tol,
+                              int32_t max_iter, int32_t* iters, double* relres)
+{
+    if (!m || !valid_state(s) || !g || !lambda || (reinterpret_cast<uintptr_t>(lambda) & 15)) {
+        set_error("pff_damage_adjoint: null mesh / state / g / lambda, or lambda not 16-byte aligned");
+        return PFF_EINVAL;
+    }
+    if (!(rel_tol > 0) || max_iter < 1) { set_error("pff_damage_adjoint: need rel_tol > 0, max_iter >= 1"); return PFF_EINVAL; }
+    return damage_adjoint(m, s, g, free_mask, lambda, rel_tol, max_iter, iters, relres);
+}
+
+pff_status pff_damage_param_terms(pff_mesh* m, const void* lambda, const void* d, double out[2])
+{
+    if (!m || !lambda || !d || !out) { set_error("pff_damage_param_terms: null argument"); return PFF_EINVAL; }
+    return damage_param_terms(m, lambda, d, out);
+}
+
 pff_status pff_damage_matvec(pff_mesh* m, const pff_state* s, const void* p, void* q)
 {
     if (!m || !valid_state(s) || !p || !q) { set_error("pff_damage_matvec: null argument"); return PFF_EINVAL; }

@@ -55,6 +55,11 @@ struct DmgArgs {
     R *lb, *r, *p, *q, *dinv;
     uint8_t* mask;  // [N]: bit0 = in the free set, bit1 = damage-Dirichlet
     const R* p_in;  // plain mat-vec / hooks
+    // adjoint solve (pff_damage_adjoint): right-hand side g instead of b(H), optional caller-given free set, and no
+    // clamp of the result
+    const R* rhs;
+    const uint8_t* free_in;
+    int no_clamp;
     R *q_out, *b_out, *D_out;
     double* part;    // [kCh][part_n] chunk-kernel block partials
     double* part2;   // [kCh][kMaxSharedBlocks] interface-kernel block partials (chunk partials folded in)
@@ -530,8 +535,10 @@ finalize:
                 if (PROJ && sc.trunc && p < R(0) && (double(l) - double(v)) / double(p) <= sc.alpha * (1.0 + 1e-12)) xn = l;
                 v = xn;
             }
-            if (v < l) v = l;
-            if (v > R(1)) v = R(1);
+            if (!a.no_clamp) {
+                if (v < l) v = l;
+                if (v > R(1)) v = R(1);
+            }
             a.x[i] = v;
         }
         if (blockIdx.x == 0 && tid == 0) *a.ctrl = s_ctrl;
@@ -577,6 +584,7 @@ __global__ void __launch_bounds__(kTPB, 2) dmg_setup_chunk(const DmgArgs<R> a)
     const int tid = threadIdx.x, lane = tid & 31, G = gridDim.x, EC = a.EC;
     const int n_my = (a.C - (int)blockIdx.x + G - 1) / G;
     constexpr int kWorkers = kTPB - 32;  // the last warp is the producer (bulk copies + halo gathers), as in the CG kernel
+    const bool adj = !HOOK && a.rhs != nullptr;
     const bool issuer = tid >= kWorkers;
     const bool have_desc = issuer && lane < a.plan.n;
     StageDesc my_desc{};
@@ -681,13 +689,18 @@ __global__ void __launch_bounds__(kTPB, 2) dmg_setup_chunk(const DmgArgs<R> a)
                         if (a.b_out) a.b_out[gid] = bs;
                         if (a.D_out) a.D_out[gid] = Ds;
                     } else {
-                        const R r = bs - qs;
-                        const bool fixed = (s_flags[fshift + i] & 4) != 0;
+                        bool fixed = (s_flags[fshift + i] & 4) != 0;
+                        R rhs = bs;
+                        if (adj) {  // adjoint: nodes outside the caller's free set are held at lambda = 0 like Dirichlet nodes
+                            fixed = fixed || (a.free_in && !a.free_in[gid]);
+                            rhs = fixed ? R(0) : a.rhs[gid];
+                        }
+                        const R r = rhs - qs;
                         a.r[gid] = r; a.dinv[gid] = R(1) / Ds; a.lb[gid] = s_x[shift + i];
                         a.mask[gid] = fixed ? 2 : 1;
-                        acc[0] += double(bs) * double(bs);
+                        acc[0] += double(rhs) * double(rhs);
                         if (!fixed) acc[1] += double(r) * double(r);
-                        if (!fixed && (a.mat.model != PFF_AT1 || r > R(0))) acc[2] += double(r) * double(r);  // solver's first free set
+                        if (!fixed && (adj || a.mat.model != PFF_AT1 || r > R(0))) acc[2] += double(r) * double(r);  // solver's first free set
                     }
                 } else {
                     const int slot = s_hdst[i - cm.n_int];
@@ -711,13 +724,18 @@ __global__ void __launch_bounds__(kTPB, 2) dmg_setup_chunk(const DmgArgs<R> a)
                 if (a.b_out) a.b_out[gid] = bs;
                 if (a.D_out) a.D_out[gid] = Ds;
             } else {
-                const R r = bs - qs;
-                const bool fixed = (a.flags[gid] & 4) != 0;
+                bool fixed = (a.flags[gid] & 4) != 0;
+                R rhs = bs;
+                if (adj) {
+                    fixed = fixed || (a.free_in && !a.free_in[gid]);
+                    rhs = fixed ? R(0) : a.rhs[gid];
+                }
+                const R r = rhs - qs;
                 a.r[gid] = r; a.dinv[gid] = R(1) / Ds; a.lb[gid] = a.x[gid];
                 a.mask[gid] = fixed ? 2 : 1;
-                acc[0] += double(bs) * double(bs);
+                acc[0] += double(rhs) * double(rhs);
                 if (!fixed) acc[1] += double(r) * double(r);
-                if (!fixed && (a.mat.model != PFF_AT1 || r > R(0))) acc[2] += double(r) * double(r);
+                if (!fixed && (adj || a.mat.model != PFF_AT1 || r > R(0))) acc[2] += double(r) * double(r);
             }
         }
     }
@@ -840,13 +858,22 @@ static pff_status set_smem(K kern, int bytes, int& granted)
     return st;
 }
 
+struct AdjointIn {
+    const void* g;
+    const uint8_t* free_mask;
+    void* lambda;
+};
+
 template <typename R, bool PROJ>
-static pff_status damage_solve_t(pff_mesh* m, pff_state* s, double rel_tol, int max_iter, int* iters, double* relres)
+static pff_status damage_solve_t(pff_mesh* m, const pff_state* s, double rel_tol, int max_iter, int* iters, double* relres,
+                                 const AdjointIn* adj = nullptr)
 {
     pff_status st = ensure_workspace(m);
     if (st != PFF_OK) return st;
     const HostMesh& hm = m->hm;
-    DmgArgs<R> a = make_args<R>(m, s), asu = a;
+    DmgArgs<R> a = make_args<R>(m, s);
+    if (adj) { a.x = (R*)adj->lambda; a.rhs = (const R*)adj->g; a.free_in = adj->free_mask; a.no_clamp = 1; }
+    DmgArgs<R> asu = a;
     set_plan<R>(m, a, 0, PROJ);
     set_plan<R>(m, asu, 2, PROJ);
     const int smem_mv = (int)m->lay_mv.total, smem_su = (int)m->lay_su.total;
@@ -915,6 +942,18 @@ pff_status damage_solve(pff_mesh* m, pff_state* s, double rel_tol, int max_iter,
                     : damage_solve_t<float, false>(m, s, rel_tol, max_iter, iters, relres);
     return proj ? damage_solve_t<double, true>(m, s, rel_tol, max_iter, iters, relres)
                 : damage_solve_t<double, false>(m, s, rel_tol, max_iter, iters, relres);
+}
+
+// Adjoint of the converged damage system (section 4.2, Eq. 23): A_FF lambda_F = g_F with the operator of state->H,
+// by the same setup + cooperative CG kernels as the forward solve (unprojected, from lambda = 0, no clamp).
+pff_status damage_adjoint(pff_mesh* m, const pff_state* s, const void* g, const uint8_t* free_mask, void* lambda, double rel_tol,
+                          int max_iter, int* iters, double* relres)
+{
+    pff_status st = cuda_check(cudaMemsetAsync(lambda, 0, (size_t)m->hm.N * m->rb, m->stream), "adjoint: zero lambda");
+    if (st != PFF_OK) return st;
+    const AdjointIn in{g, free_mask, lambda};
+    if (m->opt.precision == PFF_F32) return damage_solve_t<float, false>(m, s, rel_tol, max_iter, iters, relres, &in);
+    return damage_solve_t<double, false>(m, s, rel_tol, max_iter, iters, relres, &in);
 }
 
 template <typename R>

@@ -106,6 +106,58 @@ static pff_status energies_r(pff_mesh* m, const pff_state* s, double out[4])
     return PFF_OK;
 }
 
+// lambda^T M d and lambda^T K d with the consistent mass M^e = A (1 + delta_ij) / 12 (L185) and the P1 stiffness
+// K^e = A grad phi_i . grad phi_j: the two scalars of the (G_c, l0) gradient of Eq. 24.
+template <typename R>
+__global__ void __launch_bounds__(kTPB) param_terms_kernel(int Ne, const int4* conn, const void* ga, const void* gb,
+                                                           const R* area, const R* lam, const R* d, double* part /* [2][nblocks] */)
+{
+    __shared__ double s_red[32];
+    const int e = blockIdx.x * kTPB + threadIdx.x;
+    double tM = 0.0, tK = 0.0;
+    if (e < Ne) {
+        const int4 c = __ldg(conn + e);
+        R b1, c1, b2, c2;
+        Geo<R>::load(ga, gb, e, b1, c1, b2, c2);
+        const double A = double(area[e]);
+        const double l1 = lam[c.x], l2 = lam[c.y], l3 = lam[c.z], d1 = d[c.x], d2 = d[c.y], d3 = d[c.z];
+        const double ds = d1 + d2 + d3;
+        tM = A / 12.0 * (l1 * (d1 + ds) + l2 * (d2 + ds) + l3 * (d3 + ds));
+        const double glx = double(b1) * (l1 - l3) + double(b2) * (l2 - l3), gly = double(c1) * (l1 - l3) + double(c2) * (l2 - l3);
+        const double gdx = double(b1) * (d1 - d3) + double(b2) * (d2 - d3), gdy = double(c1) * (d1 - d3) + double(c2) * (d2 - d3);
+        tK = A * (glx * gdx + gly * gdy);
+    }
+    const double t0 = block_sum(tM, s_red);
+    const double t1 = block_sum(tK, s_red);
+    if (threadIdx.x == 0) { part[blockIdx.x] = t0; part[gridDim.x + blockIdx.x] = t1; }
+}
+
+template <typename R>
+static pff_status param_terms_r(pff_mesh* m, const void* lambda, const void* d, double out[2])
+{
+    const int nbe = (int)((m->hm.Ne + kTPB - 1) / kTPB);
+    double* part = nullptr;
+    pff_status st = cuda_check(cudaMallocAsync((void**)&part, sizeof(double) * (2 * nbe + 4), m->stream), "param terms: alloc");
+    if (st != PFF_OK) return st;
+    param_terms_kernel<R><<<nbe, kTPB, 0, m->stream>>>((int)m->hm.Ne, (const int4*)m->d_conn, m->d_ga, m->d_gb, (const R*)m->d_area,
+                                                       (const R*)lambda, (const R*)d, part);
+    double* dout = part + 2 * nbe;
+    energy_final_kernel<<<1, kTPB, 0, m->stream>>>(part, nbe, part + nbe, nbe, part, 0, dout);
+    m->n_launches += 2;
+    double h[2];
+    st = cuda_check(cudaMemcpyAsync(h, dout, sizeof(h), cudaMemcpyDeviceToHost, m->stream), "param terms: copy");
+    cudaFreeAsync(part, m->stream);
+    if (st == PFF_OK) st = cuda_check(cudaStreamSynchronize(m->stream), "param terms: sync");
+    if (st != PFF_OK) return st;
+    out[0] = h[0]; out[1] = h[1];
+    return PFF_OK;
+}
+
+pff_status damage_param_terms(pff_mesh* m, const void* lambda, const void* d, double out[2])
+{
+    return m->opt.precision == PFF_F32 ? param_terms_r<float>(m, lambda, d, out) : param_terms_r<double>(m, lambda, d, out);
+}
+
 pff_status energies(pff_mesh* m, const pff_state* s, double out[4])
 {
     return m->opt.precision == PFF_F32 ? energies_r<float>(m, s, out) : energies_r<double>(m, s, out);

@@ -94,6 +94,9 @@ inline void prof_mark(pff_mesh* m, int cls)
 pff_status launch_step(pff_mesh* m, pff_state* s, const pff_bc* bc, double dt, int mode, void* fx, void* fy, void* psi);
 pff_status damage_solve(pff_mesh* m, pff_state* s, double rel_tol, int max_iter, int* iters, double* relres);
 pff_status damage_matvec(pff_mesh* m, const pff_state* s, const void* p, void* q);
+pff_status damage_adjoint(pff_mesh* m, const pff_state* s, const void* g, const uint8_t* free_mask, void* lambda, double rel_tol,
+                          int max_iter, int* iters, double* relres);
+pff_status damage_param_terms(pff_mesh* m, const void* lambda, const void* d, double out[2]);
 pff_status damage_rhs_diag(pff_mesh* m, const pff_state* s, void* b, void* D);
 pff_status energies(pff_mesh* m, const pff_state* s, double out[4]);
 pff_status cuda_check(cudaError_t e, const char* what);

@@ -1,0 +1,111 @@
+"""GPU parity of pff_damage_adjoint / pff_damage_param_terms (through the C ABI) against oracle/pff_adjoint_oracle.py
+(assembled operator + direct solve): PAPER.md section 4.2, Eq. 22-24; SURVEY.md 8(f) NEXT-2."""
+import numpy as np
+import pytest
+
+from oracle import pff_adjoint_oracle as adj
+from pff_inputs import GLASS, config, random_mesh
+
+pytestmark = pytest.mark.gpu
+
+
+def _gpu_mesh(xy, tri, material, H, fixed=(), precision=0, chunk_elems=0):
+    import paper_2606_23458_b200 as pff
+    mesh = pff.Mesh(xy, tri, material, precision=precision, chunk_elems=chunk_elems)
+    st = mesh.new_state(H=H)
+    if len(fixed):
+        mesh.pff_set_damage_dirichlet(np.asarray(fixed, dtype=np.int32))
+    return mesh, st
+
+
+def _mask_tensor(mesh, free_user):
+    import torch
+    m = np.empty(len(free_user), dtype=np.uint8)
+    m[mesh.node_new_of_old] = free_user.astype(np.uint8)
+    return torch.from_numpy(m).to(mesh.device)
+
+
+@pytest.mark.parametrize("model", [1, 2])
+@pytest.mark.parametrize("masked", [False, True])
+def test_adjoint_solve_matches_direct_solve(model, masked):
+    """Several chunks, jittered mesh with mixed orientations, Dirichlet nodes and (masked) a caller-given free set."""
+    xy, tri = random_mesh(33, 11)
+    r = np.random.default_rng(12)
+    Gc, l0 = 3.0, 0.05
+    H = r.uniform(0.2, 3.0, len(tri)) * Gc / l0
+    material = dict(GLASS, Gc=Gc, l0=l0, model=model, split=1, plane=0)
+    fixed = np.array([0, 5, 100, 517, 1088], dtype=np.int32)
+    free = np.ones(len(xy), dtype=bool)
+    if masked:
+        free = r.uniform(size=len(xy)) < 0.8
+    g = r.standard_normal(len(xy))
+    A, _ = adj.damage_system(xy, tri, H, Gc, l0, model)
+    free_o = free.copy()
+    free_o[fixed] = False
+    lam_o = adj.adjoint_solve(A, g, free_o)
+
+    mesh, st = _gpu_mesh(xy, tri, material, H, fixed, chunk_elems=256)
+    lam_t, status, iters, relres = mesh.pff_damage_adjoint(st, mesh.nodes_to_internal(g),
+                                                          _mask_tensor(mesh, free) if masked else None,
+                                                          rel_tol=1e-13, max_iter=5000)
+    assert status == 0 and iters > 0 and relres <= 1e-13
+    lam = mesh.nodes_to_user(lam_t)
+    assert np.all(lam[~free_o] == 0.0)
+    assert np.abs(lam - lam_o).max() <= 1e-10 * np.abs(lam_o).max()
+
+    # the two scalars of Eq. 24 against the assembled M and K
+    d = r.uniform(0.0, 1.0, len(xy))
+    M, K = adj.mass_stiffness(xy, tri)
+    tM, tK = mesh.pff_damage_param_terms(lam_t, mesh.nodes_to_internal(d))
+    oM, oK = adj.param_terms(M, K, lam, d)
+    assert abs(tM - oM) <= 1e-11 * abs(oM) and abs(tK - oK) <= 1e-11 * abs(oK)
+
+
+def test_gc_gradient_end_to_end_against_forward_finite_differences():
+    """dL/dG_c from the GPU adjoint (Eq. 24) against central differences of GPU FORWARD solves at perturbed G_c."""
+    xy, tri = random_mesh(25, 21)
+    r = np.random.default_rng(22)
+    Gc, l0 = 3.0, 0.06
+    H = r.uniform(0.2, 3.0, len(tri)) * Gc / l0
+    g = r.standard_normal(len(xy))
+
+    def forward(gc):
+        mesh, st = _gpu_mesh(xy, tri, dict(GLASS, Gc=gc, l0=l0, model=2, split=1, plane=0), H)
+        status, _, _ = mesh.pff_damage_solve(st, rel_tol=1e-13, max_iter=5000)
+        assert status == 0
+        return mesh, st
+
+    mesh, st = forward(Gc)
+    d = mesh.nodes_to_user(st.d)
+    assert d.min() > 0.0 and d.max() < 1.0  # clamp inactive: the forward result solves Eq. 22
+    lam_t, status, _, _ = mesh.pff_damage_adjoint(st, mesh.nodes_to_internal(g), None, rel_tol=1e-13, max_iter=5000)
+    assert status == 0
+    tM, tK = mesh.pff_damage_param_terms(lam_t, st.d)
+    dGc = -(tM / l0 + l0 * tK)
+    eps = 1e-5
+    vals = []
+    for s in (+1, -1):
+        m2, s2 = forward(Gc * (1 + s * eps))
+        vals.append(g @ m2.nodes_to_user(s2.d))
+    fd = (vals[0] - vals[1]) / (2 * eps * Gc)
+    assert abs(fd - dGc) <= 1e-6 * abs(dGc)
+
+
+def test_adjoint_fp32_and_config_mesh():
+    """Config 1 plate (notch = damage-Dirichlet), both precisions: fp64 to 1e-9, fp32 to the north_star fp32 tolerance."""
+    cfg = config(1)
+    xy, tri, material = cfg["xy"], cfg["tri"], cfg["material"]
+    r = np.random.default_rng(31)
+    H = r.uniform(0.0, 2.0, len(tri)) * material["Gc"] / material["l0"]
+    g = r.standard_normal(len(xy))
+    A, _ = adj.damage_system(xy, tri, H, material["Gc"], material["l0"], material["model"])
+    free = np.ones(len(xy), dtype=bool)
+    free[cfg["notch"]] = False
+    lam_o = adj.adjoint_solve(A, g, free)
+    for precision, tol, cg_tol in ((0, 1e-9, 1e-12), (1, 2e-5, 1e-6)):
+        mesh, st = _gpu_mesh(xy, tri, material, H, cfg["notch"], precision=precision)
+        lam_t, status, _, relres = mesh.pff_damage_adjoint(st, mesh.nodes_to_internal(g), None, rel_tol=cg_tol, max_iter=5000,
+                                                           allow_noconv=(precision == 1))
+        assert relres <= 10 * cg_tol
+        lam = mesh.nodes_to_user(lam_t)
+        assert np.abs(lam - lam_o).max() <= tol * np.abs(lam_o).max()
