@@ -166,6 +166,13 @@ def run_ours(args, rank: int, world: int):
     # explicit step and CG iteration timed alone (device-resident), for the secondary metrics
     ms_exp, _ = timed(lambda: mesh.pff_explicit_step(st, bc, dt), args.steps)
 
+    # backward pass of the damage solve (pff_damage_adjoint, section 4.2), timed alone: seeded upstream gradient,
+    # the same setup + cooperative CG kernels as the forward solve
+    g_up = torch.from_numpy(np.random.default_rng(7).standard_normal(N).astype(mesh.np_dtype)).to(mesh.device)
+    adj_call = lambda: mesh.pff_damage_adjoint(st, g_up, None, rel_tol=REL_TOL, max_iter=MAX_ITER, allow_noconv=True)[2]
+    adj_call()
+    ms_adj, it_adj = timed(adj_call, 5)
+
     # --- end to end: host buffers in USER numbering through pff_run_host, H2D + D2H inside the timed region
     hs = dict(u=np.ascontiguousarray(cfg["u0"], dtype=np.float64), v=np.zeros((N, 2)), a=np.zeros((N, 2)),
               d=np.ascontiguousarray(cfg["d0"], dtype=np.float64), H=np.zeros(Ne),
@@ -187,7 +194,7 @@ def run_ours(args, rank: int, world: int):
     barrier()
     e2e_val = whole_job_value(Ne, ke, world, reduce_max(time.perf_counter() - t0, world, f"cuda:{dev}"))
     return dict(mesh=mesh, cfg=cfg, N=N, Ne=Ne, w=w, ms_total=ms_total, iters=iters, launches=launches, clk=clk, prof=prof,
-                iters_p=iters_p, ms_exp=ms_exp, e2e_val=e2e_val, h2d=(9 * N + Ne) * 8, d2h=(7 * N + Ne) * 8, snapshot=snapshot)
+                iters_p=iters_p, ms_exp=ms_exp, ms_adj=ms_adj / 5, it_adj=it_adj[0], e2e_val=e2e_val, h2d=(9 * N + Ne) * 8, d2h=(7 * N + Ne) * 8, snapshot=snapshot)
 
 
 def ncu_traffic(workload: str, dtype: str, kernel: str, k: dict):
@@ -294,6 +301,10 @@ def main():
                 explicit_step_hbm_frac=ab["step"] / (r["ms_exp"] / K / 1e3) / 1e9 / peak,
                 cg_iterations_per_s=world * iters_prof / (prof["matvec_chunk"][0] / 1e3) if prof["matvec_chunk"][0] else None,
                 cg_iteration_hbm_frac=kern["cg_solve"]["frac"] if "cg_solve" in kern else None,
+                adjoint=dict(ms_per_solve=r["ms_adj"], cg_iterations=r["it_adj"],
+                             hbm_frac=(ab["cg_iter"] * r["it_adj"] + ab["matvec"]) / (r["ms_adj"] / 1e3) / 1e9 / peak,
+                             note="one pff_damage_adjoint (setup pass + all CG iterations), seeded upstream gradient; "
+                                  "algorithmic bytes = iterations x CG iteration + one operator pass for the setup"),
                 clocks=r["clk"], gpu_launches=int(r["launches"]),
                 e2e=dict(value=r["e2e_val"], unit=UNIT, h2d_bytes_per_step=r["h2d"], d2h_bytes_per_step=r["d2h"]),
                 roofline=dict(bound="hbm", kernel=dom, achieved=kern[dom]["achieved_gbs"], peak=peak, unit="GB/s",
