@@ -208,6 +208,16 @@ pff_status pff_damage_adjoint(pff_mesh *mesh, const pff_state *state, const void
  * lambda, d: device [n_nodes], precision of the mesh, internal order.  Synchronises the stream. */
 pff_status pff_damage_param_terms(pff_mesh *mesh, const void *lambda, const void *d, double out[2]);
 
+/* ---- matrix-free stiffness action (Eq. 11-15) ---------------------------
+ * q = K(u) p = f_int(u + p) - f_int(u) (Eq. 13) at the reference state u = state->u with the damage state->d held fixed:
+ * the operator a Krylov solver of the quasi-static mechanics problem needs, never assembled.  Both forces are evaluated
+ * in ONE fused element pass of the explicit-step kernel (same staging, same ordered gather: bit-reproducible).  Exact
+ * tangent action for the isotropic split; for the other splits it is the paper's shifted difference, exact as long as p
+ * does not change the sign pattern of the split (L140).  No boundary masking: the caller zeroes constrained dofs.
+ * px, py (in) and qx, qy (out): device [n_nodes], precision of the mesh, internal order, px / py 16-byte aligned.
+ * Gather scatter only (PFF_EUNSUPPORTED with PFF_SCATTER_ATOMIC).  Asynchronous. */
+pff_status pff_stiffness_action(pff_mesh *mesh, const pff_state *state, const void *px, const void *py, void *qx, void *qy);
+
 /* ---- test hooks (device vectors, internal order, precision of the mesh) ---------------------- */
 /* f_int(u, d) of the current state (no predictor), and psi+ per element (psi_plus may be NULL). */
 pff_status pff_internal_force(pff_mesh *mesh, const pff_state *state, void *fx, void *fy, void *psi_plus);

@@ -146,6 +146,11 @@ class OracleMesh:
         self.L.orc_internal_force(self.N, self.Ne, self.tri, self.gradphi, self.area, C.byref(self._m), u, d, f, pp)
         return f, pp
 
+    def stiffness_action(self, p, u=None, d=None):
+        """K(u) p = f_int(u + p) - f_int(u) with d held fixed: PAPER.md Eq. 13 written out with the internal force."""
+        u = self.u if u is None else np.ascontiguousarray(u, dtype=np.float64)
+        return self.internal_force(u + np.asarray(p, dtype=np.float64), d)[0] - self.internal_force(u, d)[0]
+
     def init_accel(self, S=1.0):
         self.L.orc_init_accel(self.N, self.Ne, self.tri, self.gradphi, self.area, self.mass, C.byref(self._m),
                               self.u, self.d, self.fext, S, len(self.dir_dof), self.dir_dof, self.a)

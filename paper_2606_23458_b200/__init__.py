@@ -183,6 +183,13 @@ class Mesh:
         _check(self.L.pff_damage_param_terms(self.h, lam.data_ptr(), d.data_ptr(), out))
         return out[0], out[1]
 
+    def pff_stiffness_action(self, state: State, px, py):
+        """q = f_int(u + p) - f_int(u) (Eq. 13) at the state's u, d; device tensors in internal order."""
+        import torch
+        qx, qy = torch.empty_like(px), torch.empty_like(py)
+        _check(self.L.pff_stiffness_action(self.h, C.byref(state.c), px.data_ptr(), py.data_ptr(), qx.data_ptr(), qy.data_ptr()))
+        return qx, qy
+
     def pff_internal_force(self, state: State):
         import torch
         fx = torch.empty(self.n_nodes, dtype=self.dtype, device=self.device)

@@ -391,6 +391,15 @@ pff_status pff_run_steps(pff_mesh* m, pff_state* s, const pff_bc* bc, double dt,
     return worst;
 }
 
+pff_status pff_stiffness_action(pff_mesh* m, const pff_state* s, const void* px, const void* py, void* qx, void* qy)
+{
+    if (!m || !valid_state(s) || !px || !py || !qx || !qy) { set_error("pff_stiffness_action: null argument"); return PFF_EINVAL; }
+    if ((reinterpret_cast<uintptr_t>(px) | reinterpret_cast<uintptr_t>(py)) & 15) {
+        set_error("pff_stiffness_action: px, py must be 16-byte aligned"); return PFF_EINVAL;
+    }
+    return launch_step(m, const_cast<pff_state*>(s), nullptr, 0.0, /*MODE_TANGENT*/ 3, qx, qy, nullptr, px, py);
+}
+
 pff_status pff_damage_adjoint(pff_mesh* m, const pff_state* s, const void* g, const uint8_t* free_mask, void* lambda, double rel_tol,
                               int32_t max_iter, int32_t* iters, double* relres)
 {

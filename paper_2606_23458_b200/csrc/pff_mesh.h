@@ -91,7 +91,8 @@ inline void prof_mark(pff_mesh* m, int cls)
         ++(m)->n_launches;                 \
     } while (0)
 // implemented in pff_step.cu / pff_damage.cu / pff_energy.cu
-pff_status launch_step(pff_mesh* m, pff_state* s, const pff_bc* bc, double dt, int mode, void* fx, void* fy, void* psi);
+pff_status launch_step(pff_mesh* m, pff_state* s, const pff_bc* bc, double dt, int mode, void* fx, void* fy, void* psi,
+                       const void* px = nullptr, const void* py = nullptr);
 pff_status damage_solve(pff_mesh* m, pff_state* s, double rel_tol, int max_iter, int* iters, double* relres);
 pff_status damage_matvec(pff_mesh* m, const pff_state* s, const void* p, void* q);
 pff_status damage_adjoint(pff_mesh* m, const pff_state* s, const void* g, const uint8_t* free_mask, void* lambda, double rel_tol,

@@ -21,7 +21,8 @@
 
 namespace pff {
 
-enum { MODE_STEP = 0, MODE_INIT = 1, MODE_FORCE = 2 };
+// MODE_TANGENT: matrix-free stiffness action q = f_int(u + p) - f_int(u) (Eq. 13), both forces in ONE element pass
+enum { MODE_STEP = 0, MODE_INIT = 1, MODE_FORCE = 2, MODE_TANGENT = 3 };
 
 template <typename R>
 struct StepArgs {
@@ -48,6 +49,7 @@ struct StepArgs {
     R* H;
     const R *fex, *fey;
     R *fx_out, *fy_out, *psi_out;
+    const R *px, *py;  // MODE_TANGENT: trial direction
     R *fwx, *fwy;
     R dt, hdt, hdt2, S;
     MatC<R> mat;
@@ -70,7 +72,7 @@ __device__ __forceinline__ void predict(const StepArgs<R>& a, int gid, R& upx, R
 template <typename R, int MODE>
 __device__ __forceinline__ void finish_node(const StepArgs<R>& a, int gid, R upx, R upy, R fx, R fy)
 {
-    if (MODE == MODE_FORCE) { a.fx_out[gid] = fx; a.fy_out[gid] = fy; return; }
+    if (MODE == MODE_FORCE || MODE == MODE_TANGENT) { a.fx_out[gid] = fx; a.fy_out[gid] = fy; return; }
     const uint8_t fl = a.flags[gid];
     const R minv = a.minv[gid];
     R axn = (a.S * a.fex[gid] - fx) * minv;
@@ -123,6 +125,10 @@ __device__ __forceinline__ void step_halo_gather(const StepArgs<R>& a, const Sta
         cp_async<B>(reinterpret_cast<R*>(stg + L.node[5]) + slot, a.ax + gid);
         cp_async<B>(reinterpret_cast<R*>(stg + L.node[6]) + slot, a.ay + gid);
         cp_async<4>(reinterpret_cast<int*>(stg + L.hflag) + j, a.flags + (gid & ~3));
+    }
+    if (MODE == MODE_TANGENT) {  // the trial direction travels in the velocity slots
+        cp_async<B>(reinterpret_cast<R*>(stg + L.node[3]) + slot, a.px + gid);
+        cp_async<B>(reinterpret_cast<R*>(stg + L.node[4]) + slot, a.py + gid);
     }
 }
 
@@ -255,6 +261,14 @@ __global__ void __launch_bounds__(kTPB, 2) step_chunk_kernel(const StepArgs<R> a
                 R psi_p, f[6];
                 element_forces<R, SPLIT>(a.mat, b1, c1, b2, c2, s_area[e], s_ux[c.x], s_uy[c.x], s_ux[c.y], s_uy[c.y], s_ux[c.z],
                                          s_uy[c.z], s_d[c.x] + s_d[c.y] + s_d[c.z], psi_p, f);
+                if (MODE == MODE_TANGENT) {  // Eq. 13: f_int(u + p) - f_int(u), element by element (s_vx, s_vy hold p)
+                    R f1[6], pp1;
+                    element_forces<R, SPLIT>(a.mat, b1, c1, b2, c2, s_area[e], s_ux[c.x] + s_vx[c.x], s_uy[c.x] + s_vy[c.x],
+                                             s_ux[c.y] + s_vx[c.y], s_uy[c.y] + s_vy[c.y], s_ux[c.z] + s_vx[c.z],
+                                             s_uy[c.z] + s_vy[c.z], s_d[c.x] + s_d[c.y] + s_d[c.z], pp1, f1);
+#pragma unroll
+                    for (int k = 0; k < 6; ++k) f[k] = f1[k] - f[k];
+                }
                 *Geo<R>::slot(s_geo, s_shared_slots, e, EC) = Geo<R>::pair(f[0], f[1]);
                 *Geo<R>::slot(s_geo, s_shared_slots, EC + e, EC) = Geo<R>::pair(f[2], f[3]);
                 *Geo<R>::slot(s_geo, s_shared_slots, 2 * EC + e, EC) = Geo<R>::pair(f[4], f[5]);
@@ -277,7 +291,7 @@ __global__ void __launch_bounds__(kTPB, 2) step_chunk_kernel(const StepArgs<R> a
                 }
                 if (i < cm.n_int) {
                     const int gid = cm.node_start + i, s = shift + i;
-                    if (MODE == MODE_FORCE) { a.fx_out[gid] = fx; a.fy_out[gid] = fy; continue; }
+                    if (MODE == MODE_FORCE || MODE == MODE_TANGENT) { a.fx_out[gid] = fx; a.fy_out[gid] = fy; continue; }
                     const uint8_t fl = s_flags[fshift + i];
                     const R minv = s_minv[s];
                     R axn = (a.S * s_fex[s] - fx) * minv;
@@ -451,7 +465,7 @@ static pff_status launch_step_s(pff_mesh* m, const StepArgs<R>& a)
 
 template <typename R>
 static pff_status launch_step_r(pff_mesh* m, pff_state* s, const pff_bc* bc, double dt, int mode, void* fx, void* fy,
-                                void* psi)
+                                void* psi, const void* px, const void* py)
 {
     const HostMesh& hm = m->hm;
     StepArgs<R> a{};
@@ -465,6 +479,7 @@ static pff_status launch_step_r(pff_mesh* m, pff_state* s, const pff_bc* bc, dou
     a.ux = (R*)s->ux; a.uy = (R*)s->uy; a.vx = (R*)s->vx; a.vy = (R*)s->vy; a.ax = (R*)s->ax; a.ay = (R*)s->ay;
     a.d = (const R*)s->d; a.H = (R*)s->H; a.fex = (const R*)s->fext_x; a.fey = (const R*)s->fext_y;
     a.fx_out = (R*)fx; a.fy_out = (R*)fy; a.psi_out = (R*)psi;
+    a.px = (const R*)px; a.py = (const R*)py;
     a.fwx = (R*)m->d_fwx; a.fwy = (R*)m->d_fwy;
     a.dt = R(dt); a.hdt = R(0.5 * dt); a.hdt2 = R(0.5 * dt * dt);
     a.S = R(bc ? bc->load_scale : 1.0);
@@ -489,7 +504,8 @@ static pff_status launch_step_r(pff_mesh* m, pff_state* s, const pff_bc* bc, dou
             add(s->vx, L.node[3], lr, 1); add(s->vy, L.node[4], lr, 1);
             add(s->ax, L.node[5], lr, 1); add(s->ay, L.node[6], lr, 1);
         }
-        if (mode != MODE_FORCE) {
+        if (mode == MODE_TANGENT) { add(a.px, L.node[3], lr, 1); add(a.py, L.node[4], lr, 1); }
+        if (mode != MODE_FORCE && mode != MODE_TANGENT) {
             add(s->fext_x, L.node[7], lr, 1); add(s->fext_y, L.node[8], lr, 1); add(m->d_minv, L.node[9], lr, 1);
             add(m->d_flags, L.flags, 0, 1);
         }
@@ -502,14 +518,18 @@ static pff_status launch_step_r(pff_mesh* m, pff_state* s, const pff_bc* bc, dou
         case MODE_STEP: return launch_step_s<R, MODE_STEP>(m, a);
         case MODE_INIT: return launch_step_s<R, MODE_INIT>(m, a);
         case MODE_FORCE: return launch_step_s<R, MODE_FORCE>(m, a);
+        case MODE_TANGENT:
+            if (m->opt.scatter == PFF_SCATTER_ATOMIC) { set_error("stiffness action: gather scatter only"); return PFF_EUNSUPPORTED; }
+            return launch_step_s<R, MODE_TANGENT>(m, a);
     }
     return PFF_EINVAL;
 }
 
-pff_status launch_step(pff_mesh* m, pff_state* s, const pff_bc* bc, double dt, int mode, void* fx, void* fy, void* psi)
+pff_status launch_step(pff_mesh* m, pff_state* s, const pff_bc* bc, double dt, int mode, void* fx, void* fy, void* psi,
+                       const void* px, const void* py)
 {
-    if (m->opt.precision == PFF_F32) return launch_step_r<float>(m, s, bc, dt, mode, fx, fy, psi);
-    return launch_step_r<double>(m, s, bc, dt, mode, fx, fy, psi);
+    if (m->opt.precision == PFF_F32) return launch_step_r<float>(m, s, bc, dt, mode, fx, fy, psi, px, py);
+    return launch_step_r<double>(m, s, bc, dt, mode, fx, fy, psi, px, py);
 }
 
 }  // namespace pff

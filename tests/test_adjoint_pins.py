@@ -103,3 +103,40 @@ def test_adjoint_identity_and_masking():
     assert np.all(lam[~free] == 0.0)
     res = (A @ lam - g)[free]
     assert np.abs(res).max() <= 1e-11 * np.abs(g).max()
+
+
+# ---------------------------------------------------------------- matrix-free stiffness action, Eq. 11-15 (L126-159)
+@pytest.mark.parametrize("plane", [0, 1])
+def test_stiffness_action_equals_assembled_operator_for_the_isotropic_split(plane):
+    """Eq. 13 (difference of the C oracle's internal forces) against Eq. 14 (K assembled from B^T C B in Python)."""
+    from oracle import pff_stiffness_oracle as sto
+    xy, tri = random_mesh(9, 8)
+    m = mat(split=0, plane=plane)
+    orc = OracleMesh(xy, tri, m)
+    r = np.random.default_rng(9)
+    orc.u[:] = 1e-4 * r.standard_normal((len(xy), 2))
+    orc.d[:] = r.uniform(0.0, 0.9, len(xy))
+    p = 1e-4 * r.standard_normal((len(xy), 2))
+    K = sto.assemble_stiffness(xy, tri, m.E, m.nu, plane, orc.d, m.eta)
+    q = orc.stiffness_action(p)
+    q_ref = (K @ p.ravel()).reshape(-1, 2)
+    assert np.abs(q - q_ref).max() <= 1e-10 * np.abs(q_ref).max()  # cancellation in f(u + p) - f(u): ~|u|/|p| ulp
+    f, _ = orc.internal_force()
+    assert np.abs(f - (K @ orc.u.ravel()).reshape(-1, 2)).max() <= 1e-12 * np.abs(f).max()  # Eq. 10: f_int = K u
+    assert abs(K - K.T).max() <= 1e-12 * abs(K).max()
+    rigid = np.tile([1.0, 0.0], len(xy))
+    assert np.abs(K @ rigid).max() <= 1e-9 * abs(K).max()
+
+
+def test_stiffness_action_is_the_tangent_when_the_sign_pattern_is_fixed():
+    """Spectral split: the shifted difference equals the directional derivative (Eq. 12) for a small p (L140)."""
+    xy, tri = random_mesh(7, 10)
+    orc = OracleMesh(xy, tri, mat(split=1))
+    r = np.random.default_rng(11)
+    orc.u[:] = 1e-4 * r.standard_normal((len(xy), 2))
+    orc.d[:] = r.uniform(0.0, 0.5, len(xy))
+    p = 1e-9 * r.standard_normal((len(xy), 2))
+    q = orc.stiffness_action(p)
+    eps = 0.5
+    fd = (orc.internal_force(orc.u + eps * p)[0] - orc.internal_force(orc.u - eps * p)[0]) / (2 * eps)
+    assert np.abs(q - fd).max() <= 1e-4 * np.abs(fd).max()

@@ -109,3 +109,50 @@ def test_adjoint_fp32_and_config_mesh():
         assert relres <= 10 * cg_tol
         lam = mesh.nodes_to_user(lam_t)
         assert np.abs(lam - lam_o).max() <= tol * np.abs(lam_o).max()
+
+
+# ---------------------------------------------------------------- matrix-free stiffness action (Eq. 11-15, NEXT-3)
+@pytest.mark.parametrize("split", [0, 1, 2, 3])
+@pytest.mark.parametrize("plane", [0, 1])
+def test_stiffness_action_matches_oracle(split, plane):
+    """q = f_int(u + p) - f_int(u) in one fused pass against the C oracle's difference of two internal forces (Eq. 13),
+    several chunks with halos, every split; for the isotropic split also against the assembled K (Eq. 14)."""
+    from oracle import Material, OracleMesh
+    xy, tri = random_mesh(33, 41)
+    material = dict(GLASS, model=2, split=split, plane=plane, gamma_star=1.0 if split == 3 else 0.0)
+    r = np.random.default_rng(42)
+    u = 1e-4 * r.standard_normal((len(xy), 2))
+    d = r.uniform(0.0, 0.9, len(xy))
+    p = 1e-4 * r.standard_normal((len(xy), 2))
+    orc = OracleMesh(xy, tri, Material(**material))
+    orc.u[:] = u
+    orc.d[:] = d
+    q_o = orc.stiffness_action(p)
+
+    import paper_2606_23458_b200 as pff
+    mesh = pff.Mesh(xy, tri, material, chunk_elems=256)
+    st = mesh.new_state(u=u, d=d)
+    qx, qy = mesh.pff_stiffness_action(st, mesh.nodes_to_internal(p[:, 0]), mesh.nodes_to_internal(p[:, 1]))
+    q = np.stack([mesh.nodes_to_user(qx), mesh.nodes_to_user(qy)], 1)
+    assert np.abs(q - q_o).max() <= 1e-10 * np.abs(q_o).max()
+    qx2, qy2 = mesh.pff_stiffness_action(st, mesh.nodes_to_internal(p[:, 0]), mesh.nodes_to_internal(p[:, 1]))
+    assert np.array_equal(qx.cpu().numpy(), qx2.cpu().numpy()) and np.array_equal(qy.cpu().numpy(), qy2.cpu().numpy())
+    if split == 0:
+        from oracle import pff_stiffness_oracle as sto
+        K = sto.assemble_stiffness(xy, tri, material["E"], material["nu"], plane, d, material["eta"])
+        q_K = (K @ p.ravel()).reshape(-1, 2)
+        assert np.abs(q - q_K).max() <= 1e-10 * np.abs(q_K).max()
+
+
+def test_stiffness_action_full_size():
+    """cfg5_1001 (the bench mesh and launch configuration): the action at every node against the oracle."""
+    cfg = config(5, n=1001)
+    from _harness import gpu_from, oracle_from
+    orc = oracle_from(cfg)
+    mesh, st = gpu_from(cfg)
+    r = np.random.default_rng(43)
+    p = 1e-6 * r.standard_normal((len(cfg["xy"]), 2))
+    q_o = orc.stiffness_action(p)
+    qx, qy = mesh.pff_stiffness_action(st, mesh.nodes_to_internal(p[:, 0]), mesh.nodes_to_internal(p[:, 1]))
+    q = np.stack([mesh.nodes_to_user(qx), mesh.nodes_to_user(qy)], 1)
+    assert np.abs(q - q_o).max() <= 1e-8 * np.abs(q_o).max()  # cancellation: |u| / |p| ~ 1e2..1e3 ulp amplification
