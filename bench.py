@@ -173,6 +173,14 @@ def run_ours(args, rank: int, world: int):
     adj_call()
     ms_adj, it_adj = timed(adj_call, 5)
 
+    # matrix-free stiffness action (pff_stiffness_action, Eq. 13), timed alone: one fused element pass per call
+    p_try = [torch.from_numpy((1e-6 * np.random.default_rng(8 + k).standard_normal(N)).astype(mesh.np_dtype)).to(mesh.device)
+             for k in range(2)]
+    q_out = [torch.empty_like(p_try[0]), torch.empty_like(p_try[1])]
+    act_call = lambda: mesh.pff_stiffness_action(st, p_try[0], p_try[1], q_out[0], q_out[1]) and None
+    act_call()
+    ms_act, _ = timed(act_call, args.steps)
+
     # --- end to end: host buffers in USER numbering through pff_run_host, H2D + D2H inside the timed region
     hs = dict(u=np.ascontiguousarray(cfg["u0"], dtype=np.float64), v=np.zeros((N, 2)), a=np.zeros((N, 2)),
               d=np.ascontiguousarray(cfg["d0"], dtype=np.float64), H=np.zeros(Ne),
@@ -194,7 +202,7 @@ def run_ours(args, rank: int, world: int):
     barrier()
     e2e_val = whole_job_value(Ne, ke, world, reduce_max(time.perf_counter() - t0, world, f"cuda:{dev}"))
     return dict(mesh=mesh, cfg=cfg, N=N, Ne=Ne, w=w, ms_total=ms_total, iters=iters, launches=launches, clk=clk, prof=prof,
-                iters_p=iters_p, ms_exp=ms_exp, ms_adj=ms_adj / 5, it_adj=it_adj[0], e2e_val=e2e_val, h2d=(9 * N + Ne) * 8, d2h=(7 * N + Ne) * 8, snapshot=snapshot)
+                iters_p=iters_p, ms_exp=ms_exp, ms_adj=ms_adj / 5, it_adj=it_adj[0], ms_act=ms_act / args.steps, e2e_val=e2e_val, h2d=(9 * N + Ne) * 8, d2h=(7 * N + Ne) * 8, snapshot=snapshot)
 
 
 def ncu_traffic(workload: str, dtype: str, kernel: str, k: dict):
@@ -305,6 +313,9 @@ def main():
                              hbm_frac=(ab["cg_iter"] * r["it_adj"] + ab["matvec"]) / (r["ms_adj"] / 1e3) / 1e9 / peak,
                              note="one pff_damage_adjoint (setup pass + all CG iterations), seeded upstream gradient; "
                                   "algorithmic bytes = iterations x CG iteration + one operator pass for the setup"),
+                stiffness_action=dict(us_per_pass=1e3 * r["ms_act"], algorithmic_bytes=int(Ne * (12 + 5 * w) + N * 7 * w),
+                                      hbm_frac=(Ne * (12 + 5 * w) + N * 7 * w) / (r["ms_act"] / 1e3) / 1e9 / peak,
+                                      note="q = f_int(u + p) - f_int(u), one pass: conn + geometry per element; u, d, p read, q written per node"),
                 clocks=r["clk"], gpu_launches=int(r["launches"]),
                 e2e=dict(value=r["e2e_val"], unit=UNIT, h2d_bytes_per_step=r["h2d"], d2h_bytes_per_step=r["d2h"]),
                 roofline=dict(bound="hbm", kernel=dom, achieved=kern[dom]["achieved_gbs"], peak=peak, unit="GB/s",

@@ -218,6 +218,19 @@ pff_status pff_damage_param_terms(pff_mesh *mesh, const void *lambda, const void
  * Gather scatter only (PFF_EUNSUPPORTED with PFF_SCATTER_ATOMIC).  Asynchronous. */
 pff_status pff_stiffness_action(pff_mesh *mesh, const pff_state *state, const void *px, const void *py, void *qx, void *qy);
 
+/* Quasi-static mechanics solve (PAPER.md L126-159 with L337 "staggered quasi-static mode"): one linear solve
+ *     K(u_ref) du = S f_ext - f_int(u_ref)  on the free dofs,   state->u <- u_ref + du,
+ * u_ref = state->u on entry (Dirichlet dofs first overwritten with bc->dir_u when it is given; bc->dir_v is not used),
+ * S = bc->load_scale, d = state->d fixed, by Jacobi-preconditioned conjugate gradients whose operator is
+ * pff_stiffness_action (one fused element pass per iteration); alpha, beta and the norms stay on the device.
+ * Stops when ||r_free||_2 <= rel_tol ||r0_free||_2 or after max_iter iterations (PFF_ENOCONV, result written).
+ * Exact equilibrium for the isotropic split (linear problem); for the other splits one step of the paper's shifted-
+ * difference iteration (the caller repeats it; exact when du does not change the sign pattern of the split).
+ * The constrained problem must be non-singular (enough Dirichlet dofs to remove the rigid-body modes).
+ * v, a, H are not touched.  Gather scatter only.  Synchronises the stream. */
+pff_status pff_equilibrium_solve(pff_mesh *mesh, pff_state *state, const pff_bc *bc, double rel_tol, int32_t max_iter,
+                                 int32_t *iters_out, double *relres_out);
+
 /* ---- test hooks (device vectors, internal order, precision of the mesh) ---------------------- */
 /* f_int(u, d) of the current state (no predictor), and psi+ per element (psi_plus may be NULL). */
 pff_status pff_internal_force(pff_mesh *mesh, const pff_state *state, void *fx, void *fy, void *psi_plus);

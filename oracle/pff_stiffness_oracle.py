@@ -40,3 +40,17 @@ def assemble_stiffness(xy, tri, E, nu, plane, d, eta):
     rows = np.repeat(dofs, 6, axis=1).ravel()
     cols = np.tile(dofs, (1, 6)).ravel()
     return sp.coo_matrix((Ke.reshape(-1), (rows, cols)), shape=(2 * n, 2 * n)).tocsr()
+
+
+def equilibrium_solve(K, u_ref, fext, S, fixed_dofs):
+    """u = u_ref + du with K_ff du_f = (S f_ext - K u_ref)_f and du = 0 on the fixed dofs (2 * node + component):
+    the quasi-static equilibrium f_int(u) = S f_ext of the linear (isotropic-split) problem, by a direct solve."""
+    import scipy.sparse.linalg as spla
+    n2 = K.shape[0]
+    free = np.ones(n2, dtype=bool)
+    free[np.asarray(fixed_dofs, dtype=np.int64)] = False
+    u0 = np.asarray(u_ref, dtype=np.float64).ravel()
+    r = S * np.asarray(fext, dtype=np.float64).ravel() - K @ u0
+    du = np.zeros(n2)
+    du[free] = spla.spsolve(K[free][:, free].tocsc(), r[free])
+    return (u0 + du).reshape(-1, 2)

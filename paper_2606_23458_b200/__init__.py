@@ -183,12 +183,20 @@ class Mesh:
         _check(self.L.pff_damage_param_terms(self.h, lam.data_ptr(), d.data_ptr(), out))
         return out[0], out[1]
 
-    def pff_stiffness_action(self, state: State, px, py):
+    def pff_stiffness_action(self, state: State, px, py, qx=None, qy=None):
         """q = f_int(u + p) - f_int(u) (Eq. 13) at the state's u, d; device tensors in internal order."""
         import torch
-        qx, qy = torch.empty_like(px), torch.empty_like(py)
+        if qx is None:
+            qx, qy = torch.empty_like(px), torch.empty_like(py)
         _check(self.L.pff_stiffness_action(self.h, C.byref(state.c), px.data_ptr(), py.data_ptr(), qx.data_ptr(), qy.data_ptr()))
         return qx, qy
+
+    def pff_equilibrium_solve(self, state: State, bc=None, rel_tol=1e-8, max_iter=10000, allow_noconv=False):
+        it, rr = C.c_int32(0), C.c_double(0.0)
+        st = _check(self.L.pff_equilibrium_solve(self.h, C.byref(state.c), C.byref(bc) if bc is not None else None,
+                                                 rel_tol, max_iter, C.byref(it), C.byref(rr)),
+                    allow=(PFF_ENOCONV,) if allow_noconv else ())
+        return st, it.value, rr.value
 
     def pff_internal_force(self, state: State):
         import torch

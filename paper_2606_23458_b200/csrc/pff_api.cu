@@ -72,7 +72,7 @@ void pff_mesh_destroy(pff_mesh* m)
                     m->d_halo_ids, m->d_sh_rowptr, m->d_halo_dst, m->d_ell, m->d_flags, m->d_halo_part,
                     m->d_fwx, m->d_fwy, m->d_dir_dof, m->d_ca, m->d_cb, m->d_lb, m->d_r, m->d_p, m->d_q, m->d_dinv, m->d_mask,
                     m->d_part, m->d_part2, m->d_ctrl, m->d_ticket, m->d_step_bar, m->d_stage, m->d_hstate, m->d_node_old_of_new,
-                    m->d_elem_old_of_new};
+                    m->d_elem_old_of_new, m->d_n2e_ptr, m->d_n2e, m->d_eq_vec, m->d_eq_part, m->d_eq_sc};
     for (void* p : ptrs) if (p) cudaFree(p);
     if (m->h_ctrl) cudaFreeHost(m->h_ctrl);
     if (m->h_ring) cudaFreeHost(m->h_ring);
@@ -398,6 +398,14 @@ pff_status pff_stiffness_action(pff_mesh* m, const pff_state* s, const void* px,
         set_error("pff_stiffness_action: px, py must be 16-byte aligned"); return PFF_EINVAL;
     }
     return launch_step(m, const_cast<pff_state*>(s), nullptr, 0.0, /*MODE_TANGENT*/ 3, qx, qy, nullptr, px, py);
+}
+
+pff_status pff_equilibrium_solve(pff_mesh* m, pff_state* s, const pff_bc* bc, double rel_tol, int32_t max_iter, int32_t* iters,
+                                 double* relres)
+{
+    if (!m || !valid_state(s)) { set_error("pff_equilibrium_solve: null mesh, null or misaligned (16 B) state pointer"); return PFF_EINVAL; }
+    if (!(rel_tol > 0) || max_iter < 1) { set_error("pff_equilibrium_solve: need rel_tol > 0, max_iter >= 1"); return PFF_EINVAL; }
+    return equilibrium_solve(m, s, bc, rel_tol, max_iter, iters, relres);
 }
 
 pff_status pff_damage_adjoint(pff_mesh* m, const pff_state* s, const void* g, const uint8_t* free_mask, void* lambda, double rel_tol,

@@ -63,6 +63,10 @@ struct pff_mesh {
     DamageCtrl* h_ring = nullptr;      // pinned ring of deferred read-backs (pff_run_steps)
     DamageCtrl* defer_slot = nullptr;  // non-null: damage_solve copies the control block here and does not synchronise
     unsigned int* d_ticket = nullptr;
+    // quasi-static mechanics solve (pff_equilibrium.cu), allocated at its first call
+    int32_t *d_n2e_ptr = nullptr, *d_n2e = nullptr;  // node -> (4 * element + corner) table
+    void* d_eq_vec = nullptr;                        // 10 nodal vectors
+    double *d_eq_part = nullptr, *d_eq_sc = nullptr;
     unsigned int* d_step_bar = nullptr;  // grid-barrier counter of the step kernel
     unsigned int step_bar_count = 0;     // its value after the launches enqueued so far
 
@@ -98,6 +102,7 @@ pff_status damage_matvec(pff_mesh* m, const pff_state* s, const void* p, void* q
 pff_status damage_adjoint(pff_mesh* m, const pff_state* s, const void* g, const uint8_t* free_mask, void* lambda, double rel_tol,
                           int max_iter, int* iters, double* relres);
 pff_status damage_param_terms(pff_mesh* m, const void* lambda, const void* d, double out[2]);
+pff_status equilibrium_solve(pff_mesh* m, pff_state* s, const pff_bc* bc, double rel_tol, int max_iter, int* iters, double* relres);
 pff_status damage_rhs_diag(pff_mesh* m, const pff_state* s, void* b, void* D);
 pff_status energies(pff_mesh* m, const pff_state* s, double out[4]);
 pff_status cuda_check(cudaError_t e, const char* what);

@@ -140,3 +140,44 @@ def test_stiffness_action_is_the_tangent_when_the_sign_pattern_is_fixed():
     eps = 0.5
     fd = (orc.internal_force(orc.u + eps * p)[0] - orc.internal_force(orc.u - eps * p)[0]) / (2 * eps)
     assert np.abs(q - fd).max() <= 1e-4 * np.abs(fd).max()
+
+
+def _boundary_nodes(n):
+    i, j = np.arange(n * n) % n, np.arange(n * n) // n
+    return np.nonzero((i == 0) | (i == n - 1) | (j == 0) | (j == n - 1))[0]
+
+
+def test_equilibrium_oracle_patch_test_and_force_balance():
+    """Assembled direct solve: (i) affine Dirichlet data on the whole boundary with uniform damage reproduce the affine
+    field in the interior (patch test); (ii) with non-uniform damage and a traction load the C oracle's internal force
+    (an independent code) balances S f_ext on every free dof."""
+    from oracle import pff_stiffness_oracle as sto
+    from pff_inputs import edge_segments
+    n = 9
+    xy, tri = random_mesh(n, 12)
+    m = mat(split=0)
+    G = np.array([[1e-4, -2e-4], [3e-4, 0.5e-4]])
+    u_aff = xy @ G.T
+    bn = _boundary_nodes(n)
+    fixed = np.concatenate([2 * bn, 2 * bn + 1])
+    u0 = np.zeros_like(u_aff)
+    u0[bn] = u_aff[bn]
+    K = sto.assemble_stiffness(xy, tri, m.E, m.nu, 0, np.full(len(xy), 0.3), m.eta)
+    u = sto.equilibrium_solve(K, u0, np.zeros_like(u0), 1.0, fixed)
+    assert np.abs(u - u_aff).max() <= 1e-12 * np.abs(u_aff).max()
+
+    orc = OracleMesh(xy, tri, m)
+    orc.d[:] = np.random.default_rng(13).uniform(0.0, 0.9, len(xy))
+    top = edge_segments(n, n, "top")
+    orc.add_traction(top, np.tile([2e5, 1e6], (len(top), 1)))
+    bottom = np.arange(n)
+    fixed = np.concatenate([2 * bottom, 2 * bottom + 1])
+    K = sto.assemble_stiffness(xy, tri, m.E, m.nu, 0, orc.d, m.eta)
+    S = 0.7
+    u = sto.equilibrium_solve(K, np.zeros((len(xy), 2)), orc.fext, S, fixed)
+    f, _ = orc.internal_force(u)
+    res = (f - S * orc.fext).ravel()
+    free = np.ones(2 * len(xy), dtype=bool)
+    free[fixed] = False
+    assert np.abs(res[free]).max() <= 1e-10 * np.abs(orc.fext).max()
+    assert np.all(u[bottom] == 0.0)

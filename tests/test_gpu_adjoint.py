@@ -156,3 +156,101 @@ def test_stiffness_action_full_size():
     qx, qy = mesh.pff_stiffness_action(st, mesh.nodes_to_internal(p[:, 0]), mesh.nodes_to_internal(p[:, 1]))
     q = np.stack([mesh.nodes_to_user(qx), mesh.nodes_to_user(qy)], 1)
     assert np.abs(q - q_o).max() <= 1e-8 * np.abs(q_o).max()  # cancellation: |u| / |p| ~ 1e2..1e3 ulp amplification
+
+
+# ---------------------------------------------------------------- quasi-static mechanics solve (L126-159, L337)
+def _equilibrium_case(n, seed, split=0):
+    from pff_inputs import edge_segments
+    xy, tri = random_mesh(n, seed)
+    material = dict(GLASS, model=2, split=split, plane=0)
+    d = np.random.default_rng(seed + 1).uniform(0.0, 0.9, len(xy))
+    top = edge_segments(n, n, "top")
+    trac = np.tile([2e5, 1e6], (len(top), 1))
+    bottom = np.arange(n)
+    dir_dof = np.concatenate([2 * bottom, 2 * bottom + 1]).astype(np.int32)
+    return xy, tri, material, d, top, trac, dir_dof
+
+
+@pytest.mark.parametrize("precision", [0, 1])
+def test_equilibrium_solve_matches_assembled_direct_solve(precision):
+    """Isotropic split (linear problem): clamped bottom edge with prescribed values, traction on top, damaged solid,
+    several chunks; the GPU CG on the matrix-free action against the assembled K + direct solve."""
+    from oracle import pff_stiffness_oracle as sto
+    import paper_2606_23458_b200 as pff
+    n = 33
+    xy, tri, material, d, top, trac, dir_dof = _equilibrium_case(n, 51)
+    r = np.random.default_rng(52)
+    dir_u = 1e-5 * r.standard_normal(len(dir_dof))
+    S = 0.7
+    mesh = pff.Mesh(xy, tri, material, precision=precision, chunk_elems=256)
+    st = mesh.new_state(d=d)
+    mesh.pff_set_traction(st, top, trac)
+    mesh.pff_set_dirichlet(dir_dof)
+    bc = mesh.bc(dir_u=dir_u, dir_v=np.zeros(len(dir_dof)), load_scale=S)
+    status, iters, relres = mesh.pff_equilibrium_solve(st, bc, rel_tol=1e-12 if precision == 0 else 1e-6, max_iter=20000,
+                                                       allow_noconv=(precision == 1))
+    assert iters > 0 and relres <= (1e-12 if precision == 0 else 1e-4)
+    u = np.stack([mesh.nodes_to_user(st.ux), mesh.nodes_to_user(st.uy)], 1)
+
+    fext = np.stack([mesh.nodes_to_user(st.fext_x), mesh.nodes_to_user(st.fext_y)], 1)
+    K = sto.assemble_stiffness(xy, tri, material["E"], material["nu"], 0, d, material["eta"])
+    u0 = np.zeros((len(xy), 2))
+    u0.ravel()[dir_dof] = dir_u
+    u_o = sto.equilibrium_solve(K, u0, fext, S, dir_dof)
+    assert np.abs(u - u_o).max() <= (1e-8 if precision == 0 else 2e-3) * np.abs(u_o).max()
+    assert np.abs(u.ravel()[dir_dof] - dir_u).max() <= (0 if precision == 0 else 1e-12)
+
+
+def test_equilibrium_solve_balances_forces_and_is_reproducible():
+    """The solved state satisfies f_int(u) = S f_ext on the free dofs according to the C ORACLE's internal force, and a
+    second solve from the same start gives the same bits."""
+    from oracle import Material, OracleMesh
+    import paper_2606_23458_b200 as pff
+    n = 25
+    xy, tri, material, d, top, trac, dir_dof = _equilibrium_case(n, 61)
+    orc = OracleMesh(xy, tri, Material(**material))
+    orc.d[:] = d
+    orc.add_traction(top, trac)
+    out = []
+    for _ in range(2):
+        mesh = pff.Mesh(xy, tri, material)
+        st = mesh.new_state(d=d)
+        mesh.pff_set_traction(st, top, trac)
+        mesh.pff_set_dirichlet(dir_dof)
+        status, iters, relres = mesh.pff_equilibrium_solve(st, mesh.bc(), rel_tol=1e-12, max_iter=20000)
+        assert status == 0
+        out.append(np.stack([mesh.nodes_to_user(st.ux), mesh.nodes_to_user(st.uy)], 1))
+    assert np.array_equal(out[0], out[1])
+    f, _ = orc.internal_force(out[0])
+    res = (f - orc.fext).ravel()
+    free = np.ones(2 * len(xy), dtype=bool)
+    free[dir_dof] = False
+    assert np.abs(res[free]).max() <= 1e-9 * np.abs(orc.fext).max()
+
+
+def test_equilibrium_step_for_the_spectral_split_under_tension():
+    """Spectral split with every principal strain positive (biaxial pre-stretch): psi+ = psi, the shifted difference is
+    linear and one solve reaches the same equilibrium as the assembled isotropic operator."""
+    from oracle import pff_stiffness_oracle as sto
+    import paper_2606_23458_b200 as pff
+    n = 17
+    xy, tri, material, d, top, trac, dir_dof = _equilibrium_case(n, 71, split=1)
+    d = 0.2 * d  # mild stiffness contrast: the equilibrium strain field stays tensile in every element
+    i, j = np.arange(n * n) % n, np.arange(n * n) // n
+    bn = np.nonzero((i == 0) | (i == n - 1) | (j == 0) | (j == n - 1))[0]
+    dir_dof = np.concatenate([2 * bn, 2 * bn + 1]).astype(np.int32)
+    stretch = 1e-3 * xy                                  # eps = 1e-3 I: both principal strains positive
+    u_start = stretch.copy()
+    inner = np.setdiff1d(np.arange(n * n), bn)
+    u_start[inner] += 1e-7 * np.random.default_rng(72).standard_normal((len(inner), 2))  # off equilibrium, still tensile
+    mesh = pff.Mesh(xy, tri, material)
+    st = mesh.new_state(u=u_start, d=d)
+    mesh.pff_set_dirichlet(dir_dof)
+    status, _, _ = mesh.pff_equilibrium_solve(st, mesh.bc(), rel_tol=1e-12, max_iter=20000)
+    assert status == 0
+    u = np.stack([mesh.nodes_to_user(st.ux), mesh.nodes_to_user(st.uy)], 1)
+    K = sto.assemble_stiffness(xy, tri, material["E"], material["nu"], 0, d, material["eta"])
+    u0 = np.zeros_like(u)
+    u0[bn] = stretch[bn]
+    u_o = sto.equilibrium_solve(K, u0, np.zeros_like(u0), 1.0, dir_dof)
+    assert np.abs(u - u_o).max() <= 1e-8 * np.abs(u_o).max()
