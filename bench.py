@@ -36,6 +36,9 @@ def make_workload(name: str):
     return config(int(name[3:]))
 
 
+EQ_ITERS = 100  # CG iterations of the timed quasi-static solve
+
+
 def algorithmic_bytes(N: int, Ne: int, w: int) -> dict:
     """SURVEY.md 8(d) / DESIGN.md "Algorithmic bytes": every persistent array touched once per pass."""
     step = Ne * (12 + 5 * w + 2 * w) + N * 16 * w          # conn + geometry + H r/w ; u,v,a r/w, d, f_ext, m^-1
@@ -201,8 +204,17 @@ def run_ours(args, rank: int, world: int):
         e2e_step()
     barrier()
     e2e_val = whole_job_value(Ne, ke, world, reduce_max(time.perf_counter() - t0, world, f"cuda:{dev}"))
+
+    # quasi-static mechanics solve (pff_equilibrium_solve), timed LAST because it installs a Dirichlet set (bottom edge
+    # clamped): exactly EQ_ITERS CG iterations on the matrix-free stiffness action (the tolerance is unreachable)
+    yb = cfg["xy"][:, 1]
+    bottom = np.nonzero(yb == yb.min())[0]
+    mesh.pff_set_dirichlet(np.concatenate([2 * bottom, 2 * bottom + 1]).astype(np.int32))
+    eq_call = lambda: mesh.pff_equilibrium_solve(st, None, rel_tol=1e-300, max_iter=EQ_ITERS, allow_noconv=True)[1]
+    eq_call()
+    ms_eq, it_eq = timed(eq_call, 1)
     return dict(mesh=mesh, cfg=cfg, N=N, Ne=Ne, w=w, ms_total=ms_total, iters=iters, launches=launches, clk=clk, prof=prof,
-                iters_p=iters_p, ms_exp=ms_exp, ms_adj=ms_adj / 5, it_adj=it_adj[0], ms_act=ms_act / args.steps, e2e_val=e2e_val, h2d=(9 * N + Ne) * 8, d2h=(7 * N + Ne) * 8, snapshot=snapshot)
+                iters_p=iters_p, ms_exp=ms_exp, ms_adj=ms_adj / 5, it_adj=it_adj[0], ms_act=ms_act / args.steps, ms_eq=ms_eq, it_eq=it_eq[0], e2e_val=e2e_val, h2d=(9 * N + Ne) * 8, d2h=(7 * N + Ne) * 8, snapshot=snapshot)
 
 
 def ncu_traffic(workload: str, dtype: str, kernel: str, k: dict):
@@ -316,6 +328,10 @@ def main():
                 stiffness_action=dict(us_per_pass=1e3 * r["ms_act"], algorithmic_bytes=int(Ne * (12 + 5 * w) + N * 7 * w),
                                       hbm_frac=(Ne * (12 + 5 * w) + N * 7 * w) / (r["ms_act"] / 1e3) / 1e9 / peak,
                                       note="q = f_int(u + p) - f_int(u), one pass: conn + geometry per element; u, d, p read, q written per node"),
+                equilibrium=dict(us_per_iteration=1e3 * r["ms_eq"] / max(r["it_eq"], 1), cg_iterations=r["it_eq"],
+                                 hbm_frac=(Ne * (12 + 5 * w) + N * 23 * w) * max(r["it_eq"], 1) / (r["ms_eq"] / 1e3) / 1e9 / peak,
+                                 note="pff_equilibrium_solve, bottom edge clamped: per iteration one stiffness-action pass + the "
+                                      "CG vector kernels (du, r, p read + written, q, 1/D read: 16 reals per node)"),
                 clocks=r["clk"], gpu_launches=int(r["launches"]),
                 e2e=dict(value=r["e2e_val"], unit=UNIT, h2d_bytes_per_step=r["h2d"], d2h_bytes_per_step=r["d2h"]),
                 roofline=dict(bound="hbm", kernel=dom, achieved=kern[dom]["achieved_gbs"], peak=peak, unit="GB/s",
