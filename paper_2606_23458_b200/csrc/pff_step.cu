@@ -209,19 +209,23 @@ __global__ void __launch_bounds__(kTPB, 2) step_chunk_kernel(const StepArgs<R> a
             const int shift = cm.node_start & (A - 1), hb = (shift + cm.n_int + A - 1) & ~(A - 1), fshift = cm.node_start & 15;
             const int* s_hdst = reinterpret_cast<const int*>(stg + L.hdst) + (cm.halo_off & 3);
 
+            // ---- prefetch chunk k + 1 into the other stage, bulk copies FIRST: they do not depend on this chunk's data, so
+            // two stages are in flight whenever the CTA is waiting for memory (the other stage was freed by the barrier that
+            // ended the previous chunk)
+            if (k + 1 < n_ep && issuer) {
+                const ChunkMeta cn = s_meta[k + 1];
+                const ChunkRange cr{cn.elem_start, cn.n_elem, a.Ne, cn.node_start, cn.n_int, a.N, cn.ell_off,
+                                    cn.ell_w * (cn.n_int + cn.n_halo), (int)a.ell_total, cn.halo_off, cn.n_halo, (int)a.n_entries,
+                                    k + 2 < n_ep ? s_meta[k + 2].halo_off : 0, k + 2 < n_ep ? s_meta[k + 2].n_halo : 0};
+                fence_proxy_async();
+                stage_issue_desc(my_desc, have_desc, smem + (st ^ 1) * L.stage_bytes, bar + 2 * (st ^ 1), lane, cr);
+            }
             // bulk copies AND every thread's halo gathers of this chunk (all issued one iteration ago)
             mbar_wait(bar + 2 * st, (it >> 1) & 1);
-            // ---- prefetch chunk k + 1 into the other stage (its halo ids arrived with THIS stage)
+            // ---- halo gathers of chunk k + 1 (its halo ids arrived with THIS stage)
             if (k + 1 < n_ep) {
                 const ChunkMeta cn = s_meta[k + 1];
                 unsigned char* stn = smem + (st ^ 1) * L.stage_bytes;
-                if (issuer) {
-                    const ChunkRange cr{cn.elem_start, cn.n_elem, a.Ne, cn.node_start, cn.n_int, a.N, cn.ell_off,
-                                        cn.ell_w * (cn.n_int + cn.n_halo), (int)a.ell_total, cn.halo_off, cn.n_halo, (int)a.n_entries,
-                                        k + 2 < n_ep ? s_meta[k + 2].halo_off : 0, k + 2 < n_ep ? s_meta[k + 2].n_halo : 0};
-                    fence_proxy_async();
-                    stage_issue_desc(my_desc, have_desc, stn, bar + 2 * (st ^ 1), lane, cr);
-                }
                 if (issuer) {
                     const int hbn = ((cn.node_start & (A - 1)) + cn.n_int + A - 1) & ~(A - 1);
                     const int* ids = reinterpret_cast<const int*>(stg + L.hnext) + (cn.halo_off & 3);
