@@ -2,8 +2,9 @@
 // L337 "staggered quasi-static mode"):
 //     K(u_ref) du = S f_ext - f_int(u_ref)   on the free dofs,   u = u_ref + du,
 // with K(u_ref) p = f_int(u_ref + p) - f_int(u_ref) evaluated by ONE fused pass of the explicit-step kernel per
-// iteration (pff_step.cu, MODE_TANGENT).  The CG recurrence around it is a handful of small node kernels; alpha, beta and
-// the norms stay on the device (the host reads the scalar block once per batch of iterations).  Jacobi preconditioner:
+// iteration (pff_step.cu, MODE_TANGENT), which also leaves the block partials of p . q.  The rest of the CG recurrence is a
+// handful of small node kernels; alpha, beta and the norms stay on the device (the host reads the scalar block once per
+// batch of iterations).  Jacobi preconditioner:
 // the diagonal of the ISOTROPIC degraded stiffness g(d_e) A_e B^T C B, summed per node over a node -> element table in a
 // fixed order (any SPD diagonal is a valid preconditioner for the other splits).  Every reduction is ordered: the solve
 // is bit-reproducible run to run.  First correct path of this NEXT row; the vector kernels are not fused into the
@@ -80,18 +81,6 @@ __global__ void __launch_bounds__(kTPB) eq_init_kernel(int N, const uint8_t* fla
     const double t0 = block_sum(rz, s_red);
     const double t1 = block_sum(rr, s_red);
     if (threadIdx.x == 0) { part[blockIdx.x] = t0; part[gridDim.x + blockIdx.x] = t1; }
-}
-
-template <typename R>
-__global__ void __launch_bounds__(kTPB) eq_dot_kernel(int N, EqVec<R> v, const double* sc, double* part)
-{
-    __shared__ double s_red[32];
-    if (sc[SC_DONE] != 0.0) return;
-    const int i = blockIdx.x * kTPB + threadIdx.x;
-    double pq = 0.0;
-    if (i < N) pq = double(v.px[i]) * double(v.qx[i]) + double(v.py[i]) * double(v.qy[i]);  // p = 0 on constrained dofs
-    const double t = block_sum(pq, s_red);
-    if (threadIdx.x == 0) part[blockIdx.x] = t;
 }
 
 // du += alpha p, r -= alpha q (free dofs), partials of r.z and r.r
@@ -182,7 +171,7 @@ static pff_status ensure_eq_workspace(pff_mesh* m)
     if ((st = cuda_check(cudaMemcpy(m->d_n2e, adj.data(), sizeof(int32_t) * 3 * Ne, cudaMemcpyHostToDevice), "equilibrium: table")) != PFF_OK) return st;
     if ((st = cuda_check(cudaMalloc(&m->d_eq_vec, 10 * ((N + 15) & ~size_t(15)) * m->rb), "equilibrium: vectors")) != PFF_OK) return st;
     const size_t nb = (N + kTPB - 1) / kTPB;
-    if ((st = cuda_check(cudaMalloc((void**)&m->d_eq_part, sizeof(double) * 2 * nb), "equilibrium: partials")) != PFF_OK) return st;
+    if ((st = cuda_check(cudaMalloc((void**)&m->d_eq_part, sizeof(double) * (2 * nb + (size_t)hm.C)), "equilibrium: partials")) != PFF_OK) return st;
     if ((st = cuda_check(cudaMalloc((void**)&m->d_eq_sc, sizeof(double) * SC_N), "equilibrium: scalars")) != PFF_OK) return st;
     return PFF_OK;
 }
@@ -220,9 +209,12 @@ static pff_status equilibrium_solve_t(pff_mesh* m, pff_state* s, const pff_bc* b
     while (enq < max_iter) {
         const int batch = std::min(25, max_iter - enq);
         for (int k = 0; k < batch; ++k) {
-            if ((st = launch_step(m, s, nullptr, 0.0, /*MODE_TANGENT*/ 3, v.qx, v.qy, nullptr, v.px, v.py)) != PFF_OK) return st;
-            PFF_LAUNCH(m, PFF_K_OTHER, (eq_dot_kernel<R><<<nb, kTPB, 0, cs>>>(N, v, sc, m->d_eq_part)));
-            PFF_LAUNCH(m, PFF_K_OTHER, (eq_reduce_kernel<1><<<1, kTPB, 0, cs>>>(m->d_eq_part, (int)nb, sc)));
+            // q = K p; the action kernel also leaves the block partials of p . q (p is zero on the constrained dofs)
+            m->tangent_pq_part = m->d_eq_part;
+            st = launch_step(m, s, nullptr, 0.0, /*MODE_TANGENT*/ 3, v.qx, v.qy, nullptr, v.px, v.py);
+            m->tangent_pq_part = nullptr;
+            if (st != PFF_OK) return st;
+            PFF_LAUNCH(m, PFF_K_OTHER, (eq_reduce_kernel<1><<<1, kTPB, 0, cs>>>(m->d_eq_part, m->last_step_grid, sc)));
             PFF_LAUNCH(m, PFF_K_OTHER, (eq_update_kernel<R><<<nb, kTPB, 0, cs>>>(N, m->d_flags, v, sc, m->d_eq_part)));
             PFF_LAUNCH(m, PFF_K_OTHER, (eq_reduce_kernel<2><<<1, kTPB, 0, cs>>>(m->d_eq_part, (int)nb, sc)));
             PFF_LAUNCH(m, PFF_K_OTHER, (eq_dir_kernel<R><<<nb, kTPB, 0, cs>>>(N, v, sc)));

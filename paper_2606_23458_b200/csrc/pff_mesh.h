@@ -67,6 +67,8 @@ struct pff_mesh {
     int32_t *d_n2e_ptr = nullptr, *d_n2e = nullptr;  // node -> (4 * element + corner) table
     void* d_eq_vec = nullptr;                        // 10 nodal vectors
     double *d_eq_part = nullptr, *d_eq_sc = nullptr;
+    double* tangent_pq_part = nullptr;  // set around a stiffness-action launch that should also leave the p . q block partials
+    int last_step_grid = 0;             // CTAs of the last step-kernel launch (length of those partials)
     unsigned int* d_step_bar = nullptr;  // grid-barrier counter of the step kernel
     unsigned int step_bar_count = 0;     // its value after the launches enqueued so far
 

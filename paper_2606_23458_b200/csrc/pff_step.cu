@@ -50,6 +50,7 @@ struct StepArgs {
     const R *fex, *fey;
     R *fx_out, *fy_out, *psi_out;
     const R *px, *py;  // MODE_TANGENT: trial direction
+    double* pq_part;   // MODE_TANGENT, may be null: [gridDim.x] block partials of p . q (fixed order within the block)
     R *fwx, *fwy;
     R dt, hdt, hdt2, S;
     MatC<R> mat;
@@ -163,6 +164,7 @@ __global__ void __launch_bounds__(kTPB, 2) step_chunk_kernel(const StepArgs<R> a
         *Geo<R>::slot(smem, s_shared_slots, 3 * EC, EC) = Geo<R>::pair(R(0), R(0));  // the zero pair (lives in the shared region)
     }
     int it = 0;  // stage uses so far: stage = it & 1, mbarrier parity = (it >> 1) & 1
+    double acc_pq = 0.0;  // MODE_TANGENT: this thread's share of p . q
     for (int e0 = 0; e0 < n_my; e0 += kMetaCap) {
         const int n_ep = min(kMetaCap, n_my - e0);
         __syncthreads();  // previous epoch fully consumed (also publishes the mbarrier init)
@@ -295,6 +297,7 @@ __global__ void __launch_bounds__(kTPB, 2) step_chunk_kernel(const StepArgs<R> a
                 }
                 if (i < cm.n_int) {
                     const int gid = cm.node_start + i, s = shift + i;
+                    if (MODE == MODE_TANGENT) acc_pq += double(s_vx[s]) * double(fx) + double(s_vy[s]) * double(fy);
                     if (MODE == MODE_FORCE || MODE == MODE_TANGENT) { a.fx_out[gid] = fx; a.fy_out[gid] = fy; continue; }
                     const uint8_t fl = s_flags[fshift + i];
                     const R minv = s_minv[s];
@@ -331,7 +334,13 @@ __global__ void __launch_bounds__(kTPB, 2) step_chunk_kernel(const StepArgs<R> a
             R px, py;
             predict<R, MODE>(a, gid, px, py);
             finish_node<R, MODE>(a, gid, px, py, fx, fy);
+            if (MODE == MODE_TANGENT) acc_pq += double(a.px[gid]) * double(fx) + double(a.py[gid]) * double(fy);
         }
+    }
+    if (MODE == MODE_TANGENT && a.pq_part) {  // one ordered block sum per CTA; the caller sums the CTAs in index order
+        __shared__ double s_red[32];
+        const double t = block_sum(acc_pq, s_red);
+        if (tid == 0) a.pq_part[blockIdx.x] = t;
     }
 }
 
@@ -436,6 +445,7 @@ static pff_status launch_step_t(pff_mesh* m, const StepArgs<R>& a)
         }
         {   // ONE cooperative launch: chunk phase, grid barrier, interface phase (all CTAs co-resident by construction)
             const unsigned g = (unsigned)std::min<int64_t>(grid, hm.C);
+            m->last_step_grid = (int)g;
             StepArgs<R> b = a;
             b.gbar = m->d_step_bar;
             b.gb_base = m->step_bar_count;
@@ -484,6 +494,7 @@ static pff_status launch_step_r(pff_mesh* m, pff_state* s, const pff_bc* bc, dou
     a.d = (const R*)s->d; a.H = (R*)s->H; a.fex = (const R*)s->fext_x; a.fey = (const R*)s->fext_y;
     a.fx_out = (R*)fx; a.fy_out = (R*)fy; a.psi_out = (R*)psi;
     a.px = (const R*)px; a.py = (const R*)py;
+    a.pq_part = mode == MODE_TANGENT ? m->tangent_pq_part : nullptr;
     a.fwx = (R*)m->d_fwx; a.fwy = (R*)m->d_fwy;
     a.dt = R(dt); a.hdt = R(0.5 * dt); a.hdt2 = R(0.5 * dt * dt);
     a.S = R(bc ? bc->load_scale : 1.0);
