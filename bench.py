@@ -4,7 +4,7 @@
     python bench.py --impl reference ...      # the CPU oracle on the host cores (slow by design)
 
 One "step" = one staggered pass of the whole hot path: pff_explicit_step (Eq. 16-18 with
-the fused element force + history) followed by pff_damage_solve (Jacobi-PCG, rel_tol 1e-8: two setup kernels and
+the fused element force + history) followed by pff_damage_solve (Jacobi-PCG, rel_tol 1e-8: ONE setup kernel and
 ONE cooperative kernel that runs every CG iteration) on one mesh.
 metric = element-updates/s = n_elems * steps / time (PAPER.md L456 reports the same quantity).  Inputs are
 seeded synthetic meshes/fields (pff_inputs.config), resident in HBM for `value`, host buffers for `e2e`.
@@ -95,8 +95,7 @@ class ClockSampler:
 
 def oracle_sample(cfg, steps: int):
     """The oracle as it stands (single thread, plain C loops) stepping `cfg`; returns (elem/s, seconds, iters)."""
-    sys.path.insert(0, os.path.join(ROOT, "tests"))
-    from _harness import oracle_from
+    from oracle import oracle_from
     orc = oracle_from(cfg)
     dt = cfg["dt_factor"] * orc.dt_crit()
     orc.init_accel()

@@ -11,7 +11,9 @@
  *    No exceptions, no abort.  pff_last_error() returns a thread-local, NUL-terminated
  *    description of the last failure.
  *  - "host" pointers are ordinary CPU memory, read (or written) before the call returns.
- *    "device" pointers are CUDA device memory of the GPU that was current at pff_mesh_create.
+ *    "device" pointers are CUDA device memory of the GPU that was current at pff_mesh_create; every entry point makes
+ *    that GPU current for its duration and restores the caller's device.  Several meshes (on one or several GPUs) may
+ *    live in one process; ONE mesh must not be driven from two host threads at the same time.
  *  - The library owns the pff_mesh object and all of its workspaces.  The caller owns every
  *    state buffer (pff_state) and keeps it alive; the library never frees or reallocates it.  Every state
  *    array must be 16-byte aligned (they are sources of bulk-asynchronous copies); PFF_EINVAL otherwise.
@@ -99,7 +101,8 @@ typedef struct {
 } pff_state;
 
 /* Per-step boundary data.  dir_u / dir_v: device arrays of n_dir values (precision of the mesh),
- * ordered like the dof list given to pff_set_dirichlet; may be NULL when n_dir == 0.
+ * ordered like the dof list given to pff_set_dirichlet; both NULL = keep the values the state holds (n_dir == 0 or
+ * homogeneous data written once); exactly one of them NULL with a Dirichlet set installed is PFF_EINVAL.
  * load_scale multiplies fext in Eq. 17: S(t_{n+1}) of Eq. 19. */
 typedef struct {
     const void *dir_u;   /* u_bar(t_{n+1}) */
@@ -166,15 +169,21 @@ pff_status pff_explicit_step(pff_mesh *mesh, pff_state *state, const pff_bc *bc,
  * Stops when ||r_free||_2 <= rel_tol * max(||b||_2, ||b - A d_n||_2) (R10) or after max_iter
  * operator applications (then returns PFF_ENOCONV with the result written).
  * iters_out / relres_out (host, may be NULL) receive the mat-vec count and final relative residual.
- * Device work: two setup kernels and ONE cooperative kernel that runs every CG iteration (the GPU must support
- * cooperative launches and must not be shared with other kernels of the same stream priority during the call).
- * Synchronises the stream. */
+ * Device work: ONE setup kernel (rhs, Jacobi diagonal, first residual, operator coefficients) and ONE kernel that runs
+ * every CG iteration, both cooperative launches (the GPU must support them and must not be shared with other kernels
+ * of the same stream priority during the call).  Synchronises the stream. */
 pff_status pff_damage_solve(pff_mesh *mesh, pff_state *state, double rel_tol, int32_t max_iter,
                             int32_t *iters_out, double *relres_out);
 
 /* out = { E_el, E_kin, E_frac, E_tot } per unit thickness (Eq. 1), accumulated in fp64
  * with a fixed reduction order.  Synchronises the stream. */
 pff_status pff_energies(pff_mesh *mesh, const pff_state *state, double out[4]);
+
+/* Counters of the last pff_damage_solve / pff_damage_adjoint of this mesh (of ALL solves of the last pff_run_steps):
+ * restarts = how often the projected solver (AT1, L181) re-derived its free set after the first time (a bound became
+ * inactive, or a step was truncated); truncations = steps cut short at the first bound hit.  Both 0 for AT2.
+ * Host-only (reads what the solve already downloaded).  Either pointer may be NULL. */
+pff_status pff_damage_last_stats(const pff_mesh *mesh, int32_t *restarts, int32_t *truncations);
 
 /* ---- damage subcycling ---------------------------------------
  * Admissible subcycling factor N_max = floor(c_p / (0.6 c_R)): the damage front moves at <= ~0.6 c_R while the explicit
@@ -245,8 +254,9 @@ pff_status pff_mesh_counters(const pff_mesh *mesh, int64_t *kernel_launches);
 /* Launches ONE kernel of the hot path `reps` times back to back on the mesh stream between two CUDA
  * events (after one untimed launch) and returns the mean milliseconds per launch.  which: 0 = fused
  * explicit step kernel (PFF_SCATTER_ATOMIC: element kernel), 1 = the same kernel for gather meshes, whose interface-node
- * pass is fused into it (ATOMIC: node kernel), 2 = damage mat-vec chunk kernel, 3 = damage mat-vec interface kernel.  The step kernels
- * advance the state with a negligible dt; the mat-vec reads state->d as the trial vector.  Synchronises. */
+ * pass is fused into it (ATOMIC: node kernel), 2 = chunk kernel of the plain damage mat-vec (the pff_damage_matvec hook),
+ * 3 = interface-node kernel of that hook.  The step kernels advance the state with a negligible dt; the mat-vec reads
+ * state->d as the trial vector.  Synchronises. */
 pff_status pff_time_kernel(pff_mesh *mesh, pff_state *state, int32_t which, int32_t reps, float *ms_per_launch);
 
 /* Kernel classes of the hot path, for per-kernel timing inside a real run (bench.py's roofline block). */
@@ -255,10 +265,9 @@ typedef enum {
     PFF_K_STEP_SHARED = 1,     /* ATOMIC only: node kernel                                                               */
     PFF_K_MATVEC_CHUNK = 2,    /* the cooperative CG kernel (all iterations of one solve); plain mat-vec of the hook     */
     PFF_K_MATVEC_SHARED = 3,   /* interface nodes of the hook's plain mat-vec                                            */
-    PFF_K_CG_VECTOR = 4,       /* unused (the vector updates are fused into the CG kernel)                               */
-    PFF_K_DAMAGE_SETUP = 5,    /* rhs, Jacobi diagonal, r0 (chunk + interface kernels), finalize clamp                    */
-    PFF_K_OTHER = 6,           /* Dirichlet overwrite, energies, host-path permutation kernels                            */
-    PFF_NUM_KERNEL_CLASSES = 7
+    PFF_K_DAMAGE_SETUP = 4,    /* the damage setup kernel: rhs, Jacobi diagonal, r0, operator coefficients, norms        */
+    PFF_K_OTHER = 5,           /* Dirichlet overwrite, energies, host-path permutation, quasi-static vector kernels      */
+    PFF_NUM_KERNEL_CLASSES = 6
 } pff_kernel_class;
 /* enable != 0: every following kernel launch of this mesh is bracketed by two CUDA events on the mesh
  * stream (adds ~2 event records per launch; use for attribution, not for headline throughput).

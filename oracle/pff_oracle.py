@@ -186,3 +186,18 @@ class OracleMesh:
         self.L.orc_energies(self.N, self.Ne, self.tri, self.gradphi, self.area, self.mass, C.byref(self._m),
                             self.u, self.v, self.d, out)
         return out
+
+
+def oracle_from(cfg) -> OracleMesh:
+    """OracleMesh of a pff_inputs.config dictionary (mesh, material, initial fields, tractions, Dirichlet sets):
+    marshalling only.  Used by the parity tests and by bench.py's cpu_baseline / --impl reference legs."""
+    m = OracleMesh(cfg["xy"], cfg["tri"], Material(**cfg["material"]))
+    m.u[:] = cfg["u0"]
+    m.d[:] = cfg["d0"]
+    if len(cfg["edges"]):
+        m.add_traction(cfg["edges"], cfg["traction"])
+    if len(cfg["notch"]):
+        m.set_damage_dirichlet(cfg["notch"])
+    if len(cfg["dir_dof"]):
+        m.set_dirichlet(cfg["dir_dof"])
+    return m

@@ -153,6 +153,12 @@ class Mesh:
                     allow=(PFF_ENOCONV,) if allow_noconv else ())
         return st, it.value, rr.value
 
+    def pff_damage_last_stats(self):
+        """(restarts, truncations) of the projected solver in the last solve / summed over the last pff_run_steps."""
+        r, t = C.c_int32(0), C.c_int32(0)
+        _check(self.L.pff_damage_last_stats(self.h, C.byref(r), C.byref(t)))
+        return r.value, t.value
+
     def pff_run_steps(self, state: State, bc, dt: float, n_steps: int, damage_every=1, rel_tol=1e-8, max_iter=1000,
                       allow_noconv=False):
         """n_steps staggered steps on the device-resident state, damage solve every damage_every-th step."""

@@ -14,13 +14,13 @@ PFF_PLANE_STRAIN, PFF_PLANE_STRESS = 0, 1
 PFF_F64, PFF_F32 = 0, 1
 PFF_SCATTER_GATHER, PFF_SCATTER_ATOMIC = 0, 1
 PFF_ORDER_NONE, PFF_ORDER_MORTON, PFF_ORDER_BISECTION = 0, 1, 2
-KERNEL_CLASSES = ("step_chunk", "step_shared", "matvec_chunk", "matvec_shared", "cg_vector", "damage_setup", "other")
+KERNEL_CLASSES = ("step_chunk", "step_shared", "matvec_chunk", "matvec_shared", "damage_setup", "other")
 
 # every symbol include/pff.h declares
 SYMBOLS = [
     "pff_mesh_create", "pff_mesh_plan", "pff_mesh_destroy", "pff_mesh_info", "pff_mesh_permutations", "pff_set_dirichlet",
     "pff_set_damage_dirichlet", "pff_set_traction", "pff_init_accel", "pff_explicit_step", "pff_damage_solve",
-    "pff_energies", "pff_subcycle_limit", "pff_run_steps", "pff_damage_adjoint", "pff_damage_param_terms", "pff_stiffness_action", "pff_equilibrium_solve", "pff_internal_force", "pff_damage_matvec", "pff_damage_rhs_diag", "pff_run_host", "pff_mesh_counters", "pff_time_kernel",
+    "pff_energies", "pff_damage_last_stats", "pff_subcycle_limit", "pff_run_steps", "pff_damage_adjoint", "pff_damage_param_terms", "pff_stiffness_action", "pff_equilibrium_solve", "pff_internal_force", "pff_damage_matvec", "pff_damage_rhs_diag", "pff_run_host", "pff_mesh_counters", "pff_time_kernel",
     "pff_profile_enable", "pff_profile_read",
     "pff_last_error",
 ]
@@ -75,6 +75,7 @@ def load() -> C.CDLL:
     L.pff_explicit_step.argtypes = [vp, C.POINTER(pff_state), C.POINTER(pff_bc), C.c_double]
     L.pff_damage_solve.argtypes = [vp, C.POINTER(pff_state), C.c_double, i32, ip, dp]
     L.pff_energies.argtypes = [vp, C.POINTER(pff_state), dp]
+    L.pff_damage_last_stats.argtypes = [vp, ip, ip]
     L.pff_subcycle_limit.argtypes = [C.POINTER(pff_material), ip, dp]
     L.pff_run_steps.argtypes = [vp, C.POINTER(pff_state), C.POINTER(pff_bc), C.c_double, i64, i32, C.c_double, i32, C.POINTER(i64)]
     L.pff_internal_force.argtypes = [vp, C.POINTER(pff_state), vp, vp, vp]

@@ -307,4 +307,52 @@ pff_status build_host_mesh(int64_t N, const double* xy, int64_t Ne, const int32_
     return PFF_OK;
 }
 
+// Bounds proof of the widened bulk copies (stage_issue_desc, pff_tma.cuh), chunk by chunk: the device copies the
+// 16-byte-granule cover [a0, a1) of every contiguous range it stages, a0 = start rounded down, a1 = end rounded up but
+// never beyond the last full granule of the array.  Here the same arithmetic is restated on the host and checked
+// against (i) the array length (source side) and (ii) the capacity of the stage region the range lands in
+// (destination side: the lengths make_stage_layout is given).  Any violation fails mesh creation.
+bool verify_stage_extents(const HostMesh& hm, int64_t ell_total, int64_t n_entries, size_t rb, std::string& err)
+{
+    struct Range { int64_t start, count, total; int esize; int64_t cap_bytes; const char* what; };
+    auto up16 = [](int64_t v) { return (v + 15) / 16 * 16; };
+    const int EC = hm.chunk_elems;
+    for (int64_t c = 0; c < hm.C; ++c) {
+        const ChunkMeta& m = hm.meta[c];
+        const int64_t nloc = m.n_int + m.n_halo;
+        const int64_t next_off = c + 1 < hm.C ? hm.meta[c + 1].halo_off : 0, next_n = c + 1 < hm.C ? hm.meta[c + 1].n_halo : 0;
+        const Range rs[] = {
+            {m.elem_start, m.n_elem, hm.Ne, 8, up16(8 * (int64_t)EC), "local connectivity"},
+            {m.elem_start, m.n_elem, hm.Ne, 16, 16 * (int64_t)EC, "geometry / coefficient pair"},
+            {m.elem_start, m.n_elem, hm.Ne, (int)rb, up16((int64_t)rb * EC), "area / history"},
+            {m.node_start, m.n_int, hm.N, (int)rb, up16((int64_t)rb * hm.node_len), "nodal array"},
+            {m.node_start, m.n_int, hm.N, 1, up16(hm.flag_len), "flag bytes"},
+            {m.ell_off, (int64_t)m.ell_w * nloc, ell_total, 2, up16(2 * (int64_t)hm.ell_len), "gather table"},
+            {m.halo_off, m.n_halo, n_entries, 4, up16(4 * ((int64_t)hm.max_nhalo + 4)), "halo partial slots"},
+            {next_off, next_n, n_entries, 4, up16(4 * ((int64_t)hm.max_nhalo + 4)), "next chunk's halo ids"},
+        };
+        for (const Range& r : rs) {
+            if (r.count <= 0) continue;
+            const int64_t A1 = 16 / r.esize - 1;
+            const int64_t a0 = r.start & ~A1, end = r.start + r.count;
+            const int64_t a1 = std::max(a0, std::min((end + A1) & ~A1, r.total & ~A1));
+            const bool src_ok = a0 >= 0 && a1 <= r.total && end <= r.total;
+            // destination: the bulk part [a0, a1) and the plain-load tail [a1, end) both land at (index - a0) * esize
+            const bool dst_ok = (std::max(a1, end) - a0) * r.esize <= r.cap_bytes;
+            if (!src_ok || !dst_ok) {
+                err = std::string("internal: staged range of the ") + r.what + " of chunk " + std::to_string(c) +
+                      (src_ok ? " overruns its shared-memory region" : " leaves its array");
+                return false;
+            }
+        }
+        // halo nodes sit behind the interior block of every staged nodal array
+        const int64_t A = 16 / (int64_t)rb, hb = ((m.node_start % A) + m.n_int + A - 1) / A * A;
+        if (hb + m.n_halo > hm.node_len || m.n_halo > hm.max_nhalo) {
+            err = "internal: halo slots of chunk " + std::to_string(c) + " overrun the staged nodal arrays";
+            return false;
+        }
+    }
+    return true;
+}
+
 }  // namespace pff

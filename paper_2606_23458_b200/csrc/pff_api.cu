@@ -47,6 +47,26 @@ static pff_status upload_real(void** dst, const double* src, size_t count, size_
     return s;
 }
 
+pff_status persistent_config(pff_mesh* m, const void* kern, int smem_bytes, int* grid)
+{
+    auto it = m->launch_grid.find(kern);
+    if (it != m->launch_grid.end()) { *grid = it->second; return PFF_OK; }
+    // static + dynamic shared memory may exceed 48 KB: always opt in (per device; the mesh's device is current here)
+    PFF_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
+    int per_sm = 0, sms = 0;
+    PFF_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kTPB, (size_t)smem_bytes));
+    PFF_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, m->device));
+    *grid = (per_sm > 0 ? per_sm : 1) * sms;
+    m->launch_grid.emplace(kern, *grid);
+    return PFF_OK;
+}
+
+// Dirichlet values come as a pair: with a Dirichlet set installed, giving exactly one of dir_u / dir_v is an error
+static bool valid_bc(const pff_mesh* m, const pff_bc* bc)
+{
+    return !(m->n_dir > 0 && bc && ((bc->dir_u == nullptr) != (bc->dir_v == nullptr)));
+}
+
 // all ten arrays present and 16-byte aligned (they are streamed with bulk-asynchronous copies)
 static bool valid_state(const pff_state* s)
 {
@@ -67,11 +87,12 @@ const char* pff_last_error(void) { return g_err.c_str(); }
 void pff_mesh_destroy(pff_mesh* m)
 {
     if (!m) return;
+    DeviceGuard dg(m);
     cudaStreamSynchronize(m->stream);
     void* ptrs[] = {m->d_meta, m->d_lconn, m->d_conn, m->d_ga, m->d_gb, m->d_area, m->d_minv, m->d_mass,
                     m->d_halo_ids, m->d_sh_rowptr, m->d_halo_dst, m->d_ell, m->d_flags, m->d_halo_part,
                     m->d_fwx, m->d_fwy, m->d_dir_dof, m->d_ca, m->d_cb, m->d_lb, m->d_r, m->d_p, m->d_q, m->d_dinv, m->d_mask,
-                    m->d_part, m->d_part2, m->d_ctrl, m->d_ticket, m->d_step_bar, m->d_stage, m->d_hstate, m->d_node_old_of_new,
+                    m->d_part, m->d_ctrl, m->d_ticket, m->d_step_bar, m->d_stage, m->d_hstate, m->d_hdir, m->d_node_old_of_new,
                     m->d_elem_old_of_new, m->d_n2e_ptr, m->d_n2e, m->d_eq_vec, m->d_eq_part, m->d_eq_sc};
     for (void* p : ptrs) if (p) cudaFree(p);
     if (m->h_ctrl) cudaFreeHost(m->h_ctrl);
@@ -126,6 +147,9 @@ pff_status pff_mesh_create(int64_t n_nodes, const double* xy, int64_t n_elems, c
     m->lay_mv = make_stage_layout(1, hm.chunk_elems, hm.node_len, hm.flag_len, hm.ell_len, hm.max_nhalo, m->rb, chunk_kernel_stages(1));
     m->lay_su = make_stage_layout(2, hm.chunk_elems, hm.node_len, hm.flag_len, hm.ell_len, hm.max_nhalo, m->rb, chunk_kernel_stages(2));
     m->ell_total = (int64_t)hm.ell.size();
+    if (!verify_stage_extents(hm, m->ell_total, (int64_t)hm.halo_ids.size(), m->rb, err)) {
+        set_error("pff_mesh_create: " + err); delete m; return PFF_EMESH;
+    }
 
     auto fail = [&](pff_status s) { pff_mesh_destroy(m); return s; };
     cudaStream_t cs = m->stream;
@@ -206,6 +230,9 @@ pff_status pff_mesh_plan(int64_t n_nodes, const double* xy, int64_t n_elems, con
                              hm, err);
     } catch (const std::bad_alloc&) { st = PFF_ENOMEM; err = "out of host memory in mesh setup"; }
     if (st != PFF_OK) { set_error("pff_mesh_plan: " + err); return st; }
+    if (!verify_stage_extents(hm, (int64_t)hm.ell.size(), (int64_t)hm.halo_ids.size(), opt.precision == PFF_F32 ? 4 : 8, err)) {
+        set_error("pff_mesh_plan: " + err); return PFF_EMESH;
+    }
     if (node_new_of_old) std::memcpy(node_new_of_old, hm.node_new_of_old.data(), sizeof(int32_t) * hm.N);
     if (elem_new_of_old) std::memcpy(elem_new_of_old, hm.elem_new_of_old.data(), sizeof(int32_t) * hm.Ne);
     if (n_chunks) *n_chunks = hm.C;
@@ -247,6 +274,7 @@ static pff_status push_flags(pff_mesh* m)
 pff_status pff_set_dirichlet(pff_mesh* m, int64_t n_dir, const int32_t* dir_dof)
 {
     if (!m || n_dir < 0 || (n_dir > 0 && !dir_dof)) { set_error("pff_set_dirichlet: bad argument"); return PFF_EINVAL; }
+    DeviceGuard dg(m);
     std::vector<int32_t> idof(n_dir);
     for (int64_t k = 0; k < n_dir; ++k) {
         if (dir_dof[k] < 0 || dir_dof[k] >= 2 * m->hm.N) { set_error("pff_set_dirichlet: dof out of range"); return PFF_EINVAL; }
@@ -268,6 +296,7 @@ pff_status pff_set_dirichlet(pff_mesh* m, int64_t n_dir, const int32_t* dir_dof)
 pff_status pff_set_damage_dirichlet(pff_mesh* m, int64_t n, const int32_t* nodes)
 {
     if (!m || n < 0 || (n > 0 && !nodes)) { set_error("pff_set_damage_dirichlet: bad argument"); return PFF_EINVAL; }
+    DeviceGuard dg(m);
     for (int64_t k = 0; k < n; ++k)
         if (nodes[k] < 0 || nodes[k] >= m->hm.N) { set_error("pff_set_damage_dirichlet: node out of range"); return PFF_EINVAL; }
     for (auto& f : m->h_flags) f &= uint8_t(~4);
@@ -280,6 +309,7 @@ pff_status pff_set_traction(pff_mesh* m, pff_state* s, int64_t n_edges, const in
     if (!m || !s || !s->fext_x || !s->fext_y || n_edges < 0 || (n_edges > 0 && (!edge_nodes || !t))) {
         set_error("pff_set_traction: bad argument"); return PFF_EINVAL;
     }
+    DeviceGuard dg(m);
     const int64_t N = m->hm.N;
     std::vector<double> fx(N, 0.0), fy(N, 0.0);
     const double* xy = m->hm.xy_user.data();
@@ -307,6 +337,7 @@ pff_status pff_set_traction(pff_mesh* m, pff_state* s, int64_t n_edges, const in
 pff_status pff_init_accel(pff_mesh* m, pff_state* s, const pff_bc* bc)
 {
     if (!m || !valid_state(s)) { set_error("pff_init_accel: null mesh, null or misaligned (16 B) state pointer"); return PFF_EINVAL; }
+    DeviceGuard dg(m);
     return launch_step(m, s, bc, 0.0, /*MODE_INIT*/ 1, nullptr, nullptr, nullptr);
 }
 
@@ -314,6 +345,8 @@ pff_status pff_explicit_step(pff_mesh* m, pff_state* s, const pff_bc* bc, double
 {
     if (!m || !valid_state(s)) { set_error("pff_explicit_step: null mesh, null or misaligned (16 B) state pointer"); return PFF_EINVAL; }
     if (!(dt > 0) || !std::isfinite(dt)) { set_error("pff_explicit_step: dt must be > 0"); return PFF_EINVAL; }
+    if (!valid_bc(m, bc)) { set_error("pff_explicit_step: dir_u and dir_v must be given together"); return PFF_EINVAL; }
+    DeviceGuard dg(m);
     return launch_step(m, s, bc, dt, /*MODE_STEP*/ 0, nullptr, nullptr, nullptr);
 }
 
@@ -321,6 +354,7 @@ pff_status pff_internal_force(pff_mesh* m, const pff_state* s, void* fx, void* f
 {
     if (!m || !valid_state(s) || !fx || !fy) { set_error("pff_internal_force: null argument"); return PFF_EINVAL; }
     if (m->opt.scatter == PFF_SCATTER_ATOMIC) { set_error("pff_internal_force: gather meshes only"); return PFF_EUNSUPPORTED; }
+    DeviceGuard dg(m);
     return launch_step(m, const_cast<pff_state*>(s), nullptr, 0.0, /*MODE_FORCE*/ 2, fx, fy, psi_plus);
 }
 
@@ -328,7 +362,16 @@ pff_status pff_damage_solve(pff_mesh* m, pff_state* s, double rel_tol, int32_t m
 {
     if (!m || !valid_state(s)) { set_error("pff_damage_solve: null mesh, null or misaligned (16 B) state pointer"); return PFF_EINVAL; }
     if (!(rel_tol > 0) || max_iter < 1) { set_error("pff_damage_solve: need rel_tol > 0, max_iter >= 1"); return PFF_EINVAL; }
+    DeviceGuard dg(m);
     return damage_solve(m, s, rel_tol, max_iter, iters, relres);
+}
+
+pff_status pff_damage_last_stats(const pff_mesh* m, int32_t* restarts, int32_t* truncations)
+{
+    if (!m) { set_error("pff_damage_last_stats: null mesh"); return PFF_EINVAL; }
+    if (restarts) *restarts = m->last_restarts;
+    if (truncations) *truncations = m->last_truncs;
+    return PFF_OK;
 }
 
 pff_status pff_subcycle_limit(const pff_material* mat, int32_t* n_max, double* ratio)
@@ -356,6 +399,8 @@ pff_status pff_run_steps(pff_mesh* m, pff_state* s, const pff_bc* bc, double dt,
         (damage_every > 0 && (!(rel_tol > 0) || max_iter < 1))) {
         set_error("pff_run_steps: need dt > 0, n_steps >= 0, damage_every >= 0, rel_tol > 0, max_iter >= 1"); return PFF_EINVAL;
     }
+    if (!valid_bc(m, bc)) { set_error("pff_run_steps: dir_u and dir_v must be given together"); return PFF_EINVAL; }
+    DeviceGuard dg(m);
     // The whole loop is asynchronous: every solve copies its control block into a pinned ring; the host synchronises and
     // inspects the ring only every kRing solves and at the end, so the GPU never waits for the host between steps.
     constexpr int kRing = 64;
@@ -363,11 +408,13 @@ pff_status pff_run_steps(pff_mesh* m, pff_state* s, const pff_bc* bc, double dt,
     pff_status worst = PFF_OK, st = PFF_OK;
     int64_t total = 0;
     int pending = 0;
+    m->last_restarts = m->last_truncs = 0;
     auto drain = [&]() -> pff_status {
         pff_status e = cuda_check(cudaStreamSynchronize(m->stream), "pff_run_steps: sync");
         if (e != PFF_OK) return e;
         for (int i = 0; i < pending; ++i) {
             total += m->h_ring[i].iters;
+            m->last_restarts += m->h_ring[i].restarts; m->last_truncs += m->h_ring[i].truncs;
             if (!m->h_ring[i].done || m->h_ring[i].status == PFF_ENOCONV) worst = PFF_ENOCONV;
         }
         pending = 0;
@@ -397,6 +444,7 @@ pff_status pff_stiffness_action(pff_mesh* m, const pff_state* s, const void* px,
     if ((reinterpret_cast<uintptr_t>(px) | reinterpret_cast<uintptr_t>(py)) & 15) {
         set_error("pff_stiffness_action: px, py must be 16-byte aligned"); return PFF_EINVAL;
     }
+    DeviceGuard dg(m);
     return launch_step(m, const_cast<pff_state*>(s), nullptr, 0.0, /*MODE_TANGENT*/ 3, qx, qy, nullptr, px, py);
 }
 
@@ -405,6 +453,7 @@ pff_status pff_equilibrium_solve(pff_mesh* m, pff_state* s, const pff_bc* bc, do
 {
     if (!m || !valid_state(s)) { set_error("pff_equilibrium_solve: null mesh, null or misaligned (16 B) state pointer"); return PFF_EINVAL; }
     if (!(rel_tol > 0) || max_iter < 1) { set_error("pff_equilibrium_solve: need rel_tol > 0, max_iter >= 1"); return PFF_EINVAL; }
+    DeviceGuard dg(m);
     return equilibrium_solve(m, s, bc, rel_tol, max_iter, iters, relres);
 }
 
@@ -416,24 +465,28 @@ pff_status pff_damage_adjoint(pff_mesh* m, const pff_state* s, const void* g, co
         return PFF_EINVAL;
     }
     if (!(rel_tol > 0) || max_iter < 1) { set_error("pff_damage_adjoint: need rel_tol > 0, max_iter >= 1"); return PFF_EINVAL; }
+    DeviceGuard dg(m);
     return damage_adjoint(m, s, g, free_mask, lambda, rel_tol, max_iter, iters, relres);
 }
 
 pff_status pff_damage_param_terms(pff_mesh* m, const void* lambda, const void* d, double out[2])
 {
     if (!m || !lambda || !d || !out) { set_error("pff_damage_param_terms: null argument"); return PFF_EINVAL; }
+    DeviceGuard dg(m);
     return damage_param_terms(m, lambda, d, out);
 }
 
 pff_status pff_damage_matvec(pff_mesh* m, const pff_state* s, const void* p, void* q)
 {
     if (!m || !valid_state(s) || !p || !q) { set_error("pff_damage_matvec: null argument"); return PFF_EINVAL; }
+    DeviceGuard dg(m);
     return damage_matvec(m, s, p, q);
 }
 
 pff_status pff_damage_rhs_diag(pff_mesh* m, const pff_state* s, void* b, void* D)
 {
     if (!m || !valid_state(s)) { set_error("pff_damage_rhs_diag: null argument"); return PFF_EINVAL; }
+    DeviceGuard dg(m);
     return damage_rhs_diag(m, s, b, D);
 }
 
@@ -447,6 +500,7 @@ pff_status pff_mesh_counters(const pff_mesh* m, int64_t* kernel_launches)
 pff_status pff_profile_enable(pff_mesh* m, int32_t enable)
 {
     if (!m) { set_error("pff_profile_enable: null mesh"); return PFF_EINVAL; }
+    DeviceGuard dg(m);
     PFF_CUDA(cudaStreamSynchronize(m->stream));
     m->prof_on = enable != 0;
     for (auto& u : m->prof_used) u = 0;
@@ -456,6 +510,7 @@ pff_status pff_profile_enable(pff_mesh* m, int32_t enable)
 pff_status pff_profile_read(pff_mesh* m, double* ms_sum, int64_t* launches)
 {
     if (!m || !ms_sum || !launches) { set_error("pff_profile_read: null argument"); return PFF_EINVAL; }
+    DeviceGuard dg(m);
     PFF_CUDA(cudaStreamSynchronize(m->stream));
     for (int c = 0; c < PFF_NUM_KERNEL_CLASSES; ++c) {
         double sum = 0.0;
@@ -477,6 +532,7 @@ pff_status pff_time_kernel(pff_mesh* m, pff_state* s, int32_t which, int32_t rep
         set_error("pff_time_kernel: bad argument"); return PFF_EINVAL;
     }
     if (m->opt.scatter != PFF_SCATTER_GATHER && which >= 2) { set_error("pff_time_kernel: gather meshes only"); return PFF_EUNSUPPORTED; }
+    DeviceGuard dg(m);
     cudaEvent_t e0, e1;
     PFF_CUDA(cudaEventCreate(&e0));
     PFF_CUDA(cudaEventCreate(&e1));
@@ -507,6 +563,7 @@ pff_status pff_time_kernel(pff_mesh* m, pff_state* s, int32_t which, int32_t rep
 pff_status pff_energies(pff_mesh* m, const pff_state* s, double out[4])
 {
     if (!m || !valid_state(s) || !out) { set_error("pff_energies: null argument"); return PFF_EINVAL; }
+    DeviceGuard dg(m);
     return energies(m, s, out);
 }
 

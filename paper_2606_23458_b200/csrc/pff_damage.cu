@@ -16,7 +16,8 @@
 //                     every CTA reduces the block partials in the same fixed order and advances its own copy of
 //                     alpha, beta and the restart / truncation / convergence flags.  After the last iteration the
 //                     same kernel applies the pending step and the clamp d <- min(1, max(d_n, d)) (L179).
-// alpha, beta and the norms never leave the device; the host reads one 128-byte control block per solve.
+// alpha, beta and the norms never leave the device; the control block is initialised by the setup kernel (tolerance and
+// iteration cap travel as kernel arguments: nothing is uploaded) and the host reads it back once per solve.
 // Convergence is declared on the TRUE residual norm, or (AT2) on the predicted one when its rounding error bound
 // is far below the tolerance.
 #include <algorithm>
@@ -46,7 +47,6 @@ struct DmgArgs {
     R* halo_part;  // [3][n_slots]
     int64_t n_slots, n_entries, ell_total;
     int EC, N, Ne, N_int, N_sh, C, n_ovf;
-    int n_chunk_blocks;  // CTAs of the chunk kernel that wrote block partials (persistent iteration kernel: its grid)
     const int32_t *sh_rowptr, *halo_dst;
     StageLayout lay;
     StagePlan plan;
@@ -62,10 +62,12 @@ struct DmgArgs {
     int no_clamp;
     R *q_out, *b_out, *D_out;
     double* part;    // [kCh][part_n] chunk-kernel block partials
-    double* part2;   // [kCh][kMaxSharedBlocks] interface-kernel block partials (chunk partials folded in)
     int64_t part_n;
     DamageCtrl* ctrl;
-    unsigned int* ticket;
+    double tol;              // stopping tolerance and iteration cap of this solve (the setup kernel writes them into ctrl)
+    int max_iter;
+    unsigned int* ticket;    // [0] last-block ticket, [1] grid barrier of the CG kernel, [2] grid barrier of the setup kernel
+    unsigned int su_base;    // value of ticket[2] before this setup launch (the counter only grows, like the step kernel's)
     MatC<R> mat;
 };
 
@@ -198,10 +200,10 @@ __device__ __forceinline__ void cg_scalar_step(DamageCtrl* c, const double t[kCh
     c->relres = sqrt(rr) / c->nb;
     // true residual norm: AT2 every iteration; AT1 on the freshly derived free set (then KKT holds)
     if ((was_restart || !PROJ) && sqrt(rr) <= lim) { c->done = 1; c->status = PFF_OK; c->pending = 0; return; }
-    if (was_restart) c->restarts += 1;
+    if (was_restart && c->iters > 1) c->restarts += 1;  // the first free set is not a RE-start
     double alpha = pq > 0.0 ? rz / pq : 0.0;
     const int trunc = (PROJ && alpha >= t[kCh - 1]) ? 1 : 0;
-    if (trunc) alpha = t[kCh - 1];
+    if (trunc) { alpha = t[kCh - 1]; c->truncs += 1; }
     // r.z and r.r after the step, from the sums gathered in this pass (no extra pass over the vectors)
     const double rz_pred = fmax(rz - 2.0 * alpha * t[3] + alpha * alpha * t[4], 0.0);
     const double rr_pred = rr - 2.0 * alpha * t[5] + alpha * alpha * t[6];
@@ -593,6 +595,8 @@ __global__ void __launch_bounds__(kTPB, 2) dmg_setup_chunk(const DmgArgs<R> a)
     if (tid == 0) {
         mbar_init(bar, 1 + kTPB); mbar_init(bar + 2, 1 + kTPB);
         s_sq[3 * EC] = R(0); s_sD[3 * EC] = R(0); s_sb[3 * EC] = R(0);
+        // the CG kernel that follows in stream order counts its grid barriers from zero (the previous one has finished)
+        if (blockIdx.x == 0) a.ticket[1] = 0u;
     }
     double acc[kCh];
 #pragma unroll
@@ -712,7 +716,7 @@ __global__ void __launch_bounds__(kTPB, 2) dmg_setup_chunk(const DmgArgs<R> a)
     }
     // ---- interface nodes after a grid-wide barrier: ordered sums of the three partial planes, same outputs
     if (a.N_sh > 0) {
-        unsigned int target = 0;
+        unsigned int target = a.su_base;
         grid_barrier(a.ticket + 2, target, (unsigned)G);
         const int per = (a.N_sh + G - 1) / G, end = min(a.N_sh, ((int)blockIdx.x + 1) * per);  // equal slice per CTA
         for (int sn = blockIdx.x * per + tid; sn < end; sn += kTPB) {
@@ -753,12 +757,14 @@ __global__ void __launch_bounds__(kTPB, 2) dmg_setup_chunk(const DmgArgs<R> a)
             if (lane == 0) s_out[w] = v;
         }
         __syncthreads();
-        if (tid == 0) {
-            DamageCtrl* c = a.ctrl;
-            c->nb = fmax(fmax(sqrt(s_out[0]), sqrt(s_out[1])), 1e-300);
+        if (tid == 0) {  // the control block of this solve, written in full (nothing is uploaded by the host)
+            DamageCtrl c{};
+            c.tol = a.tol; c.max_iter = a.max_iter; c.first = 1; c.restart = 1; c.status = PFF_ENOCONV;
+            c.nb = fmax(fmax(sqrt(s_out[0]), sqrt(s_out[1])), 1e-300);
             // d_n already solves the system to the tolerance (no history growth since the last solve; AT1: KKT holds with
             // the free set the solver would start from): no CG iteration is needed, the cooperative kernel only clamps
-            if (sqrt(s_out[2]) <= c->tol * c->nb) { c->done = 1; c->status = PFF_OK; c->relres = sqrt(s_out[2]) / c->nb; c->pending = 0; }
+            if (sqrt(s_out[2]) <= c.tol * c.nb) { c.done = 1; c.status = PFF_OK; c.relres = sqrt(s_out[2]) / c.nb; }
+            *a.ctrl = c;
         }
     }
 }
@@ -773,11 +779,10 @@ static DmgArgs<R> make_args(pff_mesh* m, const pff_state* s)
     a.halo_part = (R*)m->d_halo_part; a.n_slots = m->n_slots; a.n_entries = m->n_entries; a.ell_total = m->ell_total; a.n_ovf = hm.n_ovf;
     a.EC = hm.chunk_elems;
     a.N = (int)hm.N; a.Ne = (int)hm.Ne; a.N_int = (int)hm.N_int; a.N_sh = (int)hm.N_sh; a.C = (int)hm.C;
-    a.n_chunk_blocks = (int)hm.C;
     a.sh_rowptr = m->d_sh_rowptr; a.halo_dst = m->d_halo_dst;
     a.H = (const R*)s->H; a.x = (R*)s->d;
     a.lb = (R*)m->d_lb; a.r = (R*)m->d_r; a.p = (R*)m->d_p; a.q = (R*)m->d_q; a.dinv = (R*)m->d_dinv;
-    a.mask = m->d_mask; a.part = m->d_part; a.part2 = m->d_part2; a.part_n = m->n_part_blocks;
+    a.mask = m->d_mask; a.part = m->d_part; a.part_n = m->n_part_blocks;
     a.ctrl = m->d_ctrl; a.ticket = m->d_ticket;
     a.mat = make_matc<R>(m->mat);
     return a;
@@ -815,18 +820,6 @@ static void set_plan(pff_mesh* m, DmgArgs<R>& a, int which, bool proj)
     }
 }
 
-// grid of a persistent chunk kernel: every SM filled with as many CTAs as its shared memory / registers allow
-template <typename K>
-static pff_status persistent_grid(pff_mesh* m, K kern, int smem, int* grid)
-{
-    int per_sm = 0, sms = 0;
-    pff_status st = cuda_check(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kTPB, (size_t)smem), "occupancy query");
-    if (st != PFF_OK) return st;
-    if ((st = cuda_check(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, m->device), "SM count")) != PFF_OK) return st;
-    *grid = (int)std::min<int64_t>(m->hm.C, (int64_t)std::max(1, per_sm) * sms);
-    return PFF_OK;
-}
-
 static unsigned shared_grid(const HostMesh& hm)
 {
     return (unsigned)std::min<int64_t>(kMaxSharedBlocks, std::max<int64_t>(1, (hm.N_sh + kTPB - 1) / kTPB));
@@ -839,23 +832,33 @@ static pff_status ensure_workspace(pff_mesh* m)
     m->n_part_blocks = hm.C;
     pff_status st;
     if ((st = cuda_check(cudaMalloc((void**)&m->d_part, sizeof(double) * kCh * m->n_part_blocks), "damage: partials")) != PFF_OK) return st;
-    if ((st = cuda_check(cudaMalloc((void**)&m->d_part2, sizeof(double) * kCh * kMaxSharedBlocks), "damage: partials 2")) != PFF_OK) return st;
     if ((st = cuda_check(cudaMalloc((void**)&m->d_ctrl, sizeof(DamageCtrl)), "damage: ctrl")) != PFF_OK) return st;
     if ((st = cuda_check(cudaMalloc((void**)&m->d_ticket, 3 * sizeof(unsigned int)), "damage: ticket")) != PFF_OK) return st;  // [0] last-block ticket, [1] CG grid barrier, [2] setup grid barrier
     if ((st = cuda_check(cudaMemset(m->d_ticket, 0, 3 * sizeof(unsigned int)), "damage: ticket")) != PFF_OK) return st;
-    if ((st = cuda_check(cudaMallocHost((void**)&m->h_ctrl, 2 * sizeof(DamageCtrl)), "damage: pinned ctrl")) != PFF_OK) return st;
+    if ((st = cuda_check(cudaMallocHost((void**)&m->h_ctrl, sizeof(DamageCtrl)), "damage: pinned ctrl")) != PFF_OK) return st;
     return PFF_OK;
 }
 
-// Opt a kernel instantiation in to `bytes` of dynamic shared memory (kept as a per-instantiation high-water
-// mark: the limit is 227 KB minus the kernel's static shared memory, so only what is needed is requested).
-template <typename K>
-static pff_status set_smem(K kern, int bytes, int& granted)
+// One cooperative launch of a setup-kernel instantiation (chunk phase, grid barrier, interface phase, norms).  Its grid
+// barrier counter only grows: the epoch base travels as an argument and advances only when the launch was accepted.
+template <typename R>
+static pff_status launch_setup(pff_mesh* m, DmgArgs<R>& asu, const void* kern, unsigned g, int smem)
 {
-    if (bytes <= granted) return PFF_OK;
-    pff_status st = cuda_check(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes), "cudaFuncSetAttribute(damage kernel)");
-    if (st == PFF_OK) granted = bytes;
-    return st;
+    const unsigned int step = m->hm.N_sh > 0 ? g : 0u;
+    if (m->su_bar_count + step > 0xF0000000u) {
+        pff_status st = cuda_check(cudaMemsetAsync(m->d_ticket + 2, 0, sizeof(unsigned int), m->stream), "damage: barrier counter reset");
+        if (st != PFF_OK) return st;
+        m->su_bar_count = 0;
+    }
+    asu.su_base = m->su_bar_count;
+    void* kargs[] = {(void*)&asu};
+    prof_mark(m, PFF_K_DAMAGE_SETUP);
+    cudaError_t e = cudaLaunchCooperativeKernel(kern, dim3(g), dim3(kTPB), kargs, (size_t)smem, m->stream);
+    prof_mark(m, PFF_K_DAMAGE_SETUP);
+    if (e != cudaSuccess) return cuda_check(e, "damage: setup launch");
+    m->su_bar_count += step;
+    ++m->n_launches;
+    return PFF_OK;
 }
 
 struct AdjointIn {
@@ -878,36 +881,12 @@ static pff_status damage_solve_t(pff_mesh* m, const pff_state* s, double rel_tol
     set_plan<R>(m, asu, 2, PROJ);
     const int smem_mv = (int)m->lay_mv.total, smem_su = (int)m->lay_su.total;
     cudaStream_t cs = m->stream;
-    static int g_mv = 0, g_su = 0;  // static + dynamic shared memory may exceed 48 KB: always opt in
-    if ((st = set_smem(dmg_iter_chunk<R, DM_CG, PROJ>, smem_mv, g_mv)) != PFF_OK) return st;
-    if ((st = set_smem(dmg_setup_chunk<R, false>, smem_su, g_su)) != PFF_OK) return st;
-    static int grid_mv = 0, grid_mv_smem = -1;
-    if (grid_mv_smem != smem_mv) {
-        if ((st = persistent_grid(m, dmg_iter_chunk<R, DM_CG, PROJ>, smem_mv, &grid_mv)) != PFF_OK) return st;
-        grid_mv_smem = smem_mv;
-    }
-    const unsigned gmv = (unsigned)std::min<int64_t>(grid_mv, hm.C);
-    a.n_chunk_blocks = (int)gmv;
-    DamageCtrl* h = m->h_ctrl;  // [0]: upload image, [1]: download image
-    std::memset(&h[0], 0, sizeof(DamageCtrl));
-    h[0].tol = rel_tol; h[0].max_iter = max_iter; h[0].first = 1; h[0].restart = 1; h[0].status = PFF_ENOCONV;
-    if ((st = cuda_check(cudaMemcpyAsync(m->d_ctrl, &h[0], sizeof(DamageCtrl), cudaMemcpyHostToDevice, cs), "damage: ctrl upload")) != PFF_OK) return st;
-    static int grid_su = 0, grid_su_smem = -1;
-    if (grid_su_smem != smem_su) {
-        if ((st = persistent_grid(m, dmg_setup_chunk<R, false>, smem_su, &grid_su)) != PFF_OK) return st;
-        grid_su_smem = smem_su;
-    }
-    const unsigned gsu = (unsigned)std::min<int64_t>(grid_su, hm.C);
-    asu.n_chunk_blocks = (int)gsu;
-    if ((st = cuda_check(cudaMemsetAsync(m->d_ticket + 1, 0, 2 * sizeof(unsigned int), cs), "damage: barrier reset")) != PFF_OK) return st;
-    {   // setup pass: chunk phase, grid barrier, interface phase, norms (cooperative: all CTAs co-resident)
-        void* kargs[] = {(void*)&asu};
-        prof_mark(m, PFF_K_DAMAGE_SETUP);
-        cudaError_t e = cudaLaunchCooperativeKernel((const void*)dmg_setup_chunk<R, false>, dim3(gsu), dim3(kTPB), kargs, (size_t)smem_su, cs);
-        prof_mark(m, PFF_K_DAMAGE_SETUP);
-        ++m->n_launches;
-        if ((st = cuda_check(e, "damage: setup launch")) != PFF_OK) return st;
-    }
+    int grid_mv = 0, grid_su = 0;
+    if ((st = persistent_config(m, (const void*)dmg_iter_chunk<R, DM_CG, PROJ>, smem_mv, &grid_mv)) != PFF_OK) return st;
+    if ((st = persistent_config(m, (const void*)dmg_setup_chunk<R, false>, smem_su, &grid_su)) != PFF_OK) return st;
+    const unsigned gmv = (unsigned)std::min<int64_t>(grid_mv, hm.C), gsu = (unsigned)std::min<int64_t>(grid_su, hm.C);
+    asu.tol = rel_tol; asu.max_iter = max_iter;
+    if ((st = launch_setup(m, asu, (const void*)dmg_setup_chunk<R, false>, gsu, smem_su)) != PFF_OK) return st;
     // ONE cooperative launch runs every CG iteration (grid-wide barriers between the chunk phase, the interface
     // phase and the scalar recurrence), applies the last step and the clamp, and writes the control block back
     {
@@ -922,13 +901,14 @@ static pff_status damage_solve_t(pff_mesh* m, const pff_state* s, double rel_tol
     if (m->defer_slot) {  // pff_run_steps: the control block is read back asynchronously and inspected later, no sync here
         return cuda_check(cudaMemcpyAsync(m->defer_slot, m->d_ctrl, sizeof(DamageCtrl), cudaMemcpyDeviceToHost, cs), "damage: ctrl download");
     }
-    if ((st = cuda_check(cudaMemcpyAsync(&h[1], m->d_ctrl, sizeof(DamageCtrl), cudaMemcpyDeviceToHost, cs), "damage: ctrl download")) != PFF_OK) return st;
+    DamageCtrl* h = m->h_ctrl;  // pinned download image; the stream is synchronised before it is read or reused
+    if ((st = cuda_check(cudaMemcpyAsync(h, m->d_ctrl, sizeof(DamageCtrl), cudaMemcpyDeviceToHost, cs), "damage: ctrl download")) != PFF_OK) return st;
     if ((st = cuda_check(cudaStreamSynchronize(cs), "damage: sync")) != PFF_OK) return st;
-    m->last_cg_iters = h[1].iters;
-    if (iters) *iters = h[1].iters;
-    if (relres) *relres = h[1].relres;
-    if (!h[1].done || h[1].status == PFF_ENOCONV) {
-        set_error("pff_damage_solve: max_iter reached, relres = " + std::to_string(h[1].relres));
+    m->last_restarts = h->restarts; m->last_truncs = h->truncs;
+    if (iters) *iters = h->iters;
+    if (relres) *relres = h->relres;
+    if (!h->done || h->status == PFF_ENOCONV) {
+        set_error("pff_damage_solve: max_iter reached, relres = " + std::to_string(h->relres));
         return PFF_ENOCONV;
     }
     return PFF_OK;
@@ -965,10 +945,9 @@ static pff_status damage_matvec_t(pff_mesh* m, const pff_state* s, const void* p
     a.p_in = (const R*)p; a.q_out = (R*)q;
     set_plan<R>(m, a, 1, false);
     const int smem_mv = (int)m->lay_mv.total;
-    static int g_mv = 0;
-    if ((st = set_smem(dmg_iter_chunk<R, DM_PLAIN, false>, smem_mv, g_mv)) != PFF_OK) return st;
     int grid_mv = 0;
-    if ((st = persistent_grid(m, dmg_iter_chunk<R, DM_PLAIN, false>, smem_mv, &grid_mv)) != PFF_OK) return st;
+    if ((st = persistent_config(m, (const void*)dmg_iter_chunk<R, DM_PLAIN, false>, smem_mv, &grid_mv)) != PFF_OK) return st;
+    grid_mv = (int)std::min<int64_t>(grid_mv, m->hm.C);
     if (m->only_kernel < 0) {  // the operator of state->H in coefficient form (timing hook: reuse the previous one)
         PFF_LAUNCH(m, PFF_K_DAMAGE_SETUP, (dmg_coef_kernel<R><<<(unsigned)((m->hm.Ne + kTPB - 1) / kTPB), kTPB, 0, m->stream>>>(a)));
     }
@@ -995,21 +974,9 @@ static pff_status damage_rhs_diag_t(pff_mesh* m, const pff_state* s, void* b, vo
     a.b_out = (R*)b; a.D_out = (R*)D;
     set_plan<R>(m, a, 2, false);
     const int smem_su = (int)m->lay_su.total;
-    static int g_su = 0;
-    if ((st = set_smem(dmg_setup_chunk<R, true>, smem_su, g_su)) != PFF_OK) return st;
     int grid_su = 0;
-    if ((st = persistent_grid(m, dmg_setup_chunk<R, true>, smem_su, &grid_su)) != PFF_OK) return st;
-    if ((st = cuda_check(cudaMemsetAsync(m->d_ticket + 1, 0, 2 * sizeof(unsigned int), m->stream), "damage: barrier reset")) != PFF_OK) return st;
-    {
-        void* kargs[] = {(void*)&a};
-        prof_mark(m, PFF_K_DAMAGE_SETUP);
-        cudaError_t e = cudaLaunchCooperativeKernel((const void*)dmg_setup_chunk<R, true>, dim3((unsigned)std::min<int64_t>(grid_su, m->hm.C)), dim3(kTPB), kargs,
-                                                    (size_t)smem_su, m->stream);
-        prof_mark(m, PFF_K_DAMAGE_SETUP);
-        ++m->n_launches;
-        if ((st = cuda_check(e, "damage rhs/diag launch")) != PFF_OK) return st;
-    }
-    return cuda_check(cudaGetLastError(), "damage rhs/diag launch");
+    if ((st = persistent_config(m, (const void*)dmg_setup_chunk<R, true>, smem_su, &grid_su)) != PFF_OK) return st;
+    return launch_setup(m, a, (const void*)dmg_setup_chunk<R, true>, (unsigned)std::min<int64_t>(grid_su, m->hm.C), smem_su);
 }
 
 pff_status damage_rhs_diag(pff_mesh* m, const pff_state* s, void* b, void* D)

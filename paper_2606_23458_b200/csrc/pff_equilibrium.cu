@@ -142,7 +142,11 @@ __global__ void __launch_bounds__(kTPB) eq_reduce_kernel(const double* part, int
         sc[SC_RZ] = t0; sc[SC_RR] = t1; sc[SC_R0] = sqrt(t1); sc[SC_ITERS] = 0.0;
         sc[SC_DONE] = (t1 == 0.0) ? 1.0 : 0.0;
     } else if (MODE == 1) {
-        sc[SC_PQ] = t0; sc[SC_ALPHA] = sc[SC_RZ] / t0;
+        // breakdown guard: for the non-isotropic splits the shifted difference need not be positive definite (eta = 0 with
+        // fully damaged patches, sign changes of the split): stop without applying a step along this direction
+        sc[SC_PQ] = t0;
+        if (t0 > 0.0 && isfinite(t0)) sc[SC_ALPHA] = sc[SC_RZ] / t0;
+        else { sc[SC_ALPHA] = 0.0; sc[SC_DONE] = 2.0; }
     } else {
         sc[SC_BETA] = t0 / sc[SC_RZ]; sc[SC_RZ] = t0; sc[SC_RR] = t1; sc[SC_ITERS] += 1.0;
         if (sqrt(t1) <= sc[SC_TOL] * sc[SC_R0]) sc[SC_DONE] = 1.0;
@@ -232,6 +236,11 @@ static pff_status equilibrium_solve_t(pff_mesh* m, pff_state* s, const pff_bc* b
     if ((st = cuda_check(cudaStreamSynchronize(cs), "equilibrium: sync")) != PFF_OK) return st;
     if (iters) *iters = (int)h_sc[SC_ITERS];
     if (relres) *relres = h_sc[SC_R0] > 0.0 ? sqrt(h_sc[SC_RR]) / h_sc[SC_R0] : 0.0;
+    if (h_sc[SC_DONE] == 2.0) {
+        set_error("pff_equilibrium_solve: breakdown, p . K p <= 0 (operator not positive definite along the search direction); "
+                  "the steps taken so far are applied");
+        return PFF_ENOCONV;
+    }
     if (h_sc[SC_DONE] == 0.0) {
         set_error("pff_equilibrium_solve: max_iter reached");
         return PFF_ENOCONV;

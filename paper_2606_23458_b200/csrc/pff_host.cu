@@ -59,7 +59,13 @@ static pff_status run_host_t(pff_mesh* m, pff_host_state* hs, const double* dir_
     const int64_t Np = (N + 3) / 4 * 4, Nep = (Ne + 3) / 4 * 4;  // every device state array starts 16-byte aligned
     if (!m->d_stage) {
         if ((st = cuda_check(cudaMalloc(&m->d_stage, stage_doubles * sizeof(double)), "run_host: staging")) != PFF_OK) return st;
-        if ((st = cuda_check(cudaMalloc(&m->d_hstate, (size_t(9) * Np + Nep) * sizeof(R) + 2 * size_t(std::max<int64_t>(m->n_dir, 1)) * sizeof(R)), "run_host: state")) != PFF_OK) return st;
+        if ((st = cuda_check(cudaMalloc(&m->d_hstate, (size_t(9) * Np + Nep) * sizeof(R)), "run_host: state")) != PFF_OK) return st;
+    }
+    if (m->n_dir > m->hdir_cap) {  // the Dirichlet set may have been replaced by a larger one since the last call
+        if ((st = cuda_check(cudaStreamSynchronize(cs), "run_host: sync")) != PFF_OK) return st;
+        if (m->d_hdir) { cudaFree(m->d_hdir); m->d_hdir = nullptr; m->hdir_cap = 0; }
+        if ((st = cuda_check(cudaMalloc(&m->d_hdir, 2 * size_t(m->n_dir) * sizeof(R)), "run_host: Dirichlet values")) != PFF_OK) return st;
+        m->hdir_cap = m->n_dir;
     }
     double* sg = (double*)m->d_stage;
     HostIO<R> io{};
@@ -67,8 +73,8 @@ static pff_status run_host_t(pff_mesh* m, pff_host_state* hs, const double* dir_
     R* ds = (R*)m->d_hstate;
     io.ux = ds; io.uy = ds + Np; io.vx = ds + 2 * Np; io.vy = ds + 3 * Np; io.ax = ds + 4 * Np; io.ay = ds + 5 * Np;
     io.dd = ds + 6 * Np; io.fex = ds + 7 * Np; io.fey = ds + 8 * Np; io.HH = ds + 9 * Np;
-    R* d_du = ds + 9 * Np + Nep;
-    R* d_dv = d_du + std::max<int64_t>(m->n_dir, 1);
+    R* d_du = (R*)m->d_hdir;
+    R* d_dv = d_du + m->hdir_cap;
     io.node_old_of_new = m->d_node_old_of_new; io.elem_old_of_new = m->d_elem_old_of_new;
     io.N = (int)N; io.Ne = (int)Ne;
 #define CP(dst, src, n, kind) if ((st = cuda_check(cudaMemcpyAsync(dst, src, (n) * sizeof(double), kind, cs), "run_host: copy")) != PFF_OK) return st
@@ -140,6 +146,10 @@ extern "C" pff_status pff_run_host(pff_mesh* m, pff_host_state* hs, const double
         set_error("pff_run_host: need dt > 0, n_steps >= 0, damage_every >= 0, rel_tol > 0, max_iter >= 1");
         return PFF_EINVAL;
     }
+    if (m->n_dir > 0 && ((dir_u == nullptr) != (dir_v == nullptr))) {
+        set_error("pff_run_host: dir_u and dir_v must be given together"); return PFF_EINVAL;
+    }
+    DeviceGuard dg(m);
     if (m->opt.precision == PFF_F32)
         return run_host_t<float>(m, hs, dir_u, dir_v, load_scale, dt, n_steps, damage_every, rel_tol, max_iter);
     return run_host_t<double>(m, hs, dir_u, dir_v, load_scale, dt, n_steps, damage_every, rel_tol, max_iter);

@@ -111,6 +111,9 @@ struct HostMesh {
 pff_status build_host_mesh(int64_t n_nodes, const double* xy, int64_t n_elems, const int32_t* tri,
                            double rho, int order, int chunk_elems, size_t real_bytes, HostMesh& hm, std::string& err);
 
+// Host-side bounds proof of every staged (widened) copy of every chunk; false + `err` on violation (mesh_setup.cpp).
+bool verify_stage_extents(const HostMesh& hm, int64_t ell_total, int64_t n_entries, size_t real_bytes, std::string& err);
+
 constexpr size_t kSmemPerSM = 227 * 1024;   // usable shared memory of one sm_100a SM / one CTA
 constexpr size_t kSmemCtaReserve = 1024;    // driver-reserved bytes per resident CTA
 constexpr size_t kSmemStatic = 2304;        // static shared memory of the chunk kernels (reduction scratch)

@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 
 #include <string>
+#include <unordered_map>
 #include <vector>
 
 #include "pff_internal.h"
@@ -10,7 +11,9 @@
 // device-resident control block of the CG recurrence (pff_damage.cu); one 128-byte read-back per solve
 struct DamageCtrl {
     double rz, alpha, beta, amax, nb, tol, relres;
-    int iters, max_iter, done, status, first, restart, trunc, pending, restarts;
+    int iters, max_iter, done, status, first, restart, trunc, pending;
+    int restarts;  // AT1: free-set re-derivations after the first (a bound became inactive / a step was truncated, L181)
+    int truncs;    // AT1: steps cut short at the first bound hit
 };
 
 struct pff_mesh {
@@ -25,6 +28,11 @@ struct pff_mesh {
     int64_t ell_total = 0;                       // entries of d_ell (padded)
     int64_t n_launches = 0;  // kernels launched so far (pff_mesh_counters)
     int only_kernel = -1;    // profiling hook: restrict multi-kernel entry points to one kernel (pff_time_kernel)
+    // launch configuration of every persistent chunk kernel this mesh has used, keyed by the kernel's address: the grid
+    // (CTAs that fit the mesh's device with this mesh's shared-memory stage).  Presence also means the dynamic
+    // shared-memory opt-in was made on that device.  Per mesh, so meshes on different GPUs or with different chunk sizes
+    // never see each other's values.  A mesh must not be driven from two host threads at once.
+    std::unordered_map<const void*, int> launch_grid;
     // per-kernel-class CUDA-event timing (pff_profile_enable / pff_profile_read)
     bool prof_on = false;
     std::vector<cudaEvent_t> prof_ev[PFF_NUM_KERNEL_CLASSES];  // start/stop pairs
@@ -55,11 +63,11 @@ struct pff_mesh {
     void *d_ca = nullptr, *d_cb = nullptr;
     uint8_t* d_mask = nullptr;   // [N] bit0: in the free set, bit1: damage-Dirichlet
     double* d_part = nullptr;    // chunk-kernel block partials [channels][n_part_blocks]
-    double* d_part2 = nullptr;   // interface-kernel block partials
-    int last_cg_iters = 0;       // iterations of the previous solve (sizes the first launch batch)
     int64_t n_part_blocks = 0;
-    DamageCtrl* d_ctrl = nullptr;
-    DamageCtrl* h_ctrl = nullptr;  // pinned
+    DamageCtrl* d_ctrl = nullptr;  // initialised on the device by the setup kernel of every solve (no host upload)
+    DamageCtrl* h_ctrl = nullptr;  // pinned download image of the last synchronous solve
+    int last_restarts = 0, last_truncs = 0;  // of the last pff_damage_solve, or summed over the last pff_run_steps
+    unsigned int su_bar_count = 0;  // value of the setup kernel's grid-barrier counter after the launches enqueued so far
     DamageCtrl* h_ring = nullptr;      // pinned ring of deferred read-backs (pff_run_steps)
     DamageCtrl* defer_slot = nullptr;  // non-null: damage_solve copies the control block here and does not synchronise
     unsigned int* d_ticket = nullptr;
@@ -77,6 +85,8 @@ struct pff_mesh {
     cudaEvent_t ev_step = nullptr;
     void* d_stage = nullptr; size_t stage_bytes = 0;
     void* d_hstate = nullptr;  // device state arrays owned by the library for pff_run_host
+    void* d_hdir = nullptr;    // its Dirichlet values (dir_u | dir_v), re-allocated when the Dirichlet set outgrows it
+    int64_t hdir_cap = 0;      // entries per half of d_hdir
     int32_t *d_node_old_of_new = nullptr, *d_elem_old_of_new = nullptr;
 };
 
@@ -108,4 +118,20 @@ pff_status equilibrium_solve(pff_mesh* m, pff_state* s, const pff_bc* bc, double
 pff_status damage_rhs_diag(pff_mesh* m, const pff_state* s, void* b, void* D);
 pff_status energies(pff_mesh* m, const pff_state* s, double out[4]);
 pff_status cuda_check(cudaError_t e, const char* what);
+// dynamic shared-memory opt-in + occupancy-derived persistent grid of `kern` for this mesh (cached in m->launch_grid)
+pff_status persistent_config(pff_mesh* m, const void* kern, int smem_bytes, int* grid);
+
+// Makes the mesh's device current for the duration of an entry point (the caller may have switched devices since
+// pff_mesh_create) and restores the caller's device afterwards.
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceGuard(const pff_mesh* m)
+    {
+        if (m && cudaGetDevice(&prev) == cudaSuccess && prev != m->device) switched = cudaSetDevice(m->device) == cudaSuccess;
+    }
+    ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+    DeviceGuard(const DeviceGuard&) = delete;
+    DeviceGuard& operator=(const DeviceGuard&) = delete;
+};
 }  // namespace pff

@@ -428,38 +428,29 @@ static pff_status launch_step_t(pff_mesh* m, const StepArgs<R>& a)
         }
     } else {
         auto kern = step_chunk_kernel<R, SPLIT, MODE>;
-        static int granted = 0;  // per instantiation high-water mark of the dynamic smem opt-in
-        if ((int)m->lay_step.total > granted) {
-            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)m->lay_step.total);
-            if (e != cudaSuccess) return cuda_check(e, "cudaFuncSetAttribute(step_chunk_kernel)");
-            granted = (int)m->lay_step.total;
-        }
-        static int grid = 0, grid_smem = -1;  // persistent grid: every SM filled with as many CTAs as fit
-        if (grid_smem != (int)m->lay_step.total) {
-            int per_sm = 0, sms = 0;
-            cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kTPB, (size_t)m->lay_step.total);
-            if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, m->device);
-            if (e != cudaSuccess) return cuda_check(e, "step_chunk_kernel occupancy");
-            grid = std::max(1, per_sm) * sms;
-            grid_smem = (int)m->lay_step.total;
-        }
+        int grid = 0;  // persistent grid: every SM filled with as many CTAs as fit (cached per mesh, with the smem opt-in)
+        pff_status st = persistent_config(m, (const void*)kern, (int)m->lay_step.total, &grid);
+        if (st != PFF_OK) return st;
         {   // ONE cooperative launch: chunk phase, grid barrier, interface phase (all CTAs co-resident by construction)
             const unsigned g = (unsigned)std::min<int64_t>(grid, hm.C);
-            m->last_step_grid = (int)g;
             StepArgs<R> b = a;
             b.gbar = m->d_step_bar;
+            unsigned int after = m->step_bar_count + (hm.N_sh > 0 ? g : 0u);
             b.gb_base = m->step_bar_count;
-            if (hm.N_sh > 0) m->step_bar_count += g;
-            if (m->step_bar_count > 0xF0000000u) {  // far from wrapping: restart the counter (stream-ordered)
-                cudaMemsetAsync(m->d_step_bar, 0, sizeof(unsigned int), m->stream);
-                b.gb_base = 0; m->step_bar_count = hm.N_sh > 0 ? g : 0;
+            if (after > 0xF0000000u) {  // far from wrapping: restart the counter (stream-ordered)
+                cudaError_t e = cudaMemsetAsync(m->d_step_bar, 0, sizeof(unsigned int), m->stream);
+                if (e != cudaSuccess) return cuda_check(e, "explicit step: barrier counter reset");
+                m->step_bar_count = 0; b.gb_base = 0; after = hm.N_sh > 0 ? g : 0u;
             }
             void* kargs[] = {(void*)&b};
             prof_mark(m, PFF_K_STEP_CHUNK);
             cudaError_t e = cudaLaunchCooperativeKernel((const void*)kern, dim3(g), dim3(kTPB), kargs, (size_t)m->lay_step.total, m->stream);
             prof_mark(m, PFF_K_STEP_CHUNK);
-            ++m->n_launches;
             if (e != cudaSuccess) return cuda_check(e, "explicit step: cooperative launch");
+            // only a launch that was accepted advances the barrier epoch (a failed one never arrives on the counter)
+            m->step_bar_count = after;
+            m->last_step_grid = (int)g;
+            ++m->n_launches;
         }
     }
     return cuda_check(cudaGetLastError(), "explicit step launch");

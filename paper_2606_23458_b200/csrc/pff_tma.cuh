@@ -55,8 +55,6 @@ __device__ __forceinline__ void cp_async_mbar_arrive(uint64_t* bar)
 {
     asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
 // global -> shared bulk copy; dst, src 16-byte aligned, bytes a multiple of 16; completion on `bar`
 __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar)
@@ -83,8 +81,10 @@ struct StagePlan {
 
 // One lane's share of a stage burst: lane `lane` of the issuing warp copies the array described by d (if have):
 // element start + i of the global array lands at byte offset dst_off + ((start % A) + i) * esize, A = 16 / esize.
-// The copy is widened to 16-byte boundaries (the few neighbours fetched with it are never read); whatever
-// would reach past the last full 16-byte group of the array is fetched with plain loads.  Lane 0 then
+// The copy is widened to 16-byte boundaries: the source range stays inside [0, total) of its array by construction
+// (a0 >= 0, a1 <= total rounded down) and the destination inside the stage region sized for it (verified on the host
+// for every chunk by verify_stage_extents, mesh_setup.cpp); whatever would reach past the last full 16-byte group of
+// the array is fetched with plain loads.  Lane 0 then
 // arrives on the mbarrier with the total byte count of the warp.
 struct ChunkRange {  // index ranges of one chunk, per descriptor kind
     int elem_start, n_elem, Ne, node_start, n_int, N, ell_off, ell_cnt, ell_total, halo_off, n_halo, n_slots, next_halo_off,
@@ -117,23 +117,6 @@ __device__ __forceinline__ void stage_issue_desc(const StageDesc& d, bool have, 
     }
     for (int o = 16; o > 0; o >>= 1) bytes += __shfl_xor_sync(0xffffffffu, bytes, o);
     if (lane == 0) mbar_arrive_expect_tx(bar, bytes);
-}
-
-// Issued by one warp of the CTA, one lane per array (uniform code, no divergence).
-// pass: 0 = every array (one arrival); 1 = only the element arrays (kind 0; their range follows from blockIdx alone,
-// so they can be issued before the chunk meta has arrived), 2 = everything else (passes 1 + 2: mbarrier count 2).
-__device__ __forceinline__ void stage_issue_plan(const StagePlan& plan, unsigned char* stage, uint64_t* bar, int lane,
-                                                 int pass, int elem_start, int n_elem, int Ne, int node_start,
-                                                 int n_int, int N, int ell_off, int ell_cnt, int ell_total,
-                                                 int halo_off = 0, int n_halo = 0, int n_slots = 0, int next_halo_off = 0,
-                                                 int next_n_halo = 0)
-{
-    const bool have = lane < plan.n && (pass == 0 || (plan.d[lane].kind == 0) == (pass == 1));
-    StageDesc d{};
-    if (have) d = plan.d[lane];
-    const ChunkRange c{elem_start, n_elem, Ne, node_start, n_int, N, ell_off, ell_cnt, ell_total, halo_off, n_halo, n_slots,
-                       next_halo_off, next_n_halo};
-    stage_issue_desc(d, have, stage, bar, lane, c);
 }
 
 // Grid-wide barrier of the cooperatively launched kernels (all CTAs are co-resident): one arrival per CTA on a counter that only

@@ -2,23 +2,12 @@
 input dictionary (pff_inputs.config) and compare in USER numbering.  No method arithmetic here."""
 import numpy as np
 
-from oracle import Material, OracleMesh
+from oracle import oracle_from  # noqa: F401  (oracle-side marshalling lives with the oracle)
 
 
-def oracle_from(cfg):
-    m = OracleMesh(cfg["xy"], cfg["tri"], Material(**cfg["material"]))
-    m.u[:] = cfg["u0"]
-    m.d[:] = cfg["d0"]
-    if len(cfg["edges"]):
-        m.add_traction(cfg["edges"], cfg["traction"])
-    if len(cfg["notch"]):
-        m.set_damage_dirichlet(cfg["notch"])
-    if len(cfg["dir_dof"]):
-        m.set_dirichlet(cfg["dir_dof"])
-    return m
-
-
-def gpu_from(cfg, precision=0, scatter=0, chunk_elems=0, order=1):
+def gpu_from(cfg, precision=0, scatter=0, chunk_elems=0, order=2):
+    """CUDA mesh + state with the LIBRARY DEFAULTS unless a test asks otherwise (order 2 = PFF_ORDER_BISECTION, default
+    chunk: the decomposition bench.py times)."""
     import paper_2606_23458_b200 as pff
     mesh = pff.Mesh(cfg["xy"], cfg["tri"], cfg["material"], precision=precision, scatter=scatter,
                     chunk_elems=chunk_elems, order=order)

@@ -14,6 +14,7 @@ from _harness import gpu_fields, gpu_from, oracle_from, relmax
 pytestmark = pytest.mark.gpu
 
 TOL64, TOL32 = 1e-11, 2e-5
+BENCH_DECOMPOSITION = (5209, 148932)  # chunks, interface nodes of cfg5_1001 with the library defaults (bench.py's run)
 
 
 def _random_cfg(n_side, seed, **mat):
@@ -128,10 +129,43 @@ def test_damage_solve_parity(model):
     rc, it, rr = orc.damage_solve(rel_tol=1e-13, max_iter=4000)
     stt, it_g, rr_g = mesh.pff_damage_solve(st, rel_tol=1e-13, max_iter=4000)
     assert rc == 0 and stt == 0
+    restarts, truncs = mesh.pff_damage_last_stats()
+    if model == 2:  # AT2 never restarts (unconstrained solve, clamp afterwards); AT1 restarts are asserted in
+        assert restarts == 0 and truncs == 0  # test_at1_profile_closed_form_and_restarts / test_many_chunks...
     d = mesh.nodes_to_user(st.d)
     assert orc.d.max() == 1.0 and np.any((orc.d > 1e-3) & (orc.d < 1.0))
     assert relmax(d, orc.d) <= TOL64
     assert np.all(d >= cfg["d0"]) and d.max() <= 1.0 and d.min() >= 0.0
+
+
+@pytest.mark.parametrize("precision", [0, 1])
+def test_at1_profile_closed_form_and_restarts(precision):
+    """1-D AT1 profile: H = 0, d = 1 on the line x = 0, lower bound 0 elsewhere.  The solution
+    d = <1 - x/(2 l0)>_+^2 has compact support and is nodally exact when 2 l0 / h is an integer, so the GPU result is
+    compared with the closed form AND with the oracle.  From the start d = 0 only the first column of nodes is free; the
+    support grows column by column as frozen nodes with positive residual are released: the restart branch of the
+    projected solver (L181) MUST run, and it is asserted that it did."""
+    l0, h = 1.0, 0.25
+    nx, ny = int(6 / h) + 1, 40
+    xy, tri = grid_mesh(nx, ny, 6.0, (ny - 1) * h)
+    left = (np.arange(ny) * nx).astype(np.int32)
+    d0 = np.zeros(len(xy))
+    d0[left] = 1.0
+    cfg = dict(xy=xy, tri=tri, material=dict(GLASS, model=1, split=1, plane=0, Gc=1.0, l0=l0), notch=left,
+               edges=np.zeros((0, 2), np.int32), traction=np.zeros((0, 2)), dir_dof=np.zeros(0, np.int32),
+               d0=d0, u0=np.zeros((len(xy), 2)))
+    orc = oracle_from(cfg)
+    assert orc.damage_solve(rel_tol=1e-13, max_iter=5000)[0] == 0
+    mesh, st = gpu_from(cfg, precision=precision, chunk_elems=64)
+    tol = 1e-13 if precision == 0 else 1e-6
+    stt, it, rr = mesh.pff_damage_solve(st, rel_tol=tol, max_iter=5000)
+    restarts, truncs = mesh.pff_damage_last_stats()
+    assert stt == 0 and restarts >= 3, (restarts, truncs, it)
+    d = mesh.nodes_to_user(st.d)
+    exact = np.maximum(1 - xy[:, 0] / (2 * l0), 0) ** 2
+    bound = 1e-11 if precision == 0 else TOL32
+    assert np.abs(d - exact).max() <= bound and relmax(d, orc.d) <= bound
+    assert np.all(d[xy[:, 0] >= 2 * l0] == 0)  # compact support: bound-constrained nodes sit exactly on the bound
 
 
 @pytest.mark.parametrize("model,split,plane", [(2, 2, 0), (1, 3, 1), (2, 1, 0)])
@@ -233,13 +267,14 @@ def test_run_host_matches_device_path():
 
 
 def test_full_size_bench_configuration_cfg5_1001():
-    """BASELINE's metric size (1e6 nodes, 2e6 elements) in the launch configuration bench.py times (default
-    options: Morton order, default chunk, gather scatter, fp64): two staggered steps, every node and element
-    compared with the oracle (it finishes this size in seconds)."""
+    """BASELINE's metric size (1e6 nodes, 2e6 elements) in the launch configuration bench.py times (library
+    defaults: PFF_ORDER_BISECTION, default chunk, gather scatter, fp64 -- the decomposition printed in the bench line's
+    `config`): two staggered steps, every node and element compared with the oracle (it finishes this size in seconds)."""
     cfg = config(5, n=1001)
     orc = oracle_from(cfg)
     mesh, st = gpu_from(cfg)
     assert mesh.n_nodes == 1002001 and mesh.n_elems == 2000000
+    assert (mesh.n_chunks, mesh.n_shared) == BENCH_DECOMPOSITION  # what BENCH_r*.json config.chunks / interface_nodes print
     dt = cfg["dt_factor"] * orc.dt_crit()
     orc.init_accel()
     mesh.pff_init_accel(st, mesh.bc())
@@ -285,6 +320,9 @@ def test_many_chunks_per_cta_big_halos_and_overflow_slots(model):
     st.H.copy_(mesh.elems_to_internal(orc.H))
     stt, _, _ = mesh.pff_damage_solve(st, rel_tol=1e-12, max_iter=4000)
     assert rc == 0 and stt == 0
+    restarts, truncs = mesh.pff_damage_last_stats()
+    if model == 1:  # random lower bounds up to 0.9: steps are truncated at bounds and the free set is re-derived
+        assert truncs > 0 and restarts > 0, (restarts, truncs)
     assert relmax(mesh.nodes_to_user(st.d), o2.d) <= 1e-10
 
 
@@ -396,8 +434,12 @@ def test_second_solve_with_unchanged_history_needs_no_iteration():
 
 def test_full_size_fp32_variant_cfg5_1001():
     """The fp32 variant at BASELINE's metric size, in the configuration bench.py --precision f32 times: two staggered
-    steps against the fp64 oracle at the north_star fp32 tolerance (2e-5 max-norm relative); the damage solve is run
-    to 1e-6 (fp32 residuals stagnate below that) and compared at a tolerance that covers it."""
+    steps against the fp64 oracle.  north_star's fp32 tolerance is 2e-5 max-norm relative.  At this size (h = 1e-3,
+    |u| ~ 1e-4 L) it is met by u, H and d; the acceleration is a difference quotient of fp32-STORED displacements and
+    carries eps32 * max|u| / (h * max|strain|) ~ 6e-5 of representation error whatever the arithmetic (DESIGN.md
+    section 7), so a, and v which integrates it, are held to 1e-4 here: a documented miss of the 2e-5 target that the
+    bench line of --precision f32 runs repeats (`fp32_note`).  The damage solve runs to a tolerance fp32 reaches
+    (1e-5 relative residual, no allow_noconv: fp32 residuals stagnate near 1e-6)."""
     cfg = config(5, n=1001)
     orc = oracle_from(cfg)
     mesh, st = gpu_from(cfg, precision=1)
@@ -408,12 +450,106 @@ def test_full_size_fp32_variant_cfg5_1001():
         orc.explicit_step(dt)
         rc, _, _ = orc.damage_solve(rel_tol=1e-10, max_iter=4000)
         mesh.pff_explicit_step(st, mesh.bc(), dt)
-        stt, _, rr = mesh.pff_damage_solve(st, rel_tol=1e-6, max_iter=4000, allow_noconv=True)
-        assert rc == 0 and rr <= 1e-5
+        stt, _, rr = mesh.pff_damage_solve(st, rel_tol=1e-5, max_iter=4000)
+        assert rc == 0 and stt == 0 and rr <= 1e-5
     u, v, a, d, H = gpu_fields(mesh, st)
-    # u, H (and d below) meet the north_star fp32 tolerance.  The acceleration is a difference quotient of the fp32
-    # displacements: its rounding error grows with the mesh, eps32 * max|u| / (h * max|strain|) ~ 6e-8 * 1e-5 / (1e-3 * 1e-5)
-    # ~ 6e-5 at h = 1e-3 (fp32 variant), so a and v (which integrates a) are held to 1e-4 here.
-    assert relmax(u, orc.u) <= TOL32 and relmax(H, orc.H) <= TOL32
-    assert relmax(v, orc.v) <= 1e-4 and relmax(a, orc.a) <= 1e-4
-    assert relmax(d, orc.d) <= 1e-4
+    assert relmax(u, orc.u) <= TOL32 and relmax(H, orc.H) <= TOL32 and relmax(d, orc.d) <= TOL32
+    assert relmax(v, orc.v) <= 1e-4 and relmax(a, orc.a) <= 1e-4  # see the docstring: storage-format bound, not met at 2e-5
+
+
+def _trajectory(cfg, n_steps, S=1.0, shear=False, tip_width=None, **gpu_kw):
+    """n_steps staggered steps on both sides (solves converged to 1e-12 so that d is the unique minimiser, R13),
+    then north_star's trajectory criteria: energies within 1e-6 relative, crack tip within one element width."""
+    orc = oracle_from(cfg)
+    mesh, st = gpu_from(cfg, **gpu_kw)
+    dt = cfg["dt_factor"] * orc.dt_crit()
+    orc.init_accel(S)
+    mesh.pff_init_accel(st, mesh.bc(load_scale=S))
+    restarts = truncs = iters = 0
+    for k in range(1, n_steps + 1):
+        du, dv = shear_bc(cfg, k, dt) if shear else (None, None)
+        orc.explicit_step(dt, S=S, dir_u=du, dir_v=dv)
+        rc, _, _ = orc.damage_solve(rel_tol=1e-12, max_iter=4000)
+        mesh.pff_explicit_step(st, mesh.bc(du, dv, load_scale=S), dt)
+        stt, it, _ = mesh.pff_damage_solve(st, rel_tol=1e-12, max_iter=4000)
+        assert rc == 0 and stt == 0, k
+        r, t = mesh.pff_damage_last_stats()
+        restarts, truncs, iters = restarts + r, truncs + t, iters + it
+    e_ref, e = orc.energies(), mesh.pff_energies(st)
+    assert np.all(np.abs(e - e_ref) <= 1e-6 * np.abs(e_ref).max()), (e, e_ref)
+    u, v, a, d, H = gpu_fields(mesh, st)
+    assert relmax(u, orc.u) <= 1e-7 and relmax(H, orc.H) <= 1e-7 and relmax(d, orc.d) <= 1e-7
+    assert np.all(d >= cfg["d0"]) and d.max() <= 1.0 and d.min() >= 0.0
+    # the d >= 0.5 front ("crack"): every node of either side's front within one element width of the other side's
+    from scipy.spatial import cKDTree
+    fa, fb = cfg["xy"][d >= 0.5], cfg["xy"][orc.d >= 0.5]
+    assert (len(fa) > 0) == (len(fb) > 0)
+    if len(fb):
+        assert cKDTree(fb).query(fa)[0].max() <= tip_width + 1e-12 and cKDTree(fa).query(fb)[0].max() <= tip_width + 1e-12
+    return mesh, orc, d, dict(restarts=restarts, truncs=truncs, iters=iters)
+
+
+def test_trajectory_500_steps_config3_many_chunks_per_cta():
+    """north_star's trajectory criterion at its stated length (500 steps; config 3 is a 500-step config): AT1 projected CG,
+    star-convex split, plane stress, sheared top edge, at half scale (501^2 nodes, 500,000 elements) in chunks of 32
+    elements along plain Morton ranges: 15,625 chunks = 35 per CTA of the CG kernel and 53 per CTA of the step kernel
+    (several epochs of the 32-entry chunk-meta ring), ragged chunks with interface overflow slots, over a whole trajectory."""
+    cfg = config(3, scale=0.5)
+    mesh, orc, d, stats = _trajectory(cfg, 500, shear=True, tip_width=1.0 / 500, chunk_elems=32, order=1)
+    assert mesh.n_chunks == 15625 and mesh.n_chunks > 32 * 444
+    assert orc.H.max() > 3 * cfg["material"]["Gc"] / (16 * cfg["material"]["l0"])  # the AT1 threshold was crossed: damage grew
+    assert (d > cfg["d0"] + 1e-6).sum() > 0 and stats["restarts"] > 0, stats
+
+
+def test_trajectory_500_steps_config2_full_size():
+    """500 staggered steps of config 2 at BASELINE's full size (401 x 161 nodes, 128,000 elements, jittered nodes,
+    permuted elements, spectral split, AT2) with the library defaults."""
+    cfg = config(2)
+    mesh, orc, d, stats = _trajectory(cfg, 500, S=8.0, tip_width=0.100 / 400 * 1.2)
+    assert mesh.n_elems == 128000 and stats["iters"] > 500
+
+
+def test_two_meshes_alternating_and_grown_dirichlet_set():
+    """Library state is per mesh: two meshes with different chunk sizes (different shared-memory opt-ins and persistent
+    grids) stepped alternately give the same results as each alone; a Dirichlet set replaced by a larger one between two
+    pff_run_host calls is honoured (the value buffers are re-allocated)."""
+    cfg = config(1, scale=0.5)
+    ref = []
+    for chunk in (64, 0):
+        mesh, st = gpu_from(cfg, chunk_elems=chunk)
+        mesh.pff_init_accel(st, mesh.bc(load_scale=8.0))
+        for _ in range(6):
+            mesh.pff_explicit_step(st, mesh.bc(load_scale=8.0), 0.5 * mesh.dt_crit)
+            mesh.pff_damage_solve(st, rel_tol=1e-10)
+        ref.append([x.copy() for x in gpu_fields(mesh, st)])
+    pair = [gpu_from(cfg, chunk_elems=chunk) for chunk in (64, 0)]
+    for mesh, st in pair:
+        mesh.pff_init_accel(st, mesh.bc(load_scale=8.0))
+    for _ in range(6):
+        for mesh, st in pair:
+            mesh.pff_explicit_step(st, mesh.bc(load_scale=8.0), 0.5 * mesh.dt_crit)
+            mesh.pff_damage_solve(st, rel_tol=1e-10)
+    for (mesh, st), r in zip(pair, ref):
+        for a, b in zip(gpu_fields(mesh, st), r):
+            assert np.array_equal(a, b)
+    # grow the Dirichlet set between two host-path calls
+    mesh, st = pair[1]
+    orc = oracle_from(cfg)
+    dt = 0.5 * orc.dt_crit()
+    nx = int(round(100 * 0.5)) + 1
+    for n_fixed in (3, nx):  # first 3 bottom nodes clamped, then the whole bottom edge
+        dofs = np.concatenate([2 * np.arange(n_fixed), 2 * np.arange(n_fixed) + 1]).astype(np.int32)
+        mesh.pff_set_dirichlet(dofs)
+        orc.set_dirichlet(dofs)
+        u, v, a = orc.u.copy(), orc.v.copy(), orc.a.copy()
+        dd, H, fext = orc.d.copy(), orc.H.copy(), orc.fext.copy()
+        zeros = np.zeros(len(dofs))
+        mesh.pff_run_host(u, v, a, dd, H, fext, dt, 3, damage_every=1, rel_tol=1e-12, dir_u=zeros, dir_v=zeros)
+        for _ in range(3):
+            orc.explicit_step(dt, dir_u=zeros, dir_v=zeros)
+            assert orc.damage_solve(rel_tol=1e-12)[0] == 0
+        assert relmax(u, orc.u) <= 1e-10 and relmax(a, orc.a) <= 1e-10 and relmax(dd, orc.d) <= 1e-10
+    with pytest.raises(Exception):  # exactly one of dir_u / dir_v with a Dirichlet set installed: PFF_EINVAL
+        b = mesh.bc()
+        b.dir_u = st.ux.data_ptr()
+        mesh.pff_explicit_step(st, b, dt)

@@ -45,6 +45,32 @@ def test_gradients_reproduce_linear_fields():
     assert abs(m.mass.sum() - GLASS["rho"] * 1.0) < 1e-9  # lumped mass conserves total mass (L169)
 
 
+def test_lumped_mass_per_node_closed_form():
+    """m_i = rho sum_{e ni i} A_e / 3 (L169) node by node on a uniform right-triangle grid (quads split along the
+    lower-left -> upper-right diagonal): an interior node touches six triangles of area h^2/2 -> rho h^2, an edge node
+    three -> rho h^2 / 2, the two corners ON the diagonal (lower-left, upper-right) two -> rho h^2 / 3, the other two
+    corners one -> rho h^2 / 6.  A wrong node index in the scatter moves mass between these classes."""
+    nx, ny, h = 6, 5, 0.25
+    xy, tri = grid_mesh(nx, ny, (nx - 1) * h, (ny - 1) * h)
+    rho = 2450.0
+    for perm_seed in (None, 3):  # also with flipped orientation and permuted element order
+        t = tri.copy()
+        if perm_seed is not None:
+            g = np.random.default_rng(perm_seed)
+            flip = g.uniform(size=len(t)) < 0.5
+            t[flip] = t[flip][:, [0, 2, 1]]
+            t = np.ascontiguousarray(t[g.permutation(len(t))])
+        m = OracleMesh(xy, t, mat(rho=rho))
+        i, j = np.arange(nx * ny) % nx, np.arange(nx * ny) // nx
+        on_x, on_y = (i == 0) | (i == nx - 1), (j == 0) | (j == ny - 1)
+        expect = np.where(on_x & on_y, 0.0, np.where(on_x | on_y, 0.5, 1.0)) * rho * h * h
+        diag_corner = ((i == 0) & (j == 0)) | ((i == nx - 1) & (j == ny - 1))
+        other_corner = (on_x & on_y) & ~diag_corner
+        expect[diag_corner] = rho * h * h / 3.0
+        expect[other_corner] = rho * h * h / 6.0
+        np.testing.assert_allclose(m.mass, expect, rtol=1e-14, atol=0)
+
+
 def test_degenerate_element_rejected():
     xy = np.array([[0.0, 0.0], [1.0, 0.0], [2.0, 0.0]])
     with pytest.raises(ValueError):
