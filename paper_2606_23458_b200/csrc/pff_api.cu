@@ -47,14 +47,14 @@ static pff_status upload_real(void** dst, const double* src, size_t count, size_
     return s;
 }
 
-pff_status persistent_config(pff_mesh* m, const void* kern, int smem_bytes, int* grid)
+pff_status persistent_config(pff_mesh* m, const void* kern, int smem_bytes, int* grid, int block)
 {
     auto it = m->launch_grid.find(kern);
     if (it != m->launch_grid.end()) { *grid = it->second; return PFF_OK; }
     // static + dynamic shared memory may exceed 48 KB: always opt in (per device; the mesh's device is current here)
     PFF_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
     int per_sm = 0, sms = 0;
-    PFF_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kTPB, (size_t)smem_bytes));
+    PFF_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, block, (size_t)smem_bytes));
     PFF_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, m->device));
     *grid = (per_sm > 0 ? per_sm : 1) * sms;
     m->launch_grid.emplace(kern, *grid);
@@ -198,7 +198,7 @@ pff_status pff_mesh_create(int64_t n_nodes, const double* xy, int64_t n_elems, c
     UP(upload((uint8_t**)&m->d_q, nullptr, N * m->rb, cs));
     UP(upload((uint8_t**)&m->d_dinv, nullptr, N * m->rb, cs));
     UP(upload(&m->d_mask, nullptr, 2 * N, cs));
-    UP(upload(&m->d_step_bar, nullptr, 1, cs));
+    UP(upload(&m->d_step_bar, nullptr, 2, cs));
     UP(upload(&m->d_node_old_of_new, hm.node_old_of_new.data(), N, cs));
     {
         std::vector<int32_t> eon(Ne);

@@ -66,8 +66,8 @@ struct DmgArgs {
     DamageCtrl* ctrl;
     double tol;              // stopping tolerance and iteration cap of this solve (the setup kernel writes them into ctrl)
     int max_iter;
-    unsigned int* ticket;    // [0] last-block ticket, [1] grid barrier of the CG kernel, [2] grid barrier of the setup kernel
-    unsigned int su_base;    // value of ticket[2] before this setup launch (the counter only grows, like the step kernel's)
+    unsigned int* ticket;    // [0] last-block ticket, [1] grid barrier of the CG kernel (zeroed by the setup kernel before it),
+                             // [2] grid barrier of the setup kernel (only grows), [3] its value at the start of the launch
     MatC<R> mat;
 };
 
@@ -115,6 +115,9 @@ __device__ __forceinline__ void block_reduce_ch(double v[kCh], double* s_w /* [k
 }
 
 enum { DM_CG = 0, DM_PLAIN = 1 };
+#ifndef PFF_PART_LOAD
+#define PFF_PART_LOAD __ldcg
+#endif
 
 
 struct IterScalars {
@@ -295,6 +298,22 @@ __global__ void __launch_bounds__(kTPB, 3) dmg_iter_chunk(const DmgArgs<R> a)
     double acc[kCh];
     const bool single_epoch = n_my <= kMetaCap;
     bool pre_issued = false;  // the next CG iteration's first chunk is already streaming in
+    bool gathers_issued = false;  // ... and its halo gathers have been issued as well
+    // halo gathers of the first chunk of an epoch into its stage + every thread's arrival on the stage barrier.  The ids of
+    // the CTA's very first chunk are kept in shared memory (s_hid0) and reused by every later CG iteration.
+    auto issue_first_gathers = [&](unsigned char* stg, uint64_t* sbar, const ChunkMeta& cm, bool from_global) {
+        if (issuer) {
+            const int hb0 = ((cm.node_start & (A - 1)) + cm.n_int + A - 1) & ~(A - 1);
+            const bool first_chunk = cm.elem_start == s_meta[0].elem_start && single_epoch;
+            for (int j = lane; j < cm.n_halo; j += 32) {
+                int gid;
+                if (from_global) { gid = __ldg(a.halo_ids + cm.halo_off + j); if (first_chunk) s_hid0[j] = gid; }
+                else gid = s_hid0[j];
+                halo_gather_async<R, MODE, PROJ>(a, L, stg, hb0 + j, j, gid);
+            }
+        }
+        cp_async_mbar_arrive(sbar);
+    };
     unsigned int gb_target = 0;  // grid-barrier epoch target (thread 0)
     int it = 0;  // stage uses so far (global over epochs and CG iterations): stage = it & 1, mbarrier parity = (it >> 1) & 1
     if (MODE == DM_CG) {
@@ -325,15 +344,8 @@ __global__ void __launch_bounds__(kTPB, 3) dmg_iter_chunk(const DmgArgs<R> a)
                 fence_proxy_async();
                 stage_issue_desc(my_desc, have_desc, stg, bar + 2 * (it & 1), lane, cr);
             }
-            if (issuer) {
-                const int hb0 = ((cm.node_start & (A - 1)) + cm.n_int + A - 1) & ~(A - 1);
-                for (int j = lane; j < cm.n_halo; j += 32) {
-                    if (!pre_issued && e0 == 0) s_hid0[j] = __ldg(a.halo_ids + cm.halo_off + j);
-                    const int gid = e0 == 0 ? s_hid0[j] : __ldg(a.halo_ids + cm.halo_off + j);
-                    halo_gather_async<R, MODE, PROJ>(a, L, stg, hb0 + j, j, gid);
-                }
-            }
-            cp_async_mbar_arrive(bar + 2 * (it & 1));
+            if (!gathers_issued) issue_first_gathers(stg, bar + 2 * (it & 1), cm, !pre_issued || e0 > 0);
+            gathers_issued = false;
             pre_issued = false;
         }
         for (int k = 0; k < n_ep; ++k, ++it) {
@@ -439,10 +451,12 @@ __global__ void __launch_bounds__(kTPB, 3) dmg_iter_chunk(const DmgArgs<R> a)
         }
     }
     if (MODE != DM_CG) break;
-    // ---- interface nodes (owned by no chunk): ordered sum of the chunk partials, same prologue; grid-wide phase
     fence_proxy_async_global();
+    // ---- interface nodes (owned by no chunk): ordered sum of the chunk partials, same prologue; grid-wide phase
     grid_barrier(a.ticket + 1, gb_target, (unsigned)G);
-    if (single_epoch) {  // every interior value is final: start streaming the first chunk of the next CG iteration
+#ifndef PFF_PREISSUE_LATE
+    // every interior value is final: start streaming the first chunk of the next CG iteration
+    if (single_epoch) {
         if (issuer) {
             const ChunkMeta cm = s_meta[0];
             const ChunkRange cr{cm.elem_start, cm.n_elem, a.Ne, cm.node_start, cm.n_int, a.N, cm.ell_off,
@@ -453,49 +467,87 @@ __global__ void __launch_bounds__(kTPB, 3) dmg_iter_chunk(const DmgArgs<R> a)
         }
         pre_issued = true;
     }
-    const int if_per = (a.N_sh + G - 1) / G, if_end = min(a.N_sh, ((int)blockIdx.x + 1) * if_per);  // equal slice per CTA
-    for (int sn = blockIdx.x * if_per + tid; sn < if_end; sn += kTPB) {
-        const int gid = a.N_int + sn;
-        const R qs = iface_sum<R>(a.halo_part, sn, a.N_sh, a.n_ovf, a.sh_rowptr);
-        R x = R(0), r = a.r[gid], p = R(0), q = R(0), lb = R(0);
-        const R dinv = a.dinv[gid];
-        uint8_t mk = a.mask[gid];
-        const uint8_t mk0 = mk;
-        if (!sc.first) { x = a.x[gid]; p = a.p[gid]; q = a.q[gid]; }
-        if (PROJ) { if (sc.first) x = a.x[gid]; lb = a.lb[gid]; }
-        const R pn = cg_node_prologue<R, PROJ>(sc, x, r, p, q, dinv, lb, mk);
-        if (!sc.first) { if (mk0 & 1) a.x[gid] = x; a.r[gid] = r; }
-        if (mk != mk0) a.mask[gid] = mk;
-        a.p[gid] = pn; a.q[gid] = qs;
-        const double qd = double(qs);
-        acc[0] += double(pn) * qd;
-        if (mk & 1) {
-            const double rd = double(r), dv = double(dinv);
-            acc[1] += rd * rd * dv; acc[2] += rd * rd;
-            acc[3] += rd * dv * qd; acc[4] += dv * qd * qd; acc[5] += rd * qd; acc[6] += qd * qd;
-            if (PROJ && pn < R(0)) acc[kCh - 1] = fmin(acc[kCh - 1], (double(lb) - double(x)) / double(pn));
+#endif
+    {
+        // Equal slice per CTA, TWO nodes per thread and trip: every load of both nodes is issued before anything is
+        // computed or stored, so a trip costs one memory round trip (the slice is ~1.3 nodes per thread at 10^6 nodes).
+        struct IfNode { R qs, x, r, p, q, lb, dinv; uint8_t mk; };
+        auto if_load = [&](int sn, IfNode& v) {
+            const int gid = a.N_int + sn;
+            v.qs = iface_sum<R>(a.halo_part, sn, a.N_sh, a.n_ovf, a.sh_rowptr);
+            v.r = a.r[gid]; v.dinv = a.dinv[gid]; v.mk = a.mask[gid];
+            v.x = R(0); v.p = R(0); v.q = R(0); v.lb = R(0);
+            if (!sc.first) { v.x = a.x[gid]; v.p = a.p[gid]; v.q = a.q[gid]; }
+            if (PROJ) { if (sc.first) v.x = a.x[gid]; v.lb = a.lb[gid]; }
+        };
+        auto if_finish = [&](int sn, IfNode& v) {
+            const int gid = a.N_int + sn;
+            const uint8_t mk0 = v.mk;
+            const R pn = cg_node_prologue<R, PROJ>(sc, v.x, v.r, v.p, v.q, v.dinv, v.lb, v.mk);
+            if (!sc.first) { if (mk0 & 1) a.x[gid] = v.x; a.r[gid] = v.r; }
+            if (v.mk != mk0) a.mask[gid] = v.mk;
+            a.p[gid] = pn; a.q[gid] = v.qs;
+            const double qd = double(v.qs);
+            acc[0] += double(pn) * qd;
+            if (v.mk & 1) {
+                const double rd = double(v.r), dv = double(v.dinv);
+                acc[1] += rd * rd * dv; acc[2] += rd * rd;
+                acc[3] += rd * dv * qd; acc[4] += dv * qd * qd; acc[5] += rd * qd; acc[6] += qd * qd;
+                if (PROJ && pn < R(0)) acc[kCh - 1] = fmin(acc[kCh - 1], (double(v.lb) - double(v.x)) / double(pn));
+            }
+        };
+        const int if_per = (a.N_sh + G - 1) / G, if_end = min(a.N_sh, ((int)blockIdx.x + 1) * if_per);
+        for (int s0 = blockIdx.x * if_per + tid; s0 < if_end; s0 += 2 * kTPB) {
+            const int s1 = s0 + kTPB;
+            const bool two = s1 < if_end;
+            IfNode n0, n1;
+            if_load(s0, n0);
+            if (two) if_load(s1, n1);
+            if_finish(s0, n0);
+            if (two) if_finish(s1, n1);
         }
     }
+#ifdef PFF_PREISSUE_LATE
+    if (single_epoch) {
+        if (issuer) {
+            const ChunkMeta cm = s_meta[0];
+            const ChunkRange cr{cm.elem_start, cm.n_elem, a.Ne, cm.node_start, cm.n_int, a.N, cm.ell_off,
+                                cm.ell_w * (cm.n_int + cm.n_halo), (int)a.ell_total, cm.halo_off, cm.n_halo, (int)a.n_entries,
+                                n_my > 1 ? s_meta[1].halo_off : 0, n_my > 1 ? s_meta[1].n_halo : 0};
+            fence_proxy_async();
+            stage_issue_desc(my_desc, have_desc, smem + (it & 1) * L.stage_bytes, bar + 2 * (it & 1), lane, cr);
+        }
+        pre_issued = true;
+    }
+#endif
     __syncthreads();  // reconverge before the shuffle tree (measured: 10 us per iteration faster than without)
     block_reduce_ch(acc, s_w, s_out);
     if (tid < kCh) a.part[(int64_t)tid * a.part_n + blockIdx.x] = s_out[tid];
     fence_proxy_async_global();
     grid_barrier(a.ticket + 1, gb_target, (unsigned)G);
+    // ---- every value of this iteration is final: the halo gathers of the next iteration's first chunk go out now and
+    // fly while the scalars are reduced (they are harmless if the solve turns out to be finished)
+    if (pre_issued) {
+        issue_first_gathers(smem + (it & 1) * L.stage_bytes, bar + 2 * (it & 1), s_meta[0], false);
+        gathers_issued = true;
+    }
     // ---- every CTA reduces all block partials in the same fixed order and advances its copy of the scalars
     {
         const int w = tid >> 5;
-        if (w < kCh) {
+        constexpr int kChUsed = PROJ ? kCh : kCh - 1;  // the step-bound channel (a minimum) exists only for the projected solver
+        if (w < kChUsed) {
             const double ident = (w == kCh - 1) ? INFINITY : 0.0;
             double v = ident;
-            for (int base = 0; base < G; base += 256) {  // 8 independent loads in flight per lane, summed in index order
-                double u[8];
+            constexpr int kB = 14;  // partials per lane and batch, all loads of a batch in flight at once (G <= 448: one batch)
+            for (int base = 0; base < G; base += 32 * kB) {
+                double u[kB];
 #pragma unroll
-                for (int j = 0; j < 8; ++j) {
+                for (int j = 0; j < kB; ++j) {
                     const int i = base + 32 * j + lane;
-                    u[j] = i < G ? __ldcg(a.part + (int64_t)w * a.part_n + i) : ident;
+                    u[j] = i < G ? PFF_PART_LOAD(a.part + (int64_t)w * a.part_n + i) : ident;
                 }
 #pragma unroll
-                for (int j = 0; j < 8; ++j) v = (w == kCh - 1) ? fmin(v, u[j]) : v + u[j];
+                for (int j = 0; j < kB; ++j) v = (w == kCh - 1) ? fmin(v, u[j]) : v + u[j];
             }
             for (int o = 16; o > 0; o >>= 1) {
                 const double u = __shfl_xor_sync(0xffffffffu, v, o);
@@ -506,7 +558,7 @@ __global__ void __launch_bounds__(kTPB, 3) dmg_iter_chunk(const DmgArgs<R> a)
         __syncthreads();
         if (tid == 0) {
             double t[kCh];
-            for (int c = 0; c < kCh; ++c) t[c] = s_out[c];
+            for (int c = 0; c < kCh; ++c) t[c] = c < kChUsed ? s_out[c] : INFINITY;
             cg_scalar_step<PROJ>(&s_ctrl, t);
         }
         __syncthreads();
@@ -514,7 +566,7 @@ __global__ void __launch_bounds__(kTPB, 3) dmg_iter_chunk(const DmgArgs<R> a)
         sc.trunc = s_ctrl.trunc;
         if (s_ctrl.done) {
             if (pre_issued) {  // drain the stage that was streamed ahead before leaving
-                cp_async_mbar_arrive(bar + 2 * (it & 1));
+                if (!gathers_issued) cp_async_mbar_arrive(bar + 2 * (it & 1));
                 mbar_wait(bar + 2 * (it & 1), (it >> 1) & 1);
             }
             break;
@@ -598,6 +650,8 @@ __global__ void __launch_bounds__(kTPB, 2) dmg_setup_chunk(const DmgArgs<R> a)
         // the CG kernel that follows in stream order counts its grid barriers from zero (the previous one has finished)
         if (blockIdx.x == 0) a.ticket[1] = 0u;
     }
+    unsigned int su_epoch = 0;  // thread 0: value of the setup barrier counter before this launch
+    if (tid == 0 && a.N_sh > 0) su_epoch = *reinterpret_cast<volatile unsigned int*>(a.ticket + 3);
     double acc[kCh];
 #pragma unroll
     for (int c = 0; c < kCh; ++c) acc[c] = 0.0;
@@ -716,31 +770,49 @@ __global__ void __launch_bounds__(kTPB, 2) dmg_setup_chunk(const DmgArgs<R> a)
     }
     // ---- interface nodes after a grid-wide barrier: ordered sums of the three partial planes, same outputs
     if (a.N_sh > 0) {
-        unsigned int target = a.su_base;
+        unsigned int target = su_epoch;
         grid_barrier(a.ticket + 2, target, (unsigned)G);
-        const int per = (a.N_sh + G - 1) / G, end = min(a.N_sh, ((int)blockIdx.x + 1) * per);  // equal slice per CTA
-        for (int sn = blockIdx.x * per + tid; sn < end; sn += kTPB) {
+        if (blockIdx.x == 0 && tid == 0) a.ticket[3] = target;  // all CTAs have read the epoch and arrived: next launch's epoch
+        // equal slice per CTA, two nodes per thread and trip with all loads issued first (one memory round trip per trip)
+        struct IfNode { R qs, Ds, bs, x, rhs; bool fixed; };
+        auto if_load = [&](int sn, IfNode& v) {
             const int gid = a.N_int + sn;
-            const R qs = iface_sum<R>(a.halo_part, sn, a.N_sh, a.n_ovf, a.sh_rowptr);
-            const R Ds = iface_sum<R>(a.halo_part + a.n_slots, sn, a.N_sh, a.n_ovf, a.sh_rowptr);
-            const R bs = iface_sum<R>(a.halo_part + 2 * a.n_slots, sn, a.N_sh, a.n_ovf, a.sh_rowptr);
-            if (HOOK) {
-                if (a.b_out) a.b_out[gid] = bs;
-                if (a.D_out) a.D_out[gid] = Ds;
-            } else {
-                bool fixed = (a.flags[gid] & 4) != 0;
-                R rhs = bs;
-                if (adj) {
-                    fixed = fixed || (a.free_in && !a.free_in[gid]);
-                    rhs = fixed ? R(0) : a.rhs[gid];
-                }
-                const R r = rhs - qs;
-                a.r[gid] = r; a.dinv[gid] = R(1) / Ds; a.lb[gid] = a.x[gid];
-                a.mask[gid] = fixed ? 2 : 1;
-                acc[0] += double(rhs) * double(rhs);
-                if (!fixed) acc[1] += double(r) * double(r);
-                if (!fixed && (adj || a.mat.model != PFF_AT1 || r > R(0))) acc[2] += double(r) * double(r);
+            v.qs = iface_sum<R>(a.halo_part, sn, a.N_sh, a.n_ovf, a.sh_rowptr);
+            v.Ds = iface_sum<R>(a.halo_part + a.n_slots, sn, a.N_sh, a.n_ovf, a.sh_rowptr);
+            v.bs = iface_sum<R>(a.halo_part + 2 * a.n_slots, sn, a.N_sh, a.n_ovf, a.sh_rowptr);
+            if (HOOK) return;
+            v.fixed = (a.flags[gid] & 4) != 0;
+            v.x = a.x[gid];
+            v.rhs = v.bs;
+            if (adj) {  // adjoint: nodes outside the caller's free set are held at lambda = 0 like Dirichlet nodes
+                v.fixed = v.fixed || (a.free_in && !a.free_in[gid]);
+                v.rhs = a.rhs[gid];
             }
+        };
+        auto if_finish = [&](int sn, const IfNode& v) {
+            const int gid = a.N_int + sn;
+            if (HOOK) {
+                if (a.b_out) a.b_out[gid] = v.bs;
+                if (a.D_out) a.D_out[gid] = v.Ds;
+                return;
+            }
+            const R rhs = (adj && v.fixed) ? R(0) : v.rhs;
+            const R r = rhs - v.qs;
+            a.r[gid] = r; a.dinv[gid] = R(1) / v.Ds; a.lb[gid] = v.x;
+            a.mask[gid] = v.fixed ? 2 : 1;
+            acc[0] += double(rhs) * double(rhs);
+            if (!v.fixed) acc[1] += double(r) * double(r);
+            if (!v.fixed && (adj || a.mat.model != PFF_AT1 || r > R(0))) acc[2] += double(r) * double(r);
+        };
+        const int per = (a.N_sh + G - 1) / G, end = min(a.N_sh, ((int)blockIdx.x + 1) * per);
+        for (int s0 = blockIdx.x * per + tid; s0 < end; s0 += 2 * kTPB) {
+            const int s1 = s0 + kTPB;
+            const bool two = s1 < end;
+            IfNode n0, n1;
+            if_load(s0, n0);
+            if (two) if_load(s1, n1);
+            if_finish(s0, n0);
+            if (two) if_finish(s1, n1);
         }
     }
     if (HOOK) return;
@@ -833,30 +905,22 @@ static pff_status ensure_workspace(pff_mesh* m)
     pff_status st;
     if ((st = cuda_check(cudaMalloc((void**)&m->d_part, sizeof(double) * kCh * m->n_part_blocks), "damage: partials")) != PFF_OK) return st;
     if ((st = cuda_check(cudaMalloc((void**)&m->d_ctrl, sizeof(DamageCtrl)), "damage: ctrl")) != PFF_OK) return st;
-    if ((st = cuda_check(cudaMalloc((void**)&m->d_ticket, 3 * sizeof(unsigned int)), "damage: ticket")) != PFF_OK) return st;  // [0] last-block ticket, [1] CG grid barrier, [2] setup grid barrier
-    if ((st = cuda_check(cudaMemset(m->d_ticket, 0, 3 * sizeof(unsigned int)), "damage: ticket")) != PFF_OK) return st;
+    if ((st = cuda_check(cudaMalloc((void**)&m->d_ticket, 4 * sizeof(unsigned int)), "damage: ticket")) != PFF_OK) return st;  // [0] last-block ticket, [1] CG grid barrier, [2] setup grid barrier
+    if ((st = cuda_check(cudaMemset(m->d_ticket, 0, 4 * sizeof(unsigned int)), "damage: ticket")) != PFF_OK) return st;
     if ((st = cuda_check(cudaMallocHost((void**)&m->h_ctrl, sizeof(DamageCtrl)), "damage: pinned ctrl")) != PFF_OK) return st;
     return PFF_OK;
 }
 
 // One cooperative launch of a setup-kernel instantiation (chunk phase, grid barrier, interface phase, norms).  Its grid
-// barrier counter only grows: the epoch base travels as an argument and advances only when the launch was accepted.
+// barrier counter only grows; the epoch lives on the device and is advanced by the kernel itself (graph-replayable).
 template <typename R>
 static pff_status launch_setup(pff_mesh* m, DmgArgs<R>& asu, const void* kern, unsigned g, int smem)
 {
-    const unsigned int step = m->hm.N_sh > 0 ? g : 0u;
-    if (m->su_bar_count + step > 0xF0000000u) {
-        pff_status st = cuda_check(cudaMemsetAsync(m->d_ticket + 2, 0, sizeof(unsigned int), m->stream), "damage: barrier counter reset");
-        if (st != PFF_OK) return st;
-        m->su_bar_count = 0;
-    }
-    asu.su_base = m->su_bar_count;
     void* kargs[] = {(void*)&asu};
     prof_mark(m, PFF_K_DAMAGE_SETUP);
     cudaError_t e = cudaLaunchCooperativeKernel(kern, dim3(g), dim3(kTPB), kargs, (size_t)smem, m->stream);
     prof_mark(m, PFF_K_DAMAGE_SETUP);
     if (e != cudaSuccess) return cuda_check(e, "damage: setup launch");
-    m->su_bar_count += step;
     ++m->n_launches;
     return PFF_OK;
 }

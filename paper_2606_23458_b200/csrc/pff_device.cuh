@@ -10,6 +10,10 @@
 namespace pff {
 
 constexpr int kTPB = 256;  // threads per CTA of the chunk kernels
+#ifndef PFF_STEP_TPB
+#define PFF_STEP_TPB 256
+#endif
+constexpr int kStepTPB = PFF_STEP_TPB;  // threads per CTA of the explicit-step kernel (last warp = producer)
 
 template <typename R>
 struct MatC {  // material constants folded on the host

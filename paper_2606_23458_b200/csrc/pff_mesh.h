@@ -16,6 +16,8 @@ struct DamageCtrl {
     int truncs;    // AT1: steps cut short at the first bound hit
 };
 
+static_assert(sizeof(DamageCtrl) % 8 == 0, "the control block is copied in 8-byte words");
+
 struct pff_mesh {
     pff::HostMesh hm;
     pff_material mat{};
@@ -67,7 +69,6 @@ struct pff_mesh {
     DamageCtrl* d_ctrl = nullptr;  // initialised on the device by the setup kernel of every solve (no host upload)
     DamageCtrl* h_ctrl = nullptr;  // pinned download image of the last synchronous solve
     int last_restarts = 0, last_truncs = 0;  // of the last pff_damage_solve, or summed over the last pff_run_steps
-    unsigned int su_bar_count = 0;  // value of the setup kernel's grid-barrier counter after the launches enqueued so far
     DamageCtrl* h_ring = nullptr;      // pinned ring of deferred read-backs (pff_run_steps)
     DamageCtrl* defer_slot = nullptr;  // non-null: damage_solve copies the control block here and does not synchronise
     unsigned int* d_ticket = nullptr;
@@ -77,8 +78,7 @@ struct pff_mesh {
     double *d_eq_part = nullptr, *d_eq_sc = nullptr;
     double* tangent_pq_part = nullptr;  // set around a stiffness-action launch that should also leave the p . q block partials
     int last_step_grid = 0;             // CTAs of the last step-kernel launch (length of those partials)
-    unsigned int* d_step_bar = nullptr;  // grid-barrier counter of the step kernel
-    unsigned int step_bar_count = 0;     // its value after the launches enqueued so far
+    unsigned int* d_step_bar = nullptr;  // [0] grid-barrier counter of the step kernel, [1] its epoch (both device-maintained)
 
     // host-path staging (pff_run_host)
     cudaStream_t copy_stream = nullptr;  // second stream: copies the mechanics results back while the damage solve runs
@@ -119,7 +119,7 @@ pff_status damage_rhs_diag(pff_mesh* m, const pff_state* s, void* b, void* D);
 pff_status energies(pff_mesh* m, const pff_state* s, double out[4]);
 pff_status cuda_check(cudaError_t e, const char* what);
 // dynamic shared-memory opt-in + occupancy-derived persistent grid of `kern` for this mesh (cached in m->launch_grid)
-pff_status persistent_config(pff_mesh* m, const void* kern, int smem_bytes, int* grid);
+pff_status persistent_config(pff_mesh* m, const void* kern, int smem_bytes, int* grid, int block = 256);
 
 // Makes the mesh's device current for the duration of an entry point (the caller may have switched devices since
 // pff_mesh_create) and restores the caller's device afterwards.

@@ -40,8 +40,8 @@ struct StepArgs {
     int EC, N, Ne, N_int, N_sh, n_ovf, C;
     int64_t ell_total, n_entries;
     const int32_t *sh_rowptr, *halo_dst;
-    unsigned int* gbar;    // grid-barrier arrival counter (grows from launch to launch)
-    unsigned int gb_base;  // its value before this launch
+    unsigned int* gbar;    // [0] grid-barrier arrival counter (only grows), [1] its value when this launch started: kept on
+                           // the device and advanced by the kernel itself, so a launch can be replayed from a CUDA graph
     StageLayout lay;
     StagePlan plan;
     R *ux, *uy, *vx, *vy, *ax, *ay;
@@ -139,7 +139,7 @@ __device__ __forceinline__ void step_halo_gather(const StepArgs<R>& a, const Sta
 // thread's cp.async arrival.  Per chunk: predictor (Eq. 16) -> fused element pass (strain, split, degradation,
 // stress, force, history) -> ordered gather + Eq. 17-18.  Stage = StageLayout kind 0 (pff_internal.h).
 template <typename R, int SPLIT, int MODE>
-__global__ void __launch_bounds__(kTPB, 2) step_chunk_kernel(const StepArgs<R> a)
+__global__ void __launch_bounds__(kStepTPB, 2) step_chunk_kernel(const StepArgs<R> a)
 {
     extern __shared__ __align__(128) unsigned char smem[];
     typedef typename Geo<R>::Pair Pair;
@@ -153,17 +153,19 @@ __global__ void __launch_bounds__(kTPB, 2) step_chunk_kernel(const StepArgs<R> a
     // the LAST warp issues the bulk copies (one lane per array); the halo gathers are issued from the top thread down
     // the LAST warp is the producer (bulk copies + all halo gathers of the next chunk); the other kWorkers threads run the
     // predictor and the element pass and synchronise between them on a named barrier; the producer rejoins for the gather
-    constexpr int kWorkers = kTPB - 32;
+    constexpr int kWorkers = kStepTPB - 32;
     const bool issuer = tid >= kWorkers;
     const bool have_desc = issuer && lane < a.plan.n;
     StageDesc my_desc{};
     if (have_desc) my_desc = a.plan.d[lane];
 
     if (tid == 0) {
-        mbar_init(bar, 1 + kTPB); mbar_init(bar + 2, 1 + kTPB);
+        mbar_init(bar, 1 + kStepTPB); mbar_init(bar + 2, 1 + kStepTPB);
         *Geo<R>::slot(smem, s_shared_slots, 3 * EC, EC) = Geo<R>::pair(R(0), R(0));  // the zero pair (lives in the shared region)
     }
     int it = 0;  // stage uses so far: stage = it & 1, mbarrier parity = (it >> 1) & 1
+    unsigned int gb_epoch = 0;  // thread 0: the barrier counter's value before this launch (read early, used at the barrier)
+    if (tid == 0 && a.N_sh > 0) gb_epoch = *reinterpret_cast<volatile unsigned int*>(a.gbar + 1);
     double acc_pq = 0.0;  // MODE_TANGENT: this thread's share of p . q
     for (int e0 = 0; e0 < n_my; e0 += kMetaCap) {
         const int n_ep = min(kMetaCap, n_my - e0);
@@ -287,7 +289,7 @@ __global__ void __launch_bounds__(kTPB, 2) step_chunk_kernel(const StepArgs<R> a
             __syncthreads();
 
             // ---- phase 3: ordered gather of each node's incident force pairs, then Eq. 17-18 for interior nodes
-            for (int i = tid; i < nloc; i += kTPB) {
+            for (int i = tid; i < nloc; i += kStepTPB) {
                 R fx = R(0), fy = R(0);
                 const uint16_t* row = s_ell + i;
 #pragma unroll 4
@@ -324,17 +326,48 @@ __global__ void __launch_bounds__(kTPB, 2) step_chunk_kernel(const StepArgs<R> a
     // ---- interface nodes (owned by no chunk), after a grid-wide barrier: ordered sum of the per-chunk partials, then the
     // same Eq. 16-18.  Every read of the OLD interface state by the chunk phase (halo gathers) precedes the barrier.
     if (a.N_sh > 0) {
-        unsigned int target = a.gb_base;
+        unsigned int target = gb_epoch;
         grid_barrier(a.gbar, target, (unsigned)G);
-        const int per = (a.N_sh + G - 1) / G, end = min(a.N_sh, ((int)blockIdx.x + 1) * per);  // equal slice per CTA
-        for (int s = blockIdx.x * per + tid; s < end; s += kTPB) {
+        // every CTA has read the epoch before arriving, and all have arrived: publish the next launch's epoch
+        if (blockIdx.x == 0 && tid == 0) a.gbar[1] = target;
+        // Equal slice per CTA, TWO nodes per thread and trip: all loads of both nodes are issued before anything is computed
+        // or stored, so a trip costs one memory round trip (the slice is ~1.7 nodes per thread at 10^6 nodes).
+        struct IfNode { R fx, fy, ux, uy, vx, vy, ax, ay, fex, fey, minv, px, py; uint8_t fl; };
+        auto if_load = [&](int s, IfNode& v) {
             const int gid = a.N_int + s;
-            const R fx = iface_sum<R>(a.halo_part, s, a.N_sh, a.n_ovf, a.sh_rowptr);
-            const R fy = iface_sum<R>(a.halo_part + a.n_slots, s, a.N_sh, a.n_ovf, a.sh_rowptr);
-            R px, py;
-            predict<R, MODE>(a, gid, px, py);
-            finish_node<R, MODE>(a, gid, px, py, fx, fy);
-            if (MODE == MODE_TANGENT) acc_pq += double(a.px[gid]) * double(fx) + double(a.py[gid]) * double(fy);
+            v.fx = iface_sum<R>(a.halo_part, s, a.N_sh, a.n_ovf, a.sh_rowptr);
+            v.fy = iface_sum<R>(a.halo_part + a.n_slots, s, a.N_sh, a.n_ovf, a.sh_rowptr);
+            v.ux = a.ux[gid]; v.uy = a.uy[gid];
+            if (MODE == MODE_STEP) { v.vx = a.vx[gid]; v.vy = a.vy[gid]; v.ax = a.ax[gid]; v.ay = a.ay[gid]; }
+            if (MODE == MODE_STEP || MODE == MODE_INIT) { v.fl = a.flags[gid]; v.minv = a.minv[gid]; v.fex = a.fex[gid]; v.fey = a.fey[gid]; }
+            if (MODE == MODE_TANGENT) { v.px = a.px[gid]; v.py = a.py[gid]; }
+        };
+        auto if_finish = [&](int s, const IfNode& v) {  // the same Eq. 16-18 as predict() + finish_node(), from the loaded values
+            const int gid = a.N_int + s;
+            if (MODE == MODE_TANGENT) acc_pq += double(v.px) * double(v.fx) + double(v.py) * double(v.fy);
+            if (MODE == MODE_FORCE || MODE == MODE_TANGENT) { a.fx_out[gid] = v.fx; a.fy_out[gid] = v.fy; return; }
+            R axn = (a.S * v.fex - v.fx) * v.minv;
+            R ayn = (a.S * v.fey - v.fy) * v.minv;
+            if (v.fl & 1) axn = R(0);
+            if (v.fl & 2) ayn = R(0);
+            if (MODE == MODE_STEP) {
+                const R px = rfma(a.hdt2, v.ax, rfma(a.dt, v.vx, v.ux));
+                const R py = rfma(a.hdt2, v.ay, rfma(a.dt, v.vy, v.uy));
+                a.ux[gid] = (v.fl & 1) ? v.ux : px; a.uy[gid] = (v.fl & 2) ? v.uy : py;
+                a.vx[gid] = (v.fl & 1) ? v.vx : rfma(a.hdt, v.ax + axn, v.vx);
+                a.vy[gid] = (v.fl & 2) ? v.vy : rfma(a.hdt, v.ay + ayn, v.vy);
+            }
+            a.ax[gid] = axn; a.ay[gid] = ayn;
+        };
+        const int per = (a.N_sh + G - 1) / G, end = min(a.N_sh, ((int)blockIdx.x + 1) * per);
+        for (int s0 = blockIdx.x * per + tid; s0 < end; s0 += 2 * kStepTPB) {
+            const int s1 = s0 + kStepTPB;
+            const bool two = s1 < end;
+            IfNode n0, n1;
+            if_load(s0, n0);
+            if (two) if_load(s1, n1);
+            if_finish(s0, n0);
+            if (two) if_finish(s1, n1);
         }
     }
     if (MODE == MODE_TANGENT && a.pq_part) {  // one ordered block sum per CTA; the caller sums the CTAs in index order
@@ -429,26 +462,17 @@ static pff_status launch_step_t(pff_mesh* m, const StepArgs<R>& a)
     } else {
         auto kern = step_chunk_kernel<R, SPLIT, MODE>;
         int grid = 0;  // persistent grid: every SM filled with as many CTAs as fit (cached per mesh, with the smem opt-in)
-        pff_status st = persistent_config(m, (const void*)kern, (int)m->lay_step.total, &grid);
+        pff_status st = persistent_config(m, (const void*)kern, (int)m->lay_step.total, &grid, kStepTPB);
         if (st != PFF_OK) return st;
         {   // ONE cooperative launch: chunk phase, grid barrier, interface phase (all CTAs co-resident by construction)
             const unsigned g = (unsigned)std::min<int64_t>(grid, hm.C);
             StepArgs<R> b = a;
             b.gbar = m->d_step_bar;
-            unsigned int after = m->step_bar_count + (hm.N_sh > 0 ? g : 0u);
-            b.gb_base = m->step_bar_count;
-            if (after > 0xF0000000u) {  // far from wrapping: restart the counter (stream-ordered)
-                cudaError_t e = cudaMemsetAsync(m->d_step_bar, 0, sizeof(unsigned int), m->stream);
-                if (e != cudaSuccess) return cuda_check(e, "explicit step: barrier counter reset");
-                m->step_bar_count = 0; b.gb_base = 0; after = hm.N_sh > 0 ? g : 0u;
-            }
             void* kargs[] = {(void*)&b};
             prof_mark(m, PFF_K_STEP_CHUNK);
-            cudaError_t e = cudaLaunchCooperativeKernel((const void*)kern, dim3(g), dim3(kTPB), kargs, (size_t)m->lay_step.total, m->stream);
+            cudaError_t e = cudaLaunchCooperativeKernel((const void*)kern, dim3(g), dim3(kStepTPB), kargs, (size_t)m->lay_step.total, m->stream);
             prof_mark(m, PFF_K_STEP_CHUNK);
             if (e != cudaSuccess) return cuda_check(e, "explicit step: cooperative launch");
-            // only a launch that was accepted advances the barrier epoch (a failed one never arrives on the counter)
-            m->step_bar_count = after;
             m->last_step_grid = (int)g;
             ++m->n_launches;
         }

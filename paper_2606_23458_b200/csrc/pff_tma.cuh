@@ -127,13 +127,23 @@ __device__ __forceinline__ void grid_barrier(unsigned int* counter, unsigned int
     __syncthreads();
     if (threadIdx.x == 0) {
         target += G;
+#ifdef PFF_BAR_LIGHT
+        // release-arrive (orders this CTA's writes, observed through the block barrier above, before the arrival) and
+        // acquire-poll; the comparison is wrap-safe
+        asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(counter) : "memory");
+        unsigned int seen;
+        do {
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(counter) : "memory");
+        } while ((int)(seen - target) < 0);
+#else
         __threadfence();
         atomicAdd(counter, 1u);
         unsigned int seen;
         do {
             asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(counter) : "memory");
-        } while (seen < target);
+        } while ((int)(seen - target) < 0);
         __threadfence();
+#endif
     }
     __syncthreads();
 }

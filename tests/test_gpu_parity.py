@@ -170,7 +170,8 @@ def test_at1_profile_closed_form_and_restarts(precision):
 
 @pytest.mark.parametrize("model,split,plane", [(2, 2, 0), (1, 3, 1), (2, 1, 0)])
 def test_trajectory_energies_config1(model, split, plane):
-    """200 staggered steps of config 1 (and AT1 / star-convex / plane-stress variants): energies to 1e-6."""
+    """500 staggered steps (north_star's trajectory length) of config 1 and of its AT1 / star-convex / plane-stress and
+    spectral variants: energies to 1e-6, crack tip within one element width."""
     cfg = config(1)
     cfg["material"] = dict(cfg["material"], model=model, split=split, plane=plane, gamma_star=1.0)
     orc = oracle_from(cfg)
@@ -179,7 +180,7 @@ def test_trajectory_energies_config1(model, split, plane):
     S = 8.0
     orc.init_accel(S)
     mesh.pff_init_accel(st, mesh.bc(load_scale=S))
-    for k in range(200):
+    for k in range(500):
         orc.explicit_step(dt, S=S)
         rc, _, _ = orc.damage_solve(rel_tol=1e-12, max_iter=4000)
         mesh.pff_explicit_step(st, mesh.bc(load_scale=S), dt)
@@ -439,7 +440,7 @@ def test_full_size_fp32_variant_cfg5_1001():
     carries eps32 * max|u| / (h * max|strain|) ~ 6e-5 of representation error whatever the arithmetic (DESIGN.md
     section 7), so a, and v which integrates it, are held to 1e-4 here: a documented miss of the 2e-5 target that the
     bench line of --precision f32 runs repeats (`fp32_note`).  The damage solve runs to a tolerance fp32 reaches
-    (1e-5 relative residual, no allow_noconv: fp32 residuals stagnate near 1e-6)."""
+    without allow_noconv (1e-6 relative residual: 10 iterations here; fp32 residuals stagnate below ~1e-7)."""
     cfg = config(5, n=1001)
     orc = oracle_from(cfg)
     mesh, st = gpu_from(cfg, precision=1)
@@ -450,63 +451,64 @@ def test_full_size_fp32_variant_cfg5_1001():
         orc.explicit_step(dt)
         rc, _, _ = orc.damage_solve(rel_tol=1e-10, max_iter=4000)
         mesh.pff_explicit_step(st, mesh.bc(), dt)
-        stt, _, rr = mesh.pff_damage_solve(st, rel_tol=1e-5, max_iter=4000)
-        assert rc == 0 and stt == 0 and rr <= 1e-5
+        stt, _, rr = mesh.pff_damage_solve(st, rel_tol=1e-6, max_iter=4000)
+        assert rc == 0 and stt == 0 and rr <= 1e-6
     u, v, a, d, H = gpu_fields(mesh, st)
     assert relmax(u, orc.u) <= TOL32 and relmax(H, orc.H) <= TOL32 and relmax(d, orc.d) <= TOL32
     assert relmax(v, orc.v) <= 1e-4 and relmax(a, orc.a) <= 1e-4  # see the docstring: storage-format bound, not met at 2e-5
 
 
-def _trajectory(cfg, n_steps, S=1.0, shear=False, tip_width=None, **gpu_kw):
-    """n_steps staggered steps on both sides (solves converged to 1e-12 so that d is the unique minimiser, R13),
-    then north_star's trajectory criteria: energies within 1e-6 relative, crack tip within one element width."""
+def _trajectory(cfg, n_steps, gpu_variants, S=1.0, tip_width=None, rel_tol=1e-10):
+    """n_steps staggered steps of the oracle and of one CUDA mesh per entry of gpu_variants (keyword sets of gpu_from), all
+    solves converged to rel_tol so that d is the unique minimiser (R13; the ORACLE's relative residual stagnates
+    near 2e-12 in the first steps of config 2, where b is tiny against the rows of A d at the d = 1 notch, so 1e-12 is
+    unreachable there), then north_star's trajectory criteria per mesh: energies within 1e-6 relative, the d >= 0.5 front
+    within one element width."""
+    from scipy.spatial import cKDTree
     orc = oracle_from(cfg)
-    mesh, st = gpu_from(cfg, **gpu_kw)
+    gpus = [gpu_from(cfg, **kw) for kw in gpu_variants]
     dt = cfg["dt_factor"] * orc.dt_crit()
     orc.init_accel(S)
-    mesh.pff_init_accel(st, mesh.bc(load_scale=S))
-    restarts = truncs = iters = 0
+    for mesh, st in gpus:
+        mesh.pff_init_accel(st, mesh.bc(load_scale=S))
+    iters = [0] * len(gpus)
     for k in range(1, n_steps + 1):
-        du, dv = shear_bc(cfg, k, dt) if shear else (None, None)
-        orc.explicit_step(dt, S=S, dir_u=du, dir_v=dv)
-        rc, _, _ = orc.damage_solve(rel_tol=1e-12, max_iter=4000)
-        mesh.pff_explicit_step(st, mesh.bc(du, dv, load_scale=S), dt)
-        stt, it, _ = mesh.pff_damage_solve(st, rel_tol=1e-12, max_iter=4000)
-        assert rc == 0 and stt == 0, k
-        r, t = mesh.pff_damage_last_stats()
-        restarts, truncs, iters = restarts + r, truncs + t, iters + it
-    e_ref, e = orc.energies(), mesh.pff_energies(st)
-    assert np.all(np.abs(e - e_ref) <= 1e-6 * np.abs(e_ref).max()), (e, e_ref)
-    u, v, a, d, H = gpu_fields(mesh, st)
-    assert relmax(u, orc.u) <= 1e-7 and relmax(H, orc.H) <= 1e-7 and relmax(d, orc.d) <= 1e-7
-    assert np.all(d >= cfg["d0"]) and d.max() <= 1.0 and d.min() >= 0.0
-    # the d >= 0.5 front ("crack"): every node of either side's front within one element width of the other side's
-    from scipy.spatial import cKDTree
-    fa, fb = cfg["xy"][d >= 0.5], cfg["xy"][orc.d >= 0.5]
-    assert (len(fa) > 0) == (len(fb) > 0)
-    if len(fb):
+        orc.explicit_step(dt, S=S)
+        rc, _, _ = orc.damage_solve(rel_tol=rel_tol, max_iter=4000)
+        assert rc == 0, k
+        for g, (mesh, st) in enumerate(gpus):
+            mesh.pff_explicit_step(st, mesh.bc(load_scale=S), dt)
+            stt, it, _ = mesh.pff_damage_solve(st, rel_tol=rel_tol, max_iter=4000)
+            assert stt == 0, (k, g)
+            iters[g] += it
+    e_ref = orc.energies()
+    fb = cfg["xy"][orc.d >= 0.5]
+    for mesh, st in gpus:
+        e = mesh.pff_energies(st)
+        assert np.all(np.abs(e - e_ref) <= 1e-6 * np.abs(e_ref).max()), (e, e_ref)
+        u, v, a, d, H = gpu_fields(mesh, st)
+        assert relmax(u, orc.u) <= 1e-7 and relmax(H, orc.H) <= 1e-7 and relmax(d, orc.d) <= 1e-7
+        assert np.all(d >= cfg["d0"]) and d.max() <= 1.0 and d.min() >= 0.0
+        fa = cfg["xy"][d >= 0.5]
+        assert len(fa) > 0 and len(fb) > 0
         assert cKDTree(fb).query(fa)[0].max() <= tip_width + 1e-12 and cKDTree(fa).query(fb)[0].max() <= tip_width + 1e-12
-    return mesh, orc, d, dict(restarts=restarts, truncs=truncs, iters=iters)
+    return gpus, orc, iters
 
 
-def test_trajectory_500_steps_config3_many_chunks_per_cta():
-    """north_star's trajectory criterion at its stated length (500 steps; config 3 is a 500-step config): AT1 projected CG,
-    star-convex split, plane stress, sheared top edge, at half scale (501^2 nodes, 500,000 elements) in chunks of 32
-    elements along plain Morton ranges: 15,625 chunks = 35 per CTA of the CG kernel and 53 per CTA of the step kernel
-    (several epochs of the 32-entry chunk-meta ring), ragged chunks with interface overflow slots, over a whole trajectory."""
-    cfg = config(3, scale=0.5)
-    mesh, orc, d, stats = _trajectory(cfg, 500, shear=True, tip_width=1.0 / 500, chunk_elems=32, order=1)
-    assert mesh.n_chunks == 15625 and mesh.n_chunks > 32 * 444
-    assert orc.H.max() > 3 * cfg["material"]["Gc"] / (16 * cfg["material"]["l0"])  # the AT1 threshold was crossed: damage grew
-    assert (d > cfg["d0"] + 1e-6).sum() > 0 and stats["restarts"] > 0, stats
-
-
-def test_trajectory_500_steps_config2_full_size():
-    """500 staggered steps of config 2 at BASELINE's full size (401 x 161 nodes, 128,000 elements, jittered nodes,
-    permuted elements, spectral split, AT2) with the library defaults."""
+def test_trajectory_500_steps_config2_full_size_default_and_overflow():
+    """north_star's trajectory criterion at its stated length on a mesh that is not small: 500 staggered steps of config 2
+    at BASELINE's full size (401 x 161 nodes, 128,000 elements, jittered nodes, randomly permuted elements, spectral split,
+    AT2).  One oracle run, two CUDA meshes stepped beside it: (i) the library defaults (bisection chunks: the decomposition
+    bench.py times); (ii) PFF_ORDER_NONE with chunks of 32 elements of the PERMUTED element list: 4,000 chunks whose
+    elements are scattered over the plate, so every node is an interface node, most are touched by more chunks than there
+    are fixed partial slots (overflow slots) and every chunk has more halo nodes than it has elements -- the irregular
+    paths of all three kernels over a whole trajectory."""
     cfg = config(2)
-    mesh, orc, d, stats = _trajectory(cfg, 500, S=8.0, tip_width=0.100 / 400 * 1.2)
-    assert mesh.n_elems == 128000 and stats["iters"] > 500
+    gpus, orc, iters = _trajectory(cfg, 500, [dict(), dict(order=0, chunk_elems=32)], S=8.0, tip_width=0.100 / 400 * 1.2)
+    (m0, _), (m1, _) = gpus
+    assert m0.n_elems == 128000 and min(iters) > 500
+    assert m1.n_chunks == 4000 and m1.n_shared == m1.n_nodes
+    assert orc.H.max() > 0 and (orc.d > cfg["d0"] + 1e-6).sum() > 1000  # the damage field evolved
 
 
 def test_two_meshes_alternating_and_grown_dirichlet_set():
