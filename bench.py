@@ -124,6 +124,8 @@ def run_ours(args, rank: int, world: int):
         mesh.pff_set_traction(st, cfg["edges"], cfg["traction"])
     if len(cfg["notch"]):
         mesh.pff_set_damage_dirichlet(cfg["notch"])
+    if args.no_graph:
+        mesh.pff_set_graph_mode(False)
     N, Ne = mesh.n_nodes, mesh.n_elems
     dt = cfg["dt_factor"] * mesh.dt_crit
     bc = mesh.bc()
@@ -284,6 +286,7 @@ def main():
     ap.add_argument("--scatter", default="gather", choices=["gather", "atomic"],
                     help="explicit-step scatter: deterministic shared-memory gather (default) or warp-aggregated atomics")
     ap.add_argument("--repeats", type=int, default=5, help="how many times the K-step timed region is run (median reported)")
+    ap.add_argument("--no-graph", action="store_true", help="pff_run_steps launches every kernel itself instead of replaying a captured period")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
@@ -339,6 +342,7 @@ def main():
                 config=dict(workload=args.workload, scatter=args.scatter, name=r["cfg"]["name"], n_nodes=N, n_elems=Ne, rel_tol=REL_TOL,
                             cg_iters_per_solve=iters_total / K, chunks=r["mesh"].n_chunks, interface_nodes=r["mesh"].n_shared,
                             l2="working set > L2 (no flush needed)" if ab["step"] > 126e6 else "L2-resident workload",
+                            time_loop="plain launches" if args.no_graph else "CUDA graph replay of one captured step + solve",
                             parallelism=f"replicas x{world}"),
                 # the explicit step INSIDE the staggered loop (what a user gets) is the number; timed back to back alone it
                 # runs a little faster (warm instruction cache, no solve in between) and is reported as secondary

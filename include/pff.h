@@ -196,9 +196,18 @@ pff_status pff_subcycle_limit(const pff_material *material, int32_t *n_max, doub
 /* n_steps staggered steps on DEVICE-RESIDENT state (no host copies): pff_explicit_step every step (so the history
  * field and irreversibility follow the mechanical time scale, L187) and pff_damage_solve every damage_every-th step
  * (0 = never; 1 = the plain staggered scheme of L114).  Constant boundary data bc.  cg_iters_total (host, may be NULL)
- * receives the summed CG iterations.  Returns PFF_ENOCONV if any solve did (results are written).  Synchronises. */
+ * receives the summed CG iterations.  Returns PFF_ENOCONV if any solve did (results are written).  Synchronises once,
+ * at the end: the solves tally their counters on the device. */
 pff_status pff_run_steps(pff_mesh *mesh, pff_state *state, const pff_bc *bc, double dt, int64_t n_steps,
                          int32_t damage_every, double rel_tol, int32_t max_iter, int64_t *cg_iters_total);
+/* pff_run_steps replays one captured period of the loop (damage_every steps + one solve) from a CUDA graph when the run
+ * has at least four periods (SURVEY.md 8(f) NEXT-1 "whole-step CUDA graph": what small, launch-bound meshes need,
+ * PAPER.md L466).  The result is bit-identical to plain launches.  enable = 0 switches the capture off (A/B timing);
+ * it is also skipped while pff_profile_enable is on, and for good once the driver has refused to capture a launch. */
+pff_status pff_set_graph_mode(pff_mesh *mesh, int32_t enable);
+/* captured != 0: a captured period is held and will be replayed by a matching pff_run_steps; refused != 0: the driver
+ * refused a capture once (pff_run_steps then launches plainly for the life of the mesh).  Either may be NULL. */
+pff_status pff_graph_status(const pff_mesh *mesh, int32_t *captured, int32_t *refused);
 
 /* ---- implicit differentiation of the damage solve (section 4.2) -----------
  * Backward pass of A(theta) d = b(theta) (Eq. 22): ONE adjoint solve A^T lambda = g with the same matrix-free operator

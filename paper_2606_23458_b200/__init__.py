@@ -168,6 +168,14 @@ class Mesh:
                     allow=(PFF_ENOCONV,) if allow_noconv else ())
         return st, tot.value
 
+    def pff_set_graph_mode(self, enable: bool):
+        _check(self.L.pff_set_graph_mode(self.h, int(enable)))
+
+    def pff_graph_status(self):
+        c, r = C.c_int32(0), C.c_int32(0)
+        _check(self.L.pff_graph_status(self.h, C.byref(c), C.byref(r)))
+        return bool(c.value), bool(r.value)
+
     def pff_energies(self, state: State):
         out = (C.c_double * 4)()
         _check(self.L.pff_energies(self.h, C.byref(state.c), out))

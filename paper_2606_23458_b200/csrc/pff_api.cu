@@ -2,6 +2,8 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <map>
+#include <mutex>
 #include <new>
 
 #include "pff_device.cuh"
@@ -47,12 +49,25 @@ static pff_status upload_real(void** dst, const double* src, size_t count, size_
     return s;
 }
 
+// The dynamic shared-memory opt-in is an attribute of the FUNCTION on a device, shared by every mesh of the process that
+// uses the kernel there: it is only ever raised (a high-water mark per device and kernel, under a mutex), so a mesh with
+// small chunks never lowers it under a mesh with large ones.  The persistent grid depends on the mesh's own stage size
+// and is cached per mesh.
+static std::mutex g_optin_mutex;
+static std::map<std::pair<int, const void*>, int> g_optin;  // (device, kernel) -> bytes granted
+
 pff_status persistent_config(pff_mesh* m, const void* kern, int smem_bytes, int* grid, int block)
 {
     auto it = m->launch_grid.find(kern);
     if (it != m->launch_grid.end()) { *grid = it->second; return PFF_OK; }
-    // static + dynamic shared memory may exceed 48 KB: always opt in (per device; the mesh's device is current here)
-    PFF_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
+    {
+        std::lock_guard<std::mutex> lock(g_optin_mutex);
+        int& granted = g_optin[{m->device, kern}];
+        if (smem_bytes > granted) {  // static + dynamic shared memory may exceed 48 KB: always opt in
+            PFF_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
+            granted = smem_bytes;
+        }
+    }
     int per_sm = 0, sms = 0;
     PFF_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, block, (size_t)smem_bytes));
     PFF_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, m->device));
@@ -92,11 +107,12 @@ void pff_mesh_destroy(pff_mesh* m)
     void* ptrs[] = {m->d_meta, m->d_lconn, m->d_conn, m->d_ga, m->d_gb, m->d_area, m->d_minv, m->d_mass,
                     m->d_halo_ids, m->d_sh_rowptr, m->d_halo_dst, m->d_ell, m->d_flags, m->d_halo_part,
                     m->d_fwx, m->d_fwy, m->d_dir_dof, m->d_ca, m->d_cb, m->d_lb, m->d_r, m->d_p, m->d_q, m->d_dinv, m->d_mask,
-                    m->d_part, m->d_ctrl, m->d_ticket, m->d_step_bar, m->d_stage, m->d_hstate, m->d_hdir, m->d_node_old_of_new,
+                    m->d_part, m->d_tally, m->d_ctrl, m->d_ticket, m->d_step_bar, m->d_stage, m->d_hstate, m->d_hdir, m->d_node_old_of_new,
                     m->d_elem_old_of_new, m->d_n2e_ptr, m->d_n2e, m->d_eq_vec, m->d_eq_part, m->d_eq_sc};
     for (void* p : ptrs) if (p) cudaFree(p);
     if (m->h_ctrl) cudaFreeHost(m->h_ctrl);
-    if (m->h_ring) cudaFreeHost(m->h_ring);
+    if (m->h_tally) cudaFreeHost(m->h_tally);
+    if (m->graph_exec) cudaGraphExecDestroy(m->graph_exec);
     if (m->copy_stream) { cudaStreamSynchronize(m->copy_stream); cudaStreamDestroy(m->copy_stream); }
     if (m->ev_step) cudaEventDestroy(m->ev_step);
     for (auto& v : m->prof_ev) for (cudaEvent_t e : v) cudaEventDestroy(e);
@@ -266,6 +282,7 @@ pff_status pff_mesh_permutations(const pff_mesh* m, int32_t* node_new_of_old, in
 
 static pff_status push_flags(pff_mesh* m)
 {
+    ++m->flags_gen;  // invalidates a captured pff_run_steps period (the Dirichlet dof list pointer may have changed)
     PFF_CUDA(cudaMemcpyAsync(m->d_flags, m->h_flags.data(), m->h_flags.size(), cudaMemcpyHostToDevice, m->stream));
     PFF_CUDA(cudaStreamSynchronize(m->stream));
     return PFF_OK;
@@ -401,41 +418,97 @@ pff_status pff_run_steps(pff_mesh* m, pff_state* s, const pff_bc* bc, double dt,
     }
     if (!valid_bc(m, bc)) { set_error("pff_run_steps: dir_u and dir_v must be given together"); return PFF_EINVAL; }
     DeviceGuard dg(m);
-    // The whole loop is asynchronous: every solve copies its control block into a pinned ring; the host synchronises and
-    // inspects the ring only every kRing solves and at the end, so the GPU never waits for the host between steps.
-    constexpr int kRing = 64;
-    if (!m->h_ring) PFF_CUDA(cudaMallocHost((void**)&m->h_ring, kRing * sizeof(DamageCtrl)));
-    pff_status worst = PFF_OK, st = PFF_OK;
-    int64_t total = 0;
-    int pending = 0;
-    m->last_restarts = m->last_truncs = 0;
-    auto drain = [&]() -> pff_status {
-        pff_status e = cuda_check(cudaStreamSynchronize(m->stream), "pff_run_steps: sync");
-        if (e != PFF_OK) return e;
-        for (int i = 0; i < pending; ++i) {
-            total += m->h_ring[i].iters;
-            m->last_restarts += m->h_ring[i].restarts; m->last_truncs += m->h_ring[i].truncs;
-            if (!m->h_ring[i].done || m->h_ring[i].status == PFF_ENOCONV) worst = PFF_ENOCONV;
-        }
-        pending = 0;
-        return PFF_OK;
+    // The whole loop is asynchronous: every solve adds its counters to a device-resident tally, which the host reads ONCE at
+    // the end, so the GPU never waits for the host between steps.  When the run is long enough, one period of the loop
+    // (damage_every explicit steps + one solve; kernels only, no copies) is captured into a CUDA graph after it has run
+    // once the ordinary way and replayed for the remaining periods: small meshes, where a step is a handful of
+    // microsecond kernels, then pay one graph launch per period instead of a cooperative launch per kernel.
+    if (!m->d_tally) {
+        PFF_CUDA(cudaMalloc((void**)&m->d_tally, sizeof(RunTally)));
+        PFF_CUDA(cudaMallocHost((void**)&m->h_tally, sizeof(RunTally)));
+    }
+    PFF_CUDA(cudaMemsetAsync(m->d_tally, 0, sizeof(RunTally), m->stream));
+    pff_status st = PFF_OK;
+    m->defer = true;
+    auto one_step = [&](int64_t k) -> pff_status {
+        pff_status e = launch_step(m, s, bc, dt, /*MODE_STEP*/ 0, nullptr, nullptr, nullptr);
+        if (e == PFF_OK && damage_every > 0 && k % damage_every == 0) e = damage_solve(m, s, rel_tol, max_iter, nullptr, nullptr);
+        return e;
     };
-    for (int64_t k = 1; k <= n_steps && st == PFF_OK; ++k) {
-        if ((st = launch_step(m, s, bc, dt, /*MODE_STEP*/ 0, nullptr, nullptr, nullptr)) != PFF_OK) break;
-        if (damage_every > 0 && k % damage_every == 0) {
-            m->defer_slot = &m->h_ring[pending];
-            st = damage_solve(m, s, rel_tol, max_iter, nullptr, nullptr);
-            m->defer_slot = nullptr;
-            if (st != PFF_OK) break;
-            if (++pending == kRing) st = drain();
+    const int64_t period = damage_every > 0 ? damage_every : 1;
+    int64_t k = 1;
+    const bool want_graph = m->graph_mode != 0 && !m->graph_unsupported && !m->prof_on && period <= 64 && n_steps >= 4 * period;
+    if (want_graph) {
+        // key of everything a captured period depends on (kernel arguments are frozen at capture time)
+        struct Key { pff_state s; pff_bc bc; double dt, tol; int32_t every, max_iter; int64_t n_dir; uint64_t flags_gen; } key{};
+        key.s = *s; if (bc) key.bc = *bc; else key.bc.load_scale = 1.0;
+        key.dt = dt; key.tol = rel_tol; key.every = damage_every; key.max_iter = max_iter; key.n_dir = m->n_dir; key.flags_gen = m->flags_gen;
+        const unsigned char* kb = reinterpret_cast<const unsigned char*>(&key);
+        const bool cached = m->graph_exec && m->graph_key.size() == sizeof(Key) && std::memcmp(m->graph_key.data(), kb, sizeof(Key)) == 0;
+        if (!cached) {
+            if (m->graph_exec) { cudaGraphExecDestroy(m->graph_exec); m->graph_exec = nullptr; }
+            for (; k <= period && st == PFF_OK; ++k) st = one_step(k);  // first period the ordinary way (also does every lazy allocation)
+            if (st == PFF_OK) {
+                const int64_t l0 = m->n_launches;
+                cudaGraph_t graph = nullptr;
+                // The period is recorded on a stream of the library's own (the caller's may be the legacy default stream,
+                // which cannot capture); recording executes nothing, and the replays go to the caller's stream.
+                cudaError_t ce = m->copy_stream ? cudaSuccess : cudaStreamCreateWithFlags(&m->copy_stream, cudaStreamNonBlocking);
+                pff_status cst = PFF_OK;
+                if (ce == cudaSuccess) ce = cudaStreamBeginCapture(m->copy_stream, cudaStreamCaptureModeThreadLocal);
+                if (ce == cudaSuccess) {
+                    cudaStream_t user = m->stream;
+                    m->stream = m->copy_stream;
+                    for (int64_t j = 1; j <= period && cst == PFF_OK; ++j) cst = one_step(j);
+                    m->stream = user;
+                    ce = cudaStreamEndCapture(m->copy_stream, &graph);
+                }
+                m->graph_launches = (int)(m->n_launches - l0);
+                m->n_launches = l0;  // captured, not launched
+                if (ce == cudaSuccess && cst == PFF_OK && graph) ce = cudaGraphInstantiate(&m->graph_exec, graph, 0);
+                if (graph) cudaGraphDestroy(graph);
+                if (ce != cudaSuccess || cst != PFF_OK || !m->graph_exec) {  // not capturable here: plain launches from now on
+                    m->graph_refusal = ce != cudaSuccess ? cudaGetErrorString(ce) : pff_last_error();
+                    cudaGetLastError();
+                    m->graph_exec = nullptr; m->graph_unsupported = true;
+                } else {
+                    m->graph_key.assign(kb, kb + sizeof(Key));
+                }
+            }
+        }
+        if (st == PFF_OK && m->graph_exec) {
+            for (; k + period - 1 <= n_steps && st == PFF_OK; k += period) {
+                st = cuda_check(cudaGraphLaunch(m->graph_exec, m->stream), "pff_run_steps: graph launch");
+                m->n_launches += m->graph_launches;
+            }
         }
     }
-    const pff_status e = drain();
+    for (; k <= n_steps && st == PFF_OK; ++k) st = one_step(k);
+    m->defer = false;
+    pff_status e = cuda_check(cudaMemcpyAsync(m->h_tally, m->d_tally, sizeof(RunTally), cudaMemcpyDeviceToHost, m->stream), "pff_run_steps: tally");
+    if (e == PFF_OK) e = cuda_check(cudaStreamSynchronize(m->stream), "pff_run_steps: sync");
     if (st != PFF_OK) return st;
     if (e != PFF_OK) return e;
-    if (cg_iters_total) *cg_iters_total = total;
-    if (worst == PFF_ENOCONV) set_error("pff_run_steps: a damage solve reached max_iter");
-    return worst;
+    m->last_restarts = m->h_tally->restarts; m->last_truncs = m->h_tally->truncs;
+    if (cg_iters_total) *cg_iters_total = m->h_tally->iters;
+    if (m->h_tally->noconv > 0) { set_error("pff_run_steps: a damage solve reached max_iter"); return PFF_ENOCONV; }
+    return PFF_OK;
+}
+
+pff_status pff_graph_status(const pff_mesh* m, int32_t* captured, int32_t* refused)
+{
+    if (!m) { set_error("pff_graph_status: null mesh"); return PFF_EINVAL; }
+    if (captured) *captured = m->graph_exec != nullptr;
+    if (refused) *refused = m->graph_unsupported;
+    if (m->graph_unsupported) set_error("graph capture refused: " + m->graph_refusal);  // readable through pff_last_error()
+    return PFF_OK;
+}
+
+pff_status pff_set_graph_mode(pff_mesh* m, int32_t enable)
+{
+    if (!m) { set_error("pff_set_graph_mode: null mesh"); return PFF_EINVAL; }
+    m->graph_mode = enable != 0;
+    return PFF_OK;
 }
 
 pff_status pff_stiffness_action(pff_mesh* m, const pff_state* s, const void* px, const void* py, void* qx, void* qy)

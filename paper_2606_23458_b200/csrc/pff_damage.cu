@@ -64,6 +64,7 @@ struct DmgArgs {
     double* part;    // [kCh][part_n] chunk-kernel block partials
     int64_t part_n;
     DamageCtrl* ctrl;
+    RunTally* tally;         // may be null: device-resident counters of a pff_run_steps call
     double tol;              // stopping tolerance and iteration cap of this solve (the setup kernel writes them into ctrl)
     int max_iter;
     unsigned int* ticket;    // [0] last-block ticket, [1] grid barrier of the CG kernel (zeroed by the setup kernel before it),
@@ -115,9 +116,7 @@ __device__ __forceinline__ void block_reduce_ch(double v[kCh], double* s_w /* [k
 }
 
 enum { DM_CG = 0, DM_PLAIN = 1 };
-#ifndef PFF_PART_LOAD
-#define PFF_PART_LOAD __ldcg
-#endif
+
 
 
 struct IterScalars {
@@ -454,7 +453,6 @@ __global__ void __launch_bounds__(kTPB, 3) dmg_iter_chunk(const DmgArgs<R> a)
     fence_proxy_async_global();
     // ---- interface nodes (owned by no chunk): ordered sum of the chunk partials, same prologue; grid-wide phase
     grid_barrier(a.ticket + 1, gb_target, (unsigned)G);
-#ifndef PFF_PREISSUE_LATE
     // every interior value is final: start streaming the first chunk of the next CG iteration
     if (single_epoch) {
         if (issuer) {
@@ -467,7 +465,6 @@ __global__ void __launch_bounds__(kTPB, 3) dmg_iter_chunk(const DmgArgs<R> a)
         }
         pre_issued = true;
     }
-#endif
     {
         // Equal slice per CTA, TWO nodes per thread and trip: every load of both nodes is issued before anything is
         // computed or stored, so a trip costs one memory round trip (the slice is ~1.3 nodes per thread at 10^6 nodes).
@@ -507,19 +504,6 @@ __global__ void __launch_bounds__(kTPB, 3) dmg_iter_chunk(const DmgArgs<R> a)
             if (two) if_finish(s1, n1);
         }
     }
-#ifdef PFF_PREISSUE_LATE
-    if (single_epoch) {
-        if (issuer) {
-            const ChunkMeta cm = s_meta[0];
-            const ChunkRange cr{cm.elem_start, cm.n_elem, a.Ne, cm.node_start, cm.n_int, a.N, cm.ell_off,
-                                cm.ell_w * (cm.n_int + cm.n_halo), (int)a.ell_total, cm.halo_off, cm.n_halo, (int)a.n_entries,
-                                n_my > 1 ? s_meta[1].halo_off : 0, n_my > 1 ? s_meta[1].n_halo : 0};
-            fence_proxy_async();
-            stage_issue_desc(my_desc, have_desc, smem + (it & 1) * L.stage_bytes, bar + 2 * (it & 1), lane, cr);
-        }
-        pre_issued = true;
-    }
-#endif
     __syncthreads();  // reconverge before the shuffle tree (measured: 10 us per iteration faster than without)
     block_reduce_ch(acc, s_w, s_out);
     if (tid < kCh) a.part[(int64_t)tid * a.part_n + blockIdx.x] = s_out[tid];
@@ -544,7 +528,7 @@ __global__ void __launch_bounds__(kTPB, 3) dmg_iter_chunk(const DmgArgs<R> a)
 #pragma unroll
                 for (int j = 0; j < kB; ++j) {
                     const int i = base + 32 * j + lane;
-                    u[j] = i < G ? PFF_PART_LOAD(a.part + (int64_t)w * a.part_n + i) : ident;
+                    u[j] = i < G ? __ldcg(a.part + (int64_t)w * a.part_n + i) : ident;
                 }
 #pragma unroll
                 for (int j = 0; j < kB; ++j) v = (w == kCh - 1) ? fmin(v, u[j]) : v + u[j];
@@ -595,7 +579,14 @@ finalize:
             }
             a.x[i] = v;
         }
-        if (blockIdx.x == 0 && tid == 0) *a.ctrl = s_ctrl;
+        if (blockIdx.x == 0 && tid == 0) {
+            *a.ctrl = s_ctrl;
+            if (a.tally) {  // single writer, stream-ordered between solves
+                a.tally->iters += s_ctrl.iters; a.tally->solves += 1;
+                a.tally->noconv += (!s_ctrl.done || s_ctrl.status == PFF_ENOCONV) ? 1 : 0;
+                a.tally->restarts += s_ctrl.restarts; a.tally->truncs += s_ctrl.truncs;
+            }
+        }
     }
 }
 
@@ -918,7 +909,7 @@ static pff_status launch_setup(pff_mesh* m, DmgArgs<R>& asu, const void* kern, u
 {
     void* kargs[] = {(void*)&asu};
     prof_mark(m, PFF_K_DAMAGE_SETUP);
-    cudaError_t e = cudaLaunchCooperativeKernel(kern, dim3(g), dim3(kTPB), kargs, (size_t)smem, m->stream);
+    cudaError_t e = launch_cooperative(kern, g, kTPB, kargs, (size_t)smem, m->stream);
     prof_mark(m, PFF_K_DAMAGE_SETUP);
     if (e != cudaSuccess) return cuda_check(e, "damage: setup launch");
     ++m->n_launches;
@@ -950,21 +941,19 @@ static pff_status damage_solve_t(pff_mesh* m, const pff_state* s, double rel_tol
     if ((st = persistent_config(m, (const void*)dmg_setup_chunk<R, false>, smem_su, &grid_su)) != PFF_OK) return st;
     const unsigned gmv = (unsigned)std::min<int64_t>(grid_mv, hm.C), gsu = (unsigned)std::min<int64_t>(grid_su, hm.C);
     asu.tol = rel_tol; asu.max_iter = max_iter;
+    a.tally = m->defer ? m->d_tally : nullptr;
     if ((st = launch_setup(m, asu, (const void*)dmg_setup_chunk<R, false>, gsu, smem_su)) != PFF_OK) return st;
     // ONE cooperative launch runs every CG iteration (grid-wide barriers between the chunk phase, the interface
     // phase and the scalar recurrence), applies the last step and the clamp, and writes the control block back
     {
         void* kargs[] = {(void*)&a};
         prof_mark(m, PFF_K_MATVEC_CHUNK);
-        cudaError_t e = cudaLaunchCooperativeKernel((const void*)dmg_iter_chunk<R, DM_CG, PROJ>, dim3(gmv), dim3(kTPB), kargs,
-                                                    (size_t)smem_mv, cs);
+        cudaError_t e = launch_cooperative((const void*)dmg_iter_chunk<R, DM_CG, PROJ>, gmv, kTPB, kargs, (size_t)smem_mv, cs);
         prof_mark(m, PFF_K_MATVEC_CHUNK);
         ++m->n_launches;
         if ((st = cuda_check(e, "damage: cooperative launch")) != PFF_OK) return st;
     }
-    if (m->defer_slot) {  // pff_run_steps: the control block is read back asynchronously and inspected later, no sync here
-        return cuda_check(cudaMemcpyAsync(m->defer_slot, m->d_ctrl, sizeof(DamageCtrl), cudaMemcpyDeviceToHost, cs), "damage: ctrl download");
-    }
+    if (m->defer) return PFF_OK;  // pff_run_steps: the kernel has tallied its counters on the device; nothing is read back here
     DamageCtrl* h = m->h_ctrl;  // pinned download image; the stream is synchronised before it is read or reused
     if ((st = cuda_check(cudaMemcpyAsync(h, m->d_ctrl, sizeof(DamageCtrl), cudaMemcpyDeviceToHost, cs), "damage: ctrl download")) != PFF_OK) return st;
     if ((st = cuda_check(cudaStreamSynchronize(cs), "damage: sync")) != PFF_OK) return st;

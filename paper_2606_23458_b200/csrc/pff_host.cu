@@ -96,10 +96,8 @@ static pff_status run_host_t(pff_mesh* m, pff_host_state* hs, const double* dir_
     pff_status worst = PFF_OK;
     // The results of the LAST explicit step (u, v, a, H) are final before its damage solve: they are permuted and copied
     // back on a second stream while the solve runs on the mesh stream; d follows when the solve is done.
-    if (!m->copy_stream) {
-        if ((st = cuda_check(cudaStreamCreateWithFlags(&m->copy_stream, cudaStreamNonBlocking), "run_host: stream")) != PFF_OK) return st;
-        if ((st = cuda_check(cudaEventCreateWithFlags(&m->ev_step, cudaEventDisableTiming), "run_host: event")) != PFF_OK) return st;
-    }
+    if (!m->copy_stream && (st = cuda_check(cudaStreamCreateWithFlags(&m->copy_stream, cudaStreamNonBlocking), "run_host: stream")) != PFF_OK) return st;
+    if (!m->ev_step && (st = cuda_check(cudaEventCreateWithFlags(&m->ev_step, cudaEventDisableTiming), "run_host: event")) != PFF_OK) return st;
     cudaStream_t cp = m->copy_stream;
     bool mech_out = false;
     auto mechanics_out = [&]() -> pff_status {

@@ -16,6 +16,11 @@ struct DamageCtrl {
     int truncs;    // AT1: steps cut short at the first bound hit
 };
 
+// counters of all solves of one pff_run_steps call (device-resident, added to by the last phase of the CG kernel)
+struct RunTally {
+    long long iters;
+    int solves, noconv, restarts, truncs;
+};
 static_assert(sizeof(DamageCtrl) % 8 == 0, "the control block is copied in 8-byte words");
 
 struct pff_mesh {
@@ -69,8 +74,19 @@ struct pff_mesh {
     DamageCtrl* d_ctrl = nullptr;  // initialised on the device by the setup kernel of every solve (no host upload)
     DamageCtrl* h_ctrl = nullptr;  // pinned download image of the last synchronous solve
     int last_restarts = 0, last_truncs = 0;  // of the last pff_damage_solve, or summed over the last pff_run_steps
-    DamageCtrl* h_ring = nullptr;      // pinned ring of deferred read-backs (pff_run_steps)
-    DamageCtrl* defer_slot = nullptr;  // non-null: damage_solve copies the control block here and does not synchronise
+    // pff_run_steps: every solve adds its counters to a device-resident tally instead of being read back (no host round
+    // trip per solve, and the launches can be replayed from a CUDA graph); the host reads the tally once at the end
+    RunTally* d_tally = nullptr;
+    RunTally* h_tally = nullptr;  // pinned
+    bool defer = false;           // true inside pff_run_steps: damage_solve tallies on the device and does not synchronise
+    // one captured period of pff_run_steps (damage_every explicit steps + one solve) and the arguments it was captured with
+    cudaGraphExec_t graph_exec = nullptr;
+    std::vector<unsigned char> graph_key;
+    uint64_t flags_gen = 0;       // bumped by pff_set_dirichlet / pff_set_damage_dirichlet
+    int graph_launches = 0;       // kernel launches one replay stands for
+    int graph_mode = 1;           // 0: never capture (pff_set_graph_mode); 1: capture when a run has enough periods
+    std::string graph_refusal;    // why
+    bool graph_unsupported = false;  // capture of a cooperative launch was refused once on this driver: do not try again
     unsigned int* d_ticket = nullptr;
     // quasi-static mechanics solve (pff_equilibrium.cu), allocated at its first call
     int32_t *d_n2e_ptr = nullptr, *d_n2e = nullptr;  // node -> (4 * element + corner) table
@@ -118,6 +134,18 @@ pff_status equilibrium_solve(pff_mesh* m, pff_state* s, const pff_bc* bc, double
 pff_status damage_rhs_diag(pff_mesh* m, const pff_state* s, void* b, void* D);
 pff_status energies(pff_mesh* m, const pff_state* s, double out[4]);
 pff_status cuda_check(cudaError_t e, const char* what);
+// Cooperative launch (all CTAs co-resident: the kernels synchronise grid-wide) through the extensible launch API with the
+// cooperative attribute: unlike the legacy cooperative-launch entry point it can be captured into a CUDA graph.
+inline cudaError_t launch_cooperative(const void* kern, unsigned grid, unsigned block, void** args, size_t smem, cudaStream_t stream)
+{
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = smem; cfg.stream = stream;
+    cudaLaunchAttribute attr{};
+    attr.id = cudaLaunchAttributeCooperative;
+    attr.val.cooperative = 1;
+    cfg.attrs = &attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelExC(&cfg, kern, args);
+}
 // dynamic shared-memory opt-in + occupancy-derived persistent grid of `kern` for this mesh (cached in m->launch_grid)
 pff_status persistent_config(pff_mesh* m, const void* kern, int smem_bytes, int* grid, int block = 256);
 

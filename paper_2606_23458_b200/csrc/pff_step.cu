@@ -470,7 +470,7 @@ static pff_status launch_step_t(pff_mesh* m, const StepArgs<R>& a)
             b.gbar = m->d_step_bar;
             void* kargs[] = {(void*)&b};
             prof_mark(m, PFF_K_STEP_CHUNK);
-            cudaError_t e = cudaLaunchCooperativeKernel((const void*)kern, dim3(g), dim3(kStepTPB), kargs, (size_t)m->lay_step.total, m->stream);
+            cudaError_t e = launch_cooperative((const void*)kern, g, kStepTPB, kargs, (size_t)m->lay_step.total, m->stream);
             prof_mark(m, PFF_K_STEP_CHUNK);
             if (e != cudaSuccess) return cuda_check(e, "explicit step: cooperative launch");
             m->last_step_grid = (int)g;

@@ -119,15 +119,13 @@ __device__ __forceinline__ void stage_issue_desc(const StageDesc& d, bool have, 
     if (lane == 0) mbar_arrive_expect_tx(bar, bytes);
 }
 
-// Grid-wide barrier of the cooperatively launched kernels (all CTAs are co-resident): one arrival per CTA on a counter that only
-// grows (zeroed by the host before the launch, or continued from launch to launch with a host-side epoch base), thread 0 spins with acquire loads until the epoch's target.
-// The gpu-scope fences order the CTA's global writes before the arrival and invalidate L1 after the wait.
+// Grid-wide barrier of the cooperatively launched kernels (all CTAs are co-resident): one arrival per CTA on a counter that
+// only grows (the epoch it starts from is kept on the device), thread 0 spins with acquire loads until the epoch's target.
 __device__ __forceinline__ void grid_barrier(unsigned int* counter, unsigned int& target, unsigned int G)
 {
     __syncthreads();
     if (threadIdx.x == 0) {
         target += G;
-#ifdef PFF_BAR_LIGHT
         // release-arrive (orders this CTA's writes, observed through the block barrier above, before the arrival) and
         // acquire-poll; the comparison is wrap-safe
         asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(counter) : "memory");
@@ -135,15 +133,6 @@ __device__ __forceinline__ void grid_barrier(unsigned int* counter, unsigned int
         do {
             asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(counter) : "memory");
         } while ((int)(seen - target) < 0);
-#else
-        __threadfence();
-        atomicAdd(counter, 1u);
-        unsigned int seen;
-        do {
-            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(counter) : "memory");
-        } while ((int)(seen - target) < 0);
-        __threadfence();
-#endif
     }
     __syncthreads();
 }
