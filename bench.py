@@ -29,10 +29,13 @@ METRIC, UNIT = "element-updates/s (explicit step + damage solve)", "elem/s"
 REL_TOL, MAX_ITER = 1e-8, 1000
 
 
-def make_workload(name: str):
+def make_workload(name: str, l0_over_h: float | None = None):
     from pff_inputs import config
     if name.startswith("cfg5_"):
-        return config(5, n=int(name.split("_")[1]))
+        cfg = config(5, n=int(name.split("_")[1]))
+        if l0_over_h is not None:  # same mesh and fields, regularisation length rescaled (config 5 has h = 1 mm, l0 = 0.5 mm)
+            cfg["material"] = dict(cfg["material"], l0=l0_over_h * 1e-3)
+        return cfg
     return config(int(name[3:]))
 
 
@@ -116,7 +119,7 @@ def run_ours(args, rank: int, world: int):
     torch.cuda.set_device(dev)
     prec = pff.PFF_F32 if args.precision == "f32" else pff.PFF_F64
     w = 4 if prec == pff.PFF_F32 else 8
-    cfg = make_workload(args.workload)
+    cfg = make_workload(args.workload, args.l0_over_h)
     mesh = pff.Mesh(cfg["xy"], cfg["tri"], cfg["material"], precision=prec, chunk_elems=args.chunk, device=f"cuda:{dev}",
                     scatter=pff.PFF_SCATTER_ATOMIC if args.scatter == "atomic" else pff.PFF_SCATTER_GATHER)
     st = mesh.new_state(u=cfg["u0"], d=cfg["d0"])
@@ -286,6 +289,9 @@ def main():
     ap.add_argument("--scatter", default="gather", choices=["gather", "atomic"],
                     help="explicit-step scatter: deterministic shared-memory gather (default) or warp-aggregated atomics")
     ap.add_argument("--repeats", type=int, default=5, help="how many times the K-step timed region is run (median reported)")
+    ap.add_argument("--l0-over-h", type=float, default=None,
+                    help="config 5 only: regularisation length in mesh widths (default 0.5, the BASELINE recipe); larger values make the "
+                         "damage operator diffusion-dominated and raise the Jacobi-PCG iteration count (PAPER.md L175, L217)")
     ap.add_argument("--no-graph", action="store_true", help="pff_run_steps launches every kernel itself instead of replaying a captured period")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -342,6 +348,7 @@ def main():
                 config=dict(workload=args.workload, scatter=args.scatter, name=r["cfg"]["name"], n_nodes=N, n_elems=Ne, rel_tol=REL_TOL,
                             cg_iters_per_solve=iters_total / K, chunks=r["mesh"].n_chunks, interface_nodes=r["mesh"].n_shared,
                             l2="working set > L2 (no flush needed)" if ab["step"] > 126e6 else "L2-resident workload",
+                            l0_over_h=args.l0_over_h if args.l0_over_h is not None else "recipe",
                             time_loop="plain launches" if args.no_graph else "CUDA graph replay of one captured step + solve",
                             parallelism=f"replicas x{world}"),
                 # the explicit step INSIDE the staggered loop (what a user gets) is the number; timed back to back alone it

@@ -298,6 +298,14 @@ pff_status pff_run_host(pff_mesh *mesh, pff_host_state *hs, const double *dir_u,
                         double load_scale, double dt, int64_t n_steps, int32_t damage_every,
                         double rel_tol, int32_t max_iter);
 
+/* Phase timestamps of the persistent kernels, for timelines like profiles/r2_timeline.md.  Only the instrumentation
+ * build of the library (libpff_trace.so: python -m paper_2606_23458_b200.build --trace) records anything; the product
+ * library returns PFF_EUNSUPPORTED.  device_words: device buffer of 2 * 256 * 1024 int64 (zeroed by the caller) or NULL to
+ * stop; thread 0 of every CTA stores SM-cycle and nanosecond stamps of its phases (chunk by chunk: data arrived, node
+ * prologue done, element pass done, gather done; then the grid-wide phases) for CG iteration cg_iteration of every
+ * following solve and for every following explicit step.  Layout: paper_2606_23458_b200/trace_timeline.py. */
+pff_status pff_trace_set(pff_mesh *mesh, void *device_words, int32_t cg_iteration);
+
 const char *pff_last_error(void);
 
 #ifdef __cplusplus

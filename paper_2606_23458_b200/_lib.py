@@ -21,7 +21,7 @@ SYMBOLS = [
     "pff_mesh_create", "pff_mesh_plan", "pff_mesh_destroy", "pff_mesh_info", "pff_mesh_permutations", "pff_set_dirichlet",
     "pff_set_damage_dirichlet", "pff_set_traction", "pff_init_accel", "pff_explicit_step", "pff_damage_solve",
     "pff_energies", "pff_damage_last_stats", "pff_subcycle_limit", "pff_run_steps", "pff_set_graph_mode", "pff_graph_status", "pff_damage_adjoint", "pff_damage_param_terms", "pff_stiffness_action", "pff_equilibrium_solve", "pff_internal_force", "pff_damage_matvec", "pff_damage_rhs_diag", "pff_run_host", "pff_mesh_counters", "pff_time_kernel",
-    "pff_profile_enable", "pff_profile_read",
+    "pff_profile_enable", "pff_profile_read", "pff_trace_set",
     "pff_last_error",
 ]
 
@@ -51,10 +51,12 @@ _lib = None
 
 
 def load() -> C.CDLL:
-    """Load libpff.so; there is NO fallback: a missing library is an error."""
-    global _lib
+    """Load libpff.so; there is NO fallback: a missing library is an error.  PFF_LIBRARY in the environment selects another
+    build of the same library (the instrumentation build libpff_trace.so)."""
+    global _lib, LIB_PATH
     if _lib is not None:
         return _lib
+    LIB_PATH = os.environ.get("PFF_LIBRARY", LIB_PATH)
     if not os.path.exists(LIB_PATH):
         raise ImportError(
             f"{LIB_PATH} not found: build it with `python -m paper_2606_23458_b200.build` "
@@ -92,6 +94,7 @@ def load() -> C.CDLL:
     L.pff_time_kernel.argtypes = [vp, C.POINTER(pff_state), i32, i32, C.POINTER(C.c_float)]
     L.pff_profile_enable.argtypes = [vp, i32]
     L.pff_profile_read.argtypes = [vp, dp, C.POINTER(i64)]
+    L.pff_trace_set.argtypes = [vp, vp, i32]
     L.pff_last_error.restype = C.c_char_p
     for name in SYMBOLS:
         if name not in ("pff_mesh_destroy", "pff_last_error"):

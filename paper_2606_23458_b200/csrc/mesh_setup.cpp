@@ -54,7 +54,7 @@ static void bisect_into_chunks(const std::vector<int32_t>& morton_order, const s
 }
 
 pff_status build_host_mesh(int64_t N, const double* xy, int64_t Ne, const int32_t* tri_in, double rho,
-                           int order, int chunk_elems, size_t real_bytes, HostMesh& hm, std::string& err)
+                           int order, int chunk_elems, size_t real_bytes, HostMesh& hm, std::string& err, int cg_ctas)
 {
     if (N < 3 || Ne < 1) { err = "mesh needs at least 3 nodes and 1 element"; return PFF_EINVAL; }
     if (N >= (int64_t(1) << 30) || Ne >= (int64_t(1) << 30)) { err = "mesh too large (>= 2^30)"; return PFF_EMESH; }
@@ -142,6 +142,7 @@ pff_status build_host_mesh(int64_t N, const double* xy, int64_t Ne, const int32_
     const size_t limit_cg = (user_chunk ? kSmemPerSM : kSmemPerSM / 3) - kSmemCtaReserve;
     const size_t limit_other = (user_chunk ? kSmemPerSM : kSmemPerSM / 2) - kSmemCtaReserve;
     std::vector<int32_t> cmin(N), cmax(N);
+    bool balanced = false;  // the balance-aware choice below has been made
     for (;;) {
         if (order == PFF_ORDER_BISECTION) bisect_into_chunks(morton_order, ccx, ccy, EC, elem_old_of_new);
         std::fill(cmin.begin(), cmin.end(), std::numeric_limits<int32_t>::max());
@@ -178,6 +179,23 @@ pff_status build_host_mesh(int64_t N, const double* xy, int64_t Ne, const int32_
         if (fits || EC <= 32) {
             if (std::max(smem_cg, std::max(smem_step, smem_su)) > kSmemPerSM - kSmemCtaReserve) {
                 err = "chunk does not fit shared memory"; return PFF_EMESH;
+            }
+            if (!user_chunk && !balanced && EC > 128) {
+                // EC is the largest chunk that fits.  The persistent CG kernel (most of a staggered step) gives CTA b the
+                // chunks b, b + G, ...: its chunk phase lasts ceil(C / G) chunks, so a chunk count just above a multiple of
+                // G leaves most CTAs idle for a whole chunk (fp32 at 10^6 nodes: 3125 chunks of 640 on 444 CTAs = 8 rounds
+                // where 7.04 would do).  Pick, among the sizes that fit, the one with the smallest modelled phase length:
+                // rounds x (chunk + a fixed per-chunk cost), weighted by the growth of the interface (~ 1 / sqrt(chunk)).
+                balanced = true;
+                const int64_t G = cg_ctas > 0 ? cg_ctas : 444;
+                auto cost = [&](int ec) {
+                    const int64_t rounds = ((Ne + ec - 1) / ec + G - 1) / G;
+                    return double(rounds) * double(ec + 60) * (1.0 + 0.3 * (std::sqrt(double(EC) / double(ec)) - 1.0));
+                };
+                int best = EC;
+                for (int ec = EC - 32; ec >= 128; ec -= 32)
+                    if (cost(ec) < 0.97 * cost(best)) best = ec;  // only a clear gain justifies more interface nodes
+                if (best != EC) { EC = best; continue; }
             }
             hm.max_nloc = max_nloc; hm.C = C;
             break;

@@ -147,8 +147,10 @@ pff_status pff_mesh_create(int64_t n_nodes, const double* xy, int64_t n_elems, c
     m->rb = opt.precision == PFF_F32 ? 4 : 8;
     std::string err;
     pff_status st;
+    int sms = 0;  // the persistent CG kernel runs 3 CTAs per SM: the chunk size is balanced for that grid
+    if (cudaGetDevice(&m->device) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, m->device);
     try {
-        st = build_host_mesh(n_nodes, xy, n_elems, tri, mat->rho, opt.order, opt.chunk_elems, m->rb, m->hm, err);
+        st = build_host_mesh(n_nodes, xy, n_elems, tri, mat->rho, opt.order, opt.chunk_elems, m->rb, m->hm, err, 3 * sms);
     } catch (const std::bad_alloc&) { st = PFF_ENOMEM; err = "out of host memory in mesh setup"; }
     if (st != PFF_OK) { set_error("pff_mesh_create: " + err); delete m; return st; }
     HostMesh& hm = m->hm;
@@ -493,6 +495,19 @@ pff_status pff_run_steps(pff_mesh* m, pff_state* s, const pff_bc* bc, double dt,
     if (cg_iters_total) *cg_iters_total = m->h_tally->iters;
     if (m->h_tally->noconv > 0) { set_error("pff_run_steps: a damage solve reached max_iter"); return PFF_ENOCONV; }
     return PFF_OK;
+}
+
+pff_status pff_trace_set(pff_mesh* m, void* device_words, int32_t cg_iteration)
+{
+    if (!m) { set_error("pff_trace_set: null mesh"); return PFF_EINVAL; }
+#ifdef PFF_TRACE
+    m->d_trace = (long long*)device_words; m->trace_iter = cg_iteration;
+    return PFF_OK;
+#else
+    (void)device_words; (void)cg_iteration;
+    set_error("pff_trace_set: this build has no phase timestamps (build with python -m paper_2606_23458_b200.build --trace)");
+    return PFF_EUNSUPPORTED;
+#endif
 }
 
 pff_status pff_graph_status(const pff_mesh* m, int32_t* captured, int32_t* refused)

@@ -63,6 +63,8 @@ struct DmgArgs {
     R *q_out, *b_out, *D_out;
     double* part;    // [kCh][part_n] chunk-kernel block partials
     int64_t part_n;
+    long long* trace;        // phase timestamps (PFF_TRACE builds), CG iteration trace_iter only
+    int trace_iter;
     DamageCtrl* ctrl;
     RunTally* tally;         // may be null: device-resident counters of a pff_run_steps call
     double tol;              // stopping tolerance and iteration cap of this solve (the setup kernel writes them into ctrl)
@@ -314,12 +316,16 @@ __global__ void __launch_bounds__(kTPB, 3) dmg_iter_chunk(const DmgArgs<R> a)
         cp_async_mbar_arrive(sbar);
     };
     unsigned int gb_target = 0;  // grid-barrier epoch target (thread 0)
+    int cg_it = 0;  // CG iterations done (phase trace)
     int it = 0;  // stage uses so far (global over epochs and CG iterations): stage = it & 1, mbarrier parity = (it >> 1) & 1
     if (MODE == DM_CG) {
         __syncthreads();  // s_ctrl loaded
         if (s_ctrl.done) goto finalize;  // converged before the first iteration (setup pass)
     }
   for (;;) {  // CG iterations (DM_CG); one pass otherwise
+    const bool tr_on = MODE == DM_CG && cg_it == a.trace_iter;
+    int tr_k = 0;
+    PFF_TR(a.trace, tr_on, 0);
 #pragma unroll
     for (int c = 0; c < kCh; ++c) acc[c] = 0.0;
     acc[kCh - 1] = INFINITY;
@@ -367,6 +373,7 @@ __global__ void __launch_bounds__(kTPB, 3) dmg_iter_chunk(const DmgArgs<R> a)
 
             // bulk copies AND every thread's halo gathers of this chunk (all issued one iteration ago)
             mbar_wait(bar + 2 * st, (it >> 1) & 1);
+            PFF_TR(a.trace, tr_on && tr_k < 24, 1 + 4 * tr_k);
             // ---- prefetch chunk k + 1 into the other stage: bulk copies (with the halo ids of chunk k + 2) and
             // asynchronous halo gathers; the ids it needs arrived with THIS stage.  No register is held in flight.
             if (k + 1 < n_ep) {
@@ -412,6 +419,7 @@ __global__ void __launch_bounds__(kTPB, 3) dmg_iter_chunk(const DmgArgs<R> a)
                 }
             }
             if (!issuer) asm volatile("bar.sync 1, %0;" ::"n"(kWorkers) : "memory");  // workers only
+            PFF_TR(a.trace, tr_on && tr_k < 24, 2 + 4 * tr_k);
 
             // ---- element pass (workers)
             for (int e = tid; e < (issuer ? 0 : cm.n_elem); e += kWorkers) {
@@ -422,6 +430,7 @@ __global__ void __launch_bounds__(kTPB, 3) dmg_iter_chunk(const DmgArgs<R> a)
                 s_slot[e] = q1; s_slot[EC + e] = q2; s_slot[2 * EC + e] = q3;
             }
             __syncthreads();
+            PFF_TR(a.trace, tr_on && tr_k < 24, 3 + 4 * tr_k);
 
             // ---- ordered node gather, q, partial sums
             for (int i = tid; i < nloc; i += kTPB) {
@@ -447,12 +456,16 @@ __global__ void __launch_bounds__(kTPB, 3) dmg_iter_chunk(const DmgArgs<R> a)
                 }
             }
             __syncthreads();  // stage st and the slots are free again
+            PFF_TR(a.trace, tr_on && tr_k < 24, 4 + 4 * tr_k);
+            ++tr_k;
         }
     }
     if (MODE != DM_CG) break;
+    PFF_TR(a.trace, tr_on, 100);
     fence_proxy_async_global();
     // ---- interface nodes (owned by no chunk): ordered sum of the chunk partials, same prologue; grid-wide phase
     grid_barrier(a.ticket + 1, gb_target, (unsigned)G);
+    PFF_TR(a.trace, tr_on, 101);
     // every interior value is final: start streaming the first chunk of the next CG iteration
     if (single_epoch) {
         if (issuer) {
@@ -504,11 +517,14 @@ __global__ void __launch_bounds__(kTPB, 3) dmg_iter_chunk(const DmgArgs<R> a)
             if (two) if_finish(s1, n1);
         }
     }
+    PFF_TR(a.trace, tr_on, 102);
     __syncthreads();  // reconverge before the shuffle tree (measured: 10 us per iteration faster than without)
     block_reduce_ch(acc, s_w, s_out);
     if (tid < kCh) a.part[(int64_t)tid * a.part_n + blockIdx.x] = s_out[tid];
+    PFF_TR(a.trace, tr_on, 103);
     fence_proxy_async_global();
     grid_barrier(a.ticket + 1, gb_target, (unsigned)G);
+    PFF_TR(a.trace, tr_on, 104);
     // ---- every value of this iteration is final: the halo gathers of the next iteration's first chunk go out now and
     // fly while the scalars are reduced (they are harmless if the solve turns out to be finished)
     if (pre_issued) {
@@ -548,6 +564,8 @@ __global__ void __launch_bounds__(kTPB, 3) dmg_iter_chunk(const DmgArgs<R> a)
         __syncthreads();
         sc.alpha = s_ctrl.alpha; sc.beta = s_ctrl.beta; sc.first = s_ctrl.first; sc.restart = s_ctrl.restart;
         sc.trunc = s_ctrl.trunc;
+        PFF_TR(a.trace, tr_on, 105);
+        ++cg_it;
         if (s_ctrl.done) {
             if (pre_issued) {  // drain the stage that was streamed ahead before leaving
                 if (!gathers_issued) cp_async_mbar_arrive(bar + 2 * (it & 1));
@@ -846,7 +864,7 @@ static DmgArgs<R> make_args(pff_mesh* m, const pff_state* s)
     a.H = (const R*)s->H; a.x = (R*)s->d;
     a.lb = (R*)m->d_lb; a.r = (R*)m->d_r; a.p = (R*)m->d_p; a.q = (R*)m->d_q; a.dinv = (R*)m->d_dinv;
     a.mask = m->d_mask; a.part = m->d_part; a.part_n = m->n_part_blocks;
-    a.ctrl = m->d_ctrl; a.ticket = m->d_ticket;
+    a.ctrl = m->d_ctrl; a.ticket = m->d_ticket; a.trace = m->d_trace; a.trace_iter = m->trace_iter;
     a.mat = make_matc<R>(m->mat);
     return a;
 }

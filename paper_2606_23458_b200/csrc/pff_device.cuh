@@ -15,6 +15,24 @@ constexpr int kTPB = 256;  // threads per CTA of the chunk kernels
 #endif
 constexpr int kStepTPB = PFF_STEP_TPB;  // threads per CTA of the explicit-step kernel (last warp = producer)
 
+// Phase timestamps of the persistent kernels (instrumentation build only: -DPFF_TRACE, libpff_trace.so; the product
+// library compiles the macro away).  Thread 0 of every CTA stores clock64 and %globaltimer into slot `slot` of its row of
+// the buffer given to pff_trace_set: 256 words per CTA, [0,128) SM cycles, [128,256) nanoseconds.
+#ifdef PFF_TRACE
+#define PFF_TR(buf, on, slot)                                                                             \
+    do {                                                                                                  \
+        if ((buf) && threadIdx.x == 0 && (on)) {                                                          \
+            unsigned long long gt_;                                                                       \
+            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt_));                                        \
+            (buf)[(size_t)blockIdx.x * 256 + (slot)] = clock64();                                         \
+            (buf)[(size_t)blockIdx.x * 256 + 128 + (slot)] = (long long)gt_;                              \
+        }                                                                                                 \
+    } while (0)
+#else
+#define PFF_TR(buf, on, slot) do { } while (0)
+#endif
+constexpr int kTraceStepOffset = 256 * 1024;  // words: the step kernel's rows start here, the CG kernel's at 0
+
 template <typename R>
 struct MatC {  // material constants folded on the host
     R lam;     // lambda_PE or lambda_PS

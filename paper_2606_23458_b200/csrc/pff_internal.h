@@ -106,10 +106,12 @@ struct HostMesh {
     std::vector<double> xy_user;    // copy of the input coordinates (traction lengths)
 };
 
-// Builds everything above. chunk_elems = 0 picks the default and shrinks it until three CTAs fit one SM;
+// Builds everything above. chunk_elems = 0 picks the default: the largest size for which three CTAs fit one SM, then the
+// best-balanced size at or below it for the persistent CG kernel's grid (mesh_setup.cpp);
 // an explicit chunk_elems is only shrunk when a single CTA would not fit.  Returns PFF_OK or an error with `err` filled.
 pff_status build_host_mesh(int64_t n_nodes, const double* xy, int64_t n_elems, const int32_t* tri,
-                           double rho, int order, int chunk_elems, size_t real_bytes, HostMesh& hm, std::string& err);
+                           double rho, int order, int chunk_elems, size_t real_bytes, HostMesh& hm, std::string& err,
+                           int cg_ctas = 0);  // CTAs of the persistent CG kernel on the target GPU (0: a B200's 444)
 
 // Host-side bounds proof of every staged (widened) copy of every chunk; false + `err` on violation (mesh_setup.cpp).
 bool verify_stage_extents(const HostMesh& hm, int64_t ell_total, int64_t n_entries, size_t real_bytes, std::string& err);

@@ -34,6 +34,8 @@ struct pff_mesh {
     pff::StageLayout lay_step{}, lay_mv{}, lay_su{};  // shared-memory stages of the step / CG iteration / setup chunk kernels
     int64_t ell_total = 0;                       // entries of d_ell (padded)
     int64_t n_launches = 0;  // kernels launched so far (pff_mesh_counters)
+    long long* d_trace = nullptr;  // pff_trace_set (instrumentation build)
+    int trace_iter = 3;
     int only_kernel = -1;    // profiling hook: restrict multi-kernel entry points to one kernel (pff_time_kernel)
     // launch configuration of every persistent chunk kernel this mesh has used, keyed by the kernel's address: the grid
     // (CTAs that fit the mesh's device with this mesh's shared-memory stage).  Presence also means the dynamic

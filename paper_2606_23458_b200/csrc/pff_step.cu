@@ -54,6 +54,7 @@ struct StepArgs {
     R *fwx, *fwy;
     R dt, hdt, hdt2, S;
     MatC<R> mat;
+    long long* trace;  // phase timestamps (PFF_TRACE builds)
 };
 
 // Eq. 16 with the Dirichlet overwrite: flagged dofs hold u_bar already (dirichlet_kernel).
@@ -164,6 +165,9 @@ __global__ void __launch_bounds__(kStepTPB, 2) step_chunk_kernel(const StepArgs<
         *Geo<R>::slot(smem, s_shared_slots, 3 * EC, EC) = Geo<R>::pair(R(0), R(0));  // the zero pair (lives in the shared region)
     }
     int it = 0;  // stage uses so far: stage = it & 1, mbarrier parity = (it >> 1) & 1
+    const bool tr_on = MODE == MODE_STEP;
+    int tr_k = 0;
+    PFF_TR(a.trace, tr_on, 0);
     unsigned int gb_epoch = 0;  // thread 0: the barrier counter's value before this launch (read early, used at the barrier)
     if (tid == 0 && a.N_sh > 0) gb_epoch = *reinterpret_cast<volatile unsigned int*>(a.gbar + 1);
     double acc_pq = 0.0;  // MODE_TANGENT: this thread's share of p . q
@@ -226,6 +230,7 @@ __global__ void __launch_bounds__(kStepTPB, 2) step_chunk_kernel(const StepArgs<
             }
             // bulk copies AND every thread's halo gathers of this chunk (all issued one iteration ago)
             mbar_wait(bar + 2 * st, (it >> 1) & 1);
+            PFF_TR(a.trace, tr_on && tr_k < 24, 1 + 4 * tr_k);
             // ---- halo gathers of chunk k + 1 (its halo ids arrived with THIS stage)
             if (k + 1 < n_ep) {
                 const ChunkMeta cn = s_meta[k + 1];
@@ -260,6 +265,7 @@ __global__ void __launch_bounds__(kStepTPB, 2) step_chunk_kernel(const StepArgs<
                 }
             }
             if (!issuer) asm volatile("bar.sync 1, %0;" ::"n"(kWorkers) : "memory");  // workers only
+            PFF_TR(a.trace, tr_on && tr_k < 24, 2 + 4 * tr_k);
 
             // ---- phase 2: fused element pass (workers); nodal force pairs go to the slots corner * EC + e
             for (int e = tid; e < (issuer ? 0 : cm.n_elem); e += kWorkers) {
@@ -287,6 +293,7 @@ __global__ void __launch_bounds__(kStepTPB, 2) step_chunk_kernel(const StepArgs<
                 }
             }
             __syncthreads();
+            PFF_TR(a.trace, tr_on && tr_k < 24, 3 + 4 * tr_k);
 
             // ---- phase 3: ordered gather of each node's incident force pairs, then Eq. 17-18 for interior nodes
             for (int i = tid; i < nloc; i += kStepTPB) {
@@ -321,13 +328,17 @@ __global__ void __launch_bounds__(kStepTPB, 2) step_chunk_kernel(const StepArgs<
                 }
             }
             __syncthreads();  // stage st and the slots are free again
+            PFF_TR(a.trace, tr_on && tr_k < 24, 4 + 4 * tr_k);
+            ++tr_k;
         }
     }
+    PFF_TR(a.trace, tr_on, 100);
     // ---- interface nodes (owned by no chunk), after a grid-wide barrier: ordered sum of the per-chunk partials, then the
     // same Eq. 16-18.  Every read of the OLD interface state by the chunk phase (halo gathers) precedes the barrier.
     if (a.N_sh > 0) {
         unsigned int target = gb_epoch;
         grid_barrier(a.gbar, target, (unsigned)G);
+        PFF_TR(a.trace, tr_on, 101);
         // every CTA has read the epoch before arriving, and all have arrived: publish the next launch's epoch
         if (blockIdx.x == 0 && tid == 0) a.gbar[1] = target;
         // Equal slice per CTA, TWO nodes per thread and trip: all loads of both nodes are issued before anything is computed
@@ -370,6 +381,7 @@ __global__ void __launch_bounds__(kStepTPB, 2) step_chunk_kernel(const StepArgs<
             if (two) if_finish(s1, n1);
         }
     }
+    PFF_TR(a.trace, tr_on, 102);
     if (MODE == MODE_TANGENT && a.pq_part) {  // one ordered block sum per CTA; the caller sums the CTAs in index order
         __shared__ double s_red[32];
         const double t = block_sum(acc_pq, s_red);
@@ -514,6 +526,7 @@ static pff_status launch_step_r(pff_mesh* m, pff_state* s, const pff_bc* bc, dou
     a.dt = R(dt); a.hdt = R(0.5 * dt); a.hdt2 = R(0.5 * dt * dt);
     a.S = R(bc ? bc->load_scale : 1.0);
     a.mat = make_matc<R>(m->mat);
+    a.trace = m->d_trace ? m->d_trace + kTraceStepOffset : nullptr;
     {   // TMA plan: one descriptor per contiguous array the chosen mode reads (kind 0 elements, 1 nodes, 2 gather table)
         const StageLayout& L = m->lay_step;
         a.lay = L;
