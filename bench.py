@@ -367,8 +367,9 @@ def main():
                                       note="q = f_int(u + p) - f_int(u), one pass: conn + geometry per element; u, d, p read, q written per node"),
                 equilibrium=dict(us_per_iteration=1e3 * r["ms_eq"] / max(r["it_eq"], 1), cg_iterations=r["it_eq"],
                                  hbm_frac=(Ne * (12 + 5 * w) + N * 23 * w) * max(r["it_eq"], 1) / (r["ms_eq"] / 1e3) / 1e9 / peak,
-                                 note="pff_equilibrium_solve, bottom edge clamped: per iteration one stiffness-action pass + the "
-                                      "CG vector kernels (du, r, p read + written, q, 1/D read: 16 reals per node)"),
+                                 note="pff_equilibrium_solve, bottom edge clamped: ONE launch per iteration (node prologue with the "
+                                      "previous step, fused stiffness action, gather, sums, scalar step by the last CTA); algorithmic "
+                                      "bytes per iteration = one stiffness-action pass + du, r, p read and written, q, 1/D read"),
                 clocks=r["clk"], gpu_launches=int(r["launches"]),
                 e2e=dict(value=r["e2e_val"], unit=UNIT, h2d_bytes_per_step=r["h2d"], d2h_bytes_per_step=r["d2h"]),
                 roofline=dict(bound="hbm", kernel=dom, achieved=kern[dom]["achieved_gbs"], peak=peak, unit="GB/s",

@@ -240,8 +240,11 @@ pff_status pff_stiffness_action(pff_mesh *mesh, const pff_state *state, const vo
  *     K(u_ref) du = S f_ext - f_int(u_ref)  on the free dofs,   state->u <- u_ref + du,
  * u_ref = state->u on entry (Dirichlet dofs first overwritten with bc->dir_u when it is given; bc->dir_v is not used),
  * S = bc->load_scale, d = state->d fixed, by Jacobi-preconditioned conjugate gradients whose operator is
- * pff_stiffness_action (one fused element pass per iteration); alpha, beta and the norms stay on the device.
- * Stops when ||r_free||_2 <= rel_tol ||r0_free||_2 or after max_iter iterations (PFF_ENOCONV, result written).
+ * pff_stiffness_action: ONE kernel launch per iteration (vector updates of the previous step in the node prologue, fused
+ * element pass, ordered gather, predicted beta); alpha, beta and the norms stay on the device.
+ * Stops when ||r_free||_2 <= rel_tol ||r0_free||_2, after max_iter iterations, or on a breakdown p . K p <= 0 (possible for
+ * the non-isotropic splits, whose shifted difference need not be positive definite): the last two return PFF_ENOCONV with
+ * the steps taken so far applied.
  * Exact equilibrium for the isotropic split (linear problem); for the other splits one step of the paper's shifted-
  * difference iteration (the caller repeats it; exact when du does not change the sign pattern of the split).
  * The constrained problem must be non-singular (enough Dirichlet dofs to remove the rigid-body modes).

@@ -108,10 +108,11 @@ void pff_mesh_destroy(pff_mesh* m)
                     m->d_halo_ids, m->d_sh_rowptr, m->d_halo_dst, m->d_ell, m->d_flags, m->d_halo_part,
                     m->d_fwx, m->d_fwy, m->d_dir_dof, m->d_ca, m->d_cb, m->d_lb, m->d_r, m->d_p, m->d_q, m->d_dinv, m->d_mask,
                     m->d_part, m->d_tally, m->d_ctrl, m->d_ticket, m->d_step_bar, m->d_stage, m->d_hstate, m->d_hdir, m->d_node_old_of_new,
-                    m->d_elem_old_of_new, m->d_n2e_ptr, m->d_n2e, m->d_eq_vec, m->d_eq_part, m->d_eq_sc};
+                    m->d_elem_old_of_new, m->d_n2e_ptr, m->d_n2e, m->d_eq_vec, m->d_eq_part, m->d_eq_ctrl, m->d_eq_ticket};
     for (void* p : ptrs) if (p) cudaFree(p);
     if (m->h_ctrl) cudaFreeHost(m->h_ctrl);
     if (m->h_tally) cudaFreeHost(m->h_tally);
+    if (m->h_eq_ctrl) cudaFreeHost(m->h_eq_ctrl);
     if (m->graph_exec) cudaGraphExecDestroy(m->graph_exec);
     if (m->copy_stream) { cudaStreamSynchronize(m->copy_stream); cudaStreamDestroy(m->copy_stream); }
     if (m->ev_step) cudaEventDestroy(m->ev_step);
@@ -163,6 +164,7 @@ pff_status pff_mesh_create(int64_t n_nodes, const double* xy, int64_t n_elems, c
     }
     m->lay_step = make_stage_layout(0, hm.chunk_elems, hm.node_len, hm.flag_len, hm.ell_len, hm.max_nhalo, m->rb, chunk_kernel_stages(0));
     m->lay_mv = make_stage_layout(1, hm.chunk_elems, hm.node_len, hm.flag_len, hm.ell_len, hm.max_nhalo, m->rb, chunk_kernel_stages(1));
+    m->lay_eq = make_stage_layout(3, hm.chunk_elems, hm.node_len, hm.flag_len, hm.ell_len, hm.max_nhalo, m->rb, chunk_kernel_stages(0));
     m->lay_su = make_stage_layout(2, hm.chunk_elems, hm.node_len, hm.flag_len, hm.ell_len, hm.max_nhalo, m->rb, chunk_kernel_stages(2));
     m->ell_total = (int64_t)hm.ell.size();
     if (!verify_stage_extents(hm, m->ell_total, (int64_t)hm.halo_ids.size(), m->rb, err)) {

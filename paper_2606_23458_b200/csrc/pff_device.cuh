@@ -229,4 +229,51 @@ __device__ __forceinline__ double block_min(double v, double* s_red)
     return t;
 }
 
+constexpr int kCh = 8;  // partial-sum channels of the CG kernels: p.q, r.z, r.r, z.q, q.Dinv.q, r.q, q.q, min step bound
+
+// true in every thread of the LAST CTA of the grid to get here (self-resetting ticket); its reads that follow see every
+// other CTA's earlier global writes
+__device__ __forceinline__ bool last_block(unsigned int* ticket)
+{
+    __shared__ bool s_last;
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const unsigned t = atomicAdd(ticket, 1u);
+        s_last = (t == gridDim.x - 1);
+        if (s_last) *ticket = 0u;
+    }
+    __syncthreads();
+    if (s_last) __threadfence();
+    return s_last;
+}
+
+// Deterministic block reduction of kCh values at once (channels 0..6 summed, channel 7 minimised): fixed
+// shuffle tree, fixed warp order, two barriers.  Results land in s_out[0..kCh) (visible after the call).
+__device__ __forceinline__ void block_reduce_ch(double v[kCh], double* s_w /* [kCh][32] */, double* s_out /* [kCh] */)
+{
+#pragma unroll
+    for (int c = 0; c < kCh; ++c)
+        for (int o = 16; o > 0; o >>= 1) {
+            const double t = __shfl_xor_sync(0xffffffffu, v[c], o);
+            v[c] = (c == kCh - 1) ? fmin(v[c], t) : v[c] + t;
+        }
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31, nw = (blockDim.x + 31) >> 5;
+    __syncthreads();
+    if (l == 0) {
+#pragma unroll
+        for (int c = 0; c < kCh; ++c) s_w[c * 32 + w] = v[c];
+    }
+    __syncthreads();
+    if (w < kCh) {  // warp c reduces channel c
+        double t = l < nw ? s_w[w * 32 + l] : (w == kCh - 1 ? INFINITY : 0.0);
+        for (int o = 16; o > 0; o >>= 1) {
+            const double u = __shfl_xor_sync(0xffffffffu, t, o);
+            t = (w == kCh - 1) ? fmin(t, u) : t + u;
+        }
+        if (l == 0) s_out[w] = t;
+    }
+    __syncthreads();
+}
+
 }  // namespace pff

@@ -27,9 +27,11 @@ struct ChunkMeta {
 //                           staged geometry and corner 3 follows contiguously (pair index); fp32: separate pair slots
 //   kind 1: damage iteration  x r p q 1/D lb + mask; scalar slots [3 EC + 1]
 //   kind 2: damage setup      x; scalar slots q, D, b each [3 EC + 1]
+//   kind 3: quasi-static CG iteration (explicit-step kernel, MODE_EQ): 13 nodal arrays u_x u_y d p_x p_y r_x r_y q_x q_y
+//                           1/D_x 1/D_y du_x du_y, no history array; force-pair slots as kind 0
 struct StageLayout {
     // offsets relative to the base of a stage (stage s starts at s * stage_bytes)
-    uint32_t lconn, geo, area, H, node[10], flags, ell;
+    uint32_t lconn, geo, area, H, node[13], flags, ell;
     uint32_t hids, hflag, hdst;  // per halo node: global id, the 32-bit word holding its flag byte, its partial slot
     uint32_t hnext;              // global ids of the NEXT chunk's halo nodes (arrive with this stage, feed its gathers)
     uint32_t stage_bytes, n_stages;
@@ -52,8 +54,8 @@ inline StageLayout make_stage_layout(int kind, int EC, int node_len, int flag_le
     L.lconn = o; o += up16(size_t(8) * EC);
     L.geo = o; o += up16(size_t(4) * rb * EC);
     L.area = o; o += up16(kind == 1 ? 0 : rb * EC);  // kind 1 stages the 4 element-operator coefficients as "geometry"
-    L.H = o; o += up16(kind == 1 ? 0 : rb * EC);
-    const int nn = kind == 0 ? 10 : (kind == 1 ? 6 : 1);
+    L.H = o; o += up16(kind == 1 || kind == 3 ? 0 : rb * EC);
+    const int nn = kind == 0 ? 10 : (kind == 1 ? 6 : (kind == 3 ? 13 : 1));
     for (int k = 0; k < nn; ++k) { L.node[k] = o; o += up16(rb * node_len); }
     L.flags = o; o += up16(flag_len);
     L.ell = o; o += up16(size_t(2) * ell_len);
@@ -64,7 +66,7 @@ inline StageLayout make_stage_layout(int kind, int EC, int node_len, int flag_le
     L.stage_bytes = (o + 127) / 128 * 128;
     L.n_stages = uint32_t(n_stages);
     o = L.stage_bytes * uint32_t(n_stages);
-    if (kind == 0) {  // force-pair slots corner * EC + e (+ one zero pair).  fp64: corners 1, 2 overwrite the element's
+    if (kind == 0 || kind == 3) {  // force-pair slots corner * EC + e (+ one zero pair).  fp64: corners 1, 2 overwrite the element's
         // own staged geometry (pair index into the stage's geometry) and only corner 3 + the zero pair live here
         L.slot_base = o; o += up16(rb == 8 ? size_t(16) * (EC + 1) : size_t(8) * (3 * EC + 1));
     }

@@ -31,7 +31,7 @@ struct pff_mesh {
     int device = 0;
     size_t rb = 8;  // bytes per real
     double dt_crit = 0.0;
-    pff::StageLayout lay_step{}, lay_mv{}, lay_su{};  // shared-memory stages of the step / CG iteration / setup chunk kernels
+    pff::StageLayout lay_step{}, lay_mv{}, lay_su{}, lay_eq{};  // shared-memory stages of the step / CG iteration / setup / quasi-static CG kernels
     int64_t ell_total = 0;                       // entries of d_ell (padded)
     int64_t n_launches = 0;  // kernels launched so far (pff_mesh_counters)
     long long* d_trace = nullptr;  // pff_trace_set (instrumentation build)
@@ -93,9 +93,11 @@ struct pff_mesh {
     // quasi-static mechanics solve (pff_equilibrium.cu), allocated at its first call
     int32_t *d_n2e_ptr = nullptr, *d_n2e = nullptr;  // node -> (4 * element + corner) table
     void* d_eq_vec = nullptr;                        // 10 nodal vectors
-    double *d_eq_part = nullptr, *d_eq_sc = nullptr;
-    double* tangent_pq_part = nullptr;  // set around a stiffness-action launch that should also leave the p . q block partials
-    int last_step_grid = 0;             // CTAs of the last step-kernel launch (length of those partials)
+    double* d_eq_part = nullptr;                     // block partials [kCh][grid] of the fused CG iteration
+    DamageCtrl *d_eq_ctrl = nullptr, *h_eq_ctrl = nullptr;  // its recurrence scalars (device; pinned read-back image)
+    unsigned int* d_eq_ticket = nullptr;
+    struct { void *ex, *ey, *rx, *ry, *dix, *diy; } eq{};  // CG vectors of the running quasi-static solve (MODE_EQ launches)
+    int last_step_grid = 0;             // CTAs of the last step-kernel launch
     unsigned int* d_step_bar = nullptr;  // [0] grid-barrier counter of the step kernel, [1] its epoch (both device-maintained)
 
     // host-path staging (pff_run_host)

@@ -22,7 +22,10 @@
 namespace pff {
 
 // MODE_TANGENT: matrix-free stiffness action q = f_int(u + p) - f_int(u) (Eq. 13), both forces in ONE element pass
-enum { MODE_STEP = 0, MODE_INIT = 1, MODE_FORCE = 2, MODE_TANGENT = 3 };
+// MODE_EQ: one WHOLE iteration of the quasi-static mechanics CG (pff_equilibrium.cu) in one pass: the node prologue applies
+// the previous step (du += alpha p, r -= alpha q) and forms p = D^-1 r + beta p, the element pass is MODE_TANGENT's, the
+// gather leaves q = K p and the sums that give alpha and PREDICT beta; the last CTA advances the scalars.
+enum { MODE_STEP = 0, MODE_INIT = 1, MODE_FORCE = 2, MODE_TANGENT = 3, MODE_EQ = 4 };
 
 template <typename R>
 struct StepArgs {
@@ -50,7 +53,12 @@ struct StepArgs {
     const R *fex, *fey;
     R *fx_out, *fy_out, *psi_out;
     const R *px, *py;  // MODE_TANGENT: trial direction
-    double* pq_part;   // MODE_TANGENT, may be null: [gridDim.x] block partials of p . q (fixed order within the block)
+    // MODE_EQ: CG vectors of the quasi-static solve (du, r, p, q in/out; 1/D in), its control block, block partials, ticket
+    R *ex, *ey, *rx, *ry, *cpx, *cpy;
+    const R *dix, *diy;
+    DamageCtrl* eq_ctrl;
+    double* eq_part;   // [kCh][gridDim.x]
+    unsigned int* eq_ticket;
     R *fwx, *fwy;
     R dt, hdt, hdt2, S;
     MatC<R> mat;
@@ -132,6 +140,42 @@ __device__ __forceinline__ void step_halo_gather(const StepArgs<R>& a, const Sta
         cp_async<B>(reinterpret_cast<R*>(stg + L.node[3]) + slot, a.px + gid);
         cp_async<B>(reinterpret_cast<R*>(stg + L.node[4]) + slot, a.py + gid);
     }
+    if (MODE == MODE_EQ) {  // old p, r, old q, 1/D: the prologue of a halo node is recomputed by every chunk that touches it
+        cp_async<B>(reinterpret_cast<R*>(stg + L.node[3]) + slot, a.cpx + gid);
+        cp_async<B>(reinterpret_cast<R*>(stg + L.node[4]) + slot, a.cpy + gid);
+        cp_async<B>(reinterpret_cast<R*>(stg + L.node[5]) + slot, a.rx + gid);
+        cp_async<B>(reinterpret_cast<R*>(stg + L.node[6]) + slot, a.ry + gid);
+        cp_async<B>(reinterpret_cast<R*>(stg + L.node[7]) + slot, a.fx_out + gid);
+        cp_async<B>(reinterpret_cast<R*>(stg + L.node[8]) + slot, a.fy_out + gid);
+        cp_async<B>(reinterpret_cast<R*>(stg + L.node[9]) + slot, a.dix + gid);
+        cp_async<B>(reinterpret_cast<R*>(stg + L.node[10]) + slot, a.diy + gid);
+    }
+}
+
+// Scalar step of the quasi-static CG, run by one thread of the last CTA of a MODE_EQ launch after the fixed-order sums
+// t[] = p.q, r.z, r.r (residual BEFORE the coming step), z.q, q.Dinv.q, r.q, q.q.  Same predicted-beta recurrence as the
+// damage CG (pff_damage.cu): r.z and r.r after the step follow from the sums of this pass, so the next pass can form
+// p = z + beta p in its prologue.  Stops on ||r|| <= tol ||r0||, on the iteration cap, or on a breakdown p.Kp <= 0 (the
+// shifted difference of a non-isotropic split need not be positive definite): then no step is applied along p.
+__device__ __forceinline__ void eq_scalar_step(DamageCtrl* c, const double* t)
+{
+    const double pq = t[0], rz = t[1], rr = t[2];
+    if (c->first) { c->nb = sqrt(rr); c->first = 0; }
+    c->pending = 0;
+    c->relres = c->nb > 0.0 ? sqrt(rr) / c->nb : 0.0;
+    const double lim = c->tol * c->nb;
+    if (sqrt(rr) <= lim) { c->done = 1; c->status = PFF_OK; return; }
+    if (c->iters >= c->max_iter) { c->done = 1; c->status = PFF_ENOCONV; return; }
+    if (!(pq > 0.0) || !isfinite(pq)) { c->done = 1; c->status = PFF_ENOCONV; c->restart = 1; return; }  // restart = breakdown flag
+    c->iters += 1;
+    const double alpha = rz / pq;
+    const double rz_pred = fmax(rz - 2.0 * alpha * t[3] + alpha * alpha * t[4], 0.0);
+    const double rr_pred = rr - 2.0 * alpha * t[5] + alpha * alpha * t[6];
+    c->alpha = alpha; c->rz = rz;
+    c->beta = rz > 0.0 ? rz_pred / rz : 0.0;
+    c->pending = 1;  // du += alpha p is applied by the next pass (or by the finish kernel)
+    const double err = 64.0 * 2.220446049250313e-16 * (rr + 2.0 * alpha * fabs(t[5]) + alpha * alpha * t[6]);
+    if (rr_pred + err <= lim * lim) { c->done = 1; c->status = PFF_OK; c->relres = sqrt(fmax(rr_pred, 0.0)) / c->nb; }
 }
 
 // PERSISTENT, double-buffered explicit-step kernel: gridDim.x CTAs, CTA b owns chunks b, b + G, b + 2G, ...
@@ -170,7 +214,21 @@ __global__ void __launch_bounds__(kStepTPB, 2) step_chunk_kernel(const StepArgs<
     PFF_TR(a.trace, tr_on, 0);
     unsigned int gb_epoch = 0;  // thread 0: the barrier counter's value before this launch (read early, used at the barrier)
     if (tid == 0 && a.N_sh > 0) gb_epoch = *reinterpret_cast<volatile unsigned int*>(a.gbar + 1);
-    double acc_pq = 0.0;  // MODE_TANGENT: this thread's share of p . q
+    // MODE_EQ: the recurrence scalars of this iteration (written by the previous launch, or by the host for the first one)
+    // and this thread's share of the seven sums p.q, r.z, r.r, z.q, q.Dinv.q, r.q, q.q (channels of cg scalar step)
+    __shared__ DamageCtrl s_eq;
+    __shared__ double s_w[MODE == MODE_EQ ? kCh * 32 : 1], s_out[kCh];
+    double acc[kCh];
+    R eq_alpha = R(0), eq_beta = R(0);
+    bool eq_first = true;
+    if (MODE == MODE_EQ) {
+        if (tid == 0) s_eq = *a.eq_ctrl;
+        __syncthreads();
+        if (s_eq.done) return;  // converged (or broke down) in an earlier launch of this batch: nothing to do
+        eq_alpha = R(s_eq.alpha); eq_beta = R(s_eq.beta); eq_first = s_eq.first != 0;
+#pragma unroll
+        for (int c = 0; c < kCh; ++c) acc[c] = 0.0;
+    }
     for (int e0 = 0; e0 < n_my; e0 += kMetaCap) {
         const int n_ep = min(kMetaCap, n_my - e0);
         __syncthreads();  // previous epoch fully consumed (also publishes the mbarrier init)
@@ -210,6 +268,17 @@ __global__ void __launch_bounds__(kStepTPB, 2) step_chunk_kernel(const StepArgs<
             const R* s_fex = reinterpret_cast<const R*>(stg + L.node[7]);
             const R* s_fey = reinterpret_cast<const R*>(stg + L.node[8]);
             const R* s_minv = reinterpret_cast<const R*>(stg + L.node[9]);
+            // MODE_EQ (layout kind 3): [3],[4] = p, [5],[6] = r, [7],[8] = old q, [9],[10] = 1/D, [11],[12] = du
+            R* s_px = reinterpret_cast<R*>(stg + L.node[3]);
+            R* s_py = reinterpret_cast<R*>(stg + L.node[4]);
+            R* s_rx = reinterpret_cast<R*>(stg + L.node[5]);
+            R* s_ry = reinterpret_cast<R*>(stg + L.node[6]);
+            const R* s_qx = reinterpret_cast<const R*>(stg + L.node[7]);
+            const R* s_qy = reinterpret_cast<const R*>(stg + L.node[8]);
+            const R* s_dix = reinterpret_cast<const R*>(stg + L.node[9]);
+            const R* s_diy = reinterpret_cast<const R*>(stg + L.node[MODE == MODE_EQ ? 10 : 9]);
+            const R* s_ex = reinterpret_cast<const R*>(stg + L.node[MODE == MODE_EQ ? 11 : 9]);
+            const R* s_ey = reinterpret_cast<const R*>(stg + L.node[MODE == MODE_EQ ? 12 : 9]);
             const uint8_t* s_flags = stg + L.flags;
             const uint16_t* s_ell = reinterpret_cast<const uint16_t*>(stg + L.ell);
             const ChunkMeta cm = s_meta[k];
@@ -264,6 +333,35 @@ __global__ void __launch_bounds__(kStepTPB, 2) step_chunk_kernel(const StepArgs<
                     s_uy[s] = (fl & 2) ? uy : py;
                 }
             }
+            // ---- MODE_EQ phase 1: CG node prologue for every local node (halo nodes redundantly, from gathered values):
+            // apply the previous step, form the new direction in the p slots; interior nodes are written back
+            if (MODE == MODE_EQ && !issuer) {
+                for (int i = tid; i < nloc; i += kWorkers) {
+                    const bool interior = i < cm.n_int;
+                    const int s = interior ? shift + i : hb + (i - cm.n_int);
+                    const R dx = s_dix[s], dy = s_diy[s];  // 0 on constrained dofs: r, p stay 0 there
+                    R rx = s_rx[s], ry = s_ry[s], px = s_px[s], py = s_py[s];
+                    if (!eq_first) {
+                        rx = dx != R(0) ? rfma(-eq_alpha, s_qx[s], rx) : R(0);
+                        ry = dy != R(0) ? rfma(-eq_alpha, s_qy[s], ry) : R(0);
+                        if (interior) {
+                            const int gid = cm.node_start + i;
+                            a.ex[gid] = rfma(eq_alpha, px, s_ex[s]); a.ey[gid] = rfma(eq_alpha, py, s_ey[s]);
+                            a.rx[gid] = rx; a.ry[gid] = ry;
+                        }
+                    }
+                    const R zx = dx * rx, zy = dy * ry;
+                    px = eq_first ? zx : rfma(eq_beta, px, zx);
+                    py = eq_first ? zy : rfma(eq_beta, py, zy);
+                    s_px[s] = px; s_py[s] = py; s_rx[s] = rx; s_ry[s] = ry;
+                    if (interior) {
+                        const int gid = cm.node_start + i;
+                        a.cpx[gid] = px; a.cpy[gid] = py;
+                        acc[1] += double(rx) * double(zx) + double(ry) * double(zy);
+                        acc[2] += double(rx) * double(rx) + double(ry) * double(ry);
+                    }
+                }
+            }
             if (!issuer) asm volatile("bar.sync 1, %0;" ::"n"(kWorkers) : "memory");  // workers only
             PFF_TR(a.trace, tr_on && tr_k < 24, 2 + 4 * tr_k);
 
@@ -275,7 +373,7 @@ __global__ void __launch_bounds__(kStepTPB, 2) step_chunk_kernel(const StepArgs<
                 R psi_p, f[6];
                 element_forces<R, SPLIT>(a.mat, b1, c1, b2, c2, s_area[e], s_ux[c.x], s_uy[c.x], s_ux[c.y], s_uy[c.y], s_ux[c.z],
                                          s_uy[c.z], s_d[c.x] + s_d[c.y] + s_d[c.z], psi_p, f);
-                if (MODE == MODE_TANGENT) {  // Eq. 13: f_int(u + p) - f_int(u), element by element (s_vx, s_vy hold p)
+                if (MODE == MODE_TANGENT || MODE == MODE_EQ) {  // Eq. 13: f_int(u + p) - f_int(u), element by element (s_vx, s_vy hold p)
                     R f1[6], pp1;
                     element_forces<R, SPLIT>(a.mat, b1, c1, b2, c2, s_area[e], s_ux[c.x] + s_vx[c.x], s_uy[c.x] + s_vy[c.x],
                                              s_ux[c.y] + s_vx[c.y], s_uy[c.y] + s_vy[c.y], s_ux[c.z] + s_vx[c.z],
@@ -306,8 +404,15 @@ __global__ void __launch_bounds__(kStepTPB, 2) step_chunk_kernel(const StepArgs<
                 }
                 if (i < cm.n_int) {
                     const int gid = cm.node_start + i, s = shift + i;
-                    if (MODE == MODE_TANGENT) acc_pq += double(s_vx[s]) * double(fx) + double(s_vy[s]) * double(fy);
-                    if (MODE == MODE_FORCE || MODE == MODE_TANGENT) { a.fx_out[gid] = fx; a.fy_out[gid] = fy; continue; }
+                    if (MODE == MODE_EQ) {  // q = K p of an interior node and its share of the sums (free dofs: 1/D != 0)
+                        const double qx = double(fx), qy = double(fy), dx = double(s_dix[s]), dy = double(s_diy[s]);
+                        const double rx = double(s_rx[s]), ry = double(s_ry[s]);
+                        acc[0] += double(s_px[s]) * qx + double(s_py[s]) * qy;
+                        acc[3] += dx * rx * qx + dy * ry * qy; acc[4] += dx * qx * qx + dy * qy * qy;
+                        acc[5] += rx * qx + ry * qy;
+                        acc[6] += (dx != 0.0 ? qx * qx : 0.0) + (dy != 0.0 ? qy * qy : 0.0);
+                    }
+                    if (MODE == MODE_FORCE || MODE == MODE_TANGENT || MODE == MODE_EQ) { a.fx_out[gid] = fx; a.fy_out[gid] = fy; continue; }
                     const uint8_t fl = s_flags[fshift + i];
                     const R minv = s_minv[s];
                     R axn = (a.S * s_fex[s] - fx) * minv;
@@ -343,11 +448,17 @@ __global__ void __launch_bounds__(kStepTPB, 2) step_chunk_kernel(const StepArgs<
         if (blockIdx.x == 0 && tid == 0) a.gbar[1] = target;
         // Equal slice per CTA, TWO nodes per thread and trip: all loads of both nodes are issued before anything is computed
         // or stored, so a trip costs one memory round trip (the slice is ~1.7 nodes per thread at 10^6 nodes).
-        struct IfNode { R fx, fy, ux, uy, vx, vy, ax, ay, fex, fey, minv, px, py; uint8_t fl; };
+        struct IfNode { R fx, fy, ux, uy, vx, vy, ax, ay, fex, fey, minv, px, py, rx, ry, qx, qy, dx, dy, ex, ey; uint8_t fl; };
         auto if_load = [&](int s, IfNode& v) {
             const int gid = a.N_int + s;
             v.fx = iface_sum<R>(a.halo_part, s, a.N_sh, a.n_ovf, a.sh_rowptr);
             v.fy = iface_sum<R>(a.halo_part + a.n_slots, s, a.N_sh, a.n_ovf, a.sh_rowptr);
+            if (MODE == MODE_EQ) {  // CG state of an interface node (u is not needed: the element pass is over)
+                v.px = a.cpx[gid]; v.py = a.cpy[gid]; v.rx = a.rx[gid]; v.ry = a.ry[gid];
+                v.dx = a.dix[gid]; v.dy = a.diy[gid];
+                if (!eq_first) { v.qx = a.fx_out[gid]; v.qy = a.fy_out[gid]; v.ex = a.ex[gid]; v.ey = a.ey[gid]; }
+                return;
+            }
             v.ux = a.ux[gid]; v.uy = a.uy[gid];
             if (MODE == MODE_STEP) { v.vx = a.vx[gid]; v.vy = a.vy[gid]; v.ax = a.ax[gid]; v.ay = a.ay[gid]; }
             if (MODE == MODE_STEP || MODE == MODE_INIT) { v.fl = a.flags[gid]; v.minv = a.minv[gid]; v.fex = a.fex[gid]; v.fey = a.fey[gid]; }
@@ -355,7 +466,27 @@ __global__ void __launch_bounds__(kStepTPB, 2) step_chunk_kernel(const StepArgs<
         };
         auto if_finish = [&](int s, const IfNode& v) {  // the same Eq. 16-18 as predict() + finish_node(), from the loaded values
             const int gid = a.N_int + s;
-            if (MODE == MODE_TANGENT) acc_pq += double(v.px) * double(v.fx) + double(v.py) * double(v.fy);
+            if (MODE == MODE_EQ) {  // the same prologue as in the chunk phase, then q = K p from the ordered partials
+                R rx = v.rx, ry = v.ry, px = v.px, py = v.py;
+                if (!eq_first) {
+                    rx = v.dx != R(0) ? rfma(-eq_alpha, v.qx, rx) : R(0);
+                    ry = v.dy != R(0) ? rfma(-eq_alpha, v.qy, ry) : R(0);
+                    a.ex[gid] = rfma(eq_alpha, px, v.ex); a.ey[gid] = rfma(eq_alpha, py, v.ey);
+                    a.rx[gid] = rx; a.ry[gid] = ry;
+                }
+                const R zx = v.dx * rx, zy = v.dy * ry;
+                px = eq_first ? zx : rfma(eq_beta, px, zx);
+                py = eq_first ? zy : rfma(eq_beta, py, zy);
+                a.cpx[gid] = px; a.cpy[gid] = py; a.fx_out[gid] = v.fx; a.fy_out[gid] = v.fy;
+                const double qx = double(v.fx), qy = double(v.fy), dx = double(v.dx), dy = double(v.dy);
+                acc[0] += double(px) * qx + double(py) * qy;
+                acc[1] += double(rx) * double(zx) + double(ry) * double(zy);
+                acc[2] += double(rx) * double(rx) + double(ry) * double(ry);
+                acc[3] += dx * double(rx) * qx + dy * double(ry) * qy; acc[4] += dx * qx * qx + dy * qy * qy;
+                acc[5] += double(rx) * qx + double(ry) * qy;
+                acc[6] += (dx != 0.0 ? qx * qx : 0.0) + (dy != 0.0 ? qy * qy : 0.0);
+                return;
+            }
             if (MODE == MODE_FORCE || MODE == MODE_TANGENT) { a.fx_out[gid] = v.fx; a.fy_out[gid] = v.fy; return; }
             R axn = (a.S * v.fex - v.fx) * v.minv;
             R ayn = (a.S * v.fey - v.fy) * v.minv;
@@ -382,10 +513,27 @@ __global__ void __launch_bounds__(kStepTPB, 2) step_chunk_kernel(const StepArgs<
         }
     }
     PFF_TR(a.trace, tr_on, 102);
-    if (MODE == MODE_TANGENT && a.pq_part) {  // one ordered block sum per CTA; the caller sums the CTAs in index order
-        __shared__ double s_red[32];
-        const double t = block_sum(acc_pq, s_red);
-        if (tid == 0) a.pq_part[blockIdx.x] = t;
+    if (MODE == MODE_EQ) {
+        // ---- one ordered block reduction per CTA; the LAST CTA to finish sums the block partials in index order and
+        // advances the recurrence scalars for the next launch (alpha, predicted beta, convergence: eq_scalar_step)
+        acc[kCh - 1] = INFINITY;
+        __syncthreads();
+        block_reduce_ch(acc, s_w, s_out);
+        if (tid < kCh) a.eq_part[(size_t)tid * G + blockIdx.x] = s_out[tid];
+        if (last_block(a.eq_ticket)) {
+            const int w = tid >> 5;
+            if (w < kCh - 1) {
+                double v = 0.0;
+                for (int i = lane; i < G; i += 32) v += __ldcg(a.eq_part + (size_t)w * G + i);
+                for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+                if (lane == 0) s_out[w] = v;
+            }
+            __syncthreads();
+            if (tid == 0) {
+                eq_scalar_step(&s_eq, s_out);
+                *a.eq_ctrl = s_eq;
+            }
+        }
     }
 }
 
@@ -474,7 +622,9 @@ static pff_status launch_step_t(pff_mesh* m, const StepArgs<R>& a)
     } else {
         auto kern = step_chunk_kernel<R, SPLIT, MODE>;
         int grid = 0;  // persistent grid: every SM filled with as many CTAs as fit (cached per mesh, with the smem opt-in)
-        pff_status st = persistent_config(m, (const void*)kern, (int)m->lay_step.total, &grid, kStepTPB);
+        const size_t smem = MODE == MODE_EQ ? m->lay_eq.total : m->lay_step.total;
+        if (smem + 4096 > kSmemPerSM) { set_error("quasi-static CG: the chunk does not fit shared memory (use a smaller chunk_elems)"); return PFF_EUNSUPPORTED; }
+        pff_status st = persistent_config(m, (const void*)kern, (int)smem, &grid, kStepTPB);
         if (st != PFF_OK) return st;
         {   // ONE cooperative launch: chunk phase, grid barrier, interface phase (all CTAs co-resident by construction)
             const unsigned g = (unsigned)std::min<int64_t>(grid, hm.C);
@@ -482,7 +632,7 @@ static pff_status launch_step_t(pff_mesh* m, const StepArgs<R>& a)
             b.gbar = m->d_step_bar;
             void* kargs[] = {(void*)&b};
             prof_mark(m, PFF_K_STEP_CHUNK);
-            cudaError_t e = launch_cooperative((const void*)kern, g, kStepTPB, kargs, (size_t)m->lay_step.total, m->stream);
+            cudaError_t e = launch_cooperative((const void*)kern, g, kStepTPB, kargs, smem, m->stream);
             prof_mark(m, PFF_K_STEP_CHUNK);
             if (e != cudaSuccess) return cuda_check(e, "explicit step: cooperative launch");
             m->last_step_grid = (int)g;
@@ -521,14 +671,19 @@ static pff_status launch_step_r(pff_mesh* m, pff_state* s, const pff_bc* bc, dou
     a.d = (const R*)s->d; a.H = (R*)s->H; a.fex = (const R*)s->fext_x; a.fey = (const R*)s->fext_y;
     a.fx_out = (R*)fx; a.fy_out = (R*)fy; a.psi_out = (R*)psi;
     a.px = (const R*)px; a.py = (const R*)py;
-    a.pq_part = mode == MODE_TANGENT ? m->tangent_pq_part : nullptr;
+    if (mode == MODE_EQ) {  // CG vectors and control of the quasi-static solve (pff_equilibrium.cu set them up)
+        a.ex = (R*)m->eq.ex; a.ey = (R*)m->eq.ey; a.rx = (R*)m->eq.rx; a.ry = (R*)m->eq.ry;
+        a.cpx = (R*)const_cast<void*>(px); a.cpy = (R*)const_cast<void*>(py);
+        a.dix = (const R*)m->eq.dix; a.diy = (const R*)m->eq.diy;
+        a.eq_ctrl = m->d_eq_ctrl; a.eq_part = m->d_eq_part; a.eq_ticket = m->d_eq_ticket;
+    }
     a.fwx = (R*)m->d_fwx; a.fwy = (R*)m->d_fwy;
     a.dt = R(dt); a.hdt = R(0.5 * dt); a.hdt2 = R(0.5 * dt * dt);
     a.S = R(bc ? bc->load_scale : 1.0);
     a.mat = make_matc<R>(m->mat);
     a.trace = m->d_trace ? m->d_trace + kTraceStepOffset : nullptr;
     {   // TMA plan: one descriptor per contiguous array the chosen mode reads (kind 0 elements, 1 nodes, 2 gather table)
-        const StageLayout& L = m->lay_step;
+        const StageLayout& L = mode == MODE_EQ ? m->lay_eq : m->lay_step;
         a.lay = L;
         StagePlan& P = a.plan;
         P.n = 0;
@@ -548,7 +703,12 @@ static pff_status launch_step_r(pff_mesh* m, pff_state* s, const pff_bc* bc, dou
             add(s->ax, L.node[5], lr, 1); add(s->ay, L.node[6], lr, 1);
         }
         if (mode == MODE_TANGENT) { add(a.px, L.node[3], lr, 1); add(a.py, L.node[4], lr, 1); }
-        if (mode != MODE_FORCE && mode != MODE_TANGENT) {
+        if (mode == MODE_EQ) {
+            add(a.cpx, L.node[3], lr, 1); add(a.cpy, L.node[4], lr, 1); add(a.rx, L.node[5], lr, 1); add(a.ry, L.node[6], lr, 1);
+            add(a.fx_out, L.node[7], lr, 1); add(a.fy_out, L.node[8], lr, 1); add(a.dix, L.node[9], lr, 1); add(a.diy, L.node[10], lr, 1);
+            add(a.ex, L.node[11], lr, 1); add(a.ey, L.node[12], lr, 1);
+        }
+        if (mode != MODE_FORCE && mode != MODE_TANGENT && mode != MODE_EQ) {
             add(s->fext_x, L.node[7], lr, 1); add(s->fext_y, L.node[8], lr, 1); add(m->d_minv, L.node[9], lr, 1);
             add(m->d_flags, L.flags, 0, 1);
         }
@@ -564,6 +724,9 @@ static pff_status launch_step_r(pff_mesh* m, pff_state* s, const pff_bc* bc, dou
         case MODE_TANGENT:
             if (m->opt.scatter == PFF_SCATTER_ATOMIC) { set_error("stiffness action: gather scatter only"); return PFF_EUNSUPPORTED; }
             return launch_step_s<R, MODE_TANGENT>(m, a);
+        case MODE_EQ:
+            if (m->opt.scatter == PFF_SCATTER_ATOMIC) { set_error("quasi-static CG: gather scatter only"); return PFF_EUNSUPPORTED; }
+            return launch_step_s<R, MODE_EQ>(m, a);
     }
     return PFF_EINVAL;
 }

@@ -81,7 +81,14 @@ def test_bisection_chunks_are_more_compact_than_morton_ranges(lib):
     ns_b = _plan(lib, cfg["xy"], cfg["tri"], chunk=352, order=2)[4]
     assert ns_b < 0.7 * ns_m
     st, _, _, nc, _, ec, ml, _ = _plan(lib, cfg["xy"], cfg["tri"], chunk=0, order=2)
-    assert st == 0 and ec % 32 == 0 and 256 <= ec <= 512 and nc == -(-len(cfg["tri"]) // ec)
+    assert st == 0 and ec % 32 == 0 and 128 <= ec <= 512 and nc == -(-len(cfg["tri"]) // ec)
+    # balance-aware default (mesh_setup.cpp): 80,000 elements fit ONE round of the CG kernel's 444 CTAs with chunks of 192
+    # (417 chunks) instead of two rounds of 384-element chunks (209 chunks on 209 CTAs would leave half the GPU idle)
+    assert ec == 192 and nc <= 444
+    # at the bench size the largest chunk that keeps 3 CG CTAs per SM stays (11.7 chunks per CTA: nothing to gain)
+    big = config(5, n=1001)
+    st, _, _, nc, ns, ec, _, _ = _plan(lib, big["xy"], big["tri"], chunk=0, order=2)
+    assert st == 0 and (ec, nc, ns) == (384, 5209, 148932)
 
 
 def test_chunk_shrinks_to_fit_shared_memory(lib):
