@@ -408,6 +408,7 @@ def test_damage_subcycling_run_steps():
                 assert orc.damage_solve(rel_tol=1e-12, max_iter=4000)[0] == 0
         stt, iters = mesh.pff_run_steps(st, bc, dt, 30, damage_every=every, rel_tol=1e-12, max_iter=4000)
         assert stt == 0 and iters > 0
+        assert mesh.pff_graph_status() == (True, False)  # 30 steps >= 4 periods: one captured period was replayed
         u, v, a, d, H = gpu_fields(mesh, st)
         assert relmax(u, orc.u) <= 1e-10 and relmax(v, orc.v) <= 1e-10 and relmax(H, orc.H) <= 1e-10
         assert relmax(d, orc.d) <= 1e-10
@@ -557,3 +558,28 @@ def test_two_meshes_alternating_and_grown_dirichlet_set():
         b = mesh.bc()
         b.dir_u = st.ux.data_ptr()
         mesh.pff_explicit_step(st, b, dt)
+
+
+def test_graph_replay_is_bit_identical_to_plain_launches_and_trace_hook_is_gated():
+    """pff_run_steps with the CUDA-graph replay of a captured period against the same run with every kernel launched the
+    ordinary way (pff_set_graph_mode(0)): identical bits in every field and the same iteration tally; a second call with
+    the same arguments reuses the captured graph, a call with another dt re-captures.  The phase-timestamp hook of the
+    instrumentation build is refused by the product library (PFF_EUNSUPPORTED)."""
+    import ctypes as C
+    cfg = config(1)
+    outs = []
+    for graph in (True, False):
+        mesh, st = gpu_from(cfg)
+        mesh.pff_set_graph_mode(graph)
+        bc = mesh.bc(load_scale=8.0)
+        dt = 0.5 * mesh.dt_crit
+        mesh.pff_init_accel(st, bc)
+        tally = [mesh.pff_run_steps(st, bc, dt, 40, damage_every=2, rel_tol=1e-10)[1]]
+        tally.append(mesh.pff_run_steps(st, bc, dt, 17, damage_every=2, rel_tol=1e-10)[1])       # cached graph + remainder
+        tally.append(mesh.pff_run_steps(st, bc, 0.9 * dt, 12, damage_every=1, rel_tol=1e-10)[1])  # other arguments: re-capture
+        assert mesh.pff_graph_status() == (graph, False)
+        outs.append([x.copy() for x in gpu_fields(mesh, st)] + [np.array(tally)])
+        if graph:
+            assert mesh.L.pff_trace_set(mesh.h, None, 0) == 6  # PFF_EUNSUPPORTED in the product build
+    for a, b in zip(*outs):
+        assert np.array_equal(a, b)
