@@ -129,6 +129,8 @@ def run_ours(args, rank: int, world: int):
         mesh.pff_set_damage_dirichlet(cfg["notch"])
     if args.no_graph:
         mesh.pff_set_graph_mode(False)
+    if args.cg == "two-rendezvous":
+        mesh.pff_set_cg_variant(1)
     N, Ne = mesh.n_nodes, mesh.n_elems
     dt = cfg["dt_factor"] * mesh.dt_crit
     bc = mesh.bc()
@@ -292,6 +294,8 @@ def main():
     ap.add_argument("--l0-over-h", type=float, default=None,
                     help="config 5 only: regularisation length in mesh widths (default 0.5, the BASELINE recipe); larger values make the "
                          "damage operator diffusion-dominated and raise the Jacobi-PCG iteration count (PAPER.md L175, L217)")
+    ap.add_argument("--cg", default="auto", choices=["auto", "two-rendezvous"],
+                    help="CG kernel of the damage solve: auto = the one-rendezvous kernel where it applies (AT2), or always the two-rendezvous one")
     ap.add_argument("--no-graph", action="store_true", help="pff_run_steps launches every kernel itself instead of replaying a captured period")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -348,6 +352,7 @@ def main():
                 config=dict(workload=args.workload, scatter=args.scatter, name=r["cfg"]["name"], n_nodes=N, n_elems=Ne, rel_tol=REL_TOL,
                             cg_iters_per_solve=iters_total / K, chunks=r["mesh"].n_chunks, interface_nodes=r["mesh"].n_shared,
                             l2="working set > L2 (no flush needed)" if ab["step"] > 126e6 else "L2-resident workload",
+                            cg_kernel=args.cg,
                             l0_over_h=args.l0_over_h if args.l0_over_h is not None else "recipe",
                             time_loop="plain launches" if args.no_graph else "CUDA graph replay of one captured step + solve",
                             parallelism=f"replicas x{world}"),

@@ -179,6 +179,14 @@ pff_status pff_damage_solve(pff_mesh *mesh, pff_state *state, double rel_tol, in
  * with a fixed reduction order.  Synchronises the stream. */
 pff_status pff_energies(pff_mesh *mesh, const pff_state *state, double out[4]);
 
+/* Which kernel runs the CG iterations of pff_damage_solve / pff_damage_adjoint.  0 (default): chosen per solve -- unconstrained
+ * solves (AT2, adjoint) on meshes without overflow partial slots run the ONE-rendezvous kernel (Chronopoulos-Gear form of
+ * CG: the operator is applied to z = D^-1 r, s = A p follows by recurrence, both inner products are linear in the applied
+ * operator so the interface sums are deferred into the next pass; one grid barrier per pass, no interface phase, one pass
+ * more per solve); AT1 (projected CG, L181) always runs the two-rendezvous kernel.  1: always the two-rendezvous kernel.
+ * Both converge to the same unique solution; iteration counts differ by the extra pass. */
+pff_status pff_set_cg_variant(pff_mesh *mesh, int32_t variant);
+
 /* Counters of the last pff_damage_solve / pff_damage_adjoint of this mesh (of ALL solves of the last pff_run_steps):
  * restarts = how often the projected solver (AT1, L181) re-derived its free set after the first time (a bound became
  * inactive, or a step was truncated); truncations = steps cut short at the first bound hit.  Both 0 for AT2.

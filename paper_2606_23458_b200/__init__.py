@@ -153,6 +153,9 @@ class Mesh:
                     allow=(PFF_ENOCONV,) if allow_noconv else ())
         return st, it.value, rr.value
 
+    def pff_set_cg_variant(self, variant: int):
+        _check(self.L.pff_set_cg_variant(self.h, int(variant)))
+
     def pff_damage_last_stats(self):
         """(restarts, truncations) of the projected solver in the last solve / summed over the last pff_run_steps."""
         r, t = C.c_int32(0), C.c_int32(0)

@@ -107,7 +107,7 @@ void pff_mesh_destroy(pff_mesh* m)
     void* ptrs[] = {m->d_meta, m->d_lconn, m->d_conn, m->d_ga, m->d_gb, m->d_area, m->d_minv, m->d_mass,
                     m->d_halo_ids, m->d_sh_rowptr, m->d_halo_dst, m->d_ell, m->d_flags, m->d_halo_part,
                     m->d_fwx, m->d_fwy, m->d_dir_dof, m->d_ca, m->d_cb, m->d_lb, m->d_r, m->d_p, m->d_q, m->d_dinv, m->d_mask,
-                    m->d_part, m->d_tally, m->d_ctrl, m->d_ticket, m->d_step_bar, m->d_stage, m->d_hstate, m->d_hdir, m->d_node_old_of_new,
+                    m->d_part, m->d_tally, m->d_cg2, m->d_ctrl, m->d_ticket, m->d_step_bar, m->d_stage, m->d_hstate, m->d_hdir, m->d_node_old_of_new,
                     m->d_elem_old_of_new, m->d_n2e_ptr, m->d_n2e, m->d_eq_vec, m->d_eq_part, m->d_eq_ctrl, m->d_eq_ticket};
     for (void* p : ptrs) if (p) cudaFree(p);
     if (m->h_ctrl) cudaFreeHost(m->h_ctrl);
@@ -510,6 +510,13 @@ pff_status pff_trace_set(pff_mesh* m, void* device_words, int32_t cg_iteration)
     set_error("pff_trace_set: this build has no phase timestamps (build with python -m paper_2606_23458_b200.build --trace)");
     return PFF_EUNSUPPORTED;
 #endif
+}
+
+pff_status pff_set_cg_variant(pff_mesh* m, int32_t variant)
+{
+    if (!m || variant < 0 || variant > 1) { set_error("pff_set_cg_variant: null mesh or variant not 0 / 1"); return PFF_EINVAL; }
+    m->cg_variant = variant;
+    return PFF_OK;
 }
 
 pff_status pff_graph_status(const pff_mesh* m, int32_t* captured, int32_t* refused)

@@ -59,6 +59,7 @@ struct DmgArgs {
     const R* rhs;
     const uint8_t* free_in;
     int no_clamp;
+    int zero_dinv_fixed;  // setup pass: store 1/D = 0 on nodes outside the free set (the one-rendezvous CG masks with it)
     R *q_out, *b_out, *D_out;
     double* part;    // [kCh][part_n] chunk-kernel block partials
     int64_t part_n;
@@ -229,7 +230,7 @@ template <typename R, int MODE, bool PROJ>
 __global__ void __launch_bounds__(kTPB, 3) dmg_iter_chunk(const DmgArgs<R> a)
 {
     extern __shared__ __align__(128) unsigned char smem[];
-    __shared__ double s_w[kCh * 32], s_out[kCh];
+    __shared__ double s_w[kCh * kRedWarps], s_out[kCh];
     constexpr int A = 16 / sizeof(R);
     __shared__ DamageCtrl s_ctrl;  // every CTA keeps its own, identical copy of the recurrence scalars
     IterScalars sc{0.0, 0.0, 1, 1, 0};
@@ -564,6 +565,10 @@ finalize:
     }
 }
 
+}  // namespace pff
+#include "pff_damage_cg2.cuh"
+namespace pff {
+
 // interface nodes of a plain operator apply (test hook pff_damage_matvec): ordered sum of the chunk partials
 template <typename R>
 __global__ void __launch_bounds__(kTPB) dmg_plain_shared(const DmgArgs<R> a)
@@ -592,7 +597,7 @@ template <typename R, bool HOOK>
 __global__ void __launch_bounds__(kTPB, 2) dmg_setup_chunk(const DmgArgs<R> a)
 {
     extern __shared__ __align__(128) unsigned char smem[];
-    __shared__ double s_w[kCh * 32], s_out[kCh];
+    __shared__ double s_w[kCh * kRedWarps], s_out[kCh];
     constexpr int A = 16 / sizeof(R), B = sizeof(R);
     const StageLayout& L = a.lay;
     R* s_sq = reinterpret_cast<R*>(smem + L.slot_base);
@@ -719,7 +724,7 @@ __global__ void __launch_bounds__(kTPB, 2) dmg_setup_chunk(const DmgArgs<R> a)
                             rhs = fixed ? R(0) : a.rhs[gid];
                         }
                         const R r = rhs - qs;
-                        a.r[gid] = r; a.dinv[gid] = R(1) / Ds; a.lb[gid] = s_x[shift + i];
+                        a.r[gid] = r; a.dinv[gid] = (a.zero_dinv_fixed && fixed) ? R(0) : R(1) / Ds; a.lb[gid] = s_x[shift + i];
                         a.mask[gid] = fixed ? 2 : 1;
                         acc[0] += double(rhs) * double(rhs);
                         if (!fixed) acc[1] += double(r) * double(r);
@@ -763,7 +768,7 @@ __global__ void __launch_bounds__(kTPB, 2) dmg_setup_chunk(const DmgArgs<R> a)
             }
             const R rhs = (adj && v.fixed) ? R(0) : v.rhs;
             const R r = rhs - v.qs;
-            a.r[gid] = r; a.dinv[gid] = R(1) / v.Ds; a.lb[gid] = v.x;
+            a.r[gid] = r; a.dinv[gid] = (a.zero_dinv_fixed && v.fixed) ? R(0) : R(1) / v.Ds; a.lb[gid] = v.x;
             a.mask[gid] = v.fixed ? 2 : 1;
             acc[0] += double(rhs) * double(rhs);
             if (!v.fixed) acc[1] += double(r) * double(r);
@@ -911,18 +916,58 @@ static pff_status damage_solve_t(pff_mesh* m, const pff_state* s, double rel_tol
     const int smem_mv = (int)m->lay_mv.total, smem_su = (int)m->lay_su.total;
     cudaStream_t cs = m->stream;
     int grid_mv = 0, grid_su = 0;
-    if ((st = persistent_config(m, (const void*)dmg_iter_chunk<R, DM_CG, PROJ>, smem_mv, &grid_mv)) != PFF_OK) return st;
+    // Unconstrained solves (AT2, adjoint) on meshes without overflow partial slots run the one-rendezvous kernel
+    // (pff_damage_cg2.cuh) as long as a CTA owns at most 16 chunks: a pass is then 6 % (10^6 nodes) to 33 % (10^4 nodes)
+    // shorter because the grid-wide tail is a large part of it, which pays for the one extra pass per solve; on larger
+    // meshes the tail is amortised and the extra pass is a loss (4e6 nodes, 12 passes: +6 %).  The projected solver (AT1)
+    // and irregular decompositions keep the two-rendezvous kernel.
+    int grid_cg2 = 0;
+    if ((st = persistent_config(m, (const void*)dmg_cg2_chunk<R>, (int)m->lay_mv.total, &grid_cg2)) != PFF_OK) return st;
+    const bool cg2 = !PROJ && m->cg_variant != 1 && hm.n_ovf == 0 && hm.C <= (int64_t)16 * grid_cg2;
+    const void* cg_kernel = cg2 ? (const void*)dmg_cg2_chunk<R> : (const void*)dmg_iter_chunk<R, DM_CG, PROJ>;
+    Cg2Args<R> c2{};
+    if (cg2) {
+        const size_t ld = ((size_t)hm.N + 15) & ~size_t(15);
+        if (!m->d_cg2) {
+            if ((st = cuda_check(cudaMalloc(&m->d_cg2, 6 * ld * m->rb), "damage: second vector set")) != PFF_OK) return st;
+        }
+        R* base = (R*)m->d_cg2;
+        c2.x[0] = a.x; c2.x[1] = base; c2.r[0] = a.r; c2.r[1] = base + ld; c2.p[0] = a.p; c2.p[1] = base + 2 * ld;
+        c2.s[0] = a.q; c2.s[1] = base + 3 * ld; c2.w[0] = base + 4 * ld; c2.w[1] = base + 5 * ld;
+        c2.hpart[0] = a.halo_part; c2.hpart[1] = a.halo_part + m->n_slots;
+        c2.x_out = a.x;
+        asu.zero_dinv_fixed = 1;
+    }
+    if ((st = persistent_config(m, cg_kernel, smem_mv, &grid_mv)) != PFF_OK) return st;
     if ((st = persistent_config(m, (const void*)dmg_setup_chunk<R, false>, smem_su, &grid_su)) != PFF_OK) return st;
     const unsigned gmv = (unsigned)std::min<int64_t>(grid_mv, hm.C), gsu = (unsigned)std::min<int64_t>(grid_su, hm.C);
     asu.tol = rel_tol; asu.max_iter = max_iter;
     a.tally = m->defer ? m->d_tally : nullptr;
+    if (cg2) {  // bulk-copy plans of the two vector sets (StageLayout kind 1 re-read: r, p, s, w, 1/D, halo partial slots)
+        for (int par = 0; par < 2; ++par) {
+            StagePlan& P = par == 0 ? a.plan : c2.plan1;
+            const StageLayout& L = m->lay_mv;
+            P.n = 0;
+            const uint16_t lr = sizeof(R) == 8 ? 3 : 2;
+            auto add = [&](const void* src, uint32_t off, uint16_t l, uint16_t kind) { P.d[P.n++] = StageDesc{src, off, l, kind}; };
+            add(m->d_lconn, L.lconn, 3, 0);
+            if (sizeof(R) == 8) { add(m->d_ca, L.geo, 4, 0); add(m->d_cb, L.geo + 16u * (uint32_t)hm.chunk_elems, 4, 0); }
+            else add(m->d_ca, L.geo, 4, 0);
+            add(m->d_ell, L.ell, 1, 2);
+            add(m->d_halo_dst, L.hdst, 2, 3);
+            add(m->d_halo_ids, L.hnext, 2, 4);
+            add(c2.r[par], L.node[0], lr, 1); add(c2.p[par], L.node[1], lr, 1); add(c2.s[par], L.node[2], lr, 1);
+            add(c2.w[par], L.node[3], lr, 1); add(a.dinv, L.node[4], lr, 1);
+        }
+        c2.d = a;
+    }
     if ((st = launch_setup(m, asu, (const void*)dmg_setup_chunk<R, false>, gsu, smem_su)) != PFF_OK) return st;
     // ONE cooperative launch runs every CG iteration (grid-wide barriers between the chunk phase, the interface
     // phase and the scalar recurrence), applies the last step and the clamp, and writes the control block back
     {
-        void* kargs[] = {(void*)&a};
+        void* kargs[] = {cg2 ? (void*)&c2 : (void*)&a};
         prof_mark(m, PFF_K_MATVEC_CHUNK);
-        cudaError_t e = launch_cooperative((const void*)dmg_iter_chunk<R, DM_CG, PROJ>, gmv, kTPB, kargs, (size_t)smem_mv, cs);
+        cudaError_t e = launch_cooperative(cg_kernel, gmv, kTPB, kargs, (size_t)smem_mv, cs);
         prof_mark(m, PFF_K_MATVEC_CHUNK);
         ++m->n_launches;
         if ((st = cuda_check(e, "damage: cooperative launch")) != PFF_OK) return st;

@@ -229,6 +229,8 @@ __device__ __forceinline__ double block_min(double v, double* s_red)
     return t;
 }
 
+constexpr int kRedWarps = 16;  // warps per CTA the block reductions provide for (scratch: kCh x kRedWarps doubles)
+static_assert(kTPB <= 32 * kRedWarps && kStepTPB <= 32 * kRedWarps, "block reduction scratch too small");
 constexpr int kCh = 8;  // partial-sum channels of the CG kernels: p.q, r.z, r.r, z.q, q.Dinv.q, r.q, q.q, min step bound
 
 // true in every thread of the LAST CTA of the grid to get here (self-resetting ticket); its reads that follow see every
@@ -250,7 +252,7 @@ __device__ __forceinline__ bool last_block(unsigned int* ticket)
 
 // Deterministic block reduction of kCh values at once (channels 0..6 summed, channel 7 minimised): fixed
 // shuffle tree, fixed warp order, two barriers.  Results land in s_out[0..kCh) (visible after the call).
-__device__ __forceinline__ void block_reduce_ch(double v[kCh], double* s_w /* [kCh][32] */, double* s_out /* [kCh] */)
+__device__ __forceinline__ void block_reduce_ch(double v[kCh], double* s_w /* [kCh][kRedWarps] */, double* s_out /* [kCh] */)
 {
 #pragma unroll
     for (int c = 0; c < kCh; ++c)
@@ -262,11 +264,11 @@ __device__ __forceinline__ void block_reduce_ch(double v[kCh], double* s_w /* [k
     __syncthreads();
     if (l == 0) {
 #pragma unroll
-        for (int c = 0; c < kCh; ++c) s_w[c * 32 + w] = v[c];
+        for (int c = 0; c < kCh; ++c) s_w[c * kRedWarps + w] = v[c];
     }
     __syncthreads();
     if (w < kCh) {  // warp c reduces channel c
-        double t = l < nw ? s_w[w * 32 + l] : (w == kCh - 1 ? INFINITY : 0.0);
+        double t = l < nw ? s_w[w * kRedWarps + l] : (w == kCh - 1 ? INFINITY : 0.0);
         for (int o = 16; o > 0; o >>= 1) {
             const double u = __shfl_xor_sync(0xffffffffu, t, o);
             t = (w == kCh - 1) ? fmin(t, u) : t + u;

@@ -25,10 +25,11 @@ struct ChunkMeta {
 // that the padding entries of the gather table point to.
 //   kind 0: explicit step   10 nodal arrays + flags; fp64: the force pairs of corners 1, 2 overwrite the element's own
 //                           staged geometry and corner 3 follows contiguously (pair index); fp32: separate pair slots
-//   kind 1: damage iteration  x r p q 1/D lb + mask; scalar slots [3 EC + 1]
+//   kind 1: damage iteration  x r p q 1/D lb + mask; scalar slots [3 EC + 1]  (one-rendezvous kernel: r p s w 1/D + halo partials)
 //   kind 2: damage setup      x; scalar slots q, D, b each [3 EC + 1]
 //   kind 3: quasi-static CG iteration (explicit-step kernel, MODE_EQ): 13 nodal arrays u_x u_y d p_x p_y r_x r_y q_x q_y
 //                           1/D_x 1/D_y du_x du_y, no history array; force-pair slots as kind 0
+constexpr int kIfaceWidth = 4;  // fixed partial slots per interface node (one per touching chunk)
 struct StageLayout {
     // offsets relative to the base of a stage (stage s starts at s * stage_bytes)
     uint32_t lconn, geo, area, H, node[13], flags, ell;
@@ -43,7 +44,6 @@ struct StageLayout {
     uint32_t bar;          // one mbarrier per stage
     uint32_t total;
 };
-constexpr int kIfaceWidth = 4;  // fixed partial slots per interface node (one per touching chunk)
 constexpr int kMetaCap = 32;  // chunk metas a persistent CTA keeps in shared memory per epoch
 inline StageLayout make_stage_layout(int kind, int EC, int node_len, int flag_len, int ell_len, int max_nhalo, size_t rb,
                                      int n_stages = 1)
@@ -56,7 +56,12 @@ inline StageLayout make_stage_layout(int kind, int EC, int node_len, int flag_le
     L.area = o; o += up16(kind == 1 ? 0 : rb * EC);  // kind 1 stages the 4 element-operator coefficients as "geometry"
     L.H = o; o += up16(kind == 1 || kind == 3 ? 0 : rb * EC);
     const int nn = kind == 0 ? 10 : (kind == 1 ? 6 : (kind == 3 ? 13 : 1));
-    for (int k = 0; k < nn; ++k) { L.node[k] = o; o += up16(rb * node_len); }
+    for (int k = 0; k < nn; ++k) {
+        // kind 1, array 5: the lower bounds of the projected solver, or (one-rendezvous CG kernel) the kIfaceWidth partial
+        // slots of every halo node
+        const int len = (kind == 1 && k == 5) ? (node_len > kIfaceWidth * max_nhalo ? node_len : kIfaceWidth * max_nhalo) : node_len;
+        L.node[k] = o; o += up16(rb * len);
+    }
     L.flags = o; o += up16(flag_len);
     L.ell = o; o += up16(size_t(2) * ell_len);
     L.hids = o; o += up16(size_t(4) * max_nhalo);
@@ -120,7 +125,8 @@ bool verify_stage_extents(const HostMesh& hm, int64_t ell_total, int64_t n_entri
 
 constexpr size_t kSmemPerSM = 227 * 1024;   // usable shared memory of one sm_100a SM / one CTA
 constexpr size_t kSmemCtaReserve = 1024;    // driver-reserved bytes per resident CTA
-constexpr size_t kSmemStatic = 2304;        // static shared memory of the chunk kernels (reduction scratch)
+constexpr size_t kSmemStatic = 1280;        // static shared memory of the damage chunk kernels (reduction scratch 8 x 16 doubles,
+                                            // control block; checked against ptxas: 1,208 B)
 
 void set_error(const std::string& s);
 

@@ -217,7 +217,7 @@ __global__ void __launch_bounds__(kStepTPB, 2) step_chunk_kernel(const StepArgs<
     // MODE_EQ: the recurrence scalars of this iteration (written by the previous launch, or by the host for the first one)
     // and this thread's share of the seven sums p.q, r.z, r.r, z.q, q.Dinv.q, r.q, q.q (channels of cg scalar step)
     __shared__ DamageCtrl s_eq;
-    __shared__ double s_w[MODE == MODE_EQ ? kCh * 32 : 1], s_out[kCh];
+    __shared__ double s_w[MODE == MODE_EQ ? kCh * kRedWarps : 1], s_out[kCh];
     double acc[kCh];
     R eq_alpha = R(0), eq_beta = R(0);
     bool eq_first = true;

@@ -583,3 +583,31 @@ def test_graph_replay_is_bit_identical_to_plain_launches_and_trace_hook_is_gated
             assert mesh.L.pff_trace_set(mesh.h, None, 0) == 6  # PFF_EUNSUPPORTED in the product build
     for a, b in zip(*outs):
         assert np.array_equal(a, b)
+
+
+def test_one_rendezvous_and_two_rendezvous_cg_kernels_agree_with_the_oracle():
+    """The damage solve has two CG kernels (include/pff.h, pff_set_cg_variant): the default for unconstrained solves on
+    meshes of this size is the one-rendezvous kernel (Chronopoulos-Gear recurrence, interface sums deferred into the next
+    pass), variant 1 forces the two-rendezvous kernel that AT1 always uses.  Both are converged to 1e-12 on the jittered,
+    permuted mesh of config 2 after 30 loaded steps and must give the oracle's unique solution; the one-rendezvous kernel
+    needs exactly one operator application more (its first pass only applies the operator to z_0)."""
+    cfg = config(2, scale=0.5)
+    orc = oracle_from(cfg)
+    dt = 0.5 * orc.dt_crit()
+    orc.init_accel(20.0)
+    for _ in range(30):
+        orc.explicit_step(dt, S=20.0)
+    assert orc.damage_solve(rel_tol=1e-12, max_iter=4000)[0] == 0
+    its = []
+    for variant in (0, 1):
+        mesh, st = gpu_from(cfg)
+        mesh.pff_set_cg_variant(variant)
+        mesh.pff_init_accel(st, mesh.bc(load_scale=20.0))
+        for _ in range(30):
+            mesh.pff_explicit_step(st, mesh.bc(load_scale=20.0), dt)
+        stt, it, rr = mesh.pff_damage_solve(st, rel_tol=1e-12, max_iter=4000)
+        assert stt == 0 and rr <= 1e-12
+        d = mesh.nodes_to_user(st.d)
+        assert relmax(d, orc.d) <= TOL64 and np.all(d >= cfg["d0"]) and d.max() <= 1.0
+        its.append(it)
+    assert 0 <= its[0] - its[1] <= 2, its
