@@ -129,8 +129,7 @@ def run_ours(args, rank: int, world: int):
         mesh.pff_set_damage_dirichlet(cfg["notch"])
     if args.no_graph:
         mesh.pff_set_graph_mode(False)
-    if args.cg == "two-rendezvous":
-        mesh.pff_set_cg_variant(1)
+    mesh.pff_set_cg_variant({"auto": 0, "two-rendezvous": 1, "one-rendezvous": 2}[args.cg])
     N, Ne = mesh.n_nodes, mesh.n_elems
     dt = cfg["dt_factor"] * mesh.dt_crit
     bc = mesh.bc()
@@ -181,6 +180,21 @@ def run_ours(args, rank: int, world: int):
     # explicit step and CG iteration timed alone (device-resident), for the secondary metrics
     ms_exp, _ = timed(lambda: mesh.pff_explicit_step(st, bc, dt), args.steps)
 
+    # both CG kernels of the damage solve on this workload (the timed region above used the one `--cg` selects)
+    cg_kernels = {}
+    if cfg["material"]["model"] == 2 and args.scatter == "gather":
+        for name, variant in (("two_rendezvous", 1), ("one_rendezvous", 2)):
+            mesh.pff_set_cg_variant(variant)
+            step()
+            mesh.pff_profile_enable(True)
+            _, it_v = timed(step, min(args.steps, 10))
+            pv = mesh.pff_profile_read()
+            mesh.pff_profile_enable(False)
+            ms_v, n_v = pv["matvec_chunk"]
+            if n_v and sum(it_v):
+                cg_kernels[name] = dict(ms_per_solve=ms_v / n_v, passes_per_solve=sum(it_v) / n_v, us_per_pass=1e3 * ms_v / sum(it_v))
+        mesh.pff_set_cg_variant({"auto": 0, "two-rendezvous": 1, "one-rendezvous": 2}[args.cg])
+
     # backward pass of the damage solve (pff_damage_adjoint, section 4.2), timed alone: seeded upstream gradient,
     # the same setup + cooperative CG kernels as the forward solve
     g_up = torch.from_numpy(np.random.default_rng(7).standard_normal(N).astype(mesh.np_dtype)).to(mesh.device)
@@ -225,7 +239,7 @@ def run_ours(args, rank: int, world: int):
     eq_call = lambda: mesh.pff_equilibrium_solve(st, None, rel_tol=1e-300, max_iter=EQ_ITERS, allow_noconv=True)[1]
     eq_call()
     ms_eq, it_eq = timed(eq_call, 1)
-    return dict(mesh=mesh, cfg=cfg, N=N, Ne=Ne, w=w, ms_total=ms_total, ms_runs=ms_runs, iters=iters, launches=launches, clk=clk, prof=prof,
+    return dict(mesh=mesh, cfg=cfg, N=N, Ne=Ne, w=w, cg_kernels=cg_kernels, ms_total=ms_total, ms_runs=ms_runs, iters=iters, launches=launches, clk=clk, prof=prof,
                 iters_p=iters_p, ms_exp=ms_exp, ms_adj=ms_adj / 5, it_adj=it_adj[0], ms_act=ms_act / args.steps, ms_eq=ms_eq, it_eq=it_eq[0], e2e_val=e2e_val, h2d=(9 * N + Ne) * 8, d2h=(7 * N + Ne) * 8, snapshot=snapshot)
 
 
@@ -294,8 +308,9 @@ def main():
     ap.add_argument("--l0-over-h", type=float, default=None,
                     help="config 5 only: regularisation length in mesh widths (default 0.5, the BASELINE recipe); larger values make the "
                          "damage operator diffusion-dominated and raise the Jacobi-PCG iteration count (PAPER.md L175, L217)")
-    ap.add_argument("--cg", default="auto", choices=["auto", "two-rendezvous"],
-                    help="CG kernel of the damage solve: auto = the one-rendezvous kernel where it applies (AT2), or always the two-rendezvous one")
+    ap.add_argument("--cg", default="auto", choices=["auto", "two-rendezvous", "one-rendezvous"],
+                    help="CG kernel of the damage solve (include/pff.h, pff_set_cg_variant): auto = chosen per solve from the mesh "
+                         "size and the previous solve's pass count")
     ap.add_argument("--no-graph", action="store_true", help="pff_run_steps launches every kernel itself instead of replaying a captured period")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -363,6 +378,7 @@ def main():
                 explicit_step_alone_hbm_frac=ab["step"] / (r["ms_exp"] / K / 1e3) / 1e9 / peak,
                 cg_iterations_per_s=world * iters_prof / (prof["matvec_chunk"][0] / 1e3) if prof["matvec_chunk"][0] else None,
                 cg_iteration_hbm_frac=kern["cg_solve"]["frac"] if "cg_solve" in kern else None,
+                cg_kernels={k: dict(v, hbm_frac=ab["cg_iter"] / (v["us_per_pass"] * 1e-6) / 1e9 / peak) for k, v in r["cg_kernels"].items()},
                 adjoint=dict(ms_per_solve=r["ms_adj"], cg_iterations=r["it_adj"],
                              hbm_frac=(ab["cg_iter"] * r["it_adj"] + ab["matvec"]) / (r["ms_adj"] / 1e3) / 1e9 / peak,
                              note="one pff_damage_adjoint (setup pass + all CG iterations), seeded upstream gradient; "

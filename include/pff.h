@@ -179,12 +179,17 @@ pff_status pff_damage_solve(pff_mesh *mesh, pff_state *state, double rel_tol, in
  * with a fixed reduction order.  Synchronises the stream. */
 pff_status pff_energies(pff_mesh *mesh, const pff_state *state, double out[4]);
 
-/* Which kernel runs the CG iterations of pff_damage_solve / pff_damage_adjoint.  0 (default): chosen per solve -- unconstrained
- * solves (AT2, adjoint) on meshes without overflow partial slots run the ONE-rendezvous kernel (Chronopoulos-Gear form of
- * CG: the operator is applied to z = D^-1 r, s = A p follows by recurrence, both inner products are linear in the applied
- * operator so the interface sums are deferred into the next pass; one grid barrier per pass, no interface phase, one pass
- * more per solve); AT1 (projected CG, L181) always runs the two-rendezvous kernel.  1: always the two-rendezvous kernel.
- * Both converge to the same unique solution; iteration counts differ by the extra pass. */
+/* Which kernel runs the CG iterations of pff_damage_solve / pff_damage_adjoint.
+ *   1: the two-rendezvous kernel (standard Jacobi-PCG recurrence with predicted beta; interface nodes summed in a phase of
+ *      their own between two grid barriers per iteration).  AT1 (projected CG, L181) always runs it.
+ *   2: the ONE-rendezvous kernel wherever it applies (unconstrained solves -- AT2, adjoint -- on meshes without overflow
+ *      partial slots): Chronopoulos-Gear form of CG, the operator is applied to z = D^-1 r, s = A p follows by recurrence,
+ *      both inner products are linear in the applied operator, so the interface sums are deferred into the next pass: one
+ *      grid barrier per pass, no interface phase, one pass more per solve.
+ *   0 (default): chosen per solve from measurements on B200 (profiles/r2_cg_kernels.md): kernel 2 where it applies and a
+ *      CTA of the persistent grid owns at most 4 chunks (up to ~3.5e5 nodes in fp64), or at most 16 chunks (~1.4e6 nodes)
+ *      and the previous solve of this mesh took 20 passes or more; kernel 1 otherwise.
+ * Both converge to the same unique solution (same iterates in exact arithmetic); both are bit-reproducible run to run. */
 pff_status pff_set_cg_variant(pff_mesh *mesh, int32_t variant);
 
 /* Counters of the last pff_damage_solve / pff_damage_adjoint of this mesh (of ALL solves of the last pff_run_steps):

@@ -588,7 +588,7 @@ def test_graph_replay_is_bit_identical_to_plain_launches_and_trace_hook_is_gated
 def test_one_rendezvous_and_two_rendezvous_cg_kernels_agree_with_the_oracle():
     """The damage solve has two CG kernels (include/pff.h, pff_set_cg_variant): the default for unconstrained solves on
     meshes of this size is the one-rendezvous kernel (Chronopoulos-Gear recurrence, interface sums deferred into the next
-    pass), variant 1 forces the two-rendezvous kernel that AT1 always uses.  Both are converged to 1e-12 on the jittered,
+    pass; variant 2 forces it), variant 1 forces the two-rendezvous kernel that AT1 always uses.  Both are converged to 1e-12 on the jittered,
     permuted mesh of config 2 after 30 loaded steps and must give the oracle's unique solution; the one-rendezvous kernel
     needs exactly one operator application more (its first pass only applies the operator to z_0)."""
     cfg = config(2, scale=0.5)
@@ -599,7 +599,7 @@ def test_one_rendezvous_and_two_rendezvous_cg_kernels_agree_with_the_oracle():
         orc.explicit_step(dt, S=20.0)
     assert orc.damage_solve(rel_tol=1e-12, max_iter=4000)[0] == 0
     its = []
-    for variant in (0, 1):
+    for variant in (2, 1):
         mesh, st = gpu_from(cfg)
         mesh.pff_set_cg_variant(variant)
         mesh.pff_init_accel(st, mesh.bc(load_scale=20.0))
