@@ -269,13 +269,15 @@ def test_run_host_matches_device_path():
     assert relmax(H, orc.H) <= 1e-10
 
 
-def test_full_size_bench_configuration_cfg5_1001():
+@pytest.mark.parametrize("cg_variant", [0, 2])
+def test_full_size_bench_configuration_cfg5_1001(cg_variant):
     """BASELINE's metric size (1e6 nodes, 2e6 elements) in the launch configuration bench.py times (library
     defaults: PFF_ORDER_BISECTION, default chunk, gather scatter, fp64 -- the decomposition printed in the bench line's
     `config`): two staggered steps, every node and element compared with the oracle (it finishes this size in seconds)."""
     cfg = config(5, n=1001)
     orc = oracle_from(cfg)
     mesh, st = gpu_from(cfg)
+    mesh.pff_set_cg_variant(cg_variant)  # 0: what bench.py runs (two-rendezvous CG kernel at this size); 2: the one-rendezvous kernel
     assert mesh.n_nodes == 1002001 and mesh.n_elems == 2000000
     assert (mesh.n_chunks, mesh.n_shared) == BENCH_DECOMPOSITION  # what BENCH_r*.json config.chunks / interface_nodes print
     dt = cfg["dt_factor"] * orc.dt_crit()
