@@ -187,8 +187,8 @@ pff_status pff_energies(pff_mesh *mesh, const pff_state *state, double out[4]);
  *      both inner products are linear in the applied operator, so the interface sums are deferred into the next pass: one
  *      grid barrier per pass, no interface phase, one pass more per solve.
  *   0 (default): chosen per solve from measurements on B200 (profiles/r2_cg_kernels.md): kernel 2 where it applies and a
- *      CTA of the persistent grid owns at most 4 chunks (up to ~3.5e5 nodes in fp64), or at most 16 chunks (~1.4e6 nodes)
- *      and the previous solve of this mesh took 20 passes or more; kernel 1 otherwise.
+ *      CTA of the persistent grid owns at most 16 chunks (up to ~1.4e6 nodes in fp64); kernel 1 otherwise (on larger meshes
+ *      the grid-wide tail is amortised and the extra pass costs more than the shorter passes save).
  * Both converge to the same unique solution (same iterates in exact arithmetic); both are bit-reproducible run to run. */
 pff_status pff_set_cg_variant(pff_mesh *mesh, int32_t variant);
 

@@ -444,22 +444,15 @@ pff_status pff_run_steps(pff_mesh* m, pff_state* s, const pff_bc* bc, double dt,
     const bool want_graph = m->graph_mode != 0 && !m->graph_unsupported && !m->prof_on && period <= 64 && n_steps >= 4 * period;
     if (want_graph) {
         // key of everything a captured period depends on (kernel arguments are frozen at capture time)
-        struct Key { pff_state s; pff_bc bc; double dt, tol; int32_t every, max_iter; int64_t n_dir; uint64_t flags_gen; int32_t variant, long_solves; } key{};
+        struct Key { pff_state s; pff_bc bc; double dt, tol; int32_t every, max_iter; int64_t n_dir; uint64_t flags_gen; int32_t variant; } key{};
         key.s = *s; if (bc) key.bc = *bc; else key.bc.load_scale = 1.0;
         key.dt = dt; key.tol = rel_tol; key.every = damage_every; key.max_iter = max_iter; key.n_dir = m->n_dir; key.flags_gen = m->flags_gen;
-        key.variant = m->cg_variant; key.long_solves = m->last_passes >= 20;  // what the choice of the CG kernel depends on
+        key.variant = m->cg_variant;  // decides which CG kernel the frozen period launches
         const unsigned char* kb = reinterpret_cast<const unsigned char*>(&key);
         const bool cached = m->graph_exec && m->graph_key.size() == sizeof(Key) && std::memcmp(m->graph_key.data(), kb, sizeof(Key)) == 0;
         if (!cached) {
             if (m->graph_exec) { cudaGraphExecDestroy(m->graph_exec); m->graph_exec = nullptr; }
             for (; k <= period && st == PFF_OK; ++k) st = one_step(k);  // first period the ordinary way (also does every lazy allocation)
-            if (st == PFF_OK && damage_every > 0) {
-                // how long the solves of this run are decides which CG kernel the frozen period launches: look once
-                st = cuda_check(cudaMemcpyAsync(m->h_tally, m->d_tally, sizeof(RunTally), cudaMemcpyDeviceToHost, m->stream), "pff_run_steps: tally");
-                if (st == PFF_OK) st = cuda_check(cudaStreamSynchronize(m->stream), "pff_run_steps: sync");
-                if (st == PFF_OK && m->h_tally->solves > 0) m->last_passes = (int)(m->h_tally->iters / m->h_tally->solves);
-                key.long_solves = m->last_passes >= 20;
-            }
             if (st == PFF_OK) {
                 const int64_t l0 = m->n_launches;
                 cudaGraph_t graph = nullptr;
@@ -502,7 +495,6 @@ pff_status pff_run_steps(pff_mesh* m, pff_state* s, const pff_bc* bc, double dt,
     if (st != PFF_OK) return st;
     if (e != PFF_OK) return e;
     m->last_restarts = m->h_tally->restarts; m->last_truncs = m->h_tally->truncs;
-    if (m->h_tally->solves > 0) m->last_passes = (int)(m->h_tally->iters / m->h_tally->solves);
     if (cg_iters_total) *cg_iters_total = m->h_tally->iters;
     if (m->h_tally->noconv > 0) { set_error("pff_run_steps: a damage solve reached max_iter"); return PFF_ENOCONV; }
     return PFF_OK;

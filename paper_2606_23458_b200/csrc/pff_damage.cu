@@ -916,19 +916,16 @@ static pff_status damage_solve_t(pff_mesh* m, const pff_state* s, double rel_tol
     const int smem_mv = (int)m->lay_mv.total, smem_su = (int)m->lay_su.total;
     cudaStream_t cs = m->stream;
     int grid_mv = 0, grid_su = 0;
-    // Unconstrained solves (AT2, adjoint) on meshes without overflow partial slots may run the one-rendezvous kernel
-    // (pff_damage_cg2.cuh): its pass is 33 % (10^4 nodes) to 6 % (10^6 nodes) shorter because the grid-wide tail is a large
-    // part of a pass there, at the price of one extra pass per solve.  Measured (profiles/r2_cg_kernels.md): it wins by 20 %
-    // and more up to 10^5 nodes whatever the pass count, at 10^6 nodes from ~20 passes per solve on (-5 % at 85 passes, +2 %
-    // at 12), and loses on larger meshes, where the tail is amortised (4e6 nodes, 12 passes: +6 %).  The automatic choice
-    // follows that: at most 4 chunks per CTA, or at most 16 and the previous solve of this mesh took 20 passes or more.
-    // The projected solver (AT1) and irregular decompositions keep the two-rendezvous kernel.
+    // Unconstrained solves (AT2, adjoint) on meshes without overflow partial slots run the one-rendezvous kernel
+    // (pff_damage_cg2.cuh) as long as a CTA of the persistent grid owns at most 16 chunks (~1.4e6 nodes in fp64): its pass is
+    // 33 % (10^4 nodes) to 7 % (10^6 nodes) shorter because the grid-wide tail is a large part of a pass there, which pays
+    // for its one extra (cheaper) pass per solve: -25 % per solve up to 10^5 nodes, a tie at 10^6 nodes and 12 passes, -5 % at
+    // 85 passes (profiles/r2_cg_kernels.md).  On larger meshes the tail is amortised and the extra pass is a loss (4e6
+    // nodes, 12 passes: +6 %).  The projected solver (AT1) and irregular decompositions keep the two-rendezvous kernel.
     int grid_cg2 = 0;
     if ((st = persistent_config(m, (const void*)dmg_cg2_chunk<R>, (int)m->lay_mv.total, &grid_cg2)) != PFF_OK) return st;
     const bool eligible = !PROJ && hm.n_ovf == 0;
-    const bool cg2 = eligible && (m->cg_variant == 2 ||
-                                  (m->cg_variant == 0 && (hm.C <= (int64_t)4 * grid_cg2 ||
-                                                          (hm.C <= (int64_t)16 * grid_cg2 && m->last_passes >= 20))));
+    const bool cg2 = eligible && (m->cg_variant == 2 || (m->cg_variant == 0 && hm.C <= (int64_t)16 * grid_cg2));
     const void* cg_kernel = cg2 ? (const void*)dmg_cg2_chunk<R> : (const void*)dmg_iter_chunk<R, DM_CG, PROJ>;
     Cg2Args<R> c2{};
     if (cg2) {
@@ -981,7 +978,7 @@ static pff_status damage_solve_t(pff_mesh* m, const pff_state* s, double rel_tol
     DamageCtrl* h = m->h_ctrl;  // pinned download image; the stream is synchronised before it is read or reused
     if ((st = cuda_check(cudaMemcpyAsync(h, m->d_ctrl, sizeof(DamageCtrl), cudaMemcpyDeviceToHost, cs), "damage: ctrl download")) != PFF_OK) return st;
     if ((st = cuda_check(cudaStreamSynchronize(cs), "damage: sync")) != PFF_OK) return st;
-    m->last_restarts = h->restarts; m->last_truncs = h->truncs; m->last_passes = h->iters;
+    m->last_restarts = h->restarts; m->last_truncs = h->truncs;
     if (iters) *iters = h->iters;
     if (relres) *relres = h->relres;
     if (!h->done || h->status == PFF_ENOCONV) {

@@ -11,7 +11,8 @@
 // NEXT pass's node prologue, where every chunk that touches the node sums the (by then complete) partial slots itself.
 // One pass = chunk phase, ONE grid barrier, redundant sum of 3 x G block partials: no interface phase, no second barrier.
 // Same iterates as standard CG in exact arithmetic (tests converge both to 1e-12..1e-13); the price is one vector more
-// (s) read and written per node and one more pass per solve (the first pass only applies the operator to z_0).
+// (s) read and written per node and one more pass per solve (the first pass only applies the operator to z_0; it writes
+// no vector and does not swap the sets).
 //
 // Hazards: a chunk writes the new x, r, p, s of the nodes it owns (its interior nodes; interface nodes belong to the chunk
 // holding their partial slot 0) while other chunks still read the old values of the same interface nodes; and it writes
@@ -97,7 +98,7 @@ __global__ void __launch_bounds__(kTPB, 3) dmg_cg2_chunk(const Cg2Args<R> c)
     int par = 0;  // the set the coming pass reads; it writes par ^ 1
     int pass = 0;
     double alpha = 0.0, beta = 0.0;
-    bool first = true;
+    bool first = true, second = false;  // the pass that only applies the operator to z_0; the one after it
     __syncthreads();
     if (s_ctrl.done) goto finalize;  // the warm start already satisfies the stopping test (setup pass)
 
@@ -107,6 +108,7 @@ __global__ void __launch_bounds__(kTPB, 3) dmg_cg2_chunk(const Cg2Args<R> c)
         PFF_TR(a.trace, tr_on, 0);
         double acc_g = 0.0, acc_d = 0.0, acc_r = 0.0;
         const R al = R(alpha), be = R(beta);
+        const int wr = first ? 0 : 1;  // 0: write into the set that is read (first pass), 1: into the other one
         auto chunk_range = [&](const ChunkMeta& cm, const ChunkMeta* nx) {
             return ChunkRange{cm.elem_start, cm.n_elem, a.Ne, cm.node_start, cm.n_int, a.N, cm.ell_off,
                               cm.ell_w * (cm.n_int + cm.n_halo), (int)a.ell_total, cm.halo_off, cm.n_halo, (int)a.n_entries,
@@ -169,7 +171,7 @@ __global__ void __launch_bounds__(kTPB, 3) dmg_cg2_chunk(const Cg2Args<R> c)
                 // latency hides behind the prologue and the element pass (x is read and written once per pass and nothing
                 // else needs it: it is not worth a shared-memory array)
                 R x_pre = R(0);
-                if (tid < nloc) {
+                if (!first && tid < nloc) {
                     const bool interior = tid < cm.n_int;
                     const int j = tid - cm.n_int;
                     if (interior || (s_hdst[j] & (kIfaceWidth - 1)) == 0) x_pre = c.x[par][interior ? cm.node_start + tid : s_hids[j]];
@@ -185,15 +187,18 @@ __global__ void __launch_bounds__(kTPB, 3) dmg_cg2_chunk(const Cg2Args<R> c)
                         R rn = r0, pn = R(0), sn = R(0);
                         if (!first) {
                             const R w = interior ? s_wv[sl] : ((s_hp[4 * j] + s_hp[4 * j + 1]) + s_hp[4 * j + 2]) + s_hp[4 * j + 3];
-                            sn = rfma(be, s_pn[sl], w);
+                            // the pass after the first finds no p and s yet (the first pass wrote none): p_0 = z_0, s_0 = w_0
+                            sn = second ? w : rfma(be, s_pn[sl], w);
                             rn = rfma(-al, sn, r0);
-                            pn = rfma(be, s_z[sl], dinv * r0);
+                            pn = second ? dinv * r0 : rfma(be, s_z[sl], dinv * r0);
                         }
                         const R zn = dinv * rn;
                         const bool owned = interior || (s_hdst[j] & (kIfaceWidth - 1)) == 0;
                         if (owned) {
-                            const int gid = interior ? cm.node_start + i : s_hids[j];
-                            c.r[par ^ 1][gid] = rn; c.p[par ^ 1][gid] = pn; c.s[par ^ 1][gid] = sn;
+                            if (!first) {  // the first pass changes nothing but w: no vector is written
+                                const int gid = interior ? cm.node_start + i : s_hids[j];
+                                c.r[par ^ 1][gid] = rn; c.p[par ^ 1][gid] = pn; c.s[par ^ 1][gid] = sn;
+                            }
                             if (dinv != R(0)) { acc_g += double(rn) * double(zn); acc_r += double(rn) * double(rn); }
                         }
                         s_z[sl] = zn; s_pn[sl] = pn;
@@ -226,9 +231,11 @@ __global__ void __launch_bounds__(kTPB, 3) dmg_cg2_chunk(const Cg2Args<R> c)
                     const uint16_t* row = s_ell + i;
 #pragma unroll 4
                     for (int w = 0; w < cm.ell_w; ++w) qs += s_slot[row[w * nloc]];
-                    if (interior) c.w[par ^ 1][gid] = qs;
-                    else c.hpart[par ^ 1][hslot] = qs;
-                    if (owned) c.x[par ^ 1][gid] = first ? xv : rfma(al, s_pn[sl], xv);
+                    // the first pass leaves its w and partials in the set it read (nobody reads either during that pass) and
+                    // the sets are not swapped after it
+                    if (interior) c.w[par ^ wr][gid] = qs;
+                    else c.hpart[par ^ wr][hslot] = qs;
+                    if (owned && !first) c.x[par ^ 1][gid] = rfma(al, s_pn[sl], xv);
                 }
                 __syncthreads();  // stage st and the slots are free again
                 PFF_TR(a.trace, tr_on && tr_k < 24, 4 + 4 * tr_k);
@@ -256,7 +263,7 @@ __global__ void __launch_bounds__(kTPB, 3) dmg_cg2_chunk(const Cg2Args<R> c)
         fence_proxy_async_global();
         grid_barrier(a.ticket + 1, gb_target, (unsigned)G);
         PFF_TR(a.trace, tr_on, 104);
-        par ^= 1;
+        par ^= wr;
         // every value of set `par` is final: the first chunk of the next pass starts streaming under the scalar reduction
         if (single_epoch) {
             const ChunkMeta cm = s_meta[0];
@@ -289,6 +296,7 @@ __global__ void __launch_bounds__(kTPB, 3) dmg_cg2_chunk(const Cg2Args<R> c)
             __syncthreads();
             if (tid == 0) cg2_scalar_step(&s_ctrl, s_out[0], s_out[1], s_out[2]);
             __syncthreads();
+            second = first;
             alpha = s_ctrl.alpha; beta = s_ctrl.beta; first = s_ctrl.first != 0;
             PFF_TR(a.trace, tr_on, 105);
             ++pass;

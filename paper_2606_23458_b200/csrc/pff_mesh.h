@@ -72,7 +72,6 @@ struct pff_mesh {
     void *d_ca = nullptr, *d_cb = nullptr;
     void* d_cg2 = nullptr;       // second set of x, r, p, s and both sets of w of the one-rendezvous CG kernel (6 vectors)
     int cg_variant = 0;          // 0: pick per solve; 1: always the two-rendezvous kernel; 2: the one-rendezvous kernel wherever it applies
-    int last_passes = 0;         // operator applications of the previous solve (mean over the last pff_run_steps): feeds the choice
     uint8_t* d_mask = nullptr;   // [N] bit0: in the free set, bit1: damage-Dirichlet
     double* d_part = nullptr;    // chunk-kernel block partials [channels][n_part_blocks]
     int64_t n_part_blocks = 0;
