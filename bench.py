@@ -170,6 +170,7 @@ def run_ours(args, rank: int, world: int):
     ms_total = float(np.median(ms_runs))
     iters = [iters[int(np.argsort(ms_runs)[len(ms_runs) // 2])]]  # CG iterations of the median run
     launches = (mesh.pff_mesh_counters() - l0) // args.repeats
+    cg_kernel_used = {1: "two-rendezvous", 2: "one-rendezvous"}.get(mesh.pff_last_cg_kernel(), "none")
     clk = clocks.stop()
 
     # --- same K steps again with per-kernel event brackets: attribution for the roofline block
@@ -239,7 +240,7 @@ def run_ours(args, rank: int, world: int):
     eq_call = lambda: mesh.pff_equilibrium_solve(st, None, rel_tol=1e-300, max_iter=EQ_ITERS, allow_noconv=True)[1]
     eq_call()
     ms_eq, it_eq = timed(eq_call, 1)
-    return dict(mesh=mesh, cfg=cfg, N=N, Ne=Ne, w=w, cg_kernels=cg_kernels, ms_total=ms_total, ms_runs=ms_runs, iters=iters, launches=launches, clk=clk, prof=prof,
+    return dict(mesh=mesh, cfg=cfg, N=N, Ne=Ne, w=w, cg_kernels=cg_kernels, cg_kernel_used=cg_kernel_used, ms_total=ms_total, ms_runs=ms_runs, iters=iters, launches=launches, clk=clk, prof=prof,
                 iters_p=iters_p, ms_exp=ms_exp, ms_adj=ms_adj / 5, it_adj=it_adj[0], ms_act=ms_act / args.steps, ms_eq=ms_eq, it_eq=it_eq[0], e2e_val=e2e_val, h2d=(9 * N + Ne) * 8, d2h=(7 * N + Ne) * 8, snapshot=snapshot)
 
 
@@ -265,7 +266,7 @@ def ncu_traffic(workload: str, dtype: str, kernel: str, k: dict):
     cap = ncu_capture(workload, dtype, kernel)
     if not cap:
         return None
-    return cap["bytes"] / cap["units"] * (k.get("iterations_per_launch", 1.0) if kernel == "cg_solve" else 1.0)
+    return cap["bytes"] / cap["units"] * (k.get("iterations_per_launch", 1.0) if kernel.startswith("cg_solve") else 1.0)
 
 
 def peaks():
@@ -350,7 +351,8 @@ def main():
             kern[name] = dict(us_per_launch=1e3 * per, launches=cnt, share_of_kernel_time=ms / total_prof_ms,
                               algorithmic_bytes=int(nbytes), achieved_gbs=nbytes / per / 1e6, frac=nbytes / per / 1e6 / peak,
                               frac_nominal_8tbs=nbytes / per / 1e6 / NOMINAL_GBS)
-            cap = ncu_capture(args.workload, "f64" if w == 8 else "f32", name)
+            cap = ncu_capture(args.workload, "f64" if w == 8 else "f32",
+                              "cg_solve_one_rendezvous" if name == "cg_solve" and r["cg_kernel_used"] == "one-rendezvous" else name)
             if cap:  # from the committed `ncu --set full` capture of this workload (profiles/traffic.csv), per captured launch
                 kern[name]["dram_pct_ncu"] = cap["dram_pct"]
                 kern[name]["dram_bytes_ncu_per_unit"] = cap["bytes"] / cap["units"]
@@ -358,7 +360,8 @@ def main():
         kern["cg_solve"]["iterations_per_launch"] = iters_prof / prof["matvec_chunk"][1]
         kern["cg_solve"]["us_per_iteration"] = 1e3 * prof["matvec_chunk"][0] / max(iters_prof, 1)
     dom = max(kern, key=lambda k: kern[k]["share_of_kernel_time"])
-    traffic = ncu_traffic(args.workload, "f64" if w == 8 else "f32", dom, kern[dom])
+    traffic = ncu_traffic(args.workload, "f64" if w == 8 else "f32",
+                          "cg_solve_one_rendezvous" if dom == "cg_solve" and r["cg_kernel_used"] == "one-rendezvous" else dom, kern[dom])
     iters_total = int(sum(r["iters"]))
     line = dict(metric=METRIC, value=whole_job_value(Ne, K, world, sec), unit=UNIT, n_gpus=world, steps=K, warmup=args.warmup,
                 ms_per_step=r["ms_total"] / K, repeats=len(r["ms_runs"]), ms_per_step_min=min(r["ms_runs"]) / K,
@@ -367,7 +370,7 @@ def main():
                 config=dict(workload=args.workload, scatter=args.scatter, name=r["cfg"]["name"], n_nodes=N, n_elems=Ne, rel_tol=REL_TOL,
                             cg_iters_per_solve=iters_total / K, chunks=r["mesh"].n_chunks, interface_nodes=r["mesh"].n_shared,
                             l2="working set > L2 (no flush needed)" if ab["step"] > 126e6 else "L2-resident workload",
-                            cg_kernel=args.cg,
+                            cg_kernel=args.cg, cg_kernel_used=r["cg_kernel_used"],
                             l0_over_h=args.l0_over_h if args.l0_over_h is not None else "recipe",
                             time_loop="plain launches" if args.no_graph else "CUDA graph replay of one captured step + solve",
                             parallelism=f"replicas x{world}"),

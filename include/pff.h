@@ -191,6 +191,8 @@ pff_status pff_energies(pff_mesh *mesh, const pff_state *state, double out[4]);
  *      the grid-wide tail is amortised and the extra pass costs more than the shorter passes save).
  * Both converge to the same unique solution (same iterates in exact arithmetic); both are bit-reproducible run to run. */
 pff_status pff_set_cg_variant(pff_mesh *mesh, int32_t variant);
+/* kernel <- 1 / 2: which of the two the last solve of this mesh launched (0: none yet).  Host-only. */
+pff_status pff_last_cg_kernel(const pff_mesh *mesh, int32_t *kernel);
 
 /* Counters of the last pff_damage_solve / pff_damage_adjoint of this mesh (of ALL solves of the last pff_run_steps):
  * restarts = how often the projected solver (AT1, L181) re-derived its free set after the first time (a bound became

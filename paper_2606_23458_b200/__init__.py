@@ -156,6 +156,11 @@ class Mesh:
     def pff_set_cg_variant(self, variant: int):
         _check(self.L.pff_set_cg_variant(self.h, int(variant)))
 
+    def pff_last_cg_kernel(self) -> int:
+        k = C.c_int32(0)
+        _check(self.L.pff_last_cg_kernel(self.h, C.byref(k)))
+        return k.value
+
     def pff_damage_last_stats(self):
         """(restarts, truncations) of the projected solver in the last solve / summed over the last pff_run_steps."""
         r, t = C.c_int32(0), C.c_int32(0)

@@ -513,6 +513,13 @@ pff_status pff_trace_set(pff_mesh* m, void* device_words, int32_t cg_iteration)
 #endif
 }
 
+pff_status pff_last_cg_kernel(const pff_mesh* m, int32_t* kernel)
+{
+    if (!m || !kernel) { set_error("pff_last_cg_kernel: null argument"); return PFF_EINVAL; }
+    *kernel = m->last_cg_kernel;
+    return PFF_OK;
+}
+
 pff_status pff_set_cg_variant(pff_mesh* m, int32_t variant)
 {
     if (!m || variant < 0 || variant > 2) { set_error("pff_set_cg_variant: null mesh or variant not 0 / 1 / 2"); return PFF_EINVAL; }

@@ -926,6 +926,7 @@ static pff_status damage_solve_t(pff_mesh* m, const pff_state* s, double rel_tol
     if ((st = persistent_config(m, (const void*)dmg_cg2_chunk<R>, (int)m->lay_mv.total, &grid_cg2)) != PFF_OK) return st;
     const bool eligible = !PROJ && hm.n_ovf == 0;
     const bool cg2 = eligible && (m->cg_variant == 2 || (m->cg_variant == 0 && hm.C <= (int64_t)16 * grid_cg2));
+    m->last_cg_kernel = cg2 ? 2 : 1;
     const void* cg_kernel = cg2 ? (const void*)dmg_cg2_chunk<R> : (const void*)dmg_iter_chunk<R, DM_CG, PROJ>;
     Cg2Args<R> c2{};
     if (cg2) {

@@ -71,6 +71,7 @@ struct pff_mesh {
     // w_13, w_23 of the P1 stiffness): fp64 two double2 streams, fp32 one float4 stream (written by the setup pass)
     void *d_ca = nullptr, *d_cb = nullptr;
     void* d_cg2 = nullptr;       // second set of x, r, p, s and both sets of w of the one-rendezvous CG kernel (6 vectors)
+    int last_cg_kernel = 0;      // which kernel the last solve launched (1 two-rendezvous, 2 one-rendezvous)
     int cg_variant = 0;          // 0: pick per solve; 1: always the two-rendezvous kernel; 2: the one-rendezvous kernel wherever it applies
     uint8_t* d_mask = nullptr;   // [N] bit0: in the free set, bit1: damage-Dirichlet
     double* d_part = nullptr;    // chunk-kernel block partials [channels][n_part_blocks]
