@@ -440,12 +440,11 @@ def test_second_solve_with_unchanged_history_needs_no_iteration():
 
 def test_full_size_fp32_variant_cfg5_1001():
     """The fp32 variant at BASELINE's metric size, in the configuration bench.py --precision f32 times: two staggered
-    steps against the fp64 oracle.  north_star's fp32 tolerance is 2e-5 max-norm relative.  At this size (h = 1e-3,
-    |u| ~ 1e-4 L) it is met by u, H and d; the acceleration is a difference quotient of fp32-STORED displacements and
-    carries eps32 * max|u| / (h * max|strain|) ~ 6e-5 of representation error whatever the arithmetic (DESIGN.md
-    section 7), so a, and v which integrates it, are held to 1e-4 here: a documented miss of the 2e-5 target that the
-    bench line of --precision f32 runs repeats (`fp32_note`).  The damage solve runs to a tolerance fp32 reaches
-    without allow_noconv (1e-6 relative residual: 10 iterations here; fp32 residuals stagnate below ~1e-7)."""
+    steps against the fp64 oracle at north_star's fp32 tolerance, 2e-5 max-norm relative: met by u, v, H and d, MISSED by
+    the acceleration (3.7e-5, held to 1e-4 here).  The acceleration is a difference quotient of displacements STORED in
+    fp32: its a-priori representation error is eps32 * max|u| / (h * max|strain|) ~ 6e-5 at h = 1e-3 whatever the arithmetic
+    (DESIGN.md section 7); fp32 bench lines say so (`fp32_note`).  The damage solve runs to a tolerance fp32 reaches without allow_noconv (1e-6 relative residual: 10
+    iterations here; fp32 residuals stagnate below ~1e-7)."""
     cfg = config(5, n=1001)
     orc = oracle_from(cfg)
     mesh, st = gpu_from(cfg, precision=1)
@@ -460,7 +459,9 @@ def test_full_size_fp32_variant_cfg5_1001():
         assert rc == 0 and stt == 0 and rr <= 1e-6
     u, v, a, d, H = gpu_fields(mesh, st)
     assert relmax(u, orc.u) <= TOL32 and relmax(H, orc.H) <= TOL32 and relmax(d, orc.d) <= TOL32
-    assert relmax(v, orc.v) <= 1e-4 and relmax(a, orc.a) <= 1e-4  # see the docstring: storage-format bound, not met at 2e-5
+    # v: 1.6e-5, inside 2e-5 with the margin this workload has.  a: 3.7e-5 after two steps, a documented MISS of north_star's
+    # fp32 tolerance at this size (storage-format bound ~6e-5, docstring); held to 1e-4
+    assert relmax(v, orc.v) <= TOL32 and relmax(a, orc.a) <= 1e-4
 
 
 def _trajectory(cfg, n_steps, gpu_variants, S=1.0, tip_width=None, rel_tol=1e-10):
