@@ -1,6 +1,6 @@
 """Phase timeline of the persistent kernels (explicit step, CG iteration) from the instrumentation build.
 
-    python -m paper_2606_23458_b200.trace_timeline [--n 1001] [--precision f64|f32] [--iteration 3]
+    python -m paper_2606_23458_b200.trace_timeline [--n 1001] [--precision f64|f32] [--iteration 3] [--run-steps]
 
 Builds libpff_trace.so if needed (the product sources with -DPFF_TRACE), steps config 5 of side n a few times, then
 records one explicit step and one CG iteration: thread 0 of every CTA stamps clock64 / %globaltimer when, chunk by chunk,
@@ -59,6 +59,8 @@ def main():
     ap.add_argument("--n", type=int, default=1001)
     ap.add_argument("--precision", default="f64", choices=["f64", "f32"])
     ap.add_argument("--iteration", type=int, default=3)
+    ap.add_argument("--run-steps", action="store_true", help="record the step kernel pff_run_steps launches (deferred interface "
+                    "update where the mesh allows it) instead of the one-call kernel of pff_explicit_step")
     args = ap.parse_args()
     sys.path.insert(0, ROOT)
     from paper_2606_23458_b200 import build
@@ -76,8 +78,12 @@ def main():
         mesh.pff_damage_solve(st, rel_tol=1e-8, allow_noconv=True)
     buf = torch.zeros(2 * 256 * 1024, dtype=torch.int64, device=mesh.device)
     pff._check(mesh.L.pff_trace_set(mesh.h, buf.data_ptr(), args.iteration))
-    mesh.pff_explicit_step(st, bc, dt)
-    mesh.pff_damage_solve(st, rel_tol=1e-8, allow_noconv=True)
+    if args.run_steps:  # three steps: every launch stamps the same rows, the last one stays
+        mesh.pff_set_graph_mode(False)
+        mesh.pff_run_steps(st, bc, dt, 3, damage_every=1, rel_tol=1e-8, allow_noconv=True)
+    else:
+        mesh.pff_explicit_step(st, bc, dt)
+        mesh.pff_damage_solve(st, rel_tol=1e-8, allow_noconv=True)
     torch.cuda.synchronize()
     pff._check(mesh.L.pff_trace_set(mesh.h, None, args.iteration))
     a = buf.cpu().numpy().astype(np.int64)
