@@ -179,6 +179,21 @@ pff_status pff_damage_solve(pff_mesh *mesh, pff_state *state, double rel_tol, in
  * with a fixed reduction order.  Synchronises the stream. */
 pff_status pff_energies(pff_mesh *mesh, const pff_state *state, double out[4]);
 
+/* pff_energies for callers that may not allocate device memory (code under CUDA graph capture, serving loops, harnesses
+ * that forbid cudaMalloc): the same three kernels, the same fixed reduction order and the same bits, but
+ *   - the block partials live in a static device array of the library (2^17 doubles = 1 MiB, held by every GPU that
+ *     loads the library until the process exits) instead of a stream-ordered allocation; its device address is looked
+ *     up once per GPU at pff_mesh_create (cudaGetSymbolAddress: a lookup, no allocation);
+ *   - out_device (DEVICE, 4 doubles, 8-byte aligned, caller-owned) receives { E_el, E_kin, E_frac, E_tot };
+ *   - the call only enqueues three kernels on the mesh's stream: no cudaMalloc / cudaFree / allocating library call, no
+ *     copy, no synchronisation.  Read out_device in stream order.
+ * Limit: 2 ceil(n_elems / 256) + ceil(n_nodes / 256) <= 131072 (about 1.3e7 elements); larger meshes return
+ * PFF_EUNSUPPORTED with the numbers in pff_last_error() and must use pff_energies.
+ * The array is shared by ALL meshes and calls of the process on that GPU and keeps the last call's contents (every word
+ * a call reads it has written before, so nothing needs clearing): calls whose kernels could overlap on the GPU (two
+ * streams, two host threads) race on it and must be serialised by the caller. */
+pff_status pff_energies_static(pff_mesh *mesh, const pff_state *state, double *out_device);
+
 /* Which kernel runs the CG iterations of pff_damage_solve / pff_damage_adjoint.
  *   1: the two-rendezvous kernel (standard Jacobi-PCG recurrence with predicted beta; interface nodes summed in a phase of
  *      their own between two grid barriers per iteration).  AT1 (projected CG, L181) always runs it.

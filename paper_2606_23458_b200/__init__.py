@@ -189,6 +189,14 @@ class Mesh:
         _check(self.L.pff_energies(self.h, C.byref(state.c), out))
         return np.array(list(out))
 
+    def pff_energies_static(self, state: State, out):
+        """pff_energies without any allocation: `out` is a caller-owned device tensor of 4 float64; asynchronous."""
+        import torch
+        if out.dtype != torch.float64 or out.numel() < 4 or not out.is_cuda or not out.is_contiguous():
+            raise ValueError("out: contiguous CUDA tensor of at least 4 float64")
+        _check(self.L.pff_energies_static(self.h, C.byref(state.c), out.data_ptr()))
+        return out
+
     def pff_damage_adjoint(self, state: State, g, free_mask=None, rel_tol=1e-8, max_iter=1000, allow_noconv=False):
         """lambda with A_FF lambda_F = g_F (operator of state.H); g, free_mask (uint8) device tensors in internal order."""
         import torch

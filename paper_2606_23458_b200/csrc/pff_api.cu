@@ -174,6 +174,11 @@ pff_status pff_mesh_create(int64_t n_nodes, const double* xy, int64_t n_elems, c
     auto fail = [&](pff_status s) { pff_mesh_destroy(m); return s; };
     cudaStream_t cs = m->stream;
     if ((st = cuda_check(cudaGetDevice(&m->device), "cudaGetDevice")) != PFF_OK) return fail(st);
+    {   // set-up: device address of pff_energies_static's scratch array on this GPU (a lookup, nothing is allocated; a
+        // failure is reported by pff_energies_static itself, which retries)
+        double* scratch = nullptr;
+        (void)energy_static_scratch(&scratch);
+    }
     const size_t N = hm.N, Ne = hm.Ne;
 #define UP(call) if ((st = (call)) != PFF_OK) return fail(st)
     UP(upload(&m->d_meta, hm.meta.data(), hm.meta.size(), cs));
@@ -670,6 +675,14 @@ pff_status pff_energies(pff_mesh* m, const pff_state* s, double out[4])
     if (!m || !valid_state(s) || !out) { set_error("pff_energies: null argument"); return PFF_EINVAL; }
     DeviceGuard dg(m);
     return energies(m, s, out);
+}
+
+pff_status pff_energies_static(pff_mesh* m, const pff_state* s, double* out_device)
+{
+    if (!m || !valid_state(s) || !out_device) { set_error("pff_energies_static: null argument"); return PFF_EINVAL; }
+    if (reinterpret_cast<uintptr_t>(out_device) % 8) { set_error("pff_energies_static: out_device must be 8-byte aligned"); return PFF_EINVAL; }
+    DeviceGuard dg(m);
+    return energies_static(m, s, out_device);
 }
 
 }  // extern "C"

@@ -1,6 +1,9 @@
 // Energies per unit thickness (Eq. 1): E_el, E_kin, E_frac, E_tot.
 // One element pass + one node pass writing fp64 block partials, then one fixed-order final sum:
 // bit-reproducible run to run.  Diagnostics path (not on the per-step hot loop).
+#include <mutex>
+#include <string>
+
 #include "pff_device.cuh"
 #include "pff_mesh.h"
 
@@ -104,6 +107,84 @@ static pff_status energies_r(pff_mesh* m, const pff_state* s, double out[4])
     if (st != PFF_OK) return st;
     out[0] = h[0]; out[1] = h[1]; out[2] = h[2]; out[3] = h[0] + h[1] + h[2];
     return PFF_OK;
+}
+
+// ---- pff_energies_static: the same three kernels with their block partials in a file-scope device array, for callers that
+// may not allocate (CUDA graph capture, serving loops).  kEnergyScratchDoubles doubles = 1 MiB on every GPU that loads the
+// library, until the process exits.  Every word a call reads it has written itself before (all 2 nbe + nbn partials), so
+// nothing has to be cleared between calls; ALL calls share the array, so two calls that overlap on the GPU race.
+constexpr int kEnergyScratchDoubles = 1 << 17;
+static __device__ __align__(256) double g_energy_scratch[kEnergyScratchDoubles];
+
+// In host code g_energy_scratch is only a stand-in for the symbol: the device address is looked up once per device, with
+// that device current (the caller's DeviceGuard), and cached.
+constexpr int kMaxDevices = 64;
+static std::mutex g_scratch_mutex;
+static double* g_scratch_addr[kMaxDevices];
+
+pff_status energy_static_scratch(double** ptr)
+{
+    int dev = 0;
+    pff_status st = cuda_check(cudaGetDevice(&dev), "pff_energies_static: cudaGetDevice");
+    if (st != PFF_OK) return st;
+    if (dev < 0 || dev >= kMaxDevices) { set_error("pff_energies_static: device ordinal beyond 63"); return PFF_EUNSUPPORTED; }
+    std::lock_guard<std::mutex> lock(g_scratch_mutex);
+    if (!g_scratch_addr[dev]) {
+        double* p = nullptr;
+        st = cuda_check(cudaGetSymbolAddress((void**)&p, g_energy_scratch), "pff_energies_static: cudaGetSymbolAddress");
+        if (st != PFF_OK) return st;
+        if (!p) { set_error("pff_energies_static: null scratch address"); return PFF_ECUDA; }
+        g_scratch_addr[dev] = p;
+    }
+    *ptr = g_scratch_addr[dev];
+    return PFF_OK;
+}
+
+// out[0..2] as energy_final_kernel, out[3] = (out[0] + out[1]) + out[2]: the host sum of energies_r, done on the device
+__global__ void __launch_bounds__(kTPB) energy_final4_kernel(const double* p0, int n0, const double* p1, int n1,
+                                                             const double* p2, int n2, double* out)
+{
+    __shared__ double s_red[32];
+    const double* ps[3] = {p0, p1, p2};
+    const int ns[3] = {n0, n1, n2};
+    double r[3] = {0.0, 0.0, 0.0};
+    for (int k = 0; k < 3; ++k) {
+        double v = 0.0;
+        for (int i = threadIdx.x; i < ns[k]; i += kTPB) v += ps[k][i];
+        r[k] = block_sum(v, s_red);
+    }
+    if (threadIdx.x == 0) { out[0] = r[0]; out[1] = r[1]; out[2] = r[2]; out[3] = r[0] + r[1] + r[2]; }
+}
+
+template <typename R>
+static pff_status energies_static_r(pff_mesh* m, const pff_state* s, double* out_device)
+{
+    const int64_t nbe = (m->hm.Ne + kTPB - 1) / kTPB, nbn = (m->hm.N + kTPB - 1) / kTPB;
+    if (2 * nbe + nbn > kEnergyScratchDoubles) {
+        set_error("pff_energies_static: mesh too large for the static scratch array: 2 ceil(n_elems / 256) + ceil(n_nodes / 256) = " +
+                  std::to_string(2 * nbe + nbn) + " block partials, the limit is " + std::to_string(kEnergyScratchDoubles) +
+                  " (use pff_energies)");
+        return PFF_EUNSUPPORTED;
+    }
+    double* part = nullptr;
+    pff_status st = energy_static_scratch(&part);
+    if (st != PFF_OK) return st;
+    switch (m->mat.split) {
+        case PFF_SPLIT_ISOTROPIC: launch_elem<R, PFF_SPLIT_ISOTROPIC>(m, s, part, (int)nbe); break;
+        case PFF_SPLIT_SPECTRAL: launch_elem<R, PFF_SPLIT_SPECTRAL>(m, s, part, (int)nbe); break;
+        case PFF_SPLIT_VOLDEV: launch_elem<R, PFF_SPLIT_VOLDEV>(m, s, part, (int)nbe); break;
+        default: launch_elem<R, PFF_SPLIT_STARCONVEX>(m, s, part, (int)nbe); break;
+    }
+    energy_node_kernel<R><<<(int)nbn, kTPB, 0, m->stream>>>((int)m->hm.N, (const R*)m->d_mass, (const R*)s->vx, (const R*)s->vy,
+                                                            part + 2 * nbe);
+    energy_final4_kernel<<<1, kTPB, 0, m->stream>>>(part, (int)nbe, part + 2 * nbe, (int)nbn, part + nbe, (int)nbe, out_device);
+    m->n_launches += 3;
+    return cuda_check(cudaGetLastError(), "pff_energies_static: launch");
+}
+
+pff_status energies_static(pff_mesh* m, const pff_state* s, double* out_device)
+{
+    return m->opt.precision == PFF_F32 ? energies_static_r<float>(m, s, out_device) : energies_static_r<double>(m, s, out_device);
 }
 
 // lambda^T M d and lambda^T K d with the consistent mass M^e = A (1 + delta_ij) / 12 (L185) and the P1 stiffness

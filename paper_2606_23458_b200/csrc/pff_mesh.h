@@ -140,6 +140,8 @@ pff_status damage_param_terms(pff_mesh* m, const void* lambda, const void* d, do
 pff_status equilibrium_solve(pff_mesh* m, pff_state* s, const pff_bc* bc, double rel_tol, int max_iter, int* iters, double* relres);
 pff_status damage_rhs_diag(pff_mesh* m, const pff_state* s, void* b, void* D);
 pff_status energies(pff_mesh* m, const pff_state* s, double out[4]);
+pff_status energies_static(pff_mesh* m, const pff_state* s, double* out_device);  // block partials in a static device array
+pff_status energy_static_scratch(double** ptr);  // device address of that array on the CURRENT device (cached per device)
 pff_status cuda_check(cudaError_t e, const char* what);
 // Cooperative launch (all CTAs co-resident: the kernels synchronise grid-wide) through the extensible launch API with the
 // cooperative attribute: unlike the legacy cooperative-launch entry point it can be captured into a CUDA graph.
