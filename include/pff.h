@@ -194,6 +194,37 @@ pff_status pff_energies(pff_mesh *mesh, const pff_state *state, double out[4]);
  * streams, two host threads) race on it and must be serialised by the caller. */
 pff_status pff_energies_static(pff_mesh *mesh, const pff_state *state, double *out_device);
 
+/* ---- geometric-multigrid-preconditioned damage solve (a preconditioner stronger
+ * than Jacobi cuts the CG iteration count 5-20x on fine meshes, where the count grows like l0 / h) ------------------------
+ * pff_mg_attach: coarse[0 .. n_coarse) are ordinary meshes of the SAME domain, material, precision, device and stream,
+ * finest first, each coarser than the one before (any triangulations: every node and element centroid of a level must lie
+ * in a triangle of the next one; nested refinements give the best transfer).  The library builds the P1 interpolation
+ * between consecutive levels (point location, barycentric weights), its transpose and the parent element of every element
+ * on the host and uploads them.  The caller keeps the coarse meshes alive while the hierarchy is attached and destroys
+ * them itself; attaching again replaces the hierarchy; pff_mesh_destroy(mesh) releases it.
+ * Errors: PFF_EINVAL (arguments), PFF_EMESH (a node outside the next level's triangles), PFF_ECUDA. */
+pff_status pff_mg_attach(pff_mesh *mesh, int32_t n_coarse, pff_mesh *const *coarse);
+
+/* Smoother weight (damped Jacobi, default 2/3; 0 < omega < 1 keeps the cycle positive definite for P1 mass + stiffness,
+ * lambda_max(D^-1 A) <= 2) and the number of Jacobi sweeps that stand for the coarsest-level solve (default 4). */
+pff_status pff_mg_set_params(pff_mesh *mesh, double omega, int32_t coarse_sweeps);
+
+/* pff_damage_solve for AT2 with one V(1,1) cycle per iteration as the preconditioner:
+ *   level l:  x = w D^-1 b;  r = b - A x;  x += P V_{l+1}(P^T r);  x += w D^-1 (b - A x);   coarsest: Jacobi sweeps.
+ * Coarse operators are re-discretised: the operator (Gc / l0 + 2 H) M + Gc l0 K (L173, L185) of the coarse mesh with H
+ * averaged over every coarse element's children (area weights).  Same right-hand side, warm start, damage-Dirichlet
+ * nodes, stopping rule (R10) and final clamp d <- min(1, max(d_n, d)) (L179) as pff_damage_solve, and the same
+ * unique solution: only the iteration count differs.  iters_out counts outer iterations (one V-cycle + one operator
+ * application each; a V-cycle costs about 2.7 fine-level operator applications).  AT1 returns PFF_EUNSUPPORTED: the
+ * projected solver's free set, and with it the operator a hierarchy would have to represent, changes between iterations,
+ * so AT1 keeps the Jacobi preconditioner.  Synchronises the stream every iteration (host-side convergence test);
+ * bit-reproducible run to run.  Pays off where l0 / h is large (profiles/r2_multigrid.md); not used by pff_run_steps. */
+pff_status pff_damage_solve_mg(pff_mesh *mesh, pff_state *state, double rel_tol, int32_t max_iter,
+                               int32_t *iters_out, double *relres_out);
+
+/* Test hook: z = V(r), one cycle of the preconditioner with the operator of state->H; r, z device [n_nodes]. */
+pff_status pff_mg_apply(pff_mesh *mesh, const pff_state *state, const void *r, void *z);
+
 /* Which kernel runs the CG iterations of pff_damage_solve / pff_damage_adjoint.
  *   1: the two-rendezvous kernel (standard Jacobi-PCG recurrence with predicted beta; interface nodes summed in a phase of
  *      their own between two grid barriers per iteration).  AT1 (projected CG, L181) always runs it.

@@ -189,6 +189,27 @@ class Mesh:
         _check(self.L.pff_energies(self.h, C.byref(state.c), out))
         return np.array(list(out))
 
+    def pff_mg_attach(self, coarse_meshes):
+        """Attach coarser meshes (finest first) as the multigrid hierarchy of this mesh; they are kept alive here."""
+        arr = (C.c_void_p * len(coarse_meshes))(*[m.h for m in coarse_meshes])
+        _check(self.L.pff_mg_attach(self.h, len(coarse_meshes), arr))
+        self._mg_levels = list(coarse_meshes)
+
+    def pff_mg_set_params(self, omega=2.0 / 3.0, coarse_sweeps=4):
+        _check(self.L.pff_mg_set_params(self.h, omega, coarse_sweeps))
+
+    def pff_damage_solve_mg(self, state: State, rel_tol=1e-8, max_iter=200, allow_noconv=False):
+        it, rr = C.c_int32(0), C.c_double(0.0)
+        st = _check(self.L.pff_damage_solve_mg(self.h, C.byref(state.c), rel_tol, max_iter, C.byref(it), C.byref(rr)),
+                    allow=(PFF_ENOCONV,) if allow_noconv else ())
+        return st, it.value, rr.value
+
+    def pff_mg_apply(self, state: State, r):
+        import torch
+        z = torch.empty_like(r)
+        _check(self.L.pff_mg_apply(self.h, C.byref(state.c), r.data_ptr(), z.data_ptr()))
+        return z
+
     def pff_energies_static(self, state: State, out):
         """pff_energies without any allocation: `out` is a caller-owned device tensor of 4 float64; asynchronous."""
         import torch

@@ -18,7 +18,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libpff.so")
 LIB_TRACE = os.path.join(HERE, "libpff_trace.so")
-SOURCES = ["mesh_setup.cpp", "pff_api.cu", "pff_step.cu", "pff_damage.cu", "pff_energy.cu", "pff_host.cu", "pff_equilibrium.cu"]
+SOURCES = ["mesh_setup.cpp", "pff_api.cu", "pff_step.cu", "pff_damage.cu", "pff_energy.cu", "pff_host.cu", "pff_equilibrium.cu", "pff_multigrid.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
          "-Xcompiler", "-fPIC", "-I", os.path.join(ROOT, "include"), "-I", CSRC]

@@ -104,6 +104,7 @@ void pff_mesh_destroy(pff_mesh* m)
     if (!m) return;
     DeviceGuard dg(m);
     cudaStreamSynchronize(m->stream);
+    mg_free(m);
     void* ptrs[] = {m->d_meta, m->d_lconn, m->d_conn, m->d_ga, m->d_gb, m->d_area, m->d_minv, m->d_mass,
                     m->d_halo_ids, m->d_sh_rowptr, m->d_halo_dst, m->d_ell, m->d_flags, m->d_halo_part,
                     m->d_fwx, m->d_fwy, m->d_dir_dof, m->d_ca, m->d_cb, m->d_lb, m->d_r, m->d_p, m->d_q, m->d_dinv, m->d_mask,
@@ -675,6 +676,35 @@ pff_status pff_energies(pff_mesh* m, const pff_state* s, double out[4])
     if (!m || !valid_state(s) || !out) { set_error("pff_energies: null argument"); return PFF_EINVAL; }
     DeviceGuard dg(m);
     return energies(m, s, out);
+}
+
+pff_status pff_mg_attach(pff_mesh* m, int32_t n_coarse, pff_mesh* const* coarse)
+{
+    if (!m || n_coarse < 1 || n_coarse > 16 || !coarse) { set_error("pff_mg_attach: null mesh or n_coarse outside 1..16"); return PFF_EINVAL; }
+    if (m->opt.scatter != PFF_SCATTER_GATHER) { set_error("pff_mg_attach: gather meshes only"); return PFF_EUNSUPPORTED; }
+    DeviceGuard dg(m);
+    return mg_attach(m, n_coarse, coarse);
+}
+
+pff_status pff_mg_set_params(pff_mesh* m, double omega, int32_t coarse_sweeps)
+{
+    if (!m) { set_error("pff_mg_set_params: null mesh"); return PFF_EINVAL; }
+    return mg_set_params(m, omega, coarse_sweeps);
+}
+
+pff_status pff_mg_apply(pff_mesh* m, const pff_state* s, const void* r, void* z)
+{
+    if (!m || !valid_state(s) || !r || !z) { set_error("pff_mg_apply: null argument"); return PFF_EINVAL; }
+    DeviceGuard dg(m);
+    return mg_apply(m, s, r, z);
+}
+
+pff_status pff_damage_solve_mg(pff_mesh* m, pff_state* s, double rel_tol, int32_t max_iter, int32_t* iters, double* relres)
+{
+    if (!m || !valid_state(s)) { set_error("pff_damage_solve_mg: null mesh, null or misaligned (16 B) state pointer"); return PFF_EINVAL; }
+    if (!(rel_tol > 0) || max_iter < 1) { set_error("pff_damage_solve_mg: need rel_tol > 0, max_iter >= 1"); return PFF_EINVAL; }
+    DeviceGuard dg(m);
+    return mg_solve(m, s, rel_tol, max_iter, iters, relres);
 }
 
 pff_status pff_energies_static(pff_mesh* m, const pff_state* s, double* out_device)

@@ -1012,7 +1012,7 @@ pff_status damage_adjoint(pff_mesh* m, const pff_state* s, const void* g, const 
 }
 
 template <typename R>
-static pff_status damage_matvec_t(pff_mesh* m, const pff_state* s, const void* p, void* q)
+static pff_status damage_matvec_t(pff_mesh* m, const pff_state* s, const void* p, void* q, bool refresh_coef)
 {
     pff_status st = ensure_workspace(m);
     if (st != PFF_OK) return st;
@@ -1023,7 +1023,7 @@ static pff_status damage_matvec_t(pff_mesh* m, const pff_state* s, const void* p
     int grid_mv = 0;
     if ((st = persistent_config(m, (const void*)dmg_iter_chunk<R, DM_PLAIN, false>, smem_mv, &grid_mv)) != PFF_OK) return st;
     grid_mv = (int)std::min<int64_t>(grid_mv, m->hm.C);
-    if (m->only_kernel < 0) {  // the operator of state->H in coefficient form (timing hook: reuse the previous one)
+    if (refresh_coef && m->only_kernel < 0) {  // the operator of state->H in coefficient form (timing hook, multigrid cycles: reuse the previous one)
         PFF_LAUNCH(m, PFF_K_DAMAGE_SETUP, (dmg_coef_kernel<R><<<(unsigned)((m->hm.Ne + kTPB - 1) / kTPB), kTPB, 0, m->stream>>>(a)));
     }
     if (m->only_kernel != 3) {
@@ -1035,9 +1035,25 @@ static pff_status damage_matvec_t(pff_mesh* m, const pff_state* s, const void* p
     return cuda_check(cudaGetLastError(), "damage matvec launch");
 }
 
-pff_status damage_matvec(pff_mesh* m, const pff_state* s, const void* p, void* q)
+// operator coefficients of state->H alone (multigrid set-up: the cycles then apply the operator with refresh_coef = false)
+template <typename R>
+static pff_status damage_refresh_coef_t(pff_mesh* m, const pff_state* s)
 {
-    return m->opt.precision == PFF_F32 ? damage_matvec_t<float>(m, s, p, q) : damage_matvec_t<double>(m, s, p, q);
+    pff_status st = ensure_workspace(m);
+    if (st != PFF_OK) return st;
+    DmgArgs<R> a = make_args<R>(m, s);
+    PFF_LAUNCH(m, PFF_K_DAMAGE_SETUP, (dmg_coef_kernel<R><<<(unsigned)((m->hm.Ne + kTPB - 1) / kTPB), kTPB, 0, m->stream>>>(a)));
+    return cuda_check(cudaGetLastError(), "damage coefficients launch");
+}
+
+pff_status damage_refresh_coef(pff_mesh* m, const pff_state* s)
+{
+    return m->opt.precision == PFF_F32 ? damage_refresh_coef_t<float>(m, s) : damage_refresh_coef_t<double>(m, s);
+}
+
+pff_status damage_matvec(pff_mesh* m, const pff_state* s, const void* p, void* q, bool refresh_coef)
+{
+    return m->opt.precision == PFF_F32 ? damage_matvec_t<float>(m, s, p, q, refresh_coef) : damage_matvec_t<double>(m, s, p, q, refresh_coef);
 }
 
 template <typename R>

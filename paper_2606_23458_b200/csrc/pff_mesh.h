@@ -36,6 +36,7 @@ struct pff_mesh {
     int64_t n_launches = 0;  // kernels launched so far (pff_mesh_counters)
     long long* d_trace = nullptr;  // pff_trace_set (instrumentation build)
     int trace_iter = 3;
+    void* mg = nullptr;      // multigrid hierarchy attached to this (finest) mesh: pff_multigrid.cu
     int only_kernel = -1;    // profiling hook: restrict multi-kernel entry points to one kernel (pff_time_kernel)
     // launch configuration of every persistent chunk kernel this mesh has used, keyed by the kernel's address: the grid
     // (CTAs that fit the mesh's device with this mesh's shared-memory stage).  Presence also means the dynamic
@@ -133,7 +134,14 @@ inline void prof_mark(pff_mesh* m, int cls)
 pff_status launch_step(pff_mesh* m, pff_state* s, const pff_bc* bc, double dt, int mode, void* fx, void* fy, void* psi,
                        const void* px = nullptr, const void* py = nullptr);
 pff_status damage_solve(pff_mesh* m, pff_state* s, double rel_tol, int max_iter, int* iters, double* relres);
-pff_status damage_matvec(pff_mesh* m, const pff_state* s, const void* p, void* q);
+pff_status damage_matvec(pff_mesh* m, const pff_state* s, const void* p, void* q, bool refresh_coef = true);
+pff_status damage_refresh_coef(pff_mesh* m, const pff_state* s);
+// pff_multigrid.cu: geometric-multigrid-preconditioned CG for the AT2 damage solve
+pff_status mg_attach(pff_mesh* m, int n_coarse, pff_mesh* const* coarse);
+pff_status mg_apply(pff_mesh* m, const pff_state* s, const void* r, void* z);
+pff_status mg_solve(pff_mesh* m, pff_state* s, double rel_tol, int max_iter, int* iters, double* relres);
+pff_status mg_set_params(pff_mesh* m, double omega, int coarse_sweeps);
+void mg_free(pff_mesh* m);
 pff_status damage_adjoint(pff_mesh* m, const pff_state* s, const void* g, const uint8_t* free_mask, void* lambda, double rel_tol,
                           int max_iter, int* iters, double* relres);
 pff_status damage_param_terms(pff_mesh* m, const void* lambda, const void* d, double out[2]);

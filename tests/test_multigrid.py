@@ -1,0 +1,199 @@
+"""Multigrid-preconditioned damage solve (pff_damage_solve_mg, include/pff.h).
+
+-m "not gpu": pins of the dense CPU restatement (oracle/pff_mg_oracle.py) against what the mathematics fixes.
+-m gpu: the CUDA cycle against that restatement, element by element, and the CUDA solve against the oracle's converged
+Jacobi solve (the unique minimiser both methods must reach).
+"""
+import numpy as np
+import pytest
+
+from pff_inputs import GLASS, grid_mesh
+from oracle import Material, OracleMesh
+from oracle.pff_mg_oracle import Hierarchy, interpolation, restrict_history
+
+
+def _levels(n_fine, n_levels, L=0.01, jitter=0.0, seed=0):
+    """Nested structured grids n, (n - 1) / 2 + 1, ... on [0, L]^2; optional jitter of the finest level's inner nodes."""
+    meshes, n = [], n_fine
+    for l in range(n_levels):
+        xy, tri = grid_mesh(n, n, L, L)
+        if l == 0 and jitter > 0:
+            h = L / (n - 1)
+            ii, jj = np.arange(n * n) % n, np.arange(n * n) // n
+            inner = (ii > 0) & (ii < n - 1) & (jj > 0) & (jj < n - 1)
+            xy = xy + np.random.default_rng(seed).uniform(-jitter * h, jitter * h, xy.shape) * inner[:, None]
+        meshes.append((xy, tri))
+        assert (n - 1) % 2 == 0 or l == n_levels - 1
+        n = (n - 1) // 2 + 1
+    return meshes
+
+
+def _material(meshes, l0_over_h):
+    h = meshes[0][0][1, 0] - meshes[0][0][0, 0]
+    return dict(GLASS, l0=l0_over_h * h, model=2, split=1, plane=0)
+
+
+def _history(xy, tri, material, seed=1):
+    """Smooth background + a sharp band (a crack's history field): several decades, like a loaded specimen."""
+    cen = xy[tri].mean(axis=1)
+    L = xy[:, 0].max()
+    psi_c = material["Gc"] / (2 * material["l0"])
+    band = np.exp(-((cen[:, 1] - 0.53 * L) / (0.04 * L)) ** 2) * (cen[:, 0] < 0.6 * L)
+    return psi_c * (0.05 + 0.1 * np.random.default_rng(seed).uniform(size=len(tri)) + 30.0 * band)
+
+
+# ---- CPU pins of the restatement ------------------------------------------------------------------------------------------
+def test_interpolation_has_linear_precision_and_history_restriction_preserves_the_integral():
+    meshes = _levels(17, 2, jitter=0.2)
+    mat = Material(**_material(meshes, 2.0))
+    f, c = OracleMesh(*meshes[0], mat), OracleMesh(*meshes[1], mat)
+    P = interpolation(f, c)
+    assert np.allclose(P.sum(axis=1), 1.0, atol=1e-14) and P.min() >= 0.0
+    for g in (lambda p: 3.0 + 0 * p[:, 0], lambda p: 2.0 * p[:, 0] - 5.0 * p[:, 1] + 0.1):  # affine functions are reproduced
+        assert np.allclose(P @ g(c.xy), g(f.xy), rtol=0, atol=1e-12 * 10)
+    assert (np.count_nonzero(P, axis=1) <= 3).all()
+    assert np.allclose(restrict_history(f, c, np.full(f.Ne, 7.0)), 7.0)
+    nested = _levels(17, 2)  # nested triangulations: the children tile their parent, so the integral of H is kept
+    f, c = OracleMesh(*nested[0], mat), OracleMesh(*nested[1], mat)
+    H = np.random.default_rng(0).uniform(1.0, 2.0, f.Ne)
+    Hc = restrict_history(f, c, H)
+    assert np.isclose((Hc * c.area).sum(), (H * f.area).sum(), rtol=1e-12)
+    assert np.allclose(Hc[0], H[[0, 1, 2, 2 * 16 + 1]].mean()) or np.isclose(Hc.sum() * 4, H.sum(), rtol=1e-12)
+
+
+@pytest.mark.parametrize("fixed", [(), (40, 41, 42, 100)])
+def test_cycle_matrix_is_symmetric_positive_definite_and_improves_the_condition_number(fixed):
+    meshes = _levels(13, 3)
+    material = _material(meshes, 4.0)
+    H = _history(*meshes[0], material)
+    hier = Hierarchy(meshes, material, H, fixed=fixed)
+    M = hier.matrix()
+    assert np.abs(M - M.T).max() <= 1e-12 * np.abs(M).max()
+    fr = hier.free
+    ev = np.linalg.eigvalsh(0.5 * (M + M.T)[np.ix_(fr, fr)])
+    assert ev.min() > 0
+    assert np.abs(M[~fr]).max() == 0 if len(fixed) else True
+    A = hier.A[0][np.ix_(fr, fr)]
+    Ms = 0.5 * (M + M.T)[np.ix_(fr, fr)]
+    lam_mg = np.linalg.eigvals(Ms @ A).real
+    lam_j = np.linalg.eigvals(np.diag(1.0 / np.diag(A)) @ A).real
+    # (re-discretised coarse operators: the coarse correction may overshoot, so I - M A need not be a contraction; PCG only
+    # needs M symmetric positive definite, and a small spread of the eigenvalues of M A)
+    assert lam_mg.min() > 0
+    assert lam_mg.max() / lam_mg.min() < 0.25 * lam_j.max() / lam_j.min()
+
+
+def test_two_level_cycle_with_exact_coarse_solve_is_the_textbook_two_grid_operator():
+    """One coarse level whose 'Jacobi sweeps' are converged (200 sweeps) = exact coarse solve: the cycle matrix must be
+    S + S - S A S + (I - S A) P A_c^-1 P^T (I - A S), S = w D^-1, assembled here from its factors."""
+    meshes = _levels(9, 2)
+    material = _material(meshes, 1.0)
+    H = _history(*meshes[0], material)
+    hier = Hierarchy(meshes, material, H, coarse_sweeps=400, omega=0.6)
+    A, Ac, P = hier.A[0], hier.A[1], hier.P[0]
+    S = np.diag(0.6 * hier.Dinv[0])
+    I = np.eye(len(A))
+    ref = 2 * S - S @ A @ S + (I - S @ A) @ P @ np.linalg.solve(Ac, P.T) @ (I - A @ S)
+    M = hier.matrix()
+    assert np.abs(M - ref).max() <= 1e-9 * np.abs(ref).max()
+
+
+def test_pcg_with_the_cycle_reaches_the_oracles_jacobi_solution_in_fewer_iterations():
+    meshes = _levels(17, 3, jitter=0.15)
+    material = _material(meshes, 4.0)
+    H = _history(*meshes[0], material)
+    fixed = np.array([5, 6, 150], dtype=np.int32)
+    orc = OracleMesh(*meshes[0], Material(**material))
+    orc.H[:] = H
+    orc.d[:] = 0.0
+    orc.d[fixed] = 1.0
+    orc.set_damage_dirichlet(fixed)
+    d0 = orc.d.copy()
+    b, _ = orc.damage_rhs_diag()
+    rc, it_j, _ = orc.damage_solve(rel_tol=1e-13, max_iter=5000)
+    assert rc == 0
+    hier = Hierarchy(meshes, material, H, fixed=fixed)
+    x, it_mg = hier.pcg(b, d0, rel_tol=1e-13)
+    x = np.minimum(1.0, np.maximum(d0, x))
+    assert np.abs(x - orc.d).max() <= 1e-10 * np.abs(orc.d).max()
+    assert it_mg < it_j / 3
+
+
+# ---- GPU: the CUDA cycle and solve ------------------------------------------------------------------------------------------
+def _gpu_hierarchy(meshes, material, precision=0, H=None, d=None, fixed=()):
+    import paper_2606_23458_b200 as pff
+    ms = [pff.Mesh(xy, tri, material, precision=precision) for xy, tri in meshes]
+    st = ms[0].new_state(d=d, H=H)
+    if len(fixed):
+        ms[0].pff_set_damage_dirichlet(np.asarray(fixed, dtype=np.int32))
+    ms[0].pff_mg_attach(ms[1:])
+    return ms[0], st
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("fixed", [(), (40, 41, 42, 100)])
+def test_cuda_cycle_matches_the_dense_restatement(fixed):
+    meshes = _levels(13, 3, jitter=0.1)
+    material = _material(meshes, 4.0)
+    H = _history(*meshes[0], material)
+    hier = Hierarchy(meshes, material, H, fixed=fixed)
+    mesh, st = _gpu_hierarchy(meshes, material, H=H, fixed=fixed)
+    rng = np.random.default_rng(3)
+    for _ in range(3):
+        r = rng.normal(size=mesh.n_nodes)
+        z = mesh.nodes_to_user(mesh.pff_mg_apply(st, mesh.nodes_to_internal(r)))
+        ref = hier.vcycle(np.where(hier.free, r, 0.0) if len(fixed) else r)
+        assert np.abs(z - ref).max() <= 1e-11 * np.abs(ref).max()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("precision,l0_over_h", [(0, 4.0), (0, 1.0), (1, 4.0)])
+def test_cuda_mg_solve_reaches_the_oracles_solution_and_needs_fewer_iterations(precision, l0_over_h):
+    meshes = _levels(65, 4, jitter=0.15)
+    material = _material(meshes, l0_over_h)
+    H = _history(*meshes[0], material)
+    N = len(meshes[0][0])
+    fixed = np.array([5, 6, 2000], dtype=np.int32)
+    d0 = np.random.default_rng(5).uniform(0.0, 0.05, N)
+    d0[fixed] = 1.0
+    orc = OracleMesh(*meshes[0], Material(**material))
+    orc.H[:] = H
+    orc.d[:] = d0
+    orc.set_damage_dirichlet(fixed)
+    rc, it_j, _ = orc.damage_solve(rel_tol=1e-12, max_iter=5000)
+    assert rc == 0
+    mesh, st = _gpu_hierarchy(meshes, material, precision=precision, H=H, d=d0, fixed=fixed)
+    tol = 1e-12 if precision == 0 else 1e-6
+    stt, it_mg, rr = mesh.pff_damage_solve_mg(st, rel_tol=tol, max_iter=100)
+    assert stt == 0 and rr <= tol
+    d = mesh.nodes_to_user(st.d)
+    assert np.abs(d - orc.d).max() <= (1e-9 if precision == 0 else 2e-5) * np.abs(orc.d).max()
+    assert d.min() >= 0 and d.max() <= 1 and (d >= d0.astype(mesh.np_dtype) - 1e-7).all()
+    if precision == 0:
+        assert it_mg < it_j / (3 if l0_over_h >= 4 else 2)
+        # bit-reproducible, and the Jacobi path on the same mesh agrees
+        mesh2, st2 = _gpu_hierarchy(meshes, material, precision=precision, H=H, d=d0, fixed=fixed)
+        mesh2.pff_damage_solve_mg(st2, rel_tol=tol, max_iter=100)
+        assert np.array_equal(mesh2.nodes_to_user(st2.d), d)
+        st3 = mesh2.new_state(d=d0, H=H)
+        mesh2.pff_damage_solve(st3, rel_tol=1e-12, max_iter=5000)
+        assert np.abs(mesh2.nodes_to_user(st3.d) - d).max() <= 1e-9
+
+
+@pytest.mark.gpu
+def test_mg_rejects_at1_missing_hierarchy_and_meshes_of_another_domain():
+    import paper_2606_23458_b200 as pff
+    meshes = _levels(9, 2)
+    material = _material(meshes, 2.0)
+    fine = pff.Mesh(*meshes[0], material)
+    st = fine.new_state()
+    with pytest.raises(pff.PffError):
+        fine.pff_damage_solve_mg(st)                                    # nothing attached
+    xy_far = meshes[1][0] + 1.0
+    with pytest.raises(pff.PffError):
+        fine.pff_mg_attach([pff.Mesh(xy_far, meshes[1][1], material)])  # not the same domain
+    at1 = dict(material, model=1)
+    fine1, coarse1 = pff.Mesh(*meshes[0], at1), pff.Mesh(*meshes[1], at1)
+    fine1.pff_mg_attach([coarse1])
+    with pytest.raises(pff.PffError):
+        fine1.pff_damage_solve_mg(fine1.new_state())                    # AT1 keeps Jacobi
