@@ -232,6 +232,47 @@ def run_ours(args, rank: int, world: int):
     barrier()
     e2e_val = whole_job_value(Ne, ke, world, reduce_max(time.perf_counter() - t0, world, f"cuda:{dev}"))
 
+    # multigrid-preconditioned damage solve (pff_damage_solve_mg) against the Jacobi kernels on the same
+    # mesh with l0 = 4 h (the paper's meshes resolve l0 with h <= l0 / 2; config 5 itself has h = 2 l0, where
+    # Jacobi needs 13 passes and multigrid cannot pay): nested grids down to ~1.6e4 nodes, both solvers from the same state
+    mg = None
+    if args.workload.startswith("cfg5_") and args.scatter == "gather" and cfg["material"]["model"] == 2 and not args.no_multigrid:
+        from pff_inputs import grid_mesh
+        n_side = int(args.workload.split("_")[1])
+        Ls = float(cfg["xy"][:, 0].max())
+        sides, ms_ = [], n_side
+        while (ms_ - 1) % 2 == 0 and ms_ > 60:
+            ms_ = (ms_ - 1) // 2 + 1
+            sides.append(ms_)
+        if sides:
+            mat4 = dict(cfg["material"], l0=args.mg_l0_over_h * Ls / (n_side - 1))
+            fine = pff.Mesh(cfg["xy"], cfg["tri"], mat4, precision=prec, device=f"cuda:{dev}")
+            fine.pff_mg_attach([pff.Mesh(*grid_mesh(k, k, Ls, Ls), mat4, precision=prec, device=f"cuda:{dev}") for k in sides])
+            fst = fine.new_state(u=cfg["u0"], d=cfg["d0"])
+            fdt = cfg["dt_factor"] * fine.dt_crit
+            fine.pff_init_accel(fst, bc)
+            for _ in range(5):
+                fine.pff_explicit_step(fst, bc, fdt)
+                fine.pff_damage_solve(fst, rel_tol=REL_TOL, max_iter=MAX_ITER, allow_noconv=True)
+            fsnap = {k: getattr(fst, k).clone() for k in fst.FIELDS}
+            mg = dict(l0_over_h=args.mg_l0_over_h, level_nodes=[n_side * n_side] + [k * k for k in sides])
+            sol = {}
+            for name in ("jacobi", "multigrid"):
+                fine.pff_set_damage_solver(name)
+                ts, it_s = [], 0
+                for rep in range(4):
+                    for k in fst.FIELDS:
+                        getattr(fst, k).copy_(fsnap[k])
+                    fine.pff_explicit_step(fst, bc, fdt)
+                    t_ms, o = timed(lambda: fine.pff_damage_solve(fst, rel_tol=REL_TOL, max_iter=MAX_ITER, allow_noconv=True)[1], 1)
+                    ts.append(t_ms); it_s = o[0]
+                mg[name] = dict(ms_per_solve=float(np.median(ts[1:])), iterations=it_s)
+                sol[name] = fst.d.clone()
+            mg["max_abs_diff_d"] = float((sol["multigrid"] - sol["jacobi"]).abs().max())
+            mg["note"] = ("one damage solve to rel_tol 1e-8 from the same state, l0 = %g h: Jacobi-PCG kernels against one V(1,1) cycle per "
+                          "iteration (iterations = outer iterations, each one cycle + one operator application)" % args.mg_l0_over_h)
+            del fine, fst, fsnap, sol
+
     # quasi-static mechanics solve (pff_equilibrium_solve), timed LAST because it installs a Dirichlet set (bottom edge
     # clamped): exactly EQ_ITERS CG iterations on the matrix-free stiffness action (the tolerance is unreachable)
     yb = cfg["xy"][:, 1]
@@ -241,7 +282,7 @@ def run_ours(args, rank: int, world: int):
     eq_call()
     ms_eq, it_eq = timed(eq_call, 1)
     return dict(mesh=mesh, cfg=cfg, N=N, Ne=Ne, w=w, cg_kernels=cg_kernels, cg_kernel_used=cg_kernel_used, ms_total=ms_total, ms_runs=ms_runs, iters=iters, launches=launches, clk=clk, prof=prof,
-                iters_p=iters_p, ms_exp=ms_exp, ms_adj=ms_adj / 5, it_adj=it_adj[0], ms_act=ms_act / args.steps, ms_eq=ms_eq, it_eq=it_eq[0], e2e_val=e2e_val, h2d=(9 * N + Ne) * 8, d2h=(7 * N + Ne) * 8, snapshot=snapshot)
+                iters_p=iters_p, ms_exp=ms_exp, ms_adj=ms_adj / 5, it_adj=it_adj[0], ms_act=ms_act / args.steps, ms_eq=ms_eq, it_eq=it_eq[0], mg=mg, e2e_val=e2e_val, h2d=(9 * N + Ne) * 8, d2h=(7 * N + Ne) * 8, snapshot=snapshot)
 
 
 NOMINAL_GBS = 8000.0  # the "~8 TB/s" north_star names; reported beside the measured copy peak
@@ -312,6 +353,8 @@ def main():
     ap.add_argument("--cg", default="auto", choices=["auto", "two-rendezvous", "one-rendezvous"],
                     help="CG kernel of the damage solve (include/pff.h, pff_set_cg_variant): auto = chosen per solve from the mesh "
                          "size and the previous solve's pass count")
+    ap.add_argument("--no-multigrid", action="store_true", help="skip the multigrid-against-Jacobi leg (cfg5 workloads)")
+    ap.add_argument("--mg-l0-over-h", type=float, default=4.0, help="regularisation length of the multigrid leg's mesh, in mesh sizes")
     ap.add_argument("--no-graph", action="store_true", help="pff_run_steps launches every kernel itself instead of replaying a captured period")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -394,6 +437,7 @@ def main():
                                  note="pff_equilibrium_solve, bottom edge clamped: ONE launch per iteration (node prologue with the "
                                       "previous step, fused stiffness action, gather, sums, scalar step by the last CTA); algorithmic "
                                       "bytes per iteration = one stiffness-action pass + du, r, p read and written, q, 1/D read"),
+                multigrid=r["mg"],
                 clocks=r["clk"], gpu_launches=int(r["launches"]),
                 e2e=dict(value=r["e2e_val"], unit=UNIT, h2d_bytes_per_step=r["h2d"], d2h_bytes_per_step=r["d2h"]),
                 roofline=dict(bound="hbm", kernel=dom, achieved=kern[dom]["achieved_gbs"], peak=peak, unit="GB/s",

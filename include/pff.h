@@ -218,9 +218,17 @@ pff_status pff_mg_set_params(pff_mesh *mesh, double omega, int32_t coarse_sweeps
  * application each; a V-cycle costs about 2.7 fine-level operator applications).  AT1 returns PFF_EUNSUPPORTED: the
  * projected solver's free set, and with it the operator a hierarchy would have to represent, changes between iterations,
  * so AT1 keeps the Jacobi preconditioner.  Synchronises the stream every iteration (host-side convergence test);
- * bit-reproducible run to run.  Pays off where l0 / h is large (profiles/r2_multigrid.md); not used by pff_run_steps. */
+ * bit-reproducible run to run.  Pays off where l0 / h is large (profiles/r2_multigrid.md); pff_damage_solve and
+ * pff_run_steps use it after pff_set_damage_solver(mesh, 1). */
 pff_status pff_damage_solve_mg(pff_mesh *mesh, pff_state *state, double rel_tol, int32_t max_iter,
                                int32_t *iters_out, double *relres_out);
+
+/* Which solver pff_damage_solve and pff_run_steps use for this mesh: 0 (default) the Jacobi-PCG kernels, 1 the
+ * multigrid-preconditioned CG above (needs an attached hierarchy: PFF_EINVAL otherwise; AT2 only: PFF_EUNSUPPORTED).
+ * With solver 1, pff_run_steps launches every kernel itself (no graph replay of a period: the solver tests convergence on
+ * the host) and its iteration total counts outer multigrid iterations.  pff_mg_attach replacing the hierarchy keeps the
+ * choice; pff_damage_adjoint always uses the Jacobi kernels. */
+pff_status pff_set_damage_solver(pff_mesh *mesh, int32_t solver);
 
 /* Test hook: z = V(r), one cycle of the preconditioner with the operator of state->H; r, z device [n_nodes]. */
 pff_status pff_mg_apply(pff_mesh *mesh, const pff_state *state, const void *r, void *z);

@@ -195,6 +195,10 @@ class Mesh:
         _check(self.L.pff_mg_attach(self.h, len(coarse_meshes), arr))
         self._mg_levels = list(coarse_meshes)
 
+    def pff_set_damage_solver(self, solver: str):
+        """'jacobi' (default) or 'multigrid' (after pff_mg_attach, AT2) for pff_damage_solve / pff_run_steps."""
+        _check(self.L.pff_set_damage_solver(self.h, {"jacobi": 0, "multigrid": 1}[solver]))
+
     def pff_mg_set_params(self, omega=2.0 / 3.0, coarse_sweeps=4):
         _check(self.L.pff_mg_set_params(self.h, omega, coarse_sweeps))
 

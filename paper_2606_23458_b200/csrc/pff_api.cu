@@ -447,7 +447,9 @@ pff_status pff_run_steps(pff_mesh* m, pff_state* s, const pff_bc* bc, double dt,
     };
     const int64_t period = damage_every > 0 ? damage_every : 1;
     int64_t k = 1;
-    const bool want_graph = m->graph_mode != 0 && !m->graph_unsupported && !m->prof_on && period <= 64 && n_steps >= 4 * period;
+    // (the multigrid solver tests convergence on the host every iteration: its solves cannot be part of a captured period)
+    const bool mg_solver = m->damage_solver == 1 && m->mg && m->mat.model == PFF_AT2 && damage_every > 0;
+    const bool want_graph = m->graph_mode != 0 && !m->graph_unsupported && !m->prof_on && period <= 64 && n_steps >= 4 * period && !mg_solver;
     if (want_graph) {
         // key of everything a captured period depends on (kernel arguments are frozen at capture time)
         struct Key { pff_state s; pff_bc bc; double dt, tol; int32_t every, max_iter; int64_t n_dir; uint64_t flags_gen; int32_t variant; } key{};
@@ -684,6 +686,15 @@ pff_status pff_mg_attach(pff_mesh* m, int32_t n_coarse, pff_mesh* const* coarse)
     if (m->opt.scatter != PFF_SCATTER_GATHER) { set_error("pff_mg_attach: gather meshes only"); return PFF_EUNSUPPORTED; }
     DeviceGuard dg(m);
     return mg_attach(m, n_coarse, coarse);
+}
+
+pff_status pff_set_damage_solver(pff_mesh* m, int32_t solver)
+{
+    if (!m || solver < 0 || solver > 1) { set_error("pff_set_damage_solver: null mesh or solver not 0 / 1"); return PFF_EINVAL; }
+    if (solver == 1 && !m->mg) { set_error("pff_set_damage_solver: no hierarchy attached (pff_mg_attach)"); return PFF_EINVAL; }
+    if (solver == 1 && m->mat.model != PFF_AT2) { set_error("pff_set_damage_solver: the multigrid solver is AT2 only"); return PFF_EUNSUPPORTED; }
+    m->damage_solver = solver;
+    return PFF_OK;
 }
 
 pff_status pff_mg_set_params(pff_mesh* m, double omega, int32_t coarse_sweeps)

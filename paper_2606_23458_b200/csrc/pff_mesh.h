@@ -37,6 +37,7 @@ struct pff_mesh {
     long long* d_trace = nullptr;  // pff_trace_set (instrumentation build)
     int trace_iter = 3;
     void* mg = nullptr;      // multigrid hierarchy attached to this (finest) mesh: pff_multigrid.cu
+    int damage_solver = 0;   // pff_set_damage_solver: 0 Jacobi-PCG kernels, 1 multigrid-preconditioned CG (AT2, hierarchy attached)
     int only_kernel = -1;    // profiling hook: restrict multi-kernel entry points to one kernel (pff_time_kernel)
     // launch configuration of every persistent chunk kernel this mesh has used, keyed by the kernel's address: the grid
     // (CTAs that fit the mesh's device with this mesh's shared-memory stage).  Presence also means the dynamic

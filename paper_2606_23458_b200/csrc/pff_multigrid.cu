@@ -298,6 +298,8 @@ __global__ void __launch_bounds__(kTPB) mg_direction_kernel(int N, const R* z, R
 }
 
 __global__ void mg_init_rz_kernel(double* sc) { sc[SC_RZ] = 1.0; }
+// pff_run_steps: counters of this solve into the device-resident tally (as the CG kernels do for the Jacobi solver)
+__global__ void mg_tally_kernel(RunTally* t, int iters, int noconv) { t->iters += iters; t->solves += 1; t->noconv += noconv; }
 
 // d <- min(1, max(d_n, d)) (L179)
 template <typename R>
@@ -643,6 +645,11 @@ static pff_status mg_solve_t(pff_mesh* m, pff_state* s0, double rel_tol, int max
     ++m->n_launches;
     if ((st = cuda_check(cudaStreamSynchronize(s), "pff_damage_solve_mg: sync")) != PFF_OK) return st;
     g->last_cycles = it;
+    if (m->defer && m->d_tally) {  // inside pff_run_steps: tallied on the device, reported once at the end of the run
+        mg_tally_kernel<<<1, 1, 0, s>>>(m->d_tally, it, result == PFF_ENOCONV ? 1 : 0);
+        ++m->n_launches;
+        return PFF_OK;
+    }
     if (iters) *iters = it;
     if (relres) *relres = nrm > 0.0 ? std::sqrt(rr) / nrm : 0.0;
     return result;

@@ -197,3 +197,35 @@ def test_mg_rejects_at1_missing_hierarchy_and_meshes_of_another_domain():
     fine1.pff_mg_attach([coarse1])
     with pytest.raises(pff.PffError):
         fine1.pff_damage_solve_mg(fine1.new_state())                    # AT1 keeps Jacobi
+
+
+@pytest.mark.gpu
+def test_run_steps_with_the_multigrid_solver_follows_the_jacobi_trajectory():
+    """pff_set_damage_solver('multigrid'): the staggered loop with the multigrid-preconditioned solve against the same loop
+    with the Jacobi kernels, both converged to 1e-11: the same trajectory (the solves have one solution), fewer
+    iterations; a single pff_damage_solve is routed the same way."""
+    import paper_2606_23458_b200 as pff
+    from pff_inputs import config
+    n = 129
+    cfg = config(5, n=n)
+    L = cfg["xy"][:, 0].max()
+    material = dict(cfg["material"], l0=4.0 * L / (n - 1))
+    levels = [grid_mesh(m, m, L, L) for m in (65, 33, 17)]
+    out = {}
+    for solver in ("jacobi", "multigrid"):
+        mesh = pff.Mesh(cfg["xy"], cfg["tri"], material)
+        mesh.pff_mg_attach([pff.Mesh(xy, tri, material) for xy, tri in levels])
+        mesh.pff_set_damage_solver(solver)
+        st = mesh.new_state(u=cfg["u0"], d=cfg["d0"])
+        bc = mesh.bc()
+        dt = 0.5 * mesh.dt_crit
+        mesh.pff_init_accel(st, bc)
+        _, its = mesh.pff_run_steps(st, bc, dt, 30, damage_every=2, rel_tol=1e-11, max_iter=2000)
+        mesh.pff_explicit_step(st, bc, dt)
+        _, it1, _ = mesh.pff_damage_solve(st, rel_tol=1e-11, max_iter=2000)
+        out[solver] = (mesh.nodes_to_user(st.d), mesh.nodes_to_user(st.ux), mesh.elems_to_user(st.H), its, it1)
+    dj, uj, Hj, its_j, it1_j = out["jacobi"]
+    dm, um, Hm, its_m, it1_m = out["multigrid"]
+    assert np.abs(dm - dj).max() <= 1e-9 * np.abs(dj).max()
+    assert np.abs(um - uj).max() <= 1e-9 * np.abs(uj).max() and np.abs(Hm - Hj).max() <= 1e-9 * np.abs(Hj).max()
+    assert 0 < its_m < its_j / 3 and 0 < it1_m < it1_j / 3
