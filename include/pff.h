@@ -216,8 +216,9 @@ pff_status pff_mg_set_params(pff_mesh *mesh, double omega, int32_t coarse_sweeps
  * nodes, stopping rule (R10) and final clamp d <- min(1, max(d_n, d)) (L179) as pff_damage_solve, and the same
  * unique solution: only the iteration count differs.  iters_out counts outer iterations (one V-cycle + one operator
  * application each; a V-cycle costs about 2.7 fine-level operator applications).  AT1 returns PFF_EUNSUPPORTED: the
- * projected solver's free set, and with it the operator a hierarchy would have to represent, changes between iterations,
- * so AT1 keeps the Jacobi preconditioner.  Synchronises the stream every iteration (host-side convergence test);
+ * projected solver (L181) truncates every step at the first bound hit, and with a global (multilevel) correction that
+ * hit comes after a near-zero step (measured: it stalls), so AT1 keeps the Jacobi preconditioner.
+ * Synchronises the stream every iteration (host-side convergence test);
  * bit-reproducible run to run.  Pays off where l0 / h is large (profiles/r2_multigrid.md); pff_damage_solve and
  * pff_run_steps use it after pff_set_damage_solver(mesh, 1). */
 pff_status pff_damage_solve_mg(pff_mesh *mesh, pff_state *state, double rel_tol, int32_t max_iter,

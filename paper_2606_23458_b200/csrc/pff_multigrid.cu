@@ -238,7 +238,7 @@ __global__ void __launch_bounds__(kTPB) mg_prolong_kernel(int N, const int32_t* 
     x[i] += c;
 }
 
-// r = mask (b - t), lb = x (the lower bound d_n of the clamp);  sc[RR] = r.r, sc[BB] = (mask b).(mask b)
+// r = mask (b - t), lb = x (the lower bound d_n of the clamp);  sc[RR] = r.r, sc[BB] = b.b
 // (the kernels with a reduction walk the vector with a grid stride: at most kRedBlocks block partials)
 template <typename R>
 __global__ void __launch_bounds__(kTPB) mg_residual0_kernel(int N, const R* dinv, const R* b, const R* t, const R* x, R* r, R* lb,
@@ -250,7 +250,7 @@ __global__ void __launch_bounds__(kTPB) mg_residual0_kernel(int N, const R* dinv
         const R ri = fr ? b[i] - t[i] : R(0);
         r[i] = ri; lb[i] = x[i];
         v[0] += double(ri) * double(ri);
-        v[1] += fr ? double(b[i]) * double(b[i]) : 0.0;
+        v[1] += double(b[i]) * double(b[i]);  // ||b|| over all nodes, as the oracle's stopping rule (R10)
     }
     const int slots[2] = {SC_RR, SC_BB};
     reduce_to_scalars<2>(v, slots, part, n_part, sc, ticket);
@@ -659,8 +659,11 @@ static pff_status mg_check(pff_mesh* m, const char* who)
 {
     if (!m->mg) { set_error(std::string(who) + ": no hierarchy attached (pff_mg_attach)"); return PFF_EINVAL; }
     if (m->mat.model != PFF_AT2) {
-        // the projected solver's free set changes between iterations and with it the operator the hierarchy would have to
-        // represent (A restricted to the free nodes); the AT1 solve stays with pff_damage_solve (Jacobi)
+        // Tried: the oracle's active-set CG (truncate the step at the first bound hit, snap, restart)
+        // with the cycle restricted to the free set as the preconditioner.  It stalls: the cycle's direction is global and
+        // pushes many nearly-active nodes towards their bound at once, so every step is a near-zero truncation (400
+        // iterations, 399 truncations, no progress; Jacobi directions are local and need 122 truncations in 200).  A
+        // multilevel AT1 solver needs another outer method (projected line search / primal-dual active set)
         set_error(std::string(who) + ": AT2 only (the projected AT1 solver keeps the Jacobi preconditioner: pff_damage_solve)");
         return PFF_EUNSUPPORTED;
     }
