@@ -1014,7 +1014,7 @@ pff_status damage_adjoint(pff_mesh* m, const pff_state* s, const void* g, const 
 }
 
 template <typename R>
-static pff_status damage_matvec_t(pff_mesh* m, const pff_state* s, const void* p, void* q, bool refresh_coef)
+static pff_status damage_matvec_t(pff_mesh* m, const pff_state* s, const void* p, void* q, bool refresh_coef, bool skip_interface)
 {
     pff_status st = ensure_workspace(m);
     if (st != PFF_OK) return st;
@@ -1031,7 +1031,7 @@ static pff_status damage_matvec_t(pff_mesh* m, const pff_state* s, const void* p
     if (m->only_kernel != 3) {
         PFF_LAUNCH(m, PFF_K_MATVEC_CHUNK, (dmg_iter_chunk<R, DM_PLAIN, false><<<(unsigned)grid_mv, kTPB, smem_mv, m->stream>>>(a)));
     }
-    if (m->only_kernel != 2) {
+    if (m->only_kernel != 2 && !skip_interface) {  // (multigrid: the consumer of q sums the interface partials itself)
         PFF_LAUNCH(m, PFF_K_MATVEC_SHARED, (dmg_plain_shared<R><<<shared_grid(m->hm), kTPB, 0, m->stream>>>(a)));
     }
     return cuda_check(cudaGetLastError(), "damage matvec launch");
@@ -1053,9 +1053,10 @@ pff_status damage_refresh_coef(pff_mesh* m, const pff_state* s)
     return m->opt.precision == PFF_F32 ? damage_refresh_coef_t<float>(m, s) : damage_refresh_coef_t<double>(m, s);
 }
 
-pff_status damage_matvec(pff_mesh* m, const pff_state* s, const void* p, void* q, bool refresh_coef)
+pff_status damage_matvec(pff_mesh* m, const pff_state* s, const void* p, void* q, bool refresh_coef, bool skip_interface)
 {
-    return m->opt.precision == PFF_F32 ? damage_matvec_t<float>(m, s, p, q, refresh_coef) : damage_matvec_t<double>(m, s, p, q, refresh_coef);
+    return m->opt.precision == PFF_F32 ? damage_matvec_t<float>(m, s, p, q, refresh_coef, skip_interface)
+                                       : damage_matvec_t<double>(m, s, p, q, refresh_coef, skip_interface);
 }
 
 template <typename R>

@@ -135,7 +135,7 @@ inline void prof_mark(pff_mesh* m, int cls)
 pff_status launch_step(pff_mesh* m, pff_state* s, const pff_bc* bc, double dt, int mode, void* fx, void* fy, void* psi,
                        const void* px = nullptr, const void* py = nullptr);
 pff_status damage_solve(pff_mesh* m, pff_state* s, double rel_tol, int max_iter, int* iters, double* relres);
-pff_status damage_matvec(pff_mesh* m, const pff_state* s, const void* p, void* q, bool refresh_coef = true);
+pff_status damage_matvec(pff_mesh* m, const pff_state* s, const void* p, void* q, bool refresh_coef = true, bool skip_interface = false);
 pff_status damage_refresh_coef(pff_mesh* m, const pff_state* s);
 // pff_multigrid.cu: geometric-multigrid-preconditioned CG for the AT2 damage solve
 pff_status mg_attach(pff_mesh* m, int n_coarse, pff_mesh* const* coarse);

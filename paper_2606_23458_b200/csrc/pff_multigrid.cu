@@ -177,6 +177,19 @@ __global__ void __launch_bounds__(kTPB) mg_restrict_H_kernel(int NeC, const int3
     Hc[E] = s;
 }
 
+// The operator's chunk kernel leaves A x of an interface node as per-chunk partials (pff_damage.cu); the vector kernel
+// that consumes A x sums them itself, in slot order, instead of a separate interface kernel per application.
+template <typename R>
+struct IfaceSum {
+    const R* part;
+    const int32_t* rowptr;
+    int N_int, N_sh, n_ovf;
+    __device__ __forceinline__ R operator()(const R* t, int i) const
+    {
+        return i < N_int ? t[i] : iface_sum<R>(part, i - N_int, N_sh, n_ovf, rowptr);
+    }
+};
+
 // x = w D^-1 b  (first smoothing step from a zero guess)
 template <typename R>
 __global__ void __launch_bounds__(kTPB) mg_smooth0_kernel(int N, R omega, const R* dinv, const R* b, R* x)
@@ -187,21 +200,21 @@ __global__ void __launch_bounds__(kTPB) mg_smooth0_kernel(int N, R omega, const 
 
 // x += w D^-1 (b - t), t = A x
 template <typename R>
-__global__ void __launch_bounds__(kTPB) mg_smooth_kernel(int N, R omega, const R* dinv, const R* b, const R* t, R* x)
+__global__ void __launch_bounds__(kTPB) mg_smooth_kernel(int N, R omega, const R* dinv, const R* b, const R* t, IfaceSum<R> ifs, R* x)
 {
     const int i = blockIdx.x * kTPB + threadIdx.x;
-    if (i < N) x[i] = rfma(omega * dinv[i], b[i] - t[i], x[i]);
+    if (i < N) x[i] = rfma(omega * dinv[i], b[i] - ifs(t, i), x[i]);
 }
 
 // x += w D^-1 (b - t) and sc[RZN] = b . x: the last smoothing step of level 0 inside the solve, where b is the residual r
 // and x becomes z
 template <typename R>
-__global__ void __launch_bounds__(kTPB) mg_smooth_dot_kernel(int N, R omega, const R* dinv, const R* b, const R* t, R* x, double* part,
-                                                             int n_part, double* sc, unsigned int* ticket)
+__global__ void __launch_bounds__(kTPB) mg_smooth_dot_kernel(int N, R omega, const R* dinv, const R* b, const R* t, IfaceSum<R> ifs, R* x,
+                                                             double* part, int n_part, double* sc, unsigned int* ticket)
 {
     double v[1] = {0.0};
     for (int i = blockIdx.x * kTPB + threadIdx.x; i < N; i += gridDim.x * kTPB) {
-        const R bi = b[i], xi = rfma(omega * dinv[i], bi - t[i], x[i]);
+        const R bi = b[i], xi = rfma(omega * dinv[i], bi - ifs(t, i), x[i]);
         x[i] = xi;
         v[0] += double(bi) * double(xi);
     }
@@ -211,10 +224,10 @@ __global__ void __launch_bounds__(kTPB) mg_smooth_dot_kernel(int N, R omega, con
 
 // t <- b - t on the free nodes, 0 elsewhere (the residual the restriction gathers)
 template <typename R>
-__global__ void __launch_bounds__(kTPB) mg_residual_kernel(int N, const R* dinv, const R* b, R* t)
+__global__ void __launch_bounds__(kTPB) mg_residual_kernel(int N, const R* dinv, const R* b, IfaceSum<R> ifs, R* t)
 {
     const int i = blockIdx.x * kTPB + threadIdx.x;
-    if (i < N) t[i] = dinv[i] != R(0) ? b[i] - t[i] : R(0);
+    if (i < N) t[i] = dinv[i] != R(0) ? b[i] - ifs(t, i) : R(0);
 }
 
 // b_c[I] = sum_j P[j, I] res[j]
@@ -264,6 +277,21 @@ __global__ void __launch_bounds__(kTPB) mg_dot_kernel(int N, const R* a, const R
     double v[1] = {0.0};
     for (int i = blockIdx.x * kTPB + threadIdx.x; i < N; i += gridDim.x * kTPB) v[0] += double(a[i]) * double(b[i]);
     const int slots[1] = {slot};
+    reduce_to_scalars<1>(v, slots, part, n_part, sc, ticket);
+}
+
+// sc[PQ] = p . q, with q of the interface nodes completed (summed and stored) on the way
+template <typename R>
+__global__ void __launch_bounds__(kTPB) mg_pq_kernel(int N, const R* p, R* q, IfaceSum<R> ifs, double* part, int n_part, double* sc,
+                                                     unsigned int* ticket)
+{
+    double v[1] = {0.0};
+    for (int i = blockIdx.x * kTPB + threadIdx.x; i < N; i += gridDim.x * kTPB) {
+        R qi = q[i];
+        if (i >= ifs.N_int) { qi = ifs(q, i); q[i] = qi; }
+        v[0] += double(p[i]) * double(qi);
+    }
+    const int slots[1] = {SC_PQ};
     reduce_to_scalars<1>(v, slots, part, n_part, sc, ticket);
 }
 
@@ -500,6 +528,12 @@ static pff_status mg_setup_operators(MgData* g, const pff_state* s0)
 }
 
 // x_l = V(b_l) on level l (b_l, x_l, t_l are the level's vectors)
+template <typename R>
+static IfaceSum<R> iface_of(const pff_mesh* m)
+{
+    return IfaceSum<R>{(const R*)m->d_halo_part, m->d_sh_rowptr, (int)m->hm.N_int, (int)m->hm.N_sh, m->hm.n_ovf};
+}
+
 constexpr int kRedBlocks = 592;  // 4 per SM of a B200
 static inline unsigned nred(int64_t n) { return (unsigned)std::min<int64_t>(kRedBlocks, std::max<int64_t>(1, (n + kTPB - 1) / kTPB)); }
 
@@ -516,27 +550,27 @@ static pff_status mg_vcycle(MgData* g, size_t l, bool dot_rz = false)
     ++m0->n_launches;
     if (l + 1 == g->lv.size()) {  // coarsest level: a fixed number of damped-Jacobi sweeps (a fixed symmetric operator)
         for (int k = 1; k < g->coarse_sweeps; ++k) {
-            if ((st = damage_matvec(L.m, &L.st, L.x, L.t, false)) != PFF_OK) return st;
-            mg_smooth_kernel<R><<<nblk(N), kTPB, 0, s>>>(N, om, (const R*)L.dinv, (const R*)L.b, (const R*)L.t, (R*)L.x);
+            if ((st = damage_matvec(L.m, &L.st, L.x, L.t, false, true)) != PFF_OK) return st;
+            mg_smooth_kernel<R><<<nblk(N), kTPB, 0, s>>>(N, om, (const R*)L.dinv, (const R*)L.b, (const R*)L.t, iface_of<R>(L.m), (R*)L.x);
             ++m0->n_launches;
         }
         return PFF_OK;
     }
     MgLevel& Cl = g->lv[l + 1];
     const int NC = (int)Cl.m->hm.N;
-    if ((st = damage_matvec(L.m, &L.st, L.x, L.t, false)) != PFF_OK) return st;
-    mg_residual_kernel<R><<<nblk(N), kTPB, 0, s>>>(N, (const R*)L.dinv, (const R*)L.b, (R*)L.t);
+    if ((st = damage_matvec(L.m, &L.st, L.x, L.t, false, true)) != PFF_OK) return st;
+    mg_residual_kernel<R><<<nblk(N), kTPB, 0, s>>>(N, (const R*)L.dinv, (const R*)L.b, iface_of<R>(L.m), (R*)L.t);
     mg_restrict_kernel<R><<<nblk(NC), kTPB, 0, s>>>(NC, L.tr.r_ptr, L.tr.r_idx, (const R*)L.tr.r_w, (const R*)L.t, (R*)Cl.b);
     m0->n_launches += 2;
     if ((st = mg_vcycle<R>(g, l + 1)) != PFF_OK) return st;
     mg_prolong_kernel<R><<<nblk(N), kTPB, 0, s>>>(N, L.tr.p_idx, (const R*)L.tr.p_w, (const R*)L.dinv, (const R*)Cl.x, (R*)L.x);
     ++m0->n_launches;
-    if ((st = damage_matvec(L.m, &L.st, L.x, L.t, false)) != PFF_OK) return st;
+    if ((st = damage_matvec(L.m, &L.st, L.x, L.t, false, true)) != PFF_OK) return st;
     if (dot_rz)
-        mg_smooth_dot_kernel<R><<<nred(N), kTPB, 0, s>>>(N, om, (const R*)L.dinv, (const R*)L.b, (const R*)L.t, (R*)L.x, g->part, g->n_part,
-                                                         g->sc, g->ticket);
+        mg_smooth_dot_kernel<R><<<nred(N), kTPB, 0, s>>>(N, om, (const R*)L.dinv, (const R*)L.b, (const R*)L.t, iface_of<R>(L.m), (R*)L.x,
+                                                         g->part, g->n_part, g->sc, g->ticket);
     else
-        mg_smooth_kernel<R><<<nblk(N), kTPB, 0, s>>>(N, om, (const R*)L.dinv, (const R*)L.b, (const R*)L.t, (R*)L.x);
+        mg_smooth_kernel<R><<<nblk(N), kTPB, 0, s>>>(N, om, (const R*)L.dinv, (const R*)L.b, (const R*)L.t, iface_of<R>(L.m), (R*)L.x);
     ++m0->n_launches;
     return PFF_OK;
 }
@@ -596,8 +630,8 @@ static pff_status mg_solve_t(pff_mesh* m, pff_state* s0, double rel_tol, int max
             ++m->n_launches;
         }
         mg_direction_kernel<R><<<nb, kTPB, 0, cs>>>(N, (const R*)F.x, (R*)g->p, g->sc);
-        if ((e = damage_matvec(m, s0, g->p, g->q, false)) != PFF_OK) return e;  // q = A p
-        mg_dot_kernel<R><<<nred(N), kTPB, 0, cs>>>(N, (const R*)g->p, (const R*)g->q, SC_PQ, g->part, g->n_part, g->sc, g->ticket);
+        if ((e = damage_matvec(m, s0, g->p, g->q, false, true)) != PFF_OK) return e;  // q = A p (interface sums in the next kernel)
+        mg_pq_kernel<R><<<nred(N), kTPB, 0, cs>>>(N, (const R*)g->p, (R*)g->q, iface_of<R>(m), g->part, g->n_part, g->sc, g->ticket);
         mg_update_kernel<R><<<nred(N), kTPB, 0, cs>>>(N, (const R*)F.dinv, (const R*)g->p, (const R*)g->q, x, (R*)g->r, g->part, g->n_part,
                                                       g->sc, g->ticket);
         m->n_launches += 3;
