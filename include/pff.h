@@ -225,10 +225,12 @@ pff_status pff_damage_solve_mg(pff_mesh *mesh, pff_state *state, double rel_tol,
                                int32_t *iters_out, double *relres_out);
 
 /* Which solver pff_damage_solve and pff_run_steps use for this mesh: 0 (default) the Jacobi-PCG kernels, 1 the
- * multigrid-preconditioned CG above (needs an attached hierarchy: PFF_EINVAL otherwise; AT2 only: PFF_EUNSUPPORTED).
+ * multigrid-preconditioned CG above (needs an attached hierarchy: PFF_EINVAL otherwise; on an AT1 mesh the forward
+ * solves keep the Jacobi kernels, only the adjoint solve changes).
  * With solver 1, pff_run_steps launches every kernel itself (no graph replay of a period: the solver tests convergence on
  * the host) and its iteration total counts outer multigrid iterations.  pff_mg_attach replacing the hierarchy keeps the
- * choice; pff_damage_adjoint always uses the Jacobi kernels. */
+ * choice.  pff_damage_adjoint follows the choice as well, for AT1 and AT2 alike (it is a linear solve on a given free set:
+ * nodes outside it are masked on the finest level like damage-Dirichlet nodes). */
 pff_status pff_set_damage_solver(pff_mesh *mesh, int32_t solver);
 
 /* Test hook: z = V(r), one cycle of the preconditioner with the operator of state->H; r, z device [n_nodes]. */

@@ -692,7 +692,6 @@ pff_status pff_set_damage_solver(pff_mesh* m, int32_t solver)
 {
     if (!m || solver < 0 || solver > 1) { set_error("pff_set_damage_solver: null mesh or solver not 0 / 1"); return PFF_EINVAL; }
     if (solver == 1 && !m->mg) { set_error("pff_set_damage_solver: no hierarchy attached (pff_mg_attach)"); return PFF_EINVAL; }
-    if (solver == 1 && m->mat.model != PFF_AT2) { set_error("pff_set_damage_solver: the multigrid solver is AT2 only"); return PFF_EUNSUPPORTED; }
     m->damage_solver = solver;
     return PFF_OK;
 }

@@ -1008,6 +1008,8 @@ pff_status damage_adjoint(pff_mesh* m, const pff_state* s, const void* g, const 
 {
     pff_status st = cuda_check(cudaMemsetAsync(lambda, 0, (size_t)m->hm.N * m->rb, m->stream), "adjoint: zero lambda");
     if (st != PFF_OK) return st;
+    // a linear solve on a given free set: the multigrid solver takes it for both models where the caller selected it
+    if (m->damage_solver == 1 && m->mg) return mg_adjoint(m, s, g, free_mask, lambda, rel_tol, max_iter, iters, relres);
     const AdjointIn in{g, free_mask, lambda};
     if (m->opt.precision == PFF_F32) return damage_solve_t<float, false>(m, s, rel_tol, max_iter, iters, relres, &in);
     return damage_solve_t<double, false>(m, s, rel_tol, max_iter, iters, relres, &in);

@@ -142,6 +142,8 @@ pff_status mg_attach(pff_mesh* m, int n_coarse, pff_mesh* const* coarse);
 pff_status mg_apply(pff_mesh* m, const pff_state* s, const void* r, void* z);
 pff_status mg_solve(pff_mesh* m, pff_state* s, double rel_tol, int max_iter, int* iters, double* relres);
 pff_status mg_set_params(pff_mesh* m, double omega, int coarse_sweeps);
+pff_status mg_adjoint(pff_mesh* m, const pff_state* s, const void* g, const uint8_t* free_mask, void* lambda, double rel_tol,
+                      int max_iter, int* iters, double* relres);
 void mg_free(pff_mesh* m);
 pff_status damage_adjoint(pff_mesh* m, const pff_state* s, const void* g, const uint8_t* free_mask, void* lambda, double rel_tol,
                           int max_iter, int* iters, double* relres);

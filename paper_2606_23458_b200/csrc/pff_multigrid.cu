@@ -55,12 +55,23 @@ struct MgData {
     int last_cycles = 0;
     // one outer iteration (V-cycle, both inner products, direction and update: ~50 small launches) captured once and
     // replayed; key = everything the captured kernel arguments depend on
-    cudaGraphExec_t graph = nullptr;
+    // (two entries: the forward solve iterates on state->d, the adjoint solve on lambda)
+    struct Graph {
+        cudaGraphExec_t exec = nullptr;
+        const void *x = nullptr, *b = nullptr;
+        double omega = 0.0;
+        int sweeps = 0, launches = 0;
+        unsigned long long used = 0;
+    } graphs[2];
+    unsigned long long graph_clock = 0;
     cudaStream_t cap_stream = nullptr;
-    const void* graph_x = nullptr;
-    double graph_omega = 0.0;
-    int graph_sweeps = 0, graph_launches = 0;
     bool graph_refused = false;
+};
+
+struct MgAdjoint {  // pff_damage_adjoint through the multigrid solver: right-hand side g, caller-given free set, result lambda
+    const void* g;
+    const uint8_t* free_mask;
+    void* lambda;
 };
 
 enum { SC_PQ = 0, SC_RZ = 1, SC_RR = 2, SC_RZN = 3, SC_BB = 4, SC_N = 8 };
@@ -166,6 +177,14 @@ __global__ void __launch_bounds__(kTPB) mg_dinv_kernel(int N, const R* D, const 
     if (i < N) dinv[i] = (flags && (flags[i] & 4)) ? R(0) : R(1) / D[i];
 }
 
+// adjoint solve: nodes outside the caller's free set are fixed as well
+template <typename R>
+__global__ void __launch_bounds__(kTPB) mg_mask_kernel(int N, const uint8_t* free_mask, R* dinv)
+{
+    const int i = blockIdx.x * kTPB + threadIdx.x;
+    if (i < N && !free_mask[i]) dinv[i] = R(0);
+}
+
 // H_c[E] = sum over the children e of E of w_e H[e]
 template <typename R>
 __global__ void __launch_bounds__(kTPB) mg_restrict_H_kernel(int NeC, const int32_t* ptr, const int32_t* idx, const R* w, const R* H, R* Hc)
@@ -254,7 +273,7 @@ __global__ void __launch_bounds__(kTPB) mg_prolong_kernel(int N, const int32_t* 
 // r = mask (b - t), lb = x (the lower bound d_n of the clamp);  sc[RR] = r.r, sc[BB] = b.b
 // (the kernels with a reduction walk the vector with a grid stride: at most kRedBlocks block partials)
 template <typename R>
-__global__ void __launch_bounds__(kTPB) mg_residual0_kernel(int N, const R* dinv, const R* b, const R* t, const R* x, R* r, R* lb,
+__global__ void __launch_bounds__(kTPB) mg_residual0_kernel(int N, int mask_b, const R* dinv, const R* b, const R* t, const R* x, R* r, R* lb,
                                                             double* part, int n_part, double* sc, unsigned int* ticket)
 {
     double v[2] = {0.0, 0.0};
@@ -263,7 +282,8 @@ __global__ void __launch_bounds__(kTPB) mg_residual0_kernel(int N, const R* dinv
         const R ri = fr ? b[i] - t[i] : R(0);
         r[i] = ri; lb[i] = x[i];
         v[0] += double(ri) * double(ri);
-        v[1] += double(b[i]) * double(b[i]);  // ||b|| over all nodes, as the oracle's stopping rule (R10)
+        v[1] += (fr || !mask_b) ? double(b[i]) * double(b[i]) : 0.0;  // ||b|| over all nodes, as the oracle's stopping rule
+                                                                        // (R10); adjoint: over the free set (g_F is the rhs)
     }
     const int slots[2] = {SC_RR, SC_BB};
     reduce_to_scalars<2>(v, slots, part, n_part, sc, ticket);
@@ -437,7 +457,7 @@ void mg_free(pff_mesh* m)
     void* ps[] = {g->r, g->p, g->q, g->lb, g->part, g->sc, g->ticket};
     for (void* p : ps) if (p) cudaFree(p);
     if (g->h_sc) cudaFreeHost(g->h_sc);
-    if (g->graph) cudaGraphExecDestroy(g->graph);
+    for (auto& gr : g->graphs) if (gr.exec) cudaGraphExecDestroy(gr.exec);
     if (g->cap_stream) cudaStreamDestroy(g->cap_stream);
     delete g;
     m->mg = nullptr;
@@ -590,23 +610,30 @@ static pff_status mg_apply_t(pff_mesh* m, const pff_state* s0, const void* r, vo
 }
 
 template <typename R>
-static pff_status mg_solve_t(pff_mesh* m, pff_state* s0, double rel_tol, int max_iter, int* iters, double* relres)
+static pff_status mg_solve_t(pff_mesh* m, const pff_state* s0, double rel_tol, int max_iter, int* iters, double* relres,
+                             const MgAdjoint* adj = nullptr)
 {
     MgData* g = static_cast<MgData*>(m->mg);
     MgLevel& F = g->lv[0];
     cudaStream_t s = m->stream;
     const int N = (int)m->hm.N;
     const unsigned nb = nblk(N);
-    R* x = (R*)s0->d;
+    R* x = adj ? (R*)adj->lambda : (R*)s0->d;
     pff_status st = mg_setup_operators<R>(g, s0);  // F.b = b(H)
     if (st != PFF_OK) return st;
+    void* const b_own = F.b;
+    if (adj) {  // A_FF lambda_F = g_F from lambda = 0 (the caller zeroed it): rhs g, free set = the caller's minus the fixed nodes
+        if (adj->free_mask) { mg_mask_kernel<R><<<nb, kTPB, 0, s>>>(N, adj->free_mask, (R*)F.dinv); ++m->n_launches; }
+        F.b = const_cast<void*>(adj->g);
+    }
+    struct Restore { MgLevel& F; void* b; ~Restore() { F.b = b; } } restore{F, b_own};
     auto read_scalars = [&]() -> pff_status {
         MG_CUDA(cudaMemcpyAsync(g->h_sc, g->sc, sizeof(double) * SC_N, cudaMemcpyDeviceToHost, s));
         return cuda_check(cudaStreamSynchronize(s), "pff_damage_solve_mg: sync");
     };
     // r0 = mask (b - A d_n), lb = d_n; stopping rule of pff_damage_solve (R10)
     if ((st = damage_matvec(m, s0, x, F.t, false)) != PFF_OK) return st;
-    mg_residual0_kernel<R><<<nred(N), kTPB, 0, s>>>(N, (const R*)F.dinv, (const R*)F.b, (const R*)F.t, x, (R*)g->r, (R*)g->lb, g->part, g->n_part,
+    mg_residual0_kernel<R><<<nred(N), kTPB, 0, s>>>(N, adj ? 1 : 0, (const R*)F.dinv, (const R*)F.b, (const R*)F.t, x, (R*)g->r, (R*)g->lb, g->part, g->n_part,
                                                g->sc, g->ticket);
     ++m->n_launches;
     if ((st = read_scalars()) != PFF_OK) return st;
@@ -640,46 +667,55 @@ static pff_status mg_solve_t(pff_mesh* m, pff_state* s0, double rel_tol, int max
     // captured once per (x, omega, sweeps): recorded on a stream of the library's own (the caller's may be the legacy
     // default stream, which cannot capture); every level launches on the recording stream while it is recorded
     const bool want_graph = m->graph_mode != 0 && !g->graph_refused && !m->prof_on;
-    if (want_graph && (!g->graph || g->graph_x != (const void*)x || g->graph_omega != g->omega || g->graph_sweeps != g->coarse_sweeps)) {
-        if (g->graph) { cudaGraphExecDestroy(g->graph); g->graph = nullptr; }
-        cudaError_t ce = g->cap_stream ? cudaSuccess : cudaStreamCreateWithFlags(&g->cap_stream, cudaStreamNonBlocking);
-        cudaGraph_t graph = nullptr;
-        pff_status cst = PFF_OK;
-        if (ce == cudaSuccess) ce = cudaStreamBeginCapture(g->cap_stream, cudaStreamCaptureModeThreadLocal);
-        if (ce == cudaSuccess) {
-            std::vector<int64_t> before;
-            for (MgLevel& L : g->lv) { before.push_back(L.m->n_launches); L.m->stream = g->cap_stream; }
-            cst = iteration();
-            g->graph_launches = 0;
-            for (size_t l = 0; l < g->lv.size(); ++l) {
-                MgLevel& L = g->lv[l];
-                L.m->stream = s;
-                g->graph_launches += int(L.m->n_launches - before[l]);
-                L.m->n_launches = before[l];  // recorded, not launched
+    MgData::Graph* gr = nullptr;
+    if (want_graph) {
+        for (auto& c : g->graphs)
+            if (c.exec && c.x == (const void*)x && c.b == (const void*)b_keep && c.omega == g->omega && c.sweeps == g->coarse_sweeps) gr = &c;
+        if (!gr) {  // record into the least recently used entry
+            gr = g->graphs[0].used <= g->graphs[1].used ? &g->graphs[0] : &g->graphs[1];
+            if (gr->exec) { cudaGraphExecDestroy(gr->exec); gr->exec = nullptr; }
+            cudaError_t ce = g->cap_stream ? cudaSuccess : cudaStreamCreateWithFlags(&g->cap_stream, cudaStreamNonBlocking);
+            cudaGraph_t graph = nullptr;
+            pff_status cst = PFF_OK;
+            if (ce == cudaSuccess) ce = cudaStreamBeginCapture(g->cap_stream, cudaStreamCaptureModeThreadLocal);
+            if (ce == cudaSuccess) {
+                std::vector<int64_t> before;
+                for (MgLevel& L : g->lv) { before.push_back(L.m->n_launches); L.m->stream = g->cap_stream; }
+                cst = iteration();
+                gr->launches = 0;
+                for (size_t l = 0; l < g->lv.size(); ++l) {
+                    MgLevel& L = g->lv[l];
+                    L.m->stream = s;
+                    gr->launches += int(L.m->n_launches - before[l]);
+                    L.m->n_launches = before[l];  // recorded, not launched
+                }
+                ce = cudaStreamEndCapture(g->cap_stream, &graph);
             }
-            ce = cudaStreamEndCapture(g->cap_stream, &graph);
+            if (ce == cudaSuccess && cst == PFF_OK && graph) ce = cudaGraphInstantiate(&gr->exec, graph, 0);
+            if (graph) cudaGraphDestroy(graph);
+            if (ce != cudaSuccess || cst != PFF_OK || !gr->exec) { cudaGetLastError(); gr->exec = nullptr; gr = nullptr; g->graph_refused = true; }
+            else { gr->x = x; gr->b = b_keep; gr->omega = g->omega; gr->sweeps = g->coarse_sweeps; }
         }
-        if (ce == cudaSuccess && cst == PFF_OK && graph) ce = cudaGraphInstantiate(&g->graph, graph, 0);
-        if (graph) cudaGraphDestroy(graph);
-        if (ce != cudaSuccess || cst != PFF_OK || !g->graph) { cudaGetLastError(); g->graph = nullptr; g->graph_refused = true; }
-        else { g->graph_x = x; g->graph_omega = g->omega; g->graph_sweeps = g->coarse_sweeps; }
+        if (gr) gr->used = ++g->graph_clock;
     }
     while (std::sqrt(rr) > lim) {
         if (it >= max_iter) { set_error("pff_damage_solve_mg: max_iter reached"); result = PFF_ENOCONV; break; }
-        if (want_graph && g->graph) {
-            MG_CUDA(cudaGraphLaunch(g->graph, s));
-            m->n_launches += g->graph_launches;
+        if (gr) {
+            MG_CUDA(cudaGraphLaunch(gr->exec, s));
+            m->n_launches += gr->launches;
         } else if ((st = iteration()) != PFF_OK) return st;
         ++it;
         if ((st = read_scalars()) != PFF_OK) return st;
         rr = g->h_sc[SC_RR];
         if (!(g->h_sc[SC_PQ] > 0.0) || !std::isfinite(rr)) { set_error("pff_damage_solve_mg: breakdown (p.Ap <= 0)"); result = PFF_ENOCONV; break; }
     }
-    mg_clamp_kernel<R><<<nb, kTPB, 0, s>>>(N, (const R*)g->lb, x);
-    ++m->n_launches;
+    if (!adj) {
+        mg_clamp_kernel<R><<<nb, kTPB, 0, s>>>(N, (const R*)g->lb, x);
+        ++m->n_launches;
+    }
     if ((st = cuda_check(cudaStreamSynchronize(s), "pff_damage_solve_mg: sync")) != PFF_OK) return st;
     g->last_cycles = it;
-    if (m->defer && m->d_tally) {  // inside pff_run_steps: tallied on the device, reported once at the end of the run
+    if (!adj && m->defer && m->d_tally) {  // inside pff_run_steps: tallied on the device, reported once at the end of the run
         mg_tally_kernel<<<1, 1, 0, s>>>(m->d_tally, it, result == PFF_ENOCONV ? 1 : 0);
         ++m->n_launches;
         return PFF_OK;
@@ -717,6 +753,16 @@ pff_status mg_solve(pff_mesh* m, pff_state* s, double rel_tol, int max_iter, int
     if (st != PFF_OK) return st;
     return m->opt.precision == PFF_F32 ? mg_solve_t<float>(m, s, rel_tol, max_iter, iters, relres)
                                        : mg_solve_t<double>(m, s, rel_tol, max_iter, iters, relres);
+}
+
+// pff_damage_adjoint with the multigrid solver (a linear solve on a given free set: AT1 and AT2 alike)
+pff_status mg_adjoint(pff_mesh* m, const pff_state* s, const void* gvec, const uint8_t* free_mask, void* lambda, double rel_tol,
+                      int max_iter, int* iters, double* relres)
+{
+    if (!m->mg) { set_error("pff_damage_adjoint: no hierarchy attached"); return PFF_EINVAL; }
+    const MgAdjoint adj{gvec, free_mask, lambda};
+    return m->opt.precision == PFF_F32 ? mg_solve_t<float>(m, s, rel_tol, max_iter, iters, relres, &adj)
+                                       : mg_solve_t<double>(m, s, rel_tol, max_iter, iters, relres, &adj);
 }
 
 pff_status mg_set_params(pff_mesh* m, double omega, int coarse_sweeps)
