@@ -46,7 +46,10 @@ def algorithmic_bytes(N: int, Ne: int, w: int) -> dict:
     """SURVEY.md 8(d) / DESIGN.md "Algorithmic bytes": every persistent array touched once per pass."""
     step = Ne * (12 + 5 * w + 2 * w) + N * 16 * w          # conn + geometry + H r/w ; u,v,a r/w, d, f_ext, m^-1
     matvec = Ne * (12 + 5 * w + w) + N * 2 * w             # conn + geometry + H ; p read, q write
-    return dict(step=step, matvec=matvec, cg_iter=matvec + N * 8 * w)
+    # the setup pass of the damage solve, when the explicit-step kernel performs it too (pff_set_fused_setup): what it adds
+    # to that kernel's traffic -- 4 operator coefficients per element and r0, 1/D, d_n, mask per node, all written
+    fused_extra = Ne * 4 * w + N * (3 * w + 1)
+    return dict(step=step, matvec=matvec, cg_iter=matvec + N * 8 * w, fused_extra=fused_extra)
 
 
 def reduce_max(value: float, world: int, device) -> float:
@@ -129,6 +132,8 @@ def run_ours(args, rank: int, world: int):
         mesh.pff_set_damage_dirichlet(cfg["notch"])
     if args.no_graph:
         mesh.pff_set_graph_mode(False)
+    if args.no_fused_setup:
+        mesh.pff_set_fused_setup(False)
     mesh.pff_set_cg_variant({"auto": 0, "two-rendezvous": 1, "one-rendezvous": 2}[args.cg])
     N, Ne = mesh.n_nodes, mesh.n_elems
     dt = cfg["dt_factor"] * mesh.dt_crit
@@ -171,11 +176,15 @@ def run_ours(args, rank: int, world: int):
     iters = [iters[int(np.argsort(ms_runs)[len(ms_runs) // 2])]]  # CG iterations of the median run
     launches = (mesh.pff_mesh_counters() - l0) // args.repeats
     cg_kernel_used = {1: "two-rendezvous", 2: "one-rendezvous"}.get(mesh.pff_last_cg_kernel(), "none")
+    fused_used = mesh.pff_fused_setup_used()
     clk = clocks.stop()
 
     # --- same K steps again with per-kernel event brackets: attribution for the roofline block
+    # (through the same pff_run_steps call as the timed region, so that the kernels attributed are the ones it launches:
+    # the event brackets only switch the graph replay off)
     mesh.pff_profile_enable(True)
-    _, iters_p = timed(step, args.steps)
+    _, iters_p = timed(lambda: mesh.pff_run_steps(st, bc, dt, args.steps, damage_every=1, rel_tol=REL_TOL, max_iter=MAX_ITER,
+                                                  allow_noconv=True)[1], 1)
     prof = mesh.pff_profile_read()
     mesh.pff_profile_enable(False)
     # explicit step and CG iteration timed alone (device-resident), for the secondary metrics
@@ -282,7 +291,7 @@ def run_ours(args, rank: int, world: int):
     eq_call()
     ms_eq, it_eq = timed(eq_call, 1)
     return dict(mesh=mesh, cfg=cfg, N=N, Ne=Ne, w=w, cg_kernels=cg_kernels, cg_kernel_used=cg_kernel_used, ms_total=ms_total, ms_runs=ms_runs, iters=iters, launches=launches, clk=clk, prof=prof,
-                iters_p=iters_p, ms_exp=ms_exp, ms_adj=ms_adj / 5, it_adj=it_adj[0], ms_act=ms_act / args.steps, ms_eq=ms_eq, it_eq=it_eq[0], mg=mg, e2e_val=e2e_val, h2d=(9 * N + Ne) * 8, d2h=(7 * N + Ne) * 8, snapshot=snapshot)
+                iters_p=iters_p, ms_exp=ms_exp, ms_adj=ms_adj / 5, it_adj=it_adj[0], ms_act=ms_act / args.steps, ms_eq=ms_eq, it_eq=it_eq[0], mg=mg, fused=fused_used, e2e_val=e2e_val, h2d=(9 * N + Ne) * 8, d2h=(7 * N + Ne) * 8, snapshot=snapshot)
 
 
 NOMINAL_GBS = 8000.0  # the "~8 TB/s" north_star names; reported beside the measured copy peak
@@ -355,6 +364,8 @@ def main():
                          "size and the previous solve's pass count")
     ap.add_argument("--no-multigrid", action="store_true", help="skip the multigrid-against-Jacobi leg (cfg5 workloads)")
     ap.add_argument("--mg-l0-over-h", type=float, default=4.0, help="regularisation length of the multigrid leg's mesh, in mesh sizes")
+    ap.add_argument("--no-fused-setup", action="store_true", help="pff_run_steps launches the damage setup kernel separately instead of "
+                    "performing that pass inside the explicit-step kernel")
     ap.add_argument("--no-graph", action="store_true", help="pff_run_steps launches every kernel itself instead of replaying a captured period")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -386,7 +397,8 @@ def main():
     iters_prof = int(sum(r["iters_p"]))  # CG iterations of the event-bracketed pass
     # step_chunk: one launch = one explicit step of the whole mesh; cg_solve: one cooperative launch = ALL CG iterations
     # of one damage solve, credited with the per-iteration algorithmic bytes x the iterations it ran
-    for name, cls, nbytes in (("step_chunk", "step_chunk", ab["step"]),
+    fused = bool(r["fused"])
+    for name, cls, nbytes in (("step_chunk", "step_chunk", ab["step"] + (ab["fused_extra"] if fused else 0)),
                               ("cg_solve", "matvec_chunk", ab["cg_iter"] * iters_prof / max(prof["matvec_chunk"][1], 1))):
         ms, cnt = prof[cls]
         if cnt:
@@ -395,7 +407,10 @@ def main():
                               algorithmic_bytes=int(nbytes), achieved_gbs=nbytes / per / 1e6, frac=nbytes / per / 1e6 / peak,
                               frac_nominal_8tbs=nbytes / per / 1e6 / NOMINAL_GBS)
             cap = ncu_capture(args.workload, "f64" if w == 8 else "f32",
-                              "cg_solve_one_rendezvous" if name == "cg_solve" and r["cg_kernel_used"] == "one-rendezvous" else name)
+                              "cg_solve_one_rendezvous" if name == "cg_solve" and r["cg_kernel_used"] == "one-rendezvous"
+                              else ("step_chunk_fused" if name == "step_chunk" and fused else name))
+            if name == "step_chunk":
+                kern[name]["fused_damage_setup"] = fused
             if cap:  # from the committed `ncu --set full` capture of this workload (profiles/traffic.csv), per captured launch
                 kern[name]["dram_pct_ncu"] = cap["dram_pct"]
                 kern[name]["dram_bytes_ncu_per_unit"] = cap["bytes"] / cap["units"]
@@ -416,6 +431,8 @@ def main():
                             cg_kernel=args.cg, cg_kernel_used=r["cg_kernel_used"],
                             l0_over_h=args.l0_over_h if args.l0_over_h is not None else "recipe",
                             time_loop="plain launches" if args.no_graph else "CUDA graph replay of one captured step + solve",
+                            kernels_per_step="2: explicit step with the damage solve's setup pass fused in, CG" if r["fused"]
+                            else "3: explicit step, damage setup, CG",
                             parallelism=f"replicas x{world}"),
                 # the explicit step INSIDE the staggered loop (what a user gets) is the number; timed back to back alone it
                 # runs a little faster (warm instruction cache, no solve in between) and is reported as secondary

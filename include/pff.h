@@ -251,6 +251,16 @@ pff_status pff_set_cg_variant(pff_mesh *mesh, int32_t variant);
 /* kernel <- 1 / 2: which of the two the last solve of this mesh launched (0: none yet).  Host-only. */
 pff_status pff_last_cg_kernel(const pff_mesh *mesh, int32_t *kernel);
 
+/* pff_run_steps: the explicit step that precedes a damage solve also performs that solve's SETUP PASS (right-hand side,
+ * Jacobi diagonal, first residual, operator coefficients, norms, control block) in the same kernel: everything the pass
+ * reads -- connectivity, geometry, area, the new history value, d -- is already in the step kernel's shared memory, so
+ * the separate setup kernel with its 120 MB of re-reads disappears (two kernels per staggered step instead of three).
+ * Same arithmetic in the same order: results are bit-identical to the three-kernel sequence.  Used where it applies: fp64,
+ * gather scatter, Jacobi solver; enable = 0 switches it off (A/B timing).  pff_explicit_step + pff_damage_solve (one call
+ * each) always run the separate kernels.  used <- whether the last pff_run_steps fused.  Host-only. */
+pff_status pff_set_fused_setup(pff_mesh *mesh, int32_t enable);
+pff_status pff_fused_setup_used(const pff_mesh *mesh, int32_t *used);
+
 /* Counters of the last pff_damage_solve / pff_damage_adjoint of this mesh (of ALL solves of the last pff_run_steps):
  * restarts = how often the projected solver (AT1, L181) re-derived its free set after the first time (a bound became
  * inactive, or a step was truncated); truncations = steps cut short at the first bound hit.  Both 0 for AT2.

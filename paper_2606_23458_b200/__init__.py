@@ -153,6 +153,14 @@ class Mesh:
                     allow=(PFF_ENOCONV,) if allow_noconv else ())
         return st, it.value, rr.value
 
+    def pff_set_fused_setup(self, enable: bool):
+        _check(self.L.pff_set_fused_setup(self.h, int(bool(enable))))
+
+    def pff_fused_setup_used(self) -> bool:
+        k = C.c_int32(0)
+        _check(self.L.pff_fused_setup_used(self.h, C.byref(k)))
+        return bool(k.value)
+
     def pff_set_cg_variant(self, variant: int):
         _check(self.L.pff_set_cg_variant(self.h, int(variant)))
 

@@ -20,7 +20,7 @@ KERNEL_CLASSES = ("step_chunk", "step_shared", "matvec_chunk", "matvec_shared", 
 SYMBOLS = [
     "pff_mesh_create", "pff_mesh_plan", "pff_mesh_destroy", "pff_mesh_info", "pff_mesh_permutations", "pff_set_dirichlet",
     "pff_set_damage_dirichlet", "pff_set_traction", "pff_init_accel", "pff_explicit_step", "pff_damage_solve",
-    "pff_energies", "pff_energies_static", "pff_mg_attach", "pff_set_damage_solver", "pff_mg_set_params", "pff_damage_solve_mg", "pff_mg_apply", "pff_set_cg_variant", "pff_last_cg_kernel", "pff_damage_last_stats", "pff_subcycle_limit", "pff_run_steps", "pff_set_graph_mode", "pff_graph_status", "pff_damage_adjoint", "pff_damage_param_terms", "pff_stiffness_action", "pff_equilibrium_solve", "pff_internal_force", "pff_damage_matvec", "pff_damage_rhs_diag", "pff_run_host", "pff_mesh_counters", "pff_time_kernel",
+    "pff_energies", "pff_set_fused_setup", "pff_fused_setup_used", "pff_energies_static", "pff_mg_attach", "pff_set_damage_solver", "pff_mg_set_params", "pff_damage_solve_mg", "pff_mg_apply", "pff_set_cg_variant", "pff_last_cg_kernel", "pff_damage_last_stats", "pff_subcycle_limit", "pff_run_steps", "pff_set_graph_mode", "pff_graph_status", "pff_damage_adjoint", "pff_damage_param_terms", "pff_stiffness_action", "pff_equilibrium_solve", "pff_internal_force", "pff_damage_matvec", "pff_damage_rhs_diag", "pff_run_host", "pff_mesh_counters", "pff_time_kernel",
     "pff_profile_enable", "pff_profile_read", "pff_trace_set",
     "pff_last_error",
 ]
@@ -85,6 +85,8 @@ def load() -> C.CDLL:
     L.pff_mg_apply.argtypes = [vp, C.POINTER(pff_state), vp, vp]
     L.pff_damage_last_stats.argtypes = [vp, ip, ip]
     L.pff_set_cg_variant.argtypes = [vp, i32]
+    L.pff_set_fused_setup.argtypes = [vp, i32]
+    L.pff_fused_setup_used.argtypes = [vp, C.POINTER(i32)]
     L.pff_last_cg_kernel.argtypes = [vp, ip]
     L.pff_subcycle_limit.argtypes = [C.POINTER(pff_material), ip, dp]
     L.pff_run_steps.argtypes = [vp, C.POINTER(pff_state), C.POINTER(pff_bc), C.c_double, i64, i32, C.c_double, i32, C.POINTER(i64)]

@@ -109,7 +109,7 @@ void pff_mesh_destroy(pff_mesh* m)
                     m->d_halo_ids, m->d_sh_rowptr, m->d_halo_dst, m->d_ell, m->d_flags, m->d_halo_part,
                     m->d_fwx, m->d_fwy, m->d_dir_dof, m->d_ca, m->d_cb, m->d_lb, m->d_r, m->d_p, m->d_q, m->d_dinv, m->d_mask,
                     m->d_part, m->d_tally, m->d_cg2, m->d_ctrl, m->d_ticket, m->d_step_bar, m->d_stage, m->d_hstate, m->d_hdir, m->d_node_old_of_new,
-                    m->d_elem_old_of_new, m->d_n2e_ptr, m->d_n2e, m->d_eq_vec, m->d_eq_part, m->d_eq_ctrl, m->d_eq_ticket};
+                    m->d_elem_old_of_new, m->d_n2e_ptr, m->d_n2e, m->d_eq_vec, m->d_eq_part, m->d_eq_ctrl, m->d_eq_ticket, m->d_su_part};
     for (void* p : ptrs) if (p) cudaFree(p);
     if (m->h_ctrl) cudaFreeHost(m->h_ctrl);
     if (m->h_tally) cudaFreeHost(m->h_tally);
@@ -165,6 +165,7 @@ pff_status pff_mesh_create(int64_t n_nodes, const double* xy, int64_t n_elems, c
     }
     m->lay_step = make_stage_layout(0, hm.chunk_elems, hm.node_len, hm.flag_len, hm.ell_len, hm.max_nhalo, m->rb, chunk_kernel_stages(0));
     m->lay_mv = make_stage_layout(1, hm.chunk_elems, hm.node_len, hm.flag_len, hm.ell_len, hm.max_nhalo, m->rb, chunk_kernel_stages(1));
+    m->lay_stepsu = make_stage_layout(5, hm.chunk_elems, hm.node_len, hm.flag_len, hm.ell_len, hm.max_nhalo, m->rb, chunk_kernel_stages(0));
     m->lay_eq = make_stage_layout(3, hm.chunk_elems, hm.node_len, hm.flag_len, hm.ell_len, hm.max_nhalo, m->rb, chunk_kernel_stages(0));
     m->lay_su = make_stage_layout(2, hm.chunk_elems, hm.node_len, hm.flag_len, hm.ell_len, hm.max_nhalo, m->rb, chunk_kernel_stages(2));
     m->ell_total = (int64_t)hm.ell.size();
@@ -440,9 +441,16 @@ pff_status pff_run_steps(pff_mesh* m, pff_state* s, const pff_bc* bc, double dt,
     PFF_CUDA(cudaMemsetAsync(m->d_tally, 0, sizeof(RunTally), m->stream));
     pff_status st = PFF_OK;
     m->defer = true;
+    // The explicit step that precedes a damage solve also performs that solve's setup pass where the mesh allows it
+    // (pff_step.cu MODE_STEPSU: everything the pass reads is already in the step kernel's shared memory).
+    const bool fuse = fused_setup_ok(m);
+    m->last_step_fused = fuse && damage_every > 0 ? 1 : 0;
     auto one_step = [&](int64_t k) -> pff_status {
-        pff_status e = launch_step(m, s, bc, dt, /*MODE_STEP*/ 0, nullptr, nullptr, nullptr);
-        if (e == PFF_OK && damage_every > 0 && k % damage_every == 0) e = damage_solve(m, s, rel_tol, max_iter, nullptr, nullptr);
+        const bool solve = damage_every > 0 && k % damage_every == 0;
+        m->su_tol = rel_tol; m->su_max_iter = max_iter;
+        pff_status e = launch_step(m, s, bc, dt, solve && fuse ? /*MODE_STEPSU*/ 5 : /*MODE_STEP*/ 0, nullptr, nullptr, nullptr);
+        if (e == PFF_OK && solve) e = damage_solve(m, s, rel_tol, max_iter, nullptr, nullptr);
+        m->su_ready = false;
         return e;
     };
     const int64_t period = damage_every > 0 ? damage_every : 1;
@@ -452,10 +460,11 @@ pff_status pff_run_steps(pff_mesh* m, pff_state* s, const pff_bc* bc, double dt,
     const bool want_graph = m->graph_mode != 0 && !m->graph_unsupported && !m->prof_on && period <= 64 && n_steps >= 4 * period && !mg_solver;
     if (want_graph) {
         // key of everything a captured period depends on (kernel arguments are frozen at capture time)
-        struct Key { pff_state s; pff_bc bc; double dt, tol; int32_t every, max_iter; int64_t n_dir; uint64_t flags_gen; int32_t variant; } key{};
+        struct Key { pff_state s; pff_bc bc; double dt, tol; int32_t every, max_iter; int64_t n_dir; uint64_t flags_gen; int32_t variant, fuse; } key{};
         key.s = *s; if (bc) key.bc = *bc; else key.bc.load_scale = 1.0;
         key.dt = dt; key.tol = rel_tol; key.every = damage_every; key.max_iter = max_iter; key.n_dir = m->n_dir; key.flags_gen = m->flags_gen;
         key.variant = m->cg_variant;  // decides which CG kernel the frozen period launches
+        key.fuse = fuse ? 1 : 0;
         const unsigned char* kb = reinterpret_cast<const unsigned char*>(&key);
         const bool cached = m->graph_exec && m->graph_key.size() == sizeof(Key) && std::memcmp(m->graph_key.data(), kb, sizeof(Key)) == 0;
         if (!cached) {
@@ -525,6 +534,20 @@ pff_status pff_last_cg_kernel(const pff_mesh* m, int32_t* kernel)
 {
     if (!m || !kernel) { set_error("pff_last_cg_kernel: null argument"); return PFF_EINVAL; }
     *kernel = m->last_cg_kernel;
+    return PFF_OK;
+}
+
+pff_status pff_set_fused_setup(pff_mesh* m, int32_t enable)
+{
+    if (!m) { set_error("pff_set_fused_setup: null mesh"); return PFF_EINVAL; }
+    m->fuse_setup = enable != 0;
+    return PFF_OK;
+}
+
+pff_status pff_fused_setup_used(const pff_mesh* m, int32_t* used)
+{
+    if (!m || !used) { set_error("pff_fused_setup_used: null argument"); return PFF_EINVAL; }
+    *used = m->last_step_fused;
     return PFF_OK;
 }
 

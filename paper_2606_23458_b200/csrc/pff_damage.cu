@@ -112,34 +112,7 @@ __device__ __forceinline__ R cg_node_prologue(const IterScalars& sc, R& x, R& r,
     return sc.restart ? z : rfma(R(sc.beta), p, z);
 }
 
-// element operator q^e = (c_e M^e + kappa K^e) p^e with M^e = A (1 + delta_ij) / 12 (L185), from the geometry
-template <typename R>
-__device__ __forceinline__ void elem_damage_apply(const MatC<R>& mat, R b1, R c1, R b2, R c2, R A, R He, R p1, R p2, R p3,
-                                                  R& q1, R& q2, R& q3)
-{
-    const R ce = mat.c0 + R(2) * He;  // reaction coefficient (Eq. 6 / Eq. 8)
-    const R m12 = ce * A * R(1.0 / 12.0), sum = p1 + p2 + p3;
-    const R gx = b1 * (p1 - p3) + b2 * (p2 - p3), gy = c1 * (p1 - p3) + c2 * (p2 - p3);
-    const R kA = mat.kappa * A;
-    const R k1 = kA * (b1 * gx + c1 * gy), k2 = kA * (b2 * gx + c2 * gy);
-    q1 = m12 * (p1 + sum) + k1;
-    q2 = m12 * (p2 + sum) + k2;
-    q3 = m12 * (p3 + sum) - (k1 + k2);
-}
-
-// The same operator from its 4 coefficients (what the CG iterations stream instead of geometry + area + H):
-// m = c_e A / 12 and the edge weights w_ij = -kappa A grad phi_i . grad phi_j of the P1 stiffness (rows sum to zero,
-// so K^e p = sum_j w_ij (p_i - p_j)).
-template <typename R>
-__device__ __forceinline__ void elem_coefficients(const MatC<R>& mat, R b1, R c1, R b2, R c2, R A, R He, R& m, R& w12, R& w13,
-                                                  R& w23)
-{
-    const R kA = mat.kappa * A;
-    m = (mat.c0 + R(2) * He) * A * R(1.0 / 12.0);
-    w12 = -kA * (b1 * b2 + c1 * c2);
-    w13 = kA * (b1 * (b1 + b2) + c1 * (c1 + c2));
-    w23 = kA * (b2 * (b1 + b2) + c2 * (c1 + c2));
-}
+// (elem_damage_apply and elem_coefficients live in pff_device.cuh: the explicit-step kernel's fused setup uses them too)
 template <typename R>
 __device__ __forceinline__ void elem_damage_apply_coef(R m, R w12, R w13, R w23, R p1, R p2, R p3, R& q1, R& q2, R& q3)
 {
@@ -895,6 +868,20 @@ static pff_status launch_setup(pff_mesh* m, DmgArgs<R>& asu, const void* kern, u
     return PFF_OK;
 }
 
+// Which CG kernel an unconstrained / projected forward solve of this mesh runs (see damage_solve_t): true = the
+// one-rendezvous kernel.  Shared with the fused setup of the explicit-step kernel, which must store 1/D the same way.
+template <typename R>
+static pff_status solve_uses_cg2(pff_mesh* m, bool proj, bool* cg2, int* grid_cg2_out = nullptr)
+{
+    int grid_cg2 = 0;
+    pff_status st = persistent_config(m, (const void*)dmg_cg2_chunk<R>, (int)m->lay_mv.total, &grid_cg2);
+    if (st != PFF_OK) return st;
+    const bool eligible = !proj && m->hm.n_ovf == 0;
+    *cg2 = eligible && (m->cg_variant == 2 || (m->cg_variant == 0 && m->hm.C <= (int64_t)16 * grid_cg2));
+    if (grid_cg2_out) *grid_cg2_out = grid_cg2;
+    return PFF_OK;
+}
+
 struct AdjointIn {
     const void* g;
     const uint8_t* free_mask;
@@ -922,10 +909,8 @@ static pff_status damage_solve_t(pff_mesh* m, const pff_state* s, double rel_tol
     // for its one extra (cheaper) pass per solve: -25 % per solve up to 10^5 nodes, a tie at 10^6 nodes and 12 passes, -5 % at
     // 85 passes (profiles/r2_cg_kernels.md).  On larger meshes the tail is amortised and the extra pass is a loss (4e6
     // nodes, 12 passes: +6 %).  The projected solver (AT1) and irregular decompositions keep the two-rendezvous kernel.
-    int grid_cg2 = 0;
-    if ((st = persistent_config(m, (const void*)dmg_cg2_chunk<R>, (int)m->lay_mv.total, &grid_cg2)) != PFF_OK) return st;
-    const bool eligible = !PROJ && hm.n_ovf == 0;
-    const bool cg2 = eligible && (m->cg_variant == 2 || (m->cg_variant == 0 && hm.C <= (int64_t)16 * grid_cg2));
+    bool cg2 = false;
+    if ((st = solve_uses_cg2<R>(m, PROJ, &cg2)) != PFF_OK) return st;
     m->last_cg_kernel = cg2 ? 2 : 1;
     const void* cg_kernel = cg2 ? (const void*)dmg_cg2_chunk<R> : (const void*)dmg_iter_chunk<R, DM_CG, PROJ>;
     Cg2Args<R> c2{};
@@ -964,7 +949,10 @@ static pff_status damage_solve_t(pff_mesh* m, const pff_state* s, double rel_tol
         }
         c2.d = a;
     }
-    if ((st = launch_setup(m, asu, (const void*)dmg_setup_chunk<R, false>, gsu, smem_su)) != PFF_OK) return st;
+    // the explicit-step kernel of pff_run_steps may have done this solve's setup pass already (pff_step.cu MODE_STEPSU)
+    const bool fused = m->su_ready && !adj && m->su_tol == rel_tol && m->su_max_iter == max_iter && m->su_zero_dinv == asu.zero_dinv_fixed;
+    m->su_ready = false;
+    if (!fused && (st = launch_setup(m, asu, (const void*)dmg_setup_chunk<R, false>, gsu, smem_su)) != PFF_OK) return st;
     // ONE cooperative launch runs every CG iteration (grid-wide barriers between the chunk phase, the interface
     // phase and the scalar recurrence), applies the last step and the clamp, and writes the control block back
     {
@@ -987,6 +975,34 @@ static pff_status damage_solve_t(pff_mesh* m, const pff_state* s, double rel_tol
         return PFF_ENOCONV;
     }
     return PFF_OK;
+}
+
+// Buffers and options of the setup pass of the NEXT forward solve of this mesh (tolerance and cap in m->su_tol /
+// m->su_max_iter), for the explicit-step kernel that performs it (pff_step.cu MODE_STEPSU).
+pff_status damage_fused_setup(pff_mesh* m, FusedSetup* fs)
+{
+    pff_status st = ensure_workspace(m);
+    if (st != PFF_OK) return st;
+    bool cg2 = false;
+    if ((st = solve_uses_cg2<double>(m, m->mat.model == PFF_AT1, &cg2)) != PFF_OK) return st;
+    if (!m->d_su_part) {
+        const size_t nb = size_t(3) * std::max<int64_t>(m->n_slots, 1) * m->rb;
+        if ((st = cuda_check(cudaMalloc(&m->d_su_part, nb), "fused setup: partial planes")) != PFF_OK) return st;
+        if ((st = cuda_check(cudaMemsetAsync(m->d_su_part, 0, nb, m->stream), "fused setup: partial planes")) != PFF_OK) return st;  // unused slots stay zero
+    }
+    fs->ca = m->d_ca; fs->cb = m->d_cb; fs->r = m->d_r; fs->dinv = m->d_dinv; fs->lb = m->d_lb; fs->mask = m->d_mask;
+    fs->part3 = m->d_su_part; fs->part = m->d_part; fs->part_n = m->n_part_blocks; fs->ticket = m->d_ticket; fs->ctrl = m->d_ctrl;
+    fs->tol = m->su_tol; fs->max_iter = m->su_max_iter; fs->zero_dinv_fixed = cg2 ? 1 : 0;
+    m->su_zero_dinv = fs->zero_dinv_fixed;
+    m->su_ready = true;
+    return PFF_OK;
+}
+
+// fp64 gather meshes with the Jacobi solver; off with pff_set_fused_setup(mesh, 0)
+bool fused_setup_ok(const pff_mesh* m)
+{
+    return m->fuse_setup != 0 && m->opt.precision == PFF_F64 && m->opt.scatter == PFF_SCATTER_GATHER && !(m->damage_solver == 1 && m->mg) &&
+           2 * (m->lay_stepsu.total + kSmemCtaReserve) <= kSmemPerSM;
 }
 
 pff_status damage_solve(pff_mesh* m, pff_state* s, double rel_tol, int max_iter, int* iters, double* relres)

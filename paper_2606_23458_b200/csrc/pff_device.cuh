@@ -187,6 +187,35 @@ template <> struct Geo<float> {
     }
 };
 
+// element operator q^e = (c_e M^e + kappa K^e) p^e with M^e = A (1 + delta_ij) / 12 (L185), from the geometry
+template <typename R>
+__device__ __forceinline__ void elem_damage_apply(const MatC<R>& mat, R b1, R c1, R b2, R c2, R A, R He, R p1, R p2, R p3,
+                                                  R& q1, R& q2, R& q3)
+{
+    const R ce = mat.c0 + R(2) * He;  // reaction coefficient (Eq. 6 / Eq. 8)
+    const R m12 = ce * A * R(1.0 / 12.0), sum = p1 + p2 + p3;
+    const R gx = b1 * (p1 - p3) + b2 * (p2 - p3), gy = c1 * (p1 - p3) + c2 * (p2 - p3);
+    const R kA = mat.kappa * A;
+    const R k1 = kA * (b1 * gx + c1 * gy), k2 = kA * (b2 * gx + c2 * gy);
+    q1 = m12 * (p1 + sum) + k1;
+    q2 = m12 * (p2 + sum) + k2;
+    q3 = m12 * (p3 + sum) - (k1 + k2);
+}
+
+// The same operator from its 4 coefficients (what the CG iterations stream instead of geometry + area + H):
+// m = c_e A / 12 and the edge weights w_ij = -kappa A grad phi_i . grad phi_j of the P1 stiffness (rows sum to zero,
+// so K^e p = sum_j w_ij (p_i - p_j)).
+template <typename R>
+__device__ __forceinline__ void elem_coefficients(const MatC<R>& mat, R b1, R c1, R b2, R c2, R A, R He, R& m, R& w12, R& w13,
+                                                  R& w23)
+{
+    const R kA = mat.kappa * A;
+    m = (mat.c0 + R(2) * He) * A * R(1.0 / 12.0);
+    w12 = -kA * (b1 * b2 + c1 * c2);
+    w13 = kA * (b1 * (b1 + b2) + c1 * (c1 + c2));
+    w23 = kA * (b2 * (b1 + b2) + c2 * (c1 + c2));
+}
+
 // Ordered sum of one interface node's per-chunk partials: kIfaceWidth fixed slots (unused ones hold zero) and,
 // on irregular meshes only, its overflow slots.  No index has to be loaded first on regular meshes.
 template <typename R>

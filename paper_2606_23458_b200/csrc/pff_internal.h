@@ -27,6 +27,7 @@ struct ChunkMeta {
 //                           staged geometry and corner 3 follows contiguously (pair index); fp32: separate pair slots
 //   kind 1: damage iteration  x r p q 1/D lb + mask; scalar slots [3 EC + 1]  (one-rendezvous kernel: r p s w 1/D + halo partials)
 //   kind 2: damage setup      x; scalar slots q, D, b each [3 EC + 1]
+//   kind 5: kind 0 + the hold region of the fused damage setup (pff_step.cu MODE_STEPSU)
 //   kind 3: quasi-static CG iteration (explicit-step kernel, MODE_EQ): 13 nodal arrays u_x u_y d p_x p_y r_x r_y q_x q_y
 //                           1/D_x 1/D_y du_x du_y, no history array; force-pair slots as kind 0
 constexpr int kIfaceWidth = 4;  // fixed partial slots per interface node (one per touching chunk)
@@ -41,6 +42,7 @@ struct StageLayout {
     uint32_t slot_stride;  // kind 2: bytes between the q, D, b slot arrays
     uint32_t meta;         // persistent kernels: ring of ChunkMeta of the chunks this CTA owns
     uint32_t hid0;         // persistent kernels: halo ids of the CTA's FIRST chunk (re-gathered every CG iteration)
+    uint32_t hold;         // kind 5: (q, D) pairs of element corners 1 and 2 of the fused damage setup [2 EC] (one copy)
     uint32_t bar;          // one mbarrier per stage
     uint32_t total;
 };
@@ -55,6 +57,8 @@ inline StageLayout make_stage_layout(int kind, int EC, int node_len, int flag_le
     L.geo = o; o += up16(size_t(4) * rb * EC);
     L.area = o; o += up16(kind == 1 ? 0 : rb * EC);  // kind 1 stages the 4 element-operator coefficients as "geometry"
     L.H = o; o += up16(kind == 1 || kind == 3 ? 0 : rb * EC);
+    const bool fused = kind == 5;  // kind 5 = kind 0 + the hold region (explicit step with the damage setup fused in, fp64)
+    if (fused) kind = 0;
     const int nn = kind == 0 ? 10 : (kind == 1 ? 6 : (kind == 3 ? 13 : 1));
     for (int k = 0; k < nn; ++k) {
         // kind 1, array 5: the lower bounds of the projected solver, or (one-rendezvous CG kernel) the kIfaceWidth partial
@@ -77,6 +81,7 @@ inline StageLayout make_stage_layout(int kind, int EC, int node_len, int flag_le
     }
     if (kind == 1) { L.slot_base = o; o += up16(rb * (size_t(3) * EC + 1)); }
     if (kind == 2) { L.slot_base = o; L.slot_stride = up16(rb * (size_t(3) * EC + 1)); o += 3 * L.slot_stride; }
+    L.hold = o; o += up16(fused ? size_t(2) * rb * 2 * EC : 0);
     L.meta = o; o += n_stages > 1 ? uint32_t(32 * kMetaCap) : 0;
     L.hid0 = o; o += up16(n_stages > 1 ? size_t(4) * max_nhalo : 0);
     L.bar = o; o += 16 * uint32_t(n_stages);

@@ -23,6 +23,21 @@ struct RunTally {
 };
 static_assert(sizeof(DamageCtrl) % 8 == 0, "the control block is copied in 8-byte words");
 
+// Outputs of the damage setup pass when the explicit-step kernel performs it as well (pff_step.cu MODE_STEPSU); filled in
+// by damage_fused_setup (pff_damage.cu) with exactly the buffers and options the next damage_solve will use.
+struct FusedSetup {
+    void *ca, *cb;            // operator coefficients of the solve
+    void *r, *dinv, *lb;      // first residual, Jacobi diagonal (inverse), lower bound d_n
+    uint8_t* mask;
+    void* part3;              // [3][n_slots] reals: per (chunk, interface node) partials of A d_n, D, b
+    double* part;             // [kCh][part_n] block partials of the norms
+    int64_t part_n;
+    unsigned int* ticket;     // the damage workspace's tickets ([0] last block, [1] CG barrier counter)
+    DamageCtrl* ctrl;
+    double tol;
+    int max_iter, zero_dinv_fixed;
+};
+
 struct pff_mesh {
     pff::HostMesh hm;
     pff_material mat{};
@@ -31,12 +46,20 @@ struct pff_mesh {
     int device = 0;
     size_t rb = 8;  // bytes per real
     double dt_crit = 0.0;
-    pff::StageLayout lay_step{}, lay_mv{}, lay_su{}, lay_eq{};  // shared-memory stages of the step / CG iteration / setup / quasi-static CG kernels
+    pff::StageLayout lay_step{}, lay_stepsu{}, lay_mv{}, lay_su{}, lay_eq{};  // shared-memory stages of the step / CG iteration / setup / quasi-static CG kernels
     int64_t ell_total = 0;                       // entries of d_ell (padded)
     int64_t n_launches = 0;  // kernels launched so far (pff_mesh_counters)
     long long* d_trace = nullptr;  // pff_trace_set (instrumentation build)
     int trace_iter = 3;
     void* mg = nullptr;      // multigrid hierarchy attached to this (finest) mesh: pff_multigrid.cu
+    // fused explicit step + damage setup (pff_run_steps): option, the partial planes of the fused setup, and what the last
+    // fused launch prepared (consumed by the next damage_solve, which then skips its own setup kernel)
+    int fuse_setup = 1;
+    void* d_su_part = nullptr;
+    bool su_ready = false;
+    double su_tol = 0.0;
+    int su_max_iter = 0, su_zero_dinv = 0;
+    int last_step_fused = 0;
     int damage_solver = 0;   // pff_set_damage_solver: 0 Jacobi-PCG kernels, 1 multigrid-preconditioned CG (AT2, hierarchy attached)
     int only_kernel = -1;    // profiling hook: restrict multi-kernel entry points to one kernel (pff_time_kernel)
     // launch configuration of every persistent chunk kernel this mesh has used, keyed by the kernel's address: the grid
@@ -137,6 +160,8 @@ pff_status launch_step(pff_mesh* m, pff_state* s, const pff_bc* bc, double dt, i
 pff_status damage_solve(pff_mesh* m, pff_state* s, double rel_tol, int max_iter, int* iters, double* relres);
 pff_status damage_matvec(pff_mesh* m, const pff_state* s, const void* p, void* q, bool refresh_coef = true, bool skip_interface = false);
 pff_status damage_refresh_coef(pff_mesh* m, const pff_state* s);
+pff_status damage_fused_setup(pff_mesh* m, FusedSetup* fs);  // tolerance / iteration cap: m->su_tol, m->su_max_iter
+bool fused_setup_ok(const pff_mesh* m);
 // pff_multigrid.cu: geometric-multigrid-preconditioned CG for the AT2 damage solve
 pff_status mg_attach(pff_mesh* m, int n_coarse, pff_mesh* const* coarse);
 pff_status mg_apply(pff_mesh* m, const pff_state* s, const void* r, void* z);

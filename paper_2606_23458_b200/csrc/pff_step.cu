@@ -25,7 +25,13 @@ namespace pff {
 // MODE_EQ: one WHOLE iteration of the quasi-static mechanics CG (pff_equilibrium.cu) in one pass: the node prologue applies
 // the previous step (du += alpha p, r -= alpha q) and forms p = D^-1 r + beta p, the element pass is MODE_TANGENT's, the
 // gather leaves q = K p and the sums that give alpha and PREDICT beta; the last CTA advances the scalars.
-enum { MODE_STEP = 0, MODE_INIT = 1, MODE_FORCE = 2, MODE_TANGENT = 3, MODE_EQ = 4 };
+// MODE_STEPSU: the explicit step with the SETUP PASS of the damage solve that follows it fused in (pff_run_steps, fp64): the
+// step kernel already has everything that pass reads in shared memory -- connectivity, geometry, area, the new history
+// value, d -- so the element pass also forms the damage operator's coefficients (streamed to HBM for the CG iterations),
+// its action on d_n, its diagonal and the right-hand side, and the one gather walk sums them next to the forces: the
+// setup kernel's 120 MB of re-reads, its pipeline fill and its grid-wide tail disappear.  Same arithmetic in the same
+// order as dmg_setup_chunk (pff_damage.cu): bit-identical r0, 1/D, coefficients, norms.
+enum { MODE_STEP = 0, MODE_INIT = 1, MODE_FORCE = 2, MODE_TANGENT = 3, MODE_EQ = 4, MODE_STEPSU = 5 };
 
 template <typename R>
 struct StepArgs {
@@ -60,6 +66,7 @@ struct StepArgs {
     double* eq_part;   // [kCh][gridDim.x]
     unsigned int* eq_ticket;
     R *fwx, *fwy;
+    FusedSetup su;  // MODE_STEPSU: outputs of the fused damage setup (pff_mesh.h)
     R dt, hdt, hdt2, S;
     MatC<R> mat;
     long long* trace;  // phase timestamps (PFF_TRACE builds)
@@ -209,7 +216,10 @@ __global__ void __launch_bounds__(kStepTPB, 2) step_chunk_kernel(const StepArgs<
         *Geo<R>::slot(smem, s_shared_slots, 3 * EC, EC) = Geo<R>::pair(R(0), R(0));  // the zero pair (lives in the shared region)
     }
     int it = 0;  // stage uses so far: stage = it & 1, mbarrier parity = (it >> 1) & 1
-    const bool tr_on = MODE == MODE_STEP;
+    constexpr bool SU = MODE == MODE_STEPSU;
+    constexpr bool STEP = MODE == MODE_STEP || SU;  // the explicit step proper
+    constexpr int HALO_MODE = SU ? (int)MODE_STEP : MODE;
+    [[maybe_unused]] const bool tr_on = STEP;
     int tr_k = 0;
     PFF_TR(a.trace, tr_on, 0);
     unsigned int gb_epoch = 0;  // thread 0: the barrier counter's value before this launch (read early, used at the barrier)
@@ -217,7 +227,7 @@ __global__ void __launch_bounds__(kStepTPB, 2) step_chunk_kernel(const StepArgs<
     // MODE_EQ: the recurrence scalars of this iteration (written by the previous launch, or by the host for the first one)
     // and this thread's share of the seven sums p.q, r.z, r.r, z.q, q.Dinv.q, r.q, q.q (channels of cg scalar step)
     __shared__ DamageCtrl s_eq;
-    __shared__ double s_w[MODE == MODE_EQ ? kCh * kRedWarps : 1], s_out[kCh];
+    __shared__ double s_w[(MODE == MODE_EQ || SU) ? kCh * kRedWarps : 1], s_out[kCh];
     double acc[kCh];
     R eq_alpha = R(0), eq_beta = R(0);
     bool eq_first = true;
@@ -228,6 +238,12 @@ __global__ void __launch_bounds__(kStepTPB, 2) step_chunk_kernel(const StepArgs<
         eq_alpha = R(s_eq.alpha); eq_beta = R(s_eq.beta); eq_first = s_eq.first != 0;
 #pragma unroll
         for (int c = 0; c < kCh; ++c) acc[c] = 0.0;
+    }
+    if (SU) {
+#pragma unroll
+        for (int c = 0; c < kCh; ++c) acc[c] = 0.0;
+        // the CG kernel that follows in stream order counts its grid barriers from zero (as dmg_setup_chunk does)
+        if (blockIdx.x == 0 && tid == 0) a.su.ticket[1] = 0u;
     }
     for (int e0 = 0; e0 < n_my; e0 += kMetaCap) {
         const int n_ep = min(kMetaCap, n_my - e0);
@@ -247,7 +263,7 @@ __global__ void __launch_bounds__(kStepTPB, 2) step_chunk_kernel(const StepArgs<
             if (issuer) {
                 const int hb0 = ((cm.node_start & (A - 1)) + cm.n_int + A - 1) & ~(A - 1);
                 for (int j = lane; j < cm.n_halo; j += 32)
-                    step_halo_gather<R, MODE>(a, L, stg, hb0 + j, j, __ldg(a.halo_ids + cm.halo_off + j));
+                    step_halo_gather<R, HALO_MODE>(a, L, stg, hb0 + j, j, __ldg(a.halo_ids + cm.halo_off + j));
             }
             cp_async_mbar_arrive(bar + 2 * (it & 1));
         }
@@ -307,13 +323,13 @@ __global__ void __launch_bounds__(kStepTPB, 2) step_chunk_kernel(const StepArgs<
                 if (issuer) {
                     const int hbn = ((cn.node_start & (A - 1)) + cn.n_int + A - 1) & ~(A - 1);
                     const int* ids = reinterpret_cast<const int*>(stg + L.hnext) + (cn.halo_off & 3);
-                    for (int j = lane; j < cn.n_halo; j += 32) step_halo_gather<R, MODE>(a, L, stn, hbn + j, j, ids[j]);
+                    for (int j = lane; j < cn.n_halo; j += 32) step_halo_gather<R, HALO_MODE>(a, L, stn, hbn + j, j, ids[j]);
                 }
                 cp_async_mbar_arrive(bar + 2 * (st ^ 1));
             }
             // ---- phase 1: predictor (Eq. 16) in place, halo nodes by the middle warps, interior by the low warps;
             // Dirichlet dofs hold u_bar already (dirichlet_kernel)
-            if (MODE == MODE_STEP && !issuer) {
+            if (STEP && !issuer) {
                 for (int j = (tid + kWorkers / 2) % kWorkers; j < cm.n_halo; j += kWorkers) {
                     const int s = hb + j, gid = reinterpret_cast<const int*>(stg + L.hids)[j];
                     const unsigned fl = reinterpret_cast<const unsigned*>(stg + L.hflag)[j] >> (8 * (gid & 3));
@@ -384,8 +400,27 @@ __global__ void __launch_bounds__(kStepTPB, 2) step_chunk_kernel(const StepArgs<
                 *Geo<R>::slot(s_geo, s_shared_slots, e, EC) = Geo<R>::pair(f[0], f[1]);
                 *Geo<R>::slot(s_geo, s_shared_slots, EC + e, EC) = Geo<R>::pair(f[2], f[3]);
                 *Geo<R>::slot(s_geo, s_shared_slots, 2 * EC + e, EC) = Geo<R>::pair(f[4], f[5]);
-                if (MODE == MODE_STEP) {
-                    if (psi_p > s_H[e]) a.H[cm.elem_start + e] = psi_p;  // H <- max(H, psi+)  (L98, L114)
+                if (STEP) {
+                    const R Hold = s_H[e];
+                    if (psi_p > Hold) a.H[cm.elem_start + e] = psi_p;  // H <- max(H, psi+)  (L98, L114)
+                    if (SU) {  // damage setup for this element with the NEW history value (dmg_setup_chunk's element pass)
+                        const R He = psi_p > Hold ? psi_p : Hold, Ar = s_area[e];
+                        R q1, q2, q3, cm_, w12, w13, w23;
+                        elem_damage_apply<R>(a.mat, b1, c1, b2, c2, Ar, He, s_d[c.x], s_d[c.y], s_d[c.z], q1, q2, q3);
+                        elem_coefficients<R>(a.mat, b1, c1, b2, c2, Ar, He, cm_, w12, w13, w23);
+                        Geo<R>::store_global(a.su.ca, a.su.cb, cm.elem_start + e, cm_, w12, w13, w23);
+                        const R ce = a.mat.c0 + R(2) * He, se = R(2) * He - a.mat.s0;
+                        const R m12 = ce * Ar * R(1.0 / 12.0), kA = a.mat.kappa * Ar;
+                        const R b3 = -(b1 + b2), c3 = -(c1 + c2);
+                        // (q, D) of corners 1, 2 go to the hold region; corner 3's and the element's share of the right-hand
+                        // side replace what only this thread needed from the stage: H, the connectivity word, the area
+                        Pair* hold = reinterpret_cast<Pair*>(smem + L.hold);
+                        hold[e] = Geo<R>::pair(q1, R(2) * m12 + kA * (b1 * b1 + c1 * c1));
+                        hold[EC + e] = Geo<R>::pair(q2, R(2) * m12 + kA * (b2 * b2 + c2 * c2));
+                        const_cast<R*>(s_H)[e] = q3;
+                        reinterpret_cast<R*>(stg + L.lconn)[e] = R(2) * m12 + kA * (b3 * b3 + c3 * c3);
+                        const_cast<R*>(s_area)[e] = se * Ar * R(1.0 / 3.0);
+                    }
                 } else if (MODE == MODE_FORCE) {
                     if (a.psi_out) a.psi_out[cm.elem_start + e] = psi_p;
                 }
@@ -396,11 +431,20 @@ __global__ void __launch_bounds__(kStepTPB, 2) step_chunk_kernel(const StepArgs<
             // ---- phase 3: ordered gather of each node's incident force pairs, then Eq. 17-18 for interior nodes
             for (int i = tid; i < nloc; i += kStepTPB) {
                 R fx = R(0), fy = R(0);
+                [[maybe_unused]] R qs = R(0), Ds = R(0), bs = R(0);  // MODE_STEPSU: A d_n, diagonal, right-hand side of this node
                 const uint16_t* row = s_ell + i;
 #pragma unroll 4
                 for (int w = 0; w < cm.ell_w; ++w) {
-                    const Pair v = *Geo<R>::slot(s_geo, s_shared_slots, row[w * nloc], EC);
+                    const int idx = row[w * nloc];
+                    const Pair v = *Geo<R>::slot(s_geo, s_shared_slots, idx, EC);
                     fx += v.x; fy += v.y;
+                    if (SU && idx < 3 * EC) {  // same order of sums as dmg_setup_chunk (padding entries add nothing there either)
+                        const int kc = (idx >= EC) + (idx >= 2 * EC), e = idx - kc * EC;
+                        Pair h;
+                        if (kc < 2) h = reinterpret_cast<const Pair*>(smem + L.hold)[idx];
+                        else h = Geo<R>::pair(s_H[e], reinterpret_cast<const R*>(stg + L.lconn)[e]);
+                        qs += h.x; Ds += h.y; bs += s_area[e];
+                    }
                 }
                 if (i < cm.n_int) {
                     const int gid = cm.node_start + i, s = shift + i;
@@ -419,17 +463,32 @@ __global__ void __launch_bounds__(kStepTPB, 2) step_chunk_kernel(const StepArgs<
                     R ayn = (a.S * s_fey[s] - fy) * minv;
                     if (fl & 1) axn = R(0);
                     if (fl & 2) ayn = R(0);
-                    if (MODE == MODE_STEP) {
+                    if (STEP) {
                         const R vxo = s_vx[s], vyo = s_vy[s];
                         a.ux[gid] = s_ux[s]; a.uy[gid] = s_uy[s];
                         a.vx[gid] = (fl & 1) ? vxo : rfma(a.hdt, s_ax[s] + axn, vxo);
                         a.vy[gid] = (fl & 2) ? vyo : rfma(a.hdt, s_ay[s] + ayn, vyo);
                     }
                     a.ax[gid] = axn; a.ay[gid] = ayn;
+                    if (SU) {  // dmg_setup_chunk's node epilogue
+                        const bool fixed = (fl & 4) != 0;
+                        const R r = bs - qs;
+                        reinterpret_cast<R*>(a.su.r)[gid] = r;
+                        reinterpret_cast<R*>(a.su.dinv)[gid] = (a.su.zero_dinv_fixed && fixed) ? R(0) : R(1) / Ds;
+                        reinterpret_cast<R*>(a.su.lb)[gid] = s_d[s];
+                        a.su.mask[gid] = fixed ? 2 : 1;
+                        acc[0] += double(bs) * double(bs);
+                        if (!fixed) acc[1] += double(r) * double(r);
+                        if (!fixed && (a.mat.model != PFF_AT1 || r > R(0))) acc[2] += double(r) * double(r);
+                    }
                 } else {
                     const int slot = s_hdst[i - cm.n_int];
                     a.halo_part[slot] = fx;
                     a.halo_part[a.n_slots + slot] = fy;
+                    if (SU) {
+                        R* sp = reinterpret_cast<R*>(a.su.part3);
+                        sp[slot] = qs; sp[a.n_slots + slot] = Ds; sp[2 * a.n_slots + slot] = bs;
+                    }
                 }
             }
             __syncthreads();  // stage st and the slots are free again
@@ -448,7 +507,7 @@ __global__ void __launch_bounds__(kStepTPB, 2) step_chunk_kernel(const StepArgs<
         if (blockIdx.x == 0 && tid == 0) a.gbar[1] = target;
         // Equal slice per CTA, TWO nodes per thread and trip: all loads of both nodes are issued before anything is computed
         // or stored, so a trip costs one memory round trip (the slice is ~1.7 nodes per thread at 10^6 nodes).
-        struct IfNode { R fx, fy, ux, uy, vx, vy, ax, ay, fex, fey, minv, px, py, rx, ry, qx, qy, dx, dy, ex, ey; uint8_t fl; };
+        struct IfNode { R fx, fy, ux, uy, vx, vy, ax, ay, fex, fey, minv, px, py, rx, ry, qx, qy, dx, dy, ex, ey, sq, sD, sb, sd; uint8_t fl; };
         auto if_load = [&](int s, IfNode& v) {
             const int gid = a.N_int + s;
             v.fx = iface_sum<R>(a.halo_part, s, a.N_sh, a.n_ovf, a.sh_rowptr);
@@ -460,8 +519,15 @@ __global__ void __launch_bounds__(kStepTPB, 2) step_chunk_kernel(const StepArgs<
                 return;
             }
             v.ux = a.ux[gid]; v.uy = a.uy[gid];
-            if (MODE == MODE_STEP) { v.vx = a.vx[gid]; v.vy = a.vy[gid]; v.ax = a.ax[gid]; v.ay = a.ay[gid]; }
-            if (MODE == MODE_STEP || MODE == MODE_INIT) { v.fl = a.flags[gid]; v.minv = a.minv[gid]; v.fex = a.fex[gid]; v.fey = a.fey[gid]; }
+            if (STEP) { v.vx = a.vx[gid]; v.vy = a.vy[gid]; v.ax = a.ax[gid]; v.ay = a.ay[gid]; }
+            if (STEP || MODE == MODE_INIT) { v.fl = a.flags[gid]; v.minv = a.minv[gid]; v.fex = a.fex[gid]; v.fey = a.fey[gid]; }
+            if (SU) {  // the three partial planes of the fused damage setup and d_n
+                const R* sp = reinterpret_cast<const R*>(a.su.part3);
+                v.sq = iface_sum<R>(sp, s, a.N_sh, a.n_ovf, a.sh_rowptr);
+                v.sD = iface_sum<R>(sp + a.n_slots, s, a.N_sh, a.n_ovf, a.sh_rowptr);
+                v.sb = iface_sum<R>(sp + 2 * a.n_slots, s, a.N_sh, a.n_ovf, a.sh_rowptr);
+                v.sd = a.d[gid];
+            }
             if (MODE == MODE_TANGENT) { v.px = a.px[gid]; v.py = a.py[gid]; }
         };
         auto if_finish = [&](int s, const IfNode& v) {  // the same Eq. 16-18 as predict() + finish_node(), from the loaded values
@@ -492,7 +558,7 @@ __global__ void __launch_bounds__(kStepTPB, 2) step_chunk_kernel(const StepArgs<
             R ayn = (a.S * v.fey - v.fy) * v.minv;
             if (v.fl & 1) axn = R(0);
             if (v.fl & 2) ayn = R(0);
-            if (MODE == MODE_STEP) {
+            if (STEP) {
                 const R px = rfma(a.hdt2, v.ax, rfma(a.dt, v.vx, v.ux));
                 const R py = rfma(a.hdt2, v.ay, rfma(a.dt, v.vy, v.uy));
                 a.ux[gid] = (v.fl & 1) ? v.ux : px; a.uy[gid] = (v.fl & 2) ? v.uy : py;
@@ -500,6 +566,17 @@ __global__ void __launch_bounds__(kStepTPB, 2) step_chunk_kernel(const StepArgs<
                 a.vy[gid] = (v.fl & 2) ? v.vy : rfma(a.hdt, v.ay + ayn, v.vy);
             }
             a.ax[gid] = axn; a.ay[gid] = ayn;
+            if (SU) {  // dmg_setup_chunk's interface epilogue
+                const bool fixed = (v.fl & 4) != 0;
+                const R r = v.sb - v.sq;
+                reinterpret_cast<R*>(a.su.r)[gid] = r;
+                reinterpret_cast<R*>(a.su.dinv)[gid] = (a.su.zero_dinv_fixed && fixed) ? R(0) : R(1) / v.sD;
+                reinterpret_cast<R*>(a.su.lb)[gid] = v.sd;
+                a.su.mask[gid] = fixed ? 2 : 1;
+                acc[0] += double(v.sb) * double(v.sb);
+                if (!fixed) acc[1] += double(r) * double(r);
+                if (!fixed && (a.mat.model != PFF_AT1 || r > R(0))) acc[2] += double(r) * double(r);
+            }
         };
         const int per = (a.N_sh + G - 1) / G, end = min(a.N_sh, ((int)blockIdx.x + 1) * per);
         for (int s0 = blockIdx.x * per + tid; s0 < end; s0 += 2 * kStepTPB) {
@@ -513,6 +590,30 @@ __global__ void __launch_bounds__(kStepTPB, 2) step_chunk_kernel(const StepArgs<
         }
     }
     PFF_TR(a.trace, tr_on, 102);
+    if (SU) {
+        // ---- norms of the fused damage setup and the control block of the solve (dmg_setup_chunk's tail): one block
+        // reduction per CTA, the last CTA to arrive sums the block partials in a fixed order
+        __syncthreads();
+        block_reduce_ch(acc, s_w, s_out);
+        if (tid < kCh) a.su.part[(int64_t)tid * a.su.part_n + blockIdx.x] = s_out[tid];
+        if (last_block(a.su.ticket)) {
+            const int w = tid >> 5;
+            if (w < 3) {
+                double v = 0.0;
+                for (int i = lane; i < G; i += 32) v += __ldcg(a.su.part + (int64_t)w * a.su.part_n + i);
+                for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+                if (lane == 0) s_out[w] = v;
+            }
+            __syncthreads();
+            if (tid == 0) {
+                DamageCtrl c{};
+                c.tol = a.su.tol; c.max_iter = a.su.max_iter; c.first = 1; c.restart = 1; c.status = PFF_ENOCONV;
+                c.nb = fmax(fmax(sqrt(s_out[0]), sqrt(s_out[1])), 1e-300);
+                if (sqrt(s_out[2]) <= c.tol * c.nb) { c.done = 1; c.status = PFF_OK; c.relres = sqrt(s_out[2]) / c.nb; }
+                *a.su.ctrl = c;
+            }
+        }
+    }
     if (MODE == MODE_EQ) {
         // ---- one ordered block reduction per CTA; the LAST CTA to finish sums the block partials in index order and
         // advances the recurrence scalars for the next launch (alpha, predicted beta, convergence: eq_scalar_step)
@@ -622,7 +723,7 @@ static pff_status launch_step_t(pff_mesh* m, const StepArgs<R>& a)
     } else {
         auto kern = step_chunk_kernel<R, SPLIT, MODE>;
         int grid = 0;  // persistent grid: every SM filled with as many CTAs as fit (cached per mesh, with the smem opt-in)
-        const size_t smem = MODE == MODE_EQ ? m->lay_eq.total : m->lay_step.total;
+        const size_t smem = MODE == MODE_EQ ? m->lay_eq.total : (MODE == MODE_STEPSU ? m->lay_stepsu.total : m->lay_step.total);
         if (smem + 4096 > kSmemPerSM) { set_error("quasi-static CG: the chunk does not fit shared memory (use a smaller chunk_elems)"); return PFF_EUNSUPPORTED; }
         pff_status st = persistent_config(m, (const void*)kern, (int)smem, &grid, kStepTPB);
         if (st != PFF_OK) return st;
@@ -678,12 +779,16 @@ static pff_status launch_step_r(pff_mesh* m, pff_state* s, const pff_bc* bc, dou
         a.eq_ctrl = m->d_eq_ctrl; a.eq_part = m->d_eq_part; a.eq_ticket = m->d_eq_ticket;
     }
     a.fwx = (R*)m->d_fwx; a.fwy = (R*)m->d_fwy;
+    if (mode == MODE_STEPSU) {  // outputs of the damage setup this launch performs as well (pff_damage.cu fills them in)
+        pff_status fst = damage_fused_setup(m, &a.su);
+        if (fst != PFF_OK) return fst;
+    }
     a.dt = R(dt); a.hdt = R(0.5 * dt); a.hdt2 = R(0.5 * dt * dt);
     a.S = R(bc ? bc->load_scale : 1.0);
     a.mat = make_matc<R>(m->mat);
     a.trace = m->d_trace ? m->d_trace + kTraceStepOffset : nullptr;
     {   // TMA plan: one descriptor per contiguous array the chosen mode reads (kind 0 elements, 1 nodes, 2 gather table)
-        const StageLayout& L = mode == MODE_EQ ? m->lay_eq : m->lay_step;
+        const StageLayout& L = mode == MODE_EQ ? m->lay_eq : (mode == MODE_STEPSU ? m->lay_stepsu : m->lay_step);
         a.lay = L;
         StagePlan& P = a.plan;
         P.n = 0;
@@ -693,12 +798,13 @@ static pff_status launch_step_r(pff_mesh* m, pff_state* s, const pff_bc* bc, dou
         if (sizeof(R) == 8) { add(m->d_ga, L.geo, 4, 0); add(m->d_gb, L.geo + 16u * (uint32_t)hm.chunk_elems, 4, 0); }
         else add(m->d_ga, L.geo, 4, 0);
         add(m->d_area, L.area, lr, 0);
-        if (mode == MODE_STEP) add(s->H, L.H, lr, 0);
+        const bool step_like = mode == MODE_STEP || mode == MODE_STEPSU;
+        if (step_like) add(s->H, L.H, lr, 0);
         add(m->d_ell, L.ell, 1, 2);
         add(m->d_halo_dst, L.hdst, 2, 3);   // partial slots of the chunk's halo nodes
         add(m->d_halo_ids, L.hnext, 2, 4);  // ids of the next chunk's halo nodes
         add(s->ux, L.node[0], lr, 1); add(s->uy, L.node[1], lr, 1); add(s->d, L.node[2], lr, 1);
-        if (mode == MODE_STEP) {
+        if (step_like) {
             add(s->vx, L.node[3], lr, 1); add(s->vy, L.node[4], lr, 1);
             add(s->ax, L.node[5], lr, 1); add(s->ay, L.node[6], lr, 1);
         }
@@ -713,7 +819,7 @@ static pff_status launch_step_r(pff_mesh* m, pff_state* s, const pff_bc* bc, dou
             add(m->d_flags, L.flags, 0, 1);
         }
     }
-    if (mode == MODE_STEP && m->n_dir > 0 && bc && bc->dir_u && bc->dir_v) {
+    if ((mode == MODE_STEP || mode == MODE_STEPSU) && m->n_dir > 0 && bc && bc->dir_u && bc->dir_v) {
         PFF_LAUNCH(m, PFF_K_OTHER, (dirichlet_kernel<R><<<(unsigned)((m->n_dir + 127) / 128), 128, 0, m->stream>>>(
             (int)m->n_dir, m->d_dir_dof, (const R*)bc->dir_u, (const R*)bc->dir_v, a.ux, a.uy, a.vx, a.vy)));
     }
@@ -727,6 +833,12 @@ static pff_status launch_step_r(pff_mesh* m, pff_state* s, const pff_bc* bc, dou
         case MODE_EQ:
             if (m->opt.scatter == PFF_SCATTER_ATOMIC) { set_error("quasi-static CG: gather scatter only"); return PFF_EUNSUPPORTED; }
             return launch_step_s<R, MODE_EQ>(m, a);
+        case MODE_STEPSU:
+            if constexpr (sizeof(R) == 8) {
+                if (m->opt.scatter != PFF_SCATTER_ATOMIC) return launch_step_s<R, MODE_STEPSU>(m, a);
+            }
+            set_error("fused step + damage setup: fp64 gather meshes only");
+            return PFF_EUNSUPPORTED;
     }
     return PFF_EINVAL;
 }
