@@ -255,7 +255,7 @@ pff_status pff_last_cg_kernel(const pff_mesh *mesh, int32_t *kernel);
  * Jacobi diagonal, first residual, operator coefficients, norms, control block) in the same kernel: everything the pass
  * reads -- connectivity, geometry, area, the new history value, d -- is already in the step kernel's shared memory, so
  * the separate setup kernel with its 120 MB of re-reads disappears (two kernels per staggered step instead of three).
- * Same arithmetic in the same order: results are bit-identical to the three-kernel sequence.  Used where it applies: fp64,
+ * Same arithmetic in the same order: results are bit-identical to the three-kernel sequence.  Used where it applies:
  * gather scatter, Jacobi solver; enable = 0 switches it off (A/B timing).  pff_explicit_step + pff_damage_solve (one call
  * each) always run the separate kernels.  used <- whether the last pff_run_steps fused.  Host-only. */
 pff_status pff_set_fused_setup(pff_mesh *mesh, int32_t enable);

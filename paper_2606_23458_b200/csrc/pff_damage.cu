@@ -984,7 +984,9 @@ pff_status damage_fused_setup(pff_mesh* m, FusedSetup* fs)
     pff_status st = ensure_workspace(m);
     if (st != PFF_OK) return st;
     bool cg2 = false;
-    if ((st = solve_uses_cg2<double>(m, m->mat.model == PFF_AT1, &cg2)) != PFF_OK) return st;
+    st = m->opt.precision == PFF_F32 ? solve_uses_cg2<float>(m, m->mat.model == PFF_AT1, &cg2)
+                                     : solve_uses_cg2<double>(m, m->mat.model == PFF_AT1, &cg2);
+    if (st != PFF_OK) return st;
     if (!m->d_su_part) {
         const size_t nb = size_t(3) * std::max<int64_t>(m->n_slots, 1) * m->rb;
         if ((st = cuda_check(cudaMalloc(&m->d_su_part, nb), "fused setup: partial planes")) != PFF_OK) return st;
@@ -998,10 +1000,10 @@ pff_status damage_fused_setup(pff_mesh* m, FusedSetup* fs)
     return PFF_OK;
 }
 
-// fp64 gather meshes with the Jacobi solver; off with pff_set_fused_setup(mesh, 0)
+// gather meshes with the Jacobi solver whose fused stage still leaves two CTAs per SM; off with pff_set_fused_setup(mesh, 0)
 bool fused_setup_ok(const pff_mesh* m)
 {
-    return m->fuse_setup != 0 && m->opt.precision == PFF_F64 && m->opt.scatter == PFF_SCATTER_GATHER && !(m->damage_solver == 1 && m->mg) &&
+    return m->fuse_setup != 0 && m->opt.scatter == PFF_SCATTER_GATHER && !(m->damage_solver == 1 && m->mg) &&
            2 * (m->lay_stepsu.total + kSmemCtaReserve) <= kSmemPerSM;
 }
 

@@ -42,7 +42,7 @@ struct StageLayout {
     uint32_t slot_stride;  // kind 2: bytes between the q, D, b slot arrays
     uint32_t meta;         // persistent kernels: ring of ChunkMeta of the chunks this CTA owns
     uint32_t hid0;         // persistent kernels: halo ids of the CTA's FIRST chunk (re-gathered every CG iteration)
-    uint32_t hold;         // kind 5: (q, D) pairs of element corners 1 and 2 of the fused damage setup [2 EC] (one copy)
+    uint32_t hold;         // kind 5: (q, D) pairs of element corners 1 and 2 (fp32: 1, 2, 3) of the fused damage setup (one copy)
     uint32_t bar;          // one mbarrier per stage
     uint32_t total;
 };
@@ -81,7 +81,7 @@ inline StageLayout make_stage_layout(int kind, int EC, int node_len, int flag_le
     }
     if (kind == 1) { L.slot_base = o; o += up16(rb * (size_t(3) * EC + 1)); }
     if (kind == 2) { L.slot_base = o; L.slot_stride = up16(rb * (size_t(3) * EC + 1)); o += 3 * L.slot_stride; }
-    L.hold = o; o += up16(fused ? size_t(2) * rb * 2 * EC : 0);
+    L.hold = o; o += up16(fused ? size_t(2) * rb * (rb == 8 ? 2 : 3) * EC : 0);  // fp32: all three corners (nothing to reuse there)
     L.meta = o; o += n_stages > 1 ? uint32_t(32 * kMetaCap) : 0;
     L.hid0 = o; o += up16(n_stages > 1 ? size_t(4) * max_nhalo : 0);
     L.bar = o; o += 16 * uint32_t(n_stages);

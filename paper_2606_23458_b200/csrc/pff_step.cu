@@ -25,7 +25,7 @@ namespace pff {
 // MODE_EQ: one WHOLE iteration of the quasi-static mechanics CG (pff_equilibrium.cu) in one pass: the node prologue applies
 // the previous step (du += alpha p, r -= alpha q) and forms p = D^-1 r + beta p, the element pass is MODE_TANGENT's, the
 // gather leaves q = K p and the sums that give alpha and PREDICT beta; the last CTA advances the scalars.
-// MODE_STEPSU: the explicit step with the SETUP PASS of the damage solve that follows it fused in (pff_run_steps, fp64): the
+// MODE_STEPSU: the explicit step with the SETUP PASS of the damage solve that follows it fused in (pff_run_steps): the
 // step kernel already has everything that pass reads in shared memory -- connectivity, geometry, area, the new history
 // value, d -- so the element pass also forms the damage operator's coefficients (streamed to HBM for the CG iterations),
 // its action on d_n, its diagonal and the right-hand side, and the one gather walk sums them next to the forces: the
@@ -417,8 +417,9 @@ __global__ void __launch_bounds__(kStepTPB, 2) step_chunk_kernel(const StepArgs<
                         Pair* hold = reinterpret_cast<Pair*>(smem + L.hold);
                         hold[e] = Geo<R>::pair(q1, R(2) * m12 + kA * (b1 * b1 + c1 * c1));
                         hold[EC + e] = Geo<R>::pair(q2, R(2) * m12 + kA * (b2 * b2 + c2 * c2));
-                        const_cast<R*>(s_H)[e] = q3;
-                        reinterpret_cast<R*>(stg + L.lconn)[e] = R(2) * m12 + kA * (b3 * b3 + c3 * c3);
+                        const R D3 = R(2) * m12 + kA * (b3 * b3 + c3 * c3);
+                        if (sizeof(R) == 8) { const_cast<R*>(s_H)[e] = q3; reinterpret_cast<R*>(stg + L.lconn)[e] = D3; }
+                        else hold[2 * EC + e] = Geo<R>::pair(q3, D3);  // fp32: the hold region has room for all three corners
                         const_cast<R*>(s_area)[e] = se * Ar * R(1.0 / 3.0);
                     }
                 } else if (MODE == MODE_FORCE) {
@@ -441,7 +442,7 @@ __global__ void __launch_bounds__(kStepTPB, 2) step_chunk_kernel(const StepArgs<
                     if (SU && idx < 3 * EC) {  // same order of sums as dmg_setup_chunk (padding entries add nothing there either)
                         const int kc = (idx >= EC) + (idx >= 2 * EC), e = idx - kc * EC;
                         Pair h;
-                        if (kc < 2) h = reinterpret_cast<const Pair*>(smem + L.hold)[idx];
+                        if (kc < 2 || sizeof(R) == 4) h = reinterpret_cast<const Pair*>(smem + L.hold)[idx];
                         else h = Geo<R>::pair(s_H[e], reinterpret_cast<const R*>(stg + L.lconn)[e]);
                         qs += h.x; Ds += h.y; bs += s_area[e];
                     }
@@ -834,11 +835,8 @@ static pff_status launch_step_r(pff_mesh* m, pff_state* s, const pff_bc* bc, dou
             if (m->opt.scatter == PFF_SCATTER_ATOMIC) { set_error("quasi-static CG: gather scatter only"); return PFF_EUNSUPPORTED; }
             return launch_step_s<R, MODE_EQ>(m, a);
         case MODE_STEPSU:
-            if constexpr (sizeof(R) == 8) {
-                if (m->opt.scatter != PFF_SCATTER_ATOMIC) return launch_step_s<R, MODE_STEPSU>(m, a);
-            }
-            set_error("fused step + damage setup: fp64 gather meshes only");
-            return PFF_EUNSUPPORTED;
+            if (m->opt.scatter == PFF_SCATTER_ATOMIC) { set_error("fused step + damage setup: gather meshes only"); return PFF_EUNSUPPORTED; }
+            return launch_step_s<R, MODE_STEPSU>(m, a);
     }
     return PFF_EINVAL;
 }
