@@ -117,6 +117,7 @@ void pff_mesh_destroy(pff_mesh* m)
     if (m->graph_exec) cudaGraphExecDestroy(m->graph_exec);
     if (m->copy_stream) { cudaStreamSynchronize(m->copy_stream); cudaStreamDestroy(m->copy_stream); }
     if (m->ev_step) cudaEventDestroy(m->ev_step);
+    if (m->ev_out) cudaEventDestroy(m->ev_out);
     for (auto& v : m->prof_ev) for (cudaEvent_t e : v) cudaEventDestroy(e);
     delete m;
 }

@@ -98,6 +98,7 @@ static pff_status run_host_t(pff_mesh* m, pff_host_state* hs, const double* dir_
     // back on a second stream while the solve runs on the mesh stream; d follows when the solve is done.
     if (!m->copy_stream && (st = cuda_check(cudaStreamCreateWithFlags(&m->copy_stream, cudaStreamNonBlocking), "run_host: stream")) != PFF_OK) return st;
     if (!m->ev_step && (st = cuda_check(cudaEventCreateWithFlags(&m->ev_step, cudaEventDisableTiming), "run_host: event")) != PFF_OK) return st;
+    if (!m->ev_out && (st = cuda_check(cudaEventCreateWithFlags(&m->ev_out, cudaEventDisableTiming), "run_host: event")) != PFF_OK) return st;
     cudaStream_t cp = m->copy_stream;
     bool mech_out = false;
     auto mechanics_out = [&]() -> pff_status {
@@ -105,17 +106,28 @@ static pff_status run_host_t(pff_mesh* m, pff_host_state* hs, const double* dir_
         if ((e = cuda_check(cudaEventRecord(m->ev_step, cs), "run_host: record")) != PFF_OK) return e;
         if ((e = cuda_check(cudaStreamWaitEvent(cp, m->ev_step, 0), "run_host: wait")) != PFF_OK) return e;
         host_out_kernel<R><<<nb, 256, 0, cp>>>(io, 1);
+        // The mesh stream goes on only when this permutation kernel is done: the persistent CG kernel that may come next
+        // fills every SM (3 CTAs of 74 KB each) and would keep the permutation kernel, and with it the copies below, waiting
+        // until the whole solve is over (measured: the end-to-end step 0.4 ms longer when the CG kernel follows the step
+        // kernel directly, as it does with the fused setup).  The copies themselves then overlap the solve.
+        if ((e = cuda_check(cudaEventRecord(m->ev_out, cp), "run_host: record")) != PFF_OK) return e;
+        if ((e = cuda_check(cudaStreamWaitEvent(cs, m->ev_out, 0), "run_host: wait")) != PFF_OK) return e;
 #define CPC(dst, src, n) if ((e = cuda_check(cudaMemcpyAsync(dst, src, (n) * sizeof(double), cudaMemcpyDeviceToHost, cp), "run_host: copy")) != PFF_OK) return e
         CPC(hs->u, io.u, 2 * N); CPC(hs->v, io.v, 2 * N); CPC(hs->a, io.a, 2 * N); CPC(hs->H, io.H, Ne);
 #undef CPC
         mech_out = true;
         return PFF_OK;
     };
+    const bool fuse = fused_setup_ok(m);  // the step before a solve performs the solve's setup pass as well (as pff_run_steps)
     for (int64_t k = 1; k <= n_steps; ++k) {
-        if ((st = launch_step(m, &s, &bc, dt, 0, nullptr, nullptr, nullptr)) != PFF_OK) return st;
-        if (k == n_steps && (st = mechanics_out()) != PFF_OK) return st;
-        if (damage_every > 0 && k % damage_every == 0) {
+        const bool solve = damage_every > 0 && k % damage_every == 0;
+        m->su_tol = rel_tol; m->su_max_iter = max_iter;
+        st = launch_step(m, &s, &bc, dt, solve && fuse ? /*MODE_STEPSU*/ 5 : /*MODE_STEP*/ 0, nullptr, nullptr, nullptr);
+        if (st != PFF_OK) { m->su_ready = false; return st; }
+        if (k == n_steps && (st = mechanics_out()) != PFF_OK) { m->su_ready = false; return st; }
+        if (solve) {
             st = damage_solve(m, &s, rel_tol, max_iter, nullptr, nullptr);
+            m->su_ready = false;
             if (st == PFF_ENOCONV) worst = st;
             else if (st != PFF_OK) return st;
         }

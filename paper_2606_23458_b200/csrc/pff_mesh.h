@@ -130,7 +130,7 @@ struct pff_mesh {
 
     // host-path staging (pff_run_host)
     cudaStream_t copy_stream = nullptr;  // second stream: copies the mechanics results back while the damage solve runs
-    cudaEvent_t ev_step = nullptr;
+    cudaEvent_t ev_step = nullptr, ev_out = nullptr;  // pff_run_host: step done (copy stream waits) / permutation done (mesh stream waits)
     void* d_stage = nullptr; size_t stage_bytes = 0;
     void* d_hstate = nullptr;  // device state arrays owned by the library for pff_run_host
     void* d_hdir = nullptr;    // its Dirichlet values (dir_u | dir_v), re-allocated when the Dirichlet set outgrows it
