@@ -276,3 +276,32 @@ def test_adjoint_solve_through_the_multigrid_solver_matches_the_direct_solve(mod
         mesh.pff_damage_solve(st, rel_tol=1e-10, max_iter=200)
     lam2, _, it2, _ = mesh.pff_damage_adjoint(st, gt, mask, rel_tol=1e-12, max_iter=200)
     assert it2 == it_m and torch.equal(lam2, lam_t)
+
+
+@pytest.mark.gpu
+def test_mg_solve_on_a_non_nested_hierarchy_with_flipped_and_permuted_elements():
+    """Every level jittered on its own (no level is a refinement of the next), clockwise elements and a random element
+    order on the finest level, a coarsest level that is not a 2:1 coarsening (65 -> 33 -> 20 nodes per side): the transfer
+    is built by point location, so the solve must still reach the oracle's solution in far fewer iterations."""
+    from pff_inputs import random_mesh
+    import paper_2606_23458_b200 as pff
+    xy0, tri0 = random_mesh(65, seed=41, jitter=0.3)
+    xy1, tri1 = random_mesh(33, seed=42, jitter=0.25)
+    xy2, tri2 = grid_mesh(20, 20, 1.0, 1.0)
+    meshes = [(xy0, tri0), (xy1, tri1), (xy2, tri2)]
+    h = 1.0 / 64
+    material = dict(GLASS, Gc=3.0, l0=4.0 * h, model=2, split=1, plane=0)
+    r = np.random.default_rng(43)
+    cen = xy0[tri0].mean(axis=1)
+    H = material["Gc"] / (2 * material["l0"]) * (0.1 + 20.0 * np.exp(-((cen[:, 0] - cen[:, 1]) / 0.05) ** 2) * r.uniform(0.5, 1.0, len(tri0)))
+    d0 = r.uniform(0.0, 0.03, len(xy0))
+    orc = OracleMesh(xy0, tri0, Material(**material))
+    orc.H[:] = H
+    orc.d[:] = d0
+    rc, it_j, _ = orc.damage_solve(rel_tol=1e-12, max_iter=5000)
+    assert rc == 0
+    mesh, st = _gpu_hierarchy(meshes, material, H=H, d=d0)
+    stt, it_mg, rr = mesh.pff_damage_solve_mg(st, rel_tol=1e-12, max_iter=100)
+    assert stt == 0 and rr <= 1e-12 and it_mg < it_j / 3
+    d = mesh.nodes_to_user(st.d)
+    assert np.abs(d - orc.d).max() <= 1e-9 * np.abs(orc.d).max()
