@@ -457,7 +457,7 @@ pff_status pff_run_steps(pff_mesh* m, pff_state* s, const pff_bc* bc, double dt,
     const int64_t period = damage_every > 0 ? damage_every : 1;
     int64_t k = 1;
     // (the multigrid solver tests convergence on the host every iteration: its solves cannot be part of a captured period)
-    const bool mg_solver = m->damage_solver == 1 && m->mg && m->mat.model == PFF_AT2 && damage_every > 0;
+    const bool mg_solver = m->damage_solver == 1 && m->mg && damage_every > 0;
     const bool want_graph = m->graph_mode != 0 && !m->graph_unsupported && !m->prof_on && period <= 64 && n_steps >= 4 * period && !mg_solver;
     if (want_graph) {
         // key of everything a captured period depends on (kernel arguments are frozen at capture time)

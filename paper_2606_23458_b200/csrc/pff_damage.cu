@@ -1010,7 +1010,7 @@ bool fused_setup_ok(const pff_mesh* m)
 pff_status damage_solve(pff_mesh* m, pff_state* s, double rel_tol, int max_iter, int* iters, double* relres)
 {
     // the multigrid-preconditioned solver where the caller selected it (pff_set_damage_solver) and it applies
-    if (m->damage_solver == 1 && m->mg && m->mat.model == PFF_AT2) return mg_solve(m, s, rel_tol, max_iter, iters, relres);
+    if (m->damage_solver == 1 && m->mg) return mg_solve(m, s, rel_tol, max_iter, iters, relres);
     const bool proj = m->mat.model == PFF_AT1;
     if (m->opt.precision == PFF_F32)
         return proj ? damage_solve_t<float, true>(m, s, rel_tol, max_iter, iters, relres)

@@ -47,6 +47,7 @@ struct MgLevel {
 struct MgData {
     std::vector<MgLevel> lv;
     void *r = nullptr, *p = nullptr, *q = nullptr, *lb = nullptr;  // outer PCG vectors (finest level; z is level 0's x)
+    void* dfull = nullptr;  // AT1: 1/D of every non-fixed node (level 0's dinv then holds the inactive set's)
     double *part = nullptr, *sc = nullptr, *h_sc = nullptr;
     unsigned int* ticket = nullptr;
     int n_part = 0;
@@ -74,7 +75,7 @@ struct MgAdjoint {  // pff_damage_adjoint through the multigrid solver: right-ha
     void* lambda;
 };
 
-enum { SC_PQ = 0, SC_RZ = 1, SC_RR = 2, SC_RZN = 3, SC_BB = 4, SC_N = 8 };
+enum { SC_PQ = 0, SC_RZ = 1, SC_RR = 2, SC_RZN = 3, SC_BB = 4, SC_R0 = 5, SC_CHG = 6, SC_N = 8 };
 
 // ---- host: point location of the nodes / element centroids of a fine mesh in the triangles of a coarse mesh --------------
 struct Locator {
@@ -273,14 +274,15 @@ __global__ void __launch_bounds__(kTPB) mg_prolong_kernel(int N, const int32_t* 
 // r = mask (b - t), lb = x (the lower bound d_n of the clamp);  sc[RR] = r.r, sc[BB] = b.b
 // (the kernels with a reduction walk the vector with a grid stride: at most kRedBlocks block partials)
 template <typename R>
-__global__ void __launch_bounds__(kTPB) mg_residual0_kernel(int N, int mask_b, const R* dinv, const R* b, const R* t, const R* x, R* r, R* lb,
-                                                            double* part, int n_part, double* sc, unsigned int* ticket)
+__global__ void __launch_bounds__(kTPB) mg_residual0_kernel(int N, int mask_b, int write_lb, const R* dinv, const R* b, const R* t, const R* x,
+                                                            R* r, R* lb, double* part, int n_part, double* sc, unsigned int* ticket)
 {
     double v[2] = {0.0, 0.0};
     for (int i = blockIdx.x * kTPB + threadIdx.x; i < N; i += gridDim.x * kTPB) {
         const bool fr = dinv[i] != R(0);
         const R ri = fr ? b[i] - t[i] : R(0);
-        r[i] = ri; lb[i] = x[i];
+        r[i] = ri;
+        if (write_lb) lb[i] = x[i];
         v[0] += double(ri) * double(ri);
         v[1] += (fr || !mask_b) ? double(b[i]) * double(b[i]) : 0.0;  // ||b|| over all nodes, as the oracle's stopping rule
                                                                         // (R10); adjoint: over the free set (g_F is the rhs)
@@ -348,6 +350,33 @@ __global__ void __launch_bounds__(kTPB) mg_direction_kernel(int N, const R* z, R
 __global__ void mg_init_rz_kernel(double* sc) { sc[SC_RZ] = 1.0; }
 // pff_run_steps: counters of this solve into the device-resident tally (as the CG kernels do for the Jacobi solver)
 __global__ void mg_tally_kernel(RunTally* t, int iters, int noconv) { t->iters += iters; t->solves += 1; t->noconv += noconv; }
+
+// ---- AT1 (L181): primal-dual active set around the multigrid-preconditioned linear solve ---------------------------------
+// One outer step: with r = b - A x (t = A x, all nodes), a non-fixed node is ACTIVE when r / D + (x - lb) < 0 (the multiplier
+// estimate -r outweighs the distance to the bound, scaled by the diagonal): it is put on its bound and masked (dinv = 0)
+// for the linear solve that follows; the others form the inactive set (dinv = 1 / D).  first = 1 also stores lb = x.
+// sc[CHG] = nodes that changed sets, sc[R0] = |r|^2 over the non-fixed nodes, sc[BB] = |b|^2.
+template <typename R>
+__global__ void __launch_bounds__(kTPB) mg_pdas_sets_kernel(int N, int first, const R* dfull, const R* b, const R* t, R* x, R* lb, R* dinv,
+                                                            double* part, int n_part, double* sc, unsigned int* ticket)
+{
+    double v[3] = {0.0, 0.0, 0.0};
+    for (int i = blockIdx.x * kTPB + threadIdx.x; i < N; i += gridDim.x * kTPB) {
+        const R xi = x[i], ri = b[i] - t[i], di = dfull[i];
+        if (first) lb[i] = xi;
+        const R lo = first ? xi : lb[i];
+        const bool fixed = di == R(0);
+        const bool was_inactive = first ? !fixed : dinv[i] != R(0);
+        const bool act = !fixed && (ri * di + (xi - lo) < R(0));
+        if (act) x[i] = lo;
+        dinv[i] = (!fixed && !act) ? di : R(0);
+        v[0] += (!fixed && was_inactive == act) ? 1.0 : 0.0;
+        v[1] += fixed ? 0.0 : double(ri) * double(ri);
+        v[2] += double(b[i]) * double(b[i]);
+    }
+    const int slots[3] = {SC_CHG, SC_R0, SC_BB};
+    reduce_to_scalars<3>(v, slots, part, n_part, sc, ticket);
+}
 
 // d <- min(1, max(d_n, d)) (L179)
 template <typename R>
@@ -454,7 +483,7 @@ void mg_free(pff_mesh* m)
         void* ps[] = {L.b, L.x, L.t, L.dinv, L.zero, L.H, L.tr.p_idx, L.tr.p_w, L.tr.r_ptr, L.tr.r_idx, L.tr.r_w, L.tr.c_ptr, L.tr.c_idx, L.tr.c_w};
         for (void* p : ps) if (p) cudaFree(p);
     }
-    void* ps[] = {g->r, g->p, g->q, g->lb, g->part, g->sc, g->ticket};
+    void* ps[] = {g->r, g->p, g->q, g->lb, g->dfull, g->part, g->sc, g->ticket};
     for (void* p : ps) if (p) cudaFree(p);
     if (g->h_sc) cudaFreeHost(g->h_sc);
     for (auto& gr : g->graphs) if (gr.exec) cudaGraphExecDestroy(gr.exec);
@@ -491,9 +520,9 @@ static pff_status mg_attach_t(pff_mesh* m, int n_coarse, pff_mesh* const* coarse
         }
     }
     const size_t nb0 = size_t(m->hm.N) * sizeof(R);
-    for (void** p : {&g->r, &g->p, &g->q, &g->lb}) MG_CUDA(cudaMalloc(p, nb0));
+    for (void** p : {&g->r, &g->p, &g->q, &g->lb, &g->dfull}) MG_CUDA(cudaMalloc(p, nb0));
     g->n_part = (int)max_blocks;
-    MG_CUDA(cudaMalloc((void**)&g->part, sizeof(double) * 2 * g->n_part));
+    MG_CUDA(cudaMalloc((void**)&g->part, sizeof(double) * 4 * g->n_part));
     MG_CUDA(cudaMalloc((void**)&g->sc, sizeof(double) * SC_N));
     MG_CUDA(cudaMalloc((void**)&g->ticket, sizeof(unsigned int)));
     MG_CUDA(cudaMemsetAsync(g->ticket, 0, sizeof(unsigned int), s));
@@ -631,15 +660,21 @@ static pff_status mg_solve_t(pff_mesh* m, const pff_state* s0, double rel_tol, i
         MG_CUDA(cudaMemcpyAsync(g->h_sc, g->sc, sizeof(double) * SC_N, cudaMemcpyDeviceToHost, s));
         return cuda_check(cudaStreamSynchronize(s), "pff_damage_solve_mg: sync");
     };
-    // r0 = mask (b - A d_n), lb = d_n; stopping rule of pff_damage_solve (R10)
-    if ((st = damage_matvec(m, s0, x, F.t, false)) != PFF_OK) return st;
-    mg_residual0_kernel<R><<<nred(N), kTPB, 0, s>>>(N, adj ? 1 : 0, (const R*)F.dinv, (const R*)F.b, (const R*)F.t, x, (R*)g->r, (R*)g->lb, g->part, g->n_part,
-                                               g->sc, g->ticket);
-    ++m->n_launches;
-    if ((st = read_scalars()) != PFF_OK) return st;
-    const double nrm = std::sqrt(std::max(g->h_sc[SC_BB], g->h_sc[SC_RR]));
-    const double lim = rel_tol * nrm;
-    double rr = g->h_sc[SC_RR];
+    const bool pdas = !adj && m->mat.model == PFF_AT1;  // bound-constrained problem: active-set outer loop (below)
+    double nrm = 0.0, lim = 0.0, rr = 0.0;
+    if (!pdas) {
+        // r0 = mask (b - A d_n), lb = d_n; stopping rule of pff_damage_solve (R10)
+        if ((st = damage_matvec(m, s0, x, F.t, false)) != PFF_OK) return st;
+        mg_residual0_kernel<R><<<nred(N), kTPB, 0, s>>>(N, adj ? 1 : 0, 1, (const R*)F.dinv, (const R*)F.b, (const R*)F.t, x, (R*)g->r, (R*)g->lb,
+                                                        g->part, g->n_part, g->sc, g->ticket);
+        ++m->n_launches;
+        if ((st = read_scalars()) != PFF_OK) return st;
+        nrm = std::sqrt(std::max(g->h_sc[SC_BB], g->h_sc[SC_RR]));
+        lim = rel_tol * nrm;
+        rr = g->h_sc[SC_RR];
+    } else {
+        MG_CUDA(cudaMemcpyAsync(g->dfull, F.dinv, size_t(N) * sizeof(R), cudaMemcpyDeviceToDevice, s));
+    }
     int it = 0;
     void* b_keep = F.b;  // the V-cycle's right-hand side on level 0 is the residual: swap the buffer in, b stays in b_keep
     pff_status result = PFF_OK;
@@ -698,16 +733,60 @@ static pff_status mg_solve_t(pff_mesh* m, const pff_state* s0, double rel_tol, i
         }
         if (gr) gr->used = ++g->graph_clock;
     }
-    while (std::sqrt(rr) > lim) {
-        if (it >= max_iter) { set_error("pff_damage_solve_mg: max_iter reached"); result = PFF_ENOCONV; break; }
-        if (gr) {
-            MG_CUDA(cudaGraphLaunch(gr->exec, s));
-            m->n_launches += gr->launches;
-        } else if ((st = iteration()) != PFF_OK) return st;
-        ++it;
-        if ((st = read_scalars()) != PFF_OK) return st;
-        rr = g->h_sc[SC_RR];
-        if (!(g->h_sc[SC_PQ] > 0.0) || !std::isfinite(rr)) { set_error("pff_damage_solve_mg: breakdown (p.Ap <= 0)"); result = PFF_ENOCONV; break; }
+    // PCG on the masked system from the current x, r (p = 0, (r.z)_old = 1 set by the caller) until |r| <= target
+    auto pcg = [&](double target) -> pff_status {
+        while (std::sqrt(rr) > target) {
+            if (it >= max_iter) { set_error("pff_damage_solve_mg: max_iter reached"); result = PFF_ENOCONV; return PFF_OK; }
+            if (gr) {
+                MG_CUDA(cudaGraphLaunch(gr->exec, s));
+                m->n_launches += gr->launches;
+            } else {
+                pff_status e = iteration();
+                if (e != PFF_OK) return e;
+            }
+            ++it;
+            pff_status e = read_scalars();
+            if (e != PFF_OK) return e;
+            rr = g->h_sc[SC_RR];
+            if (!(g->h_sc[SC_PQ] > 0.0) || !std::isfinite(rr)) {
+                set_error("pff_damage_solve_mg: breakdown (p.Ap <= 0)"); result = PFF_ENOCONV; return PFF_OK;
+            }
+        }
+        return PFF_OK;
+    };
+    int outer = 0;
+    if (!pdas) {
+        if ((st = pcg(lim)) != PFF_OK) return st;
+    } else {
+        // AT1 (L181): min 1/2 d'Ad - b'd, d >= d_n by a primal-dual active set method: the active nodes sit on their bound,
+        // the inactive ones solve their linear system (PCG with the cycle masked to them, the loop above), the sets are
+        // re-derived from the multiplier estimate, until they stop changing and the inactive residual meets the tolerance.
+        // Early linear solves are inexact (two decades per outer step) -- their only job is to move the sets.
+        for (;; ++outer) {
+            if ((st = damage_matvec(m, s0, x, F.t, false)) != PFF_OK) return st;
+            mg_pdas_sets_kernel<R><<<nred(N), kTPB, 0, s>>>(N, outer == 0, (const R*)g->dfull, (const R*)F.b, (const R*)F.t, x, (R*)g->lb,
+                                                           (R*)F.dinv, g->part, g->n_part, g->sc, g->ticket);
+            ++m->n_launches;
+            if ((st = read_scalars()) != PFF_OK) return st;
+            const double changed = g->h_sc[SC_CHG];
+            if (outer == 0) { nrm = std::max(std::sqrt(std::max(g->h_sc[SC_BB], g->h_sc[SC_R0])), 1e-300); lim = rel_tol * nrm; }
+            // residual of the inactive set after the projection
+            if ((st = damage_matvec(m, s0, x, F.t, false)) != PFF_OK) return st;
+            mg_residual0_kernel<R><<<nred(N), kTPB, 0, s>>>(N, 0, 0, (const R*)F.dinv, (const R*)F.b, (const R*)F.t, x, (R*)g->r, (R*)g->lb,
+                                                            g->part, g->n_part, g->sc, g->ticket);
+            MG_CUDA(cudaMemsetAsync(g->p, 0, size_t(N) * sizeof(R), s));
+            mg_init_rz_kernel<<<1, 1, 0, s>>>(g->sc);
+            m->n_launches += 2;
+            if ((st = read_scalars()) != PFF_OK) return st;
+            rr = g->h_sc[SC_RR];
+            if (outer > 0 && changed == 0.0 && std::sqrt(rr) <= lim) break;  // KKT: sets stable, inactive residual converged
+            if (outer >= 100 || it >= max_iter || result != PFF_OK) {
+                if (result == PFF_OK) set_error("pff_damage_solve_mg: the active set did not settle (max_iter / 100 outer steps)");
+                result = PFF_ENOCONV; break;
+            }
+            if ((st = pcg(changed == 0.0 ? lim : std::max(lim, 1e-2 * std::sqrt(rr)))) != PFF_OK) return st;
+        }
+        m->last_restarts = outer; m->last_truncs = 0;
     }
     if (!adj) {
         mg_clamp_kernel<R><<<nb, kTPB, 0, s>>>(N, (const R*)g->lb, x);
@@ -728,15 +807,6 @@ static pff_status mg_solve_t(pff_mesh* m, const pff_state* s0, double rel_tol, i
 static pff_status mg_check(pff_mesh* m, const char* who)
 {
     if (!m->mg) { set_error(std::string(who) + ": no hierarchy attached (pff_mg_attach)"); return PFF_EINVAL; }
-    if (m->mat.model != PFF_AT2) {
-        // Tried: the oracle's active-set CG (truncate the step at the first bound hit, snap, restart)
-        // with the cycle restricted to the free set as the preconditioner.  It stalls: the cycle's direction is global and
-        // pushes many nearly-active nodes towards their bound at once, so every step is a near-zero truncation (400
-        // iterations, 399 truncations, no progress; Jacobi directions are local and need 122 truncations in 200).  A
-        // multilevel AT1 solver needs another outer method (projected line search / primal-dual active set)
-        set_error(std::string(who) + ": AT2 only (the projected AT1 solver keeps the Jacobi preconditioner: pff_damage_solve)");
-        return PFF_EUNSUPPORTED;
-    }
     return PFF_OK;
 }
 

@@ -181,7 +181,7 @@ def test_cuda_mg_solve_reaches_the_oracles_solution_and_needs_fewer_iterations(p
 
 
 @pytest.mark.gpu
-def test_mg_rejects_at1_missing_hierarchy_and_meshes_of_another_domain():
+def test_mg_rejects_a_missing_hierarchy_and_meshes_of_another_domain():
     import paper_2606_23458_b200 as pff
     meshes = _levels(9, 2)
     material = _material(meshes, 2.0)
@@ -192,11 +192,6 @@ def test_mg_rejects_at1_missing_hierarchy_and_meshes_of_another_domain():
     xy_far = meshes[1][0] + 1.0
     with pytest.raises(pff.PffError):
         fine.pff_mg_attach([pff.Mesh(xy_far, meshes[1][1], material)])  # not the same domain
-    at1 = dict(material, model=1)
-    fine1, coarse1 = pff.Mesh(*meshes[0], at1), pff.Mesh(*meshes[1], at1)
-    fine1.pff_mg_attach([coarse1])
-    with pytest.raises(pff.PffError):
-        fine1.pff_damage_solve_mg(fine1.new_state())                    # AT1 keeps Jacobi
 
 
 @pytest.mark.gpu
@@ -305,3 +300,44 @@ def test_mg_solve_on_a_non_nested_hierarchy_with_flipped_and_permuted_elements()
     assert stt == 0 and rr <= 1e-12 and it_mg < it_j / 3
     d = mesh.nodes_to_user(st.d)
     assert np.abs(d - orc.d).max() <= 1e-9 * np.abs(orc.d).max()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("precision", [0, 1])
+def test_cuda_mg_at1_active_set_solve_reaches_the_oracles_constrained_minimiser(precision):
+    """AT1 (L181): the bound-constrained problem min 1/2 d'Ad - b'd, d >= d_n has one solution; the oracle reaches it with
+    Jacobi-preconditioned active-set CG (step truncated at the first bound hit), pff_damage_solve_mg with a primal-dual
+    active set around the multigrid-preconditioned linear solve of the inactive nodes.  The history field is below the
+    AT1 threshold in the background (bound active, d stays d_n) and far above it in a band (d grows): the sets must be
+    found, not guessed."""
+    meshes = _levels(65, 4, jitter=0.15)
+    material = dict(_material(meshes, 4.0), model=1)
+    H = _history(*meshes[0], material)
+    N = len(meshes[0][0])
+    fixed = np.array([7, 2100], dtype=np.int32)
+    d0 = np.random.default_rng(6).uniform(0.0, 0.02, N)
+    d0[fixed] = 1.0
+    orc = OracleMesh(*meshes[0], Material(**material))
+    orc.H[:] = H
+    orc.d[:] = d0
+    orc.set_damage_dirichlet(fixed)
+    rc, it_j, _ = orc.damage_solve(rel_tol=1e-11, max_iter=20000)
+    assert rc == 0
+    active = np.isclose(orc.d, d0, rtol=0, atol=1e-14)
+    assert 0.2 * N < active.sum() < 0.95 * N       # a real mix of active and inactive nodes
+    mesh, st = _gpu_hierarchy(meshes, material, precision=precision, H=H, d=d0, fixed=fixed)
+    tol = 1e-11 if precision == 0 else 1e-6
+    stt, it_mg, rr = mesh.pff_damage_solve_mg(st, rel_tol=tol, max_iter=400)
+    assert stt == 0 and rr <= tol
+    d = mesh.nodes_to_user(st.d)
+    assert np.abs(d - orc.d).max() <= (1e-8 if precision == 0 else 2e-5) * np.abs(orc.d).max()
+    assert (d >= d0.astype(mesh.np_dtype) - 1e-7).all() and d.max() <= 1
+    if precision == 0:
+        outer, _ = mesh.pff_damage_last_stats()
+        assert 2 <= outer <= 30 and it_mg < it_j
+        assert np.array_equal(np.isclose(d, d0, rtol=0, atol=1e-13), active)   # the same active set
+        # routed through pff_damage_solve as well, same bits
+        mesh.pff_set_damage_solver("multigrid")
+        st2 = mesh.new_state(d=d0, H=H)
+        _, it2, _ = mesh.pff_damage_solve(st2, rel_tol=tol, max_iter=400)
+        assert it2 == it_mg and np.array_equal(mesh.nodes_to_user(st2.d), d)
