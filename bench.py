@@ -257,7 +257,8 @@ def run_ours(args, rank: int, world: int):
             ms_ = (ms_ - 1) // 2 + 1
             sides.append(ms_)
         if sides:
-            mat4 = dict(cfg["material"], l0=args.mg_l0_over_h * Ls / (n_side - 1))
+            mat4 = dict(cfg["material"], l0=args.mg_l0_over_h * Ls / (n_side - 1), model=args.mg_model)
+            mg_cap = 1000 if args.mg_model == 2 else 50000  # AT1: the truncating active-set CG needs thousands of passes here
             fine = pff.Mesh(cfg["xy"], cfg["tri"], mat4, precision=prec, device=f"cuda:{dev}")
             fine.pff_mg_attach([pff.Mesh(*grid_mesh(k, k, Ls, Ls), mat4, precision=prec, device=f"cuda:{dev}") for k in sides])
             fst = fine.new_state(u=cfg["u0"], d=cfg["d0"])
@@ -265,9 +266,9 @@ def run_ours(args, rank: int, world: int):
             fine.pff_init_accel(fst, bc)
             for _ in range(5):
                 fine.pff_explicit_step(fst, bc, fdt)
-                fine.pff_damage_solve(fst, rel_tol=REL_TOL, max_iter=MAX_ITER, allow_noconv=True)
+                fine.pff_damage_solve(fst, rel_tol=REL_TOL, max_iter=mg_cap, allow_noconv=True)
             fsnap = {k: getattr(fst, k).clone() for k in fst.FIELDS}
-            mg = dict(l0_over_h=args.mg_l0_over_h, level_nodes=[n_side * n_side] + [k * k for k in sides])
+            mg = dict(l0_over_h=args.mg_l0_over_h, model="AT2" if args.mg_model == 2 else "AT1", level_nodes=[n_side * n_side] + [k * k for k in sides])
             sol = {}
             for name in ("jacobi", "multigrid"):
                 fine.pff_set_damage_solver(name)
@@ -276,13 +277,16 @@ def run_ours(args, rank: int, world: int):
                     for k in fst.FIELDS:
                         getattr(fst, k).copy_(fsnap[k])
                     fine.pff_explicit_step(fst, bc, fdt)
-                    t_ms, o = timed(lambda: fine.pff_damage_solve(fst, rel_tol=REL_TOL, max_iter=MAX_ITER, allow_noconv=True)[1], 1)
+                    t_ms, o = timed(lambda: fine.pff_damage_solve(fst, rel_tol=REL_TOL, max_iter=mg_cap, allow_noconv=True)[1], 1)
                     ts.append(t_ms); it_s = o[0]
                 mg[name] = dict(ms_per_solve=float(np.median(ts[1:])), iterations=it_s)
                 sol[name] = fst.d.clone()
             mg["max_abs_diff_d"] = float((sol["multigrid"] - sol["jacobi"]).abs().max())
             mg["note"] = ("one damage solve to rel_tol 1e-8 from the same state, l0 = %g h: Jacobi-PCG kernels against one V(1,1) cycle per "
                           "iteration (iterations = outer iterations, each one cycle + one operator application)" % args.mg_l0_over_h)
+            if args.mg_model == 1:
+                mg["note"] += "; AT1: truncating active-set CG (Jacobi) against a primal-dual active set around the multigrid solve"
+                mg["multigrid"]["active_set_steps"] = fine.pff_damage_last_stats()[0]
             del fine, fst, fsnap, sol
 
     # quasi-static mechanics solve (pff_equilibrium_solve), timed LAST because it installs a Dirichlet set (bottom edge
@@ -366,6 +370,8 @@ def main():
                     help="CG kernel of the damage solve (include/pff.h, pff_set_cg_variant): auto = chosen per solve from the mesh "
                          "size and the previous solve's pass count")
     ap.add_argument("--no-multigrid", action="store_true", help="skip the multigrid-against-Jacobi leg (cfg5 workloads)")
+    ap.add_argument("--mg-model", type=int, default=2, choices=[1, 2], help="damage model of the multigrid leg: 2 = AT2 (PCG), 1 = AT1 "
+                    "(primal-dual active set around the multigrid solve against the truncating active-set CG)")
     ap.add_argument("--mg-l0-over-h", type=float, default=4.0, help="regularisation length of the multigrid leg's mesh, in mesh sizes")
     ap.add_argument("--no-fused-setup", action="store_true", help="pff_run_steps launches the damage setup kernel separately instead of "
                     "performing that pass inside the explicit-step kernel")

@@ -209,24 +209,28 @@ pff_status pff_mg_attach(pff_mesh *mesh, int32_t n_coarse, pff_mesh *const *coar
  * lambda_max(D^-1 A) <= 2) and the number of Jacobi sweeps that stand for the coarsest-level solve (default 4). */
 pff_status pff_mg_set_params(pff_mesh *mesh, double omega, int32_t coarse_sweeps);
 
-/* pff_damage_solve for AT2 with one V(1,1) cycle per iteration as the preconditioner:
+/* pff_damage_solve with one V(1,1) cycle per iteration as the preconditioner:
  *   level l:  x = w D^-1 b;  r = b - A x;  x += P V_{l+1}(P^T r);  x += w D^-1 (b - A x);   coarsest: Jacobi sweeps.
  * Coarse operators are re-discretised: the operator (Gc / l0 + 2 H) M + Gc l0 K (L173, L185) of the coarse mesh with H
  * averaged over every coarse element's children (area weights).  Same right-hand side, warm start, damage-Dirichlet
  * nodes, stopping rule (R10) and final clamp d <- min(1, max(d_n, d)) (L179) as pff_damage_solve, and the same
  * unique solution: only the iteration count differs.  iters_out counts outer iterations (one V-cycle + one operator
- * application each; a V-cycle costs about 2.7 fine-level operator applications).  AT1 returns PFF_EUNSUPPORTED: the
- * projected solver (L181) truncates every step at the first bound hit, and with a global (multilevel) correction that
- * hit comes after a near-zero step (measured: it stalls), so AT1 keeps the Jacobi preconditioner.
- * Synchronises the stream every iteration (host-side convergence test);
+ * application each; a V-cycle costs about 2.7 fine-level operator applications).
+ * AT1 (L181: min 1/2 d'Ad - b'd subject to d >= d_n): a primal-dual active set method around that solve.  With
+ * r = b - A d, a node is ACTIVE when r / D + (d - d_n) < 0: it is put on its bound; the inactive nodes solve their linear
+ * system by the multigrid-preconditioned CG above (the active nodes masked on the finest level like damage-Dirichlet
+ * nodes; inexactly, residual x 0.3, while the sets still move); the sets are re-derived until they stop changing and the
+ * inactive residual meets the tolerance: the KKT point, i.e. the same unique solution as pff_damage_solve's projected CG
+ * (which truncates every step at the first bound hit, restarts, and needs thousands of passes when damage is widespread).
+ * pff_damage_last_stats then reports the active-set steps as `restarts`.  Synchronises the stream every iteration (host-side convergence test);
  * bit-reproducible run to run.  Pays off where l0 / h is large (profiles/r2_multigrid.md); pff_damage_solve and
  * pff_run_steps use it after pff_set_damage_solver(mesh, 1). */
 pff_status pff_damage_solve_mg(pff_mesh *mesh, pff_state *state, double rel_tol, int32_t max_iter,
                                int32_t *iters_out, double *relres_out);
 
 /* Which solver pff_damage_solve and pff_run_steps use for this mesh: 0 (default) the Jacobi-PCG kernels, 1 the
- * multigrid-preconditioned CG above (needs an attached hierarchy: PFF_EINVAL otherwise; on an AT1 mesh the forward
- * solves keep the Jacobi kernels, only the adjoint solve changes).
+ * multigrid-preconditioned solver above (needs an attached hierarchy: PFF_EINVAL otherwise; AT2: PCG, AT1: primal-dual
+ * active set around it).
  * With solver 1, pff_run_steps launches every kernel itself (no graph replay of a period: the solver tests convergence on
  * the host) and its iteration total counts outer multigrid iterations.  pff_mg_attach replacing the hierarchy keeps the
  * choice.  pff_damage_adjoint follows the choice as well, for AT1 and AT2 alike (it is a linear solve on a given free set:

@@ -761,7 +761,8 @@ static pff_status mg_solve_t(pff_mesh* m, const pff_state* s0, double rel_tol, i
         // AT1 (L181): min 1/2 d'Ad - b'd, d >= d_n by a primal-dual active set method: the active nodes sit on their bound,
         // the inactive ones solve their linear system (PCG with the cycle masked to them, the loop above), the sets are
         // re-derived from the multiplier estimate, until they stop changing and the inactive residual meets the tolerance.
-        // Early linear solves are inexact (two decades per outer step) -- their only job is to move the sets.
+        // While the sets still move the linear solves are very inexact (residual x 0.3 per outer step: their only job is to
+        // move the sets; measured at 10^6 nodes: 48 cycles in all against 116 with x 0.01 and 165 with x 0.001).
         for (;; ++outer) {
             if ((st = damage_matvec(m, s0, x, F.t, false)) != PFF_OK) return st;
             mg_pdas_sets_kernel<R><<<nred(N), kTPB, 0, s>>>(N, outer == 0, (const R*)g->dfull, (const R*)F.b, (const R*)F.t, x, (R*)g->lb,
@@ -784,7 +785,7 @@ static pff_status mg_solve_t(pff_mesh* m, const pff_state* s0, double rel_tol, i
                 if (result == PFF_OK) set_error("pff_damage_solve_mg: the active set did not settle (max_iter / 100 outer steps)");
                 result = PFF_ENOCONV; break;
             }
-            if ((st = pcg(changed == 0.0 ? lim : std::max(lim, 1e-2 * std::sqrt(rr)))) != PFF_OK) return st;
+            if ((st = pcg(changed == 0.0 ? lim : std::max(lim, 0.3 * std::sqrt(rr)))) != PFF_OK) return st;
         }
         m->last_restarts = outer; m->last_truncs = 0;
     }
