@@ -202,6 +202,9 @@ pff_status pff_energies_static(pff_mesh *mesh, const pff_state *state, double *o
  * between consecutive levels (point location, barycentric weights), its transpose and the parent element of every element
  * on the host and uploads them.  The caller keeps the coarse meshes alive while the hierarchy is attached and destroys
  * them itself; attaching again replaces the hierarchy; pff_mesh_destroy(mesh) releases it.
+ * n_coarse = 0 is allowed: the "cycle" is then `coarse_sweeps` damped-Jacobi sweeps on the mesh itself (a polynomial
+ * preconditioner, no coarse meshes needed) -- of interest for AT1, whose active-set outer method (below) does not depend
+ * on the hierarchy.
  * Errors: PFF_EINVAL (arguments), PFF_EMESH (a node outside the next level's triangles), PFF_ECUDA. */
 pff_status pff_mg_attach(pff_mesh *mesh, int32_t n_coarse, pff_mesh *const *coarse);
 

@@ -706,7 +706,7 @@ pff_status pff_energies(pff_mesh* m, const pff_state* s, double out[4])
 
 pff_status pff_mg_attach(pff_mesh* m, int32_t n_coarse, pff_mesh* const* coarse)
 {
-    if (!m || n_coarse < 1 || n_coarse > 16 || !coarse) { set_error("pff_mg_attach: null mesh or n_coarse outside 1..16"); return PFF_EINVAL; }
+    if (!m || n_coarse < 0 || n_coarse > 16 || (n_coarse > 0 && !coarse)) { set_error("pff_mg_attach: null mesh or n_coarse outside 0..16"); return PFF_EINVAL; }
     if (m->opt.scatter != PFF_SCATTER_GATHER) { set_error("pff_mg_attach: gather meshes only"); return PFF_EUNSUPPORTED; }
     DeviceGuard dg(m);
     return mg_attach(m, n_coarse, coarse);

@@ -341,3 +341,28 @@ def test_cuda_mg_at1_active_set_solve_reaches_the_oracles_constrained_minimiser(
         st2 = mesh.new_state(d=d0, H=H)
         _, it2, _ = mesh.pff_damage_solve(st2, rel_tol=tol, max_iter=400)
         assert it2 == it_mg and np.array_equal(mesh.nodes_to_user(st2.d), d)
+
+
+@pytest.mark.gpu
+def test_at1_active_set_solver_without_coarse_levels():
+    """pff_mg_attach with no coarse mesh: the cycle degenerates to damped-Jacobi sweeps on the mesh itself, the AT1
+    primal-dual active set around it still reaches the oracle's constrained minimiser (and an AT2 solve its solution)."""
+    import paper_2606_23458_b200 as pff
+    meshes = _levels(33, 1, jitter=0.15)
+    xy, tri = meshes[0]
+    for model in (1, 2):
+        material = dict(_material(meshes, 2.0), model=model)
+        H = _history(xy, tri, material)
+        d0 = np.random.default_rng(8).uniform(0.0, 0.02, len(xy))
+        orc = OracleMesh(xy, tri, Material(**material))
+        orc.H[:] = H
+        orc.d[:] = d0
+        rc, _, _ = orc.damage_solve(rel_tol=1e-11, max_iter=20000)
+        assert rc == 0
+        mesh = pff.Mesh(xy, tri, material)
+        mesh.pff_mg_attach([])
+        st = mesh.new_state(d=d0, H=H)
+        stt, it, rr = mesh.pff_damage_solve_mg(st, rel_tol=1e-11, max_iter=2000)
+        assert stt == 0 and rr <= 1e-11
+        d = mesh.nodes_to_user(st.d)
+        assert np.abs(d - orc.d).max() <= 1e-8 * np.abs(orc.d).max()
