@@ -366,3 +366,28 @@ def test_at1_active_set_solver_without_coarse_levels():
         assert stt == 0 and rr <= 1e-11
         d = mesh.nodes_to_user(st.d)
         assert np.abs(d - orc.d).max() <= 1e-8 * np.abs(orc.d).max()
+
+
+@pytest.mark.gpu
+def test_run_steps_at1_with_the_active_set_solver_follows_the_projected_cg_trajectory():
+    """AT1 time loop (config 2's notched plate, jittered and permuted, damage-Dirichlet notch) with the hierarchy-free
+    active-set solver against the default projected CG, both converged to 1e-11: same trajectory."""
+    import paper_2606_23458_b200 as pff
+    from pff_inputs import config
+    from _harness import gpu_from, gpu_fields
+    cfg = config(2, scale=0.2)
+    cfg = dict(cfg, material=dict(cfg["material"], model=1))
+    out = {}
+    for solver in ("jacobi", "multigrid"):
+        mesh, st = gpu_from(cfg)
+        mesh.pff_mg_attach([])
+        mesh.pff_mg_set_params(2.0 / 3.0, 2)
+        mesh.pff_set_damage_solver(solver)
+        bc = mesh.bc(load_scale=25.0)
+        dt = 0.5 * mesh.dt_crit
+        mesh.pff_init_accel(st, bc)
+        _, its = mesh.pff_run_steps(st, bc, dt, 30, damage_every=1, rel_tol=1e-11, max_iter=20000)
+        out[solver] = gpu_fields(mesh, st) + (its,)
+    for a, b in zip(out["jacobi"][:5], out["multigrid"][:5]):
+        assert np.abs(a - b).max() <= 1e-8 * max(np.abs(a).max(), 1e-300)
+    assert out["jacobi"][3].max() == 1.0 and (out["jacobi"][3] > 0.01).sum() > 10
