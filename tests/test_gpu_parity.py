@@ -643,3 +643,31 @@ def test_fused_step_and_damage_setup_is_bit_identical_to_the_three_kernel_sequen
         for a, b in zip(*outs):
             assert np.array_equal(a, b)
         assert outs[0][5].min() > 0 and np.abs(outs[0][3]).max() > 0
+
+
+@pytest.mark.parametrize("order,chunk", [(0, 128), (1, 32)])
+def test_fused_setup_bitwise_on_irregular_decompositions_and_with_displacement_dirichlet(order, chunk):
+    """The fused step + damage setup on the corner cases of the decomposition (random element order without renumbering:
+    every node an interface node, overflow partial slots; tiny chunks: several meta epochs per CTA) and with a
+    displacement-Dirichlet set driven by per-step values (config 3's sheared square): bit-identical to the three-kernel
+    sequence."""
+    cfg = config(5, n=201)
+    rng = np.random.default_rng(12)
+    cfg["tri"] = cfg["tri"][rng.permutation(len(cfg["tri"]))]
+    cases = [(cfg, dict(order=order, chunk_elems=chunk), None)]
+    cfg3 = config(3, scale=0.08)
+    cases.append((cfg3, dict(chunk_elems=chunk), shear_bc(cfg3, 40, 1e-3)))
+    for c, kw, dirv in cases:
+        outs = []
+        for fused in (True, False):
+            mesh, st = gpu_from(c, **kw)
+            mesh.pff_set_fused_setup(fused)
+            bc = mesh.bc(*dirv) if dirv is not None else mesh.bc()
+            dt = 0.5 * mesh.dt_crit
+            mesh.pff_init_accel(st, bc)
+            _, its = mesh.pff_run_steps(st, bc, dt, 12, damage_every=2, rel_tol=1e-9, max_iter=4000)
+            assert mesh.pff_fused_setup_used() == fused
+            outs.append([x.copy() for x in gpu_fields(mesh, st)] + [np.array([its])])
+        for a, b in zip(*outs):
+            assert np.array_equal(a, b)
+        assert np.isfinite(outs[0][0]).all() and np.abs(outs[0][0]).max() > 0
