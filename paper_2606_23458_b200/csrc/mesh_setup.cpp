@@ -6,6 +6,7 @@
 #include <cstring>
 #include <limits>
 #include <numeric>
+#include <thread>
 
 #include "pff_internal.h"
 
@@ -370,10 +371,22 @@ pff_status build_host_mesh(int64_t N, const double* xy, int64_t Ne, const int32_
                 int32_t l = lloc[3 * (en - m.elem_start) + k];
                 hm.ell[size_t(m.ell_off) + size_t(val[l]++) * nloc + l] = uint16_t(k * EC + (en - m.elem_start));
             }
-        balance_gather_columns(hm.ell.data() + m.ell_off, nloc, w, uint16_t(3 * EC), int(128 / real_bytes));
         hm.max_ell_w = std::max(hm.max_ell_w, w);
     }
     hm.ell.resize((hm.ell.size() + 7) / 8 * 8 + 8, uint16_t(3 * EC));  // the widened TMA copy stays in bounds
+    {   // bank balance of every chunk's table (chunks are independent: spread over the host cores; the result does not
+        // depend on the thread count)
+        const unsigned nt = std::max(1u, std::min(16u, std::thread::hardware_concurrency()));
+        std::vector<std::thread> pool;
+        for (unsigned t = 0; t < nt; ++t)
+            pool.emplace_back([&, t]() {
+                for (int64_t c = t; c < C; c += nt) {
+                    const ChunkMeta& m = hm.meta[c];
+                    balance_gather_columns(hm.ell.data() + m.ell_off, m.n_int + m.n_halo, m.ell_w, uint16_t(3 * EC), int(128 / real_bytes));
+                }
+            });
+        for (auto& th : pool) th.join();
+    }
     // interface-node CSR over halo slots, ascending chunk (chunks were visited in order)
     // Partial slots: kIfaceWidth fixed slots per interface node (slot kIfaceWidth * s + k for the k-th touching chunk,
     // ascending chunk order; never-written slots stay zero), the rare further ones in an overflow CSR behind them.
