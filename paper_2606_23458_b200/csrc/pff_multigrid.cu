@@ -13,7 +13,10 @@
 // Every operator application is the chunk kernel of pff_damage.cu (plain mode); everything else is the small vector
 // kernels below.  All reductions have a fixed order (block partials summed by the last block in index order).
 #include <algorithm>
+#include <atomic>
 #include <cmath>
+#include <functional>
+#include <thread>
 #include <string>
 #include <vector>
 
@@ -416,21 +419,31 @@ static pff_status build_transfer(const pff_mesh* mf, const pff_mesh* mc, MgTrans
     std::vector<int32_t> p_idx(size_t(3) * f.N);
     std::vector<double> p_w(size_t(3) * f.N);
     std::vector<int32_t> r_cnt(c.N + 1, 0);
-    for (int64_t i = 0; i < f.N; ++i) {
+    // (point location is independent per node / element: spread over the host cores; the tables do not depend on the
+    // thread count)
+    const unsigned nt = std::max(1u, std::min(16u, std::thread::hardware_concurrency()));
+    auto parallel_for = [&](int64_t n, const std::function<void(int64_t)>& body) {
+        std::vector<std::thread> pool;
+        for (unsigned t = 0; t < nt; ++t)
+            pool.emplace_back([&, t]() { for (int64_t i = t; i < n; i += nt) body(i); });
+        for (auto& th : pool) th.join();
+    };
+    std::atomic<int> outside{0};
+    parallel_for(f.N, [&](int64_t i) {
         const double* p = &f.xy_user[2 * size_t(f.node_old_of_new[i])];
         double w[3];
         const int32_t e = loc.locate(p[0], p[1], w);
-        if (e < 0) {
-            set_error("pff_mg_attach: a node of level " + std::to_string(level) + " lies in no triangle of level " +
-                      std::to_string(level + 1) + " (the meshes must cover the same domain)");
-            return PFF_EMESH;
-        }
-        for (int k = 0; k < 3; ++k) {
-            p_idx[3 * i + k] = c.conn4[4 * size_t(e) + k];
-            p_w[3 * i + k] = w[k];
-            if (w[k] != 0.0) ++r_cnt[p_idx[3 * i + k] + 1];
-        }
+        if (e < 0) { outside = 1; return; }
+        for (int k = 0; k < 3; ++k) { p_idx[3 * i + k] = c.conn4[4 * size_t(e) + k]; p_w[3 * i + k] = w[k]; }
+    });
+    if (outside) {
+        set_error("pff_mg_attach: a node of level " + std::to_string(level) + " lies in no triangle of level " +
+                  std::to_string(level + 1) + " (the meshes must cover the same domain)");
+        return PFF_EMESH;
     }
+    for (int64_t i = 0; i < f.N; ++i)
+        for (int k = 0; k < 3; ++k)
+            if (p_w[3 * i + k] != 0.0) ++r_cnt[p_idx[3 * i + k] + 1];
     // its transpose, rows = coarse nodes, entries ascending in the fine index (fixed summation order)
     std::vector<int32_t> r_ptr(c.N + 1, 0);
     for (int64_t I = 0; I < c.N; ++I) r_ptr[I + 1] = r_ptr[I] + r_cnt[I + 1];
@@ -445,7 +458,7 @@ static pff_status build_transfer(const pff_mesh* mf, const pff_mesh* mc, MgTrans
     // parent element of every fine element (centroid), child weights = area fractions
     std::vector<int32_t> parent(f.Ne), c_ptr(c.Ne + 1, 0);
     std::vector<double> asum(c.Ne, 0.0);
-    for (int64_t e = 0; e < f.Ne; ++e) {
+    parallel_for(f.Ne, [&](int64_t e) {
         double cx = 0.0, cy = 0.0;
         for (int k = 0; k < 3; ++k) {
             const double* p = &f.xy_user[2 * size_t(f.node_old_of_new[f.conn4[4 * e + k]])];
@@ -453,9 +466,11 @@ static pff_status build_transfer(const pff_mesh* mf, const pff_mesh* mc, MgTrans
         }
         double w[3];
         const int32_t E = loc.locate(cx, cy, w);
-        if (E < 0) { set_error("pff_mg_attach: an element of level " + std::to_string(level) + " lies in no triangle of the next level"); return PFF_EMESH; }
-        parent[e] = E; ++c_ptr[E + 1]; asum[E] += f.area[e];
-    }
+        if (E < 0) outside = 1;
+        parent[e] = E;
+    });
+    if (outside) { set_error("pff_mg_attach: an element of level " + std::to_string(level) + " lies in no triangle of the next level"); return PFF_EMESH; }
+    for (int64_t e = 0; e < f.Ne; ++e) { ++c_ptr[parent[e] + 1]; asum[parent[e]] += f.area[e]; }
     for (int64_t E = 0; E < c.Ne; ++E) c_ptr[E + 1] += c_ptr[E];
     std::vector<int32_t> c_idx(f.Ne), cfill(c.Ne, 0);
     std::vector<double> c_w(f.Ne);
