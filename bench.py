@@ -477,7 +477,7 @@ def main():
     if not args.no_cpu_baseline:
         import oracle
         oracle.build()
-        ns = 10 if Ne > 500000 else 50
+        ns = 20 if Ne > 500000 else 50  # ~13 s of single-thread oracle time at 2e6 elements
         val, osec, _ = oracle_sample(r["cfg"], ns)
         line["cpu_baseline"] = dict(value=val, unit=UNIT, cores=1, kind="oracle", host_cores=os.cpu_count(),
                                     sample=f"{ns} staggered steps of the same mesh ({Ne} elements) in {osec:.1f} s, single thread")
