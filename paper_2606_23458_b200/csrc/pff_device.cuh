@@ -222,7 +222,18 @@ template <typename R>
 __device__ __forceinline__ R iface_sum(const R* plane, int s, int N_sh, int n_ovf, const int32_t* ovf_rowptr)
 {
     const R* hp = plane + (size_t)kIfaceWidth * s;
-    R v = ((hp[0] + hp[1]) + hp[2]) + hp[3];
+    R v;
+    if ((reinterpret_cast<uintptr_t>(hp) & 15) == 0) {  // the usual case: the four slots in one or two 16-byte loads
+        if (sizeof(R) == 8) {
+            const double2 lo = reinterpret_cast<const double2*>(hp)[0], hi = reinterpret_cast<const double2*>(hp)[1];
+            v = R(((lo.x + lo.y) + hi.x) + hi.y);
+        } else {
+            const float4 q = *reinterpret_cast<const float4*>(hp);
+            v = R(((q.x + q.y) + q.z) + q.w);
+        }
+    } else {
+        v = ((hp[0] + hp[1]) + hp[2]) + hp[3];
+    }
     if (n_ovf > 0)
         for (int k = ovf_rowptr[s]; k < ovf_rowptr[s + 1]; ++k) v += plane[(size_t)kIfaceWidth * N_sh + k];
     return v;
